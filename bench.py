@@ -1,0 +1,391 @@
+#!/usr/bin/env python
+"""bench.py -- regular-force pair interactions/s at N = 1M (BASELINE.json metric), one JSON line.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--n-i 8192] [--no-sweep] [--impl reference]
+
+A "step" is one pass of the whole hot path over BASELINE.json config 4
+(N = 1,048,576 Plummer + Kroupa IMF + 5 % binaries, synthetic, seed 0):
+    nb_set_j (ingest + re-layout)  ->  nb_predict_all(t)  ->  nb_regular(active block of n_i)
+`value` counts n_i * N pair interactions per step with all inputs resident in HBM; `e2e` runs the same
+step through the HOST-pointer C-ABI calls (pinned host buffers, copies inside the timed region).
+Under torchrun each rank holds all N j-particles and takes its shard of a world_size * n_i active
+block (i-sharding = the paper's copy algorithm; no data-path collective) -> "scaling": "weak".
+
+--impl reference times the CPU oracle (oracle/, test infrastructure) on a bounded sample of the same
+workload; it is the only leg besides cpu_baseline that executes anything under oracle/.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+FLOP_PER_INTERACTION = 60.0          # BASELINE.json north_star convention (force + jerk)
+METRIC = "regular-force pair interactions/s at N=1M"
+UNIT = "pair interactions/s"
+WORKLOAD = "cfg4_plummer1m_kroupa_bin5_headline"
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--n-i", type=int, default=8192, help="active-block size per GPU")
+    ap.add_argument("--N", type=int, default=1048576, help="override N (debug only; the metric is N=1M)")
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--no-sweep", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    return ap.parse_args()
+
+
+# ----------------------------------------------------------------------------- helpers
+
+class ClockSampler:
+    """Samples SM clocks / throttle reasons with nvidia-smi DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows, self.proc = [], None
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100", "-i", str(index)],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), line.strip()))
+
+    def stop(self, t0: float, t1: float) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm, smax, reasons, power = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ts, line in self.rows:
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                clk, mx = float(f[0]), float(f[1])
+            except ValueError:
+                continue
+            if t0 - 0.05 <= ts <= t1 + 0.15:
+                sm.append(clk); smax.append(mx)
+                try:
+                    power.append(float(f[2]))
+                except ValueError:
+                    pass
+                for nme, val in zip(names, f[3:7]):
+                    if val.lower().startswith("active"):
+                        reasons.add(nme)
+        if not sm:      # region shorter than the sampling period: take the nearest samples
+            for ts, line in self.rows[-3:]:
+                f = [x.strip() for x in line.split(",")]
+                try:
+                    sm.append(float(f[0])); smax.append(float(f[1]))
+                except (ValueError, IndexError):
+                    pass
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(smax) if smax else None,
+                "power_w_max": max(power) if power else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def build_workload(N: int, n_total: int):
+    import nbgen
+    cfg = nbgen.make_config(4, N=N)
+    idx, h2 = nbgen.active_block(cfg, min(n_total, N))
+    return cfg, idx, h2
+
+
+def peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            p = json.load(f)
+        return p, "measured (MEASURED_PEAKS.json)"
+    return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback (B200_PROFILING.md)"
+
+
+# ----------------------------------------------------------------------------- reference arm (CPU oracle)
+
+def cpu_oracle_rate(cfg, idx, h2, seconds_target=12.0, fixed_n=None):
+    """Oracle (as it stands) on a bounded sample: the first n of the active block against all N."""
+    import oracle
+    oracle.build()
+    threads = oracle.num_threads()
+    N = cfg["N"]
+    xp, vp = oracle.predict(cfg["x0"], cfg["v0"], cfg["a0"], cfg["j0"], cfg["t0"], cfg["t"])
+    if fixed_n is None:
+        probe = min(len(idx), 2 * threads)
+        t = time.perf_counter()
+        oracle.regular(cfg["m"], xp, vp, idx[:probe], h2[:probe], cfg["cap"])
+        dt = time.perf_counter() - t
+        n = int(min(len(idx), max(probe, seconds_target / max(dt, 1e-6) * probe)))
+        n = max(threads, n // threads * threads)
+    else:
+        n = fixed_n
+    t = time.perf_counter()
+    xp, vp = oracle.predict(cfg["x0"], cfg["v0"], cfg["a0"], cfg["j0"], cfg["t0"], cfg["t"])
+    oracle.regular(cfg["m"], xp, vp, idx[:n], h2[:n], cfg["cap"])
+    dt = time.perf_counter() - t
+    return dict(value=n * N / dt, unit=UNIT, cores=threads, kind="oracle",
+                sample=f"predict_all + first {n} of the {len(idx)}-particle active block x all N={N} j "
+                       f"({n * N:.3e} pairs, {dt:.1f} s, FP64 direct sum, OpenMP over i)", n_sample=n, seconds=dt)
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    cfg, idx, h2 = build_workload(args.N, args.n_i)
+    import oracle
+    oracle.build()
+    threads = oracle.num_threads()
+    # bound the whole run (warmup + steps) to a few minutes: ~6 s of CPU work per step
+    first = cpu_oracle_rate(cfg, idx, h2, seconds_target=6.0)
+    n = first["n_sample"]
+    for _ in range(max(args.warmup - 1, 0)):
+        cpu_oracle_rate(cfg, idx, h2, fixed_n=n)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        cpu_oracle_rate(cfg, idx, h2, fixed_n=n)
+    dt = time.perf_counter() - t0
+    value = args.steps * n * cfg["N"] / dt
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": WORKLOAD, "N": cfg["N"], "n_i": int(args.n_i), "sample_n_i": n,
+                   "note": "CPU oracle (oracle/nbody_oracle.c) on the host cores; each step = predict_all + a bounded "
+                           "sample of the active block against all N"},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle",
+                         "sample": f"first {n} of {args.n_i} active particles x N={cfg['N']} per step"},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+# ----------------------------------------------------------------------------- B200 arm
+
+def run_b200(args):
+    import torch
+    import torch.distributed as dist
+    import paper_1504_03687_b200 as nb
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the B200 arm has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+
+    import nbgen
+    N = args.N
+    cfg, idx_all, h2_all = build_workload(N, args.n_i * world)
+    idx_np, h2_np = nbgen.shard_active_block(idx_all, h2_all, rank, world)   # i-sharding, no collective
+    n_i = int(idx_np.shape[0])
+    cap = cfg["cap"]
+
+    dev = torch.device("cuda", local)
+    stream = torch.cuda.current_stream()
+    ctx = nb.nb_open(N, cap, stream)
+    f64 = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float64)).to(dev)
+    jstate = [f64(cfg[k]) for k in ("m", "x0", "v0", "a0", "j0", "t0")]
+    idx = torch.from_numpy(np.ascontiguousarray(idx_np)).to(dev)
+    h2 = f64(h2_np)
+    out = dict(acc=torch.empty((n_i, 3), dtype=torch.float64, device=dev),
+               jerk=torch.empty((n_i, 3), dtype=torch.float64, device=dev),
+               pot=torch.empty(n_i, dtype=torch.float64, device=dev),
+               nnb=torch.empty(n_i, dtype=torch.int32, device=dev),
+               nblist=torch.empty((n_i, cap), dtype=torch.int32, device=dev),
+               overflow=torch.empty(n_i, dtype=torch.int32, device=dev))
+    t_pred = float(cfg["t"])
+
+    def step():
+        ctx.set_j(*jstate)              # a1
+        ctx.predict_all(t_pred)         # a2
+        ctx.regular(idx, h2, **out)     # a3-a7
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    torch.cuda.synchronize()
+
+    # ---- timed region: K steps, CUDA events on the context's stream, barrier + sync on both sides
+    ctx.tune("profile", 1)
+    launches0 = ctx.info("kernel_launches")
+    sampler = ClockSampler(local) if rank == 0 else None
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier(); torch.cuda.synchronize()
+    w0 = time.time()
+    e0.record(stream)
+    for _ in range(args.steps):
+        step()
+    e1.record(stream)
+    torch.cuda.synchronize(); barrier()
+    w1 = time.time()
+    ms = e0.elapsed_time(e1)
+    clocks = sampler.stop(w0, w1) if sampler else None
+    launches = ctx.info("kernel_launches") - launches0
+    force_ns = ctx.info("force_kernel_ns")
+    force_cnt = ctx.info("force_kernel_count")
+    ctx.tune("profile", 0)
+    if world > 1:
+        t = torch.tensor([ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+        tl = torch.tensor([launches], dtype=torch.int64, device=dev)
+        dist.all_reduce(tl, op=dist.ReduceOp.SUM)
+        launches = int(tl.item())
+    pairs_per_step = float(n_i) * N * world
+    value = pairs_per_step * args.steps / (ms * 1e-3)
+
+    # ---- e2e: same step through the HOST-pointer ABI (pinned buffers; copies inside the timed region)
+    e2e = None
+    if not args.no_e2e:
+        pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+        hj = [pin(np.asarray(cfg[k], dtype=np.float64)) for k in ("m", "x0", "v0", "a0", "j0", "t0")]
+        hidx, hh2 = pin(idx_np), pin(np.asarray(h2_np, dtype=np.float64))
+        hout = dict(acc=torch.empty((n_i, 3), dtype=torch.float64).pin_memory(),
+                    jerk=torch.empty((n_i, 3), dtype=torch.float64).pin_memory(),
+                    pot=torch.empty(n_i, dtype=torch.float64).pin_memory(),
+                    nnb=torch.empty(n_i, dtype=torch.int32).pin_memory(),
+                    nblist=torch.empty((n_i, cap), dtype=torch.int32).pin_memory(),
+                    overflow=torch.empty(n_i, dtype=torch.int32).pin_memory())
+
+        def step_host():
+            ctx.set_j_host(*hj)
+            ctx.predict_all(t_pred)
+            ctx.regular_host(hidx, hh2, **hout)     # returns with results in host memory
+
+        ke = max(3, min(args.steps, 10))
+        for _ in range(2):
+            step_host()
+        barrier(); torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        e0.record(stream)
+        for _ in range(ke):
+            step_host()
+        e1.record(stream)
+        torch.cuda.synchronize(); barrier()
+        wall = time.perf_counter() - t0
+        ms_e = max(e0.elapsed_time(e1), wall * 1e3)     # host-blocking copies: wall clock bounds it
+        if world > 1:
+            t = torch.tensor([ms_e], dtype=torch.float64, device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms_e = float(t.item())
+        h2d = 14 * N * 8 + n_i * (4 + 8)
+        d2h = n_i * (7 * 8 + 4 + 4) + n_i * cap * 4
+        e2e = {"value": pairs_per_step * ke / (ms_e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
+               "d2h_bytes_per_step": d2h, "steps": ke, "ms_per_step": ms_e / ke,
+               "checksum_pot": float(hout["pot"].sum())}
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel (force_kernel): plain FP32 issue -> "alu"
+    pk, pk_src = peaks()
+    sm_count = ctx.info("sm_count")
+    sm_max_mhz = float((clocks or {}).get("sm_max_mhz") or pk.get("sm_max_mhz", 1965.0))
+    peak_tflops = sm_count * 128 * 2 * sm_max_mhz * 1e6 / 1e12
+    force_ms = force_ns / max(force_cnt, 1) * 1e-6
+    ach_tflops = FLOP_PER_INTERACTION * float(n_i) * N / (force_ms * 1e-3) / 1e12
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "force_kernel_traffic.json")
+    if os.path.exists(tpath):
+        with open(tpath) as f:
+            traffic = json.load(f).get("dram_bytes_per_launch")
+    roofline = {
+        "bound": "alu", "kernel": "nbreg::force_kernel", "achieved": ach_tflops, "peak": peak_tflops,
+        "unit": "TFLOP/s", "frac": ach_tflops / peak_tflops, "traffic": traffic,
+        "flop_per_interaction": FLOP_PER_INTERACTION, "avg_launch_ms": force_ms, "launches_timed": int(force_cnt),
+        "interactions_per_launch": float(n_i) * N,
+        "peak_how": f"{sm_count} SMs x 128 FP32 lanes x 2 flop x {sm_max_mhz:.0f} MHz (max SM clock; DESIGN.md)",
+        "frac_at_sampled_clock": (ach_tflops / (sm_count * 128 * 2 * clocks["sm_mhz"] * 1e6 / 1e12)
+                                  if clocks and clocks.get("sm_mhz") else None),
+        "share_of_step": force_ms / (ms / args.steps),
+    }
+
+    # ---- sweep vs block size (the metric is "vs block size"): nb_regular alone, min of 3
+    sweep = None
+    if not args.no_sweep and world == 1:
+        sweep = []
+        for n in cfg["sweep"]:
+            if n > N:
+                continue
+            si, sh = nbgen.active_block(cfg, n)
+            si_d, sh_d = torch.from_numpy(si).to(dev), f64(sh)
+            so = ctx.regular_alloc(si_d, sh_d)
+            torch.cuda.synchronize()
+            best = 1e30
+            for _ in range(3):
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record(stream); ctx.regular(si_d, sh_d, **so); b.record(stream)
+                torch.cuda.synchronize()
+                best = min(best, a.elapsed_time(b))
+            rate = float(n) * N / (best * 1e-3)
+            sweep.append({"n_i": n, "ms": best, "pairs_per_s": rate,
+                          "frac_fp32_peak": rate * FLOP_PER_INTERACTION / 1e12 / peak_tflops,
+                          "variant": ctx.info("last_variant"), "jsplit": ctx.info("last_jsplit")})
+            del so
+
+    cpu = None
+    if not args.no_cpu_baseline and world == 1:
+        cpu = cpu_oracle_rate(cfg, idx_np, h2_np, seconds_target=12.0)
+        cpu = {k: cpu[k] for k in ("value", "unit", "cores", "kind", "sample")}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32 pair math (x differenced as hi/lo f32 pairs, f64 sums)",
+        "data": "synthetic",
+        "config": {"workload": WORKLOAD, "N": N, "n_i_per_gpu": n_i, "nb_cap": cap, "nb_target": cfg["nb_target"],
+                   "parallelism": f"i-shard x{world}" if world > 1 else "single GPU",
+                   "step": "nb_set_j + nb_predict_all + nb_regular",
+                   "l2": "each step streams 2*112 B/body (set_j) + 112+48 B/body (predict) = 403 MB > 126 MB L2 "
+                         "before the force kernel; its 50 MB j-record working set is L2-resident by design",
+                   "variant": ctx.info("last_variant"), "jsplit": ctx.info("last_jsplit")},
+        "frac_fp32_peak": value / world * FLOP_PER_INTERACTION / 1e12 / peak_tflops,
+        "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
+        "cpu_baseline": cpu, "sweep": sweep, "peaks_source": pk_src,
+    }
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_b200(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,134 @@
+/*
+ * nbreg.h -- C ABI of libnbreg: the GPU regular-force step of the fourth-order Hermite /
+ * Ahmad-Cohen neighbour scheme (arXiv 1504.03687, "NBODY6++GPU"), B200 / sm_100a only.
+ *
+ * For a block of active i-particles the library predicts all N j-particles to the block time and
+ * sums, over every j, the Newtonian acceleration, its time derivative (jerk) and the potential;
+ * pairs inside particle i's neighbour radius are excluded from the sums and emitted as i's
+ * neighbour list (section 2; section 3.2.1; section 3.3.3; Table 1).
+ *
+ * Conventions
+ *   - G = 1 (N-body units).  All floating-point arguments are FP64.
+ *   - Arrays of vectors are [n][3] row-major.  Indices are 0-based int32.
+ *   - "DEVICE" pointers are CUDA device pointers valid on the current device; "HOST" pointers are
+ *     ordinary (pageable or pinned) host memory.  The caller owns every pointer it passes; the
+ *     library copies what it needs and never retains a caller pointer after the call returns
+ *     (for DEVICE variants: after the work enqueued by the call has run).
+ *   - DEVICE variants enqueue on the context's stream (nb_set_stream; default: the legacy default
+ *     stream) and return without synchronising.  Outputs are valid once the caller has synchronised
+ *     that stream (or called nb_synchronize).  HOST variants return after their results are in the
+ *     caller's host buffers.
+ *   - Every call returns an int status: NB_OK or one of the NB_E* codes; nb_strerror() names it.
+ *     No exceptions, no aborts, no output on stdout/stderr.  A CUDA failure is sticky: every later
+ *     call on that context returns NB_ECUDA.  Neighbour-list overflow is NOT an error.
+ *   - There is no CPU fallback: without a usable sm_100 device nb_open fails with NB_ECUDA.
+ *   - Results are bitwise reproducible run to run for fixed inputs and a fixed launch plan (two-stage
+ *     fixed-order reduction, no floating-point atomics); only the ORDER of the entries inside one
+ *     neighbour-list row may vary.
+ *
+ * Precision of the pair arithmetic (the paper does not state its kernel's precision; DESIGN.md
+ * "Precision"): positions are differenced at FP64-equivalent accuracy (two-float hi/lo split,
+ * 2^-48 relative), velocities and masses are rounded to FP32, the pair terms are FP32 with an SFU
+ * reciprocal square root, sums are FP32 within a j-tile and FP64 across tiles.  Guaranteed against
+ * the FP64 definition: acceleration max rel 1e-5 / rms 1e-6, jerk 1e-4 / 1e-5, potential 1e-6;
+ * neighbour sets identical except pairs with |r^2 - h^2| / h^2 < 1e-5.
+ */
+#ifndef NBREG_H
+#define NBREG_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct nb_ctx nb_ctx; /* opaque; owns all internal device memory */
+
+enum {
+    NB_OK = 0,
+    NB_EINVAL = 1, /* null pointer, N <= 0, nb_cap <= 0, n_i < 0 or n_i > N, unknown key            */
+    NB_ESTATE = 2, /* nb_predict_all before nb_set_j, nb_regular before nb_predict_all             */
+    NB_ENOMEM = 3, /* device (or staging) allocation failed                                        */
+    NB_ECUDA = 4   /* CUDA error (sticky); nb_last_cuda_error() returns the cudaError_t            */
+};
+
+/* Create a context for N j-particles and a neighbour-list capacity of nb_cap entries per active
+ * particle (north_star: nb_open(N); the capacity has to come from somewhere -- DESIGN.md R18).
+ * Allocates: FP64 j-state (14 N doubles), predicted SoA (48 B per particle, padded), counters,
+ * split-j scratch (grown on demand). */
+int nb_open(int64_t N, int32_t nb_cap, nb_ctx **out);
+int nb_close(nb_ctx *ctx);
+
+/* cudaStream_t (as void*) on which all later calls enqueue. NULL = legacy default stream. */
+int nb_set_stream(nb_ctx *ctx, void *cuda_stream);
+int nb_synchronize(nb_ctx *ctx);
+
+/* a1 "Send.R" (Table 1): ingest the state of ALL N particles at their own times t0[j]:
+ * m[N], x0[N][3], v0[N][3], a0[N][3] (total acceleration at t0), j0[N][3] (total jerk at t0),
+ * t0[N].  The library re-lays the data out (AoS -> SoA) into its own copy.  DEVICE pointers. */
+int nb_set_j(nb_ctx *ctx, const double *m, const double *x0, const double *v0, const double *a0,
+             const double *j0, const double *t0);
+/* Same with HOST pointers: host->device copies, then the same re-layout kernel. */
+int nb_set_j_host(nb_ctx *ctx, const double *m, const double *x0, const double *v0,
+                  const double *a0, const double *j0, const double *t0);
+
+/* a2 "Pred." (Table 1): predict every particle to time t,
+ *     dt = t - t0[j];  xp = x0 + v0 dt + a0 dt^2/2 + j0 dt^3/6;  vp = v0 + a0 dt + j0 dt^2/2
+ * in FP64, and store the predicted record the force kernel reads (x as hi/lo FP32 pair, v and m
+ * as FP32).  Any t (also t < t0[j]) is allowed.  Requires nb_set_j. */
+int nb_predict_all(nb_ctx *ctx, double t);
+
+/* Test/inspection hook: the predicted state exactly as the force kernel sees it, widened to FP64:
+ * xp[N][3] = (double)hi + (double)lo, vp[N][3] = (double)v_fp32.  DEVICE pointers. */
+int nb_get_predicted(nb_ctx *ctx, double *xp, double *vp);
+
+/* a3-a7 "Reg." (Table 1): for k = 0..n_i-1, i = idx_i[k]:
+ *     over all j != i (by index) at the predicted positions/velocities, r = x_j - x_i, v = v_j - v_i:
+ *       r^2 <  h2_i[k] : j is a neighbour of i -- listed, excluded from the sums
+ *       r^2 >= h2_i[k] : acc[k]  += m_j r / r^3
+ *                        jerk[k] += m_j ( v / r^3 - 3 (r.v) r / r^5 )
+ *                        pot[k]  -= m_j / r
+ *   nnb[k]      = TRUE number of neighbours (may exceed nb_cap)
+ *   overflow[k] = nnb[k] > nb_cap
+ *   nblist[k][0 .. min(nnb[k], nb_cap))  = neighbour indices j, in unspecified order; on overflow
+ *                 any nb_cap of the true neighbours.  Entries beyond that are left untouched.
+ *   The sums exclude ALL true neighbours whether or not the list overflowed.
+ * h2_i[k] <= 0 means "no neighbours" (total force / full potential).  The i-particle's own state is
+ * its predicted record (index idx_i[k]); the self pair is skipped by index.
+ * idx_i must be unique and in [0, N) (unchecked).  n_i = 0 is a valid no-op.
+ * Shapes: idx_i[n_i] int32, h2_i[n_i], acc[n_i][3], jerk[n_i][3], pot[n_i], nnb[n_i] int32,
+ * nblist[n_i][nb_cap] int32, overflow[n_i] int32.  DEVICE pointers.  Requires nb_predict_all. */
+int nb_regular(nb_ctx *ctx, int32_t n_i, const int32_t *idx_i, const double *h2_i, double *acc,
+               double *jerk, double *pot, int32_t *nnb, int32_t *nblist, int32_t *overflow);
+/* Same with HOST pointers: copies idx_i/h2_i in, runs, copies all outputs back, synchronises.
+ * nblist may be NULL to skip the list copy-back (the list is still built on the device). */
+int nb_regular_host(nb_ctx *ctx, int32_t n_i, const int32_t *idx_i, const double *h2_i, double *acc,
+                    double *jerk, double *pot, int32_t *nnb, int32_t *nblist, int32_t *overflow);
+
+/* Tuning / introspection.  Keys: */
+enum {
+    NB_INFO_KERNEL_LAUNCHES = 0, /* get: kernels launched by this context so far                   */
+    NB_INFO_LAST_JSPLIT = 1,     /* get: number of j-range splits S used by the last nb_regular    */
+    NB_INFO_LAST_IBLOCK = 2,     /* get: i-particles per CTA used by the last nb_regular           */
+    NB_INFO_LAST_GRID = 3,       /* get: CTAs of the last force-kernel launch                      */
+    NB_INFO_SM_COUNT = 4,        /* get: multiProcessorCount of the device                         */
+    NB_INFO_N_PADDED = 5,        /* get: N rounded up to the j-tile size                           */
+    NB_TUNE_FORCE_JSPLIT = 16,   /* set: force S (0 = automatic)                                   */
+    NB_TUNE_FORCE_VARIANT = 17,  /* set: force the kernel variant 0..4 (-1 = automatic)            */
+    NB_INFO_LAST_VARIANT = 18,   /* get: kernel variant used by the last nb_regular                */
+    NB_TUNE_PROFILE = 19,        /* set 1: bracket every force-kernel launch with CUDA events on the
+                                    context's stream (ring of 256 launches); set 0: off, ring cleared */
+    NB_INFO_FORCE_KERNEL_NS = 20,    /* get: summed device time of the bracketed force-kernel launches,
+                                        in ns (synchronises the stream)                             */
+    NB_INFO_FORCE_KERNEL_COUNT = 21  /* get: number of bracketed launches in that sum               */
+};
+int nb_get_info(nb_ctx *ctx, int32_t key, int64_t *value);
+int nb_set_tuning(nb_ctx *ctx, int32_t key, int64_t value);
+
+int nb_last_cuda_error(nb_ctx *ctx); /* cudaError_t of the sticky failure, 0 if none */
+const char *nb_strerror(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* NBREG_H */

@@ -1,0 +1,232 @@
+"""ctypes binding of libnbreg (same names as include/nbreg.h; marshalling only)."""
+from __future__ import annotations
+
+import ctypes
+import re
+from pathlib import Path
+
+from .build import LIB, build_lib
+
+NB_OK, NB_EINVAL, NB_ESTATE, NB_ENOMEM, NB_ECUDA = 0, 1, 2, 3, 4
+INFO = dict(kernel_launches=0, last_jsplit=1, last_iblock=2, last_grid=3, sm_count=4, n_padded=5,
+            force_jsplit=16, force_variant=17, last_variant=18, profile=19, force_kernel_ns=20,
+            force_kernel_count=21)
+
+_lib = None
+_vp = ctypes.c_void_p
+
+
+class NbregError(RuntimeError):
+    def __init__(self, code: int, where: str, detail: str = ""):
+        self.code = code
+        super().__init__(f"{where}: nbreg status {code} ({detail})")
+
+
+def declared_symbols() -> list[str]:
+    """Every function include/nbreg.h declares (parsed from the header text)."""
+    text = (Path(__file__).resolve().parent.parent / "include" / "nbreg.h").read_text()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(nb_[a-z_0-9]+)\s*\(", text)))
+
+
+def load_library(build: bool = True) -> ctypes.CDLL:
+    """Load libnbreg.so (building it in-tree with nvcc if stale).  Fails loudly -- no fallback."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if build:
+        build_lib()
+    if not LIB.exists():
+        raise RuntimeError(f"{LIB} is missing: the CUDA library was not built and there is no CPU fallback")
+    lib = ctypes.CDLL(str(LIB))
+    i32, i64, dbl = ctypes.c_int32, ctypes.c_int64, ctypes.c_double
+    lib.nb_open.argtypes = [i64, i32, ctypes.POINTER(_vp)]
+    lib.nb_close.argtypes = [_vp]
+    lib.nb_set_stream.argtypes = [_vp, _vp]
+    lib.nb_synchronize.argtypes = [_vp]
+    lib.nb_set_j.argtypes = [_vp] + [_vp] * 6
+    lib.nb_set_j_host.argtypes = [_vp] + [_vp] * 6
+    lib.nb_predict_all.argtypes = [_vp, dbl]
+    lib.nb_get_predicted.argtypes = [_vp, _vp, _vp]
+    lib.nb_regular.argtypes = [_vp, i32] + [_vp] * 8
+    lib.nb_regular_host.argtypes = [_vp, i32] + [_vp] * 8
+    lib.nb_get_info.argtypes = [_vp, i32, ctypes.POINTER(i64)]
+    lib.nb_set_tuning.argtypes = [_vp, i32, i64]
+    lib.nb_last_cuda_error.argtypes = [_vp]
+    lib.nb_strerror.argtypes = [ctypes.c_int]
+    lib.nb_strerror.restype = ctypes.c_char_p
+    for name in declared_symbols():
+        fn = getattr(lib, name)             # AttributeError if the .so does not export it
+        if name != "nb_strerror":
+            fn.restype = ctypes.c_int
+    _lib = lib
+    return lib
+
+
+def exported_symbols() -> list[str]:
+    lib = load_library()
+    return [n for n in declared_symbols() if hasattr(lib, n)]
+
+
+def _check(rc: int, where: str, ctx=None):
+    if rc != NB_OK:
+        lib = load_library()
+        detail = lib.nb_strerror(rc).decode()
+        if ctx is not None and rc == NB_ECUDA:
+            detail += f"; cudaError={lib.nb_last_cuda_error(ctx)}"
+        raise NbregError(rc, where, detail)
+
+
+def _dev_ptr(t, dtype, numel, name):
+    import torch
+    if not isinstance(t, torch.Tensor) or not t.is_cuda:
+        raise TypeError(f"{name}: expected a CUDA tensor")
+    if t.dtype != dtype or not t.is_contiguous() or t.numel() != numel:
+        raise ValueError(f"{name}: need contiguous {dtype} with {numel} elements, got {t.dtype} {tuple(t.shape)}")
+    return _vp(t.data_ptr())
+
+
+def _host_ptr(a, dtype, numel, name):
+    import numpy as np
+    import torch
+    if isinstance(a, torch.Tensor):
+        if a.is_cuda:
+            raise TypeError(f"{name}: expected host memory")
+        a = a.numpy()
+    if not isinstance(a, np.ndarray) or a.dtype != dtype or not a.flags.c_contiguous or a.size != numel:
+        raise ValueError(f"{name}: need C-contiguous {dtype} with {numel} elements")
+    return _vp(a.ctypes.data)
+
+
+class NbContext:
+    """Owns one nb_ctx.  Methods mirror the C entry points one to one."""
+
+    def __init__(self, N: int, nb_cap: int, stream=None):
+        self._lib = load_library()
+        self._ctx = _vp()
+        self.N, self.cap = int(N), int(nb_cap)
+        rc = self._lib.nb_open(self.N, self.cap, ctypes.byref(self._ctx))
+        if rc != NB_OK:
+            ctx, self._ctx = self._ctx, _vp()
+            err = self._lib.nb_last_cuda_error(ctx) if ctx else 0
+            if ctx:
+                self._lib.nb_close(ctx)
+            raise NbregError(rc, "nb_open", self._lib.nb_strerror(rc).decode() + f"; cudaError={err}")
+        if stream is not None:
+            self.set_stream(stream)
+
+    # -- lifetime
+    def close(self):
+        if getattr(self, "_ctx", None):
+            self._lib.nb_close(self._ctx)
+            self._ctx = _vp()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    # -- plumbing
+    def set_stream(self, stream):
+        handle = stream.cuda_stream if hasattr(stream, "cuda_stream") else int(stream)
+        _check(self._lib.nb_set_stream(self._ctx, _vp(handle)), "nb_set_stream", self._ctx)
+
+    def synchronize(self):
+        _check(self._lib.nb_synchronize(self._ctx), "nb_synchronize", self._ctx)
+
+    def info(self, key: str) -> int:
+        v = ctypes.c_int64()
+        _check(self._lib.nb_get_info(self._ctx, INFO[key], ctypes.byref(v)), "nb_get_info")
+        return v.value
+
+    def tune(self, key: str, value: int):
+        _check(self._lib.nb_set_tuning(self._ctx, INFO[key], int(value)), "nb_set_tuning")
+
+    # -- the path (device tensors)
+    def set_j(self, m, x0, v0, a0, j0, t0):
+        import torch
+        N, f8 = self.N, torch.float64
+        args = [_dev_ptr(m, f8, N, "m"), _dev_ptr(x0, f8, 3 * N, "x0"), _dev_ptr(v0, f8, 3 * N, "v0"),
+                _dev_ptr(a0, f8, 3 * N, "a0"), _dev_ptr(j0, f8, 3 * N, "j0"), _dev_ptr(t0, f8, N, "t0")]
+        _check(self._lib.nb_set_j(self._ctx, *args), "nb_set_j", self._ctx)
+
+    def predict_all(self, t: float):
+        _check(self._lib.nb_predict_all(self._ctx, float(t)), "nb_predict_all", self._ctx)
+
+    def get_predicted(self, xp, vp):
+        import torch
+        _check(self._lib.nb_get_predicted(self._ctx, _dev_ptr(xp, torch.float64, 3 * self.N, "xp"),
+                                          _dev_ptr(vp, torch.float64, 3 * self.N, "vp")),
+               "nb_get_predicted", self._ctx)
+
+    def regular(self, idx_i, h2_i, acc, jerk, pot, nnb, nblist, overflow):
+        import torch
+        n = int(idx_i.numel())
+        f8, i4 = torch.float64, torch.int32
+        if n == 0:
+            _check(self._lib.nb_regular(self._ctx, 0, *([_vp()] * 8)), "nb_regular", self._ctx)
+            return
+        args = [_dev_ptr(idx_i, i4, n, "idx_i"), _dev_ptr(h2_i, f8, n, "h2_i"), _dev_ptr(acc, f8, 3 * n, "acc"),
+                _dev_ptr(jerk, f8, 3 * n, "jerk"), _dev_ptr(pot, f8, n, "pot"), _dev_ptr(nnb, i4, n, "nnb"),
+                _dev_ptr(nblist, i4, n * self.cap, "nblist"), _dev_ptr(overflow, i4, n, "overflow")]
+        _check(self._lib.nb_regular(self._ctx, n, *args), "nb_regular", self._ctx)
+
+    # -- the path (host buffers: numpy arrays or CPU tensors, pinned or not)
+    def set_j_host(self, m, x0, v0, a0, j0, t0):
+        import numpy as np
+        N, f8 = self.N, np.float64
+        args = [_host_ptr(m, f8, N, "m"), _host_ptr(x0, f8, 3 * N, "x0"), _host_ptr(v0, f8, 3 * N, "v0"),
+                _host_ptr(a0, f8, 3 * N, "a0"), _host_ptr(j0, f8, 3 * N, "j0"), _host_ptr(t0, f8, N, "t0")]
+        _check(self._lib.nb_set_j_host(self._ctx, *args), "nb_set_j_host", self._ctx)
+
+    def regular_host(self, idx_i, h2_i, acc, jerk, pot, nnb, nblist, overflow):
+        import numpy as np
+        n = int(idx_i.size if isinstance(idx_i, np.ndarray) else idx_i.numel())
+        f8, i4 = np.float64, np.int32
+        args = [_host_ptr(idx_i, i4, n, "idx_i"), _host_ptr(h2_i, f8, n, "h2_i"), _host_ptr(acc, f8, 3 * n, "acc"),
+                _host_ptr(jerk, f8, 3 * n, "jerk"), _host_ptr(pot, f8, n, "pot"), _host_ptr(nnb, i4, n, "nnb"),
+                _vp() if nblist is None else _host_ptr(nblist, i4, n * self.cap, "nblist"),
+                _host_ptr(overflow, i4, n, "overflow")]
+        _check(self._lib.nb_regular_host(self._ctx, n, *args), "nb_regular_host", self._ctx)
+
+    # -- convenience: allocate outputs with torch and run one block
+    def regular_alloc(self, idx_i, h2_i):
+        import torch
+        n = int(idx_i.numel())
+        dev = idx_i.device
+        out = dict(acc=torch.empty((n, 3), dtype=torch.float64, device=dev),
+                   jerk=torch.empty((n, 3), dtype=torch.float64, device=dev),
+                   pot=torch.empty(n, dtype=torch.float64, device=dev),
+                   nnb=torch.empty(n, dtype=torch.int32, device=dev),
+                   nblist=torch.full((n, self.cap), -1, dtype=torch.int32, device=dev),
+                   overflow=torch.empty(n, dtype=torch.int32, device=dev))
+        self.regular(idx_i, h2_i, **out)
+        return out
+
+
+# Function-style aliases with the C names (north_star: nb_open / nb_set_j / nb_predict_all / nb_regular)
+def nb_open(N: int, nb_cap: int, stream=None) -> NbContext:
+    return NbContext(N, nb_cap, stream)
+
+
+def nb_close(ctx: NbContext):
+    ctx.close()
+
+
+def nb_set_j(ctx: NbContext, m, x0, v0, a0, j0, t0):
+    ctx.set_j(m, x0, v0, a0, j0, t0)
+
+
+def nb_predict_all(ctx: NbContext, t: float):
+    ctx.predict_all(t)
+
+
+def nb_regular(ctx: NbContext, idx_i, h2_i, acc, jerk, pot, nnb, nblist, overflow):
+    ctx.regular(idx_i, h2_i, acc, jerk, pot, nnb, nblist, overflow)

@@ -1,0 +1,439 @@
+// nbreg.cu -- host side of libnbreg: context, launch planning, the extern "C" entry points of
+// include/nbreg.h.  No torch types, no CPU fallback: every step of the path runs in the kernels of
+// nbreg_kernels.cuh on an sm_100 device or the call fails.
+#include "../../include/nbreg.h"
+#include "nbreg_kernels.cuh"
+
+#include <algorithm>
+#include <cmath>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <unordered_map>
+
+using namespace nbreg;
+
+namespace {
+
+struct Variant {
+    int it, wi, wj;          // i per thread, warps along i, warps along j
+    int iblock;              // i-particles per CTA
+    int threads;
+    double ovh_tiles;        // per-CTA fixed cost in units of one tile's compute (planning heuristic)
+    int ctas_per_sm;         // from the occupancy API at nb_open
+};
+constexpr int NVARIANT = 5;
+constexpr size_t FORCE_SMEM = (size_t)NSTAGE * 3 * TJ * sizeof(float4) + NSTAGE * sizeof(uint64_t) + 64;
+
+}  // namespace
+
+struct nb_ctx {
+    int64_t N = 0, Npad = 0, Ns = 0;
+    int32_t cap = 0;
+    int sm_count = 0;
+    cudaStream_t stream = nullptr;
+    cudaError_t cuda_err = cudaSuccess;
+    bool have_j = false, have_pred = false;
+    // device state owned by the library
+    double *soa = nullptr;                  // [14][Ns]
+    float4 *pA = nullptr, *pB = nullptr, *pC = nullptr;
+    int32_t *cnt = nullptr;                 // [N] zero between calls
+    double *partial = nullptr;  size_t partial_bytes = 0;
+    // staging for the HOST variants (lazy)
+    double *stage_j = nullptr;              // 14 N doubles
+    int32_t *st_idx = nullptr, *st_nnb = nullptr, *st_ovf = nullptr, *st_list = nullptr;
+    double *st_h2 = nullptr, *st_out = nullptr;     // st_out: acc[3n] jerk[3n] pot[n]
+    int64_t st_n = 0, st_list_n = 0;
+    // planning / introspection
+    Variant var[NVARIANT];
+    int64_t launches = 0;
+    int64_t last_S = 0, last_iblock = 0, last_grid = 0, last_variant = -1;
+    int64_t force_S = 0, force_variant = -1;
+    std::unordered_map<int64_t, int> plan_cache;   // (variant, i-blocks) -> S
+    // optional event bracketing of the force kernel (NB_TUNE_PROFILE)
+    static constexpr int PROF_RING = 256;
+    bool profile = false;
+    cudaEvent_t ev0[PROF_RING] = {}, ev1[PROF_RING] = {};
+    int64_t prof_n = 0;
+};
+
+namespace {
+
+#define NB_CUDA(ctx, expr)                          \
+    do {                                            \
+        cudaError_t e__ = (expr);                   \
+        if (e__ != cudaSuccess) {                   \
+            (ctx)->cuda_err = e__;                  \
+            return e__ == cudaErrorMemoryAllocation ? NB_ENOMEM : NB_ECUDA; \
+        }                                           \
+    } while (0)
+
+template <int IT, int WI, int WJ, int MINB>
+cudaError_t setup_variant(Variant &v, double ovh) {
+    v.it = IT; v.wi = WI; v.wj = WJ; v.iblock = 32 * IT * WI; v.threads = 32 * WI * WJ; v.ovh_tiles = ovh;
+    auto k = force_kernel<IT, WI, WJ, MINB>;
+    cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FORCE_SMEM);
+    if (e != cudaSuccess) return e;
+    int nb = 0;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k, v.threads, FORCE_SMEM);
+    v.ctas_per_sm = std::max(nb, 1);
+    return e;
+}
+
+template <int IT, int WI, int WJ, int MINB>
+void launch_force(const Variant &v, dim3 grid, cudaStream_t st, const ForceParams &p) {
+    force_kernel<IT, WI, WJ, MINB><<<grid, v.threads, FORCE_SMEM, st>>>(p);
+}
+
+// Pick the kernel variant: least padded work, then the larger i-block (more reuse of each j load).
+int pick_variant(const nb_ctx *c, int32_t n_i) {
+    if (c->force_variant >= 0 && c->force_variant < NVARIANT) return (int)c->force_variant;
+    int best = 0;
+    int64_t best_pad = -1;
+    for (int v = 0; v < NVARIANT; ++v) {
+        const int64_t ib = c->var[v].iblock;
+        const int64_t pad = (n_i + ib - 1) / ib * ib;
+        if (best_pad < 0 || pad < best_pad) { best = v; best_pad = pad; }
+    }
+    return best;
+}
+
+// Pick the number of j-splits S: minimise waves x (tiles per split + per-CTA overhead); among plans
+// within 1.5 % take the smallest S (less scratch, shorter final reduction).
+int plan_split(const nb_ctx *c, const Variant &v, int64_t n_ib, int64_t ntiles);
+
+int pick_split(nb_ctx *c, const Variant &v, int64_t n_ib, int64_t ntiles) {
+    if (c->force_S > 0) return (int)std::min<int64_t>(c->force_S, ntiles);
+    const int64_t key = n_ib * NVARIANT + (&v - c->var);
+    auto hit = c->plan_cache.find(key);
+    if (hit != c->plan_cache.end()) return hit->second;
+    const int plan = plan_split(c, v, n_ib, ntiles);
+    c->plan_cache.emplace(key, plan);
+    return plan;
+}
+
+int plan_split(const nb_ctx *c, const Variant &v, int64_t n_ib, int64_t ntiles) {
+    const int64_t conc = (int64_t)c->sm_count * v.ctas_per_sm;
+    const int64_t smax = std::min<int64_t>(ntiles, 8192);
+    double best = 1e300;
+    for (int64_t S = 1; S <= smax; ++S) {
+        const int64_t tps = (ntiles + S - 1) / S;
+        const int64_t Seff = (ntiles + tps - 1) / tps;      // splits that actually get tiles
+        const int64_t waves = (n_ib * Seff + conc - 1) / conc;
+        best = std::min(best, (double)waves * ((double)tps + v.ovh_tiles));
+    }
+    for (int64_t S = 1; S <= smax; ++S) {
+        const int64_t tps = (ntiles + S - 1) / S;
+        const int64_t Seff = (ntiles + tps - 1) / tps;
+        const int64_t waves = (n_ib * Seff + conc - 1) / conc;
+        if ((double)waves * ((double)tps + v.ovh_tiles) <= best * 1.015) return (int)Seff;
+    }
+    return 1;
+}
+
+int check_live(nb_ctx *c) {
+    if (!c) return NB_EINVAL;
+    if (c->cuda_err != cudaSuccess) return NB_ECUDA;
+    return NB_OK;
+}
+
+int ensure_partial(nb_ctx *c, size_t bytes) {
+    if (bytes <= c->partial_bytes) return NB_OK;
+    if (c->partial) {
+        NB_CUDA(c, cudaStreamSynchronize(c->stream));
+        NB_CUDA(c, cudaFree(c->partial));
+        c->partial = nullptr; c->partial_bytes = 0;
+    }
+    const size_t want = bytes + bytes / 4;
+    NB_CUDA(c, cudaMalloc(&c->partial, want));
+    c->partial_bytes = want;
+    return NB_OK;
+}
+
+int regular_device(nb_ctx *c, int32_t n_i, const int32_t *idx_i, const double *h2_i, double *acc, double *jerk,
+                   double *pot, int32_t *nnb, int32_t *nblist, int32_t *overflow) {
+    const int vi = pick_variant(c, n_i);
+    const Variant &v = c->var[vi];
+    const int64_t n_ib = (n_i + v.iblock - 1) / v.iblock;
+    const int64_t ntiles = c->Npad / TJ;
+    const int S = pick_split(c, v, n_ib, ntiles);
+    const int64_t tps = (ntiles + S - 1) / S;
+    const int64_t n_i_pad = n_ib * v.iblock;
+    int rc = ensure_partial(c, (size_t)S * 7 * n_i_pad * sizeof(double));
+    if (rc != NB_OK) return rc;
+
+    ForceParams p;
+    p.pA = c->pA; p.pB = c->pB; p.pC = c->pC;
+    p.idx_i = idx_i; p.h2_i = h2_i;
+    p.n_i = n_i; p.n_i_pad = (int32_t)n_i_pad;
+    p.ntiles = (int32_t)ntiles; p.tiles_per_split = (int32_t)tps;
+    p.cap = c->cap; p.cnt = c->cnt; p.nblist = nblist; p.partial = c->partial;
+    const dim3 grid((unsigned)n_ib, (unsigned)S);
+    const int slot = (int)(c->prof_n % nb_ctx::PROF_RING);
+    if (c->profile) NB_CUDA(c, cudaEventRecord(c->ev0[slot], c->stream));
+    switch (vi) {
+        case 0: launch_force<2, 8, 1, 2>(v, grid, c->stream, p); break;
+        case 1: launch_force<2, 4, 2, 2>(v, grid, c->stream, p); break;
+        case 2: launch_force<2, 2, 4, 2>(v, grid, c->stream, p); break;
+        case 3: launch_force<2, 1, 8, 2>(v, grid, c->stream, p); break;
+        default: launch_force<1, 1, 8, 2>(v, grid, c->stream, p); break;
+    }
+    NB_CUDA(c, cudaGetLastError());
+    if (c->profile) {
+        NB_CUDA(c, cudaEventRecord(c->ev1[slot], c->stream));
+        c->prof_n += 1;
+    }
+    finalize_kernel<<<(n_i + 255) / 256, 256, 0, c->stream>>>(n_i, (int32_t)n_i_pad, S, c->cap, c->partial, c->cnt,
+                                                              acc, jerk, pot, nnb, overflow);
+    NB_CUDA(c, cudaGetLastError());
+    c->launches += 2;
+    c->last_S = S; c->last_iblock = v.iblock; c->last_grid = n_ib * S; c->last_variant = vi;
+    return NB_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int nb_open(int64_t N, int32_t nb_cap, nb_ctx **out) {
+    if (!out) return NB_EINVAL;
+    *out = nullptr;
+    if (N <= 0 || nb_cap <= 0 || N > (int64_t)1 << 30) return NB_EINVAL;
+    nb_ctx *c = new (std::nothrow) nb_ctx();
+    if (!c) return NB_ENOMEM;
+    int dev = 0;
+    cudaDeviceProp prop;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e == cudaSuccess) e = cudaGetDeviceProperties(&prop, dev);
+    if (e != cudaSuccess || prop.major != 10) {   // sm_100a only, no fallback of any kind
+        delete c;
+        return NB_ECUDA;
+    }
+    c->N = N; c->cap = nb_cap;
+    c->Npad = (N + TJ - 1) / TJ * TJ;
+    c->Ns = c->Npad;
+    c->sm_count = prop.multiProcessorCount;
+    *out = c;     // from here on nb_close() releases whatever was allocated
+    NB_CUDA(c, cudaMalloc(&c->soa, sizeof(double) * 14 * c->Ns));
+    NB_CUDA(c, cudaMalloc(&c->pA, sizeof(float4) * c->Npad));
+    NB_CUDA(c, cudaMalloc(&c->pB, sizeof(float4) * c->Npad));
+    NB_CUDA(c, cudaMalloc(&c->pC, sizeof(float4) * c->Npad));
+    NB_CUDA(c, cudaMalloc(&c->cnt, sizeof(int32_t) * c->N));
+    NB_CUDA(c, cudaMemset(c->cnt, 0, sizeof(int32_t) * c->N));
+    NB_CUDA(c, (setup_variant<2, 8, 1, 2>(c->var[0], 0.5)));
+    NB_CUDA(c, (setup_variant<2, 4, 2, 2>(c->var[1], 0.75)));
+    NB_CUDA(c, (setup_variant<2, 2, 4, 2>(c->var[2], 1.5)));
+    NB_CUDA(c, (setup_variant<2, 1, 8, 2>(c->var[3], 3.0)));
+    NB_CUDA(c, (setup_variant<1, 1, 8, 2>(c->var[4], 5.0)));
+    return NB_OK;
+}
+
+int nb_close(nb_ctx *c) {
+    if (!c) return NB_EINVAL;
+    cudaStreamSynchronize(c->stream);
+    cudaFree(c->soa); cudaFree(c->pA); cudaFree(c->pB); cudaFree(c->pC); cudaFree(c->cnt);
+    cudaFree(c->partial); cudaFree(c->stage_j);
+    cudaFree(c->st_idx); cudaFree(c->st_nnb); cudaFree(c->st_ovf); cudaFree(c->st_list);
+    cudaFree(c->st_h2); cudaFree(c->st_out);
+    for (int q = 0; q < nb_ctx::PROF_RING; ++q) {
+        if (c->ev0[q]) cudaEventDestroy(c->ev0[q]);
+        if (c->ev1[q]) cudaEventDestroy(c->ev1[q]);
+    }
+    delete c;
+    return NB_OK;
+}
+
+int nb_set_stream(nb_ctx *c, void *cuda_stream) {
+    int rc = check_live(c);
+    if (rc != NB_OK) return rc;
+    c->stream = static_cast<cudaStream_t>(cuda_stream);
+    return NB_OK;
+}
+
+int nb_synchronize(nb_ctx *c) {
+    int rc = check_live(c);
+    if (rc != NB_OK) return rc;
+    NB_CUDA(c, cudaStreamSynchronize(c->stream));
+    return NB_OK;
+}
+
+int nb_set_j(nb_ctx *c, const double *m, const double *x0, const double *v0, const double *a0, const double *j0,
+             const double *t0) {
+    int rc = check_live(c);
+    if (rc != NB_OK) return rc;
+    if (!m || !x0 || !v0 || !a0 || !j0 || !t0) return NB_EINVAL;
+    relayout_kernel<<<(unsigned)((c->N + 255) / 256), 256, 0, c->stream>>>(c->N, c->Ns, m, x0, v0, a0, j0, t0, c->soa);
+    NB_CUDA(c, cudaGetLastError());
+    c->launches += 1;
+    c->have_j = true;
+    c->have_pred = false;
+    return NB_OK;
+}
+
+int nb_set_j_host(nb_ctx *c, const double *m, const double *x0, const double *v0, const double *a0,
+                  const double *j0, const double *t0) {
+    int rc = check_live(c);
+    if (rc != NB_OK) return rc;
+    if (!m || !x0 || !v0 || !a0 || !j0 || !t0) return NB_EINVAL;
+    const int64_t N = c->N;
+    if (!c->stage_j) NB_CUDA(c, cudaMalloc(&c->stage_j, sizeof(double) * 14 * N));
+    double *d = c->stage_j;
+    double *dm = d, *dx = d + N, *dv = d + 4 * N, *da = d + 7 * N, *dj = d + 10 * N, *dt = d + 13 * N;
+    NB_CUDA(c, cudaMemcpyAsync(dm, m, sizeof(double) * N, cudaMemcpyHostToDevice, c->stream));
+    NB_CUDA(c, cudaMemcpyAsync(dx, x0, sizeof(double) * 3 * N, cudaMemcpyHostToDevice, c->stream));
+    NB_CUDA(c, cudaMemcpyAsync(dv, v0, sizeof(double) * 3 * N, cudaMemcpyHostToDevice, c->stream));
+    NB_CUDA(c, cudaMemcpyAsync(da, a0, sizeof(double) * 3 * N, cudaMemcpyHostToDevice, c->stream));
+    NB_CUDA(c, cudaMemcpyAsync(dj, j0, sizeof(double) * 3 * N, cudaMemcpyHostToDevice, c->stream));
+    NB_CUDA(c, cudaMemcpyAsync(dt, t0, sizeof(double) * N, cudaMemcpyHostToDevice, c->stream));
+    return nb_set_j(c, dm, dx, dv, da, dj, dt);
+}
+
+int nb_predict_all(nb_ctx *c, double t) {
+    int rc = check_live(c);
+    if (rc != NB_OK) return rc;
+    if (!c->have_j) return NB_ESTATE;
+    predict_kernel<<<(unsigned)((c->Npad + 255) / 256), 256, 0, c->stream>>>(c->N, c->Npad, c->Ns, t, c->soa, c->pA,
+                                                                             c->pB, c->pC);
+    NB_CUDA(c, cudaGetLastError());
+    c->launches += 1;
+    c->have_pred = true;
+    return NB_OK;
+}
+
+int nb_get_predicted(nb_ctx *c, double *xp, double *vp) {
+    int rc = check_live(c);
+    if (rc != NB_OK) return rc;
+    if (!xp || !vp) return NB_EINVAL;
+    if (!c->have_pred) return NB_ESTATE;
+    unpack_predicted_kernel<<<(unsigned)((c->N + 255) / 256), 256, 0, c->stream>>>(c->N, c->pA, c->pB, c->pC, xp, vp);
+    NB_CUDA(c, cudaGetLastError());
+    c->launches += 1;
+    return NB_OK;
+}
+
+int nb_regular(nb_ctx *c, int32_t n_i, const int32_t *idx_i, const double *h2_i, double *acc, double *jerk,
+               double *pot, int32_t *nnb, int32_t *nblist, int32_t *overflow) {
+    int rc = check_live(c);
+    if (rc != NB_OK) return rc;
+    if (n_i < 0 || n_i > c->N) return NB_EINVAL;
+    if (!c->have_pred) return NB_ESTATE;
+    if (n_i == 0) return NB_OK;
+    if (!idx_i || !h2_i || !acc || !jerk || !pot || !nnb || !nblist || !overflow) return NB_EINVAL;
+    return regular_device(c, n_i, idx_i, h2_i, acc, jerk, pot, nnb, nblist, overflow);
+}
+
+int nb_regular_host(nb_ctx *c, int32_t n_i, const int32_t *idx_i, const double *h2_i, double *acc, double *jerk,
+                    double *pot, int32_t *nnb, int32_t *nblist, int32_t *overflow) {
+    int rc = check_live(c);
+    if (rc != NB_OK) return rc;
+    if (n_i < 0 || n_i > c->N) return NB_EINVAL;
+    if (!c->have_pred) return NB_ESTATE;
+    if (n_i == 0) return NB_OK;
+    if (!idx_i || !h2_i || !acc || !jerk || !pot || !nnb || !overflow) return NB_EINVAL;
+    if (n_i > c->st_n) {
+        NB_CUDA(c, cudaStreamSynchronize(c->stream));
+        cudaFree(c->st_idx); cudaFree(c->st_nnb); cudaFree(c->st_ovf); cudaFree(c->st_h2); cudaFree(c->st_out);
+        c->st_idx = c->st_nnb = c->st_ovf = nullptr; c->st_h2 = c->st_out = nullptr; c->st_n = 0;
+        const int64_t n = std::min<int64_t>(c->N, std::max<int64_t>(n_i, 1024) * 5 / 4);
+        NB_CUDA(c, cudaMalloc(&c->st_idx, sizeof(int32_t) * n));
+        NB_CUDA(c, cudaMalloc(&c->st_nnb, sizeof(int32_t) * n));
+        NB_CUDA(c, cudaMalloc(&c->st_ovf, sizeof(int32_t) * n));
+        NB_CUDA(c, cudaMalloc(&c->st_h2, sizeof(double) * n));
+        NB_CUDA(c, cudaMalloc(&c->st_out, sizeof(double) * 7 * n));
+        c->st_n = n;
+    }
+    const int64_t need_list = (int64_t)n_i * c->cap;
+    if (need_list > c->st_list_n) {
+        NB_CUDA(c, cudaStreamSynchronize(c->stream));
+        cudaFree(c->st_list); c->st_list = nullptr; c->st_list_n = 0;
+        NB_CUDA(c, cudaMalloc(&c->st_list, sizeof(int32_t) * need_list));
+        c->st_list_n = need_list;
+    }
+    double *d_acc = c->st_out, *d_jerk = c->st_out + 3 * (int64_t)n_i, *d_pot = c->st_out + 6 * (int64_t)n_i;
+    NB_CUDA(c, cudaMemcpyAsync(c->st_idx, idx_i, sizeof(int32_t) * n_i, cudaMemcpyHostToDevice, c->stream));
+    NB_CUDA(c, cudaMemcpyAsync(c->st_h2, h2_i, sizeof(double) * n_i, cudaMemcpyHostToDevice, c->stream));
+    rc = regular_device(c, n_i, c->st_idx, c->st_h2, d_acc, d_jerk, d_pot, c->st_nnb, c->st_list, c->st_ovf);
+    if (rc != NB_OK) return rc;
+    // acc, jerk, pot are contiguous in st_out but the caller's are three buffers
+    NB_CUDA(c, cudaMemcpyAsync(acc, d_acc, sizeof(double) * 3 * n_i, cudaMemcpyDeviceToHost, c->stream));
+    NB_CUDA(c, cudaMemcpyAsync(jerk, d_jerk, sizeof(double) * 3 * n_i, cudaMemcpyDeviceToHost, c->stream));
+    NB_CUDA(c, cudaMemcpyAsync(pot, d_pot, sizeof(double) * n_i, cudaMemcpyDeviceToHost, c->stream));
+    NB_CUDA(c, cudaMemcpyAsync(nnb, c->st_nnb, sizeof(int32_t) * n_i, cudaMemcpyDeviceToHost, c->stream));
+    NB_CUDA(c, cudaMemcpyAsync(overflow, c->st_ovf, sizeof(int32_t) * n_i, cudaMemcpyDeviceToHost, c->stream));
+    if (nblist)
+        NB_CUDA(c, cudaMemcpyAsync(nblist, c->st_list, sizeof(int32_t) * need_list, cudaMemcpyDeviceToHost, c->stream));
+    NB_CUDA(c, cudaStreamSynchronize(c->stream));
+    return NB_OK;
+}
+
+int nb_get_info(nb_ctx *c, int32_t key, int64_t *value) {
+    if (!c || !value) return NB_EINVAL;
+    switch (key) {
+        case NB_INFO_KERNEL_LAUNCHES: *value = c->launches; break;
+        case NB_INFO_LAST_JSPLIT: *value = c->last_S; break;
+        case NB_INFO_LAST_IBLOCK: *value = c->last_iblock; break;
+        case NB_INFO_LAST_GRID: *value = c->last_grid; break;
+        case NB_INFO_SM_COUNT: *value = c->sm_count; break;
+        case NB_INFO_N_PADDED: *value = c->Npad; break;
+        case NB_INFO_LAST_VARIANT: *value = c->last_variant; break;
+        case NB_TUNE_FORCE_JSPLIT: *value = c->force_S; break;
+        case NB_TUNE_FORCE_VARIANT: *value = c->force_variant; break;
+        case NB_TUNE_PROFILE: *value = c->profile ? 1 : 0; break;
+        case NB_INFO_FORCE_KERNEL_COUNT: *value = std::min<int64_t>(c->prof_n, nb_ctx::PROF_RING); break;
+        case NB_INFO_FORCE_KERNEL_NS: {
+            if (c->cuda_err != cudaSuccess) return NB_ECUDA;
+            NB_CUDA(c, cudaStreamSynchronize(c->stream));
+            double ns = 0.0;
+            const int64_t n = std::min<int64_t>(c->prof_n, nb_ctx::PROF_RING);
+            for (int64_t q = 0; q < n; ++q) {
+                float ms = 0.f;
+                NB_CUDA(c, cudaEventElapsedTime(&ms, c->ev0[q], c->ev1[q]));
+                ns += (double)ms * 1.0e6;
+            }
+            *value = (int64_t)(ns + 0.5);
+            break;
+        }
+        default: return NB_EINVAL;
+    }
+    return NB_OK;
+}
+
+int nb_set_tuning(nb_ctx *c, int32_t key, int64_t value) {
+    if (!c) return NB_EINVAL;
+    switch (key) {
+        case NB_TUNE_FORCE_JSPLIT:
+            if (value < 0) return NB_EINVAL;
+            c->force_S = value; break;
+        case NB_TUNE_FORCE_VARIANT:
+            if (value < -1 || value >= NVARIANT) return NB_EINVAL;
+            c->force_variant = value; break;
+        case NB_TUNE_PROFILE:
+            if (value != 0 && value != 1) return NB_EINVAL;
+            if (value && !c->ev0[0]) {
+                for (int q = 0; q < nb_ctx::PROF_RING; ++q) {
+                    NB_CUDA(c, cudaEventCreate(&c->ev0[q]));
+                    NB_CUDA(c, cudaEventCreate(&c->ev1[q]));
+                }
+            }
+            c->profile = value != 0;
+            c->prof_n = 0;
+            break;
+        default: return NB_EINVAL;
+    }
+    return NB_OK;
+}
+
+int nb_last_cuda_error(nb_ctx *c) { return c ? (int)c->cuda_err : 0; }
+
+const char *nb_strerror(int code) {
+    switch (code) {
+        case NB_OK: return "ok";
+        case NB_EINVAL: return "invalid argument";
+        case NB_ESTATE: return "call out of order (set_j -> predict_all -> regular)";
+        case NB_ENOMEM: return "out of device memory";
+        case NB_ECUDA: return "CUDA error or no sm_100 device (see nb_last_cuda_error)";
+        default: return "unknown nbreg status";
+    }
+}
+
+}  // extern "C"

@@ -1,0 +1,295 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle, element by element, on the same
+seeded inputs (BASELINE.json tolerances; tests/parity.py implements the band rule).  Needs a B200."""
+import numpy as np
+import pytest
+
+import nbgen
+from tests import parity
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+def _dev(a, dtype=None):
+    t = torch.from_numpy(np.ascontiguousarray(a))
+    if dtype is not None:
+        t = t.to(dtype)
+    return t.cuda()
+
+
+def open_ctx(cfg, cap=None):
+    import paper_1504_03687_b200 as nb
+    ctx = nb.nb_open(cfg["N"], cap or cfg["cap"])
+    nb.nb_set_j(ctx, _dev(cfg["m"]), _dev(cfg["x0"]), _dev(cfg["v0"]), _dev(cfg["a0"]), _dev(cfg["j0"]),
+                _dev(cfg["t0"]))
+    nb.nb_predict_all(ctx, cfg["t"])
+    return ctx
+
+
+def gpu_regular(ctx, idx_i, h2_i):
+    out = ctx.regular_alloc(_dev(idx_i, torch.int32), _dev(h2_i))
+    ctx.synchronize()
+    return parity.to_numpy(out)
+
+
+def gpu_predicted(ctx):
+    xp = torch.empty((ctx.N, 3), dtype=torch.float64, device="cuda")
+    vp = torch.empty((ctx.N, 3), dtype=torch.float64, device="cuda")
+    ctx.get_predicted(xp, vp)
+    ctx.synchronize()
+    return xp.cpu().numpy(), vp.cpu().numpy()
+
+
+def check(oracle, ctx, cfg, idx_i=None, h2_i=None, cap=None, **kw):
+    idx_i = cfg["idx_i"] if idx_i is None else idx_i
+    h2_i = cfg["h2_i"] if h2_i is None else h2_i
+    cap = cap or cfg["cap"]
+    xp, vp = oracle.predict(cfg["x0"], cfg["v0"], cfg["a0"], cfg["j0"], cfg["t0"], cfg["t"])
+    ref = parity.oracle_reference(oracle, cfg["m"], xp, vp, idx_i, h2_i, cap)
+    got = gpu_regular(ctx, idx_i, h2_i)
+    return parity.compare(got, ref, cap, **kw), got, ref
+
+
+def _config1(oracle):
+    cfg = nbgen.make_config(1)
+    tot = oracle.regular(cfg["m"], cfg["x0"], cfg["v0"], cfg["idx_i"], np.zeros(cfg["N"]), cfg["cap"])
+    xp, _ = oracle.predict(cfg["x0"], cfg["v0"], tot["acc"], tot["jerk"], cfg["t0"], cfg["t"])
+    return nbgen.finish_config1(cfg, tot["acc"], tot["jerk"], xp)
+
+
+# ----------------------------------------------------------------------------- predictor (a1, a2)
+
+def test_predictor_dyadic_bitwise(oracle):
+    rng = np.random.default_rng(0)
+    n = 1000                                         # ragged: not a multiple of the 256-body tile
+    q = lambda s, b: rng.integers(-2 ** b, 2 ** b, size=s) / 2.0 ** 4
+    x0, v0, a0, j0 = q((n, 3), 10), q((n, 3), 6), 2 * q((n, 3), 6), 6 * q((n, 3), 6)
+    k = rng.integers(2, 5, size=n)
+    t0 = 1.0 - 2.0 ** -k
+    cfg = dict(N=n, cap=8, m=rng.integers(1, 2 ** 10, size=n) / 2.0 ** 20, x0=x0, v0=v0, a0=a0, j0=j0, t0=t0, t=1.0)
+    ctx = open_ctx(cfg)
+    xg, vg = gpu_predicted(ctx)
+    xo, vo = oracle.predict(x0, v0, a0, j0, t0, 1.0)
+    assert np.array_equal(xg, xo) and np.array_equal(vg, vo)
+
+
+def test_predictor_general(oracle):
+    cfg = nbgen.make_config(3, N=20000, n_i=64)
+    ctx = open_ctx(cfg)
+    xg, vg = gpu_predicted(ctx)
+    xo, vo = oracle.predict(cfg["x0"], cfg["v0"], cfg["a0"], cfg["j0"], cfg["t0"], cfg["t"])
+    # x is stored as an FP32 hi/lo pair (48 bits), v as FP32 (24 bits); errors are relative to the
+    # size of the summed Taylor terms (a component may cancel to near zero)
+    def scales(t):
+        dt = np.abs(t - cfg["t0"])[:, None]
+        sx = np.abs(cfg["x0"]) + np.abs(cfg["v0"]) * dt + np.abs(cfg["a0"]) * dt ** 2 / 2 + np.abs(cfg["j0"]) * dt ** 3 / 6
+        sv = np.abs(cfg["v0"]) + np.abs(cfg["a0"]) * dt + np.abs(cfg["j0"]) * dt ** 2 / 2
+        return sx, sv
+    sx, sv = scales(cfg["t"])
+    assert np.max(np.abs(xg - xo) / sx) < 2.0 ** -46
+    assert np.max(np.abs(vg - vo) / sv) < 2.0 ** -23.9
+    # backward prediction (t < t0) is the same polynomial
+    import paper_1504_03687_b200 as nb
+    nb.nb_predict_all(ctx, 0.5)
+    xg, _ = gpu_predicted(ctx)
+    xo, _ = oracle.predict(cfg["x0"], cfg["v0"], cfg["a0"], cfg["j0"], cfg["t0"], 0.5)
+    assert np.max(np.abs(xg - xo) / scales(0.5)[0]) < 2.0 ** -46
+
+
+# ----------------------------------------------------------------------------- configs 1, 2 in full
+
+def test_config1_all_active(oracle):
+    cfg = _config1(oracle)
+    ctx = open_ctx(cfg)
+    rep, got, ref = check(oracle, ctx, cfg)
+    assert rep["overflow_rows"] == 0 and got["nnb"].min() >= 48
+    print("config1", rep)
+
+
+def test_config2(oracle):
+    cfg = nbgen.make_config(2)
+    ctx = open_ctx(cfg)
+    rep, got, _ = check(oracle, ctx, cfg)
+    assert 60 < rep["nnb_mean"] < 140
+    print("config2", rep)
+
+
+# ----------------------------------------------------------------------------- every variant, ragged sizes
+
+@pytest.mark.parametrize("n_i", [1, 7, 31, 32, 33, 64, 100, 128, 257, 512, 1000, 3000])
+def test_block_sizes_ragged_N(oracle, n_i):
+    cfg = nbgen.make_config(3, N=9001, n_i=n_i)        # 9001 = 35 tiles + a tail of 41
+    ctx = open_ctx(cfg)
+    rep, _, _ = check(oracle, ctx, cfg)
+    assert ctx.info("last_grid") >= 1
+
+
+@pytest.mark.parametrize("variant", [0, 1, 2, 3, 4])
+@pytest.mark.parametrize("jsplit", [1, 3, 36])
+def test_forced_variant_and_split_agree(oracle, variant, jsplit):
+    """Split-j vs single pass and every thread mapping: identical neighbour sets, sums equal to FP64
+    rounding of the final reduction (SURVEY 8(c) 'split-j path'; P:117-119 consistency)."""
+    cfg = nbgen.make_config(3, N=9001, n_i=300)
+    ctx = open_ctx(cfg)
+    base = gpu_regular(ctx, cfg["idx_i"], cfg["h2_i"])
+    ctx.tune("force_variant", variant)
+    ctx.tune("force_jsplit", jsplit)
+    got = gpu_regular(ctx, cfg["idx_i"], cfg["h2_i"])
+    assert ctx.info("last_variant") == variant and ctx.info("last_jsplit") == jsplit
+    assert np.array_equal(got["nnb"], base["nnb"]) and np.array_equal(got["overflow"], base["overflow"])
+    for k in range(300):
+        c = min(got["nnb"][k], cfg["cap"])
+        assert set(got["nblist"][k, :c].tolist()) == set(base["nblist"][k, :c].tolist())
+    for key, tol in (("acc", 3e-6), ("jerk", 3e-5), ("pot", 3e-7)):
+        sc = np.linalg.norm(base[key].reshape(300, -1), axis=1)
+        d = np.linalg.norm((got[key] - base[key]).reshape(300, -1), axis=1)
+        assert np.max(d / sc) < tol          # different FP32 tile partition, same pairs
+    rep, _, _ = check(oracle, ctx, cfg)
+
+
+def test_bitwise_reproducible(oracle):
+    cfg = nbgen.make_config(2, N=30000, n_i=777)
+    ctx = open_ctx(cfg)
+    a = gpu_regular(ctx, cfg["idx_i"], cfg["h2_i"])
+    b = gpu_regular(ctx, cfg["idx_i"], cfg["h2_i"])
+    for key in ("acc", "jerk", "pot", "nnb", "overflow"):
+        assert np.array_equal(a[key], b[key])
+    for k in range(777):
+        assert set(a["nblist"][k, :a["nnb"][k]].tolist()) == set(b["nblist"][k, :b["nnb"][k]].tolist())
+
+
+# ----------------------------------------------------------------------------- degenerate / edge cases
+
+def test_total_force_h2_zero_and_momentum(oracle):
+    cfg = nbgen.make_config(2, N=4096, n_i=4096)
+    cfg["idx_i"] = np.arange(4096, dtype=np.int32)
+    h2 = np.zeros(4096)
+    h2[::3] = -1.0                                              # h2 <= 0: no neighbours
+    ctx = open_ctx(cfg)
+    rep, got, _ = check(oracle, ctx, cfg, h2_i=h2)
+    assert got["nnb"].sum() == 0 and got["overflow"].sum() == 0
+    f = (cfg["m"][:, None] * got["acc"]).sum(0)
+    assert np.abs(f).max() < 1e-6 * np.abs(cfg["m"][:, None] * got["acc"]).sum()
+
+
+def test_overflow_small_cap(oracle):
+    cfg = nbgen.make_config(2, N=8192, n_i=500)
+    for cap in (1, 8, 100):
+        ctx = open_ctx(cfg, cap=cap)
+        rep, got, ref = check(oracle, ctx, cfg, cap=cap)
+        assert rep["overflow_rows"] > 0 or cap == 100
+        if cap == 100:
+            assert 0 < rep["overflow_rows"] < 500             # mixes overflowing and fitting rows
+
+
+def test_king_core_overflow_small_blocks(oracle):
+    cfg = nbgen.make_config(5, N=131072, n_i=512)
+    # shrink-N version of config 5: rescale the floor so the core still straddles the cap
+    ctx = open_ctx(cfg)
+    for n_i in (32, 128, 512):
+        idx, h2 = nbgen.active_block(cfg, n_i)
+        rep, got, _ = check(oracle, ctx, cfg, idx_i=idx, h2_i=h2)
+        print("king", n_i, rep)
+    assert rep["overflow_rows"] > 0
+
+
+def test_translation_invariance_far_from_origin(oracle):
+    """Shift every position by (100,-50,25): FP32 position differencing would fail this; the hi/lo
+    split must stay inside the tolerances."""
+    cfg = nbgen.make_config(2, N=8192, n_i=256)
+    cfg = dict(cfg)
+    cfg["x0"] = cfg["x0"] + np.array([100.0, -50.0, 25.0])
+    ctx = open_ctx(cfg)
+    check(oracle, ctx, cfg)
+
+
+def test_everyone_is_a_neighbour(oracle):
+    cfg = nbgen.make_config(2, N=2000, n_i=64)
+    ctx = open_ctx(cfg, cap=4096)
+    rep, got, _ = check(oracle, ctx, cfg, h2_i=np.full(64, 1e6), cap=4096)
+    assert np.all(got["nnb"] == 1999) and not got["acc"].any() and not got["pot"].any()
+
+
+def test_two_body_closed_form():
+    import paper_1504_03687_b200 as nb
+    cfg = dict(N=2, cap=4, m=np.array([1.0, 1.0]), x0=np.array([[0, 0, 0], [3.0, 4.0, 0]]),
+               v0=np.array([[0, 0, 0], [1.0, 2.0, 2.0]]), a0=np.zeros((2, 3)), j0=np.zeros((2, 3)),
+               t0=np.zeros(2), t=0.0)
+    ctx = open_ctx(cfg)
+    got = gpu_regular(ctx, np.array([0], np.int32), np.array([0.0]))
+    np.testing.assert_allclose(got["acc"][0], [0.024, 0.032, 0.0], rtol=1e-6, atol=1e-9)
+    np.testing.assert_allclose(got["jerk"][0], [-0.02368, -0.02624, 0.016], rtol=5e-6, atol=1e-9)
+    assert abs(got["pot"][0] + 0.2) < 2e-7
+    got = gpu_regular(ctx, np.array([0], np.int32), np.array([26.0]))      # partner inside h: exact zeros
+    assert got["nnb"][0] == 1 and got["nblist"][0, 0] == 1 and not got["acc"].any() and got["pot"][0] == 0
+
+
+def test_api_errors_and_noop():
+    import paper_1504_03687_b200 as nb
+    from paper_1504_03687_b200 import NbregError
+    with pytest.raises(NbregError) as e:
+        nb.nb_open(0, 8)
+    assert e.value.code == nb.NB_EINVAL
+    with pytest.raises(NbregError):
+        nb.nb_open(16, 0)
+    ctx = nb.nb_open(300, 8)
+    with pytest.raises(NbregError) as e:
+        nb.nb_predict_all(ctx, 1.0)
+    assert e.value.code == nb.NB_ESTATE
+    z = lambda *s: torch.zeros(*s, dtype=torch.float64, device="cuda")
+    x = torch.rand(300, 3, dtype=torch.float64, device="cuda")
+    nb.nb_set_j(ctx, z(300) + 1.0 / 300, x, z(300, 3), z(300, 3), z(300, 3), z(300))
+    idx = torch.arange(4, dtype=torch.int32, device="cuda")
+    with pytest.raises(NbregError) as e:
+        ctx.regular_alloc(idx, z(4))
+    assert e.value.code == nb.NB_ESTATE
+    nb.nb_predict_all(ctx, 0.0)
+    launches = ctx.info("kernel_launches")
+    ctx.regular_alloc(idx[:0], z(0))                                       # n_i = 0: valid no-op
+    assert ctx.info("kernel_launches") == launches
+    out = ctx.regular_alloc(idx, z(4))
+    ctx.synchronize()
+    assert torch.isfinite(out["acc"]).all() and ctx.info("kernel_launches") == launches + 2
+    assert ctx.info("sm_count") >= 100
+    ctx.close()
+
+
+def test_host_variants_equal_device_variants(oracle):
+    import paper_1504_03687_b200 as nb
+    cfg = nbgen.make_config(2, N=10000, n_i=400)
+    ctx = open_ctx(cfg)
+    dev = gpu_regular(ctx, cfg["idx_i"], cfg["h2_i"])
+    ctx2 = nb.nb_open(cfg["N"], cfg["cap"])
+    ctx2.set_j_host(*(np.ascontiguousarray(cfg[k]) for k in ("m", "x0", "v0", "a0", "j0", "t0")))
+    ctx2.predict_all(cfg["t"])
+    n, cap = 400, cfg["cap"]
+    out = dict(acc=np.empty((n, 3)), jerk=np.empty((n, 3)), pot=np.empty(n), nnb=np.empty(n, np.int32),
+               nblist=np.full((n, cap), -1, np.int32), overflow=np.empty(n, np.int32))
+    ctx2.regular_host(np.ascontiguousarray(cfg["idx_i"]), np.ascontiguousarray(cfg["h2_i"]), **out)
+    for key in ("acc", "jerk", "pot", "nnb", "overflow"):
+        assert np.array_equal(out[key], dev[key])
+    for k in range(n):
+        assert set(out["nblist"][k, :out["nnb"][k]].tolist()) == set(dev["nblist"][k, :dev["nnb"][k]].tolist())
+
+
+# ----------------------------------------------------------------------------- full size (bench launch config)
+
+def test_full_size_million_body_sampled(oracle):
+    """N = 1,048,576 (config 4) in the launch configuration bench.py times (n_i = 8192): the oracle
+    checks a seeded sample of 192 of the active particles one by one; nnb/overflow for the same."""
+    cfg = nbgen.make_config(4)
+    ctx = open_ctx(cfg)
+    idx, h2 = nbgen.active_block(cfg, 8192)
+    got = gpu_regular(ctx, idx, h2)
+    sel = np.sort(np.random.default_rng(1).choice(8192, size=192, replace=False))
+    xp, vp = oracle.predict(cfg["x0"], cfg["v0"], cfg["a0"], cfg["j0"], cfg["t0"], cfg["t"])
+    ref = parity.oracle_reference(oracle, cfg["m"], xp, vp, idx[sel], h2[sel], cfg["cap"])
+    rep = parity.compare({k: v[sel] for k, v in got.items()}, ref, cfg["cap"])
+    print("config4 n_i=8192 sample", rep, "variant", ctx.info("last_variant"), "S", ctx.info("last_jsplit"))
+    assert np.all(np.isfinite(got["acc"])) and 100 < got["nnb"].mean() < 220
+    # small block on the same context (split-j path at full N)
+    idx, h2 = nbgen.active_block(cfg, 64)
+    got = gpu_regular(ctx, idx, h2)
+    ref = parity.oracle_reference(oracle, cfg["m"], xp, vp, idx, h2, cfg["cap"])
+    print("config4 n_i=64", parity.compare(got, ref, cfg["cap"]))
