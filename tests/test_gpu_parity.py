@@ -156,7 +156,8 @@ def test_bitwise_reproducible(oracle):
     for key in ("acc", "jerk", "pot", "nnb", "overflow"):
         assert np.array_equal(a[key], b[key])
     for k in range(777):
-        assert set(a["nblist"][k, :a["nnb"][k]].tolist()) == set(b["nblist"][k, :b["nnb"][k]].tolist())
+        if a["nnb"][k] <= cfg["cap"]:       # an overflowed row holds ANY cap-sized subset (reading R10)
+            assert set(a["nblist"][k, :a["nnb"][k]].tolist()) == set(b["nblist"][k, :b["nnb"][k]].tolist())
 
 
 # ----------------------------------------------------------------------------- degenerate / edge cases
@@ -270,7 +271,8 @@ def test_host_variants_equal_device_variants(oracle):
     for key in ("acc", "jerk", "pot", "nnb", "overflow"):
         assert np.array_equal(out[key], dev[key])
     for k in range(n):
-        assert set(out["nblist"][k, :out["nnb"][k]].tolist()) == set(dev["nblist"][k, :dev["nnb"][k]].tolist())
+        if dev["nnb"][k] <= cap:
+            assert set(out["nblist"][k, :out["nnb"][k]].tolist()) == set(dev["nblist"][k, :dev["nnb"][k]].tolist())
 
 
 # ----------------------------------------------------------------------------- full size (bench launch config)
