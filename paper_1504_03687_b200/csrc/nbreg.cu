@@ -22,8 +22,8 @@ struct Variant {
     double ovh_tiles;        // per-CTA fixed cost in units of one tile's compute (planning heuristic)
     int ctas_per_sm;         // from the occupancy API at nb_open
 };
-constexpr int NVARIANT = 5;
-constexpr size_t FORCE_SMEM = (size_t)NSTAGE * 3 * TJ * sizeof(float4) + NSTAGE * sizeof(uint64_t) + 64;
+constexpr int NVARIANT = 4;
+constexpr size_t FORCE_SMEM = (size_t)NSTAGE * TJ * RECQ * sizeof(float4) + NSTAGE * sizeof(uint64_t) + 64;
 
 }  // namespace
 
@@ -36,7 +36,7 @@ struct nb_ctx {
     bool have_j = false, have_pred = false;
     // device state owned by the library
     double *soa = nullptr;                  // [14][Ns]
-    float4 *pA = nullptr, *pB = nullptr, *pC = nullptr;
+    float4 *rec = nullptr;                  // predicted records [Npad][RECQ]
     int32_t *cnt = nullptr;                 // [N] zero between calls
     double *partial = nullptr;  size_t partial_bytes = 0;
     // staging for the HOST variants (lazy)
@@ -68,10 +68,10 @@ namespace {
         }                                           \
     } while (0)
 
-template <int IT, int WI, int WJ, int MINB>
+template <int WI, int WJ, int MINB>
 cudaError_t setup_variant(Variant &v, double ovh) {
-    v.it = IT; v.wi = WI; v.wj = WJ; v.iblock = 32 * IT * WI; v.threads = 32 * WI * WJ; v.ovh_tiles = ovh;
-    auto k = force_kernel<IT, WI, WJ, MINB>;
+    v.it = 2; v.wi = WI; v.wj = WJ; v.iblock = 64 * WI; v.threads = 32 * WI * WJ; v.ovh_tiles = ovh;
+    auto k = force_kernel<WI, WJ, MINB>;
     cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FORCE_SMEM);
     if (e != cudaSuccess) return e;
     int nb = 0;
@@ -80,9 +80,9 @@ cudaError_t setup_variant(Variant &v, double ovh) {
     return e;
 }
 
-template <int IT, int WI, int WJ, int MINB>
+template <int WI, int WJ, int MINB>
 void launch_force(const Variant &v, dim3 grid, cudaStream_t st, const ForceParams &p) {
-    force_kernel<IT, WI, WJ, MINB><<<grid, v.threads, FORCE_SMEM, st>>>(p);
+    force_kernel<WI, WJ, MINB><<<grid, v.threads, FORCE_SMEM, st>>>(p);
 }
 
 // Pick the kernel variant: least padded work, then the larger i-block (more reuse of each j load).
@@ -163,7 +163,7 @@ int regular_device(nb_ctx *c, int32_t n_i, const int32_t *idx_i, const double *h
     if (rc != NB_OK) return rc;
 
     ForceParams p;
-    p.pA = c->pA; p.pB = c->pB; p.pC = c->pC;
+    p.rec = c->rec;
     p.idx_i = idx_i; p.h2_i = h2_i;
     p.n_i = n_i; p.n_i_pad = (int32_t)n_i_pad;
     p.ntiles = (int32_t)ntiles; p.tiles_per_split = (int32_t)tps;
@@ -172,18 +172,17 @@ int regular_device(nb_ctx *c, int32_t n_i, const int32_t *idx_i, const double *h
     const int slot = (int)(c->prof_n % nb_ctx::PROF_RING);
     if (c->profile) NB_CUDA(c, cudaEventRecord(c->ev0[slot], c->stream));
     switch (vi) {
-        case 0: launch_force<2, 8, 1, 2>(v, grid, c->stream, p); break;
-        case 1: launch_force<2, 4, 2, 2>(v, grid, c->stream, p); break;
-        case 2: launch_force<2, 2, 4, 2>(v, grid, c->stream, p); break;
-        case 3: launch_force<2, 1, 8, 2>(v, grid, c->stream, p); break;
-        default: launch_force<1, 1, 8, 2>(v, grid, c->stream, p); break;
+        case 0: launch_force<8, 1, 2>(v, grid, c->stream, p); break;
+        case 1: launch_force<4, 2, 2>(v, grid, c->stream, p); break;
+        case 2: launch_force<2, 4, 2>(v, grid, c->stream, p); break;
+        default: launch_force<1, 8, 2>(v, grid, c->stream, p); break;
     }
     NB_CUDA(c, cudaGetLastError());
     if (c->profile) {
         NB_CUDA(c, cudaEventRecord(c->ev1[slot], c->stream));
         c->prof_n += 1;
     }
-    finalize_kernel<<<(n_i + 255) / 256, 256, 0, c->stream>>>(n_i, (int32_t)n_i_pad, S, c->cap, c->partial, c->cnt,
+    finalize_kernel<<<(n_i + 7) / 8, 256, 0, c->stream>>>(n_i, (int32_t)n_i_pad, S, c->cap, c->partial, c->cnt,
                                                               acc, jerk, pot, nnb, overflow);
     NB_CUDA(c, cudaGetLastError());
     c->launches += 2;
@@ -215,23 +214,20 @@ int nb_open(int64_t N, int32_t nb_cap, nb_ctx **out) {
     c->sm_count = prop.multiProcessorCount;
     *out = c;     // from here on nb_close() releases whatever was allocated
     NB_CUDA(c, cudaMalloc(&c->soa, sizeof(double) * 14 * c->Ns));
-    NB_CUDA(c, cudaMalloc(&c->pA, sizeof(float4) * c->Npad));
-    NB_CUDA(c, cudaMalloc(&c->pB, sizeof(float4) * c->Npad));
-    NB_CUDA(c, cudaMalloc(&c->pC, sizeof(float4) * c->Npad));
+    NB_CUDA(c, cudaMalloc(&c->rec, sizeof(float4) * RECQ * c->Npad));
     NB_CUDA(c, cudaMalloc(&c->cnt, sizeof(int32_t) * c->N));
     NB_CUDA(c, cudaMemset(c->cnt, 0, sizeof(int32_t) * c->N));
-    NB_CUDA(c, (setup_variant<2, 8, 1, 2>(c->var[0], 0.5)));
-    NB_CUDA(c, (setup_variant<2, 4, 2, 2>(c->var[1], 0.75)));
-    NB_CUDA(c, (setup_variant<2, 2, 4, 2>(c->var[2], 1.5)));
-    NB_CUDA(c, (setup_variant<2, 1, 8, 2>(c->var[3], 3.0)));
-    NB_CUDA(c, (setup_variant<1, 1, 8, 2>(c->var[4], 5.0)));
+    NB_CUDA(c, (setup_variant<8, 1, 2>(c->var[0], 0.5)));
+    NB_CUDA(c, (setup_variant<4, 2, 2>(c->var[1], 0.75)));
+    NB_CUDA(c, (setup_variant<2, 4, 2>(c->var[2], 1.5)));
+    NB_CUDA(c, (setup_variant<1, 8, 2>(c->var[3], 3.0)));
     return NB_OK;
 }
 
 int nb_close(nb_ctx *c) {
     if (!c) return NB_EINVAL;
     cudaStreamSynchronize(c->stream);
-    cudaFree(c->soa); cudaFree(c->pA); cudaFree(c->pB); cudaFree(c->pC); cudaFree(c->cnt);
+    cudaFree(c->soa); cudaFree(c->rec); cudaFree(c->cnt);
     cudaFree(c->partial); cudaFree(c->stage_j);
     cudaFree(c->st_idx); cudaFree(c->st_nnb); cudaFree(c->st_ovf); cudaFree(c->st_list);
     cudaFree(c->st_h2); cudaFree(c->st_out);
@@ -292,8 +288,7 @@ int nb_predict_all(nb_ctx *c, double t) {
     int rc = check_live(c);
     if (rc != NB_OK) return rc;
     if (!c->have_j) return NB_ESTATE;
-    predict_kernel<<<(unsigned)((c->Npad + 255) / 256), 256, 0, c->stream>>>(c->N, c->Npad, c->Ns, t, c->soa, c->pA,
-                                                                             c->pB, c->pC);
+    predict_kernel<<<(unsigned)((c->Npad + 255) / 256), 256, 0, c->stream>>>(c->N, c->Npad, c->Ns, t, c->soa, c->rec);
     NB_CUDA(c, cudaGetLastError());
     c->launches += 1;
     c->have_pred = true;
@@ -305,7 +300,7 @@ int nb_get_predicted(nb_ctx *c, double *xp, double *vp) {
     if (rc != NB_OK) return rc;
     if (!xp || !vp) return NB_EINVAL;
     if (!c->have_pred) return NB_ESTATE;
-    unpack_predicted_kernel<<<(unsigned)((c->N + 255) / 256), 256, 0, c->stream>>>(c->N, c->pA, c->pB, c->pC, xp, vp);
+    unpack_predicted_kernel<<<(unsigned)((c->N + 255) / 256), 256, 0, c->stream>>>(c->N, c->rec, xp, vp);
     NB_CUDA(c, cudaGetLastError());
     c->launches += 1;
     return NB_OK;
