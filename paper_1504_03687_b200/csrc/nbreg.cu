@@ -23,7 +23,8 @@ struct Variant {
     int ctas_per_sm;         // from the occupancy API at nb_open
 };
 constexpr int NVARIANT = 4;
-constexpr size_t FORCE_SMEM = (size_t)NSTAGE * TJ * RECQ * sizeof(float4) + NSTAGE * sizeof(uint64_t) + 64;
+constexpr int NAUTO = 4;        // variants the planner picks from; the rest only by NB_TUNE_FORCE_VARIANT
+constexpr size_t FORCE_SMEM = (size_t)NSTAGE * TILE_FLOATS * sizeof(float) + NSTAGE * sizeof(uint64_t) + 64;
 
 }  // namespace
 
@@ -36,7 +37,7 @@ struct nb_ctx {
     bool have_j = false, have_pred = false;
     // device state owned by the library
     double *soa = nullptr;                  // [14][Ns]
-    float4 *rec = nullptr;                  // predicted records [Npad][RECQ]
+    float *rec = nullptr;                   // predicted records [Npad / TJ][RECF][TJ]
     int32_t *cnt = nullptr;                 // [N] zero between calls
     double *partial = nullptr;  size_t partial_bytes = 0;
     // staging for the HOST variants (lazy)
@@ -70,6 +71,7 @@ namespace {
 
 template <int WI, int WJ, int MINB>
 cudaError_t setup_variant(Variant &v, double ovh) {
+    static_assert(WJ == 1 || (size_t)WJ * 7 * 64 * WI * sizeof(double) <= FORCE_SMEM, "WJ reduction reuses the ring");
     v.it = 2; v.wi = WI; v.wj = WJ; v.iblock = 64 * WI; v.threads = 32 * WI * WJ; v.ovh_tiles = ovh;
     auto k = force_kernel<WI, WJ, MINB>;
     cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FORCE_SMEM);
@@ -90,7 +92,7 @@ int pick_variant(const nb_ctx *c, int32_t n_i) {
     if (c->force_variant >= 0 && c->force_variant < NVARIANT) return (int)c->force_variant;
     int best = 0;
     int64_t best_pad = -1;
-    for (int v = 0; v < NVARIANT; ++v) {
+    for (int v = 0; v < NAUTO; ++v) {
         const int64_t ib = c->var[v].iblock;
         const int64_t pad = (n_i + ib - 1) / ib * ib;
         if (best_pad < 0 || pad < best_pad) { best = v; best_pad = pad; }
@@ -214,7 +216,7 @@ int nb_open(int64_t N, int32_t nb_cap, nb_ctx **out) {
     c->sm_count = prop.multiProcessorCount;
     *out = c;     // from here on nb_close() releases whatever was allocated
     NB_CUDA(c, cudaMalloc(&c->soa, sizeof(double) * 14 * c->Ns));
-    NB_CUDA(c, cudaMalloc(&c->rec, sizeof(float4) * RECQ * c->Npad));
+    NB_CUDA(c, cudaMalloc(&c->rec, sizeof(float) * RECF * c->Npad));
     NB_CUDA(c, cudaMalloc(&c->cnt, sizeof(int32_t) * c->N));
     NB_CUDA(c, cudaMemset(c->cnt, 0, sizeof(int32_t) * c->N));
     NB_CUDA(c, (setup_variant<8, 1, 2>(c->var[0], 0.5)));

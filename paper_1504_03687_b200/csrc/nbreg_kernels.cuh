@@ -1,18 +1,19 @@
 // nbreg_kernels.cuh -- sm_100a device code of libnbreg (see include/nbreg.h for the contract).
 //
 //   relayout_kernel   a1  AoS [N][3] FP64 -> internal SoA FP64                    (HBM-bound)
-//   predict_kernel    a2  Hermite predictor, FP64 -> predicted record (48 B/body) (HBM-bound)
+//   predict_kernel    a2  Hermite predictor, FP64 -> predicted record (40 B/body) (HBM-bound)
 //   force_kernel      a3-a6  i-block x j-tile pairwise sum + neighbour lists      (FP32 issue-bound)
 //   finalize_kernel   a6-a7  fixed-order sum over j-splits, write-back, counters  (tiny)
 //
-// Predicted record: 80 B per body, five float4 with every value DUPLICATED into an aligned pair,
-//   q0 = (xh,xh, yh,yh)  q1 = (zh,zh, m,m)  q2 = (xl,xl, yl,yl)  q3 = (zl,zl, vx,vx)  q4 = (vy,vy, vz,vz)
-// so that one warp-uniform LDS.128 hands the force kernel two ready-made f32x2 operands: each thread
-// owns a PAIR of i-particles and every FP32 operation of the pair arithmetic is one packed
-// FADD2/FMUL2/FFMA2 (sm_100 only) -- half the issue slots of scalar FP32 at the same lane rate.
-// x = hi + lo with hi = fl32(x), lo = fl32(x - hi): positions carry 48 significant bits, so
-// (hi_j - hi_i) + (lo_j - lo_i) is the FP64 difference rounded once to FP32 -- the pair arithmetic
-// after that is plain FP32.  A j-tile (256 records, 20 KB) is ONE TMA bulk copy.
+// Predicted record: 40 B per body = ten FP32 values (xh,yh,zh, xl,yl,zl, vx,vy,vz, m), stored
+// COMPONENT-MAJOR INSIDE EACH j-TILE: rec[tile][component][TJ].  A tile (256 bodies, 10 KB) is ONE
+// contiguous TMA bulk copy, and one warp-uniform LDS.128 hands the force kernel the same component of
+// four consecutive j.  Each thread owns PAIRS of i-particles: every FP32 operation of the pair
+// arithmetic is one packed FADD2/FMUL2/FFMA2 (sm_100 f32x2) whose j-side operand is a 32-bit scalar
+// broadcast to both halves (SASS operand form `R.F32`), so a j value costs one register read and the
+// records need no duplication.  x = hi + lo with hi = fl32(x), lo = fl32(x - hi): positions carry 48
+// significant bits, so (hi_j - hi_i) + (lo_j - lo_i) is the FP64 difference rounded once to FP32 --
+// the pair arithmetic after that is plain FP32.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -20,8 +21,10 @@
 namespace nbreg {
 
 constexpr int TJ = 256;        // j-particles per shared-memory tile
-constexpr int RECQ = 5;        // float4 per predicted record (80 B)
-constexpr int NSTAGE = 3;      // tiles in flight per CTA (bulk-copy ring)
+constexpr int RECF = 10;       // floats per predicted record (40 B)
+constexpr int NSTAGE = 4;      // tiles in flight per CTA (bulk-copy ring)
+constexpr int TILE_FLOATS = TJ * RECF;
+enum { C_XH = 0, C_YH, C_ZH, C_XL, C_YL, C_ZL, C_VX, C_VY, C_VZ, C_M };   // component rows of a tile
 constexpr int UNROLL_J = 4;    // j's per neighbour-detection group
 constexpr float GHOST_POS = 1.0e15f;   // padding j's sit here with m = 0
 constexpr float TINY_H2 = 1.17549435e-38f;  // FLT_MIN: masks exactly the r2 == 0 self pair when h2 <= 0
@@ -89,21 +92,28 @@ __global__ void __launch_bounds__(256) relayout_kernel(int64_t N, int64_t Ns, co
 
 // ------------------------------------------------------------------ a2: predictor
 // xp = x0 + v0 dt + a0 dt^2/2 + j0 dt^3/6,  vp = v0 + a0 dt + j0 dt^2/2   (reading R2)
+__device__ __forceinline__ float *rec_slot(float *rec, int64_t j) {      // &rec[tile][0][j % TJ]
+    return rec + (j / TJ) * TILE_FLOATS + (j % TJ);
+}
+__device__ __forceinline__ const float *rec_slot(const float *rec, int64_t j) {
+    return rec + (j / TJ) * TILE_FLOATS + (j % TJ);
+}
+
 __global__ void __launch_bounds__(256) predict_kernel(int64_t N, int64_t Npad, int64_t Ns, double t,
-                                                      const double *__restrict__ soa, float4 *__restrict__ rec) {
+                                                      const double *__restrict__ soa, float *__restrict__ rec) {
     int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= Npad) return;
-    float4 *r = rec + j * RECQ;
+    float *r = rec_slot(rec, j);
     if (j >= N) {   // ghost padding: massless, far away, never a neighbour, contributes exactly 0
-        r[0] = make_float4(GHOST_POS, GHOST_POS, GHOST_POS, GHOST_POS);
-        r[1] = make_float4(GHOST_POS, GHOST_POS, 0.f, 0.f);
-        r[2] = r[3] = r[4] = make_float4(0.f, 0.f, 0.f, 0.f);
+        r[C_XH * TJ] = r[C_YH * TJ] = r[C_ZH * TJ] = GHOST_POS;
+        r[C_XL * TJ] = r[C_YL * TJ] = r[C_ZL * TJ] = 0.f;
+        r[C_VX * TJ] = r[C_VY * TJ] = r[C_VZ * TJ] = 0.f;
+        r[C_M * TJ] = 0.f;
         return;
     }
     const double dt = t - soa[13 * Ns + j];
     const double c2 = 0.5 * (dt * dt);                    // dt^2/2: exact for dyadic dt
     const double c3 = (dt * dt * dt) * (1.0 / 6.0);       // dt^3/6: the only inexact coefficient
-    float hi[3], lo[3], vf[3];
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
         const double x = soa[(1 + c) * Ns + j], v = soa[(4 + c) * Ns + j];
@@ -113,35 +123,29 @@ __global__ void __launch_bounds__(256) predict_kernel(int64_t N, int64_t Npad, i
         const double p3 = __dmul_rn(jk, c3);
         const double xp = __dadd_rn(fma(a, c2, fma(v, dt, x)), p3);
         const double vp = fma(jk, c2, fma(a, dt, v));
-        hi[c] = __double2float_rn(xp);
-        lo[c] = __double2float_rn(xp - (double)hi[c]);
-        vf[c] = __double2float_rn(vp);
+        const float hi = __double2float_rn(xp);
+        r[(C_XH + c) * TJ] = hi;
+        r[(C_XL + c) * TJ] = __double2float_rn(xp - (double)hi);
+        r[(C_VX + c) * TJ] = __double2float_rn(vp);
     }
-    const float mf = __double2float_rn(soa[j]);
-    r[0] = make_float4(hi[0], hi[0], hi[1], hi[1]);
-    r[1] = make_float4(hi[2], hi[2], mf, mf);
-    r[2] = make_float4(lo[0], lo[0], lo[1], lo[1]);
-    r[3] = make_float4(lo[2], lo[2], vf[0], vf[0]);
-    r[4] = make_float4(vf[1], vf[1], vf[2], vf[2]);
+    r[C_M * TJ] = __double2float_rn(soa[j]);
 }
 
-__global__ void __launch_bounds__(256) unpack_predicted_kernel(int64_t N, const float4 *__restrict__ rec,
+__global__ void __launch_bounds__(256) unpack_predicted_kernel(int64_t N, const float *__restrict__ rec,
                                                                double *__restrict__ xp, double *__restrict__ vp) {
     int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= N) return;
-    const float4 *r = rec + j * RECQ;
-    const float4 q0 = r[0], q1 = r[1], q2 = r[2], q3 = r[3], q4 = r[4];
-    xp[3 * j + 0] = (double)q0.x + (double)q2.x;
-    xp[3 * j + 1] = (double)q0.z + (double)q2.z;
-    xp[3 * j + 2] = (double)q1.x + (double)q3.x;
-    vp[3 * j + 0] = (double)q3.z;
-    vp[3 * j + 1] = (double)q4.x;
-    vp[3 * j + 2] = (double)q4.z;
+    const float *r = rec_slot(rec, j);
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        xp[3 * j + c] = (double)r[(C_XH + c) * TJ] + (double)r[(C_XL + c) * TJ];
+        vp[3 * j + c] = (double)r[(C_VX + c) * TJ];
+    }
 }
 
 // ------------------------------------------------------------------ a3-a6: force kernel
 struct ForceParams {
-    const float4 *rec;            // predicted records, Npad x RECQ
+    const float *rec;             // predicted records, [Npad / TJ][RECF][TJ]
     const int32_t *idx_i;         // [n_i]
     const double *h2_i;           // [n_i]
     int32_t n_i;
@@ -154,55 +158,66 @@ struct ForceParams {
     double *partial;              // [S][7][n_i_pad]
 };
 
-// Two active particles (lane halves .x / .y) held in registers, NEGATED so that every difference is
-// one packed add:  d = j + (-i).
+// Two active particles (halves .x / .y) held in registers, NEGATED so that every difference is one
+// packed add:  d = j + (-i).
 struct IPair {
     float2 nxh, nyh, nzh, nxl, nyl, nzl, nvx, nvy, nvz, h2;
 };
 
-__device__ __forceinline__ float2 lo2(const float4 &q) { return make_float2(q.x, q.y); }
-__device__ __forceinline__ float2 hi2(const float4 &q) { return make_float2(q.z, q.w); }
+__device__ __forceinline__ float2 bc(float s) { return make_float2(s, s); }   // -> scalar `R.F32` operand
+__device__ __forceinline__ float pick(const float4 &v, int u) { return u == 0 ? v.x : u == 1 ? v.y : u == 2 ? v.z : v.w; }
 
-// r^2 of one (i, j) pair in SCALAR FP32, operation for operation what the packed fast path does per
-// half (IEEE round-to-nearest either way), so both paths classify a pair identically.
-__device__ __forceinline__ float scalar_r2(float nxh, float nyh, float nzh, float nxl, float nyl, float nzl,
-                                           const float4 &q0, const float4 &q1, const float4 &q2, const float4 &q3) {
-    const float dx = __fadd_rn(__fadd_rn(q0.x, nxh), __fadd_rn(q2.x, nxl));
-    const float dy = __fadd_rn(__fadd_rn(q0.z, nyh), __fadd_rn(q2.z, nyl));
-    const float dz = __fadd_rn(__fadd_rn(q1.x, nzh), __fadd_rn(q3.x, nzl));
-    return __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
+// One neighbour of active particle k: take a slot of its row with an integer atomic (rows are shared
+// with the other j-splits and warps); entries past the capacity are only counted (reading R9).
+__device__ __forceinline__ void append_one(int32_t k, int32_t jg, int32_t cap, int32_t *cnt, int32_t *nblist) {
+    const int32_t pos = atomicAdd(cnt + k, 1);
+    if (pos < cap) nblist[(int64_t)k * cap + pos] = jg;
 }
 
-// Rare path: some lane saw r2 < h2 inside the last group of j's.  Lanes of one warp hold DIFFERENT i,
-// so the vote only gates the path; each flagged lane re-scans the group for each of its two particles
-// and takes one slot of that particle's row with an integer atomic (rows are shared with the other
-// j-splits and warps).
-__device__ __noinline__ void append_neighbours(float nxh, float nyh, float nzh, float nxl, float nyl, float nzl,
-                                               float h2, int32_t my_idx, int32_t k, const float4 *trec,
-                                               int32_t jglob0, int32_t cap, int32_t *cnt, int32_t *nblist) {
-    for (int u = 0; u < UNROLL_J; ++u) {
-        const float4 *r = trec + u * RECQ;
-        const float r2 = scalar_r2(nxh, nyh, nzh, nxl, nyl, nzl, r[0], r[1], r[2], r[3]);
-        const int32_t jg = jglob0 + u;
-        if (r2 < h2 && jg != my_idx) {
-            const int32_t pos = atomicAdd(cnt + k, 1);
-            if (pos < cap) nblist[(int64_t)k * cap + pos] = jg;
-        }
+// The seven FP32 partial sums of one i-pair over (a share of) one j-tile.
+struct Acc7 {
+    float2 ax, ay, az, jx, jy, jz, ph;
+};
+
+// Pair terms of one j against an i-pair, after r^2 is known.  MASKED = false is the fast path (no
+// lane of the warp has a neighbour or its self pair among the group's j's): plain MUFU.RSQ, no
+// predicates.  MASKED = true drops the pairs with r2 < h2 by zeroing 1/r BEFORE any product (no inf*0).
+template <bool MASKED>
+__device__ __forceinline__ void pair_terms(Acc7 &A, const IPair &I, float2 dx, float2 dy, float2 dz, float2 r2,
+                                           float2 rinv, float jvx, float jvy, float jvz, float jm) {
+    const float2 dvx = __fadd2_rn(bc(jvx), I.nvx);
+    const float2 dvy = __fadd2_rn(bc(jvy), I.nvy);
+    const float2 dvz = __fadd2_rn(bc(jvz), I.nvz);
+    const float2 rv = __ffma2_rn(dz, dvz, __ffma2_rn(dy, dvy, __fmul2_rn(dx, dvx)));
+    if (MASKED) {       // a select, not a product: the self pair's rsqrt(0) = inf never reaches the arithmetic
+        rinv.x = r2.x < I.h2.x ? 0.f : rinv.x;
+        rinv.y = r2.y < I.h2.y ? 0.f : rinv.y;
     }
+    const float2 rinv2 = __fmul2_rn(rinv, rinv);
+    const float2 mrinv = __fmul2_rn(bc(jm), rinv);
+    const float2 mrinv3 = __fmul2_rn(mrinv, rinv2);
+    const float2 alpha = __fmul2_rn(__fmul2_rn(rv, rinv2), make_float2(-3.0f, -3.0f));
+    A.ph = __fadd2_rn(A.ph, mrinv);
+    A.ax = __ffma2_rn(mrinv3, dx, A.ax);
+    A.ay = __ffma2_rn(mrinv3, dy, A.ay);
+    A.az = __ffma2_rn(mrinv3, dz, A.az);
+    A.jx = __ffma2_rn(mrinv3, __ffma2_rn(alpha, dx, dvx), A.jx);
+    A.jy = __ffma2_rn(mrinv3, __ffma2_rn(alpha, dy, dvy), A.jy);
+    A.jz = __ffma2_rn(mrinv3, __ffma2_rn(alpha, dz, dvz), A.jz);
 }
 
-// Each thread owns one PAIR of i-particles; WI warps along i (64 i each), WJ warps along j (each takes
-// TJ/WJ j's of every tile).  CTA = 32*WI*WJ threads, i-block = 64*WI.
+// Each thread owns one PAIR of i-particles; WI warps along i (64 i each), WJ warps along j (each
+// takes TJ/WJ j's of every tile).  CTA = 32*WI*WJ threads, i-block = 64*WI.
 template <int WI, int WJ, int MINB>
 __global__ void __launch_bounds__(32 * WI *WJ, MINB) force_kernel(const ForceParams p) {
     constexpr int NW = WI * WJ;
     constexpr int IB = 64 * WI;
     constexpr int SUB = TJ / WJ;
-    constexpr uint32_t TILE_BYTES = TJ * RECQ * sizeof(float4);
-    static_assert(SUB % UNROLL_J == 0, "sub-tile must be a multiple of the group");
+    constexpr uint32_t TILE_BYTES = TILE_FLOATS * sizeof(float);
+    static_assert(SUB % UNROLL_J == 0 && UNROLL_J == 4, "a group is one LDS.128 per component");
 
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    float4 *srec = reinterpret_cast<float4 *>(smem_raw);                       // [NSTAGE][TJ][RECQ]
+    float *srec = reinterpret_cast<float *>(smem_raw);                         // [NSTAGE][RECF][TJ]
     uint64_t *full = reinterpret_cast<uint64_t *>(smem_raw + (size_t)NSTAGE * TILE_BYTES);
     int *done = reinterpret_cast<int *>(full + NSTAGE);                        // warps finished with a stage
 
@@ -225,12 +240,10 @@ __global__ void __launch_bounds__(32 * WI *WJ, MINB) force_kernel(const ForcePar
             my_k[h] = k;
             if (k < p.n_i) {
                 const int32_t idx = p.idx_i[k];
-                const float4 *r = p.rec + (size_t)idx * RECQ;
-                const float4 q0 = r[0], q1 = r[1], q2 = r[2], q3 = r[3], q4 = r[4];
+                const float *r = rec_slot(p.rec, idx);
                 my_idx[h] = idx;
-                v[h][0] = -q0.x; v[h][1] = -q0.z; v[h][2] = -q1.x;
-                v[h][3] = -q2.x; v[h][4] = -q2.z; v[h][5] = -q3.x;
-                v[h][6] = -q3.z; v[h][7] = -q4.x; v[h][8] = -q4.z;
+#pragma unroll
+                for (int c = 0; c < 9; ++c) v[h][c] = -r[c * TJ];
                 v[h][9] = fmaxf(__double2float_rn(p.h2_i[k]), TINY_H2);
             } else {    // padding lane: far from everything (also from the ghost j's), result discarded
                 my_idx[h] = -1;
@@ -239,11 +252,11 @@ __global__ void __launch_bounds__(32 * WI *WJ, MINB) force_kernel(const ForcePar
                 v[h][9] = TINY_H2;
             }
         }
-        I.nxh = make_float2(v[0][0], v[1][0]); I.nyh = make_float2(v[0][1], v[1][1]);
-        I.nzh = make_float2(v[0][2], v[1][2]); I.nxl = make_float2(v[0][3], v[1][3]);
-        I.nyl = make_float2(v[0][4], v[1][4]); I.nzl = make_float2(v[0][5], v[1][5]);
-        I.nvx = make_float2(v[0][6], v[1][6]); I.nvy = make_float2(v[0][7], v[1][7]);
-        I.nvz = make_float2(v[0][8], v[1][8]); I.h2 = make_float2(v[0][9], v[1][9]);
+        I.nxh = make_float2(v[0][C_XH], v[1][C_XH]); I.nyh = make_float2(v[0][C_YH], v[1][C_YH]);
+        I.nzh = make_float2(v[0][C_ZH], v[1][C_ZH]); I.nxl = make_float2(v[0][C_XL], v[1][C_XL]);
+        I.nyl = make_float2(v[0][C_YL], v[1][C_YL]); I.nzl = make_float2(v[0][C_ZL], v[1][C_ZL]);
+        I.nvx = make_float2(v[0][C_VX], v[1][C_VX]); I.nvy = make_float2(v[0][C_VY], v[1][C_VY]);
+        I.nvz = make_float2(v[0][C_VZ], v[1][C_VZ]); I.h2 = make_float2(v[0][9], v[1][9]);
     }
 
     if (tid == 0) {
@@ -256,9 +269,9 @@ __global__ void __launch_bounds__(32 * WI *WJ, MINB) force_kernel(const ForcePar
     }
     __syncthreads();
 
-    auto issue = [&](int tile, int s) {     // one bulk copy per tile (20 KB), completion on full[s]
+    auto issue = [&](int tile, int s) {     // one bulk copy per tile (10 KB), completion on full[s]
         mbar_arrive_expect_tx(&full[s], TILE_BYTES);
-        bulk_g2s(srec + (size_t)s * TJ * RECQ, p.rec + (size_t)tile * TJ * RECQ, TILE_BYTES, &full[s]);
+        bulk_g2s(srec + (size_t)s * TILE_FLOATS, p.rec + (size_t)tile * TILE_FLOATS, TILE_BYTES, &full[s]);
     };
     if (tid == 0) {
         for (int s = 0; s < NSTAGE && s < ntile; ++s) issue(tile_begin + s, s);
@@ -268,68 +281,66 @@ __global__ void __launch_bounds__(32 * WI *WJ, MINB) force_kernel(const ForcePar
 #pragma unroll
     for (int h = 0; h < 2; ++h)
 #pragma unroll
-        for (int q = 0; q < 7; ++q) acc64[h][q] = 0.0;
-
-    const float2 m3 = make_float2(-3.0f, -3.0f);
+        for (int c = 0; c < 7; ++c) acc64[h][c] = 0.0;
 
     for (int it = 0; it < ntile; ++it) {
         const int s = it % NSTAGE;
         mbar_wait(&full[s], (uint32_t)((it / NSTAGE) & 1));
-        const float4 *trec = srec + ((size_t)s * TJ + wj * SUB) * RECQ;
+        const float *tsub = srec + (size_t)s * TILE_FLOATS + wj * SUB;      // &tile[0][wj * SUB]
         const int32_t jbase = (tile_begin + it) * TJ + wj * SUB;
 
-        float2 ax = make_float2(0.f, 0.f), ay = ax, az = ax, jx = ax, jy = ax, jz = ax, ph = ax;
+        Acc7 A;               // FP32 partial sums of this tile share
+        A.ax = A.ay = A.az = A.jx = A.jy = A.jz = A.ph = make_float2(0.f, 0.f);
 
 #pragma unroll 1
         for (int g = 0; g < SUB; g += UNROLL_J) {
-            bool hit = false;
+            float4 c4[RECF];                                   // component rows of 4 consecutive j
+#pragma unroll
+            for (int c = 0; c < RECF; ++c)                     // warp-uniform address: LDS.128 broadcast
+                c4[c] = *reinterpret_cast<const float4 *>(tsub + c * TJ + g);
+            // phase 1: FP64-equivalent differences and r^2 of the group's 4 j against the i-pair
+            float2 dx[UNROLL_J], dy[UNROLL_J], dz[UNROLL_J], r2[UNROLL_J], rinv[UNROLL_J];
 #pragma unroll
             for (int u = 0; u < UNROLL_J; ++u) {
-                const float4 *r = trec + (g + u) * RECQ;      // warp-uniform addresses: LDS.128 broadcasts
-                const float4 q0 = r[0], q1 = r[1], q2 = r[2], q3 = r[3], q4 = r[4];
-                const float2 dx = __fadd2_rn(__fadd2_rn(lo2(q0), I.nxh), __fadd2_rn(lo2(q2), I.nxl));
-                const float2 dy = __fadd2_rn(__fadd2_rn(hi2(q0), I.nyh), __fadd2_rn(hi2(q2), I.nyl));
-                const float2 dz = __fadd2_rn(__fadd2_rn(lo2(q1), I.nzh), __fadd2_rn(lo2(q3), I.nzl));
-                const float2 dvx = __fadd2_rn(hi2(q3), I.nvx);
-                const float2 dvy = __fadd2_rn(lo2(q4), I.nvy);
-                const float2 dvz = __fadd2_rn(hi2(q4), I.nvz);
-                const float2 r2 = __ffma2_rn(dz, dz, __ffma2_rn(dy, dy, __fmul2_rn(dx, dx)));
-                const float2 rv = __ffma2_rn(dz, dvz, __ffma2_rn(dy, dvy, __fmul2_rn(dx, dvx)));
-                const bool nb0 = r2.x < I.h2.x, nb1 = r2.y < I.h2.y;   // neighbour (or the self pair, r2 == 0)
-                hit |= nb0 | nb1;
-                float2 rinv;
-                rinv.x = nb0 ? 0.f : rsqrt_sfu(r2.x);       // masked before any product: no inf * 0
-                rinv.y = nb1 ? 0.f : rsqrt_sfu(r2.y);
-                const float2 rinv2 = __fmul2_rn(rinv, rinv);
-                const float2 mrinv = __fmul2_rn(hi2(q1), rinv);
-                const float2 mrinv3 = __fmul2_rn(mrinv, rinv2);
-                const float2 alpha = __fmul2_rn(__fmul2_rn(rv, rinv2), m3);
-                ph = __fadd2_rn(ph, mrinv);
-                ax = __ffma2_rn(mrinv3, dx, ax);
-                ay = __ffma2_rn(mrinv3, dy, ay);
-                az = __ffma2_rn(mrinv3, dz, az);
-                jx = __ffma2_rn(mrinv3, __ffma2_rn(alpha, dx, dvx), jx);
-                jy = __ffma2_rn(mrinv3, __ffma2_rn(alpha, dy, dvy), jy);
-                jz = __ffma2_rn(mrinv3, __ffma2_rn(alpha, dz, dvz), jz);
+                dx[u] = __fadd2_rn(__fadd2_rn(bc(pick(c4[C_XH], u)), I.nxh), __fadd2_rn(bc(pick(c4[C_XL], u)), I.nxl));
+                dy[u] = __fadd2_rn(__fadd2_rn(bc(pick(c4[C_YH], u)), I.nyh), __fadd2_rn(bc(pick(c4[C_YL], u)), I.nyl));
+                dz[u] = __fadd2_rn(__fadd2_rn(bc(pick(c4[C_ZH], u)), I.nzh), __fadd2_rn(bc(pick(c4[C_ZL], u)), I.nzl));
+                r2[u] = __ffma2_rn(dz[u], dz[u], __ffma2_rn(dy[u], dy[u], __fmul2_rn(dx[u], dx[u])));
+                rinv[u].x = rsqrt_sfu(r2[u].x);        // issued before the vote: SFU latency overlaps the test
+                rinv[u].y = rsqrt_sfu(r2[u].y);
             }
-            if (__any_sync(0xffffffffu, hit)) {     // ~1 % of groups at N_b ~ 150, N = 1M
-                if (hit) {
-                    const float4 *tg = trec + g * RECQ;
-                    append_neighbours(I.nxh.x, I.nyh.x, I.nzh.x, I.nxl.x, I.nyl.x, I.nzl.x, I.h2.x, my_idx[0], my_k[0],
-                                      tg, jbase + g, p.cap, p.cnt, p.nblist);
-                    append_neighbours(I.nxh.y, I.nyh.y, I.nzh.y, I.nxl.y, I.nyl.y, I.nzl.y, I.h2.y, my_idx[1], my_k[1],
-                                      tg, jbase + g, p.cap, p.cnt, p.nblist);
+            // one test per i for the whole group (FMNMX3): a neighbour, or the self pair (r2 == 0)?
+            const float mn0 = fminf(fminf(fminf(r2[0].x, r2[1].x), r2[2].x), r2[3].x);
+            const float mn1 = fminf(fminf(fminf(r2[0].y, r2[1].y), r2[2].y), r2[3].y);
+            const bool hit = (mn0 < I.h2.x) | (mn1 < I.h2.y);
+            if (!__any_sync(0xffffffffu, hit)) {    // ~95 % of groups at N_b ~ 150, N = 1M: nothing to mask
+#pragma unroll
+                for (int u = 0; u < UNROLL_J; ++u)
+                    pair_terms<false>(A, I, dx[u], dy[u], dz[u], r2[u], rinv[u], pick(c4[C_VX], u), pick(c4[C_VY], u),
+                                      pick(c4[C_VZ], u), pick(c4[C_M], u));
+            } else {
+#pragma unroll
+                for (int u = 0; u < UNROLL_J; ++u)
+                    pair_terms<true>(A, I, dx[u], dy[u], dz[u], r2[u], rinv[u], pick(c4[C_VX], u), pick(c4[C_VY], u),
+                                     pick(c4[C_VZ], u), pick(c4[C_M], u));
+                if (hit) {      // rare: lanes hold different i, each takes slots of its own rows
+#pragma unroll
+                    for (int u = 0; u < UNROLL_J; ++u) {
+                        const int32_t jg = jbase + g + u;
+                        if (r2[u].x < I.h2.x && jg != my_idx[0]) append_one(my_k[0], jg, p.cap, p.cnt, p.nblist);
+                        if (r2[u].y < I.h2.y && jg != my_idx[1]) append_one(my_k[1], jg, p.cap, p.cnt, p.nblist);
+                    }
                 }
             }
         }
         // tile flush: FP32 partial sums of <= SUB terms go into the FP64 running sums
-        acc64[0][0] += (double)ax.x; acc64[1][0] += (double)ax.y;
-        acc64[0][1] += (double)ay.x; acc64[1][1] += (double)ay.y;
-        acc64[0][2] += (double)az.x; acc64[1][2] += (double)az.y;
-        acc64[0][3] += (double)jx.x; acc64[1][3] += (double)jx.y;
-        acc64[0][4] += (double)jy.x; acc64[1][4] += (double)jy.y;
-        acc64[0][5] += (double)jz.x; acc64[1][5] += (double)jz.y;
-        acc64[0][6] += (double)ph.x; acc64[1][6] += (double)ph.y;
+        acc64[0][0] += (double)A.ax.x; acc64[1][0] += (double)A.ax.y;
+        acc64[0][1] += (double)A.ay.x; acc64[1][1] += (double)A.ay.y;
+        acc64[0][2] += (double)A.az.x; acc64[1][2] += (double)A.az.y;
+        acc64[0][3] += (double)A.jx.x; acc64[1][3] += (double)A.jx.y;
+        acc64[0][4] += (double)A.jy.x; acc64[1][4] += (double)A.jy.y;
+        acc64[0][5] += (double)A.jz.x; acc64[1][5] += (double)A.jz.y;
+        acc64[0][6] += (double)A.ph.x; acc64[1][6] += (double)A.ph.y;
 
         // Stage hand-back without a CTA barrier: the LAST warp to finish with stage s refills it, so
         // warps drift up to NSTAGE-1 tiles apart instead of meeting at a __syncthreads every tile.
@@ -355,7 +366,7 @@ __global__ void __launch_bounds__(32 * WI *WJ, MINB) force_kernel(const ForcePar
         for (int h = 0; h < 2; ++h) {
             const int il = wi * 64 + h * 32 + lane;
 #pragma unroll
-            for (int q = 0; q < 7; ++q) red[((size_t)wj * 7 + q) * IB + il] = acc64[h][q];
+            for (int c = 0; c < 7; ++c) red[((size_t)wj * 7 + c) * IB + il] = acc64[h][c];
         }
         __syncthreads();
         if (wj == 0) {
@@ -363,10 +374,10 @@ __global__ void __launch_bounds__(32 * WI *WJ, MINB) force_kernel(const ForcePar
             for (int h = 0; h < 2; ++h) {
                 const int il = wi * 64 + h * 32 + lane;
 #pragma unroll
-                for (int q = 0; q < 7; ++q) {
-                    double ssum = acc64[h][q];
-                    for (int w = 1; w < WJ; ++w) ssum += red[((size_t)w * 7 + q) * IB + il];
-                    acc64[h][q] = ssum;
+                for (int c = 0; c < 7; ++c) {
+                    double ssum = acc64[h][c];
+                    for (int w = 1; w < WJ; ++w) ssum += red[((size_t)w * 7 + c) * IB + il];
+                    acc64[h][c] = ssum;
                 }
             }
         }
@@ -376,8 +387,7 @@ __global__ void __launch_bounds__(32 * WI *WJ, MINB) force_kernel(const ForcePar
         for (int h = 0; h < 2; ++h) {
             const int k = my_k[h];    // k < n_i_pad always
 #pragma unroll
-            for (int q = 0; q < 7; ++q)
-                p.partial[((size_t)blockIdx.y * 7 + q) * p.n_i_pad + k] = acc64[h][q];
+            for (int c = 0; c < 7; ++c) p.partial[((size_t)blockIdx.y * 7 + c) * p.n_i_pad + k] = acc64[h][c];
         }
     }
 }
