@@ -164,6 +164,15 @@ struct IPair {
     float2 nxh, nyh, nzh, nxl, nyl, nzl, nvx, nvy, nvz, h2;
 };
 
+#ifdef NBREG_SCALAR_MATH
+__device__ __forceinline__ float2 padd(float2 a, float2 b) { return make_float2(__fadd_rn(a.x, b.x), __fadd_rn(a.y, b.y)); }
+__device__ __forceinline__ float2 pmul(float2 a, float2 b) { return make_float2(__fmul_rn(a.x, b.x), __fmul_rn(a.y, b.y)); }
+__device__ __forceinline__ float2 pfma(float2 a, float2 b, float2 c) { return make_float2(__fmaf_rn(a.x, b.x, c.x), __fmaf_rn(a.y, b.y, c.y)); }
+#else
+__device__ __forceinline__ float2 padd(float2 a, float2 b) { return __fadd2_rn(a, b); }
+__device__ __forceinline__ float2 pmul(float2 a, float2 b) { return __fmul2_rn(a, b); }
+__device__ __forceinline__ float2 pfma(float2 a, float2 b, float2 c) { return __ffma2_rn(a, b, c); }
+#endif
 __device__ __forceinline__ float2 bc(float s) { return make_float2(s, s); }   // -> scalar `R.F32` operand
 __device__ __forceinline__ float pick(const float4 &v, int u) { return u == 0 ? v.x : u == 1 ? v.y : u == 2 ? v.z : v.w; }
 
@@ -185,25 +194,25 @@ struct Acc7 {
 template <bool MASKED>
 __device__ __forceinline__ void pair_terms(Acc7 &A, const IPair &I, float2 dx, float2 dy, float2 dz, float2 r2,
                                            float2 rinv, float jvx, float jvy, float jvz, float jm) {
-    const float2 dvx = __fadd2_rn(bc(jvx), I.nvx);
-    const float2 dvy = __fadd2_rn(bc(jvy), I.nvy);
-    const float2 dvz = __fadd2_rn(bc(jvz), I.nvz);
-    const float2 rv = __ffma2_rn(dz, dvz, __ffma2_rn(dy, dvy, __fmul2_rn(dx, dvx)));
+    const float2 dvx = padd(bc(jvx), I.nvx);
+    const float2 dvy = padd(bc(jvy), I.nvy);
+    const float2 dvz = padd(bc(jvz), I.nvz);
+    const float2 rv = pfma(dz, dvz, pfma(dy, dvy, pmul(dx, dvx)));
     if (MASKED) {       // a select, not a product: the self pair's rsqrt(0) = inf never reaches the arithmetic
         rinv.x = r2.x < I.h2.x ? 0.f : rinv.x;
         rinv.y = r2.y < I.h2.y ? 0.f : rinv.y;
     }
-    const float2 rinv2 = __fmul2_rn(rinv, rinv);
-    const float2 mrinv = __fmul2_rn(bc(jm), rinv);
-    const float2 mrinv3 = __fmul2_rn(mrinv, rinv2);
-    const float2 alpha = __fmul2_rn(__fmul2_rn(rv, rinv2), make_float2(-3.0f, -3.0f));
-    A.ph = __fadd2_rn(A.ph, mrinv);
-    A.ax = __ffma2_rn(mrinv3, dx, A.ax);
-    A.ay = __ffma2_rn(mrinv3, dy, A.ay);
-    A.az = __ffma2_rn(mrinv3, dz, A.az);
-    A.jx = __ffma2_rn(mrinv3, __ffma2_rn(alpha, dx, dvx), A.jx);
-    A.jy = __ffma2_rn(mrinv3, __ffma2_rn(alpha, dy, dvy), A.jy);
-    A.jz = __ffma2_rn(mrinv3, __ffma2_rn(alpha, dz, dvz), A.jz);
+    const float2 rinv2 = pmul(rinv, rinv);
+    const float2 mrinv = pmul(bc(jm), rinv);
+    const float2 mrinv3 = pmul(mrinv, rinv2);
+    const float2 alpha = pmul(pmul(rv, rinv2), make_float2(-3.0f, -3.0f));
+    A.ph = padd(A.ph, mrinv);
+    A.ax = pfma(mrinv3, dx, A.ax);
+    A.ay = pfma(mrinv3, dy, A.ay);
+    A.az = pfma(mrinv3, dz, A.az);
+    A.jx = pfma(mrinv3, pfma(alpha, dx, dvx), A.jx);
+    A.jy = pfma(mrinv3, pfma(alpha, dy, dvy), A.jy);
+    A.jz = pfma(mrinv3, pfma(alpha, dz, dvz), A.jz);
 }
 
 // Each thread owns one PAIR of i-particles; WI warps along i (64 i each), WJ warps along j (each
@@ -292,7 +301,7 @@ __global__ void __launch_bounds__(32 * WI *WJ, MINB) force_kernel(const ForcePar
         Acc7 A;               // FP32 partial sums of this tile share
         A.ax = A.ay = A.az = A.jx = A.jy = A.jz = A.ph = make_float2(0.f, 0.f);
 
-#pragma unroll 1
+#pragma unroll 2
         for (int g = 0; g < SUB; g += UNROLL_J) {
             float4 c4[RECF];                                   // component rows of 4 consecutive j
 #pragma unroll
@@ -302,10 +311,10 @@ __global__ void __launch_bounds__(32 * WI *WJ, MINB) force_kernel(const ForcePar
             float2 dx[UNROLL_J], dy[UNROLL_J], dz[UNROLL_J], r2[UNROLL_J], rinv[UNROLL_J];
 #pragma unroll
             for (int u = 0; u < UNROLL_J; ++u) {
-                dx[u] = __fadd2_rn(__fadd2_rn(bc(pick(c4[C_XH], u)), I.nxh), __fadd2_rn(bc(pick(c4[C_XL], u)), I.nxl));
-                dy[u] = __fadd2_rn(__fadd2_rn(bc(pick(c4[C_YH], u)), I.nyh), __fadd2_rn(bc(pick(c4[C_YL], u)), I.nyl));
-                dz[u] = __fadd2_rn(__fadd2_rn(bc(pick(c4[C_ZH], u)), I.nzh), __fadd2_rn(bc(pick(c4[C_ZL], u)), I.nzl));
-                r2[u] = __ffma2_rn(dz[u], dz[u], __ffma2_rn(dy[u], dy[u], __fmul2_rn(dx[u], dx[u])));
+                dx[u] = padd(padd(bc(pick(c4[C_XH], u)), I.nxh), padd(bc(pick(c4[C_XL], u)), I.nxl));
+                dy[u] = padd(padd(bc(pick(c4[C_YH], u)), I.nyh), padd(bc(pick(c4[C_YL], u)), I.nyl));
+                dz[u] = padd(padd(bc(pick(c4[C_ZH], u)), I.nzh), padd(bc(pick(c4[C_ZL], u)), I.nzl));
+                r2[u] = pfma(dz[u], dz[u], pfma(dy[u], dy[u], pmul(dx[u], dx[u])));
                 rinv[u].x = rsqrt_sfu(r2[u].x);        // issued before the vote: SFU latency overlaps the test
                 rinv[u].y = rsqrt_sfu(r2[u].y);
             }
