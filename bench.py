@@ -250,6 +250,7 @@ def run_b200(args):
     ms = e0.elapsed_time(e1)
     clocks = sampler.stop(w0, w1) if sampler else None
     launches = ctx.info("kernel_launches") - launches0
+    plan = {"variant": ctx.info("last_variant"), "jsplit": ctx.info("last_jsplit"), "grid": ctx.info("last_grid")}
     force_ns = ctx.info("force_kernel_ns")
     force_cnt = ctx.info("force_kernel_count")
     ctx.tune("profile", 0)
@@ -315,11 +316,13 @@ def run_b200(args):
     peak_tflops = sm_count * 128 * 2 * sm_max_mhz * 1e6 / 1e12
     force_ms = force_ns / max(force_cnt, 1) * 1e-6
     ach_tflops = FLOP_PER_INTERACTION * float(n_i) * N / (force_ms * 1e-3) / 1e12
-    traffic = None
-    tpath = os.path.join(ROOT, "profiles", "force_kernel_traffic.json")
-    if os.path.exists(tpath):
+    traffic = None       # dram__bytes_read.sum + dram__bytes_write.sum of one launch, from the committed ncu capture
+    tpath = os.path.join(ROOT, "profiles", "force_kernel_traffic.csv")
+    if os.path.exists(tpath) and n_i == 8192 and N == 1048576:
+        import csv
         with open(tpath) as f:
-            traffic = json.load(f).get("dram_bytes_per_launch")
+            row = next(csv.DictReader(f))
+        traffic = int(row["dram_bytes_read"]) + int(row["dram_bytes_write"])
     roofline = {
         "bound": "alu", "kernel": "nbreg::force_kernel", "achieved": ach_tflops, "peak": peak_tflops,
         "unit": "TFLOP/s", "frac": ach_tflops / peak_tflops, "traffic": traffic,
@@ -367,9 +370,9 @@ def run_b200(args):
         "config": {"workload": WORKLOAD, "N": N, "n_i_per_gpu": n_i, "nb_cap": cap, "nb_target": cfg["nb_target"],
                    "parallelism": f"i-shard x{world}" if world > 1 else "single GPU",
                    "step": "nb_set_j + nb_predict_all + nb_regular",
-                   "l2": "each step streams 2*112 B/body (set_j) + 112+48 B/body (predict) = 403 MB > 126 MB L2 "
-                         "before the force kernel; its 50 MB j-record working set is L2-resident by design",
-                   "variant": ctx.info("last_variant"), "jsplit": ctx.info("last_jsplit")},
+                   "l2": "each step streams 2*112 B/body (set_j) + 112+40 B/body (predict) = 394 MB > 126 MB L2 "
+                         "before the force kernel; its 42 MB j-record working set is L2-resident by design",
+                   **plan},
         "frac_fp32_peak": value / world * FLOP_PER_INTERACTION / 1e12 / peak_tflops,
         "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
         "cpu_baseline": cpu, "sweep": sweep, "peaks_source": pk_src,
