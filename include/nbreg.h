@@ -100,7 +100,15 @@ int nb_get_predicted(nb_ctx *ctx, double *xp, double *vp);
  * nblist[n_i][nb_cap] int32, overflow[n_i] int32.  DEVICE pointers.  Requires nb_predict_all. */
 int nb_regular(nb_ctx *ctx, int32_t n_i, const int32_t *idx_i, const double *h2_i, double *acc,
                double *jerk, double *pot, int32_t *nnb, int32_t *nblist, int32_t *overflow);
-/* Same with HOST pointers: copies idx_i/h2_i in, runs, copies all outputs back, synchronises.
+/* Full-N pass (section 3.3.2: forces and neighbour lists of ALL particles are initialised with
+ * the same GPU kernel; the same pass with h2 = 0 gives every particle's full potential
+ * for the energy check): nb_regular with the identity block idx_i[k] = k, n_i = N.
+ * Shapes as nb_regular with n_i = N: h2[N], acc[N][3], jerk[N][3], pot[N], nnb[N], overflow[N],
+ * nblist[N][nb_cap] -- or nblist = NULL: neighbours are counted (nnb, overflow exact) but not stored
+ * (N x nb_cap x 4 B is 2 GiB at N = 1M, cap = 512).  DEVICE pointers.  Requires nb_predict_all. */
+int nb_regular_all(nb_ctx *ctx, const double *h2, double *acc, double *jerk, double *pot,
+                   int32_t *nnb, int32_t *nblist, int32_t *overflow);
+/* Same as nb_regular with HOST pointers: copies idx_i/h2_i in, runs, copies all outputs back, synchronises.
  * nblist may be NULL to skip the list copy-back (the list is still built on the device). */
 int nb_regular_host(nb_ctx *ctx, int32_t n_i, const int32_t *idx_i, const double *h2_i, double *acc,
                     double *jerk, double *pot, int32_t *nnb, int32_t *nblist, int32_t *overflow);

@@ -15,6 +15,7 @@ from .binding import (  # noqa: F401
     nb_set_j,
     nb_predict_all,
     nb_regular,
+    nb_regular_all,
     NB_OK, NB_EINVAL, NB_ESTATE, NB_ENOMEM, NB_ECUDA,
 )
 from .build import build_lib  # noqa: F401

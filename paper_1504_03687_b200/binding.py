@@ -50,6 +50,7 @@ def load_library(build: bool = True) -> ctypes.CDLL:
     lib.nb_get_predicted.argtypes = [_vp, _vp, _vp]
     lib.nb_regular.argtypes = [_vp, i32] + [_vp] * 8
     lib.nb_regular_host.argtypes = [_vp, i32] + [_vp] * 8
+    lib.nb_regular_all.argtypes = [_vp] + [_vp] * 7
     lib.nb_get_info.argtypes = [_vp, i32, ctypes.POINTER(i64)]
     lib.nb_set_tuning.argtypes = [_vp, i32, i64]
     lib.nb_last_cuda_error.argtypes = [_vp]
@@ -178,6 +179,16 @@ class NbContext:
                 _dev_ptr(nblist, i4, n * self.cap, "nblist"), _dev_ptr(overflow, i4, n, "overflow")]
         _check(self._lib.nb_regular(self._ctx, n, *args), "nb_regular", self._ctx)
 
+    def regular_all(self, h2, acc, jerk, pot, nnb, nblist, overflow):
+        """Full-N pass (identity block); nblist may be None: neighbours are counted, not stored."""
+        import torch
+        n, f8, i4 = self.N, torch.float64, torch.int32
+        args = [_dev_ptr(h2, f8, n, "h2"), _dev_ptr(acc, f8, 3 * n, "acc"), _dev_ptr(jerk, f8, 3 * n, "jerk"),
+                _dev_ptr(pot, f8, n, "pot"), _dev_ptr(nnb, i4, n, "nnb"),
+                _vp() if nblist is None else _dev_ptr(nblist, i4, n * self.cap, "nblist"),
+                _dev_ptr(overflow, i4, n, "overflow")]
+        _check(self._lib.nb_regular_all(self._ctx, *args), "nb_regular_all", self._ctx)
+
     # -- the path (host buffers: numpy arrays or CPU tensors, pinned or not)
     def set_j_host(self, m, x0, v0, a0, j0, t0):
         import numpy as np
@@ -230,3 +241,7 @@ def nb_predict_all(ctx: NbContext, t: float):
 
 def nb_regular(ctx: NbContext, idx_i, h2_i, acc, jerk, pot, nnb, nblist, overflow):
     ctx.regular(idx_i, h2_i, acc, jerk, pot, nnb, nblist, overflow)
+
+
+def nb_regular_all(ctx: NbContext, h2, acc, jerk, pot, nnb, nblist, overflow):
+    ctx.regular_all(h2, acc, jerk, pot, nnb, nblist, overflow)

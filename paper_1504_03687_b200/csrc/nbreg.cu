@@ -184,8 +184,13 @@ int regular_device(nb_ctx *c, int32_t n_i, const int32_t *idx_i, const double *h
         NB_CUDA(c, cudaEventRecord(c->ev1[slot], c->stream));
         c->prof_n += 1;
     }
-    finalize_kernel<<<(n_i + 7) / 8, 256, 0, c->stream>>>(n_i, (int32_t)n_i_pad, S, c->cap, c->partial, c->cnt,
-                                                              acc, jerk, pot, nnb, overflow);
+    const unsigned fgrid = (unsigned)((n_i + 31) / 32);
+    if (S <= 8)
+        finalize_kernel<4><<<fgrid, 128, 0, c->stream>>>(n_i, (int32_t)n_i_pad, S, c->cap, c->partial, c->cnt, acc,
+                                                         jerk, pot, nnb, overflow);
+    else
+        finalize_kernel<16><<<fgrid, 512, 0, c->stream>>>(n_i, (int32_t)n_i_pad, S, c->cap, c->partial, c->cnt, acc,
+                                                          jerk, pot, nnb, overflow);
     NB_CUDA(c, cudaGetLastError());
     c->launches += 2;
     c->last_S = S; c->last_iblock = v.iblock; c->last_grid = n_ib * S; c->last_variant = vi;
@@ -317,6 +322,15 @@ int nb_regular(nb_ctx *c, int32_t n_i, const int32_t *idx_i, const double *h2_i,
     if (n_i == 0) return NB_OK;
     if (!idx_i || !h2_i || !acc || !jerk || !pot || !nnb || !nblist || !overflow) return NB_EINVAL;
     return regular_device(c, n_i, idx_i, h2_i, acc, jerk, pot, nnb, nblist, overflow);
+}
+
+int nb_regular_all(nb_ctx *c, const double *h2, double *acc, double *jerk, double *pot, int32_t *nnb,
+                   int32_t *nblist, int32_t *overflow) {
+    int rc = check_live(c);
+    if (rc != NB_OK) return rc;
+    if (!c->have_pred) return NB_ESTATE;
+    if (!h2 || !acc || !jerk || !pot || !nnb || !overflow) return NB_EINVAL;
+    return regular_device(c, (int32_t)c->N, nullptr, h2, acc, jerk, pot, nnb, nblist, overflow);
 }
 
 int nb_regular_host(nb_ctx *c, int32_t n_i, const int32_t *idx_i, const double *h2_i, double *acc, double *jerk,

@@ -295,3 +295,100 @@ def test_full_size_million_body_sampled(oracle):
     got = gpu_regular(ctx, idx, h2)
     ref = parity.oracle_reference(oracle, cfg["m"], xp, vp, idx, h2, cfg["cap"])
     print("config4 n_i=64", parity.compare(got, ref, cfg["cap"]))
+
+
+def test_config5_full_size_king_core(oracle):
+    """BASELINE.json configs[4] at its full size: N = 1,048,576 King W0 = 9, n_i = 32 / 128 / 512 of the
+    innermost particles (split-j path at full N, rows above and below the 512 cap), every active
+    particle checked by the oracle."""
+    cfg = nbgen.make_config(5)
+    ctx = open_ctx(cfg)
+    xp, vp = oracle.predict(cfg["x0"], cfg["v0"], cfg["a0"], cfg["j0"], cfg["t0"], cfg["t"])
+    over = 0
+    for n_i in cfg["sweep"]:
+        idx, h2 = nbgen.active_block(cfg, n_i)
+        got = gpu_regular(ctx, idx, h2)
+        ref = parity.oracle_reference(oracle, cfg["m"], xp, vp, idx, h2, cfg["cap"])
+        rep = parity.compare(got, ref, cfg["cap"])
+        print("config5 full", n_i, rep, "variant", ctx.info("last_variant"), "S", ctx.info("last_jsplit"))
+        over = rep["overflow_rows"]
+        assert ctx.info("last_jsplit") > 1                      # the j-range really is split
+    assert 0 < over < 512                                       # mixes overflowing and fitting rows
+
+
+def test_config3_block_sweep_sampled(oracle):
+    """BASELINE.json configs[2] at its full size (N = 262,144, 5 % binaries): the five block sizes of
+    the sweep; the oracle checks every i up to n_i = 1024 and a seeded sample of 256 above."""
+    cfg = nbgen.make_config(3)
+    ctx = open_ctx(cfg)
+    xp, vp = oracle.predict(cfg["x0"], cfg["v0"], cfg["a0"], cfg["j0"], cfg["t0"], cfg["t"])
+    for n_i in cfg["sweep"]:
+        idx, h2 = nbgen.active_block(cfg, n_i)
+        got = gpu_regular(ctx, idx, h2)
+        sel = np.arange(n_i) if n_i <= 1024 else np.sort(np.random.default_rng(n_i).choice(n_i, 256, replace=False))
+        ref = parity.oracle_reference(oracle, cfg["m"], xp, vp, idx[sel], h2[sel], cfg["cap"])
+        rep = parity.compare({k: v[sel] for k, v in got.items()}, ref, cfg["cap"])
+        print("config3", n_i, rep, "variant", ctx.info("last_variant"), "S", ctx.info("last_jsplit"))
+        assert np.all(np.isfinite(got["acc"])) and np.all(np.isfinite(got["jerk"]))
+
+
+def test_config4_largest_block_sampled_and_block_independent(oracle):
+    """N = 1,048,576, n_i = 131072 (the top of the sweep): a seeded sample of 128 rows against the
+    oracle, and -- a property that holds at any size -- a particle's result does not depend on the
+    block it is computed in: the nested 8192-block gives the same counts, the same sets and sums equal
+    up to the FP64 rounding of a different split (copies must not diverge)."""
+    cfg = nbgen.make_config(4)
+    ctx = open_ctx(cfg)
+    idx, h2 = nbgen.active_block(cfg, 131072)
+    big = gpu_regular(ctx, idx, h2)
+    sel = np.sort(np.random.default_rng(7).choice(131072, size=128, replace=False))
+    xp, vp = oracle.predict(cfg["x0"], cfg["v0"], cfg["a0"], cfg["j0"], cfg["t0"], cfg["t"])
+    ref = parity.oracle_reference(oracle, cfg["m"], xp, vp, idx[sel], h2[sel], cfg["cap"])
+    rep = parity.compare({k: v[sel] for k, v in big.items()}, ref, cfg["cap"])
+    print("config4 n_i=131072 sample", rep, "S", ctx.info("last_jsplit"))
+    small = gpu_regular(ctx, idx[:8192], h2[:8192])
+    assert np.array_equal(small["nnb"], big["nnb"][:8192])
+    assert np.array_equal(small["overflow"], big["overflow"][:8192])
+    for k in range(0, 8192, 17):
+        c = min(small["nnb"][k], cfg["cap"])
+        if small["nnb"][k] <= cfg["cap"]:
+            assert set(small["nblist"][k, :c].tolist()) == set(big["nblist"][k, :c].tolist())
+    for key, tol in (("acc", 1e-6), ("jerk", 1e-5), ("pot", 1e-7)):
+        a = small[key].reshape(8192, -1); b = big[key][:8192].reshape(8192, -1)
+        assert np.max(np.linalg.norm(a - b, axis=1) / np.linalg.norm(b, axis=1)) < tol
+
+
+# ----------------------------------------------------------------------------- NEXT-1: full-N pass
+
+def test_regular_all_equals_identity_block_and_energy(oracle):
+    """nb_regular_all (P:111 initialisation pass; P:69/P:148 potential energy) = nb_regular with the
+    identity block, bit for bit; with h2 = 0 the potentials give W = 1/2 sum m phi, compared with the
+    oracle's and with the Plummer closed form -3 pi/32 G M^2 / a within finite-N scatter."""
+    cfg = nbgen.make_config(2, N=20000, n_i=64)
+    N, cap = cfg["N"], cfg["cap"]
+    ctx = open_ctx(cfg)
+    ident = np.arange(N, dtype=np.int32)
+    a = gpu_regular(ctx, ident, cfg["h2_all"])
+    mk = lambda *s, dt=torch.float64: torch.empty(*s, dtype=dt, device="cuda")
+    out = dict(acc=mk(N, 3), jerk=mk(N, 3), pot=mk(N), nnb=mk(N, dt=torch.int32),
+               nblist=torch.full((N, cap), -1, dtype=torch.int32, device="cuda"), overflow=mk(N, dt=torch.int32))
+    ctx.regular_all(_dev(cfg["h2_all"]), **out)
+    ctx.synchronize()
+    b = parity.to_numpy(out)
+    for key in ("acc", "jerk", "pot", "nnb", "overflow"):
+        assert np.array_equal(a[key], b[key])
+    xp, vp = oracle.predict(cfg["x0"], cfg["v0"], cfg["a0"], cfg["j0"], cfg["t0"], cfg["t"])
+    sel = np.sort(np.random.default_rng(3).choice(N, 300, replace=False)).astype(np.int32)
+    ref = parity.oracle_reference(oracle, cfg["m"], xp, vp, sel, cfg["h2_all"][sel], cap)
+    parity.compare({k: v[sel] for k, v in b.items()}, ref, cap)
+    # counts only (nblist = NULL), h2 = 0: full potential of every particle -> potential energy
+    out["nnb"].fill_(-1)
+    ctx.regular_all(_dev(np.zeros(N)), out["acc"], out["jerk"], out["pot"], out["nnb"], None, out["overflow"])
+    ctx.synchronize()
+    assert int(out["nnb"].abs().sum()) == 0
+    W = 0.5 * float((torch.from_numpy(cfg["m"]).cuda() * out["pot"]).sum())
+    tot = oracle.regular(cfg["m"], xp, vp, ident, np.zeros(N), cap, want_list=False)
+    W_orc = 0.5 * float((cfg["m"] * tot["pot"]).sum())
+    assert abs(W - W_orc) < 1e-6 * abs(W_orc)
+    W_plummer = -3.0 * np.pi / 32.0 / cfg["a_plummer"]
+    assert abs(W / W_plummer - 1.0) < 0.1        # Kroupa masses: scatter dominated by the few heavy stars
