@@ -69,6 +69,9 @@ def _load():
     lib.orc_band_pairs.restype = ctypes.c_int64
     lib.orc_band_pairs.argtypes = [ctypes.c_int64, dp, dp, dp, ctypes.c_int32, ip, dp, ctypes.c_double,
                                    ctypes.c_int64, ip, ip, dp, dp]
+    lib.orc_irregular.restype = ctypes.c_int
+    lib.orc_irregular.argtypes = [ctypes.c_int64, dp, dp, dp, dp, dp, dp, ctypes.c_double, ctypes.c_int32, ip, ip, ip,
+                                  ctypes.c_int32, dp, dp, dp]
     _lib = lib
     return lib
 
@@ -131,6 +134,21 @@ def band_pairs(m, xp, vp, idx_i, h2_i, band: float = 1e-5, max_pairs: int = 1 <<
         raise RuntimeError(f"{n} band pairs exceed max_pairs={max_pairs}")
     order = np.lexsort((j[:n], k[:n]))
     return dict(k=k[:n][order], j=j[:n][order], r2=r2[:n][order], terms=terms[:n][order])
+
+
+def irregular(m, x0, v0, a0, j0, t0, t: float, idx_i, nnb, nblist, cap: int) -> dict:
+    """Neighbour (irregular) force / jerk / potential over the listed neighbours, each predicted to t
+    from the state at its own t0."""
+    lib = _load()
+    m, pm = _d(m); x0, px = _d(x0); v0, pv = _d(v0); a0, pa = _d(a0); j0, pj = _d(j0); t0, pt = _d(t0)
+    idx_i, pidx = _i(idx_i); nnb, pn = _i(nnb); nblist, pl = _i(nblist)
+    n = idx_i.shape[0]
+    assert nblist.shape == (n, cap) and nnb.shape == (n,)
+    out = dict(acc=np.zeros((n, 3)), jerk=np.zeros((n, 3)), pot=np.zeros(n))
+    rc = lib.orc_irregular(m.shape[0], pm, px, pv, pa, pj, pt, float(t), n, pidx, pn, pl, int(cap),
+                           _d(out["acc"])[1], _d(out["jerk"])[1], _d(out["pot"])[1])
+    assert rc == 0
+    return out
 
 
 def regular_step(cfg: dict, want_list: bool = True) -> dict:

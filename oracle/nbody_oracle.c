@@ -174,3 +174,66 @@ int64_t orc_band_pairs(int64_t N, const double *m, const double *xp, const doubl
     }
     return found;
 }
+
+/* Neighbour ("irregular") force, jerk and potential ("the irregular
+ * force accumulates only the neighbor forces"; "predict all neighbors and do the force
+ * calculation within one loop").  For each k, i = idx_i[k]: particle i and every listed
+ * j = nblist[k][e], e < min(nnb[k], cap), are predicted to time t with the polynomial of
+ * orc_predict (reading R2), then
+ *     acc[k]  = sum m_j r / r^3
+ *     jerk[k] = sum m_j ( v / r^3 - 3 (r.v) r / r^5 )
+ *     pot[k]  = - sum m_j / r            r = xp_j - xp_i, v = vp_j - vp_i
+ * over the listed j in list order; pair terms in double, sums in long double.  The state arrays
+ * are the caller's [N][3] / [N] inputs at the particles' own times t0.  Returns 0.
+ * Pins (tests/test_oracle_pins.py): equals orc_regular's neighbour sums for the lists orc_regular
+ * itself emits; regular + irregular = total; numpy brute force; two-body golden values. */
+int orc_irregular(int64_t N, const double *m, const double *x0, const double *v0, const double *a0,
+                  const double *j0, const double *t0, double t, int32_t n_i, const int32_t *idx_i,
+                  const int32_t *nnb, const int32_t *nblist, int32_t cap, double *acc, double *jerk,
+                  double *pot)
+{
+    (void)N;
+#pragma omp parallel for schedule(dynamic, 16)
+    for (int32_t k = 0; k < n_i; ++k) {
+        const int64_t i = idx_i[k];
+        double xi[3], vi[3];
+        {
+            double dt = t - t0[i], dt2 = dt * dt, dt3 = dt2 * dt;
+            for (int c = 0; c < 3; ++c) {
+                int64_t q = 3 * i + c;
+                xi[c] = x0[q] + v0[q] * dt + a0[q] * (dt2 / 2.0) + j0[q] * (dt3 / 6.0);
+                vi[c] = v0[q] + a0[q] * dt + j0[q] * (dt2 / 2.0);
+            }
+        }
+        long double A[3] = {0, 0, 0}, J[3] = {0, 0, 0}, P = 0;
+        int32_t cnt = nnb[k] < cap ? nnb[k] : cap;
+        for (int32_t e = 0; e < cnt; ++e) {
+            const int64_t j = nblist[(int64_t)k * cap + e];
+            double dt = t - t0[j], dt2 = dt * dt, dt3 = dt2 * dt;
+            double r[3], v[3];
+            for (int c = 0; c < 3; ++c) {
+                int64_t q = 3 * j + c;
+                double xj = x0[q] + v0[q] * dt + a0[q] * (dt2 / 2.0) + j0[q] * (dt3 / 6.0);
+                double vj = v0[q] + a0[q] * dt + j0[q] * (dt2 / 2.0);
+                r[c] = xj - xi[c];
+                v[c] = vj - vi[c];
+            }
+            double r2 = r[0] * r[0] + r[1] * r[1] + r[2] * r[2];
+            double rv = r[0] * v[0] + r[1] * v[1] + r[2] * v[2];
+            double r1 = sqrt(r2);
+            double mr3 = m[j] / (r2 * r1);
+            double c3 = 3.0 * rv / r2;
+            for (int c = 0; c < 3; ++c) {
+                A[c] += mr3 * r[c];
+                J[c] += mr3 * (v[c] - c3 * r[c]);
+            }
+            P -= m[j] / r1;
+        }
+        for (int c = 0; c < 3; ++c) {
+            acc[3 * k + c] = (double)A[c];
+            jerk[3 * k + c] = (double)J[c];
+        }
+        pot[k] = (double)P;
+    }
+    return 0;
+}

@@ -332,3 +332,88 @@ def test_config1_construction(oracle):
     # radius x1.01 => ~3 % more volume => 48 + Poisson(~1.5) neighbours, never fewer than 48
     assert out["nnb"].min() >= 48 and out["nnb"].max() < 64 and 48 <= out["nnb"].mean() < 52
     assert out["overflow"].sum() == 0
+
+
+# ----------------------------------------------------------------------------- neighbour (irregular) force
+
+def _golden_rows():
+    rows = {}
+    for line in (GOLD / "two_body.txt").read_text().splitlines():
+        if line.strip() and not line.startswith("#"):
+            k, *vals = line.split()
+            rows[k] = np.array([float(s) for s in vals])
+    return rows
+
+
+def test_irregular_two_body_golden_with_prediction(oracle):
+    """The paper-derived worked example (tests/golden/two_body.txt) reached THROUGH the predictor:
+    the partner starts at t0 = 0 with exactly representable a0, j0 chosen so that at t = 1/2 it sits at
+    r = (3,4,0) with v = (1,2,2) (all terms dyadic: no rounding)."""
+    g = _golden_rows()
+    dt = 0.5
+    a0 = np.array([2.0, -4.0, 0.0]); j0 = np.array([6.0, 0.0, -12.0])
+    v0 = g["v"] - a0 * dt - j0 * dt ** 2 / 2
+    x0 = g["r"] - v0 * dt - a0 * dt ** 2 / 2 - j0 * dt ** 3 / 6
+    z = np.zeros(3)
+    st = dict(m=np.array([1.0, g["m"][0]]), x0=np.stack([z, x0]), v0=np.stack([z, v0]), a0=np.stack([z, a0]),
+              j0=np.stack([z, j0]), t0=np.zeros(2))
+    out = oracle.irregular(st["m"], st["x0"], st["v0"], st["a0"], st["j0"], st["t0"], dt,
+                           np.array([0], np.int32), np.array([1], np.int32), np.array([[1, -1]], np.int32), cap=2)
+    np.testing.assert_allclose(out["acc"][0], g["acc"], rtol=0, atol=1e-16)
+    np.testing.assert_allclose(out["jerk"][0], g["jerk"], rtol=0, atol=1e-16)
+    assert abs(out["pot"][0] - g["pot"][0]) < 1e-16
+    # empty list -> exact zeros; nnb above cap -> only the cap stored entries count
+    out = oracle.irregular(st["m"], st["x0"], st["v0"], st["a0"], st["j0"], st["t0"], dt,
+                           np.array([0, 0], np.int32), np.array([0, 7], np.int32), np.array([[1], [1]], np.int32), cap=1)
+    assert not out["acc"][0].any() and out["pot"][0] == 0
+    np.testing.assert_allclose(out["acc"][1], g["acc"], atol=1e-16)
+
+
+def test_irregular_brute_force_numpy(oracle):
+    """Second, independent statement in numpy (vectorised over the list) with random lists, random
+    individual t0 and a random time t."""
+    rng = np.random.default_rng(5)
+    N, n, cap = 60, 17, 12
+    m, x0, v0 = _rand_system(N, 11)
+    a0 = rng.normal(size=(N, 3)); j0 = rng.normal(size=(N, 3)); t0 = rng.uniform(0, 0.1, N); t = 0.17
+    idx = rng.choice(N, n, replace=False).astype(np.int32)
+    nnb = rng.integers(0, cap + 4, n).astype(np.int32)              # some rows "overflowed"
+    lst = np.full((n, cap), -1, np.int32)
+    for k in range(n):
+        others = np.setdiff1d(np.arange(N), [idx[k]])
+        c = min(nnb[k], cap)
+        lst[k, :c] = rng.choice(others, c, replace=False)
+    out = oracle.irregular(m, x0, v0, a0, j0, t0, t, idx, nnb, lst, cap)
+    dt = (t - t0)[:, None]
+    xp = x0 + v0 * dt + a0 * dt ** 2 / 2 + j0 * dt ** 3 / 6
+    vp = v0 + a0 * dt + j0 * dt ** 2 / 2
+    for k in range(n):
+        js = lst[k, :min(nnb[k], cap)]
+        r = xp[js] - xp[idx[k]]; v = vp[js] - vp[idx[k]]
+        d = np.linalg.norm(r, axis=1)
+        rv = np.einsum("ij,ij->i", r, v)
+        a = (m[js, None] * r / d[:, None] ** 3).sum(0)
+        jk = (m[js, None] * (v / d[:, None] ** 3 - 3 * rv[:, None] * r / d[:, None] ** 5)).sum(0)
+        p = -(m[js] / d).sum()
+        np.testing.assert_allclose(out["acc"][k], a, rtol=1e-12, atol=1e-14)
+        np.testing.assert_allclose(out["jerk"][k], jk, rtol=1e-11, atol=1e-13)
+        assert abs(out["pot"][k] - p) <= 1e-13 * max(abs(p), 1e-3)
+
+
+def test_irregular_plus_regular_is_total(oracle):
+    """regular = outside the neighbour radius, irregular = the neighbours.  With the lists the
+    regular pass emits, irregular equals that pass's own neighbour sums and regular + irregular is the
+    total direct force at the same time."""
+    cfg = nbgen.make_config(2, N=2048, n_i=256)
+    st = [cfg[k] for k in ("m", "x0", "v0", "a0", "j0", "t0")]
+    xp, vp = oracle.predict(*st[1:], cfg["t"])
+    h2 = cfg["h2_i"] * 4.0
+    cap = 2048
+    reg = oracle.regular(cfg["m"], xp, vp, cfg["idx_i"], h2, cap)
+    tot = oracle.regular(cfg["m"], xp, vp, cfg["idx_i"], np.zeros_like(h2), cap)
+    irr = oracle.irregular(*st, cfg["t"], cfg["idx_i"], reg["nnb"], reg["nblist"], cap)
+    assert reg["overflow"].sum() == 0 and reg["nnb"].sum() > 1000
+    for key in ("acc", "jerk", "pot"):
+        sc = np.abs(reg[key + "_nb"]).max()
+        assert np.max(np.abs(irr[key] - reg[key + "_nb"])) < 1e-13 * sc
+        assert np.max(np.abs(reg[key] + irr[key] - tot[key])) < 1e-13 * max(sc, np.abs(tot[key]).max())
