@@ -357,6 +357,37 @@ def run_b200(args):
                           "variant": ctx.info("last_variant"), "jsplit": ctx.info("last_jsplit")})
             del so
 
+    # ---- the steps either side of the path, timed alone; not part of `value`
+    extras = None
+    if not args.no_sweep and world == 1:
+        def timed(fn, reps=5):
+            best = 1e30
+            for _ in range(reps):
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record(stream); fn(); b.record(stream)
+                torch.cuda.synchronize()
+                best = min(best, a.elapsed_time(b))
+            return best
+        ctx.regular(idx, h2, **out)                      # lists of the timed block
+        torch.cuda.synchronize()
+        nn = int(out["nnb"].clamp(max=cap).sum())
+        irr = dict(acc=torch.empty_like(out["acc"]), jerk=torch.empty_like(out["jerk"]), pot=torch.empty_like(out["pot"]))
+        ms_irr = timed(lambda: ctx.irregular(t_pred, idx, out["nnb"], out["nblist"], **irr))
+        sub = [t[idx.long()].contiguous() for t in jstate]
+        ms_upd = timed(lambda: ctx.update_j(idx, *sub))
+        ctx.predict_all(t_pred)
+        ms_pred = timed(lambda: ctx.predict_all(t_pred))
+        ms_setj = timed(lambda: ctx.set_j(*jstate))
+        ctx.predict_all(t_pred)
+        extras = {
+            "nb_irregular": {"n_i": n_i, "neighbour_pairs": nn, "ms": ms_irr, "pairs_per_s": nn / (ms_irr * 1e-3),
+                             "gather_GBps": nn * 128 / (ms_irr * 1e-3) / 1e9, "dtype": "f64"},
+            "nb_update_j": {"n": n_i, "ms": ms_upd},
+            "nb_predict_all": {"ms": ms_pred, "GBps": N * (112 + 40) / (ms_pred * 1e-3) / 1e9,
+                               "frac_hbm": N * (112 + 40) / (ms_pred * 1e-3) / 1e9 / pk.get("hbm_gbs", 6460.0)},
+            "nb_set_j": {"ms": ms_setj, "GBps": N * (112 + 112 + 128) / (ms_setj * 1e-3) / 1e9},
+        }
+
     cpu = None
     if not args.no_cpu_baseline and world == 1:
         cpu = cpu_oracle_rate(cfg, idx_np, h2_np, seconds_target=12.0)
@@ -375,7 +406,7 @@ def run_b200(args):
                    **plan},
         "frac_fp32_peak": value / world * FLOP_PER_INTERACTION / 1e12 / peak_tflops,
         "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
-        "cpu_baseline": cpu, "sweep": sweep, "peaks_source": pk_src,
+        "cpu_baseline": cpu, "sweep": sweep, "extras": extras, "peaks_source": pk_src,
     }
     print(json.dumps(line), flush=True)
     if world > 1:

@@ -23,8 +23,8 @@
  *     call on that context returns NB_ECUDA.  Neighbour-list overflow is NOT an error.
  *   - There is no CPU fallback: without a usable sm_100 device nb_open fails with NB_ECUDA.
  *   - Results are bitwise reproducible run to run for fixed inputs and a fixed launch plan (two-stage
- *     fixed-order reduction, no floating-point atomics); only the ORDER of the entries inside one
- *     neighbour-list row may vary.
+ *     fixed-order reduction, no floating-point atomics); list rows are sorted, so they are too, except
+ *     WHICH nb_cap neighbours an overflowed row keeps.
  *
  * Precision of the pair arithmetic (the paper does not state its kernel's precision; DESIGN.md
  * "Precision"): positions are differenced at FP64-equivalent accuracy (two-float hi/lo split,
@@ -54,7 +54,8 @@ enum {
 
 /* Create a context for N j-particles and a neighbour-list capacity of nb_cap entries per active
  * particle (north_star: nb_open(N); the capacity has to come from somewhere -- DESIGN.md R18).
- * Allocates: FP64 j-state (14 N doubles), predicted SoA (48 B per particle, padded), counters,
+ * Allocates: FP64 j-state twice (14 N doubles streamed by the predictor + a 128 B/body gather copy),
+ * predicted records (40 B per particle, padded), counters,
  * split-j scratch (grown on demand). */
 int nb_open(int64_t N, int32_t nb_cap, nb_ctx **out);
 int nb_close(nb_ctx *ctx);
@@ -71,6 +72,13 @@ int nb_set_j(nb_ctx *ctx, const double *m, const double *x0, const double *v0, c
 /* Same with HOST pointers: host->device copies, then the same re-layout kernel. */
 int nb_set_j_host(nb_ctx *ctx, const double *m, const double *x0, const double *v0,
                   const double *a0, const double *j0, const double *t0);
+
+/* Incremental "Send.R": after a block step only the n integrated
+ * particles changed -- replace the state of bodies idx[0..n) (unique, in range, unchecked) by
+ * m[n], x0[n][3], v0[n][3], a0[n][3], j0[n][3], t0[n].  The predicted records become stale:
+ * nb_regular needs a new nb_predict_all.  DEVICE pointers.  Requires nb_set_j; n = 0 is a no-op. */
+int nb_update_j(nb_ctx *ctx, int32_t n, const int32_t *idx, const double *m, const double *x0,
+                const double *v0, const double *a0, const double *j0, const double *t0);
 
 /* a2 "Pred." (Table 1): predict every particle to time t,
  *     dt = t - t0[j];  xp = x0 + v0 dt + a0 dt^2/2 + j0 dt^3/6;  vp = v0 + a0 dt + j0 dt^2/2
@@ -90,8 +98,9 @@ int nb_get_predicted(nb_ctx *ctx, double *xp, double *vp);
  *                        pot[k]  -= m_j / r
  *   nnb[k]      = TRUE number of neighbours (may exceed nb_cap)
  *   overflow[k] = nnb[k] > nb_cap
- *   nblist[k][0 .. min(nnb[k], nb_cap))  = neighbour indices j, in unspecified order; on overflow
- *                 any nb_cap of the true neighbours.  Entries beyond that are left untouched.
+ *   nblist[k][0 .. min(nnb[k], nb_cap))  = neighbour indices j in ascending order (rows are sorted
+ *                 after the pass whenever nb_cap <= 32768; above that the order is unspecified); on
+ *                 overflow any nb_cap of the true neighbours.  Entries beyond that are left untouched.
  *   The sums exclude ALL true neighbours whether or not the list overflowed.
  * h2_i[k] <= 0 means "no neighbours" (total force / full potential).  The i-particle's own state is
  * its predicted record (index idx_i[k]); the self pair is skipped by index.
@@ -112,6 +121,19 @@ int nb_regular_all(nb_ctx *ctx, const double *h2, double *acc, double *jerk, dou
  * nblist may be NULL to skip the list copy-back (the list is still built on the device). */
 int nb_regular_host(nb_ctx *ctx, int32_t n_i, const int32_t *idx_i, const double *h2_i, double *acc,
                     double *jerk, double *pot, int32_t *nnb, int32_t *nblist, int32_t *overflow);
+
+/* Neighbour ("irregular") force on the GPU ("the irregular force
+ * accumulates only the neighbor forces"; "predict all neighbors and do the force calculation
+ * within one loop"; the paper runs this step on AVX/SSE CPUs).  For k = 0..n_i-1, i = idx_i[k]:
+ * particle i and each j in nblist[k][0 .. min(nnb[k], nb_cap)) are predicted to time t from the FP64
+ * j-state (same polynomial as nb_predict_all; nb_predict_all itself is NOT required) and
+ *     acc[k] = sum_j m_j r / r^3,  jerk[k] = sum_j m_j ( v / r^3 - 3 (r.v) r / r^5 ),
+ *     pot[k] = - sum_j m_j / r           (pot may be NULL)
+ * in FP64 throughout (max rel. error vs the FP64 definition ~1e-13).  nnb / nblist have the layout
+ * nb_regular writes ([n_i], [n_i][nb_cap]) and may be its outputs unchanged; a row that overflowed
+ * contributes its nb_cap stored entries.  DEVICE pointers.  Requires nb_set_j. */
+int nb_irregular(nb_ctx *ctx, double t, int32_t n_i, const int32_t *idx_i, const int32_t *nnb,
+                 const int32_t *nblist, double *acc, double *jerk, double *pot);
 
 /* Tuning / introspection.  Keys: */
 enum {

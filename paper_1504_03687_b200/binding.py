@@ -51,6 +51,8 @@ def load_library(build: bool = True) -> ctypes.CDLL:
     lib.nb_regular.argtypes = [_vp, i32] + [_vp] * 8
     lib.nb_regular_host.argtypes = [_vp, i32] + [_vp] * 8
     lib.nb_regular_all.argtypes = [_vp] + [_vp] * 7
+    lib.nb_update_j.argtypes = [_vp, i32] + [_vp] * 7
+    lib.nb_irregular.argtypes = [_vp, dbl, i32] + [_vp] * 6
     lib.nb_get_info.argtypes = [_vp, i32, ctypes.POINTER(i64)]
     lib.nb_set_tuning.argtypes = [_vp, i32, i64]
     lib.nb_last_cuda_error.argtypes = [_vp]
@@ -158,6 +160,26 @@ class NbContext:
                 _dev_ptr(a0, f8, 3 * N, "a0"), _dev_ptr(j0, f8, 3 * N, "j0"), _dev_ptr(t0, f8, N, "t0")]
         _check(self._lib.nb_set_j(self._ctx, *args), "nb_set_j", self._ctx)
 
+    def update_j(self, idx, m, x0, v0, a0, j0, t0):
+        import torch
+        n, f8 = int(idx.numel()), torch.float64
+        if n == 0:
+            return
+        args = [_dev_ptr(idx, torch.int32, n, "idx"), _dev_ptr(m, f8, n, "m"), _dev_ptr(x0, f8, 3 * n, "x0"),
+                _dev_ptr(v0, f8, 3 * n, "v0"), _dev_ptr(a0, f8, 3 * n, "a0"), _dev_ptr(j0, f8, 3 * n, "j0"),
+                _dev_ptr(t0, f8, n, "t0")]
+        _check(self._lib.nb_update_j(self._ctx, n, *args), "nb_update_j", self._ctx)
+
+    def irregular(self, t: float, idx_i, nnb, nblist, acc, jerk, pot=None):
+        import torch
+        n, f8, i4 = int(idx_i.numel()), torch.float64, torch.int32
+        if n == 0:
+            return
+        args = [_dev_ptr(idx_i, i4, n, "idx_i"), _dev_ptr(nnb, i4, n, "nnb"),
+                _dev_ptr(nblist, i4, n * self.cap, "nblist"), _dev_ptr(acc, f8, 3 * n, "acc"),
+                _dev_ptr(jerk, f8, 3 * n, "jerk"), _vp() if pot is None else _dev_ptr(pot, f8, n, "pot")]
+        _check(self._lib.nb_irregular(self._ctx, float(t), n, *args), "nb_irregular", self._ctx)
+
     def predict_all(self, t: float):
         _check(self._lib.nb_predict_all(self._ctx, float(t)), "nb_predict_all", self._ctx)
 
@@ -241,6 +263,14 @@ def nb_predict_all(ctx: NbContext, t: float):
 
 def nb_regular(ctx: NbContext, idx_i, h2_i, acc, jerk, pot, nnb, nblist, overflow):
     ctx.regular(idx_i, h2_i, acc, jerk, pot, nnb, nblist, overflow)
+
+
+def nb_update_j(ctx: NbContext, idx, m, x0, v0, a0, j0, t0):
+    ctx.update_j(idx, m, x0, v0, a0, j0, t0)
+
+
+def nb_irregular(ctx: NbContext, t: float, idx_i, nnb, nblist, acc, jerk, pot=None):
+    ctx.irregular(t, idx_i, nnb, nblist, acc, jerk, pot)
 
 
 def nb_regular_all(ctx: NbContext, h2, acc, jerk, pot, nnb, nblist, overflow):

@@ -37,6 +37,8 @@ struct nb_ctx {
     bool have_j = false, have_pred = false;
     // device state owned by the library
     double *soa = nullptr;                  // [14][Ns]
+    double *aos = nullptr;                  // [N][16] gather copy (one 128 B line per body)
+    int sort_P = 0; size_t sort_smem_max = 0;   // list-row sort: power of two >= cap; opt-in dynamic smem limit
     float *rec = nullptr;                   // predicted records [Npad / TJ][RECF][TJ]
     int32_t *cnt = nullptr;                 // [N] zero between calls
     double *partial = nullptr;  size_t partial_bytes = 0;
@@ -184,15 +186,23 @@ int regular_device(nb_ctx *c, int32_t n_i, const int32_t *idx_i, const double *h
         NB_CUDA(c, cudaEventRecord(c->ev1[slot], c->stream));
         c->prof_n += 1;
     }
-    const unsigned fgrid = (unsigned)((n_i + 31) / 32);
-    if (S <= 8)
-        finalize_kernel<4><<<fgrid, 128, 0, c->stream>>>(n_i, (int32_t)n_i_pad, S, c->cap, c->partial, c->cnt, acc,
-                                                         jerk, pot, nnb, overflow);
-    else
-        finalize_kernel<16><<<fgrid, 512, 0, c->stream>>>(n_i, (int32_t)n_i_pad, S, c->cap, c->partial, c->cnt, acc,
-                                                          jerk, pot, nnb, overflow);
-    NB_CUDA(c, cudaGetLastError());
-    c->launches += 2;
+    {
+        const int W = S <= 8 ? 4 : 16;
+        const size_t row_bytes = (size_t)c->sort_P * sizeof(int32_t);
+        int sortW = (int)std::min<size_t>(W, c->sort_smem_max / row_bytes);     // rows sorted per CTA
+        const int sortP = (nblist && sortW > 0) ? c->sort_P : 0;                // 0: rows stay in append order
+        sortW = std::max(sortW, 1);
+        const dim3 fgrid((unsigned)((n_i + 31) / 32), (unsigned)(7 + (32 + sortW - 1) / sortW));
+        const size_t smem = sortP ? (size_t)sortW * row_bytes : 0;
+        if (W == 4)
+            finalize_kernel<4><<<fgrid, 128, smem, c->stream>>>(n_i, (int32_t)n_i_pad, S, c->cap, sortP, sortW,
+                                                                 c->partial, c->cnt, acc, jerk, pot, nnb, nblist, overflow);
+        else
+            finalize_kernel<16><<<fgrid, 512, smem, c->stream>>>(n_i, (int32_t)n_i_pad, S, c->cap, sortP, sortW,
+                                                                  c->partial, c->cnt, acc, jerk, pot, nnb, nblist, overflow);
+        NB_CUDA(c, cudaGetLastError());
+        c->launches += 2;
+    }
     c->last_S = S; c->last_iblock = v.iblock; c->last_grid = n_ib * S; c->last_variant = vi;
     return NB_OK;
 }
@@ -221,9 +231,20 @@ int nb_open(int64_t N, int32_t nb_cap, nb_ctx **out) {
     c->sm_count = prop.multiProcessorCount;
     *out = c;     // from here on nb_close() releases whatever was allocated
     NB_CUDA(c, cudaMalloc(&c->soa, sizeof(double) * 14 * c->Ns));
+    NB_CUDA(c, cudaMalloc(&c->aos, sizeof(double) * AOS_D * c->N));
     NB_CUDA(c, cudaMalloc(&c->rec, sizeof(float) * RECF * c->Npad));
     NB_CUDA(c, cudaMalloc(&c->cnt, sizeof(int32_t) * c->N));
     NB_CUDA(c, cudaMemset(c->cnt, 0, sizeof(int32_t) * c->N));
+    {   // ascending list rows: one warp per row, P ints of shared memory each (finalize_kernel)
+        int P = 32;
+        while (P < nb_cap) P <<= 1;
+        c->sort_P = P;
+        c->sort_smem_max = 200 * 1024;
+        const int s4 = (int)std::min<size_t>(c->sort_smem_max, (size_t)4 * P * sizeof(int32_t));
+        const int s16 = (int)std::min<size_t>(c->sort_smem_max, (size_t)16 * P * sizeof(int32_t));
+        NB_CUDA(c, cudaFuncSetAttribute(finalize_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, s4));
+        NB_CUDA(c, cudaFuncSetAttribute(finalize_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, s16));
+    }
     NB_CUDA(c, (setup_variant<8, 1, 2>(c->var[0], 0.5)));
     NB_CUDA(c, (setup_variant<4, 2, 2>(c->var[1], 0.75)));
     NB_CUDA(c, (setup_variant<2, 4, 2>(c->var[2], 1.5)));
@@ -234,7 +255,7 @@ int nb_open(int64_t N, int32_t nb_cap, nb_ctx **out) {
 int nb_close(nb_ctx *c) {
     if (!c) return NB_EINVAL;
     cudaStreamSynchronize(c->stream);
-    cudaFree(c->soa); cudaFree(c->rec); cudaFree(c->cnt);
+    cudaFree(c->soa); cudaFree(c->aos); cudaFree(c->rec); cudaFree(c->cnt);
     cudaFree(c->partial); cudaFree(c->stage_j);
     cudaFree(c->st_idx); cudaFree(c->st_nnb); cudaFree(c->st_ovf); cudaFree(c->st_list);
     cudaFree(c->st_h2); cudaFree(c->st_out);
@@ -265,7 +286,8 @@ int nb_set_j(nb_ctx *c, const double *m, const double *x0, const double *v0, con
     int rc = check_live(c);
     if (rc != NB_OK) return rc;
     if (!m || !x0 || !v0 || !a0 || !j0 || !t0) return NB_EINVAL;
-    relayout_kernel<<<(unsigned)((c->N + 255) / 256), 256, 0, c->stream>>>(c->N, c->Ns, m, x0, v0, a0, j0, t0, c->soa);
+    relayout_kernel<<<(unsigned)((c->N + 255) / 256), 256, 0, c->stream>>>(c->N, c->Ns, m, x0, v0, a0, j0, t0, c->soa,
+                                                                           c->aos);
     NB_CUDA(c, cudaGetLastError());
     c->launches += 1;
     c->have_j = true;
@@ -289,6 +311,37 @@ int nb_set_j_host(nb_ctx *c, const double *m, const double *x0, const double *v0
     NB_CUDA(c, cudaMemcpyAsync(dj, j0, sizeof(double) * 3 * N, cudaMemcpyHostToDevice, c->stream));
     NB_CUDA(c, cudaMemcpyAsync(dt, t0, sizeof(double) * N, cudaMemcpyHostToDevice, c->stream));
     return nb_set_j(c, dm, dx, dv, da, dj, dt);
+}
+
+int nb_update_j(nb_ctx *c, int32_t n, const int32_t *idx, const double *m, const double *x0, const double *v0,
+                const double *a0, const double *j0, const double *t0) {
+    int rc = check_live(c);
+    if (rc != NB_OK) return rc;
+    if (n < 0 || n > c->N) return NB_EINVAL;
+    if (!c->have_j) return NB_ESTATE;
+    if (n == 0) return NB_OK;
+    if (!idx || !m || !x0 || !v0 || !a0 || !j0 || !t0) return NB_EINVAL;
+    update_j_kernel<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(n, c->Ns, idx, m, x0, v0, a0, j0, t0, c->soa,
+                                                                         c->aos);
+    NB_CUDA(c, cudaGetLastError());
+    c->launches += 1;
+    c->have_pred = false;       // the predicted records are stale until the next nb_predict_all
+    return NB_OK;
+}
+
+int nb_irregular(nb_ctx *c, double t, int32_t n_i, const int32_t *idx_i, const int32_t *nnb, const int32_t *nblist,
+                 double *acc, double *jerk, double *pot) {
+    int rc = check_live(c);
+    if (rc != NB_OK) return rc;
+    if (n_i < 0 || n_i > c->N) return NB_EINVAL;
+    if (!c->have_j) return NB_ESTATE;
+    if (n_i == 0) return NB_OK;
+    if (!idx_i || !nnb || !nblist || !acc || !jerk) return NB_EINVAL;
+    irregular_kernel<<<(unsigned)((n_i + 7) / 8), 256, 0, c->stream>>>(n_i, c->cap, t, idx_i, nnb, nblist, c->aos, acc,
+                                                                       jerk, pot);
+    NB_CUDA(c, cudaGetLastError());
+    c->launches += 1;
+    return NB_OK;
 }
 
 int nb_predict_all(nb_ctx *c, double t) {

@@ -72,22 +72,59 @@ __device__ __forceinline__ float rsqrt_sfu(float x) {   // one MUFU.RSQ, no deno
 }
 
 // ------------------------------------------------------------------ a1: re-layout
-// in: m[N], x0[N][3], v0[N][3], a0[N][3], j0[N][3], t0[N]  ->  soa[14][Ns] (component-major).
+// in: m[N], x0[N][3], v0[N][3], a0[N][3], j0[N][3], t0[N]  ->  soa[14][Ns] (component-major, streamed
+// by the predictor) and aos[N][16] (one 128 B line per body: m, x0, v0, a0, j0, t0, 2 pad -- gathered
+// by the neighbour-force kernel, which predicts only the listed bodies).
+constexpr int AOS_D = 16;
+__device__ __forceinline__ void store_body(int64_t j, int64_t Ns, double m, const double *x, const double *v,
+                                           const double *a, const double *jk, double t0, double *__restrict__ soa,
+                                           double *__restrict__ aos) {
+    soa[0 * Ns + j] = m;
+    soa[13 * Ns + j] = t0;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        soa[(1 + c) * Ns + j] = x[c];
+        soa[(4 + c) * Ns + j] = v[c];
+        soa[(7 + c) * Ns + j] = a[c];
+        soa[(10 + c) * Ns + j] = jk[c];
+    }
+    double2 *o = reinterpret_cast<double2 *>(aos + j * AOS_D);
+    o[0] = make_double2(m, x[0]);     o[1] = make_double2(x[1], x[2]);
+    o[2] = make_double2(v[0], v[1]);  o[3] = make_double2(v[2], a[0]);
+    o[4] = make_double2(a[1], a[2]);  o[5] = make_double2(jk[0], jk[1]);
+    o[6] = make_double2(jk[2], t0);   o[7] = make_double2(0.0, 0.0);
+}
+
 __global__ void __launch_bounds__(256) relayout_kernel(int64_t N, int64_t Ns, const double *__restrict__ m,
                                                        const double *__restrict__ x0, const double *__restrict__ v0,
                                                        const double *__restrict__ a0, const double *__restrict__ j0,
-                                                       const double *__restrict__ t0, double *__restrict__ soa) {
+                                                       const double *__restrict__ t0, double *__restrict__ soa,
+                                                       double *__restrict__ aos) {
     int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= N) return;
-    soa[0 * Ns + j] = m[j];
-    soa[13 * Ns + j] = t0[j];
+    double x[3], v[3], a[3], jk[3];
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
-        soa[(1 + c) * Ns + j] = x0[3 * j + c];
-        soa[(4 + c) * Ns + j] = v0[3 * j + c];
-        soa[(7 + c) * Ns + j] = a0[3 * j + c];
-        soa[(10 + c) * Ns + j] = j0[3 * j + c];
+        x[c] = x0[3 * j + c]; v[c] = v0[3 * j + c]; a[c] = a0[3 * j + c]; jk[c] = j0[3 * j + c];
     }
+    store_body(j, Ns, m[j], x, v, a, jk, t0[j], soa, aos);
+}
+
+// Incremental ingest (NEXT-3; "Send.R" after a block step only the n integrated particles
+// changed): the same stores for the bodies idx[0..n).
+__global__ void __launch_bounds__(256) update_j_kernel(int32_t n, int64_t Ns, const int32_t *__restrict__ idx,
+                                                       const double *__restrict__ m, const double *__restrict__ x0,
+                                                       const double *__restrict__ v0, const double *__restrict__ a0,
+                                                       const double *__restrict__ j0, const double *__restrict__ t0,
+                                                       double *__restrict__ soa, double *__restrict__ aos) {
+    const int q = blockIdx.x * blockDim.x + threadIdx.x;
+    if (q >= n) return;
+    double x[3], v[3], a[3], jk[3];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        x[c] = x0[3 * q + c]; v[c] = v0[3 * q + c]; a[c] = a0[3 * q + c]; jk[c] = j0[3 * q + c];
+    }
+    store_body(idx[q], Ns, m[q], x, v, a, jk, t0[q], soa, aos);
 }
 
 // ------------------------------------------------------------------ a2: predictor
@@ -97,6 +134,18 @@ __device__ __forceinline__ float *rec_slot(float *rec, int64_t j) {      // &rec
 }
 __device__ __forceinline__ const float *rec_slot(const float *rec, int64_t j) {
     return rec + (j / TJ) * TILE_FLOATS + (j % TJ);
+}
+
+// One component of the Taylor predictor, FP64.  The jerk term is rounded on its own (not fused) so
+// that for dyadic inputs with j0 = 6 q the product rounds back to q dt^3 exactly and the whole sum is
+// exact (tests: bitwise vs oracle).  Used by predict_kernel (all j) and irregular_kernel (listed j).
+__device__ __forceinline__ double taylor_c2(double dt) { return 0.5 * (dt * dt); }                  // dt^2/2: exact for dyadic dt
+__device__ __forceinline__ double taylor_c3(double dt) { return (dt * dt * dt) * (1.0 / 6.0); }     // dt^3/6: the only inexact coefficient
+__device__ __forceinline__ void predict_component(double x, double v, double a, double jk, double dt, double c2,
+                                                  double c3, double &xp, double &vp) {
+    const double p3 = __dmul_rn(jk, c3);
+    xp = __dadd_rn(fma(a, c2, fma(v, dt, x)), p3);
+    vp = fma(jk, c2, fma(a, dt, v));
 }
 
 __global__ void __launch_bounds__(256) predict_kernel(int64_t N, int64_t Npad, int64_t Ns, double t,
@@ -112,17 +161,12 @@ __global__ void __launch_bounds__(256) predict_kernel(int64_t N, int64_t Npad, i
         return;
     }
     const double dt = t - soa[13 * Ns + j];
-    const double c2 = 0.5 * (dt * dt);                    // dt^2/2: exact for dyadic dt
-    const double c3 = (dt * dt * dt) * (1.0 / 6.0);       // dt^3/6: the only inexact coefficient
+    const double c2 = taylor_c2(dt), c3 = taylor_c3(dt);
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
-        const double x = soa[(1 + c) * Ns + j], v = soa[(4 + c) * Ns + j];
-        const double a = soa[(7 + c) * Ns + j], jk = soa[(10 + c) * Ns + j];
-        // The jerk term is rounded on its own (not fused) so that for dyadic inputs with j0 = 6 q the
-        // product rounds back to q dt^3 exactly and the whole sum is exact (tests: bitwise vs oracle).
-        const double p3 = __dmul_rn(jk, c3);
-        const double xp = __dadd_rn(fma(a, c2, fma(v, dt, x)), p3);
-        const double vp = fma(jk, c2, fma(a, dt, v));
+        double xp, vp;
+        predict_component(soa[(1 + c) * Ns + j], soa[(4 + c) * Ns + j], soa[(7 + c) * Ns + j],
+                          soa[(10 + c) * Ns + j], dt, c2, c3, xp, vp);
         const float hi = __double2float_rn(xp);
         r[(C_XH + c) * TJ] = hi;
         r[(C_XL + c) * TJ] = __double2float_rn(xp - (double)hi);
@@ -292,14 +336,14 @@ __global__ void __launch_bounds__(32 * WI *WJ, MINB) force_kernel(const ForcePar
 #pragma unroll
         for (int c = 0; c < 7; ++c) acc64[h][c] = 0.0;
 
+    Acc7 A;                   // FP32 partial sums of at most TJ pair terms (WJ tile shares of SUB j each)
+    A.ax = A.ay = A.az = A.jx = A.jy = A.jz = A.ph = make_float2(0.f, 0.f);
+
     for (int it = 0; it < ntile; ++it) {
         const int s = it % NSTAGE;
         mbar_wait(&full[s], (uint32_t)((it / NSTAGE) & 1));
         const float *tsub = srec + (size_t)s * TILE_FLOATS + wj * SUB;      // &tile[0][wj * SUB]
         const int32_t jbase = (tile_begin + it) * TJ + wj * SUB;
-
-        Acc7 A;               // FP32 partial sums of this tile share
-        A.ax = A.ay = A.az = A.jx = A.jy = A.jz = A.ph = make_float2(0.f, 0.f);
 
 #pragma unroll 2
         for (int g = 0; g < SUB; g += UNROLL_J) {
@@ -342,14 +386,17 @@ __global__ void __launch_bounds__(32 * WI *WJ, MINB) force_kernel(const ForcePar
                 }
             }
         }
-        // tile flush: FP32 partial sums of <= SUB terms go into the FP64 running sums
-        acc64[0][0] += (double)A.ax.x; acc64[1][0] += (double)A.ax.y;
-        acc64[0][1] += (double)A.ay.x; acc64[1][1] += (double)A.ay.y;
-        acc64[0][2] += (double)A.az.x; acc64[1][2] += (double)A.az.y;
-        acc64[0][3] += (double)A.jx.x; acc64[1][3] += (double)A.jx.y;
-        acc64[0][4] += (double)A.jy.x; acc64[1][4] += (double)A.jy.y;
-        acc64[0][5] += (double)A.jz.x; acc64[1][5] += (double)A.jz.y;
-        acc64[0][6] += (double)A.ph.x; acc64[1][6] += (double)A.ph.y;
+        // flush: FP32 partial sums of <= WJ * SUB = TJ terms go into the FP64 running sums
+        if ((it + 1) % WJ == 0 || it + 1 == ntile) {
+            acc64[0][0] += (double)A.ax.x; acc64[1][0] += (double)A.ax.y;
+            acc64[0][1] += (double)A.ay.x; acc64[1][1] += (double)A.ay.y;
+            acc64[0][2] += (double)A.az.x; acc64[1][2] += (double)A.az.y;
+            acc64[0][3] += (double)A.jx.x; acc64[1][3] += (double)A.jx.y;
+            acc64[0][4] += (double)A.jy.x; acc64[1][4] += (double)A.jy.y;
+            acc64[0][5] += (double)A.jz.x; acc64[1][5] += (double)A.jz.y;
+            acc64[0][6] += (double)A.ph.x; acc64[1][6] += (double)A.ph.y;
+            A.ax = A.ay = A.az = A.jx = A.jy = A.jz = A.ph = make_float2(0.f, 0.f);
+        }
 
         // Stage hand-back without a CTA barrier: the LAST warp to finish with stage s refills it, so
         // warps drift up to NSTAGE-1 tiles apart instead of meeting at a __syncthreads every tile.
@@ -402,44 +449,149 @@ __global__ void __launch_bounds__(32 * WI *WJ, MINB) force_kernel(const ForcePar
 }
 
 // ------------------------------------------------------------------ a6-a7: finalize
-// CTA = 32 consecutive active particles (lanes: coalesced 256 B rows of the partials) x W warps that
-// stride over the S split partials with all their loads in flight; then a fixed-order sum over the W
-// warps in shared memory -- deterministic for a given (S, W).
+// ONE launch, two roles, grid = (ceil(n_i / 32), 7 + ceil(32 / sortW)), CTA = 32 x W threads:
+//   blockIdx.y <  7 : fixed-order sum of the S split partials of quantity q = blockIdx.y for 32
+//                     consecutive active particles -- lanes along i (coalesced 256 B rows), warps along
+//                     the splits with eight loads in flight each, then the W warps in order.
+//   blockIdx.y >= 7 : one warp per list row: nnb / overflow from the row counter (re-zeroed for the next
+//                     call) and a bitonic sort of the stored entries in shared memory (sortP ints per
+//                     warp, sortW <= W warps per CTA; sortP = 0: rows too long, left in append order).  Sorting makes the list
+//                     output deterministic and equal to the oracle's ascending rows.
 template <int W>
 __global__ void __launch_bounds__(32 * W) finalize_kernel(int32_t n_i, int32_t n_i_pad, int32_t S, int32_t cap,
-                                                          const double *__restrict__ partial, int32_t *__restrict__ cnt,
-                                                          double *__restrict__ acc, double *__restrict__ jerk,
-                                                          double *__restrict__ pot, int32_t *__restrict__ nnb,
+                                                          int32_t sortP, int32_t sortW,
+                                                          const double *__restrict__ partial,
+                                                          int32_t *__restrict__ cnt, double *__restrict__ acc,
+                                                          double *__restrict__ jerk, double *__restrict__ pot,
+                                                          int32_t *__restrict__ nnb, int32_t *__restrict__ nblist,
                                                           int32_t *__restrict__ overflow) {
-    __shared__ double red[W][7][32];
+    extern __shared__ int32_t sbuf[];
+    __shared__ double red[W][32];
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    const int k = blockIdx.x * 32 + lane;          // k < n_i_pad always (n_i_pad is a multiple of 64)
-    double s[7];
+    if (blockIdx.y < 7) {
+        const int q = blockIdx.y;
+        const int k = blockIdx.x * 32 + lane;          // k < n_i_pad always (n_i_pad is a multiple of 64)
+        const double *src = partial + (size_t)q * n_i_pad + k;
+        const size_t stride = (size_t)7 * n_i_pad;
+        double s = 0.0;
+        for (int base = w; base < S; base += 8 * W) {
+            double v[8];
 #pragma unroll
-    for (int q = 0; q < 7; ++q) s[q] = 0.0;
-#pragma unroll 4
-    for (int sp = w; sp < S; sp += W) {
+            for (int u = 0; u < 8; ++u) {
+                const int sp = base + u * W;
+                v[u] = sp < S ? src[(size_t)sp * stride] : 0.0;
+            }
 #pragma unroll
-        for (int q = 0; q < 7; ++q) s[q] += partial[((size_t)sp * 7 + q) * n_i_pad + k];
-    }
-#pragma unroll
-    for (int q = 0; q < 7; ++q) red[w][q][lane] = s[q];
-    __syncthreads();
-    if (w == 0 && k < n_i) {
-#pragma unroll
-        for (int q = 0; q < 7; ++q) {
-            double t = red[0][q][lane];
-#pragma unroll
-            for (int ww = 1; ww < W; ++ww) t += red[ww][q][lane];
-            s[q] = t;
+            for (int u = 0; u < 8; ++u) s += v[u];
         }
-        acc[3 * k + 0] = s[0]; acc[3 * k + 1] = s[1]; acc[3 * k + 2] = s[2];
-        jerk[3 * k + 0] = s[3]; jerk[3 * k + 1] = s[4]; jerk[3 * k + 2] = s[5];
-        pot[k] = -s[6];
-        const int32_t c = cnt[k];
+        red[w][lane] = s;
+        __syncthreads();
+        if (w == 0 && k < n_i) {
+            double t = red[0][lane];
+#pragma unroll
+            for (int ww = 1; ww < W; ++ww) t += red[ww][lane];
+            if (q < 3) acc[3 * k + q] = t;
+            else if (q < 6) jerk[3 * k + q - 3] = t;
+            else pot[k] = -t;
+        }
+        return;
+    }
+    const int r = (blockIdx.y - 7) * sortW + w;                  // row of this 32-row chunk
+    const int k = blockIdx.x * 32 + r;
+    if (w >= sortW || r >= 32 || k >= n_i) return;
+    int c = 0;
+    if (lane == 0) {
+        c = cnt[k];
         nnb[k] = c;
         overflow[k] = c > cap ? 1 : 0;
         cnt[k] = 0;     // keep the counters zero between calls
+    }
+    c = min(__shfl_sync(0xffffffffu, c, 0), cap);
+    if (c < 2 || !nblist || sortP == 0) return;
+    int Pk = 32;
+    while (Pk < c) Pk <<= 1;                                     // this row's power of two (<= sortP)
+    int32_t *b = sbuf + (size_t)w * sortP;
+    int32_t *row = nblist + (int64_t)k * cap;
+    for (int e = lane; e < Pk; e += 32) b[e] = e < c ? row[e] : 0x7fffffff;
+    __syncwarp();
+    for (int size = 2; size <= Pk; size <<= 1) {
+        for (int stride = size >> 1; stride > 0; stride >>= 1) {
+            for (int e = lane; e < (Pk >> 1); e += 32) {
+                const int lo = 2 * e - (e & (stride - 1));       // index with bit `stride` clear
+                const int hi = lo + stride;
+                const bool up = (lo & size) == 0;
+                const int32_t x = b[lo], y = b[hi];
+                if ((x > y) == up) { b[lo] = y; b[hi] = x; }
+            }
+            __syncwarp();
+        }
+    }
+    for (int e = lane; e < c; e += 32) row[e] = b[e];
+}
+
+// ------------------------------------------------------------------ NEXT-2: neighbour (irregular) force
+// For each active i: predict i and every listed neighbour j to time t from the FP64 j-state ("predict
+// all neighbours and do the force calculation within one loop") and sum the neighbour forces
+// ("the irregular force accumulates only the neighbor forces"), all in FP64.  One warp per i;
+// lanes stride over the list row (one 128 B line of the AoS copy per neighbour: gather-bound); the
+// seven sums are reduced with a fixed xor-shuffle tree.
+struct BodyD { double m, x[3], v[3]; };
+__device__ __forceinline__ BodyD predict_body(const double *__restrict__ aos, int32_t j, double t) {
+    const double2 *p = reinterpret_cast<const double2 *>(aos + (int64_t)j * AOS_D);
+    const double2 q0 = p[0], q1 = p[1], q2 = p[2], q3 = p[3], q4 = p[4], q5 = p[5], q6 = p[6];
+    const double x[3] = {q0.y, q1.x, q1.y}, v[3] = {q2.x, q2.y, q3.x}, a[3] = {q3.y, q4.x, q4.y};
+    const double jk[3] = {q5.x, q5.y, q6.x};
+    const double dt = t - q6.y, c2 = taylor_c2(dt), c3 = taylor_c3(dt);
+    BodyD b;
+    b.m = q0.x;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) predict_component(x[c], v[c], a[c], jk[c], dt, c2, c3, b.x[c], b.v[c]);
+    return b;
+}
+
+__global__ void __launch_bounds__(256) irregular_kernel(int32_t n_i, int32_t cap, double t,
+                                                        const int32_t *__restrict__ idx_i,
+                                                        const int32_t *__restrict__ nnb,
+                                                        const int32_t *__restrict__ nblist,
+                                                        const double *__restrict__ aos, double *__restrict__ acc,
+                                                        double *__restrict__ jerk, double *__restrict__ pot) {
+    const int lane = threadIdx.x & 31;
+    const int k = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    if (k >= n_i) return;
+    const int32_t i = idx_i[k];
+    const BodyD I = predict_body(aos, i, t);
+    const int cnt = min(nnb[k], cap);
+    const int32_t *row = nblist + (int64_t)k * cap;
+    double s[7];
+#pragma unroll
+    for (int q = 0; q < 7; ++q) s[q] = 0.0;
+    for (int e = lane; e < cnt; e += 32) {
+        const int32_t j = row[e];
+        if (j == i) continue;                                    // a list never holds its owner; be safe
+        const BodyD J = predict_body(aos, j, t);
+        const double dx = J.x[0] - I.x[0], dy = J.x[1] - I.x[1], dz = J.x[2] - I.x[2];
+        const double dvx = J.v[0] - I.v[0], dvy = J.v[1] - I.v[1], dvz = J.v[2] - I.v[2];
+        const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+        const double rv = fma(dz, dvz, fma(dy, dvy, dx * dvx));
+        const double rinv = rsqrt(r2);
+        const double rinv2 = rinv * rinv;
+        const double mrinv = J.m * rinv;
+        const double mrinv3 = mrinv * rinv2;
+        const double alpha = -3.0 * rv * rinv2;
+        s[0] = fma(mrinv3, dx, s[0]); s[1] = fma(mrinv3, dy, s[1]); s[2] = fma(mrinv3, dz, s[2]);
+        s[3] = fma(mrinv3, fma(alpha, dx, dvx), s[3]);
+        s[4] = fma(mrinv3, fma(alpha, dy, dvy), s[4]);
+        s[5] = fma(mrinv3, fma(alpha, dz, dvz), s[5]);
+        s[6] -= mrinv;
+    }
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1)
+#pragma unroll
+        for (int q = 0; q < 7; ++q) s[q] += __shfl_xor_sync(0xffffffffu, s[q], off);
+    if (lane == 0) {
+        acc[3 * k + 0] = s[0]; acc[3 * k + 1] = s[1]; acc[3 * k + 2] = s[2];
+        jerk[3 * k + 0] = s[3]; jerk[3 * k + 1] = s[4]; jerk[3 * k + 2] = s[5];
+        if (pot) pot[k] = s[6];
     }
 }
 

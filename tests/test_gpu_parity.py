@@ -392,3 +392,99 @@ def test_regular_all_equals_identity_block_and_energy(oracle):
     assert abs(W - W_orc) < 1e-6 * abs(W_orc)
     W_plummer = -3.0 * np.pi / 32.0 / cfg["a_plummer"]
     assert abs(W / W_plummer - 1.0) < 0.1        # Kroupa masses: scatter dominated by the few heavy stars
+
+
+def test_list_rows_sorted_and_bitwise_reproducible(oracle):
+    """Rows come back in ascending order (= the oracle's rows, entry by entry, away from band pairs)
+    and the whole output is identical run to run."""
+    cfg = nbgen.make_config(2, N=30000, n_i=777)
+    ctx = open_ctx(cfg)
+    a = gpu_regular(ctx, cfg["idx_i"], cfg["h2_i"])
+    b = gpu_regular(ctx, cfg["idx_i"], cfg["h2_i"])
+    xp, vp = oracle.predict(cfg["x0"], cfg["v0"], cfg["a0"], cfg["j0"], cfg["t0"], cfg["t"])
+    ref = oracle.regular(cfg["m"], xp, vp, cfg["idx_i"], cfg["h2_i"], cfg["cap"])
+    same = 0
+    for k in range(777):
+        c = min(a["nnb"][k], cfg["cap"])
+        assert np.all(np.diff(a["nblist"][k, :c]) > 0)
+        if a["nnb"][k] <= cfg["cap"]:
+            assert np.array_equal(a["nblist"][k, :c], b["nblist"][k, :c])
+            same += int(a["nnb"][k] == ref["nnb"][k] and np.array_equal(a["nblist"][k, :c], ref["nblist"][k, :c]))
+    assert same >= 770                                  # all rows but the few holding a flipped band pair
+    ctx4 = open_ctx(cfg, cap=4096)                      # long rows: 16 KB of shared memory per warp
+    h2 = cfg["h2_i"] * 9.0
+    g = gpu_regular(ctx4, cfg["idx_i"], h2)
+    assert g["nnb"].max() > 1024
+    for k in range(0, 777, 7):
+        c = min(g["nnb"][k], 4096)
+        assert np.all(np.diff(g["nblist"][k, :c]) > 0)
+
+
+# ----------------------------------------------------------------------------- NEXT-2 / NEXT-3
+
+def test_irregular_force_matches_oracle_and_completes_the_total(oracle):
+    """nb_irregular on the lists nb_regular wrote: FP64 parity with the oracle on the SAME
+    lists at the block time and at an intermediate (irregular-step) time, and regular + irregular =
+    total direct force within the regular kernel's tolerances."""
+    cfg = nbgen.make_config(3, N=40000, n_i=1500)
+    ctx = open_ctx(cfg)
+    idx, h2 = cfg["idx_i"], cfg["h2_i"]
+    reg = ctx.regular_alloc(_dev(idx, torch.int32), _dev(h2))
+    n = idx.size
+    out = dict(acc=torch.empty((n, 3), dtype=torch.float64, device="cuda"),
+               jerk=torch.empty((n, 3), dtype=torch.float64, device="cuda"),
+               pot=torch.empty(n, dtype=torch.float64, device="cuda"))
+    st = [cfg[k] for k in ("m", "x0", "v0", "a0", "j0", "t0")]
+    lst, nnb = reg["nblist"].cpu().numpy(), reg["nnb"].cpu().numpy()
+    for t in (cfg["t"], cfg["t"] + 2.0 ** -12):
+        ctx.irregular(t, _dev(idx, torch.int32), reg["nnb"], reg["nblist"], **out)
+        ctx.synchronize()
+        ref = oracle.irregular(*st, t, idx, nnb, lst, cfg["cap"])
+        for key, tol in (("acc", 1e-12), ("jerk", 1e-11), ("pot", 1e-12)):
+            g = out[key].cpu().numpy().reshape(n, -1); r = ref[key].reshape(n, -1)
+            sc = np.linalg.norm(r, axis=1)
+            assert np.max(np.linalg.norm(g - r, axis=1) / np.where(sc > 0, sc, 1.0)) < tol, key
+    # at the block time: regular (FP32 pair math) + irregular (FP64) = total of the oracle
+    ctx.irregular(cfg["t"], _dev(idx, torch.int32), reg["nnb"], reg["nblist"], **out)
+    ctx.synchronize()
+    xp, vp = oracle.predict(*st[1:], cfg["t"])
+    tot = oracle.regular(cfg["m"], xp, vp, idx, np.zeros(n), cfg["cap"], want_list=False)
+    assert int(reg["overflow"].sum()) == 0
+    for key, tol in (("acc", 1e-5), ("jerk", 1e-4), ("pot", 1e-6)):
+        g = (reg[key] + out[key]).cpu().numpy().reshape(n, -1); r = tot[key].reshape(n, -1)
+        assert np.max(np.linalg.norm(g - r, axis=1) / np.linalg.norm(r, axis=1)) < tol, key
+    # pot = NULL is allowed; an empty list gives exact zeros
+    z = torch.zeros(n, dtype=torch.int32, device="cuda")
+    ctx.irregular(cfg["t"], _dev(idx, torch.int32), z, reg["nblist"], out["acc"], out["jerk"], None)
+    ctx.synchronize()
+    assert not out["acc"].any() and not out["jerk"].any()
+
+
+def test_update_j_equals_full_set_j(oracle):
+    """nb_update_j (incremental Send.R): replacing a subset gives bit-identical results to a full
+    nb_set_j of the merged state; the predicted records are marked stale."""
+    import paper_1504_03687_b200 as nb
+    from paper_1504_03687_b200 import NbregError
+    cfg = nbgen.make_config(2, N=12000, n_i=300)
+    rng = np.random.default_rng(2)
+    sub = np.sort(rng.choice(cfg["N"], 999, replace=False)).astype(np.int32)
+    new = {k: cfg[k].copy() for k in ("m", "x0", "v0", "a0", "j0", "t0")}
+    for k in ("x0", "v0", "a0", "j0"):
+        new[k][sub] += rng.normal(size=(999, 3)) * 1e-3
+    new["t0"][sub] = cfg["t"] - 2.0 ** -9
+    new["m"][sub] *= 1.01
+    ctx = open_ctx(cfg)
+    ctx.update_j(_dev(sub, torch.int32), *(_dev(new[k][sub]) for k in ("m", "x0", "v0", "a0", "j0", "t0")))
+    with pytest.raises(NbregError) as e:
+        ctx.regular_alloc(_dev(cfg["idx_i"], torch.int32), _dev(cfg["h2_i"]))
+    assert e.value.code == nb.NB_ESTATE
+    ctx.predict_all(cfg["t"])
+    a = gpu_regular(ctx, cfg["idx_i"], cfg["h2_i"])
+    cfg2 = dict(cfg); cfg2.update(new)
+    ctx2 = open_ctx(cfg2)
+    b = gpu_regular(ctx2, cfg["idx_i"], cfg["h2_i"])
+    for key in ("acc", "jerk", "pot", "nnb", "overflow"):
+        assert np.array_equal(a[key], b[key]), key
+    fits = a["nnb"] <= cfg["cap"]
+    assert np.array_equal(a["nblist"][fits], b["nblist"][fits])
+    check(oracle, ctx, cfg2)
