@@ -43,6 +43,7 @@ def parse():
     ap.add_argument("--n-i", type=int, default=8192, help="active-block size per GPU")
     ap.add_argument("--N", type=int, default=1048576, help="override N (debug only; the metric is N=1M)")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--variant", type=int, default=-1, help="force a force-kernel variant (tuning experiments)")
     ap.add_argument("--no-sweep", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -224,6 +225,8 @@ def run_b200(args):
                nblist=torch.empty((n_i, cap), dtype=torch.int32, device=dev),
                overflow=torch.empty(n_i, dtype=torch.int32, device=dev))
     t_pred = float(cfg["t"])
+    if args.variant >= 0:
+        ctx.tune("force_variant", args.variant)
 
     def step():
         ctx.set_j(*jstate)              # a1

@@ -24,7 +24,10 @@ struct Variant {
 };
 constexpr int NVARIANT = 4;
 constexpr int NAUTO = 4;        // variants the planner picks from; the rest only by NB_TUNE_FORCE_VARIANT
-constexpr size_t FORCE_SMEM = (size_t)NSTAGE * TILE_FLOATS * sizeof(float) + NSTAGE * sizeof(uint64_t) + 64;
+constexpr size_t force_smem(int threads) {      // tile ring + FP64 sums + mbarriers + counters
+    return (size_t)NSTAGE * TILE_FLOATS * sizeof(float) + (size_t)14 * threads * sizeof(double) +
+           NSTAGE * sizeof(uint64_t) + 64;
+}
 
 }  // namespace
 
@@ -73,20 +76,20 @@ namespace {
 
 template <int WI, int WJ, int MINB>
 cudaError_t setup_variant(Variant &v, double ovh) {
-    static_assert(WJ == 1 || (size_t)WJ * 7 * 64 * WI * sizeof(double) <= FORCE_SMEM, "WJ reduction reuses the ring");
+    static_assert(WJ == 1 || (size_t)WJ * 7 * 64 * WI * sizeof(double) <= force_smem(32 * WI * WJ), "WJ reduction reuses the ring");
     v.it = 2; v.wi = WI; v.wj = WJ; v.iblock = 64 * WI; v.threads = 32 * WI * WJ; v.ovh_tiles = ovh;
     auto k = force_kernel<WI, WJ, MINB>;
-    cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FORCE_SMEM);
+    cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)force_smem(32 * WI * WJ));
     if (e != cudaSuccess) return e;
     int nb = 0;
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k, v.threads, FORCE_SMEM);
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k, v.threads, force_smem(32 * WI * WJ));
     v.ctas_per_sm = std::max(nb, 1);
     return e;
 }
 
 template <int WI, int WJ, int MINB>
 void launch_force(const Variant &v, dim3 grid, cudaStream_t st, const ForceParams &p) {
-    force_kernel<WI, WJ, MINB><<<grid, v.threads, FORCE_SMEM, st>>>(p);
+    force_kernel<WI, WJ, MINB><<<grid, v.threads, force_smem(32 * WI * WJ), st>>>(p);
 }
 
 // Pick the kernel variant: least padded work, then the larger i-block (more reuse of each j load).

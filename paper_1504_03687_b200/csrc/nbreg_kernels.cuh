@@ -22,7 +22,14 @@ namespace nbreg {
 
 constexpr int TJ = 256;        // j-particles per shared-memory tile
 constexpr int RECF = 10;       // floats per predicted record (40 B)
-constexpr int NSTAGE = 4;      // tiles in flight per CTA (bulk-copy ring)
+#ifndef NBREG_NSTAGE
+#define NBREG_NSTAGE 4
+#endif
+#ifndef NBREG_GROUP_UNROLL
+#define NBREG_GROUP_UNROLL 2
+#endif
+constexpr int NSTAGE = NBREG_NSTAGE;   // tiles in flight per CTA (bulk-copy ring)
+constexpr int GROUP_UNROLL = NBREG_GROUP_UNROLL;   // j-groups per iteration of the inner loop
 constexpr int TILE_FLOATS = TJ * RECF;
 enum { C_XH = 0, C_YH, C_ZH, C_XL, C_YL, C_ZL, C_VX, C_VY, C_VZ, C_M };   // component rows of a tile
 constexpr int UNROLL_J = 4;    // j's per neighbour-detection group
@@ -271,7 +278,11 @@ __global__ void __launch_bounds__(32 * WI *WJ, MINB) force_kernel(const ForcePar
 
     extern __shared__ __align__(128) unsigned char smem_raw[];
     float *srec = reinterpret_cast<float *>(smem_raw);                         // [NSTAGE][RECF][TJ]
-    uint64_t *full = reinterpret_cast<uint64_t *>(smem_raw + (size_t)NSTAGE * TILE_BYTES);
+    // FP64 running sums live in shared memory ([14][threads], touched once per flush): 28 registers
+    // per thread go to the pair arithmetic instead.
+    double *acc64 = reinterpret_cast<double *>(smem_raw + (size_t)NSTAGE * TILE_BYTES) + threadIdx.x;
+    constexpr int NT = 32 * WI * WJ;
+    uint64_t *full = reinterpret_cast<uint64_t *>(smem_raw + (size_t)NSTAGE * TILE_BYTES + (size_t)14 * NT * sizeof(double));
     int *done = reinterpret_cast<int *>(full + NSTAGE);                        // warps finished with a stage
 
     const int tid = threadIdx.x;
@@ -330,11 +341,8 @@ __global__ void __launch_bounds__(32 * WI *WJ, MINB) force_kernel(const ForcePar
         for (int s = 0; s < NSTAGE && s < ntile; ++s) issue(tile_begin + s, s);
     }
 
-    double acc64[2][7];
 #pragma unroll
-    for (int h = 0; h < 2; ++h)
-#pragma unroll
-        for (int c = 0; c < 7; ++c) acc64[h][c] = 0.0;
+    for (int c = 0; c < 14; ++c) acc64[c * NT] = 0.0;          // slot h * 7 + c of this thread
 
     Acc7 A;                   // FP32 partial sums of at most TJ pair terms (WJ tile shares of SUB j each)
     A.ax = A.ay = A.az = A.jx = A.jy = A.jz = A.ph = make_float2(0.f, 0.f);
@@ -345,7 +353,7 @@ __global__ void __launch_bounds__(32 * WI *WJ, MINB) force_kernel(const ForcePar
         const float *tsub = srec + (size_t)s * TILE_FLOATS + wj * SUB;      // &tile[0][wj * SUB]
         const int32_t jbase = (tile_begin + it) * TJ + wj * SUB;
 
-#pragma unroll 2
+#pragma unroll GROUP_UNROLL
         for (int g = 0; g < SUB; g += UNROLL_J) {
             float4 c4[RECF];                                   // component rows of 4 consecutive j
 #pragma unroll
@@ -388,13 +396,12 @@ __global__ void __launch_bounds__(32 * WI *WJ, MINB) force_kernel(const ForcePar
         }
         // flush: FP32 partial sums of <= WJ * SUB = TJ terms go into the FP64 running sums
         if ((it + 1) % WJ == 0 || it + 1 == ntile) {
-            acc64[0][0] += (double)A.ax.x; acc64[1][0] += (double)A.ax.y;
-            acc64[0][1] += (double)A.ay.x; acc64[1][1] += (double)A.ay.y;
-            acc64[0][2] += (double)A.az.x; acc64[1][2] += (double)A.az.y;
-            acc64[0][3] += (double)A.jx.x; acc64[1][3] += (double)A.jx.y;
-            acc64[0][4] += (double)A.jy.x; acc64[1][4] += (double)A.jy.y;
-            acc64[0][5] += (double)A.jz.x; acc64[1][5] += (double)A.jz.y;
-            acc64[0][6] += (double)A.ph.x; acc64[1][6] += (double)A.ph.y;
+            const float2 *Av = &A.ax;       // ax, ay, az, jx, jy, jz, ph
+#pragma unroll
+            for (int c = 0; c < 7; ++c) {
+                acc64[c * NT] += (double)Av[c].x;
+                acc64[(7 + c) * NT] += (double)Av[c].y;
+            }
             A.ax = A.ay = A.az = A.jx = A.jy = A.jz = A.ph = make_float2(0.f, 0.f);
         }
 
@@ -415,6 +422,11 @@ __global__ void __launch_bounds__(32 * WI *WJ, MINB) force_kernel(const ForcePar
     }
 
     // ---- a6: fixed-order reduction over the WJ warps that shared these i, then one partial per split
+    double out64[2][7];
+#pragma unroll
+    for (int h = 0; h < 2; ++h)
+#pragma unroll
+        for (int c = 0; c < 7; ++c) out64[h][c] = acc64[(h * 7 + c) * NT];
     if constexpr (WJ > 1) {
         double *red = reinterpret_cast<double *>(smem_raw);     // reuse the tile ring: [WJ][7][IB]
         __syncthreads();                                         // every warp is out of the ring
@@ -422,7 +434,7 @@ __global__ void __launch_bounds__(32 * WI *WJ, MINB) force_kernel(const ForcePar
         for (int h = 0; h < 2; ++h) {
             const int il = wi * 64 + h * 32 + lane;
 #pragma unroll
-            for (int c = 0; c < 7; ++c) red[((size_t)wj * 7 + c) * IB + il] = acc64[h][c];
+            for (int c = 0; c < 7; ++c) red[((size_t)wj * 7 + c) * IB + il] = out64[h][c];
         }
         __syncthreads();
         if (wj == 0) {
@@ -431,9 +443,9 @@ __global__ void __launch_bounds__(32 * WI *WJ, MINB) force_kernel(const ForcePar
                 const int il = wi * 64 + h * 32 + lane;
 #pragma unroll
                 for (int c = 0; c < 7; ++c) {
-                    double ssum = acc64[h][c];
+                    double ssum = out64[h][c];
                     for (int w = 1; w < WJ; ++w) ssum += red[((size_t)w * 7 + c) * IB + il];
-                    acc64[h][c] = ssum;
+                    out64[h][c] = ssum;
                 }
             }
         }
@@ -443,7 +455,7 @@ __global__ void __launch_bounds__(32 * WI *WJ, MINB) force_kernel(const ForcePar
         for (int h = 0; h < 2; ++h) {
             const int k = my_k[h];    // k < n_i_pad always
 #pragma unroll
-            for (int c = 0; c < 7; ++c) p.partial[((size_t)blockIdx.y * 7 + c) * p.n_i_pad + k] = acc64[h][c];
+            for (int c = 0; c < 7; ++c) p.partial[((size_t)blockIdx.y * 7 + c) * p.n_i_pad + k] = out64[h][c];
         }
     }
 }
