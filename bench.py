@@ -280,31 +280,46 @@ def run_b200(args):
                     nblist=torch.empty((n_i, cap), dtype=torch.int32).pin_memory(),
                     overflow=torch.empty(n_i, dtype=torch.int32).pin_memory())
 
-        def step_host():
+        def step_host():        # one C-ABI call: chunked H2D behind the force launches, results in host memory
+            ctx.step_host(*hj, t_pred, hidx, hh2, **hout)
+
+        def step_host_separate():   # the same step as three calls, nothing overlapped (context for the number above)
             ctx.set_j_host(*hj)
             ctx.predict_all(t_pred)
-            ctx.regular_host(hidx, hh2, **hout)     # returns with results in host memory
+            ctx.regular_host(hidx, hh2, **hout)
+
+        def time_host(fn, ke):
+            for _ in range(2):
+                fn()
+            barrier(); torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            e0.record(stream)
+            for _ in range(ke):
+                fn()
+            e1.record(stream)
+            torch.cuda.synchronize(); barrier()
+            wall = time.perf_counter() - t0
+            ms_e = max(e0.elapsed_time(e1), wall * 1e3)     # host-blocking calls: wall clock bounds it
+            if world > 1:
+                t = torch.tensor([ms_e], dtype=torch.float64, device=dev)
+                dist.all_reduce(t, op=dist.ReduceOp.MAX)
+                ms_e = float(t.item())
+            return ms_e
 
         ke = max(3, min(args.steps, 10))
-        for _ in range(2):
-            step_host()
-        barrier(); torch.cuda.synchronize()
-        t0 = time.perf_counter()
-        e0.record(stream)
-        for _ in range(ke):
-            step_host()
-        e1.record(stream)
-        torch.cuda.synchronize(); barrier()
-        wall = time.perf_counter() - t0
-        ms_e = max(e0.elapsed_time(e1), wall * 1e3)     # host-blocking copies: wall clock bounds it
-        if world > 1:
-            t = torch.tensor([ms_e], dtype=torch.float64, device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms_e = float(t.item())
-        h2d = 14 * N * 8 + n_i * (4 + 8)
-        d2h = n_i * (7 * 8 + 4 + 4) + n_i * cap * 4
+        l0 = ctx.info("kernel_launches")
+        ms_e = time_host(step_host, ke)
+        e2e_launches = (ctx.info("kernel_launches") - l0) // (ke + 2)
+        ms_sep = time_host(step_host_separate, ke)
+        h2d = 14 * N * 8 + n_i * (4 + 8) + 14 * n_i * 8
+        maxc = int(hout["nnb"].clamp(max=cap).max())        # list columns copied back: those some row uses
+        d2h = n_i * (7 * 8 + 4 + 4) + n_i * maxc * 4
         e2e = {"value": pairs_per_step * ke / (ms_e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
-               "d2h_bytes_per_step": d2h, "steps": ke, "ms_per_step": ms_e / ke,
+               "d2h_bytes_per_step": d2h, "list_columns_copied": maxc, "steps": ke, "ms_per_step": ms_e / ke,
+               "call": "nb_step_host (j-state sent in 5 chunks on a copy stream, force launches behind them)",
+               "gpu_launches_per_step": int(e2e_launches),
+               "separate_calls": {"value": pairs_per_step * ke / (ms_sep * 1e-3), "ms_per_step": ms_sep / ke,
+                                  "call": "nb_set_j_host + nb_predict_all + nb_regular_host"},
                "checksum_pot": float(hout["pot"].sum())}
 
     if rank != 0:

@@ -122,6 +122,23 @@ int nb_regular_all(nb_ctx *ctx, const double *h2, double *acc, double *jerk, dou
 int nb_regular_host(nb_ctx *ctx, int32_t n_i, const int32_t *idx_i, const double *h2_i, double *acc,
                     double *jerk, double *pot, int32_t *nnb, int32_t *nblist, int32_t *overflow);
 
+/* One whole block step a1-a7 through HOST buffers, pipelined: equivalent to
+ *     nb_set_j_host(m .. t0);  nb_predict_all(t);  nb_regular_host(n_i .. overflow)
+ * (Table 1: Send.R, Pred., Reg. of one regular block), but the j-state is sent in chunks
+ * (1/16, 1/16, 1/8, 1/4, 1/2 of the bodies) on a second stream, each chunk is re-laid out and
+ * predicted as it lands, and the force kernel runs chunk by chunk behind the copies, so that only
+ * the first chunk's transfer is exposed.  The active particles' own records (a3) come from their
+ * state gathered on the host (14 doubles each) and predicted with the same arithmetic, so they are
+ * bitwise the records of bodies idx_i[k].  Results equal those of the three separate calls except
+ * for the order in which the per-chunk partial sums are added (FP64, fixed and reproducible); neighbour
+ * lists, counts and flags are identical.  Leaves the context as after set_j + predict_all(t).
+ * idx_i is range-checked here (NB_EINVAL).  HOST pointers (pinned memory makes the copies
+ * asynchronous); nblist may be NULL to skip the list copy-back.  Returns with the results in place. */
+int nb_step_host(nb_ctx *ctx, const double *m, const double *x0, const double *v0, const double *a0,
+                 const double *j0, const double *t0, double t, int32_t n_i, const int32_t *idx_i,
+                 const double *h2_i, double *acc, double *jerk, double *pot, int32_t *nnb,
+                 int32_t *nblist, int32_t *overflow);
+
 /* Neighbour ("irregular") force on the GPU ("the irregular force
  * accumulates only the neighbor forces"; "predict all neighbors and do the force calculation
  * within one loop"; the paper runs this step on AVX/SSE CPUs).  For k = 0..n_i-1, i = idx_i[k]:
@@ -150,7 +167,10 @@ enum {
                                     context's stream (ring of 256 launches); set 0: off, ring cleared */
     NB_INFO_FORCE_KERNEL_NS = 20,    /* get: summed device time of the bracketed force-kernel launches,
                                         in ns (synchronises the stream)                             */
-    NB_INFO_FORCE_KERNEL_COUNT = 21  /* get: number of bracketed launches in that sum               */
+    NB_INFO_FORCE_KERNEL_COUNT = 21, /* get: number of bracketed launches in that sum               */
+    NB_TUNE_STEP_CHUNKS = 22         /* set: number of chunks nb_step_host sends the j-state in, 1..8
+                                        (1 = no overlap; sizes 1/2^(n-1), 1/2^(n-1), then doubling);
+                                        0 = automatic (5 chunks from 524288 bodies, 3 from 131072)  */
 };
 int nb_get_info(nb_ctx *ctx, int32_t key, int64_t *value);
 int nb_set_tuning(nb_ctx *ctx, int32_t key, int64_t value);

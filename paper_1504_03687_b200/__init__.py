@@ -16,6 +16,7 @@ from .binding import (  # noqa: F401
     nb_predict_all,
     nb_regular,
     nb_regular_all,
+    nb_step_host,
     nb_update_j,
     nb_irregular,
     NB_OK, NB_EINVAL, NB_ESTATE, NB_ENOMEM, NB_ECUDA,

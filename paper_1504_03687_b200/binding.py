@@ -10,7 +10,7 @@ from .build import LIB, build_lib
 NB_OK, NB_EINVAL, NB_ESTATE, NB_ENOMEM, NB_ECUDA = 0, 1, 2, 3, 4
 INFO = dict(kernel_launches=0, last_jsplit=1, last_iblock=2, last_grid=3, sm_count=4, n_padded=5,
             force_jsplit=16, force_variant=17, last_variant=18, profile=19, force_kernel_ns=20,
-            force_kernel_count=21)
+            force_kernel_count=21, step_chunks=22)
 
 _lib = None
 _vp = ctypes.c_void_p
@@ -51,6 +51,7 @@ def load_library(build: bool = True) -> ctypes.CDLL:
     lib.nb_regular.argtypes = [_vp, i32] + [_vp] * 8
     lib.nb_regular_host.argtypes = [_vp, i32] + [_vp] * 8
     lib.nb_regular_all.argtypes = [_vp] + [_vp] * 7
+    lib.nb_step_host.argtypes = [_vp] + [_vp] * 6 + [dbl, i32] + [_vp] * 8
     lib.nb_update_j.argtypes = [_vp, i32] + [_vp] * 7
     lib.nb_irregular.argtypes = [_vp, dbl, i32] + [_vp] * 6
     lib.nb_get_info.argtypes = [_vp, i32, ctypes.POINTER(i64)]
@@ -229,6 +230,23 @@ class NbContext:
                 _host_ptr(overflow, i4, n, "overflow")]
         _check(self._lib.nb_regular_host(self._ctx, n, *args), "nb_regular_host", self._ctx)
 
+    def step_host(self, m, x0, v0, a0, j0, t0, t, idx_i, h2_i, acc, jerk, pot, nnb, nblist, overflow):
+        """nb_step_host: set_j + predict_all(t) + regular through host buffers, copies pipelined."""
+        import numpy as np
+        N, f8, i4 = self.N, np.float64, np.int32
+        n = int(idx_i.size if isinstance(idx_i, np.ndarray) else idx_i.numel())
+        jargs = [_host_ptr(m, f8, N, "m"), _host_ptr(x0, f8, 3 * N, "x0"), _host_ptr(v0, f8, 3 * N, "v0"),
+                 _host_ptr(a0, f8, 3 * N, "a0"), _host_ptr(j0, f8, 3 * N, "j0"), _host_ptr(t0, f8, N, "t0")]
+        if n == 0:
+            oargs = [_vp()] * 8
+        else:
+            oargs = [_host_ptr(idx_i, i4, n, "idx_i"), _host_ptr(h2_i, f8, n, "h2_i"),
+                     _host_ptr(acc, f8, 3 * n, "acc"), _host_ptr(jerk, f8, 3 * n, "jerk"),
+                     _host_ptr(pot, f8, n, "pot"), _host_ptr(nnb, i4, n, "nnb"),
+                     _vp() if nblist is None else _host_ptr(nblist, i4, n * self.cap, "nblist"),
+                     _host_ptr(overflow, i4, n, "overflow")]
+        _check(self._lib.nb_step_host(self._ctx, *jargs, float(t), n, *oargs), "nb_step_host", self._ctx)
+
     # -- convenience: allocate outputs with torch and run one block
     def regular_alloc(self, idx_i, h2_i):
         import torch
@@ -271,6 +289,10 @@ def nb_update_j(ctx: NbContext, idx, m, x0, v0, a0, j0, t0):
 
 def nb_irregular(ctx: NbContext, t: float, idx_i, nnb, nblist, acc, jerk, pot=None):
     ctx.irregular(t, idx_i, nnb, nblist, acc, jerk, pot)
+
+
+def nb_step_host(ctx: NbContext, m, x0, v0, a0, j0, t0, t, idx_i, h2_i, acc, jerk, pot, nnb, nblist, overflow):
+    ctx.step_host(m, x0, v0, a0, j0, t0, t, idx_i, h2_i, acc, jerk, pot, nnb, nblist, overflow)
 
 
 def nb_regular_all(ctx: NbContext, h2, acc, jerk, pot, nnb, nblist, overflow):

@@ -8,6 +8,9 @@
 #include <cmath>
 #include <cstdlib>
 #include <cstring>
+#ifdef NBREG_STEP_TIMELINE
+#include <cstdio>
+#endif
 #include <new>
 #include <unordered_map>
 
@@ -50,12 +53,19 @@ struct nb_ctx {
     int32_t *st_idx = nullptr, *st_nnb = nullptr, *st_ovf = nullptr, *st_list = nullptr;
     double *st_h2 = nullptr, *st_out = nullptr;     // st_out: acc[3n] jerk[3n] pot[n]
     int64_t st_n = 0, st_list_n = 0;
+    // pipelined HOST step (nb_step_host): copy stream, per-chunk events, the active particles' own state
+    static constexpr int MAXCHUNK = 8;
+    cudaStream_t copy_stream = nullptr, prep_stream = nullptr;   // H2D copies / re-layout + predictor of landed chunks
+    cudaEvent_t ev_enter = nullptr, ev_i = nullptr, ev_copied[MAXCHUNK] = {}, ev_chunk[MAXCHUNK] = {};
+    double *h_ist = nullptr, *d_ist = nullptr;      // [14][n_i] gathered FP64 state (pinned host / device)
+    float *irec = nullptr;                          // [RECF][n_i_pad] their predicted records
+    int64_t ist_n = 0;
     // planning / introspection
     Variant var[NVARIANT];
     int64_t launches = 0;
     int64_t last_S = 0, last_iblock = 0, last_grid = 0, last_variant = -1;
-    int64_t force_S = 0, force_variant = -1;
-    std::unordered_map<int64_t, int> plan_cache;   // (variant, i-blocks) -> S
+    int64_t force_S = 0, force_variant = -1, step_chunks = 0;
+    std::unordered_map<int64_t, int> plan_cache;   // (j-tiles, variant, i-blocks) -> S
     // optional event bracketing of the force kernel (NB_TUNE_PROFILE)
     static constexpr int PROF_RING = 256;
     bool profile = false;
@@ -106,12 +116,12 @@ int pick_variant(const nb_ctx *c, int32_t n_i) {
 }
 
 // Pick the number of j-splits S: minimise waves x (tiles per split + per-CTA overhead); among plans
-// within 1.5 % take the smallest S (less scratch, shorter final reduction).
+// within 0.3 % take the smallest S (less scratch, shorter final reduction).
 int plan_split(const nb_ctx *c, const Variant &v, int64_t n_ib, int64_t ntiles);
 
 int pick_split(nb_ctx *c, const Variant &v, int64_t n_ib, int64_t ntiles) {
     if (c->force_S > 0) return (int)std::min<int64_t>(c->force_S, ntiles);
-    const int64_t key = n_ib * NVARIANT + (&v - c->var);
+    const int64_t key = (ntiles << 32) ^ (n_ib * NVARIANT + (&v - c->var));
     auto hit = c->plan_cache.find(key);
     if (hit != c->plan_cache.end()) return hit->second;
     const int plan = plan_split(c, v, n_ib, ntiles);
@@ -133,7 +143,7 @@ int plan_split(const nb_ctx *c, const Variant &v, int64_t n_ib, int64_t ntiles) 
         const int64_t tps = (ntiles + S - 1) / S;
         const int64_t Seff = (ntiles + tps - 1) / tps;
         const int64_t waves = (n_ib * Seff + conc - 1) / conc;
-        if ((double)waves * ((double)tps + v.ovh_tiles) <= best * 1.015) return (int)Seff;
+        if ((double)waves * ((double)tps + v.ovh_tiles) <= best * 1.003) return (int)Seff;
     }
     return 1;
 }
@@ -157,23 +167,19 @@ int ensure_partial(nb_ctx *c, size_t bytes) {
     return NB_OK;
 }
 
-int regular_device(nb_ctx *c, int32_t n_i, const int32_t *idx_i, const double *h2_i, double *acc, double *jerk,
-                   double *pot, int32_t *nnb, int32_t *nblist, int32_t *overflow) {
-    const int vi = pick_variant(c, n_i);
+// One force-kernel launch over the j-tiles [tile0, tile1) split S ways, writing partial rows
+// [split0, split0 + S).
+int launch_force_range(nb_ctx *c, int vi, int32_t n_i, const int32_t *idx_i, const double *h2_i, const float *irec,
+                       int32_t *nblist, int64_t tile0, int64_t tile1, int S, int64_t split0) {
     const Variant &v = c->var[vi];
     const int64_t n_ib = (n_i + v.iblock - 1) / v.iblock;
-    const int64_t ntiles = c->Npad / TJ;
-    const int S = pick_split(c, v, n_ib, ntiles);
-    const int64_t tps = (ntiles + S - 1) / S;
-    const int64_t n_i_pad = n_ib * v.iblock;
-    int rc = ensure_partial(c, (size_t)S * 7 * n_i_pad * sizeof(double));
-    if (rc != NB_OK) return rc;
-
     ForceParams p;
     p.rec = c->rec;
     p.idx_i = idx_i; p.h2_i = h2_i;
-    p.n_i = n_i; p.n_i_pad = (int32_t)n_i_pad;
-    p.ntiles = (int32_t)ntiles; p.tiles_per_split = (int32_t)tps;
+    p.n_i = n_i; p.n_i_pad = (int32_t)(n_ib * v.iblock);
+    p.irec = irec;
+    p.tile0 = (int32_t)tile0; p.ntiles = (int32_t)tile1; p.split0 = (int32_t)split0;
+    p.tiles_per_split = (int32_t)((tile1 - tile0 + S - 1) / S);
     p.cap = c->cap; p.cnt = c->cnt; p.nblist = nblist; p.partial = c->partial;
     const dim3 grid((unsigned)n_ib, (unsigned)S);
     const int slot = (int)(c->prof_n % nb_ctx::PROF_RING);
@@ -189,24 +195,94 @@ int regular_device(nb_ctx *c, int32_t n_i, const int32_t *idx_i, const double *h
         NB_CUDA(c, cudaEventRecord(c->ev1[slot], c->stream));
         c->prof_n += 1;
     }
-    {
-        const int W = S <= 8 ? 4 : 16;
-        const size_t row_bytes = (size_t)c->sort_P * sizeof(int32_t);
-        int sortW = (int)std::min<size_t>(W, c->sort_smem_max / row_bytes);     // rows sorted per CTA
-        const int sortP = (nblist && sortW > 0) ? c->sort_P : 0;                // 0: rows stay in append order
-        sortW = std::max(sortW, 1);
-        const dim3 fgrid((unsigned)((n_i + 31) / 32), (unsigned)(7 + (32 + sortW - 1) / sortW));
-        const size_t smem = sortP ? (size_t)sortW * row_bytes : 0;
-        if (W == 4)
-            finalize_kernel<4><<<fgrid, 128, smem, c->stream>>>(n_i, (int32_t)n_i_pad, S, c->cap, sortP, sortW,
-                                                                 c->partial, c->cnt, acc, jerk, pot, nnb, nblist, overflow);
-        else
-            finalize_kernel<16><<<fgrid, 512, smem, c->stream>>>(n_i, (int32_t)n_i_pad, S, c->cap, sortP, sortW,
-                                                                  c->partial, c->cnt, acc, jerk, pot, nnb, nblist, overflow);
-        NB_CUDA(c, cudaGetLastError());
-        c->launches += 2;
+    c->launches += 1;
+    c->last_iblock = v.iblock; c->last_grid = n_ib * S; c->last_variant = vi;
+    return NB_OK;
+}
+
+// a6-a7: fixed-order sum of the S partial rows, counters, sorted list rows.
+int launch_finalize(nb_ctx *c, int32_t n_i, int64_t n_i_pad, int S, double *acc, double *jerk, double *pot,
+                    int32_t *nnb, int32_t *nblist, int32_t *overflow) {
+    const int W = S <= 8 ? 4 : 16;
+    const size_t row_bytes = (size_t)c->sort_P * sizeof(int32_t);
+    int sortW = (int)std::min<size_t>(W, c->sort_smem_max / row_bytes);     // rows sorted per CTA
+    const int sortP = (nblist && sortW > 0) ? c->sort_P : 0;                // 0: rows stay in append order
+    sortW = std::max(sortW, 1);
+    const dim3 fgrid((unsigned)((n_i + 31) / 32), (unsigned)(7 + (32 + sortW - 1) / sortW));
+    const size_t smem = sortP ? (size_t)sortW * row_bytes : 0;
+    if (W == 4)
+        finalize_kernel<4><<<fgrid, 128, smem, c->stream>>>(n_i, (int32_t)n_i_pad, S, c->cap, sortP, sortW,
+                                                             c->partial, c->cnt, acc, jerk, pot, nnb, nblist, overflow);
+    else
+        finalize_kernel<16><<<fgrid, 512, smem, c->stream>>>(n_i, (int32_t)n_i_pad, S, c->cap, sortP, sortW,
+                                                              c->partial, c->cnt, acc, jerk, pot, nnb, nblist, overflow);
+    NB_CUDA(c, cudaGetLastError());
+    c->launches += 1;
+    c->last_S = S;
+    return NB_OK;
+}
+
+int regular_device(nb_ctx *c, int32_t n_i, const int32_t *idx_i, const double *h2_i, double *acc, double *jerk,
+                   double *pot, int32_t *nnb, int32_t *nblist, int32_t *overflow) {
+    const int vi = pick_variant(c, n_i);
+    const Variant &v = c->var[vi];
+    const int64_t n_ib = (n_i + v.iblock - 1) / v.iblock;
+    const int64_t ntiles = c->Npad / TJ;
+    const int S = pick_split(c, v, n_ib, ntiles);
+    const int64_t n_i_pad = n_ib * v.iblock;
+    int rc = ensure_partial(c, (size_t)S * 7 * n_i_pad * sizeof(double));
+    if (rc != NB_OK) return rc;
+    rc = launch_force_range(c, vi, n_i, idx_i, h2_i, nullptr, nblist, 0, ntiles, S, 0);
+    if (rc != NB_OK) return rc;
+    return launch_finalize(c, n_i, n_i_pad, S, acc, jerk, pot, nnb, nblist, overflow);
+}
+
+// Device-side buffers of the HOST variants, grown on demand.
+int ensure_host_staging(nb_ctx *c, int32_t n_i, bool want_list) {
+    if (n_i > c->st_n) {
+        NB_CUDA(c, cudaStreamSynchronize(c->stream));
+        cudaFree(c->st_idx); cudaFree(c->st_nnb); cudaFree(c->st_ovf); cudaFree(c->st_h2); cudaFree(c->st_out);
+        c->st_idx = c->st_nnb = c->st_ovf = nullptr; c->st_h2 = c->st_out = nullptr; c->st_n = 0;
+        const int64_t n = std::min<int64_t>(c->N, std::max<int64_t>(n_i, 1024) * 5 / 4);
+        NB_CUDA(c, cudaMalloc(&c->st_idx, sizeof(int32_t) * n));
+        NB_CUDA(c, cudaMalloc(&c->st_nnb, sizeof(int32_t) * n));
+        NB_CUDA(c, cudaMalloc(&c->st_ovf, sizeof(int32_t) * n));
+        NB_CUDA(c, cudaMalloc(&c->st_h2, sizeof(double) * n));
+        NB_CUDA(c, cudaMalloc(&c->st_out, sizeof(double) * 7 * n));
+        c->st_n = n;
     }
-    c->last_S = S; c->last_iblock = v.iblock; c->last_grid = n_ib * S; c->last_variant = vi;
+    const int64_t need_list = want_list ? (int64_t)n_i * c->cap : 0;
+    if (need_list > c->st_list_n) {
+        NB_CUDA(c, cudaStreamSynchronize(c->stream));
+        cudaFree(c->st_list); c->st_list = nullptr; c->st_list_n = 0;
+        NB_CUDA(c, cudaMalloc(&c->st_list, sizeof(int32_t) * need_list));
+        c->st_list_n = need_list;
+    }
+    return NB_OK;
+}
+
+// Copy the staged outputs of a HOST variant back and wait for them.
+int copy_back(nb_ctx *c, int32_t n_i, double *acc, double *jerk, double *pot, int32_t *nnb, int32_t *nblist,
+              int32_t *overflow) {
+    const double *d_acc = c->st_out, *d_jerk = c->st_out + 3 * (int64_t)n_i, *d_pot = c->st_out + 6 * (int64_t)n_i;
+    NB_CUDA(c, cudaMemcpyAsync(acc, d_acc, sizeof(double) * 3 * n_i, cudaMemcpyDeviceToHost, c->stream));
+    NB_CUDA(c, cudaMemcpyAsync(jerk, d_jerk, sizeof(double) * 3 * n_i, cudaMemcpyDeviceToHost, c->stream));
+    NB_CUDA(c, cudaMemcpyAsync(pot, d_pot, sizeof(double) * n_i, cudaMemcpyDeviceToHost, c->stream));
+    NB_CUDA(c, cudaMemcpyAsync(nnb, c->st_nnb, sizeof(int32_t) * n_i, cudaMemcpyDeviceToHost, c->stream));
+    NB_CUDA(c, cudaMemcpyAsync(overflow, c->st_ovf, sizeof(int32_t) * n_i, cudaMemcpyDeviceToHost, c->stream));
+    NB_CUDA(c, cudaStreamSynchronize(c->stream));
+    if (nblist) {
+        // only the first min(nnb, cap) entries of a row are defined: copy the columns some row uses
+        // (a pitched copy of [n_i][maxc] out of [n_i][cap]; 150 of 512 columns in the headline config)
+        int32_t maxc = 0;
+        for (int32_t k = 0; k < n_i; ++k) maxc = std::max(maxc, std::min(nnb[k], c->cap));
+        if (maxc > 0) {
+            const size_t pitch = sizeof(int32_t) * (size_t)c->cap;
+            NB_CUDA(c, cudaMemcpy2DAsync(nblist, pitch, c->st_list, pitch, sizeof(int32_t) * (size_t)maxc, (size_t)n_i,
+                                         cudaMemcpyDeviceToHost, c->stream));
+            NB_CUDA(c, cudaStreamSynchronize(c->stream));
+        }
+    }
     return NB_OK;
 }
 
@@ -262,6 +338,15 @@ int nb_close(nb_ctx *c) {
     cudaFree(c->partial); cudaFree(c->stage_j);
     cudaFree(c->st_idx); cudaFree(c->st_nnb); cudaFree(c->st_ovf); cudaFree(c->st_list);
     cudaFree(c->st_h2); cudaFree(c->st_out);
+    cudaFree(c->d_ist); cudaFree(c->irec); cudaFreeHost(c->h_ist);
+    if (c->ev_enter) cudaEventDestroy(c->ev_enter);
+    if (c->ev_i) cudaEventDestroy(c->ev_i);
+    for (int q = 0; q < nb_ctx::MAXCHUNK; ++q) {
+        if (c->ev_chunk[q]) cudaEventDestroy(c->ev_chunk[q]);
+        if (c->ev_copied[q]) cudaEventDestroy(c->ev_copied[q]);
+    }
+    if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
+    if (c->prep_stream) cudaStreamDestroy(c->prep_stream);
     for (int q = 0; q < nb_ctx::PROF_RING; ++q) {
         if (c->ev0[q]) cudaEventDestroy(c->ev0[q]);
         if (c->ev1[q]) cudaEventDestroy(c->ev1[q]);
@@ -289,7 +374,7 @@ int nb_set_j(nb_ctx *c, const double *m, const double *x0, const double *v0, con
     int rc = check_live(c);
     if (rc != NB_OK) return rc;
     if (!m || !x0 || !v0 || !a0 || !j0 || !t0) return NB_EINVAL;
-    relayout_kernel<<<(unsigned)((c->N + 255) / 256), 256, 0, c->stream>>>(c->N, c->Ns, m, x0, v0, a0, j0, t0, c->soa,
+    relayout_kernel<<<(unsigned)((c->N + 255) / 256), 256, 0, c->stream>>>(0, c->N, c->Ns, m, x0, v0, a0, j0, t0, c->soa,
                                                                            c->aos);
     NB_CUDA(c, cudaGetLastError());
     c->launches += 1;
@@ -351,7 +436,7 @@ int nb_predict_all(nb_ctx *c, double t) {
     int rc = check_live(c);
     if (rc != NB_OK) return rc;
     if (!c->have_j) return NB_ESTATE;
-    predict_kernel<<<(unsigned)((c->Npad + 255) / 256), 256, 0, c->stream>>>(c->N, c->Npad, c->Ns, t, c->soa, c->rec);
+    predict_kernel<<<(unsigned)((c->Npad + 255) / 256), 256, 0, c->stream>>>(0, c->Npad, c->N, c->Ns, t, c->soa, c->rec);
     NB_CUDA(c, cudaGetLastError());
     c->launches += 1;
     c->have_pred = true;
@@ -397,40 +482,200 @@ int nb_regular_host(nb_ctx *c, int32_t n_i, const int32_t *idx_i, const double *
     if (!c->have_pred) return NB_ESTATE;
     if (n_i == 0) return NB_OK;
     if (!idx_i || !h2_i || !acc || !jerk || !pot || !nnb || !overflow) return NB_EINVAL;
-    if (n_i > c->st_n) {
-        NB_CUDA(c, cudaStreamSynchronize(c->stream));
-        cudaFree(c->st_idx); cudaFree(c->st_nnb); cudaFree(c->st_ovf); cudaFree(c->st_h2); cudaFree(c->st_out);
-        c->st_idx = c->st_nnb = c->st_ovf = nullptr; c->st_h2 = c->st_out = nullptr; c->st_n = 0;
-        const int64_t n = std::min<int64_t>(c->N, std::max<int64_t>(n_i, 1024) * 5 / 4);
-        NB_CUDA(c, cudaMalloc(&c->st_idx, sizeof(int32_t) * n));
-        NB_CUDA(c, cudaMalloc(&c->st_nnb, sizeof(int32_t) * n));
-        NB_CUDA(c, cudaMalloc(&c->st_ovf, sizeof(int32_t) * n));
-        NB_CUDA(c, cudaMalloc(&c->st_h2, sizeof(double) * n));
-        NB_CUDA(c, cudaMalloc(&c->st_out, sizeof(double) * 7 * n));
-        c->st_n = n;
-    }
-    const int64_t need_list = (int64_t)n_i * c->cap;
-    if (need_list > c->st_list_n) {
-        NB_CUDA(c, cudaStreamSynchronize(c->stream));
-        cudaFree(c->st_list); c->st_list = nullptr; c->st_list_n = 0;
-        NB_CUDA(c, cudaMalloc(&c->st_list, sizeof(int32_t) * need_list));
-        c->st_list_n = need_list;
-    }
+    rc = ensure_host_staging(c, n_i, true);
+    if (rc != NB_OK) return rc;
     double *d_acc = c->st_out, *d_jerk = c->st_out + 3 * (int64_t)n_i, *d_pot = c->st_out + 6 * (int64_t)n_i;
     NB_CUDA(c, cudaMemcpyAsync(c->st_idx, idx_i, sizeof(int32_t) * n_i, cudaMemcpyHostToDevice, c->stream));
     NB_CUDA(c, cudaMemcpyAsync(c->st_h2, h2_i, sizeof(double) * n_i, cudaMemcpyHostToDevice, c->stream));
     rc = regular_device(c, n_i, c->st_idx, c->st_h2, d_acc, d_jerk, d_pot, c->st_nnb, c->st_list, c->st_ovf);
     if (rc != NB_OK) return rc;
-    // acc, jerk, pot are contiguous in st_out but the caller's are three buffers
-    NB_CUDA(c, cudaMemcpyAsync(acc, d_acc, sizeof(double) * 3 * n_i, cudaMemcpyDeviceToHost, c->stream));
-    NB_CUDA(c, cudaMemcpyAsync(jerk, d_jerk, sizeof(double) * 3 * n_i, cudaMemcpyDeviceToHost, c->stream));
-    NB_CUDA(c, cudaMemcpyAsync(pot, d_pot, sizeof(double) * n_i, cudaMemcpyDeviceToHost, c->stream));
-    NB_CUDA(c, cudaMemcpyAsync(nnb, c->st_nnb, sizeof(int32_t) * n_i, cudaMemcpyDeviceToHost, c->stream));
-    NB_CUDA(c, cudaMemcpyAsync(overflow, c->st_ovf, sizeof(int32_t) * n_i, cudaMemcpyDeviceToHost, c->stream));
-    if (nblist)
-        NB_CUDA(c, cudaMemcpyAsync(nblist, c->st_list, sizeof(int32_t) * need_list, cudaMemcpyDeviceToHost, c->stream));
-    NB_CUDA(c, cudaStreamSynchronize(c->stream));
-    return NB_OK;
+    return copy_back(c, n_i, acc, jerk, pot, nnb, nblist, overflow);
+}
+
+int nb_step_host(nb_ctx *c, const double *m, const double *x0, const double *v0, const double *a0, const double *j0,
+                 const double *t0, double t, int32_t n_i, const int32_t *idx_i, const double *h2_i, double *acc,
+                 double *jerk, double *pot, int32_t *nnb, int32_t *nblist, int32_t *overflow) {
+    int rc = check_live(c);
+    if (rc != NB_OK) return rc;
+    if (!m || !x0 || !v0 || !a0 || !j0 || !t0) return NB_EINVAL;
+    if (n_i < 0 || n_i > c->N) return NB_EINVAL;
+    if (n_i == 0) {
+        rc = nb_set_j_host(c, m, x0, v0, a0, j0, t0);
+        if (rc == NB_OK) rc = nb_predict_all(c, t);
+        if (rc == NB_OK) rc = nb_synchronize(c);
+        return rc;
+    }
+    if (!idx_i || !h2_i || !acc || !jerk || !pot || !nnb || !overflow) return NB_EINVAL;
+    for (int32_t k = 0; k < n_i; ++k)
+        if (idx_i[k] < 0 || idx_i[k] >= c->N) return NB_EINVAL;      // the host has them in hand: checked here
+    const int64_t N = c->N;
+    if (!c->copy_stream) {
+        NB_CUDA(c, cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
+        NB_CUDA(c, cudaStreamCreateWithFlags(&c->prep_stream, cudaStreamNonBlocking));
+        NB_CUDA(c, cudaEventCreateWithFlags(&c->ev_enter, cudaEventDisableTiming));
+        NB_CUDA(c, cudaEventCreateWithFlags(&c->ev_i, cudaEventDisableTiming));
+        for (int q = 0; q < nb_ctx::MAXCHUNK; ++q) {
+            NB_CUDA(c, cudaEventCreateWithFlags(&c->ev_chunk[q], cudaEventDisableTiming));
+            NB_CUDA(c, cudaEventCreateWithFlags(&c->ev_copied[q], cudaEventDisableTiming));
+        }
+    }
+    if (!c->stage_j) NB_CUDA(c, cudaMalloc(&c->stage_j, sizeof(double) * 14 * N));
+    const int vi = pick_variant(c, n_i);
+    const Variant &v = c->var[vi];
+    const int64_t n_ib = (n_i + v.iblock - 1) / v.iblock;
+    const int64_t n_i_pad = n_ib * v.iblock;
+    rc = ensure_host_staging(c, n_i, true);
+    if (rc != NB_OK) return rc;
+    if (n_i_pad > c->ist_n) {
+        NB_CUDA(c, cudaStreamSynchronize(c->stream));
+        cudaFree(c->d_ist); cudaFree(c->irec); cudaFreeHost(c->h_ist);
+        c->d_ist = nullptr; c->irec = nullptr; c->h_ist = nullptr; c->ist_n = 0;
+        const int64_t n = std::max<int64_t>(n_i_pad, 1024) * 5 / 4;
+        NB_CUDA(c, cudaMallocHost(&c->h_ist, sizeof(double) * 14 * n));
+        NB_CUDA(c, cudaMalloc(&c->d_ist, sizeof(double) * 14 * n));
+        NB_CUDA(c, cudaMalloc(&c->irec, sizeof(float) * RECF * n));
+        c->ist_n = n;
+    }
+    // the active particles' own state must not wait for the chunk that holds it.  Pinned (mapped) host
+    // arrays are gathered by the kernel itself through the bus; pageable ones by the host into a pinned
+    // staging buffer (marshalling only: 14 doubles per active particle).
+    IStateSrc isrc = {};
+    bool zero_copy = true;
+    {
+        const void *hp[7] = {m, x0, v0, a0, j0, t0, idx_i};
+        const void *dp[7];
+        for (int q = 0; q < 7 && zero_copy; ++q) {
+            cudaPointerAttributes at;
+            if (cudaPointerGetAttributes(&at, hp[q]) != cudaSuccess) { cudaGetLastError(); zero_copy = false; break; }
+            if (at.type != cudaMemoryTypeHost || !at.devicePointer) zero_copy = false;
+            dp[q] = at.devicePointer;
+        }
+        if (zero_copy) {
+            isrc.m = (const double *)dp[0]; isrc.x0 = (const double *)dp[1]; isrc.v0 = (const double *)dp[2];
+            isrc.a0 = (const double *)dp[3]; isrc.j0 = (const double *)dp[4]; isrc.t0 = (const double *)dp[5];
+            isrc.idx_i = (const int32_t *)dp[6];
+        }
+    }
+    if (!zero_copy) {
+        double *h = c->h_ist;
+        const size_t n = (size_t)n_i;
+        for (size_t k = 0; k < n; ++k) {
+            const int64_t i = idx_i[k];
+            h[k] = m[i];
+            h[13 * n + k] = t0[i];
+            for (int q = 0; q < 3; ++q) {
+                h[(1 + q) * n + k] = x0[3 * i + q];
+                h[(4 + q) * n + k] = v0[3 * i + q];
+                h[(7 + q) * n + k] = a0[3 * i + q];
+                h[(10 + q) * n + k] = j0[3 * i + q];
+            }
+        }
+        isrc.ist = c->d_ist;
+    }
+    // chunk plan: the j-range arrives as 1/16, 1/16, 1/8, 1/4, 1/2 of the tiles (first copy short,
+    // every later copy hidden behind the force launches of the chunks before it)
+    const int64_t ntiles = c->Npad / TJ;
+    int64_t ctile[nb_ctx::MAXCHUNK + 1];
+    int nchunk = 0;
+    {
+        int L = ntiles >= 2048 ? 4 : ntiles >= 512 ? 2 : 0;
+        if (c->step_chunks > 0) L = (int)std::min<int64_t>(c->step_chunks - 1, nb_ctx::MAXCHUNK - 1);
+        while (L > 0 && (ntiles >> L) == 0) --L;
+        int64_t sz = std::max<int64_t>(ntiles >> L, 1), at = 0;
+        ctile[0] = 0;
+        while (at < ntiles) {
+            const bool last = (nchunk == L) || (at + sz >= ntiles);
+            at = last ? ntiles : at + sz;
+            ctile[++nchunk] = at;
+            if (nchunk >= 2) sz *= 2;
+        }
+    }
+    int S_c[nb_ctx::MAXCHUNK], S_total = 0;
+    for (int q = 0; q < nchunk; ++q) {
+        S_c[q] = pick_split(c, v, n_ib, ctile[q + 1] - ctile[q]);
+        S_total += S_c[q];
+    }
+    rc = ensure_partial(c, (size_t)S_total * 7 * n_i_pad * sizeof(double));
+    if (rc != NB_OK) return rc;
+
+#ifdef NBREG_STEP_TIMELINE
+    static cudaEvent_t tl[64]; static bool tl_init = false; int tln = 0; const char *tlname[64];
+    if (!tl_init) { for (auto &e : tl) cudaEventCreate(&e); tl_init = true; }
+#define TL(stream_, name_) do { tlname[tln] = name_; cudaEventRecord(tl[tln++], stream_); } while (0)
+#else
+#define TL(stream_, name_) do { } while (0)
+#endif
+    cudaStream_t cs = c->copy_stream, ps = c->prep_stream;
+    TL(c->stream, "enter");
+    NB_CUDA(c, cudaEventRecord(c->ev_enter, c->stream));          // staging buffers are free once earlier work ran
+    NB_CUDA(c, cudaStreamWaitEvent(cs, c->ev_enter, 0));
+    NB_CUDA(c, cudaStreamWaitEvent(ps, c->ev_enter, 0));
+    NB_CUDA(c, cudaMemcpyAsync(c->st_idx, idx_i, sizeof(int32_t) * n_i, cudaMemcpyHostToDevice, cs));
+    NB_CUDA(c, cudaMemcpyAsync(c->st_h2, h2_i, sizeof(double) * n_i, cudaMemcpyHostToDevice, cs));
+    if (!zero_copy)
+        NB_CUDA(c, cudaMemcpyAsync(c->d_ist, c->h_ist, sizeof(double) * 14 * n_i, cudaMemcpyHostToDevice, cs));
+    NB_CUDA(c, cudaEventRecord(c->ev_i, cs));
+    TL(cs, "i-state copied");
+    double *d = c->stage_j;
+    double *dm = d, *dx = d + N, *dv = d + 4 * N, *da = d + 7 * N, *dj = d + 10 * N, *dt0 = d + 13 * N;
+    for (int q = 0; q < nchunk; ++q) {
+        const int64_t jb = ctile[q] * TJ, je_pad = ctile[q + 1] * TJ, je = std::min<int64_t>(je_pad, N);
+        const size_t n1 = sizeof(double) * (size_t)(je - jb), n3 = 3 * n1;
+        if (je > jb) {
+            NB_CUDA(c, cudaMemcpyAsync(dm + jb, m + jb, n1, cudaMemcpyHostToDevice, cs));
+            NB_CUDA(c, cudaMemcpyAsync(dx + 3 * jb, x0 + 3 * jb, n3, cudaMemcpyHostToDevice, cs));
+            NB_CUDA(c, cudaMemcpyAsync(dv + 3 * jb, v0 + 3 * jb, n3, cudaMemcpyHostToDevice, cs));
+            NB_CUDA(c, cudaMemcpyAsync(da + 3 * jb, a0 + 3 * jb, n3, cudaMemcpyHostToDevice, cs));
+            NB_CUDA(c, cudaMemcpyAsync(dj + 3 * jb, j0 + 3 * jb, n3, cudaMemcpyHostToDevice, cs));
+            NB_CUDA(c, cudaMemcpyAsync(dt0 + jb, t0 + jb, n1, cudaMemcpyHostToDevice, cs));
+            TL(cs, "chunk copied");
+            // the kernels of a landed chunk go to their own stream: they may wait for SM slots behind the
+            // running force launch, and the next chunk's copies must not queue behind them
+            NB_CUDA(c, cudaEventRecord(c->ev_copied[q], cs));
+            NB_CUDA(c, cudaStreamWaitEvent(ps, c->ev_copied[q], 0));
+            relayout_kernel<<<(unsigned)((je - jb + 255) / 256), 256, 0, ps>>>(jb, je, c->Ns, dm, dx, dv, da, dj, dt0,
+                                                                               c->soa, c->aos);
+        }
+        predict_kernel<<<(unsigned)((je_pad - jb + 255) / 256), 256, 0, ps>>>(jb, je_pad, N, c->Ns, t, c->soa, c->rec);
+        NB_CUDA(c, cudaGetLastError());
+        NB_CUDA(c, cudaEventRecord(c->ev_chunk[q], ps));
+        TL(ps, "chunk predicted");
+        c->launches += 2;
+    }
+    c->have_j = true;
+    c->have_pred = true;
+
+    NB_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_i, 0));
+    if (zero_copy)
+        predict_i_kernel<true><<<(unsigned)((n_i + 255) / 256), 256, 0, c->stream>>>(n_i, (int32_t)n_i_pad, t, isrc, c->irec);
+    else
+        predict_i_kernel<false><<<(unsigned)((n_i + 255) / 256), 256, 0, c->stream>>>(n_i, (int32_t)n_i_pad, t, isrc, c->irec);
+    NB_CUDA(c, cudaGetLastError());
+    c->launches += 1;
+    int64_t split0 = 0;
+    for (int q = 0; q < nchunk; ++q) {
+        NB_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_chunk[q], 0));
+        TL(c->stream, "force start");
+        rc = launch_force_range(c, vi, n_i, c->st_idx, c->st_h2, c->irec, c->st_list, ctile[q], ctile[q + 1], S_c[q],
+                                split0);
+        if (rc != NB_OK) return rc;
+        TL(c->stream, "force done");
+        split0 += S_c[q];
+    }
+    double *d_acc = c->st_out, *d_jerk = c->st_out + 3 * (int64_t)n_i, *d_pot = c->st_out + 6 * (int64_t)n_i;
+    rc = launch_finalize(c, n_i, n_i_pad, S_total, d_acc, d_jerk, d_pot, c->st_nnb, c->st_list, c->st_ovf);
+    if (rc != NB_OK) return rc;
+    TL(c->stream, "finalized");
+    rc = copy_back(c, n_i, acc, jerk, pot, nnb, nblist, overflow);
+#ifdef NBREG_STEP_TIMELINE
+    for (int q = 1; q < tln; ++q) {
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, tl[0], tl[q]);
+        fprintf(stderr, "[nb_step_host] %8.3f ms  %s\n", ms, tlname[q]);
+    }
+#endif
+#undef TL
+    return rc;
 }
 
 int nb_get_info(nb_ctx *c, int32_t key, int64_t *value) {
@@ -446,6 +691,7 @@ int nb_get_info(nb_ctx *c, int32_t key, int64_t *value) {
         case NB_TUNE_FORCE_JSPLIT: *value = c->force_S; break;
         case NB_TUNE_FORCE_VARIANT: *value = c->force_variant; break;
         case NB_TUNE_PROFILE: *value = c->profile ? 1 : 0; break;
+        case NB_TUNE_STEP_CHUNKS: *value = c->step_chunks; break;
         case NB_INFO_FORCE_KERNEL_COUNT: *value = std::min<int64_t>(c->prof_n, nb_ctx::PROF_RING); break;
         case NB_INFO_FORCE_KERNEL_NS: {
             if (c->cuda_err != cudaSuccess) return NB_ECUDA;
@@ -474,6 +720,9 @@ int nb_set_tuning(nb_ctx *c, int32_t key, int64_t value) {
         case NB_TUNE_FORCE_VARIANT:
             if (value < -1 || value >= NVARIANT) return NB_EINVAL;
             c->force_variant = value; break;
+        case NB_TUNE_STEP_CHUNKS:
+            if (value < 0 || value > nb_ctx::MAXCHUNK) return NB_EINVAL;
+            c->step_chunks = value; break;
         case NB_TUNE_PROFILE:
             if (value != 0 && value != 1) return NB_EINVAL;
             if (value && !c->ev0[0]) {

@@ -102,13 +102,15 @@ __device__ __forceinline__ void store_body(int64_t j, int64_t Ns, double m, cons
     o[6] = make_double2(jk[2], t0);   o[7] = make_double2(0.0, 0.0);
 }
 
-__global__ void __launch_bounds__(256) relayout_kernel(int64_t N, int64_t Ns, const double *__restrict__ m,
+// Bodies [jbeg, jend): the pipelined HOST step (nb_step_host) re-lays chunks out as they arrive.
+__global__ void __launch_bounds__(256) relayout_kernel(int64_t jbeg, int64_t jend, int64_t Ns,
+                                                       const double *__restrict__ m,
                                                        const double *__restrict__ x0, const double *__restrict__ v0,
                                                        const double *__restrict__ a0, const double *__restrict__ j0,
                                                        const double *__restrict__ t0, double *__restrict__ soa,
                                                        double *__restrict__ aos) {
-    int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (j >= N) return;
+    int64_t j = jbeg + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= jend) return;
     double x[3], v[3], a[3], jk[3];
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
@@ -155,10 +157,11 @@ __device__ __forceinline__ void predict_component(double x, double v, double a, 
     vp = fma(jk, c2, fma(a, dt, v));
 }
 
-__global__ void __launch_bounds__(256) predict_kernel(int64_t N, int64_t Npad, int64_t Ns, double t,
+// Bodies [jbeg, jend) with jend <= Npad; j >= N are the ghost padding.
+__global__ void __launch_bounds__(256) predict_kernel(int64_t jbeg, int64_t jend, int64_t N, int64_t Ns, double t,
                                                       const double *__restrict__ soa, float *__restrict__ rec) {
-    int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (j >= Npad) return;
+    int64_t j = jbeg + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= jend) return;
     float *r = rec_slot(rec, j);
     if (j >= N) {   // ghost padding: massless, far away, never a neighbour, contributes exactly 0
         r[C_XH * TJ] = r[C_YH * TJ] = r[C_ZH * TJ] = GHOST_POS;
@@ -194,6 +197,54 @@ __global__ void __launch_bounds__(256) unpack_predicted_kernel(int64_t N, const 
     }
 }
 
+// a3 for the pipelined HOST step: the active particles' own predicted records, from their FP64
+// state, into irec[RECF][n_i_pad].  Same arithmetic
+// as predict_kernel, so irec[.][k] is bitwise the record of body idx_i[k] (reading R3: r = 0 exactly
+// for the self pair) -- without waiting for the chunk that holds body idx_i[k] to arrive.
+// AOS = false: ist is the gathered copy [14][n_i]; AOS = true: the six pointers are the caller's own
+// arrays (m[N], x0[N][3], ..., t0[N]; pinned host memory read through the bus, or device memory) and
+// the kernel gathers rows idx_i[k] itself.
+struct IStateSrc {
+    const double *ist;                                       // AOS = false
+    const double *m, *x0, *v0, *a0, *j0, *t0;                // AOS = true
+    const int32_t *idx_i;
+};
+template <bool AOS>
+__global__ void __launch_bounds__(256) predict_i_kernel(int32_t n_i, int32_t n_i_pad, double t, const IStateSrc src,
+                                                        float *__restrict__ irec) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= n_i) return;
+    double m, t0, x[3], v[3], a[3], jk[3];
+    if (AOS) {
+        const int64_t i = src.idx_i[k];
+        m = src.m[i]; t0 = src.t0[i];
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            x[c] = src.x0[3 * i + c]; v[c] = src.v0[3 * i + c]; a[c] = src.a0[3 * i + c]; jk[c] = src.j0[3 * i + c];
+        }
+    } else {
+        const double *ist = src.ist;
+        m = ist[k]; t0 = ist[(size_t)13 * n_i + k];
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            x[c] = ist[(size_t)(1 + c) * n_i + k]; v[c] = ist[(size_t)(4 + c) * n_i + k];
+            a[c] = ist[(size_t)(7 + c) * n_i + k]; jk[c] = ist[(size_t)(10 + c) * n_i + k];
+        }
+    }
+    const double dt = t - t0;
+    const double c2 = taylor_c2(dt), c3 = taylor_c3(dt);
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        double xp, vp;
+        predict_component(x[c], v[c], a[c], jk[c], dt, c2, c3, xp, vp);
+        const float hi = __double2float_rn(xp);
+        irec[(size_t)(C_XH + c) * n_i_pad + k] = hi;
+        irec[(size_t)(C_XL + c) * n_i_pad + k] = __double2float_rn(xp - (double)hi);
+        irec[(size_t)(C_VX + c) * n_i_pad + k] = __double2float_rn(vp);
+    }
+    irec[(size_t)C_M * n_i_pad + k] = __double2float_rn(m);
+}
+
 // ------------------------------------------------------------------ a3-a6: force kernel
 struct ForceParams {
     const float *rec;             // predicted records, [Npad / TJ][RECF][TJ]
@@ -201,7 +252,10 @@ struct ForceParams {
     const double *h2_i;           // [n_i]
     int32_t n_i;
     int32_t n_i_pad;              // n_i rounded up to the CTA's i-block
-    int32_t ntiles;               // Npad / TJ
+    const float *irec;            // NULL, or the active particles' own records [RECF][n_i_pad] (nb_step_host)
+    int32_t tile0;                // first j-tile of this launch (0 unless the j-range arrives in chunks)
+    int32_t ntiles;               // end of this launch's j-tile range (Npad / TJ for a whole pass)
+    int32_t split0;               // first row of `partial` this launch writes
     int32_t tiles_per_split;      // contiguous tiles per blockIdx.y
     int32_t cap;
     int32_t *cnt;                 // [>= n_i] neighbour counters, zero on entry (finalize re-zeroes)
@@ -289,7 +343,7 @@ __global__ void __launch_bounds__(32 * WI *WJ, MINB) force_kernel(const ForcePar
     const int warp = tid >> 5, lane = tid & 31;
     const int wi = warp % WI, wj = warp / WI;
 
-    const int tile_begin = blockIdx.y * p.tiles_per_split;
+    const int tile_begin = p.tile0 + blockIdx.y * p.tiles_per_split;
     const int tile_end = min(tile_begin + p.tiles_per_split, p.ntiles);
     const int ntile = max(tile_end - tile_begin, 0);
 
@@ -304,10 +358,11 @@ __global__ void __launch_bounds__(32 * WI *WJ, MINB) force_kernel(const ForcePar
             my_k[h] = k;
             if (k < p.n_i) {
                 const int32_t idx = p.idx_i ? p.idx_i[k] : k;      // NULL = identity block (full-N pass)
-                const float *r = rec_slot(p.rec, idx);
+                const float *r = p.irec ? p.irec + k : rec_slot(p.rec, idx);
+                const int64_t cs = p.irec ? p.n_i_pad : TJ;        // component stride
                 my_idx[h] = idx;
 #pragma unroll
-                for (int c = 0; c < 9; ++c) v[h][c] = -r[c * TJ];
+                for (int c = 0; c < 9; ++c) v[h][c] = -r[c * cs];
                 v[h][9] = fmaxf(__double2float_rn(p.h2_i[k]), TINY_H2);
             } else {    // padding lane: far from everything (also from the ghost j's), result discarded
                 my_idx[h] = -1;
@@ -455,7 +510,8 @@ __global__ void __launch_bounds__(32 * WI *WJ, MINB) force_kernel(const ForcePar
         for (int h = 0; h < 2; ++h) {
             const int k = my_k[h];    // k < n_i_pad always
 #pragma unroll
-            for (int c = 0; c < 7; ++c) p.partial[((size_t)blockIdx.y * 7 + c) * p.n_i_pad + k] = out64[h][c];
+            for (int c = 0; c < 7; ++c)
+                p.partial[((size_t)(p.split0 + blockIdx.y) * 7 + c) * p.n_i_pad + k] = out64[h][c];
         }
     }
 }

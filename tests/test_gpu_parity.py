@@ -275,6 +275,69 @@ def test_host_variants_equal_device_variants(oracle):
             assert set(out["nblist"][k, :out["nnb"][k]].tolist()) == set(dev["nblist"][k, :dev["nnb"][k]].tolist())
 
 
+def _host_out(n, cap):
+    return dict(acc=np.empty((n, 3)), jerk=np.empty((n, 3)), pot=np.empty(n), nnb=np.empty(n, np.int32),
+                nblist=np.full((n, cap), -1, np.int32), overflow=np.empty(n, np.int32))
+
+
+@pytest.mark.parametrize("N,n_i", [(10000, 400), (140000, 300), (600000, 320)])
+def test_step_host_pipelined_matches_oracle_and_separate_calls(oracle, N, n_i):
+    """nb_step_host (chunked copies, per-chunk force launches, host-gathered i-state) against the oracle
+    and against set_j + predict_all + regular on a second context: 1, 3 and 5 chunks, ragged last tile,
+    active particles drawn from every chunk."""
+    import paper_1504_03687_b200 as nb
+    cfg = nbgen.make_config(2, N=N, n_i=n_i)
+    cap = cfg["cap"]
+    idx = np.ascontiguousarray(cfg["idx_i"]); h2 = np.ascontiguousarray(cfg["h2_i"])
+    assert idx.min() < N // 16 and idx.max() > N // 2          # first and last chunk both hold active particles
+    jst = [np.ascontiguousarray(cfg[k]) for k in ("m", "x0", "v0", "a0", "j0", "t0")]
+    ctx = nb.nb_open(N, cap)
+    out = _host_out(n_i, cap)
+    ctx.step_host(*jst, cfg["t"], idx, h2, **out)
+    xp, vp = oracle.predict(cfg["x0"], cfg["v0"], cfg["a0"], cfg["j0"], cfg["t0"], cfg["t"])
+    ref = parity.oracle_reference(oracle, cfg["m"], xp, vp, idx, h2, cap)
+    rep = parity.compare(out, ref, cap)
+    print("step_host", N, n_i, rep, "S_total", ctx.info("last_jsplit"))
+    sep = gpu_regular(open_ctx(cfg), idx, h2)
+    for key in ("nnb", "overflow"):
+        assert np.array_equal(out[key], sep[key])
+    for k in range(n_i):
+        c = min(out["nnb"][k], cap)
+        if out["nnb"][k] <= cap:
+            assert np.array_equal(out["nblist"][k, :c], sep["nblist"][k, :c])      # sorted rows: identical
+    # same pair terms; the FP32 tile sums of the WJ > 1 variants group differently when the j-range is
+    # cut into chunks, the FP64 order differs always: agreement to FP32-sum rounding, far inside the tolerances
+    for key, tol in (("acc", 5e-7), ("jerk", 5e-7), ("pot", 5e-7)):
+        scale = np.abs(sep[key]).max()
+        assert np.abs(out[key] - sep[key]).max() <= tol * scale
+    # bitwise reproducible, and the context is left as after set_j + predict_all(t)
+    out2 = _host_out(n_i, cap)
+    ctx.step_host(*jst, cfg["t"], idx, h2, **out2)
+    for key in ("acc", "jerk", "pot", "nnb", "overflow"):
+        assert np.array_equal(out[key], out2[key])
+    again = gpu_regular(ctx, idx, h2)
+    for key in ("acc", "jerk", "pot", "nnb", "overflow"):
+        assert np.array_equal(again[key], sep[key])
+    ctx.close()
+
+
+def test_step_host_errors_and_empty_block():
+    import paper_1504_03687_b200 as nb
+    cfg = nbgen.make_config(2, N=3000, n_i=10)
+    jst = [np.ascontiguousarray(cfg[k]) for k in ("m", "x0", "v0", "a0", "j0", "t0")]
+    ctx = nb.nb_open(3000, 64)
+    out = _host_out(10, 64)
+    bad = np.ascontiguousarray(cfg["idx_i"]).copy(); bad[3] = 3000
+    with pytest.raises(nb.NbregError) as e:
+        ctx.step_host(*jst, cfg["t"], bad, np.ascontiguousarray(cfg["h2_i"]), **out)
+    assert e.value.code == nb.NB_EINVAL
+    ctx.step_host(*jst, cfg["t"], np.empty(0, np.int32), None, None, None, None, None, None, None)   # = set_j + predict
+    got = gpu_regular(ctx, cfg["idx_i"], cfg["h2_i"])
+    sep = gpu_regular(open_ctx(cfg, cap=64), cfg["idx_i"], cfg["h2_i"])
+    assert np.array_equal(got["acc"], sep["acc"]) and np.array_equal(got["nnb"], sep["nnb"])
+    ctx.close()
+
+
 # ----------------------------------------------------------------------------- full size (bench launch config)
 
 def test_full_size_million_body_sampled(oracle):
@@ -295,6 +358,34 @@ def test_full_size_million_body_sampled(oracle):
     got = gpu_regular(ctx, idx, h2)
     ref = parity.oracle_reference(oracle, cfg["m"], xp, vp, idx, h2, cfg["cap"])
     print("config4 n_i=64", parity.compare(got, ref, cfg["cap"]))
+
+
+def test_full_size_step_host_bench_configuration(oracle):
+    """The e2e leg of bench.py: nb_step_host at N = 1,048,576, n_i = 8192 with pinned host buffers; a
+    seeded sample of the active particles against the oracle, everything against the separate calls."""
+    import paper_1504_03687_b200 as nb
+    cfg = nbgen.make_config(4)
+    idx, h2 = nbgen.active_block(cfg, 8192)
+    cap, n = cfg["cap"], 8192
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    jst = [pin(np.asarray(cfg[k], dtype=np.float64)) for k in ("m", "x0", "v0", "a0", "j0", "t0")]
+    out = {k: torch.from_numpy(v).pin_memory() for k, v in _host_out(n, cap).items()}
+    ctx = nb.nb_open(cfg["N"], cap)
+    ctx.step_host(*jst, cfg["t"], pin(idx), pin(h2), **out)
+    got = {k: v.numpy() for k, v in out.items()}
+    sel = np.sort(np.random.default_rng(2).choice(n, size=128, replace=False))
+    xp, vp = oracle.predict(cfg["x0"], cfg["v0"], cfg["a0"], cfg["j0"], cfg["t0"], cfg["t"])
+    ref = parity.oracle_reference(oracle, cfg["m"], xp, vp, idx[sel], h2[sel], cap)
+    print("step_host config4 n_i=8192 sample", parity.compare({k: v[sel] for k, v in got.items()}, ref, cap),
+          "S_total", ctx.info("last_jsplit"))
+    sep = gpu_regular(ctx, idx, h2)
+    assert np.array_equal(got["nnb"], sep["nnb"]) and np.array_equal(got["overflow"], sep["overflow"])
+    fits = got["nnb"] <= cap
+    m = np.arange(cap)[None, :] < got["nnb"][:, None]
+    assert np.array_equal(got["nblist"][fits][m[fits]], sep["nblist"][fits][m[fits]])
+    for key in ("acc", "jerk", "pot"):
+        assert np.abs(got[key] - sep[key]).max() <= 1e-12 * np.abs(sep[key]).max()
+    ctx.close()
 
 
 def test_config5_full_size_king_core(oracle):
