@@ -397,12 +397,19 @@ def run_b200(args):
         ms_pred = timed(lambda: ctx.predict_all(t_pred))
         ms_setj = timed(lambda: ctx.set_j(*jstate))
         ctx.predict_all(t_pred)
+        # NEXT-3: selection over all N and the corrector for the timed block (it rewrites those bodies: last)
+        ctx.set_steps(f64(2.0 ** -np.asarray(cfg["levels"], dtype=np.float64)))
+        act = torch.empty(N, dtype=torch.int32, device=dev)
+        ms_sel = timed(lambda: ctx.next_block(act))
+        ms_cor = timed(lambda: ctx.correct(t_pred, idx, out["acc"], out["jerk"], 0.02, 2.0 ** -3))
         extras = {
             "nb_irregular": {"n_i": n_i, "neighbour_pairs": nn, "ms": ms_irr, "pairs_per_s": nn / (ms_irr * 1e-3),
                              "gather_GBps": nn * 128 / (ms_irr * 1e-3) / 1e9, "dtype": "f64"},
             "nb_update_j": {"n": n_i, "ms": ms_upd},
             "nb_predict_all": {"ms": ms_pred, "GBps": N * (112 + 40) / (ms_pred * 1e-3) / 1e9,
                                "frac_hbm": N * (112 + 40) / (ms_pred * 1e-3) / 1e9 / pk.get("hbm_gbs", 6460.0)},
+            "nb_next_block": {"N": N, "ms": ms_sel, "note": "min + count + ordered scatter + 16 B D2H + sync"},
+            "nb_correct": {"n": n_i, "ms": ms_cor},
             "nb_set_j": {"ms": ms_setj, "GBps": N * (112 + 112 + 128) / (ms_setj * 1e-3) / 1e9},
         }
 

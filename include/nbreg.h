@@ -152,6 +152,43 @@ int nb_step_host(nb_ctx *ctx, const double *m, const double *x0, const double *v
 int nb_irregular(nb_ctx *ctx, double t, int32_t n_i, const int32_t *idx_i, const int32_t *nnb,
                  const int32_t *nblist, double *acc, double *jerk, double *pot);
 
+/* ---- The steps either side of the regular-force pass: block time steps, active
+ * selection, Hermite corrector.  The paper prints none of these formulas; they are the textbook
+ * fourth-order Hermite scheme with hierarchical block steps that it names (Makino 1991,
+ * Makino & Aarseth 1992) -- DESIGN.md readings R27-R31.  All pointers DEVICE unless marked HOST. */
+
+/* Block time steps dt[N] (each an integer power of 0.5 with t0[j] a multiple of dt[j]; unchecked).
+ * Copied.  Requires nb_set_j. */
+int nb_set_steps(nb_ctx *ctx, const double *dt);
+/* Start-up steps from the stored a0, j0: dt_j = largest power of 0.5 <= min(eta_s |a0| / |j0|, dt_max). */
+int nb_init_steps(nb_ctx *ctx, double eta_s, double dt_max);
+
+/* Active selection for the next block ("active particles ... are integrated together"; P:89
+ * section 3.3.1, Figures 1-2): t_next = min_j (t0_j + dt_j) and the bodies with t0_j + dt_j == t_next,
+ * ascending, into idx_act (DEVICE, room for N).  *t_next and *n_act are HOST outputs: the call
+ * synchronises the stream.  (The paper's step-sorted list exists so that a CPU never scans N bodies;
+ * here the scan is 16 B/body of HBM traffic, ~3 us at N = 1M, and the list is not kept.) */
+int nb_next_block(nb_ctx *ctx, double *t_next, int32_t *n_act, int32_t *idx_act);
+
+/* Hermite corrector and new block step for the n active bodies idx[0..n) whose new acceleration
+ * acc1[n][3] and jerk jerk1[n][3] were evaluated at time t = t0 + dt at the predicted state (the total
+ * force: nb_regular with h2 = 0, or nb_regular + nb_irregular added by the caller).  With h = dt:
+ *     a2 = ( -6 (a0 - a1) - h (4 j0 + 2 j1) ) / h^2       a3 = ( 12 (a0 - a1) + 6 h (j0 + j1) ) / h^3
+ *     x1 = x0 + v0 h + a0 h^2/2 + j0 h^3/6 + a2 h^4/24 + a3 h^5/120
+ *     v1 = v0 + a0 h + j0 h^2/2 + a2 h^3/6 + a3 h^4/24
+ *     dt_req = sqrt( eta (|a1| |a2'| + |j1|^2) / (|j1| |a3| + |a2'|^2) ),  a2' = a2 + h a3
+ *     new step: 2 dt if dt_req >= 2 dt, 2 dt <= dt_max and t is a multiple of 2 dt; else dt halved
+ *     while it exceeds dt_req.
+ * The stored state of these bodies becomes (x1, v1, a1, j1, t0 = t, new step); the predicted records
+ * become stale (nb_regular needs a new nb_predict_all).  FP64.  idx unique, in range, unchecked. */
+int nb_correct(nb_ctx *ctx, double t, int32_t n, const int32_t *idx, const double *acc1,
+               const double *jerk1, double eta, double dt_max);
+
+/* Inspection / checkpoint: the stored FP64 state in the caller's layout: m[N], x0[N][3], v0[N][3],
+ * a0[N][3], j0[N][3], t0[N] and (optional, may be NULL) the steps dt[N]. */
+int nb_get_state(nb_ctx *ctx, double *m, double *x0, double *v0, double *a0, double *j0, double *t0,
+                 double *dt);
+
 /* Tuning / introspection.  Keys: */
 enum {
     NB_INFO_KERNEL_LAUNCHES = 0, /* get: kernels launched by this context so far                   */

@@ -54,6 +54,11 @@ def load_library(build: bool = True) -> ctypes.CDLL:
     lib.nb_step_host.argtypes = [_vp] + [_vp] * 6 + [dbl, i32] + [_vp] * 8
     lib.nb_update_j.argtypes = [_vp, i32] + [_vp] * 7
     lib.nb_irregular.argtypes = [_vp, dbl, i32] + [_vp] * 6
+    lib.nb_set_steps.argtypes = [_vp, _vp]
+    lib.nb_init_steps.argtypes = [_vp, dbl, dbl]
+    lib.nb_next_block.argtypes = [_vp, ctypes.POINTER(dbl), ctypes.POINTER(i32), _vp]
+    lib.nb_correct.argtypes = [_vp, dbl, i32, _vp, _vp, _vp, dbl, dbl]
+    lib.nb_get_state.argtypes = [_vp] + [_vp] * 7
     lib.nb_get_info.argtypes = [_vp, i32, ctypes.POINTER(i64)]
     lib.nb_set_tuning.argtypes = [_vp, i32, i64]
     lib.nb_last_cuda_error.argtypes = [_vp]
@@ -211,6 +216,43 @@ class NbContext:
                 _vp() if nblist is None else _dev_ptr(nblist, i4, n * self.cap, "nblist"),
                 _dev_ptr(overflow, i4, n, "overflow")]
         _check(self._lib.nb_regular_all(self._ctx, *args), "nb_regular_all", self._ctx)
+
+    # -- block loop
+    def set_steps(self, dt):
+        import torch
+        _check(self._lib.nb_set_steps(self._ctx, _dev_ptr(dt, torch.float64, self.N, "dt")), "nb_set_steps", self._ctx)
+
+    def init_steps(self, eta_s: float, dt_max: float):
+        _check(self._lib.nb_init_steps(self._ctx, float(eta_s), float(dt_max)), "nb_init_steps", self._ctx)
+
+    def next_block(self, idx_act):
+        """-> (t_next, n_act); idx_act (int32 CUDA tensor with room for N) receives the active indices."""
+        import torch
+        t, n = ctypes.c_double(), ctypes.c_int32()
+        _check(self._lib.nb_next_block(self._ctx, ctypes.byref(t), ctypes.byref(n),
+                                       _dev_ptr(idx_act, torch.int32, self.N, "idx_act")), "nb_next_block", self._ctx)
+        return t.value, n.value
+
+    def correct(self, t: float, idx, acc1, jerk1, eta: float, dt_max: float):
+        import torch
+        n, f8 = int(idx.numel()), torch.float64
+        if n == 0:
+            return
+        _check(self._lib.nb_correct(self._ctx, float(t), n, _dev_ptr(idx, torch.int32, n, "idx"),
+                                    _dev_ptr(acc1, f8, 3 * n, "acc1"), _dev_ptr(jerk1, f8, 3 * n, "jerk1"),
+                                    float(eta), float(dt_max)), "nb_correct", self._ctx)
+
+    def get_state(self, with_steps: bool = True):
+        import torch
+        N, kw = self.N, dict(dtype=torch.float64, device="cuda")
+        st = dict(m=torch.empty(N, **kw), x0=torch.empty((N, 3), **kw), v0=torch.empty((N, 3), **kw),
+                  a0=torch.empty((N, 3), **kw), j0=torch.empty((N, 3), **kw), t0=torch.empty(N, **kw))
+        if with_steps:
+            st["dt"] = torch.empty(N, **kw)
+        args = [_vp(st[k].data_ptr()) for k in ("m", "x0", "v0", "a0", "j0", "t0")]
+        args.append(_vp(st["dt"].data_ptr()) if with_steps else _vp())
+        _check(self._lib.nb_get_state(self._ctx, *args), "nb_get_state", self._ctx)
+        return st
 
     # -- the path (host buffers: numpy arrays or CPU tensors, pinned or not)
     def set_j_host(self, m, x0, v0, a0, j0, t0):

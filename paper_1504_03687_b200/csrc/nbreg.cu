@@ -60,6 +60,12 @@ struct nb_ctx {
     double *h_ist = nullptr, *d_ist = nullptr;      // [14][n_i] gathered FP64 state (pinned host / device)
     float *irec = nullptr;                          // [RECF][n_i_pad] their predicted records
     int64_t ist_n = 0;
+    // block loop (NEXT-3): steps, selection scratch
+    double *dtj = nullptr;                          // [N] block time steps
+    bool have_steps = false;
+    unsigned long long *sel_key = nullptr;          // min_j (t0 + dt) as an ordered integer key
+    int32_t *sel_counts = nullptr;                  // [ceil(N / SEL_CHUNK)]
+    double *sel_result = nullptr, *h_sel_result = nullptr;   // {t_next, n_active}: device / pinned host
     // planning / introspection
     Variant var[NVARIANT];
     int64_t launches = 0;
@@ -339,6 +345,8 @@ int nb_close(nb_ctx *c) {
     cudaFree(c->st_idx); cudaFree(c->st_nnb); cudaFree(c->st_ovf); cudaFree(c->st_list);
     cudaFree(c->st_h2); cudaFree(c->st_out);
     cudaFree(c->d_ist); cudaFree(c->irec); cudaFreeHost(c->h_ist);
+    cudaFree(c->dtj); cudaFree(c->sel_key); cudaFree(c->sel_counts); cudaFree(c->sel_result);
+    cudaFreeHost(c->h_sel_result);
     if (c->ev_enter) cudaEventDestroy(c->ev_enter);
     if (c->ev_i) cudaEventDestroy(c->ev_i);
     for (int q = 0; q < nb_ctx::MAXCHUNK; ++q) {
@@ -676,6 +684,86 @@ int nb_step_host(nb_ctx *c, const double *m, const double *x0, const double *v0,
 #endif
 #undef TL
     return rc;
+}
+
+int nb_set_steps(nb_ctx *c, const double *dt) {
+    int rc = check_live(c);
+    if (rc != NB_OK) return rc;
+    if (!dt) return NB_EINVAL;
+    if (!c->have_j) return NB_ESTATE;
+    if (!c->dtj) NB_CUDA(c, cudaMalloc(&c->dtj, sizeof(double) * c->N));
+    NB_CUDA(c, cudaMemcpyAsync(c->dtj, dt, sizeof(double) * c->N, cudaMemcpyDeviceToDevice, c->stream));
+    c->have_steps = true;
+    return NB_OK;
+}
+
+int nb_init_steps(nb_ctx *c, double eta_s, double dt_max) {
+    int rc = check_live(c);
+    if (rc != NB_OK) return rc;
+    if (!(eta_s > 0.0) || !(dt_max > 0.0)) return NB_EINVAL;
+    if (!c->have_j) return NB_ESTATE;
+    if (!c->dtj) NB_CUDA(c, cudaMalloc(&c->dtj, sizeof(double) * c->N));
+    init_steps_kernel<<<(unsigned)((c->N + 255) / 256), 256, 0, c->stream>>>(c->N, c->Ns, eta_s, dt_max, c->soa, c->dtj);
+    NB_CUDA(c, cudaGetLastError());
+    c->launches += 1;
+    c->have_steps = true;
+    return NB_OK;
+}
+
+int nb_next_block(nb_ctx *c, double *t_next, int32_t *n_act, int32_t *idx_act) {
+    int rc = check_live(c);
+    if (rc != NB_OK) return rc;
+    if (!t_next || !n_act || !idx_act) return NB_EINVAL;
+    if (!c->have_j || !c->have_steps) return NB_ESTATE;
+    const int64_t N = c->N;
+    const unsigned nchunk = (unsigned)((N + SEL_CHUNK - 1) / SEL_CHUNK);
+    if (!c->sel_key) {
+        NB_CUDA(c, cudaMalloc(&c->sel_key, sizeof(unsigned long long)));
+        NB_CUDA(c, cudaMalloc(&c->sel_counts, sizeof(int32_t) * nchunk));
+        NB_CUDA(c, cudaMalloc(&c->sel_result, sizeof(double) * 2));
+        NB_CUDA(c, cudaMallocHost(&c->h_sel_result, sizeof(double) * 2));
+    }
+    const double *t0 = c->soa + 13 * c->Ns;
+    NB_CUDA(c, cudaMemsetAsync(c->sel_key, 0xff, sizeof(unsigned long long), c->stream));
+    const unsigned g = (unsigned)std::min<int64_t>((N + 255) / 256, (int64_t)c->sm_count * 8);
+    next_time_kernel<<<g, 256, 0, c->stream>>>(N, t0, c->dtj, c->sel_key);
+    select_active_kernel<0><<<nchunk, 256, 0, c->stream>>>(N, t0, c->dtj, c->sel_key, c->sel_counts, idx_act, c->sel_result);
+    select_active_kernel<1><<<nchunk, 256, 0, c->stream>>>(N, t0, c->dtj, c->sel_key, c->sel_counts, idx_act, c->sel_result);
+    NB_CUDA(c, cudaGetLastError());
+    c->launches += 3;
+    NB_CUDA(c, cudaMemcpyAsync(c->h_sel_result, c->sel_result, sizeof(double) * 2, cudaMemcpyDeviceToHost, c->stream));
+    NB_CUDA(c, cudaStreamSynchronize(c->stream));
+    *t_next = c->h_sel_result[0];
+    *n_act = (int32_t)c->h_sel_result[1];
+    return NB_OK;
+}
+
+int nb_correct(nb_ctx *c, double t, int32_t n, const int32_t *idx, const double *acc1, const double *jerk1,
+               double eta, double dt_max) {
+    int rc = check_live(c);
+    if (rc != NB_OK) return rc;
+    if (n < 0 || n > c->N || !(eta > 0.0) || !(dt_max > 0.0)) return NB_EINVAL;
+    if (!c->have_j || !c->have_steps) return NB_ESTATE;
+    if (n == 0) return NB_OK;
+    if (!idx || !acc1 || !jerk1) return NB_EINVAL;
+    correct_kernel<<<(unsigned)((n + 127) / 128), 128, 0, c->stream>>>(n, c->Ns, t, eta, dt_max, idx, acc1, jerk1, c->soa,
+                                                                       c->aos, c->dtj);
+    NB_CUDA(c, cudaGetLastError());
+    c->launches += 1;
+    c->have_pred = false;
+    return NB_OK;
+}
+
+int nb_get_state(nb_ctx *c, double *m, double *x0, double *v0, double *a0, double *j0, double *t0, double *dt) {
+    int rc = check_live(c);
+    if (rc != NB_OK) return rc;
+    if (!m || !x0 || !v0 || !a0 || !j0 || !t0) return NB_EINVAL;
+    if (!c->have_j || (dt && !c->have_steps)) return NB_ESTATE;
+    export_state_kernel<<<(unsigned)((c->N + 255) / 256), 256, 0, c->stream>>>(c->N, c->Ns, c->soa, c->dtj, m, x0, v0, a0,
+                                                                              j0, t0, dt);
+    NB_CUDA(c, cudaGetLastError());
+    c->launches += 1;
+    return NB_OK;
 }
 
 int nb_get_info(nb_ctx *c, int32_t key, int64_t *value) {

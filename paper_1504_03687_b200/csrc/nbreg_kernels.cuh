@@ -663,4 +663,176 @@ __global__ void __launch_bounds__(256) irregular_kernel(int32_t n_i, int32_t cap
     }
 }
 
+// ------------------------------------------------------------------ NEXT-3: block selection, corrector, steps
+// Block selection (P:47 block time steps; section 3.3.1).  The paper keeps an index list sorted by
+// step so that a CPU never scans N particles; on this chip a scan of t0 + dt over N = 1M bodies is
+// 16 MB of HBM traffic (~3 us), so the selection is the definition itself in three small launches:
+// t_next = min_j (t0_j + dt_j); per-CTA counts of {j : t0_j + dt_j == t_next}; ordered scatter.
+constexpr int SEL_CHUNK = 2048;      // bodies per CTA of the count / scatter kernels
+__device__ __forceinline__ unsigned long long ordered_key(double x) {      // monotone map double -> uint64
+    const unsigned long long b = (unsigned long long)__double_as_longlong(x);
+    return (b >> 63) ? ~b : (b | 0x8000000000000000ull);
+}
+__device__ __forceinline__ double key_to_double(unsigned long long k) {
+    const unsigned long long b = (k >> 63) ? (k & 0x7fffffffffffffffull) : ~k;
+    return __longlong_as_double((long long)b);
+}
+
+__global__ void __launch_bounds__(256) next_time_kernel(int64_t N, const double *__restrict__ t0,
+                                                        const double *__restrict__ dtj,
+                                                        unsigned long long *__restrict__ tmin_key) {
+    unsigned long long best = ~0ull;
+    for (int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; j < N; j += (int64_t)gridDim.x * blockDim.x)
+        best = min(best, ordered_key(t0[j] + dtj[j]));
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) best = min(best, __shfl_xor_sync(0xffffffffu, best, off));
+    __shared__ unsigned long long wbest[8];
+    if ((threadIdx.x & 31) == 0) wbest[threadIdx.x >> 5] = best;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int w = 1; w < 8; ++w) best = min(best, wbest[w]);
+        atomicMin(tmin_key, best);      // integer atomic: order-independent, reproducible
+    }
+}
+
+// PASS 0: counts[b] = number of active bodies in chunk b.  PASS 1: chunk b's offset = sum of the counts
+// before it (every CTA sums them itself: <= N / 2048 integers), then an ordered ballot compaction, so
+// idx_act is ascending.  The last CTA of pass 1 also writes the total and t_next to result[0..1].
+template <int PASS>
+__global__ void __launch_bounds__(256) select_active_kernel(int64_t N, const double *__restrict__ t0,
+                                                            const double *__restrict__ dtj,
+                                                            const unsigned long long *__restrict__ tmin_key,
+                                                            int32_t *__restrict__ counts,
+                                                            int32_t *__restrict__ idx_act,
+                                                            double *__restrict__ result) {
+    const double tn = key_to_double(*tmin_key);
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    __shared__ int32_t wsum[8];
+    __shared__ int32_t base_s;
+    int32_t base = 0;
+    if (PASS == 1) {
+        int32_t part = 0;
+        for (int b = threadIdx.x; b < (int)blockIdx.x; b += 256) part += counts[b];
+#pragma unroll
+        for (int off = 16; off > 0; off >>= 1) part += __shfl_xor_sync(0xffffffffu, part, off);
+        if (lane == 0) wsum[w] = part;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            int32_t tsum = 0;
+#pragma unroll
+            for (int q = 0; q < 8; ++q) tsum += wsum[q];
+            base_s = tsum;
+        }
+        __syncthreads();
+        base = base_s;
+        __syncthreads();
+    }
+    const int64_t cbeg = (int64_t)blockIdx.x * SEL_CHUNK;
+    int32_t running = 0;                                    // active bodies of this chunk before the current slab
+    for (int s = 0; s < SEL_CHUNK; s += 256) {
+        const int64_t j = cbeg + s + threadIdx.x;
+        const bool act = j < N && (t0[j] + dtj[j] == tn);
+        const unsigned bal = __ballot_sync(0xffffffffu, act);
+        if (lane == 0) wsum[w] = __popc(bal);
+        __syncthreads();
+        int32_t before = 0, slab = 0;
+#pragma unroll
+        for (int q = 0; q < 8; ++q) {
+            const int32_t cq = wsum[q];
+            before += q < w ? cq : 0;
+            slab += cq;
+        }
+        if (PASS == 1 && act) idx_act[base + running + before + __popc(bal & ((1u << lane) - 1u))] = (int32_t)j;
+        running += slab;
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) {
+        if (PASS == 0) counts[blockIdx.x] = running;
+        if (PASS == 1 && blockIdx.x == gridDim.x - 1) {
+            result[0] = tn;
+            result[1] = (double)(base + running);
+        }
+    }
+}
+
+// Largest power of two not above x (x > 0, normal): clear the mantissa.
+__device__ __forceinline__ double pow2_floor(double x) {
+    return __longlong_as_double(__double_as_longlong(x) & 0x7ff0000000000000ll);
+}
+__device__ __forceinline__ double norm3(const double *a) { return sqrt(fma(a[2], a[2], fma(a[1], a[1], a[0] * a[0]))); }
+
+// Start-up steps (textbook: dt = eta_s |a| / |j|, quantised to a power of 0.5, <= dt_max).
+__global__ void __launch_bounds__(256) init_steps_kernel(int64_t N, int64_t Ns, double eta_s, double dt_max,
+                                                         const double *__restrict__ soa, double *__restrict__ dtj) {
+    const int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= N) return;
+    double a[3], jk[3];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) { a[c] = soa[(7 + c) * Ns + j]; jk[c] = soa[(10 + c) * Ns + j]; }
+    dtj[j] = pow2_floor(fmin(eta_s * norm3(a) / norm3(jk), dt_max));
+}
+
+// Fourth-order Hermite corrector + new block step for the n active bodies (Makino & Aarseth 1992):
+// the acceleration over the step is the cubic Hermite interpolant of (a0, j0) at t0 and (a1, j1) at
+// t1 = t0 + dt; its second and third derivatives a2, a3 extend the predictor's Taylor series by the
+// dt^4, dt^5 (x) and dt^3, dt^4 (v) terms.  New step: Aarseth's criterion with the derivatives at t1,
+// then the block rule (double once if allowed and t1 is commensurate, else halve while too long).
+// One thread per active body; reads its 128 B line of the gather copy, writes both copies.  FP64.
+__global__ void __launch_bounds__(128) correct_kernel(int32_t n, int64_t Ns, double t1, double eta, double dt_max,
+                                                      const int32_t *__restrict__ idx,
+                                                      const double *__restrict__ acc1,
+                                                      const double *__restrict__ jerk1, double *__restrict__ soa,
+                                                      double *__restrict__ aos, double *__restrict__ dtj) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= n) return;
+    const int64_t i = idx[k];
+    const double2 *p = reinterpret_cast<const double2 *>(aos + i * AOS_D);
+    const double2 q0 = p[0], q1 = p[1], q2 = p[2], q3 = p[3], q4 = p[4], q5 = p[5], q6 = p[6];
+    const double m = q0.x;
+    const double x0[3] = {q0.y, q1.x, q1.y}, v0[3] = {q2.x, q2.y, q3.x}, a0[3] = {q3.y, q4.x, q4.y};
+    const double j0[3] = {q5.x, q5.y, q6.x};
+    const double h = dtj[i];                       // = t1 - t0 for an active body
+    const double h2 = h * h, h3 = h2 * h, h4 = h2 * h2, h5 = h4 * h;
+    double x1[3], v1[3], a1[3], j1[3], a2e[3], a3[3];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        a1[c] = acc1[3 * k + c];
+        j1[c] = jerk1[3 * k + c];
+        const double da = a0[c] - a1[c];
+        const double a2 = (-6.0 * da - h * (4.0 * j0[c] + 2.0 * j1[c])) / h2;
+        a3[c] = (12.0 * da + 6.0 * h * (j0[c] + j1[c])) / h3;
+        x1[c] = x0[c] + v0[c] * h + a0[c] * h2 / 2.0 + j0[c] * h3 / 6.0 + a2 * h4 / 24.0 + a3[c] * h5 / 120.0;
+        v1[c] = v0[c] + a0[c] * h + j0[c] * h2 / 2.0 + a2 * h3 / 6.0 + a3[c] * h4 / 24.0;
+        a2e[c] = a2 + h * a3[c];                   // second derivative at the end of the step
+    }
+    const double na = norm3(a1), nj = norm3(j1), n2 = norm3(a2e), n3 = norm3(a3);
+    const double req = sqrt(eta * (na * n2 + nj * nj) / (nj * n3 + n2 * n2));
+    double d = h;
+    const double d2 = 2.0 * d, ratio = t1 / d2;
+    if (req >= d2 && d2 <= dt_max && ratio == floor(ratio)) d = d2;
+    else
+        while (d > req) d *= 0.5;
+    store_body(i, Ns, m, x1, v1, a1, j1, t1, soa, aos);
+    dtj[i] = d;
+}
+
+// Inspection: the FP64 state back in the caller's layout (tests, energy checks, checkpoints).
+__global__ void __launch_bounds__(256) export_state_kernel(int64_t N, int64_t Ns, const double *__restrict__ soa,
+                                                           const double *__restrict__ dtj, double *__restrict__ m,
+                                                           double *__restrict__ x0, double *__restrict__ v0,
+                                                           double *__restrict__ a0, double *__restrict__ j0,
+                                                           double *__restrict__ t0, double *__restrict__ dt) {
+    const int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= N) return;
+    m[j] = soa[j];
+    t0[j] = soa[13 * Ns + j];
+    if (dt) dt[j] = dtj[j];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        x0[3 * j + c] = soa[(1 + c) * Ns + j]; v0[3 * j + c] = soa[(4 + c) * Ns + j];
+        a0[3 * j + c] = soa[(7 + c) * Ns + j]; j0[3 * j + c] = soa[(10 + c) * Ns + j];
+    }
+}
+
 }  // namespace nbreg

@@ -1,0 +1,168 @@
+"""SURVEY 8(f) NEXT-3 on the GPU (block selection, Hermite corrector, block time step) against
+oracle/hermite.py, element by element on the same seeded inputs, and a closed block loop
+(select -> predict -> regular force -> correct) checked for energy conservation and against the
+oracle's own integration.  Needs a B200."""
+import numpy as np
+import pytest
+
+import nbgen
+from oracle import hermite as H
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+def _dev(a, dtype=None):
+    t = torch.from_numpy(np.ascontiguousarray(a))
+    if dtype is not None:
+        t = t.to(dtype)
+    return t.cuda()
+
+
+def _open(cfg, cap=8):
+    import paper_1504_03687_b200 as nb
+    ctx = nb.nb_open(cfg["N"], cap)
+    nb.nb_set_j(ctx, *(_dev(cfg[k]) for k in ("m", "x0", "v0", "a0", "j0", "t0")))
+    return ctx
+
+
+def _state(ctx, with_steps=True):
+    ctx_state = ctx.get_state(with_steps)
+    ctx.synchronize()
+    return {k: v.cpu().numpy() for k, v in ctx_state.items()}
+
+
+def test_next_block_matches_the_definition_and_is_ascending():
+    cfg = nbgen.make_config(2, N=70001, n_i=16)
+    ctx = _open(cfg)
+    dt = 2.0 ** -cfg["levels"].astype(np.float64)
+    ctx.set_steps(_dev(dt))
+    idx = torch.empty(cfg["N"], dtype=torch.int32, device="cuda")
+    t_next, n = ctx.next_block(idx)
+    t_ref, act = H.next_block(cfg["t0"], dt)
+    assert t_next == t_ref and n == act.size
+    assert np.array_equal(idx[:n].cpu().numpy(), act)                  # ascending, like the oracle's
+    # a second time level: only the deepest level is due
+    t0 = np.floor(0.3 / dt) * dt
+    cfg2 = dict(cfg, t0=t0)
+    ctx2 = _open(cfg2)
+    ctx2.set_steps(_dev(dt))
+    t_next, n = ctx2.next_block(idx)
+    t_ref, act = H.next_block(t0, dt)
+    assert t_next == t_ref and n == act.size and np.array_equal(idx[:n].cpu().numpy(), act)
+    assert np.array_equal(act, H.sorted_list_prefix(dt, t_ref))        # = the paper's step-sorted prefix
+    ctx.close(); ctx2.close()
+
+
+def test_init_steps_match_the_oracle():
+    cfg = nbgen.make_config(2, N=20000, n_i=16)
+    ctx = _open(cfg)
+    ctx.init_steps(0.02, 2.0**-3)
+    got = _state(ctx)["dt"]
+    ref = H.initial_step(cfg["a0"], cfg["j0"], 0.02, 2.0**-3)
+    assert np.array_equal(got, ref)
+    ctx.close()
+
+
+def test_corrector_and_new_step_match_the_oracle():
+    rng = np.random.default_rng(11)
+    cfg = nbgen.make_config(2, N=30000, n_i=16)
+    N = cfg["N"]
+    dt = 2.0 ** -cfg["levels"].astype(np.float64)
+    cfg = dict(cfg, t0=np.floor(0.3 / dt) * dt)             # mid-run: only the deepest level is due next
+    ctx = _open(cfg)
+    ctx.set_steps(_dev(dt))
+    t, act = H.next_block(cfg["t0"], dt)
+    n = act.size
+    assert 1000 < n < N // 2
+    # new forces of the right magnitude: the old ones advanced by the jerk plus a perturbation, so that
+    # all three branches of the step rule (double / keep / halve) occur
+    a1 = cfg["a0"][act] + cfg["j0"][act] * dt[act, None] * (1 + 0.3 * rng.standard_normal((n, 3)))
+    j1 = cfg["j0"][act] * (1 + rng.standard_normal((n, 3)) * rng.choice([0.01, 0.3, 3.0], size=(n, 1)))
+    eta, dt_max = 0.02, 2.0**-6
+    ctx.correct(t, _dev(act), _dev(a1), _dev(j1), eta, dt_max)
+    got = _state(ctx)
+    x1, v1, a2, a3 = H.correct(cfg["x0"][act], cfg["v0"][act], cfg["a0"][act], cfg["j0"][act], dt[act], a1, j1)
+    req = H.aarseth_step(a1, j1, a2, a3, dt[act], eta)
+    new = H.quantize_step(req, dt[act], t, dt_max)
+    assert np.abs(got["x0"][act] - x1).max() <= 1e-14 * np.abs(x1).max()
+    assert np.abs(got["v0"][act] - v1).max() <= 1e-14 * np.abs(v1).max()
+    assert np.array_equal(got["a0"][act], a1) and np.array_equal(got["j0"][act], j1)
+    assert np.all(got["t0"][act] == t)
+    # the step is a floating-point decision taken in FP64 on both sides: identical except where dt_req
+    # sits within rounding of a power of two (none expected)
+    edge = np.abs(req / 2.0 ** np.round(np.log2(req)) - 1.0) < 1e-12
+    assert np.array_equal(got["dt"][act][~edge], new[~edge]) and edge.sum() <= 1
+    kinds = np.sign(np.log2(new / dt[act]))
+    assert (kinds > 0).any() and (kinds == 0).any() and (kinds < 0).any()
+    # everybody else untouched
+    rest = np.setdiff1d(np.arange(N), act)
+    for k in ("x0", "v0", "a0", "j0", "t0"):
+        assert np.array_equal(got[k][rest], cfg[k][rest])
+    assert np.array_equal(got["dt"][rest], dt[rest])
+    ctx.close()
+
+
+def _oracle_force(m, xp, vp, idx):
+    import oracle
+    out = oracle.regular(m, xp, vp, idx, np.zeros(idx.shape[0]), 8)
+    return out["acc"], out["jerk"]
+
+
+def test_block_loop_conserves_energy_and_follows_the_oracle_integration():
+    """N = 1024 Plummer sphere from t = 0 to 1/8 with the total force (nb_regular, h2 = 0): the GPU loop
+    next_block -> predict_all -> regular -> correct against oracle.hermite.integrate with the FP64 direct sum."""
+    import paper_1504_03687_b200 as nb
+    N, cap = 1024, 8
+    cfg = nbgen.make_config(1, N=N)
+    m, x, v = cfg["m"], cfg["x0"], cfg["v0"]
+    eta, eta_s, dt_max, t_end = 0.01, 0.01, 2.0**-4, 0.125
+    ref = H.integrate(m, x, v, t_end, eta, eta_s, dt_max, _oracle_force)
+
+    ctx = nb.nb_open(N, cap)
+    kw = dict(dtype=torch.float64, device="cuda")
+    buf = dict(acc=torch.empty((N, 3), **kw), jerk=torch.empty((N, 3), **kw), pot=torch.empty(N, **kw),
+               nnb=torch.empty(N, dtype=torch.int32, device="cuda"),
+               nblist=torch.empty((N, cap), dtype=torch.int32, device="cuda"),
+               overflow=torch.empty(N, dtype=torch.int32, device="cuda"))
+    view = lambda n: {k: (b[:n] if b.dim() == 1 else b[:n]) for k, b in buf.items()}
+    zeros_h2 = torch.zeros(N, **kw)
+    all_idx = torch.arange(N, dtype=torch.int32, device="cuda")
+    zero3 = torch.zeros((N, 3), **kw)
+
+    def total_force_and_energy(t):
+        ctx.predict_all(t)
+        ctx.regular(all_idx, zeros_h2, **buf)
+        ctx.synchronize()
+        st = _state(ctx, with_steps=False)
+        e = 0.5 * (st["m"] * (st["v0"] ** 2).sum(1)).sum() + 0.5 * (st["m"] * buf["pot"].cpu().numpy()).sum()
+        return e
+
+    # start-up: forces at t = 0 through the library itself, then the initial steps
+    nb.nb_set_j(ctx, _dev(m), _dev(x), _dev(v), zero3, zero3, torch.zeros(N, **kw))
+    e0 = total_force_and_energy(0.0)
+    nb.nb_set_j(ctx, _dev(m), _dev(x), _dev(v), buf["acc"].clone(), buf["jerk"].clone(), torch.zeros(N, **kw))
+    ctx.init_steps(eta_s, dt_max)
+    idx = torch.empty(N, dtype=torch.int32, device="cuda")
+    blocks = psteps = 0
+    while True:
+        t, n = ctx.next_block(idx)
+        if t > t_end:
+            break
+        ctx.predict_all(t)
+        o = view(n)
+        ctx.regular(idx[:n], zeros_h2[:n], **o)
+        ctx.correct(t, idx[:n], o["acc"], o["jerk"], eta, dt_max)
+        blocks += 1
+        psteps += n
+    st = _state(ctx)
+    assert np.all(st["t0"] == t_end)
+    e1 = total_force_and_energy(t_end)
+    print("block loop: blocks", blocks, "particle steps", psteps, "oracle", ref["blocks"], ref["particle_steps"],
+          "dE/E", (e1 - e0) / e0, "max |dx|", np.abs(st["x0"] - ref["x0"]).max())
+    assert abs((e1 - e0) / e0) < 5e-6
+    # FP32 pair arithmetic perturbs the forces by ~1e-7; a step decision may flip now and then
+    assert abs(psteps - ref["particle_steps"]) <= 0.01 * ref["particle_steps"]
+    assert np.abs(st["x0"] - ref["x0"]).max() < 1e-5 and np.abs(st["v0"] - ref["v0"]).max() < 1e-4
+    ctx.close()
