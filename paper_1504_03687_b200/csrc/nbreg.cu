@@ -216,12 +216,27 @@ int launch_finalize(nb_ctx *c, int32_t n_i, int64_t n_i_pad, int S, double *acc,
     sortW = std::max(sortW, 1);
     const dim3 fgrid((unsigned)((n_i + 31) / 32), (unsigned)(7 + (32 + sortW - 1) / sortW));
     const size_t smem = sortP ? (size_t)sortW * row_bytes : 0;
+    // Programmatic dependent launch: the finalize grid is placed while the force kernel drains and
+    // waits (griddepcontrol.wait) for its completion, so the launch latency is not on the path of
+    // small blocks.
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = fgrid;
+    cfg.blockDim = dim3(W == 4 ? 128 : 512);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = c->stream;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    const int32_t n_i_pad32 = (int32_t)n_i_pad, S32 = S, cap32 = c->cap, sortP32 = sortP, sortW32 = sortW;
+    const double *partial = c->partial;
     if (W == 4)
-        finalize_kernel<4><<<fgrid, 128, smem, c->stream>>>(n_i, (int32_t)n_i_pad, S, c->cap, sortP, sortW,
-                                                             c->partial, c->cnt, acc, jerk, pot, nnb, nblist, overflow);
+        NB_CUDA(c, cudaLaunchKernelEx(&cfg, finalize_kernel<4>, n_i, n_i_pad32, S32, cap32, sortP32, sortW32, partial,
+                                      c->cnt, acc, jerk, pot, nnb, nblist, overflow));
     else
-        finalize_kernel<16><<<fgrid, 512, smem, c->stream>>>(n_i, (int32_t)n_i_pad, S, c->cap, sortP, sortW,
-                                                              c->partial, c->cnt, acc, jerk, pot, nnb, nblist, overflow);
+        NB_CUDA(c, cudaLaunchKernelEx(&cfg, finalize_kernel<16>, n_i, n_i_pad32, S32, cap32, sortP32, sortW32, partial,
+                                      c->cnt, acc, jerk, pot, nnb, nblist, overflow));
     NB_CUDA(c, cudaGetLastError());
     c->launches += 1;
     c->last_S = S;

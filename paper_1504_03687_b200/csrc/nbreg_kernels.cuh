@@ -536,6 +536,9 @@ __global__ void __launch_bounds__(32 * W) finalize_kernel(int32_t n_i, int32_t n
     extern __shared__ int32_t sbuf[];
     __shared__ double red[W][32];
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    // launched with programmatic stream serialization: the grid is resident before the force kernel
+    // has drained; everything it reads is valid after this wait (a no-op in an ordinary launch)
+    asm volatile("griddepcontrol.wait;" ::: "memory");
     if (blockIdx.y < 7) {
         const int q = blockIdx.y;
         const int k = blockIdx.x * 32 + lane;          // k < n_i_pad always (n_i_pad is a multiple of 64)
