@@ -212,6 +212,15 @@ enum {
 int nb_get_info(nb_ctx *ctx, int32_t key, int64_t *value);
 int nb_set_tuning(nb_ctx *ctx, int32_t key, int64_t value);
 
+/* Launch planning as pure host functions (no device, no context): what nb_regular would launch for a
+ * block of n_i out of N bodies on a device with sm_count SMs holding ctas_per_sm force-kernel CTAs
+ * each -- kernel variant (0: 512, 1: 256, 2: 128, 3: 64 i-particles per CTA), its i-block, the number
+ * of j-range splits and the j-tiles (256 bodies) per split; and the chunks nb_step_host sends the
+ * j-state in (chunks = 0: automatic): first_body[0..*nchunk] (room for 9) are the chunk boundaries. */
+int nb_plan_regular(int64_t N, int64_t n_i, int32_t sm_count, int32_t ctas_per_sm, int32_t *variant,
+                    int32_t *iblock, int32_t *jsplit, int32_t *tiles_per_split);
+int nb_plan_chunks(int64_t N, int32_t chunks, int64_t *first_body, int32_t *nchunk);
+
 int nb_last_cuda_error(nb_ctx *ctx); /* cudaError_t of the sticky failure, 0 if none */
 const char *nb_strerror(int code);
 

@@ -17,6 +17,8 @@ from .binding import (  # noqa: F401
     nb_regular,
     nb_regular_all,
     nb_step_host,
+    nb_plan_regular,
+    nb_plan_chunks,
     nb_update_j,
     nb_irregular,
     NB_OK, NB_EINVAL, NB_ESTATE, NB_ENOMEM, NB_ECUDA,

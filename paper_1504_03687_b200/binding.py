@@ -59,6 +59,8 @@ def load_library(build: bool = True) -> ctypes.CDLL:
     lib.nb_next_block.argtypes = [_vp, ctypes.POINTER(dbl), ctypes.POINTER(i32), _vp]
     lib.nb_correct.argtypes = [_vp, dbl, i32, _vp, _vp, _vp, dbl, dbl]
     lib.nb_get_state.argtypes = [_vp] + [_vp] * 7
+    lib.nb_plan_regular.argtypes = [i64, i64, i32, i32] + [ctypes.POINTER(i32)] * 4
+    lib.nb_plan_chunks.argtypes = [i64, i32, ctypes.POINTER(i64), ctypes.POINTER(i32)]
     lib.nb_get_info.argtypes = [_vp, i32, ctypes.POINTER(i64)]
     lib.nb_set_tuning.argtypes = [_vp, i32, i64]
     lib.nb_last_cuda_error.argtypes = [_vp]
@@ -302,6 +304,23 @@ class NbContext:
                    overflow=torch.empty(n, dtype=torch.int32, device=dev))
         self.regular(idx_i, h2_i, **out)
         return out
+
+
+def nb_plan_regular(N: int, n_i: int, sm_count: int = 148, ctas_per_sm: int = 2) -> dict:
+    """Pure host planning (no GPU needed): variant, i-block, j-splits, tiles per split."""
+    lib = load_library()
+    v = [ctypes.c_int32() for _ in range(4)]
+    _check(lib.nb_plan_regular(N, n_i, sm_count, ctas_per_sm, *(ctypes.byref(x) for x in v)), "nb_plan_regular")
+    return dict(variant=v[0].value, iblock=v[1].value, jsplit=v[2].value, tiles_per_split=v[3].value)
+
+
+def nb_plan_chunks(N: int, chunks: int = 0) -> list[int]:
+    """Pure host planning: body boundaries of the chunks nb_step_host sends the j-state in."""
+    lib = load_library()
+    fb = (ctypes.c_int64 * 9)()
+    n = ctypes.c_int32()
+    _check(lib.nb_plan_chunks(N, chunks, fb, ctypes.byref(n)), "nb_plan_chunks")
+    return [fb[q] for q in range(n.value + 1)]
 
 
 # Function-style aliases with the C names (north_star: nb_open / nb_set_j / nb_predict_all / nb_regular)

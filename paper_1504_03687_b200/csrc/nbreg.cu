@@ -8,9 +8,6 @@
 #include <cmath>
 #include <cstdlib>
 #include <cstring>
-#ifdef NBREG_STEP_TIMELINE
-#include <cstdio>
-#endif
 #include <new>
 #include <unordered_map>
 
@@ -108,22 +105,30 @@ void launch_force(const Variant &v, dim3 grid, cudaStream_t st, const ForceParam
     force_kernel<WI, WJ, MINB><<<grid, v.threads, force_smem(32 * WI * WJ), st>>>(p);
 }
 
+// i-particles per CTA and planning overhead (in tile units) of the variants <8,1>, <4,2>, <2,4>, <1,8>
+constexpr int VAR_IBLOCK[NVARIANT] = {512, 256, 128, 64};
+constexpr double VAR_OVH[NVARIANT] = {0.5, 0.75, 1.5, 3.0};
+
 // Pick the kernel variant: least padded work, then the larger i-block (more reuse of each j load).
-int pick_variant(const nb_ctx *c, int32_t n_i) {
-    if (c->force_variant >= 0 && c->force_variant < NVARIANT) return (int)c->force_variant;
+int pick_variant_pure(int64_t n_i) {
     int best = 0;
     int64_t best_pad = -1;
     for (int v = 0; v < NAUTO; ++v) {
-        const int64_t ib = c->var[v].iblock;
+        const int64_t ib = VAR_IBLOCK[v];
         const int64_t pad = (n_i + ib - 1) / ib * ib;
         if (best_pad < 0 || pad < best_pad) { best = v; best_pad = pad; }
     }
     return best;
 }
-
+int pick_variant(const nb_ctx *c, int32_t n_i) {
+    if (c->force_variant >= 0 && c->force_variant < NVARIANT) return (int)c->force_variant;
+    return pick_variant_pure(n_i);
+}
 // Pick the number of j-splits S: minimise waves x (tiles per split + per-CTA overhead); among plans
 // within 0.3 % take the smallest S (less scratch, shorter final reduction).
 int plan_split(const nb_ctx *c, const Variant &v, int64_t n_ib, int64_t ntiles);
+int plan_split_pure(int64_t conc, double ovh_tiles, int64_t n_ib, int64_t ntiles);
+int plan_chunks_pure(int64_t ntiles, int64_t want, int64_t *ctile);
 
 int pick_split(nb_ctx *c, const Variant &v, int64_t n_ib, int64_t ntiles) {
     if (c->force_S > 0) return (int)std::min<int64_t>(c->force_S, ntiles);
@@ -136,22 +141,45 @@ int pick_split(nb_ctx *c, const Variant &v, int64_t n_ib, int64_t ntiles) {
 }
 
 int plan_split(const nb_ctx *c, const Variant &v, int64_t n_ib, int64_t ntiles) {
-    const int64_t conc = (int64_t)c->sm_count * v.ctas_per_sm;
+    return plan_split_pure((int64_t)c->sm_count * v.ctas_per_sm, v.ovh_tiles, n_ib, ntiles);
+}
+
+int plan_split_pure(int64_t conc, double ovh_tiles, int64_t n_ib, int64_t ntiles) {
     const int64_t smax = std::min<int64_t>(ntiles, 8192);
     double best = 1e300;
     for (int64_t S = 1; S <= smax; ++S) {
         const int64_t tps = (ntiles + S - 1) / S;
         const int64_t Seff = (ntiles + tps - 1) / tps;      // splits that actually get tiles
         const int64_t waves = (n_ib * Seff + conc - 1) / conc;
-        best = std::min(best, (double)waves * ((double)tps + v.ovh_tiles));
+        best = std::min(best, (double)waves * ((double)tps + ovh_tiles));
     }
     for (int64_t S = 1; S <= smax; ++S) {
         const int64_t tps = (ntiles + S - 1) / S;
         const int64_t Seff = (ntiles + tps - 1) / tps;
         const int64_t waves = (n_ib * Seff + conc - 1) / conc;
-        if ((double)waves * ((double)tps + v.ovh_tiles) <= best * 1.003) return (int)Seff;
+        if ((double)waves * ((double)tps + ovh_tiles) <= best * 1.003) return (int)Seff;
     }
     return 1;
+}
+
+// Chunk plan of nb_step_host: tile boundaries ctile[0..nchunk] of chunks sized 1/2^L, 1/2^L, then
+// doubling (L = 4: 1/16, 1/16, 1/8, 1/4, 1/2), so that the first copy is short and every later copy hides
+// behind the force launches of the chunks before it.  want = 0: automatic L from the problem size.
+int plan_chunks_pure(int64_t ntiles, int64_t want, int64_t *ctile) {
+    constexpr int MAXCHUNK = 8;
+    int L = ntiles >= 2048 ? 4 : ntiles >= 512 ? 2 : 0;
+    if (want > 0) L = (int)std::min<int64_t>(want - 1, MAXCHUNK - 1);
+    while (L > 0 && (ntiles >> L) == 0) --L;
+    int64_t sz = std::max<int64_t>(ntiles >> L, 1), at = 0;
+    int nchunk = 0;
+    ctile[0] = 0;
+    while (at < ntiles) {
+        const bool last = (nchunk == L) || (at + sz >= ntiles);
+        at = last ? ntiles : at + sz;
+        ctile[++nchunk] = at;
+        if (nchunk >= 2) sz *= 2;
+    }
+    return nchunk;
 }
 
 int check_live(nb_ctx *c) {
@@ -345,10 +373,10 @@ int nb_open(int64_t N, int32_t nb_cap, nb_ctx **out) {
         NB_CUDA(c, cudaFuncSetAttribute(finalize_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, s4));
         NB_CUDA(c, cudaFuncSetAttribute(finalize_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, s16));
     }
-    NB_CUDA(c, (setup_variant<8, 1, 2>(c->var[0], 0.5)));
-    NB_CUDA(c, (setup_variant<4, 2, 2>(c->var[1], 0.75)));
-    NB_CUDA(c, (setup_variant<2, 4, 2>(c->var[2], 1.5)));
-    NB_CUDA(c, (setup_variant<1, 8, 2>(c->var[3], 3.0)));
+    NB_CUDA(c, (setup_variant<8, 1, 2>(c->var[0], VAR_OVH[0])));
+    NB_CUDA(c, (setup_variant<4, 2, 2>(c->var[1], VAR_OVH[1])));
+    NB_CUDA(c, (setup_variant<2, 4, 2>(c->var[2], VAR_OVH[2])));
+    NB_CUDA(c, (setup_variant<1, 8, 2>(c->var[3], VAR_OVH[3])));
     return NB_OK;
 }
 
@@ -599,20 +627,7 @@ int nb_step_host(nb_ctx *c, const double *m, const double *x0, const double *v0,
     // every later copy hidden behind the force launches of the chunks before it)
     const int64_t ntiles = c->Npad / TJ;
     int64_t ctile[nb_ctx::MAXCHUNK + 1];
-    int nchunk = 0;
-    {
-        int L = ntiles >= 2048 ? 4 : ntiles >= 512 ? 2 : 0;
-        if (c->step_chunks > 0) L = (int)std::min<int64_t>(c->step_chunks - 1, nb_ctx::MAXCHUNK - 1);
-        while (L > 0 && (ntiles >> L) == 0) --L;
-        int64_t sz = std::max<int64_t>(ntiles >> L, 1), at = 0;
-        ctile[0] = 0;
-        while (at < ntiles) {
-            const bool last = (nchunk == L) || (at + sz >= ntiles);
-            at = last ? ntiles : at + sz;
-            ctile[++nchunk] = at;
-            if (nchunk >= 2) sz *= 2;
-        }
-    }
+    const int nchunk = plan_chunks_pure(ntiles, c->step_chunks, ctile);
     int S_c[nb_ctx::MAXCHUNK], S_total = 0;
     for (int q = 0; q < nchunk; ++q) {
         S_c[q] = pick_split(c, v, n_ib, ctile[q + 1] - ctile[q]);
@@ -621,15 +636,7 @@ int nb_step_host(nb_ctx *c, const double *m, const double *x0, const double *v0,
     rc = ensure_partial(c, (size_t)S_total * 7 * n_i_pad * sizeof(double));
     if (rc != NB_OK) return rc;
 
-#ifdef NBREG_STEP_TIMELINE
-    static cudaEvent_t tl[64]; static bool tl_init = false; int tln = 0; const char *tlname[64];
-    if (!tl_init) { for (auto &e : tl) cudaEventCreate(&e); tl_init = true; }
-#define TL(stream_, name_) do { tlname[tln] = name_; cudaEventRecord(tl[tln++], stream_); } while (0)
-#else
-#define TL(stream_, name_) do { } while (0)
-#endif
     cudaStream_t cs = c->copy_stream, ps = c->prep_stream;
-    TL(c->stream, "enter");
     NB_CUDA(c, cudaEventRecord(c->ev_enter, c->stream));          // staging buffers are free once earlier work ran
     NB_CUDA(c, cudaStreamWaitEvent(cs, c->ev_enter, 0));
     NB_CUDA(c, cudaStreamWaitEvent(ps, c->ev_enter, 0));
@@ -638,7 +645,6 @@ int nb_step_host(nb_ctx *c, const double *m, const double *x0, const double *v0,
     if (!zero_copy)
         NB_CUDA(c, cudaMemcpyAsync(c->d_ist, c->h_ist, sizeof(double) * 14 * n_i, cudaMemcpyHostToDevice, cs));
     NB_CUDA(c, cudaEventRecord(c->ev_i, cs));
-    TL(cs, "i-state copied");
     double *d = c->stage_j;
     double *dm = d, *dx = d + N, *dv = d + 4 * N, *da = d + 7 * N, *dj = d + 10 * N, *dt0 = d + 13 * N;
     for (int q = 0; q < nchunk; ++q) {
@@ -651,7 +657,6 @@ int nb_step_host(nb_ctx *c, const double *m, const double *x0, const double *v0,
             NB_CUDA(c, cudaMemcpyAsync(da + 3 * jb, a0 + 3 * jb, n3, cudaMemcpyHostToDevice, cs));
             NB_CUDA(c, cudaMemcpyAsync(dj + 3 * jb, j0 + 3 * jb, n3, cudaMemcpyHostToDevice, cs));
             NB_CUDA(c, cudaMemcpyAsync(dt0 + jb, t0 + jb, n1, cudaMemcpyHostToDevice, cs));
-            TL(cs, "chunk copied");
             // the kernels of a landed chunk go to their own stream: they may wait for SM slots behind the
             // running force launch, and the next chunk's copies must not queue behind them
             NB_CUDA(c, cudaEventRecord(c->ev_copied[q], cs));
@@ -662,7 +667,6 @@ int nb_step_host(nb_ctx *c, const double *m, const double *x0, const double *v0,
         predict_kernel<<<(unsigned)((je_pad - jb + 255) / 256), 256, 0, ps>>>(jb, je_pad, N, c->Ns, t, c->soa, c->rec);
         NB_CUDA(c, cudaGetLastError());
         NB_CUDA(c, cudaEventRecord(c->ev_chunk[q], ps));
-        TL(ps, "chunk predicted");
         c->launches += 2;
     }
     c->have_j = true;
@@ -678,26 +682,15 @@ int nb_step_host(nb_ctx *c, const double *m, const double *x0, const double *v0,
     int64_t split0 = 0;
     for (int q = 0; q < nchunk; ++q) {
         NB_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_chunk[q], 0));
-        TL(c->stream, "force start");
         rc = launch_force_range(c, vi, n_i, c->st_idx, c->st_h2, c->irec, c->st_list, ctile[q], ctile[q + 1], S_c[q],
                                 split0);
         if (rc != NB_OK) return rc;
-        TL(c->stream, "force done");
         split0 += S_c[q];
     }
     double *d_acc = c->st_out, *d_jerk = c->st_out + 3 * (int64_t)n_i, *d_pot = c->st_out + 6 * (int64_t)n_i;
     rc = launch_finalize(c, n_i, n_i_pad, S_total, d_acc, d_jerk, d_pot, c->st_nnb, c->st_list, c->st_ovf);
     if (rc != NB_OK) return rc;
-    TL(c->stream, "finalized");
     rc = copy_back(c, n_i, acc, jerk, pot, nnb, nblist, overflow);
-#ifdef NBREG_STEP_TIMELINE
-    for (int q = 1; q < tln; ++q) {
-        float ms = 0.f;
-        cudaEventElapsedTime(&ms, tl[0], tl[q]);
-        fprintf(stderr, "[nb_step_host] %8.3f ms  %s\n", ms, tlname[q]);
-    }
-#endif
-#undef TL
     return rc;
 }
 
@@ -839,6 +832,26 @@ int nb_set_tuning(nb_ctx *c, int32_t key, int64_t value) {
             break;
         default: return NB_EINVAL;
     }
+    return NB_OK;
+}
+
+int nb_plan_regular(int64_t N, int64_t n_i, int32_t sm_count, int32_t ctas_per_sm, int32_t *variant, int32_t *iblock,
+                    int32_t *jsplit, int32_t *tiles_per_split) {
+    if (N <= 0 || n_i <= 0 || n_i > N || sm_count <= 0 || ctas_per_sm <= 0) return NB_EINVAL;
+    if (!variant || !iblock || !jsplit || !tiles_per_split) return NB_EINVAL;
+    const int vi = pick_variant_pure(n_i);
+    const int64_t ib = VAR_IBLOCK[vi], n_ib = (n_i + ib - 1) / ib, ntiles = (N + TJ - 1) / TJ;
+    const int S = plan_split_pure((int64_t)sm_count * ctas_per_sm, VAR_OVH[vi], n_ib, ntiles);
+    *variant = vi; *iblock = (int32_t)ib; *jsplit = S; *tiles_per_split = (int32_t)((ntiles + S - 1) / S);
+    return NB_OK;
+}
+
+int nb_plan_chunks(int64_t N, int32_t chunks, int64_t *first_body, int32_t *nchunk) {
+    if (N <= 0 || chunks < 0 || chunks > nb_ctx::MAXCHUNK || !first_body || !nchunk) return NB_EINVAL;
+    int64_t ctile[nb_ctx::MAXCHUNK + 1];
+    const int n = plan_chunks_pure((N + TJ - 1) / TJ, chunks, ctile);
+    for (int q = 0; q <= n; ++q) first_body[q] = std::min<int64_t>(ctile[q] * TJ, N);
+    *nchunk = n;
     return NB_OK;
 }
 

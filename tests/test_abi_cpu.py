@@ -59,3 +59,50 @@ def test_i_sharding_covers_block_exactly_once():
         assert np.array_equal(np.concatenate([p[1] for p in parts]), h2)
         sizes = [p[0].size for p in parts]
         assert max(sizes) - min(sizes) <= 1
+
+
+# ----------------------------------------------------------------------------- host logic: launch planning
+
+def test_plan_regular_fills_the_chip_and_covers_the_j_range():
+    """nb_plan_regular (pure host function of the library): the split covers every j-tile, pads the
+    block as little as any variant can, and its modelled cost (waves x tiles per split) is within
+    1 % of the best over all splits."""
+    import paper_1504_03687_b200 as nb
+    sm, per_sm = 148, 2
+    conc = sm * per_sm
+    ovh = {512: 0.5, 256: 0.75, 128: 1.5, 64: 3.0}
+    for N in (1024, 65536, 262144, 1048576, 1000003):
+        ntiles = -(-N // 256)
+        for n_i in (1, 32, 64, 100, 128, 257, 512, 1000, 4096, 8192, 65536, 131072):
+            if n_i > N:
+                continue
+            p = nb.nb_plan_regular(N, n_i, sm, per_sm)
+            ib, S, tps = p["iblock"], p["jsplit"], p["tiles_per_split"]
+            assert ib == (512, 256, 128, 64)[p["variant"]]
+            pad = -(-n_i // ib) * ib
+            assert pad == min(-(-n_i // b) * b for b in (512, 256, 128, 64))        # least padded work
+            assert 1 <= S <= ntiles and tps == -(-ntiles // S) and (S - 1) * tps < ntiles <= S * tps
+            n_ib = pad // ib
+            cost = lambda s: -(-(n_ib * -(-ntiles // -(-ntiles // s))) // conc) * (-(-ntiles // s) + ovh[ib])
+            best = min(cost(s) for s in range(1, min(ntiles, 8192) + 1))
+            assert cost(S) <= 1.01 * best
+    p = nb.nb_plan_regular(1048576, 8192, sm, per_sm)
+    assert p["jsplit"] * (8192 // p["iblock"]) % conc == 0            # the headline block: whole waves
+    with pytest.raises(nb.NbregError):
+        nb.nb_plan_regular(1024, 2048)
+
+
+def test_plan_chunks_partition_the_bodies_and_grow():
+    import paper_1504_03687_b200 as nb
+    for N in (1, 255, 10000, 131072, 140000, 600000, 1048576, 3000001):
+        for want in (0, 1, 2, 3, 5, 8):
+            b = nb.nb_plan_chunks(N, want)
+            assert b[0] == 0 and b[-1] == N and all(x < y for x, y in zip(b, b[1:]))
+            assert all(x % 256 == 0 for x in b[:-1])                   # whole j-tiles
+            sizes = np.diff(b)
+            assert len(sizes) <= 8 and (want == 0 or len(sizes) <= want)
+            if len(sizes) > 2:       # first copy short, later ones double; the last takes the rounding remainder
+                assert sizes[0] == sizes[1] and all(y == 2 * x for x, y in zip(sizes[1:-2], sizes[2:-1]))
+                assert sizes[-1] <= 2 * sizes[-2] + 256 * 2 ** (len(sizes) - 1)
+    assert nb.nb_plan_chunks(1048576) == [0, 65536, 131072, 262144, 524288, 1048576]
+    assert nb.nb_plan_chunks(1048576, 1) == [0, 1048576]
