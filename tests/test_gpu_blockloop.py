@@ -166,3 +166,59 @@ def test_block_loop_conserves_energy_and_follows_the_oracle_integration():
     assert abs(psteps - ref["particle_steps"]) <= 0.01 * ref["particle_steps"]
     assert np.abs(st["x0"] - ref["x0"]).max() < 1e-5 and np.abs(st["v0"] - ref["v0"]).max() < 1e-4
     ctx.close()
+
+
+def test_ac_split_block_loop_at_65536_bodies_follows_the_oracle():
+    """Three consecutive blocks of a 65536-body cluster with the Ahmad-Cohen split evaluated at the block
+    time: nb_regular (neighbours excluded, lists emitted) + nb_irregular (the listed neighbours, FP64)
+    added by the caller = total force -> nb_correct.  The oracle runs the same three blocks with its own
+    regular, irregular, corrector and step rule; states must agree."""
+    import oracle
+    import paper_1504_03687_b200 as nb
+    cfg = nbgen.make_config(2)
+    N, cap = cfg["N"], cfg["cap"]
+    dt = 2.0 ** -cfg["levels"].astype(np.float64)
+    st = dict(m=cfg["m"], x0=cfg["x0"].copy(), v0=cfg["v0"].copy(), a0=cfg["a0"].copy(), j0=cfg["j0"].copy(),
+              t0=np.floor(0.3 / dt) * dt, dt=dt.copy())
+    eta, dt_max = 0.02, 2.0**-6
+    ctx = nb.nb_open(N, cap)
+    nb.nb_set_j(ctx, *(_dev(st[k]) for k in ("m", "x0", "v0", "a0", "j0", "t0")))
+    ctx.set_steps(_dev(st["dt"]))
+    h2_np = np.minimum(cfg["h2_all"], 0.01)        # halo bodies would get radii that swallow the core: keep every row under cap
+    h2_all = _dev(h2_np)
+    idx = torch.empty(N, dtype=torch.int32, device="cuda")
+    sizes = []
+    for _ in range(3):
+        # ---- GPU
+        t, n = ctx.next_block(idx)
+        act = idx[:n]
+        ctx.predict_all(t)
+        reg = ctx.regular_alloc(act, h2_all[act.long()].contiguous())
+        irr = dict(acc=torch.empty_like(reg["acc"]), jerk=torch.empty_like(reg["jerk"]))
+        ctx.irregular(t, act, reg["nnb"], reg["nblist"], **irr)
+        ctx.correct(t, act, reg["acc"] + irr["acc"], reg["jerk"] + irr["jerk"], eta, dt_max)
+        # ---- oracle
+        t_ref, a_ref = H.next_block(st["t0"], st["dt"])
+        assert t == t_ref and np.array_equal(act.cpu().numpy(), a_ref)
+        xp, vp = oracle.predict(st["x0"], st["v0"], st["a0"], st["j0"], st["t0"], t_ref)
+        r = oracle.regular(st["m"], xp, vp, a_ref, h2_np[a_ref], cap)
+        assert not r["overflow"].any() and np.array_equal(r["nnb"], reg["nnb"].cpu().numpy())
+        i = oracle.irregular(st["m"], st["x0"], st["v0"], st["a0"], st["j0"], st["t0"], t_ref, a_ref, r["nnb"],
+                             r["nblist"], cap)
+        assert np.abs(i["acc"] - r["acc_nb"]).max() <= 1e-12 * np.abs(i["acc"]).max()   # same sum, two routes
+        a1, j1 = r["acc"] + i["acc"], r["jerk"] + i["jerk"]
+        x1, v1, a2, a3 = H.correct(st["x0"][a_ref], st["v0"][a_ref], st["a0"][a_ref], st["j0"][a_ref],
+                                   st["dt"][a_ref], a1, j1)
+        new = H.quantize_step(H.aarseth_step(a1, j1, a2, a3, st["dt"][a_ref], eta), st["dt"][a_ref], t_ref, dt_max)
+        st["x0"][a_ref], st["v0"][a_ref], st["a0"][a_ref], st["j0"][a_ref] = x1, v1, a1, j1
+        st["t0"][a_ref], st["dt"][a_ref] = t_ref, new
+        sizes.append(n)
+    got = _state(ctx)
+    assert len(set(sizes)) > 1 and max(sizes) > 1000 and min(sizes) >= 1      # a deep block and tiny follow-ups
+    assert np.array_equal(got["t0"], st["t0"])
+    assert np.abs(got["x0"] - st["x0"]).max() < 1e-12 and np.abs(got["v0"] - st["v0"]).max() < 1e-10
+    assert np.abs(got["a0"] - st["a0"]).max() <= 1e-5 * np.abs(st["a0"]).max()
+    flips = (got["dt"] != st["dt"]).sum()
+    print("AC-split loop: block sizes", sizes, "step decisions that differ", int(flips))
+    assert flips <= 1e-3 * sum(sizes)      # FP32 pair terms move dt_req by ~1e-7: a flip needs dt_req that close to 2^-k
+    ctx.close()
