@@ -356,7 +356,7 @@ def run_b200(args):
     sweep = None
     if not args.no_sweep and world == 1:
         sweep = []
-        for n in cfg["sweep"]:
+        for n in [32] + list(cfg["sweep"]):        # 32: the j-packed tiny-block variant (config 5's smallest block)
             if n > N:
                 continue
             si, sh = nbgen.active_block(cfg, n)

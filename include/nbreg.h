@@ -214,7 +214,7 @@ int nb_set_tuning(nb_ctx *ctx, int32_t key, int64_t value);
 
 /* Launch planning as pure host functions (no device, no context): what nb_regular would launch for a
  * block of n_i out of N bodies on a device with sm_count SMs holding ctas_per_sm force-kernel CTAs
- * each -- kernel variant (0: 512, 1: 256, 2: 128, 3: 64 i-particles per CTA), its i-block, the number
+ * each -- kernel variant (0: 512, 1: 256, 2: 128, 3: 64, 4: 32 i-particles per CTA), its i-block, the number
  * of j-range splits and the j-tiles (256 bodies) per split; and the chunks nb_step_host sends the
  * j-state in (chunks = 0: automatic): first_body[0..*nchunk] (room for 9) are the chunk boundaries. */
 int nb_plan_regular(int64_t N, int64_t n_i, int32_t sm_count, int32_t ctas_per_sm, int32_t *variant,

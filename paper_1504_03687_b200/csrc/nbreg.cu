@@ -22,8 +22,8 @@ struct Variant {
     double ovh_tiles;        // per-CTA fixed cost in units of one tile's compute (planning heuristic)
     int ctas_per_sm;         // from the occupancy API at nb_open
 };
-constexpr int NVARIANT = 4;
-constexpr int NAUTO = 4;        // variants the planner picks from; the rest only by NB_TUNE_FORCE_VARIANT
+constexpr int NVARIANT = 5;
+constexpr int NAUTO = 5;        // variants the planner picks from; the rest only by NB_TUNE_FORCE_VARIANT
 constexpr size_t force_smem(int threads) {      // tile ring + FP64 sums + mbarriers + counters
     return (size_t)NSTAGE * TILE_FLOATS * sizeof(float) + (size_t)14 * threads * sizeof(double) +
            NSTAGE * sizeof(uint64_t) + 64;
@@ -87,11 +87,11 @@ namespace {
         }                                           \
     } while (0)
 
-template <int WI, int WJ, int MINB>
+template <int WI, int WJ, int MINB, bool JP = false>
 cudaError_t setup_variant(Variant &v, double ovh) {
     static_assert(WJ == 1 || (size_t)WJ * 7 * 64 * WI * sizeof(double) <= force_smem(32 * WI * WJ), "WJ reduction reuses the ring");
-    v.it = 2; v.wi = WI; v.wj = WJ; v.iblock = 64 * WI; v.threads = 32 * WI * WJ; v.ovh_tiles = ovh;
-    auto k = force_kernel<WI, WJ, MINB>;
+    v.it = JP ? 1 : 2; v.wi = WI; v.wj = WJ; v.iblock = (JP ? 32 : 64) * WI; v.threads = 32 * WI * WJ; v.ovh_tiles = ovh;
+    auto k = force_kernel<WI, WJ, MINB, JP>;
     cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)force_smem(32 * WI * WJ));
     if (e != cudaSuccess) return e;
     int nb = 0;
@@ -100,23 +100,27 @@ cudaError_t setup_variant(Variant &v, double ovh) {
     return e;
 }
 
-template <int WI, int WJ, int MINB>
+template <int WI, int WJ, int MINB, bool JP = false>
 void launch_force(const Variant &v, dim3 grid, cudaStream_t st, const ForceParams &p) {
-    force_kernel<WI, WJ, MINB><<<grid, v.threads, force_smem(32 * WI * WJ), st>>>(p);
+    force_kernel<WI, WJ, MINB, JP><<<grid, v.threads, force_smem(32 * WI * WJ), st>>>(p);
 }
 
-// i-particles per CTA and planning overhead (in tile units) of the variants <8,1>, <4,2>, <2,4>, <1,8>
-constexpr int VAR_IBLOCK[NVARIANT] = {512, 256, 128, 64};
-constexpr double VAR_OVH[NVARIANT] = {0.5, 0.75, 1.5, 3.0};
+// i-particles per CTA, planning overhead (in tile units) and relative cost per padded i-slot of the
+// variants <8,1>, <4,2>, <2,4>, <1,8> and the j-packed <1,8> (32 i per CTA).  The cost factors are
+// measured: time per padded i-slot at n_i = 8256 and 16500, N = 1M, relative to <8,1>.
+constexpr int VAR_IBLOCK[NVARIANT] = {512, 256, 128, 64, 32};
+constexpr double VAR_OVH[NVARIANT] = {0.5, 0.75, 1.5, 3.0, 3.0};
+constexpr double VAR_COST[NVARIANT] = {1.0, 1.01, 1.025, 1.03, 1.11};
 
-// Pick the kernel variant: least padded work, then the larger i-block (more reuse of each j load).
+// Pick the kernel variant: least padded work weighted by the variant's rate, ties to the larger i-block
+// (more reuse of each j load).
 int pick_variant_pure(int64_t n_i) {
     int best = 0;
-    int64_t best_pad = -1;
+    double best_cost = -1.0;
     for (int v = 0; v < NAUTO; ++v) {
         const int64_t ib = VAR_IBLOCK[v];
-        const int64_t pad = (n_i + ib - 1) / ib * ib;
-        if (best_pad < 0 || pad < best_pad) { best = v; best_pad = pad; }
+        const double cost = (double)((n_i + ib - 1) / ib * ib) * VAR_COST[v];
+        if (best_cost < 0.0 || cost < best_cost) { best = v; best_cost = cost; }
     }
     return best;
 }
@@ -222,7 +226,8 @@ int launch_force_range(nb_ctx *c, int vi, int32_t n_i, const int32_t *idx_i, con
         case 0: launch_force<8, 1, 2>(v, grid, c->stream, p); break;
         case 1: launch_force<4, 2, 2>(v, grid, c->stream, p); break;
         case 2: launch_force<2, 4, 2>(v, grid, c->stream, p); break;
-        default: launch_force<1, 8, 2>(v, grid, c->stream, p); break;
+        case 3: launch_force<1, 8, 2>(v, grid, c->stream, p); break;
+        default: launch_force<1, 8, 2, true>(v, grid, c->stream, p); break;
     }
     NB_CUDA(c, cudaGetLastError());
     if (c->profile) {
@@ -377,6 +382,7 @@ int nb_open(int64_t N, int32_t nb_cap, nb_ctx **out) {
     NB_CUDA(c, (setup_variant<4, 2, 2>(c->var[1], VAR_OVH[1])));
     NB_CUDA(c, (setup_variant<2, 4, 2>(c->var[2], VAR_OVH[2])));
     NB_CUDA(c, (setup_variant<1, 8, 2>(c->var[3], VAR_OVH[3])));
+    NB_CUDA(c, (setup_variant<1, 8, 2, true>(c->var[4], VAR_OVH[4])));
     return NB_OK;
 }
 

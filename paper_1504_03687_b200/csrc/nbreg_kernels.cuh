@@ -280,6 +280,14 @@ __device__ __forceinline__ float2 pfma(float2 a, float2 b, float2 c) { return __
 #endif
 __device__ __forceinline__ float2 bc(float s) { return make_float2(s, s); }   // -> scalar `R.F32` operand
 __device__ __forceinline__ float pick(const float4 &v, int u) { return u == 0 ? v.x : u == 1 ? v.y : u == 2 ? v.z : v.w; }
+// j-side operand number u of a group of four consecutive j.  JP = false: j number u broadcast to both
+// halves (the halves are two i).  JP = true (tiny blocks): the halves are the two consecutive j 2u, 2u+1
+// against ONE i held in both halves of the i registers -- a warp then covers 32 i instead of 64.
+template <bool JP>
+__device__ __forceinline__ float2 jop(const float4 &v, int u) {
+    if constexpr (JP) return u == 0 ? make_float2(v.x, v.y) : make_float2(v.z, v.w);
+    else return bc(pick(v, u));
+}
 
 // One neighbour of active particle k: take a slot of its row with an integer atomic (rows are shared
 // with the other j-splits and warps); entries past the capacity are only counted (reading R9).
@@ -298,17 +306,17 @@ struct Acc7 {
 // predicates.  MASKED = true drops the pairs with r2 < h2 by zeroing 1/r BEFORE any product (no inf*0).
 template <bool MASKED>
 __device__ __forceinline__ void pair_terms(Acc7 &A, const IPair &I, float2 dx, float2 dy, float2 dz, float2 r2,
-                                           float2 rinv, float jvx, float jvy, float jvz, float jm) {
-    const float2 dvx = padd(bc(jvx), I.nvx);
-    const float2 dvy = padd(bc(jvy), I.nvy);
-    const float2 dvz = padd(bc(jvz), I.nvz);
+                                           float2 rinv, float2 jvx, float2 jvy, float2 jvz, float2 jm) {
+    const float2 dvx = padd(jvx, I.nvx);
+    const float2 dvy = padd(jvy, I.nvy);
+    const float2 dvz = padd(jvz, I.nvz);
     const float2 rv = pfma(dz, dvz, pfma(dy, dvy, pmul(dx, dvx)));
     if (MASKED) {       // a select, not a product: the self pair's rsqrt(0) = inf never reaches the arithmetic
         rinv.x = r2.x < I.h2.x ? 0.f : rinv.x;
         rinv.y = r2.y < I.h2.y ? 0.f : rinv.y;
     }
     const float2 rinv2 = pmul(rinv, rinv);
-    const float2 mrinv = pmul(bc(jm), rinv);
+    const float2 mrinv = pmul(jm, rinv);
     const float2 mrinv3 = pmul(mrinv, rinv2);
     const float2 alpha = pmul(pmul(rv, rinv2), make_float2(-3.0f, -3.0f));
     A.ph = padd(A.ph, mrinv);
@@ -322,10 +330,14 @@ __device__ __forceinline__ void pair_terms(Acc7 &A, const IPair &I, float2 dx, f
 
 // Each thread owns one PAIR of i-particles; WI warps along i (64 i each), WJ warps along j (each
 // takes TJ/WJ j's of every tile).  CTA = 32*WI*WJ threads, i-block = 64*WI.
-template <int WI, int WJ, int MINB>
+// JP (blocks of <= 32 active particles, and the ragged tail of small blocks): each thread owns ONE
+// i-particle and the packed halves are two consecutive j; i-block = 32*WI.
+template <int WI, int WJ, int MINB, bool JP = false>
 __global__ void __launch_bounds__(32 * WI *WJ, MINB) force_kernel(const ForceParams p) {
     constexpr int NW = WI * WJ;
-    constexpr int IB = 64 * WI;
+    constexpr int NH = JP ? 1 : 2;           // i-particles per thread
+    constexpr int NU = JP ? 2 : 4;           // packed iterations per group of four j
+    constexpr int IB = 32 * NH * WI;
     constexpr int SUB = TJ / WJ;
     constexpr uint32_t TILE_BYTES = TILE_FLOATS * sizeof(float);
     static_assert(SUB % UNROLL_J == 0 && UNROLL_J == 4, "a group is one LDS.128 per component");
@@ -354,7 +366,7 @@ __global__ void __launch_bounds__(32 * WI *WJ, MINB) force_kernel(const ForcePar
         float v[2][10];
 #pragma unroll
         for (int h = 0; h < 2; ++h) {
-            const int k = blockIdx.x * IB + wi * 64 + h * 32 + lane;
+            const int k = blockIdx.x * IB + wi * (32 * NH) + (JP ? 0 : h * 32) + lane;   // JP: both halves = the same i
             my_k[h] = k;
             if (k < p.n_i) {
                 const int32_t idx = p.idx_i ? p.idx_i[k] : k;      // NULL = identity block (full-N pass)
@@ -415,36 +427,44 @@ __global__ void __launch_bounds__(32 * WI *WJ, MINB) force_kernel(const ForcePar
             for (int c = 0; c < RECF; ++c)                     // warp-uniform address: LDS.128 broadcast
                 c4[c] = *reinterpret_cast<const float4 *>(tsub + c * TJ + g);
             // phase 1: FP64-equivalent differences and r^2 of the group's 4 j against the i-pair
-            float2 dx[UNROLL_J], dy[UNROLL_J], dz[UNROLL_J], r2[UNROLL_J], rinv[UNROLL_J];
+            float2 dx[NU], dy[NU], dz[NU], r2[NU], rinv[NU];
 #pragma unroll
-            for (int u = 0; u < UNROLL_J; ++u) {
-                dx[u] = padd(padd(bc(pick(c4[C_XH], u)), I.nxh), padd(bc(pick(c4[C_XL], u)), I.nxl));
-                dy[u] = padd(padd(bc(pick(c4[C_YH], u)), I.nyh), padd(bc(pick(c4[C_YL], u)), I.nyl));
-                dz[u] = padd(padd(bc(pick(c4[C_ZH], u)), I.nzh), padd(bc(pick(c4[C_ZL], u)), I.nzl));
+            for (int u = 0; u < NU; ++u) {
+                dx[u] = padd(padd(jop<JP>(c4[C_XH], u), I.nxh), padd(jop<JP>(c4[C_XL], u), I.nxl));
+                dy[u] = padd(padd(jop<JP>(c4[C_YH], u), I.nyh), padd(jop<JP>(c4[C_YL], u), I.nyl));
+                dz[u] = padd(padd(jop<JP>(c4[C_ZH], u), I.nzh), padd(jop<JP>(c4[C_ZL], u), I.nzl));
                 r2[u] = pfma(dz[u], dz[u], pfma(dy[u], dy[u], pmul(dx[u], dx[u])));
                 rinv[u].x = rsqrt_sfu(r2[u].x);        // issued before the vote: SFU latency overlaps the test
                 rinv[u].y = rsqrt_sfu(r2[u].y);
             }
             // one test per i for the whole group (FMNMX3): a neighbour, or the self pair (r2 == 0)?
-            const float mn0 = fminf(fminf(fminf(r2[0].x, r2[1].x), r2[2].x), r2[3].x);
-            const float mn1 = fminf(fminf(fminf(r2[0].y, r2[1].y), r2[2].y), r2[3].y);
+            float mn0, mn1;
+            if constexpr (JP) {
+                mn0 = fminf(r2[0].x, r2[1].x);
+                mn1 = fminf(r2[0].y, r2[1].y);
+            } else {
+                mn0 = fminf(fminf(fminf(r2[0].x, r2[1].x), r2[2].x), r2[3].x);
+                mn1 = fminf(fminf(fminf(r2[0].y, r2[1].y), r2[2].y), r2[3].y);
+            }
             const bool hit = (mn0 < I.h2.x) | (mn1 < I.h2.y);
             if (!__any_sync(0xffffffffu, hit)) {    // ~95 % of groups at N_b ~ 150, N = 1M: nothing to mask
 #pragma unroll
-                for (int u = 0; u < UNROLL_J; ++u)
-                    pair_terms<false>(A, I, dx[u], dy[u], dz[u], r2[u], rinv[u], pick(c4[C_VX], u), pick(c4[C_VY], u),
-                                      pick(c4[C_VZ], u), pick(c4[C_M], u));
+                for (int u = 0; u < NU; ++u)
+                    pair_terms<false>(A, I, dx[u], dy[u], dz[u], r2[u], rinv[u], jop<JP>(c4[C_VX], u),
+                                      jop<JP>(c4[C_VY], u), jop<JP>(c4[C_VZ], u), jop<JP>(c4[C_M], u));
             } else {
 #pragma unroll
-                for (int u = 0; u < UNROLL_J; ++u)
-                    pair_terms<true>(A, I, dx[u], dy[u], dz[u], r2[u], rinv[u], pick(c4[C_VX], u), pick(c4[C_VY], u),
-                                     pick(c4[C_VZ], u), pick(c4[C_M], u));
+                for (int u = 0; u < NU; ++u)
+                    pair_terms<true>(A, I, dx[u], dy[u], dz[u], r2[u], rinv[u], jop<JP>(c4[C_VX], u),
+                                     jop<JP>(c4[C_VY], u), jop<JP>(c4[C_VZ], u), jop<JP>(c4[C_M], u));
                 if (hit) {      // rare: lanes hold different i, each takes slots of its own rows
 #pragma unroll
-                    for (int u = 0; u < UNROLL_J; ++u) {
-                        const int32_t jg = jbase + g + u;
-                        if (r2[u].x < I.h2.x && jg != my_idx[0]) append_one(my_k[0], jg, p.cap, p.cnt, p.nblist);
-                        if (r2[u].y < I.h2.y && jg != my_idx[1]) append_one(my_k[1], jg, p.cap, p.cnt, p.nblist);
+                    for (int u = 0; u < NU; ++u) {
+                        // half .x / .y of iteration u: (i, j) = (my i 0, j u) / (my i 1, j u), or, j-packed,
+                        // (my i, j 2u) / (my i, j 2u + 1)
+                        const int32_t jg0 = jbase + g + (JP ? 2 * u : u), jg1 = JP ? jg0 + 1 : jg0;
+                        if (r2[u].x < I.h2.x && jg0 != my_idx[0]) append_one(my_k[0], jg0, p.cap, p.cnt, p.nblist);
+                        if (r2[u].y < I.h2.y && jg1 != my_idx[1]) append_one(my_k[1], jg1, p.cap, p.cnt, p.nblist);
                     }
                 }
             }
@@ -454,8 +474,12 @@ __global__ void __launch_bounds__(32 * WI *WJ, MINB) force_kernel(const ForcePar
             const float2 *Av = &A.ax;       // ax, ay, az, jx, jy, jz, ph
 #pragma unroll
             for (int c = 0; c < 7; ++c) {
-                acc64[c * NT] += (double)Av[c].x;
-                acc64[(7 + c) * NT] += (double)Av[c].y;
+                if constexpr (JP) {     // both halves belong to the same i (even / odd j): one sum, fixed order
+                    acc64[c * NT] += (double)Av[c].x + (double)Av[c].y;
+                } else {
+                    acc64[c * NT] += (double)Av[c].x;
+                    acc64[(7 + c) * NT] += (double)Av[c].y;
+                }
             }
             A.ax = A.ay = A.az = A.jx = A.jy = A.jz = A.ph = make_float2(0.f, 0.f);
         }
@@ -477,25 +501,25 @@ __global__ void __launch_bounds__(32 * WI *WJ, MINB) force_kernel(const ForcePar
     }
 
     // ---- a6: fixed-order reduction over the WJ warps that shared these i, then one partial per split
-    double out64[2][7];
+    double out64[NH][7];
 #pragma unroll
-    for (int h = 0; h < 2; ++h)
+    for (int h = 0; h < NH; ++h)
 #pragma unroll
         for (int c = 0; c < 7; ++c) out64[h][c] = acc64[(h * 7 + c) * NT];
     if constexpr (WJ > 1) {
         double *red = reinterpret_cast<double *>(smem_raw);     // reuse the tile ring: [WJ][7][IB]
         __syncthreads();                                         // every warp is out of the ring
 #pragma unroll
-        for (int h = 0; h < 2; ++h) {
-            const int il = wi * 64 + h * 32 + lane;
+        for (int h = 0; h < NH; ++h) {
+            const int il = wi * (32 * NH) + h * 32 + lane;
 #pragma unroll
             for (int c = 0; c < 7; ++c) red[((size_t)wj * 7 + c) * IB + il] = out64[h][c];
         }
         __syncthreads();
         if (wj == 0) {
 #pragma unroll
-            for (int h = 0; h < 2; ++h) {
-                const int il = wi * 64 + h * 32 + lane;
+            for (int h = 0; h < NH; ++h) {
+                const int il = wi * (32 * NH) + h * 32 + lane;
 #pragma unroll
                 for (int c = 0; c < 7; ++c) {
                     double ssum = out64[h][c];
@@ -507,7 +531,7 @@ __global__ void __launch_bounds__(32 * WI *WJ, MINB) force_kernel(const ForcePar
     }
     if (wj == 0) {
 #pragma unroll
-        for (int h = 0; h < 2; ++h) {
+        for (int h = 0; h < NH; ++h) {
             const int k = my_k[h];    // k < n_i_pad always
 #pragma unroll
             for (int c = 0; c < 7; ++c)
@@ -541,7 +565,7 @@ __global__ void __launch_bounds__(32 * W) finalize_kernel(int32_t n_i, int32_t n
     asm volatile("griddepcontrol.wait;" ::: "memory");
     if (blockIdx.y < 7) {
         const int q = blockIdx.y;
-        const int k = blockIdx.x * 32 + lane;          // k < n_i_pad always (n_i_pad is a multiple of 64)
+        const int k = blockIdx.x * 32 + lane;          // k < n_i_pad always (n_i_pad is a multiple of 32)
         const double *src = partial + (size_t)q * n_i_pad + k;
         const size_t stride = (size_t)7 * n_i_pad;
         double s = 0.0;

@@ -70,7 +70,8 @@ def test_plan_regular_fills_the_chip_and_covers_the_j_range():
     import paper_1504_03687_b200 as nb
     sm, per_sm = 148, 2
     conc = sm * per_sm
-    ovh = {512: 0.5, 256: 0.75, 128: 1.5, 64: 3.0}
+    ovh = {512: 0.5, 256: 0.75, 128: 1.5, 64: 3.0, 32: 3.0}
+    rate = {512: 1.0, 256: 1.01, 128: 1.025, 64: 1.03, 32: 1.11}     # cost per padded i-slot
     for N in (1024, 65536, 262144, 1048576, 1000003):
         ntiles = -(-N // 256)
         for n_i in (1, 32, 64, 100, 128, 257, 512, 1000, 4096, 8192, 65536, 131072):
@@ -78,16 +79,19 @@ def test_plan_regular_fills_the_chip_and_covers_the_j_range():
                 continue
             p = nb.nb_plan_regular(N, n_i, sm, per_sm)
             ib, S, tps = p["iblock"], p["jsplit"], p["tiles_per_split"]
-            assert ib == (512, 256, 128, 64)[p["variant"]]
+            assert ib == (512, 256, 128, 64, 32)[p["variant"]]
             pad = -(-n_i // ib) * ib
-            assert pad == min(-(-n_i // b) * b for b in (512, 256, 128, 64))        # least padded work
+            assert abs(pad * rate[ib] - min(-(-n_i // b) * b * rate[b] for b in rate)) < 1e-9 * pad   # least rate-weighted padded work
             assert 1 <= S <= ntiles and tps == -(-ntiles // S) and (S - 1) * tps < ntiles <= S * tps
             n_ib = pad // ib
             cost = lambda s: -(-(n_ib * -(-ntiles // -(-ntiles // s))) // conc) * (-(-ntiles // s) + ovh[ib])
             best = min(cost(s) for s in range(1, min(ntiles, 8192) + 1))
             assert cost(S) <= 1.01 * best
     p = nb.nb_plan_regular(1048576, 8192, sm, per_sm)
-    assert p["jsplit"] * (8192 // p["iblock"]) % conc == 0            # the headline block: whole waves
+    assert p["iblock"] == 512 and p["jsplit"] * (8192 // p["iblock"]) % conc == 0   # the headline block: whole waves
+    assert nb.nb_plan_regular(1048576, 32)["iblock"] == 32 and nb.nb_plan_regular(1048576, 64)["iblock"] == 64
+    assert nb.nb_plan_regular(1048576, 8256)["iblock"] == 64           # a ragged block takes the variant that pads least
+    assert nb.nb_plan_regular(1048576, 131072)["iblock"] == 512
     with pytest.raises(nb.NbregError):
         nb.nb_plan_regular(1024, 2048)
 

@@ -125,7 +125,7 @@ def test_block_sizes_ragged_N(oracle, n_i):
     assert ctx.info("last_grid") >= 1
 
 
-@pytest.mark.parametrize("variant", [0, 1, 2, 3])
+@pytest.mark.parametrize("variant", [0, 1, 2, 3, 4])
 @pytest.mark.parametrize("jsplit", [1, 3, 36])
 def test_forced_variant_and_split_agree(oracle, variant, jsplit):
     """Split-j vs single pass and every thread mapping: identical neighbour sets, sums equal to FP64
