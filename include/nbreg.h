@@ -189,6 +189,25 @@ int nb_correct(nb_ctx *ctx, double t, int32_t n, const int32_t *idx, const doubl
 int nb_get_state(nb_ctx *ctx, double *m, double *x0, double *v0, double *a0, double *j0, double *t0,
                  double *dt);
 
+/* ---- j-sharding ("each GPU has a similar particle dataset size ...
+ * all GPUs in the same node together access the complete particle dataset").  A context then holds a
+ * contiguous SHARD of the bodies -- nb_open(N_shard), nb_set_j of the shard's bodies, nb_predict_all(t)
+ * -- and nb_set_j_offset gives the global index of its body 0.  nb_regular_shard sums the shard's
+ * contribution to the regular force of ANY active block: idx_i[k] are GLOBAL indices and the active
+ * particles' own FP64 state arrives as istate[14][n_i] (rows m, x0[3], v0[3], a0[3], j0[3], t0 -- the
+ * component order of the arguments of nb_set_j), predicted to t with the predictor's own arithmetic, so
+ * that a particle of this shard meets its own record at r = 0 exactly and is skipped by global index.
+ * Outputs are this shard's PARTIAL results: acc, jerk, pot over the shard's j; nnb = neighbours found
+ * in the shard; nblist rows = their GLOBAL indices, ascending; overflow = (nnb > nb_cap) for the shard
+ * alone.  The caller adds acc / jerk / pot / nnb over the shards (an all-reduce of 7 doubles + 1 int per
+ * active particle), concatenates the list rows in shard order (= ascending j) and sets
+ * overflow = total nnb > nb_cap.  n_i may exceed the shard size.  DEVICE pointers.
+ * Requires nb_predict_all(t) with the same t. */
+int nb_set_j_offset(nb_ctx *ctx, int64_t j_offset);
+int nb_regular_shard(nb_ctx *ctx, double t, int32_t n_i, const int32_t *idx_i, const double *istate,
+                     const double *h2_i, double *acc, double *jerk, double *pot, int32_t *nnb,
+                     int32_t *nblist, int32_t *overflow);
+
 /* Tuning / introspection.  Keys: */
 enum {
     NB_INFO_KERNEL_LAUNCHES = 0, /* get: kernels launched by this context so far                   */

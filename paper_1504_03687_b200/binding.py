@@ -59,6 +59,8 @@ def load_library(build: bool = True) -> ctypes.CDLL:
     lib.nb_next_block.argtypes = [_vp, ctypes.POINTER(dbl), ctypes.POINTER(i32), _vp]
     lib.nb_correct.argtypes = [_vp, dbl, i32, _vp, _vp, _vp, dbl, dbl]
     lib.nb_get_state.argtypes = [_vp] + [_vp] * 7
+    lib.nb_set_j_offset.argtypes = [_vp, i64]
+    lib.nb_regular_shard.argtypes = [_vp, dbl, i32] + [_vp] * 9
     lib.nb_plan_regular.argtypes = [i64, i64, i32, i32] + [ctypes.POINTER(i32)] * 4
     lib.nb_plan_chunks.argtypes = [i64, i32, ctypes.POINTER(i64), ctypes.POINTER(i32)]
     lib.nb_get_info.argtypes = [_vp, i32, ctypes.POINTER(i64)]
@@ -255,6 +257,23 @@ class NbContext:
         args.append(_vp(st["dt"].data_ptr()) if with_steps else _vp())
         _check(self._lib.nb_get_state(self._ctx, *args), "nb_get_state", self._ctx)
         return st
+
+    # -- j-sharding
+    def set_j_offset(self, j_offset: int):
+        _check(self._lib.nb_set_j_offset(self._ctx, int(j_offset)), "nb_set_j_offset", self._ctx)
+
+    def regular_shard(self, t: float, idx_i, istate, h2_i, acc, jerk, pot, nnb, nblist, overflow):
+        """This shard's partial sums / local neighbours for a block given by GLOBAL indices and the active
+        particles' gathered FP64 state istate[14][n_i]."""
+        import torch
+        n, f8, i4 = int(idx_i.numel()), torch.float64, torch.int32
+        if n == 0:
+            return
+        args = [_dev_ptr(idx_i, i4, n, "idx_i"), _dev_ptr(istate, f8, 14 * n, "istate"), _dev_ptr(h2_i, f8, n, "h2_i"),
+                _dev_ptr(acc, f8, 3 * n, "acc"), _dev_ptr(jerk, f8, 3 * n, "jerk"), _dev_ptr(pot, f8, n, "pot"),
+                _dev_ptr(nnb, i4, n, "nnb"), _dev_ptr(nblist, i4, n * self.cap, "nblist"),
+                _dev_ptr(overflow, i4, n, "overflow")]
+        _check(self._lib.nb_regular_shard(self._ctx, float(t), n, *args), "nb_regular_shard", self._ctx)
 
     # -- the path (host buffers: numpy arrays or CPU tensors, pinned or not)
     def set_j_host(self, m, x0, v0, a0, j0, t0):

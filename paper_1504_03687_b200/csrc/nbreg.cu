@@ -43,7 +43,8 @@ struct nb_ctx {
     double *aos = nullptr;                  // [N][16] gather copy (one 128 B line per body)
     int sort_P = 0; size_t sort_smem_max = 0;   // list-row sort: power of two >= cap; opt-in dynamic smem limit
     float *rec = nullptr;                   // predicted records [Npad / TJ][RECF][TJ]
-    int32_t *cnt = nullptr;                 // [N] zero between calls
+    int32_t *cnt = nullptr;                 // [cnt_n >= N] zero between calls
+    int64_t cnt_n = 0;
     double *partial = nullptr;  size_t partial_bytes = 0;
     // staging for the HOST variants (lazy)
     double *stage_j = nullptr;              // 14 N doubles
@@ -68,6 +69,7 @@ struct nb_ctx {
     int64_t launches = 0;
     int64_t last_S = 0, last_iblock = 0, last_grid = 0, last_variant = -1;
     int64_t force_S = 0, force_variant = -1, step_chunks = 0;
+    int64_t j_offset = 0;                           // global index of body 0 (j-sharding)
     std::unordered_map<int64_t, int> plan_cache;   // (j-tiles, variant, i-blocks) -> S
     // optional event bracketing of the force kernel (NB_TUNE_PROFILE)
     static constexpr int PROF_RING = 256;
@@ -217,6 +219,7 @@ int launch_force_range(nb_ctx *c, int vi, int32_t n_i, const int32_t *idx_i, con
     p.n_i = n_i; p.n_i_pad = (int32_t)(n_ib * v.iblock);
     p.irec = irec;
     p.tile0 = (int32_t)tile0; p.ntiles = (int32_t)tile1; p.split0 = (int32_t)split0;
+    p.j_offset = irec ? (int32_t)c->j_offset : 0;
     p.tiles_per_split = (int32_t)((tile1 - tile0 + S - 1) / S);
     p.cap = c->cap; p.cnt = c->cnt; p.nblist = nblist; p.partial = c->partial;
     const dim3 grid((unsigned)n_ib, (unsigned)S);
@@ -368,6 +371,7 @@ int nb_open(int64_t N, int32_t nb_cap, nb_ctx **out) {
     NB_CUDA(c, cudaMalloc(&c->rec, sizeof(float) * RECF * c->Npad));
     NB_CUDA(c, cudaMalloc(&c->cnt, sizeof(int32_t) * c->N));
     NB_CUDA(c, cudaMemset(c->cnt, 0, sizeof(int32_t) * c->N));
+    c->cnt_n = c->N;
     {   // ascending list rows: one warp per row, P ints of shared memory each (finalize_kernel)
         int P = 32;
         while (P < nb_cap) P <<= 1;
@@ -778,6 +782,56 @@ int nb_get_state(nb_ctx *c, double *m, double *x0, double *v0, double *a0, doubl
     NB_CUDA(c, cudaGetLastError());
     c->launches += 1;
     return NB_OK;
+}
+
+int nb_set_j_offset(nb_ctx *c, int64_t j_offset) {
+    int rc = check_live(c);
+    if (rc != NB_OK) return rc;
+    if (j_offset < 0 || j_offset + c->N > ((int64_t)1 << 31) - 1) return NB_EINVAL;
+    c->j_offset = j_offset;
+    return NB_OK;
+}
+
+int nb_regular_shard(nb_ctx *c, double t, int32_t n_i, const int32_t *idx_i, const double *istate, const double *h2_i,
+                     double *acc, double *jerk, double *pot, int32_t *nnb, int32_t *nblist, int32_t *overflow) {
+    int rc = check_live(c);
+    if (rc != NB_OK) return rc;
+    if (n_i < 0) return NB_EINVAL;
+    if (!c->have_pred) return NB_ESTATE;
+    if (n_i == 0) return NB_OK;
+    if (!idx_i || !istate || !h2_i || !acc || !jerk || !pot || !nnb || !nblist || !overflow) return NB_EINVAL;
+    const int vi = pick_variant(c, n_i);
+    const Variant &v = c->var[vi];
+    const int64_t n_ib = (n_i + v.iblock - 1) / v.iblock, n_i_pad = n_ib * v.iblock;
+    const int64_t ntiles = c->Npad / TJ;
+    const int S = pick_split(c, v, n_ib, ntiles);
+    rc = ensure_partial(c, (size_t)S * 7 * n_i_pad * sizeof(double));
+    if (rc != NB_OK) return rc;
+    if (n_i_pad > c->ist_n) {
+        NB_CUDA(c, cudaStreamSynchronize(c->stream));
+        cudaFree(c->d_ist); cudaFree(c->irec); cudaFreeHost(c->h_ist);
+        c->d_ist = nullptr; c->irec = nullptr; c->h_ist = nullptr; c->ist_n = 0;
+        const int64_t n = std::max<int64_t>(n_i_pad, 1024) * 5 / 4;
+        NB_CUDA(c, cudaMallocHost(&c->h_ist, sizeof(double) * 14 * n));
+        NB_CUDA(c, cudaMalloc(&c->d_ist, sizeof(double) * 14 * n));
+        NB_CUDA(c, cudaMalloc(&c->irec, sizeof(float) * RECF * n));
+        c->ist_n = n;
+    }
+    if ((int64_t)n_i > c->cnt_n) {      // the row counters are indexed by k: a block may be larger than the shard
+        NB_CUDA(c, cudaStreamSynchronize(c->stream));
+        cudaFree(c->cnt); c->cnt = nullptr;
+        NB_CUDA(c, cudaMalloc(&c->cnt, sizeof(int32_t) * n_i));
+        NB_CUDA(c, cudaMemsetAsync(c->cnt, 0, sizeof(int32_t) * n_i, c->stream));
+        c->cnt_n = n_i;
+    }
+    IStateSrc isrc = {};
+    isrc.ist = istate;
+    predict_i_kernel<false><<<(unsigned)((n_i + 255) / 256), 256, 0, c->stream>>>(n_i, (int32_t)n_i_pad, t, isrc, c->irec);
+    NB_CUDA(c, cudaGetLastError());
+    c->launches += 1;
+    rc = launch_force_range(c, vi, n_i, idx_i, h2_i, c->irec, nblist, 0, ntiles, S, 0);
+    if (rc != NB_OK) return rc;
+    return launch_finalize(c, n_i, n_i_pad, S, acc, jerk, pot, nnb, nblist, overflow);
 }
 
 int nb_get_info(nb_ctx *c, int32_t key, int64_t *value) {

@@ -256,6 +256,8 @@ struct ForceParams {
     int32_t tile0;                // first j-tile of this launch (0 unless the j-range arrives in chunks)
     int32_t ntiles;               // end of this launch's j-tile range (Npad / TJ for a whole pass)
     int32_t split0;               // first row of `partial` this launch writes
+    int32_t j_offset;             // global index of this context's body 0 (j-sharding; 0 otherwise): list entries and
+                                  // the self test use global indices, idx_i is global when irec is given
     int32_t tiles_per_split;      // contiguous tiles per blockIdx.y
     int32_t cap;
     int32_t *cnt;                 // [>= n_i] neighbour counters, zero on entry (finalize re-zeroes)
@@ -418,7 +420,7 @@ __global__ void __launch_bounds__(32 * WI *WJ, MINB) force_kernel(const ForcePar
         const int s = it % NSTAGE;
         mbar_wait(&full[s], (uint32_t)((it / NSTAGE) & 1));
         const float *tsub = srec + (size_t)s * TILE_FLOATS + wj * SUB;      // &tile[0][wj * SUB]
-        const int32_t jbase = (tile_begin + it) * TJ + wj * SUB;
+        const int32_t jbase = p.j_offset + (tile_begin + it) * TJ + wj * SUB;
 
 #pragma unroll GROUP_UNROLL
         for (int g = 0; g < SUB; g += UNROLL_J) {

@@ -338,6 +338,55 @@ def test_step_host_errors_and_empty_block():
     ctx.close()
 
 
+def test_j_sharding_three_shards_sum_to_the_whole(oracle):
+    """three contiguous j-shards (three contexts, run one after the other on this GPU)
+    each evaluate their part of the same active block with nb_regular_shard; the partial sums added and
+    the list rows concatenated in shard order must equal the unsharded call and the oracle."""
+    import paper_1504_03687_b200 as nb
+    from paper_1504_03687_b200 import parallel as par
+    cfg = nbgen.make_config(2, N=20011, n_i=333)
+    N, cap, t = cfg["N"], cfg["cap"], cfg["t"]
+    idx, h2 = _dev(cfg["idx_i"], torch.int32), _dev(cfg["h2_i"])
+    whole = gpu_regular(open_ctx(cfg), cfg["idx_i"], cfg["h2_i"])
+    b = par.shard_bounds(N, 3)
+    assert b[0] == 0 and b[-1] == N and all(x % 256 == 0 for x in b[:-1]) and len(set(b)) == 4
+    states = [{k: _dev(cfg[k][b[r]:b[r + 1]]) for k in par.STATE_KEYS} for r in range(3)]
+    ist = sum(par.gather_istate(states[r], b[r], idx) for r in range(3))          # what the all-reduce would give
+    assert (idx.cpu().numpy() >= b[2]).any() and (idx.cpu().numpy() < b[1]).any()  # active bodies in first and last shard
+    parts = []
+    for r in range(3):
+        n_loc = b[r + 1] - b[r]
+        ctx = nb.nb_open(n_loc, cap)
+        nb.nb_set_j(ctx, *(states[r][k] for k in par.STATE_KEYS))
+        ctx.set_j_offset(b[r])
+        ctx.predict_all(t)
+        part = dict(acc=torch.empty((333, 3), dtype=torch.float64, device="cuda"),
+                    jerk=torch.empty((333, 3), dtype=torch.float64, device="cuda"),
+                    pot=torch.empty(333, dtype=torch.float64, device="cuda"),
+                    nnb=torch.empty(333, dtype=torch.int32, device="cuda"),
+                    nblist=torch.full((333, cap), -1, dtype=torch.int32, device="cuda"),
+                    overflow=torch.empty(333, dtype=torch.int32, device="cuda"))
+        ctx.regular_shard(t, idx, ist.contiguous(), h2, **part)
+        ctx.synchronize()
+        parts.append(part)
+        ctx.close()
+    rows = torch.stack([p_["nblist"] for p_ in parts]); cnts = torch.stack([p_["nnb"].long() for p_ in parts])
+    nblist, nnb, ovf = par.merge_list_rows(rows, cnts, cap)
+    got = dict(acc=sum(p_["acc"] for p_ in parts), jerk=sum(p_["jerk"] for p_ in parts), pot=sum(p_["pot"] for p_ in parts),
+               nnb=nnb, nblist=nblist, overflow=ovf)
+    got = parity.to_numpy(got)
+    assert np.array_equal(got["nnb"], whole["nnb"]) and np.array_equal(got["overflow"], whole["overflow"])
+    for k in range(333):
+        if got["nnb"][k] <= cap:         # (an overflowed row keeps ANY cap of its neighbours, R10)
+            c = got["nnb"][k]
+            assert np.array_equal(got["nblist"][k, :c], whole["nblist"][k, :c])   # shard order = ascending j
+    for key in ("acc", "jerk", "pot"):
+        assert np.abs(got[key] - whole[key]).max() <= 5e-7 * np.abs(whole[key]).max()
+    xp, vp = oracle.predict(cfg["x0"], cfg["v0"], cfg["a0"], cfg["j0"], cfg["t0"], t)
+    ref = parity.oracle_reference(oracle, cfg["m"], xp, vp, cfg["idx_i"], cfg["h2_i"], cap)
+    print("j-sharded x3", parity.compare(got, ref, cap))
+
+
 # ----------------------------------------------------------------------------- full size (bench launch config)
 
 def test_full_size_million_body_sampled(oracle):
