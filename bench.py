@@ -45,6 +45,8 @@ def parse():
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--variant", type=int, default=-1, help="force a force-kernel variant (tuning experiments)")
     ap.add_argument("--no-sweep", action="store_true")
+    ap.add_argument("--all-configs", action="store_true",
+                    help="also sweep BASELINE.json configs 3 (N=262144) and 5 (King core, overflowing rows); slower start-up")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -352,28 +354,49 @@ def run_b200(args):
         "share_of_step": force_ms / (ms / args.steps),
     }
 
-    # ---- sweep vs block size (the metric is "vs block size"): nb_regular alone, min of 3
+    # ---- sweep vs block size (the metric is "vs block size"): nb_regular alone and predict_all + regular,
+    #      3 warm-ups, 10 timed repeats each, median and min (SURVEY 8(d) timing protocol)
+    def sweep_config(sctx, scfg, sizes, sN):
+        rows = []
+        st_pred = float(scfg["t"])
+        for n in sizes:
+            if n > sN:
+                continue
+            si, sh = nbgen.active_block(scfg, n)
+            si_d, sh_d = torch.from_numpy(si).to(dev), f64(sh)
+            so = sctx.regular_alloc(si_d, sh_d)
+            for _ in range(2):
+                sctx.regular(si_d, sh_d, **so)
+            torch.cuda.synchronize()
+            t_reg, t_blk = [], []
+            for _ in range(10):
+                a, b, c2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+                a.record(stream); sctx.regular(si_d, sh_d, **so); b.record(stream)
+                sctx.predict_all(st_pred); sctx.regular(si_d, sh_d, **so); c2.record(stream)
+                torch.cuda.synchronize()
+                t_reg.append(a.elapsed_time(b)); t_blk.append(b.elapsed_time(c2))
+            best, med = min(t_reg), float(np.median(t_reg))
+            rate = float(n) * sN / (best * 1e-3)
+            rows.append({"n_i": n, "ms": best, "ms_median": med, "ms_predict_plus_regular": float(np.median(t_blk)),
+                         "pairs_per_s": rate, "frac_fp32_peak": rate * FLOP_PER_INTERACTION / 1e12 / peak_tflops,
+                         "variant": sctx.info("last_variant"), "jsplit": sctx.info("last_jsplit"),
+                         "overflow_rows": int(so["overflow"].sum()), "nnb_mean": float(so["nnb"].float().mean())})
+            del so
+        return rows
+
     sweep = None
     if not args.no_sweep and world == 1:
-        sweep = []
-        for n in [32] + list(cfg["sweep"]):        # 32: the j-packed tiny-block variant (config 5's smallest block)
-            if n > N:
-                continue
-            si, sh = nbgen.active_block(cfg, n)
-            si_d, sh_d = torch.from_numpy(si).to(dev), f64(sh)
-            so = ctx.regular_alloc(si_d, sh_d)
-            torch.cuda.synchronize()
-            best = 1e30
-            for _ in range(3):
-                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-                a.record(stream); ctx.regular(si_d, sh_d, **so); b.record(stream)
-                torch.cuda.synchronize()
-                best = min(best, a.elapsed_time(b))
-            rate = float(n) * N / (best * 1e-3)
-            sweep.append({"n_i": n, "ms": best, "pairs_per_s": rate,
-                          "frac_fp32_peak": rate * FLOP_PER_INTERACTION / 1e12 / peak_tflops,
-                          "variant": ctx.info("last_variant"), "jsplit": ctx.info("last_jsplit")})
-            del so
+        sweep = sweep_config(ctx, cfg, [32] + list(cfg["sweep"]), N)   # 32: the j-packed tiny-block variant
+    other = None
+    if args.all_configs and world == 1 and N == 1048576:
+        other = {}
+        for kcfg in (3, 5):
+            ocfg = nbgen.make_config(kcfg)
+            octx = nb.nb_open(ocfg["N"], ocfg["cap"], stream)
+            octx.set_j(*[f64(ocfg[k]) for k in ("m", "x0", "v0", "a0", "j0", "t0")])
+            octx.predict_all(float(ocfg["t"]))
+            other[ocfg["name"]] = {"N": ocfg["N"], "nb_cap": ocfg["cap"], "sweep": sweep_config(octx, ocfg, ocfg["sweep"], ocfg["N"])}
+            octx.close()
 
     # ---- the steps either side of the path, timed alone; not part of `value`
     extras = None
@@ -431,7 +454,7 @@ def run_b200(args):
                    **plan},
         "frac_fp32_peak": value / world * FLOP_PER_INTERACTION / 1e12 / peak_tflops,
         "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
-        "cpu_baseline": cpu, "sweep": sweep, "extras": extras, "peaks_source": pk_src,
+        "cpu_baseline": cpu, "sweep": sweep, "other_configs": other, "extras": extras, "peaks_source": pk_src,
     }
     print(json.dumps(line), flush=True)
     if world > 1:
