@@ -23,7 +23,11 @@ is reproduced exactly (rational arithmetic); a2, a3 are that polynomial's deriva
 Kepler orbit with a shared step shows fourth-order convergence of the energy error; the active set
 equals the prefix of the paper's step-sorted list; block-step invariants (t0 multiple of dt, steps at
 most double, doubling only at commensurate times) hold along an integration; a Plummer sphere
-conserves energy.
+conserves energy.  ``aarseth_step``: for harmonic motion a(t) = A cos(wt) e the criterion is exactly
+sqrt(eta) / w at every phase and amplitude (closed form), plus two cases worked by hand with a2 handed
+in at the start of the step (so "a2 advanced by dt a3" is pinned); ``initial_step``: hand cases on and
+off a power of two and at the dt_max cap.  Thirteen single-term mutations of those two functions (no
+sqrt, swapped or dropped products, wrong powers, a2 at the start, ceil for floor, ...) each fail a test.
 """
 from __future__ import annotations
 

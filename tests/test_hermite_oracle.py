@@ -143,3 +143,67 @@ def test_block_step_integration_conserves_energy_and_keeps_the_block_invariants(
     st2 = H.integrate(m, x, v, t_end=0.25, eta=0.0025, eta_s=0.0025, dt_max=2.0**-4, force=_direct_force)
     e2 = energy(st2["x0"], st2["v0"])
     assert abs((e2 - e0) / e0) < 0.5 * abs((e1 - e0) / e0) + 1e-12
+
+
+# ----------------------------------------------------------------------------- time-step criterion (DESIGN R28)
+
+def _harmonic(A, w, ph, e):
+    """a(t) = A cos(phi) e and its first three time derivatives at phase phi = w t (closed forms)."""
+    e = np.asarray(e, dtype=float) / np.linalg.norm(e)
+    a = A * np.cos(ph) * e
+    j = -A * w * np.sin(ph) * e
+    a2 = -A * w * w * np.cos(ph) * e
+    a3 = A * w**3 * np.sin(ph) * e
+    return a, j, a2, a3
+
+
+def test_aarseth_step_is_sqrt_eta_over_omega_for_harmonic_motion():
+    """For a(t) = A cos(wt) e the products in Aarseth's criterion are |a||a2| + |j|^2 = A^2 w^2 and
+    |j||a3| + |a2|^2 = A^2 w^4 at EVERY phase, so dt_req = sqrt(eta) / w exactly -- independent of A and
+    of the phase.  A missing sqrt, a wrong power, swapped products or a2 not advanced to the end of the
+    step (it is handed in at the START of the step: a2_0 = a2(t1) - dt a3) all break the constancy."""
+    rows = []
+    for A, w, eta in ((1.0, 1.0, 0.02), (3.5, 7.0, 0.01), (0.02, 0.25, 0.04), (40.0, 31.0, 0.0025)):
+        for ph in (0.0, 0.3, 0.5 * np.pi, 1.1, 2.0, 3.0, 4.4, 6.0):
+            for dt in (0.5, 2.0**-5):
+                a, j, a2, a3 = _harmonic(A, w, ph, (1.0, -2.0, 0.5))
+                rows.append((a, j, a2 - dt * a3, a3, dt, eta, np.sqrt(eta) / w))
+    col = lambda q: np.array([r[q] for r in rows])
+    for eta in sorted({r[5] for r in rows}):
+        sel = col(5) == eta
+        got = H.aarseth_step(col(0)[sel], col(1)[sel], col(2)[sel], col(3)[sel], col(4)[sel], eta)
+        np.testing.assert_allclose(got, col(6)[sel], rtol=1e-12, atol=0)
+
+
+def test_aarseth_step_hand_case_with_a2_advanced_to_the_end_of_the_step():
+    """Worked by hand from the formula DESIGN R28 cites (Aarseth 1985; Makino & Aarseth 1992):
+        dt_req = sqrt( eta (|a||a2| + |j|^2) / (|j||a3| + |a2|^2) ),   a2 = a2(t0) + dt a3.
+    a1 = (0,0,3): |a| = 3;  j1 = (4,0,0): |j| = 4;  a3 = (1.5,0,0): |a3| = 1.5;  dt = 2;
+    a2(t0) = (-3,3,4)  ->  a2 at the end = (-3,3,4) + 2 (1.5,0,0) = (0,3,4): |a2| = 5.
+    numerator   = 3*5 + 4^2  = 31;   denominator = 4*1.5 + 5^2 = 31;   eta = 1/16  ->  dt_req = 1/4 exactly.
+    With a2 taken at the START (|a2|^2 = 34) the value is sqrt((3 sqrt(34) + 16) / (16 * 40)) = 0.2287...;
+    with the two products swapped it is sqrt((6 + 16) / (16 * (15 + 25))) = 0.1854...
+    Second row, unequal norms everywhere: a1 = (2,3,6) (7), j1 = (1,2,2) (3), a3 = (0,0,2) (2), dt = 1/2,
+    a2(t0) = (4,4,6) -> (4,4,7) (9): numerator 7*9 + 9 = 72, denominator 3*2 + 81 = 87, eta = 0.02:
+    dt_req = sqrt(0.02 * 72 / 87) = sqrt(1.44 / 87) = 1.2 / sqrt(87) = 0.128653504..."""
+    a1 = np.array([[0.0, 0.0, 3.0], [2.0, 3.0, 6.0]])
+    j1 = np.array([[4.0, 0.0, 0.0], [1.0, 2.0, 2.0]])
+    a2_0 = np.array([[-3.0, 3.0, 4.0], [4.0, 4.0, 6.0]])
+    a3 = np.array([[1.5, 0.0, 0.0], [0.0, 0.0, 2.0]])
+    dt = np.array([2.0, 0.5])
+    assert H.aarseth_step(a1[:1], j1[:1], a2_0[:1], a3[:1], dt[:1], 1.0 / 16.0)[0] == 0.25
+    got = H.aarseth_step(a1[1:], j1[1:], a2_0[1:], a3[1:], dt[1:], 0.02)[0]
+    assert abs(got - 0.128653504180535) < 1e-14              # 1.2 / sqrt(87) = 1.2 / 9.327379053088816
+
+
+def test_initial_step_hand_cases():
+    """dt = largest power of 0.5 not above min(eta_s |a| / |j|, dt_max), by hand:
+    |a| = 5, |j| = 2, eta_s = 0.02 -> 0.05 -> 2^-5 (0.03125 <= 0.05 < 0.0625); capped by dt_max = 2^-6;
+    |a| = 1, |j| = 4, eta_s = 1 -> exactly 2^-2 stays 2^-2 (floor of an exact power);
+    |a| = 13, |j| = 1, eta_s = 0.01 -> 0.13 -> 2^-3."""
+    a = np.array([[3.0, 4.0, 0.0], [3.0, 4.0, 0.0], [0.0, 1.0, 0.0], [3.0, 4.0, 12.0]])
+    j = np.array([[0.0, 0.0, 2.0], [0.0, 0.0, 2.0], [0.0, 0.0, 4.0], [1.0, 0.0, 0.0]])
+    assert H.initial_step(a[:1], j[:1], 0.02, 1.0)[0] == 2.0**-5
+    assert H.initial_step(a[1:2], j[1:2], 0.02, 2.0**-6)[0] == 2.0**-6
+    assert H.initial_step(a[2:3], j[2:3], 1.0, 1.0)[0] == 2.0**-2
+    assert H.initial_step(a[3:], j[3:], 0.01, 1.0)[0] == 2.0**-3
