@@ -47,7 +47,8 @@ typedef struct nb_ctx nb_ctx; /* opaque; owns all internal device memory */
 enum {
     NB_OK = 0,
     NB_EINVAL = 1, /* null pointer, N <= 0, nb_cap <= 0, n_i < 0 or n_i > N, unknown key            */
-    NB_ESTATE = 2, /* nb_predict_all before nb_set_j, nb_regular before nb_predict_all             */
+    NB_ESTATE = 2, /* nb_predict_all before nb_set_j, nb_regular before nb_predict_all; also: the
+                      current CUDA device is not the one the context was opened on                 */
     NB_ENOMEM = 3, /* device (or staging) allocation failed                                        */
     NB_ECUDA = 4   /* CUDA error (sticky); nb_last_cuda_error() returns the cudaError_t            */
 };
@@ -202,7 +203,8 @@ int nb_get_state(nb_ctx *ctx, double *m, double *x0, double *v0, double *a0, dou
  * alone.  The caller adds acc / jerk / pot / nnb over the shards (an all-reduce of 7 doubles + 1 int per
  * active particle), concatenates the list rows in shard order (= ascending j) and sets
  * overflow = total nnb > nb_cap.  n_i may exceed the shard size.  DEVICE pointers.
- * Requires nb_predict_all(t) with the same t. */
+ * Requires nb_predict_all(t) with the same t (checked: NB_ESTATE otherwise).  nb_regular / nb_regular_all on
+ * a context with an offset keep LOCAL indices in and out; nb_step_host returns NB_ESTATE there. */
 int nb_set_j_offset(nb_ctx *ctx, int64_t j_offset);
 int nb_regular_shard(nb_ctx *ctx, double t, int32_t n_i, const int32_t *idx_i, const double *istate,
                      const double *h2_i, double *acc, double *jerk, double *pot, int32_t *nnb,

@@ -35,6 +35,8 @@ struct nb_ctx {
     int64_t N = 0, Npad = 0, Ns = 0;
     int32_t cap = 0;
     int sm_count = 0;
+    int device = 0;                         // the CUDA device the context lives on
+    double pred_t = 0.0;                    // time of the last nb_predict_all / nb_step_host (valid when have_pred)
     cudaStream_t stream = nullptr;
     cudaError_t cuda_err = cudaSuccess;
     bool have_j = false, have_pred = false;
@@ -191,6 +193,8 @@ int plan_chunks_pure(int64_t ntiles, int64_t want, int64_t *ctile) {
 int check_live(nb_ctx *c) {
     if (!c) return NB_EINVAL;
     if (c->cuda_err != cudaSuccess) return NB_ECUDA;
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev != c->device) return NB_ESTATE;   // called with another device current
     return NB_OK;
 }
 
@@ -210,7 +214,7 @@ int ensure_partial(nb_ctx *c, size_t bytes) {
 // One force-kernel launch over the j-tiles [tile0, tile1) split S ways, writing partial rows
 // [split0, split0 + S).
 int launch_force_range(nb_ctx *c, int vi, int32_t n_i, const int32_t *idx_i, const double *h2_i, const float *irec,
-                       int32_t *nblist, int64_t tile0, int64_t tile1, int S, int64_t split0) {
+                       int64_t j_offset, int32_t *nblist, int64_t tile0, int64_t tile1, int S, int64_t split0) {
     const Variant &v = c->var[vi];
     const int64_t n_ib = (n_i + v.iblock - 1) / v.iblock;
     ForceParams p;
@@ -219,7 +223,7 @@ int launch_force_range(nb_ctx *c, int vi, int32_t n_i, const int32_t *idx_i, con
     p.n_i = n_i; p.n_i_pad = (int32_t)(n_ib * v.iblock);
     p.irec = irec;
     p.tile0 = (int32_t)tile0; p.ntiles = (int32_t)tile1; p.split0 = (int32_t)split0;
-    p.j_offset = irec ? (int32_t)c->j_offset : 0;
+    p.j_offset = (int32_t)j_offset;     // 0 except from nb_regular_shard (idx_i global there)
     p.tiles_per_split = (int32_t)((tile1 - tile0 + S - 1) / S);
     p.cap = c->cap; p.cnt = c->cnt; p.nblist = nblist; p.partial = c->partial;
     const dim3 grid((unsigned)n_ib, (unsigned)S);
@@ -289,7 +293,7 @@ int regular_device(nb_ctx *c, int32_t n_i, const int32_t *idx_i, const double *h
     const int64_t n_i_pad = n_ib * v.iblock;
     int rc = ensure_partial(c, (size_t)S * 7 * n_i_pad * sizeof(double));
     if (rc != NB_OK) return rc;
-    rc = launch_force_range(c, vi, n_i, idx_i, h2_i, nullptr, nblist, 0, ntiles, S, 0);
+    rc = launch_force_range(c, vi, n_i, idx_i, h2_i, nullptr, 0, nblist, 0, ntiles, S, 0);
     if (rc != NB_OK) return rc;
     return launch_finalize(c, n_i, n_i_pad, S, acc, jerk, pot, nnb, nblist, overflow);
 }
@@ -361,7 +365,7 @@ int nb_open(int64_t N, int32_t nb_cap, nb_ctx **out) {
         delete c;
         return NB_ECUDA;
     }
-    c->N = N; c->cap = nb_cap;
+    c->N = N; c->cap = nb_cap; c->device = dev;
     c->Npad = (N + TJ - 1) / TJ * TJ;
     c->Ns = c->Npad;
     c->sm_count = prop.multiProcessorCount;
@@ -376,11 +380,11 @@ int nb_open(int64_t N, int32_t nb_cap, nb_ctx **out) {
         int P = 32;
         while (P < nb_cap) P <<= 1;
         c->sort_P = P;
+        // The attribute is per function and per device, NOT per context: every nb_open sets the same fixed
+        // maximum, so a later context with a smaller cap cannot lower the limit under an older one.
         c->sort_smem_max = 200 * 1024;
-        const int s4 = (int)std::min<size_t>(c->sort_smem_max, (size_t)4 * P * sizeof(int32_t));
-        const int s16 = (int)std::min<size_t>(c->sort_smem_max, (size_t)16 * P * sizeof(int32_t));
-        NB_CUDA(c, cudaFuncSetAttribute(finalize_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, s4));
-        NB_CUDA(c, cudaFuncSetAttribute(finalize_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, s16));
+        NB_CUDA(c, cudaFuncSetAttribute(finalize_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->sort_smem_max));
+        NB_CUDA(c, cudaFuncSetAttribute(finalize_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->sort_smem_max));
     }
     NB_CUDA(c, (setup_variant<8, 1, 2>(c->var[0], VAR_OVH[0])));
     NB_CUDA(c, (setup_variant<4, 2, 2>(c->var[1], VAR_OVH[1])));
@@ -501,6 +505,7 @@ int nb_predict_all(nb_ctx *c, double t) {
     NB_CUDA(c, cudaGetLastError());
     c->launches += 1;
     c->have_pred = true;
+    c->pred_t = t;
     return NB_OK;
 }
 
@@ -560,6 +565,7 @@ int nb_step_host(nb_ctx *c, const double *m, const double *x0, const double *v0,
     if (rc != NB_OK) return rc;
     if (!m || !x0 || !v0 || !a0 || !j0 || !t0) return NB_EINVAL;
     if (n_i < 0 || n_i > c->N) return NB_EINVAL;
+    if (c->j_offset != 0) return NB_ESTATE;      // a shard context: blocks go through nb_regular_shard
     if (n_i == 0) {
         rc = nb_set_j_host(c, m, x0, v0, a0, j0, t0);
         if (rc == NB_OK) rc = nb_predict_all(c, t);
@@ -681,6 +687,7 @@ int nb_step_host(nb_ctx *c, const double *m, const double *x0, const double *v0,
     }
     c->have_j = true;
     c->have_pred = true;
+    c->pred_t = t;
 
     NB_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_i, 0));
     if (zero_copy)
@@ -692,7 +699,7 @@ int nb_step_host(nb_ctx *c, const double *m, const double *x0, const double *v0,
     int64_t split0 = 0;
     for (int q = 0; q < nchunk; ++q) {
         NB_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_chunk[q], 0));
-        rc = launch_force_range(c, vi, n_i, c->st_idx, c->st_h2, c->irec, c->st_list, ctile[q], ctile[q + 1], S_c[q],
+        rc = launch_force_range(c, vi, n_i, c->st_idx, c->st_h2, c->irec, 0, c->st_list, ctile[q], ctile[q + 1], S_c[q],
                                 split0);
         if (rc != NB_OK) return rc;
         split0 += S_c[q];
@@ -797,7 +804,7 @@ int nb_regular_shard(nb_ctx *c, double t, int32_t n_i, const int32_t *idx_i, con
     int rc = check_live(c);
     if (rc != NB_OK) return rc;
     if (n_i < 0) return NB_EINVAL;
-    if (!c->have_pred) return NB_ESTATE;
+    if (!c->have_pred || t != c->pred_t) return NB_ESTATE;   // the shard's records must be at the same time t
     if (n_i == 0) return NB_OK;
     if (!idx_i || !istate || !h2_i || !acc || !jerk || !pot || !nnb || !nblist || !overflow) return NB_EINVAL;
     const int vi = pick_variant(c, n_i);
@@ -829,7 +836,7 @@ int nb_regular_shard(nb_ctx *c, double t, int32_t n_i, const int32_t *idx_i, con
     predict_i_kernel<false><<<(unsigned)((n_i + 255) / 256), 256, 0, c->stream>>>(n_i, (int32_t)n_i_pad, t, isrc, c->irec);
     NB_CUDA(c, cudaGetLastError());
     c->launches += 1;
-    rc = launch_force_range(c, vi, n_i, idx_i, h2_i, c->irec, nblist, 0, ntiles, S, 0);
+    rc = launch_force_range(c, vi, n_i, idx_i, h2_i, c->irec, c->j_offset, nblist, 0, ntiles, S, 0);
     if (rc != NB_OK) return rc;
     return launch_finalize(c, n_i, n_i_pad, S, acc, jerk, pot, nnb, nblist, overflow);
 }
