@@ -55,9 +55,9 @@ enum {
 
 /* Create a context for N j-particles and a neighbour-list capacity of nb_cap entries per active
  * particle (north_star: nb_open(N); the capacity has to come from somewhere -- DESIGN.md R18).
- * Allocates: FP64 j-state twice (14 N doubles streamed by the predictor + a 128 B/body gather copy),
- * predicted records (40 B per particle, padded), counters,
- * split-j scratch (grown on demand). */
+ * Allocates: the FP64 j-state (14 N doubles), predicted records (40 B per particle, padded), counters,
+ * split-j scratch (grown on demand); a second, 128 B/body gather copy of the state only when the first
+ * nb_irregular / nb_correct call asks for it. */
 int nb_open(int64_t N, int32_t nb_cap, nb_ctx **out);
 int nb_close(nb_ctx *ctx);
 
@@ -84,7 +84,10 @@ int nb_update_j(nb_ctx *ctx, int32_t n, const int32_t *idx, const double *m, con
 /* a2 "Pred." (Table 1): predict every particle to time t,
  *     dt = t - t0[j];  xp = x0 + v0 dt + a0 dt^2/2 + j0 dt^3/6;  vp = v0 + a0 dt + j0 dt^2/2
  * in FP64, and store the predicted record the force kernel reads (x as hi/lo FP32 pair, v and m
- * as FP32).  Any t (also t < t0[j]) is allowed.  Requires nb_set_j. */
+ * as FP32).  Any t (also t < t0[j]) is allowed.  Requires nb_set_j.
+ * The predictor kernel itself is launched by the first call that reads the records (NB_TUNE_FUSE_PREDICT):
+ * a block of <= 128 active particles predicts inside its force kernel instead -- same arithmetic, same
+ * records, results independent of which route was taken up to the summation order. */
 int nb_predict_all(nb_ctx *ctx, double t);
 
 /* Test/inspection hook: the predicted state exactly as the force kernel sees it, widened to FP64:
@@ -226,9 +229,27 @@ enum {
     NB_INFO_FORCE_KERNEL_NS = 20,    /* get: summed device time of the bracketed force-kernel launches,
                                         in ns (synchronises the stream)                             */
     NB_INFO_FORCE_KERNEL_COUNT = 21, /* get: number of bracketed launches in that sum               */
-    NB_TUNE_STEP_CHUNKS = 22         /* set: number of chunks nb_step_host sends the j-state in, 1..8
+    NB_TUNE_STEP_CHUNKS = 22,        /* set: number of chunks nb_step_host sends the j-state in, 1..8
                                         (1 = no overlap; sizes 1/2^(n-1), 1/2^(n-1), then doubling);
                                         0 = automatic (5 chunks from 524288 bodies, 3 from 131072)  */
+    NB_TUNE_FUSE_PREDICT = 23,       /* set 1 (default): nb_predict_all defers its kernel; a block of <= 128
+                                        active particles that follows predicts inside the force kernel
+                                        (reads the FP64 state, no predicted records written), any other
+                                        consumer writes the records first.  set 0: nb_predict_all launches
+                                        the predictor at once and nb_regular always reads the records      */
+    NB_TUNE_LOCAL_G_MILLI = 24,      /* set: 1000 G of the local-frame guard |x_i - c| <= G h_i under which a
+                                        warp differences positions in its own frame (default 4000; 0 = never:
+                                        hi/lo differencing everywhere)                                      */
+    NB_TUNE_STATS = 25,              /* set 1: count, from now on, the warps of the force kernel and those
+                                        that took the local frame; set 0: off                               */
+    NB_INFO_LOCAL_WARPS = 26,        /* get: warps that took the local frame since NB_TUNE_STATS was set    */
+    NB_INFO_TOTAL_WARPS = 27,        /* get: all warps since then (both synchronise the stream)             */
+    NB_INFO_LAST_FUSED = 28,         /* get: 1 if the last nb_regular predicted inside the force kernel     */
+    NB_TUNE_REORDER_MIN = 29,        /* set: blocks of at least this many active particles are put in Morton
+                                        order inside the library before the force kernel, so that the 64
+                                        particles of a warp sit close together and take the local frame
+                                        (default 4096; 0 = never).  Outputs keep the caller's order.        */
+    NB_INFO_LAST_REORDERED = 30      /* get: 1 if the last block was reordered                              */
 };
 int nb_get_info(nb_ctx *ctx, int32_t key, int64_t *value);
 int nb_set_tuning(nb_ctx *ctx, int32_t key, int64_t value);

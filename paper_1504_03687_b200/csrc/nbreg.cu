@@ -19,15 +19,14 @@ struct Variant {
     int it, wi, wj;          // i per thread, warps along i, warps along j
     int iblock;              // i-particles per CTA
     int threads;
+    size_t smem;             // dynamic shared memory of one CTA (ForceSmem<...>::TOTAL)
     double ovh_tiles;        // per-CTA fixed cost in units of one tile's compute (planning heuristic)
     int ctas_per_sm;         // from the occupancy API at nb_open
 };
 constexpr int NVARIANT = 5;
 constexpr int NAUTO = 5;        // variants the planner picks from; the rest only by NB_TUNE_FORCE_VARIANT
-constexpr size_t force_smem(int threads) {      // tile ring + FP64 sums + mbarriers + counters
-    return (size_t)NSTAGE * TILE_FLOATS * sizeof(float) + (size_t)14 * threads * sizeof(double) +
-           NSTAGE * sizeof(uint64_t) + 64;
-}
+constexpr int FUSED_FIRST = 2;  // variants 2..4 (128, 64, 32 i per CTA) also exist reading the FP64 state (fused predictor)
+constexpr double DEFAULT_LOCAL_G = 4.0;     // local-frame guard |x_i - c| <= G h_i
 
 }  // namespace
 
@@ -40,9 +39,22 @@ struct nb_ctx {
     cudaStream_t stream = nullptr;
     cudaError_t cuda_err = cudaSuccess;
     bool have_j = false, have_pred = false;
+    bool pred_pending = false;              // nb_predict_all(t) was called but the records are not written yet:
+                                            // a small block predicts inside the force kernel instead (fused path)
+    bool fuse = true;                       // NB_TUNE_FUSE_PREDICT
+    double local_g = DEFAULT_LOCAL_G;       // NB_TUNE_LOCAL_G_MILLI / 1000
+    unsigned int *stats = nullptr;          // {warps in the local frame, warps} since NB_TUNE_STATS was set
+    // Morton reordering of large blocks (reorder_block): sort scratch, bounding box
+    int64_t reorder_min = 4096;             // NB_TUNE_REORDER_MIN: blocks of at least this many particles; 0 = never
+    unsigned long long *sort_keys = nullptr;
+    int32_t *sort_vals = nullptr;           // after the sort: perm[slot] = k
+    uint32_t *sort_box = nullptr;
+    int64_t sort_n = 0;
+    int64_t last_reordered = 0;
     // device state owned by the library
     double *soa = nullptr;                  // [14][Ns]
-    double *aos = nullptr;                  // [N][16] gather copy (one 128 B line per body)
+    double *aos = nullptr;                  // [N][16] gather copy (one 128 B line per body); allocated and built by the
+                                            // first NEXT-2 / NEXT-3 call (ensure_aos), kept current from then on
     int sort_P = 0; size_t sort_smem_max = 0;   // list-row sort: power of two >= cap; opt-in dynamic smem limit
     float *rec = nullptr;                   // predicted records [Npad / TJ][RECF][TJ]
     int32_t *cnt = nullptr;                 // [cnt_n >= N] zero between calls
@@ -67,7 +79,9 @@ struct nb_ctx {
     int32_t *sel_counts = nullptr;                  // [ceil(N / SEL_CHUNK)]
     double *sel_result = nullptr, *h_sel_result = nullptr;   // {t_next, n_active}: device / pinned host
     // planning / introspection
-    Variant var[NVARIANT];
+    Variant var[NVARIANT];                  // reading the predicted records
+    Variant fvar[NVARIANT];                 // reading the FP64 state (entries FUSED_FIRST.. only)
+    int64_t last_fused = 0;
     int64_t launches = 0;
     int64_t last_S = 0, last_iblock = 0, last_grid = 0, last_variant = -1;
     int64_t force_S = 0, force_variant = -1, step_chunks = 0;
@@ -91,22 +105,22 @@ namespace {
         }                                           \
     } while (0)
 
-template <int WI, int WJ, int MINB, bool JP = false>
+template <int WI, int WJ, int MINB, bool JP = false, int SRC = SRC_REC>
 cudaError_t setup_variant(Variant &v, double ovh) {
-    static_assert(WJ == 1 || (size_t)WJ * 7 * 64 * WI * sizeof(double) <= force_smem(32 * WI * WJ), "WJ reduction reuses the ring");
     v.it = JP ? 1 : 2; v.wi = WI; v.wj = WJ; v.iblock = (JP ? 32 : 64) * WI; v.threads = 32 * WI * WJ; v.ovh_tiles = ovh;
-    auto k = force_kernel<WI, WJ, MINB, JP>;
-    cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)force_smem(32 * WI * WJ));
+    v.smem = ForceSmem<WI, WJ, JP, SRC>::TOTAL;
+    auto k = force_kernel<WI, WJ, MINB, JP, SRC>;
+    cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)v.smem);
     if (e != cudaSuccess) return e;
     int nb = 0;
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k, v.threads, force_smem(32 * WI * WJ));
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, k, v.threads, v.smem);
     v.ctas_per_sm = std::max(nb, 1);
     return e;
 }
 
-template <int WI, int WJ, int MINB, bool JP = false>
+template <int WI, int WJ, int MINB, bool JP = false, int SRC = SRC_REC>
 void launch_force(const Variant &v, dim3 grid, cudaStream_t st, const ForceParams &p) {
-    force_kernel<WI, WJ, MINB, JP><<<grid, v.threads, force_smem(32 * WI * WJ), st>>>(p);
+    force_kernel<WI, WJ, MINB, JP, SRC><<<grid, v.threads, v.smem, st>>>(p);
 }
 
 // i-particles per CTA, planning overhead (in tile units) and relative cost per padded i-slot of the
@@ -140,7 +154,8 @@ int plan_chunks_pure(int64_t ntiles, int64_t want, int64_t *ctile);
 
 int pick_split(nb_ctx *c, const Variant &v, int64_t n_ib, int64_t ntiles) {
     if (c->force_S > 0) return (int)std::min<int64_t>(c->force_S, ntiles);
-    const int64_t key = (ntiles << 32) ^ (n_ib * NVARIANT + (&v - c->var));
+    const bool fused = &v >= c->fvar && &v < c->fvar + NVARIANT;
+    const int64_t key = (ntiles << 32) ^ (n_ib * 2 * NVARIANT + (fused ? NVARIANT + (&v - c->fvar) : (&v - c->var)));
     auto hit = c->plan_cache.find(key);
     if (hit != c->plan_cache.end()) return hit->second;
     const int plan = plan_split(c, v, n_ib, ntiles);
@@ -213,13 +228,16 @@ int ensure_partial(nb_ctx *c, size_t bytes) {
 
 // One force-kernel launch over the j-tiles [tile0, tile1) split S ways, writing partial rows
 // [split0, split0 + S).
-int launch_force_range(nb_ctx *c, int vi, int32_t n_i, const int32_t *idx_i, const double *h2_i, const float *irec,
-                       int64_t j_offset, int32_t *nblist, int64_t tile0, int64_t tile1, int S, int64_t split0) {
-    const Variant &v = c->var[vi];
+int launch_force_range(nb_ctx *c, int vi, bool fused, int32_t n_i, const int32_t *idx_i, const double *h2_i,
+                       const float *irec, const int32_t *perm, int64_t j_offset, int32_t *nblist, int64_t tile0,
+                       int64_t tile1, int S, int64_t split0) {
+    const Variant &v = fused ? c->fvar[vi] : c->var[vi];
     const int64_t n_ib = (n_i + v.iblock - 1) / v.iblock;
     ForceParams p;
     p.rec = c->rec;
-    p.idx_i = idx_i; p.h2_i = h2_i;
+    p.soa = c->soa; p.Ns = c->Ns; p.t = c->pred_t;
+    p.g2 = (float)(c->local_g * c->local_g); p.stats = c->stats;
+    p.idx_i = idx_i; p.h2_i = h2_i; p.perm = perm;
     p.n_i = n_i; p.n_i_pad = (int32_t)(n_ib * v.iblock);
     p.irec = irec;
     p.tile0 = (int32_t)tile0; p.ntiles = (int32_t)tile1; p.split0 = (int32_t)split0;
@@ -229,12 +247,20 @@ int launch_force_range(nb_ctx *c, int vi, int32_t n_i, const int32_t *idx_i, con
     const dim3 grid((unsigned)n_ib, (unsigned)S);
     const int slot = (int)(c->prof_n % nb_ctx::PROF_RING);
     if (c->profile) NB_CUDA(c, cudaEventRecord(c->ev0[slot], c->stream));
-    switch (vi) {
-        case 0: launch_force<8, 1, 2>(v, grid, c->stream, p); break;
-        case 1: launch_force<4, 2, 2>(v, grid, c->stream, p); break;
-        case 2: launch_force<2, 4, 2>(v, grid, c->stream, p); break;
-        case 3: launch_force<1, 8, 2>(v, grid, c->stream, p); break;
-        default: launch_force<1, 8, 2, true>(v, grid, c->stream, p); break;
+    if (fused) {
+        switch (vi) {
+            case 2: launch_force<2, 4, 2, false, SRC_STATE>(v, grid, c->stream, p); break;
+            case 3: launch_force<1, 8, 2, false, SRC_STATE>(v, grid, c->stream, p); break;
+            default: launch_force<1, 8, 2, true, SRC_STATE>(v, grid, c->stream, p); break;
+        }
+    } else {
+        switch (vi) {
+            case 0: launch_force<8, 1, 2>(v, grid, c->stream, p); break;
+            case 1: launch_force<4, 2, 2>(v, grid, c->stream, p); break;
+            case 2: launch_force<2, 4, 2>(v, grid, c->stream, p); break;
+            case 3: launch_force<1, 8, 2>(v, grid, c->stream, p); break;
+            default: launch_force<1, 8, 2, true>(v, grid, c->stream, p); break;
+        }
     }
     NB_CUDA(c, cudaGetLastError());
     if (c->profile) {
@@ -242,20 +268,39 @@ int launch_force_range(nb_ctx *c, int vi, int32_t n_i, const int32_t *idx_i, con
         c->prof_n += 1;
     }
     c->launches += 1;
-    c->last_iblock = v.iblock; c->last_grid = n_ib * S; c->last_variant = vi;
+    c->last_iblock = v.iblock; c->last_grid = n_ib * S; c->last_variant = vi; c->last_fused = fused ? 1 : 0;
     return NB_OK;
 }
 
-// a6-a7: fixed-order sum of the S partial rows, counters, sorted list rows.
-int launch_finalize(nb_ctx *c, int32_t n_i, int64_t n_i_pad, int S, double *acc, double *jerk, double *pot,
-                    int32_t *nnb, int32_t *nblist, int32_t *overflow) {
+// nb_predict_all defers the predictor launch (pred_pending); whoever needs the records calls this first.
+int materialize_pred(nb_ctx *c) {
+    if (!c->pred_pending) return NB_OK;
+    predict_kernel<<<(unsigned)((c->Npad + 255) / 256), 256, 0, c->stream>>>(0, c->Npad, c->N, c->Ns, c->pred_t, c->soa, c->rec);
+    NB_CUDA(c, cudaGetLastError());
+    c->launches += 1;
+    c->pred_pending = false;
+    return NB_OK;
+}
+
+// The 128 B/body gather copy of the state (NEXT-2 / NEXT-3 kernels): built on first use.
+int ensure_aos(nb_ctx *c) {
+    if (c->aos) return NB_OK;
+    NB_CUDA(c, cudaMalloc(&c->aos, sizeof(double) * AOS_D * c->N));
+    soa_to_aos_kernel<<<(unsigned)((c->N + 255) / 256), 256, 0, c->stream>>>(c->N, c->Ns, c->soa, c->aos);
+    NB_CUDA(c, cudaGetLastError());
+    c->launches += 1;
+    return NB_OK;
+}
+
+// a6-a7: fixed-order sum of the S partial rows, counters, sorted list rows.  perm (or NULL): slot -> k of
+// a block the library reordered (Morton order, reorder_block).
+int launch_finalize(nb_ctx *c, int32_t n_i, int64_t n_i_pad, int S, const int32_t *perm, double *acc, double *jerk,
+                    double *pot, int32_t *nnb, int32_t *nblist, int32_t *overflow) {
     const int W = S <= 8 ? 4 : 16;
     const size_t row_bytes = (size_t)c->sort_P * sizeof(int32_t);
-    int sortW = (int)std::min<size_t>(W, c->sort_smem_max / row_bytes);     // rows sorted per CTA
-    const int sortP = (nblist && sortW > 0) ? c->sort_P : 0;                // 0: rows stay in append order
-    sortW = std::max(sortW, 1);
-    const dim3 fgrid((unsigned)((n_i + 31) / 32), (unsigned)(7 + (32 + sortW - 1) / sortW));
-    const size_t smem = sortP ? (size_t)sortW * row_bytes : 0;
+    const int sortP = (nblist && row_bytes <= c->sort_smem_max) ? c->sort_P : 0;   // 0: rows stay in append order
+    const dim3 fgrid((unsigned)((n_i + 31) / 32), (unsigned)(7 + 32));
+    const size_t smem = sortP ? row_bytes : 0;
     // Programmatic dependent launch: the finalize grid is placed while the force kernel drains and
     // waits (griddepcontrol.wait) for its completion, so the launch latency is not on the path of
     // small blocks.
@@ -269,13 +314,13 @@ int launch_finalize(nb_ctx *c, int32_t n_i, int64_t n_i_pad, int S, double *acc,
     cfg.stream = c->stream;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    const int32_t n_i_pad32 = (int32_t)n_i_pad, S32 = S, cap32 = c->cap, sortP32 = sortP, sortW32 = sortW;
+    const int32_t n_i_pad32 = (int32_t)n_i_pad, S32 = S, cap32 = c->cap, sortP32 = sortP;
     const double *partial = c->partial;
     if (W == 4)
-        NB_CUDA(c, cudaLaunchKernelEx(&cfg, finalize_kernel<4>, n_i, n_i_pad32, S32, cap32, sortP32, sortW32, partial,
+        NB_CUDA(c, cudaLaunchKernelEx(&cfg, finalize_kernel<4>, n_i, n_i_pad32, S32, cap32, sortP32, perm, partial,
                                       c->cnt, acc, jerk, pot, nnb, nblist, overflow));
     else
-        NB_CUDA(c, cudaLaunchKernelEx(&cfg, finalize_kernel<16>, n_i, n_i_pad32, S32, cap32, sortP32, sortW32, partial,
+        NB_CUDA(c, cudaLaunchKernelEx(&cfg, finalize_kernel<16>, n_i, n_i_pad32, S32, cap32, sortP32, perm, partial,
                                       c->cnt, acc, jerk, pot, nnb, nblist, overflow));
     NB_CUDA(c, cudaGetLastError());
     c->launches += 1;
@@ -283,19 +328,72 @@ int launch_finalize(nb_ctx *c, int32_t n_i, int64_t n_i_pad, int S, double *acc,
     return NB_OK;
 }
 
+// Morton order of a large block (a3): c->sort_vals[slot] = k afterwards.  Reads the predicted records of
+// the active particles (irec if given, else rec[idx_i[k]]); everything on the context's stream.
+int reorder_block(nb_ctx *c, int32_t n_i, const int32_t *idx_i, const float *irec, int64_t n_i_pad) {
+    int64_t n2 = 2;
+    while (n2 < n_i) n2 <<= 1;
+    if (n2 > c->sort_n) {
+        NB_CUDA(c, cudaStreamSynchronize(c->stream));
+        cudaFree(c->sort_keys); cudaFree(c->sort_vals);
+        c->sort_keys = nullptr; c->sort_vals = nullptr; c->sort_n = 0;
+        NB_CUDA(c, cudaMalloc(&c->sort_keys, sizeof(unsigned long long) * n2));
+        NB_CUDA(c, cudaMalloc(&c->sort_vals, sizeof(int32_t) * n2));
+        c->sort_n = n2;
+    }
+    if (!c->sort_box) NB_CUDA(c, cudaMalloc(&c->sort_box, 6 * sizeof(uint32_t)));
+    NB_CUDA(c, cudaMemsetAsync(c->sort_box, 0xff, 6 * sizeof(uint32_t), c->stream));
+    const unsigned gb = (unsigned)std::min<int64_t>((n_i + 255) / 256, (int64_t)c->sm_count * 4);
+    block_bbox_kernel<<<gb, 256, 0, c->stream>>>(n_i, n_i_pad, idx_i, c->rec, irec, c->sort_box);
+    morton_key_kernel<<<(unsigned)((n2 + 255) / 256), 256, 0, c->stream>>>(n_i, (int32_t)n2, n_i_pad, idx_i, c->rec, irec,
+                                                                          c->sort_box, c->sort_keys, c->sort_vals);
+    const int64_t ch = std::min<int64_t>(n2, SORT_CH);
+    const unsigned chunks = (unsigned)(n2 / ch);
+    const size_t smem = (size_t)ch * (sizeof(unsigned long long) + sizeof(int32_t));
+    bitonic_chunk_kernel<0><<<chunks, SORT_T, smem, c->stream>>>((int32_t)n2, 0, c->sort_keys, c->sort_vals);
+    c->launches += 3;
+    for (int64_t size = 2 * ch; size <= n2; size <<= 1) {
+        for (int64_t stride = size / 2; stride >= ch; stride >>= 1) {
+            bitonic_global_kernel<<<(unsigned)((n2 / 2 + 255) / 256), 256, 0, c->stream>>>((int32_t)n2, (int32_t)size,
+                                                                                          (int32_t)stride, c->sort_keys,
+                                                                                          c->sort_vals);
+            c->launches += 1;
+        }
+        bitonic_chunk_kernel<1><<<chunks, SORT_T, smem, c->stream>>>((int32_t)n2, (int32_t)size, c->sort_keys, c->sort_vals);
+        c->launches += 1;
+    }
+    NB_CUDA(c, cudaGetLastError());
+    return NB_OK;
+}
+bool want_reorder(const nb_ctx *c, int32_t n_i) {
+    return c->local_g > 0.0 && c->reorder_min > 0 && n_i >= c->reorder_min;
+}
+
 int regular_device(nb_ctx *c, int32_t n_i, const int32_t *idx_i, const double *h2_i, double *acc, double *jerk,
                    double *pot, int32_t *nnb, int32_t *nblist, int32_t *overflow) {
     const int vi = pick_variant(c, n_i);
-    const Variant &v = c->var[vi];
-    const int64_t n_ib = (n_i + v.iblock - 1) / v.iblock;
+    const int64_t n_ib = (n_i + c->var[vi].iblock - 1) / c->var[vi].iblock;
+    // Small blocks (one i-block: every j-tile has exactly one reader) whose prediction is still pending
+    // read the FP64 state and predict inside the force kernel; everything else needs the records.
+    const bool fused = c->pred_pending && c->fuse && vi >= FUSED_FIRST && n_ib == 1;
+    int rc = fused ? NB_OK : materialize_pred(c);
+    if (rc != NB_OK) return rc;
+    const Variant &v = fused ? c->fvar[vi] : c->var[vi];
     const int64_t ntiles = c->Npad / TJ;
     const int S = pick_split(c, v, n_ib, ntiles);
     const int64_t n_i_pad = n_ib * v.iblock;
-    int rc = ensure_partial(c, (size_t)S * 7 * n_i_pad * sizeof(double));
+    rc = ensure_partial(c, (size_t)S * 7 * n_i_pad * sizeof(double));
     if (rc != NB_OK) return rc;
-    rc = launch_force_range(c, vi, n_i, idx_i, h2_i, nullptr, 0, nblist, 0, ntiles, S, 0);
+    const int32_t *perm = nullptr;
+    c->last_reordered = 0;
+    if (!fused && want_reorder(c, n_i)) {
+        rc = reorder_block(c, n_i, idx_i, nullptr, n_i_pad);
+        if (rc != NB_OK) return rc;
+        perm = c->sort_vals; c->last_reordered = 1;
+    }
+    rc = launch_force_range(c, vi, fused, n_i, idx_i, h2_i, nullptr, perm, 0, nblist, 0, ntiles, S, 0);
     if (rc != NB_OK) return rc;
-    return launch_finalize(c, n_i, n_i_pad, S, acc, jerk, pot, nnb, nblist, overflow);
+    return launch_finalize(c, n_i, n_i_pad, S, perm, acc, jerk, pot, nnb, nblist, overflow);
 }
 
 // Device-side buffers of the HOST variants, grown on demand.
@@ -371,7 +469,11 @@ int nb_open(int64_t N, int32_t nb_cap, nb_ctx **out) {
     c->sm_count = prop.multiProcessorCount;
     *out = c;     // from here on nb_close() releases whatever was allocated
     NB_CUDA(c, cudaMalloc(&c->soa, sizeof(double) * 14 * c->Ns));
-    NB_CUDA(c, cudaMalloc(&c->aos, sizeof(double) * AOS_D * c->N));
+    NB_CUDA(c, cudaMemsetAsync(c->soa, 0, sizeof(double) * 14 * c->Ns, nullptr));
+    if (c->Npad > c->N) {     // padding bodies: massless ghosts, written once
+        ghost_pad_kernel<<<(unsigned)((c->Npad - c->N + 255) / 256), 256>>>(c->N, c->Npad, c->Ns, c->soa);
+        NB_CUDA(c, cudaGetLastError());
+    }
     NB_CUDA(c, cudaMalloc(&c->rec, sizeof(float) * RECF * c->Npad));
     NB_CUDA(c, cudaMalloc(&c->cnt, sizeof(int32_t) * c->N));
     NB_CUDA(c, cudaMemset(c->cnt, 0, sizeof(int32_t) * c->N));
@@ -391,13 +493,23 @@ int nb_open(int64_t N, int32_t nb_cap, nb_ctx **out) {
     NB_CUDA(c, (setup_variant<2, 4, 2>(c->var[2], VAR_OVH[2])));
     NB_CUDA(c, (setup_variant<1, 8, 2>(c->var[3], VAR_OVH[3])));
     NB_CUDA(c, (setup_variant<1, 8, 2, true>(c->var[4], VAR_OVH[4])));
+    NB_CUDA(c, (setup_variant<2, 4, 2, false, SRC_STATE>(c->fvar[2], VAR_OVH[2])));
+    NB_CUDA(c, (setup_variant<1, 8, 2, false, SRC_STATE>(c->fvar[3], VAR_OVH[3])));
+    NB_CUDA(c, (setup_variant<1, 8, 2, true, SRC_STATE>(c->fvar[4], VAR_OVH[4])));
+    {
+        const int sort_smem = SORT_CH * (int)(sizeof(unsigned long long) + sizeof(int32_t));
+        NB_CUDA(c, cudaFuncSetAttribute(bitonic_chunk_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, sort_smem));
+        NB_CUDA(c, cudaFuncSetAttribute(bitonic_chunk_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, sort_smem));
+    }
+    NB_CUDA(c, cudaStreamSynchronize(nullptr));     // the ghost padding is in place before any stream uses the state
     return NB_OK;
 }
 
 int nb_close(nb_ctx *c) {
     if (!c) return NB_EINVAL;
     cudaStreamSynchronize(c->stream);
-    cudaFree(c->soa); cudaFree(c->aos); cudaFree(c->rec); cudaFree(c->cnt);
+    cudaFree(c->soa); cudaFree(c->aos); cudaFree(c->rec); cudaFree(c->cnt); cudaFree(c->stats);
+    cudaFree(c->sort_keys); cudaFree(c->sort_vals); cudaFree(c->sort_box);
     cudaFree(c->partial); cudaFree(c->stage_j);
     cudaFree(c->st_idx); cudaFree(c->st_nnb); cudaFree(c->st_ovf); cudaFree(c->st_list);
     cudaFree(c->st_h2); cudaFree(c->st_out);
@@ -444,7 +556,7 @@ int nb_set_j(nb_ctx *c, const double *m, const double *x0, const double *v0, con
     NB_CUDA(c, cudaGetLastError());
     c->launches += 1;
     c->have_j = true;
-    c->have_pred = false;
+    c->have_pred = false; c->pred_pending = false;
     return NB_OK;
 }
 
@@ -478,7 +590,7 @@ int nb_update_j(nb_ctx *c, int32_t n, const int32_t *idx, const double *m, const
                                                                          c->aos);
     NB_CUDA(c, cudaGetLastError());
     c->launches += 1;
-    c->have_pred = false;       // the predicted records are stale until the next nb_predict_all
+    c->have_pred = false; c->pred_pending = false;   // the predicted records are stale until the next nb_predict_all
     return NB_OK;
 }
 
@@ -490,6 +602,8 @@ int nb_irregular(nb_ctx *c, double t, int32_t n_i, const int32_t *idx_i, const i
     if (!c->have_j) return NB_ESTATE;
     if (n_i == 0) return NB_OK;
     if (!idx_i || !nnb || !nblist || !acc || !jerk) return NB_EINVAL;
+    rc = ensure_aos(c);
+    if (rc != NB_OK) return rc;
     irregular_kernel<<<(unsigned)((n_i + 7) / 8), 256, 0, c->stream>>>(n_i, c->cap, t, idx_i, nnb, nblist, c->aos, acc,
                                                                        jerk, pot);
     NB_CUDA(c, cudaGetLastError());
@@ -501,12 +615,13 @@ int nb_predict_all(nb_ctx *c, double t) {
     int rc = check_live(c);
     if (rc != NB_OK) return rc;
     if (!c->have_j) return NB_ESTATE;
-    predict_kernel<<<(unsigned)((c->Npad + 255) / 256), 256, 0, c->stream>>>(0, c->Npad, c->N, c->Ns, t, c->soa, c->rec);
-    NB_CUDA(c, cudaGetLastError());
-    c->launches += 1;
+    // The launch is deferred: a small block that follows predicts inside its force kernel (fused path) and
+    // never needs the records; any other consumer writes them first (materialize_pred).  The result of
+    // every later call is the same either way.
     c->have_pred = true;
+    c->pred_pending = true;
     c->pred_t = t;
-    return NB_OK;
+    return c->fuse ? NB_OK : materialize_pred(c);
 }
 
 int nb_get_predicted(nb_ctx *c, double *xp, double *vp) {
@@ -514,6 +629,8 @@ int nb_get_predicted(nb_ctx *c, double *xp, double *vp) {
     if (rc != NB_OK) return rc;
     if (!xp || !vp) return NB_EINVAL;
     if (!c->have_pred) return NB_ESTATE;
+    rc = materialize_pred(c);
+    if (rc != NB_OK) return rc;
     unpack_predicted_kernel<<<(unsigned)((c->N + 255) / 256), 256, 0, c->stream>>>(c->N, c->rec, xp, vp);
     NB_CUDA(c, cudaGetLastError());
     c->launches += 1;
@@ -686,7 +803,7 @@ int nb_step_host(nb_ctx *c, const double *m, const double *x0, const double *v0,
         c->launches += 2;
     }
     c->have_j = true;
-    c->have_pred = true;
+    c->have_pred = true; c->pred_pending = false;     // every chunk is predicted as it lands
     c->pred_t = t;
 
     NB_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_i, 0));
@@ -696,16 +813,23 @@ int nb_step_host(nb_ctx *c, const double *m, const double *x0, const double *v0,
         predict_i_kernel<false><<<(unsigned)((n_i + 255) / 256), 256, 0, c->stream>>>(n_i, (int32_t)n_i_pad, t, isrc, c->irec);
     NB_CUDA(c, cudaGetLastError());
     c->launches += 1;
+    const int32_t *perm = nullptr;
+    c->last_reordered = 0;
+    if (want_reorder(c, n_i)) {        // from the active particles' own records: no chunk of the j-state is needed
+        rc = reorder_block(c, n_i, c->st_idx, c->irec, n_i_pad);
+        if (rc != NB_OK) return rc;
+        perm = c->sort_vals; c->last_reordered = 1;
+    }
     int64_t split0 = 0;
     for (int q = 0; q < nchunk; ++q) {
         NB_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_chunk[q], 0));
-        rc = launch_force_range(c, vi, n_i, c->st_idx, c->st_h2, c->irec, 0, c->st_list, ctile[q], ctile[q + 1], S_c[q],
+        rc = launch_force_range(c, vi, false, n_i, c->st_idx, c->st_h2, c->irec, perm, 0, c->st_list, ctile[q], ctile[q + 1], S_c[q],
                                 split0);
         if (rc != NB_OK) return rc;
         split0 += S_c[q];
     }
     double *d_acc = c->st_out, *d_jerk = c->st_out + 3 * (int64_t)n_i, *d_pot = c->st_out + 6 * (int64_t)n_i;
-    rc = launch_finalize(c, n_i, n_i_pad, S_total, d_acc, d_jerk, d_pot, c->st_nnb, c->st_list, c->st_ovf);
+    rc = launch_finalize(c, n_i, n_i_pad, S_total, perm, d_acc, d_jerk, d_pot, c->st_nnb, c->st_list, c->st_ovf);
     if (rc != NB_OK) return rc;
     rc = copy_back(c, n_i, acc, jerk, pot, nnb, nblist, overflow);
     return rc;
@@ -771,11 +895,13 @@ int nb_correct(nb_ctx *c, double t, int32_t n, const int32_t *idx, const double 
     if (!c->have_j || !c->have_steps) return NB_ESTATE;
     if (n == 0) return NB_OK;
     if (!idx || !acc1 || !jerk1) return NB_EINVAL;
+    rc = ensure_aos(c);
+    if (rc != NB_OK) return rc;
     correct_kernel<<<(unsigned)((n + 127) / 128), 128, 0, c->stream>>>(n, c->Ns, t, eta, dt_max, idx, acc1, jerk1, c->soa,
                                                                        c->aos, c->dtj);
     NB_CUDA(c, cudaGetLastError());
     c->launches += 1;
-    c->have_pred = false;
+    c->have_pred = false; c->pred_pending = false;
     return NB_OK;
 }
 
@@ -807,6 +933,8 @@ int nb_regular_shard(nb_ctx *c, double t, int32_t n_i, const int32_t *idx_i, con
     if (!c->have_pred || t != c->pred_t) return NB_ESTATE;   // the shard's records must be at the same time t
     if (n_i == 0) return NB_OK;
     if (!idx_i || !istate || !h2_i || !acc || !jerk || !pot || !nnb || !nblist || !overflow) return NB_EINVAL;
+    rc = materialize_pred(c);
+    if (rc != NB_OK) return rc;
     const int vi = pick_variant(c, n_i);
     const Variant &v = c->var[vi];
     const int64_t n_ib = (n_i + v.iblock - 1) / v.iblock, n_i_pad = n_ib * v.iblock;
@@ -836,9 +964,16 @@ int nb_regular_shard(nb_ctx *c, double t, int32_t n_i, const int32_t *idx_i, con
     predict_i_kernel<false><<<(unsigned)((n_i + 255) / 256), 256, 0, c->stream>>>(n_i, (int32_t)n_i_pad, t, isrc, c->irec);
     NB_CUDA(c, cudaGetLastError());
     c->launches += 1;
-    rc = launch_force_range(c, vi, n_i, idx_i, h2_i, c->irec, c->j_offset, nblist, 0, ntiles, S, 0);
+    const int32_t *perm = nullptr;
+    c->last_reordered = 0;
+    if (want_reorder(c, n_i)) {
+        rc = reorder_block(c, n_i, idx_i, c->irec, n_i_pad);
+        if (rc != NB_OK) return rc;
+        perm = c->sort_vals; c->last_reordered = 1;
+    }
+    rc = launch_force_range(c, vi, false, n_i, idx_i, h2_i, c->irec, perm, c->j_offset, nblist, 0, ntiles, S, 0);
     if (rc != NB_OK) return rc;
-    return launch_finalize(c, n_i, n_i_pad, S, acc, jerk, pot, nnb, nblist, overflow);
+    return launch_finalize(c, n_i, n_i_pad, S, perm, acc, jerk, pot, nnb, nblist, overflow);
 }
 
 int nb_get_info(nb_ctx *c, int32_t key, int64_t *value) {
@@ -855,6 +990,22 @@ int nb_get_info(nb_ctx *c, int32_t key, int64_t *value) {
         case NB_TUNE_FORCE_VARIANT: *value = c->force_variant; break;
         case NB_TUNE_PROFILE: *value = c->profile ? 1 : 0; break;
         case NB_TUNE_STEP_CHUNKS: *value = c->step_chunks; break;
+        case NB_TUNE_FUSE_PREDICT: *value = c->fuse ? 1 : 0; break;
+        case NB_TUNE_LOCAL_G_MILLI: *value = (int64_t)(c->local_g * 1000.0 + 0.5); break;
+        case NB_TUNE_STATS: *value = c->stats ? 1 : 0; break;
+        case NB_INFO_LAST_FUSED: *value = c->last_fused; break;
+        case NB_INFO_LAST_REORDERED: *value = c->last_reordered; break;
+        case NB_TUNE_REORDER_MIN: *value = c->reorder_min; break;
+        case NB_INFO_LOCAL_WARPS:
+        case NB_INFO_TOTAL_WARPS: {
+            if (!c->stats) return NB_ESTATE;
+            if (c->cuda_err != cudaSuccess) return NB_ECUDA;
+            unsigned int h[2] = {0, 0};
+            NB_CUDA(c, cudaStreamSynchronize(c->stream));
+            NB_CUDA(c, cudaMemcpy(h, c->stats, sizeof(h), cudaMemcpyDeviceToHost));
+            *value = key == NB_INFO_LOCAL_WARPS ? h[0] : h[1];
+            break;
+        }
         case NB_INFO_FORCE_KERNEL_COUNT: *value = std::min<int64_t>(c->prof_n, nb_ctx::PROF_RING); break;
         case NB_INFO_FORCE_KERNEL_NS: {
             if (c->cuda_err != cudaSuccess) return NB_ECUDA;
@@ -886,6 +1037,27 @@ int nb_set_tuning(nb_ctx *c, int32_t key, int64_t value) {
         case NB_TUNE_STEP_CHUNKS:
             if (value < 0 || value > nb_ctx::MAXCHUNK) return NB_EINVAL;
             c->step_chunks = value; break;
+        case NB_TUNE_FUSE_PREDICT:
+            if (value != 0 && value != 1) return NB_EINVAL;
+            c->fuse = value != 0;
+            if (!c->fuse) return materialize_pred(c);
+            break;
+        case NB_TUNE_LOCAL_G_MILLI:
+            if (value < 0 || value > 1000000) return NB_EINVAL;
+            c->local_g = (double)value / 1000.0; break;
+        case NB_TUNE_REORDER_MIN:
+            if (value < 0) return NB_EINVAL;
+            c->reorder_min = value; break;
+        case NB_TUNE_STATS:
+            if (value != 0 && value != 1) return NB_EINVAL;
+            if (value) {
+                if (!c->stats) NB_CUDA(c, cudaMalloc(&c->stats, 2 * sizeof(unsigned int)));
+                NB_CUDA(c, cudaMemsetAsync(c->stats, 0, 2 * sizeof(unsigned int), c->stream));
+            } else if (c->stats) {
+                NB_CUDA(c, cudaStreamSynchronize(c->stream));
+                cudaFree(c->stats); c->stats = nullptr;
+            }
+            break;
         case NB_TUNE_PROFILE:
             if (value != 0 && value != 1) return NB_EINVAL;
             if (value && !c->ev0[0]) {
@@ -921,6 +1093,13 @@ int nb_plan_chunks(int64_t N, int32_t chunks, int64_t *first_body, int32_t *nchu
     *nchunk = n;
     return NB_OK;
 }
+
+#ifdef NBREG_TIMELINE
+int nb_debug_set_timeline(void *dev_buf) {      // debug builds only: [CTA][8] uint64 stamps, NULL = off
+    unsigned long long *p = static_cast<unsigned long long *>(dev_buf);
+    return cudaMemcpyToSymbol(nbreg::g_timeline, &p, sizeof(p)) == cudaSuccess ? NB_OK : NB_ECUDA;
+}
+#endif
 
 int nb_last_cuda_error(nb_ctx *c) { return c ? (int)c->cuda_err : 0; }
 

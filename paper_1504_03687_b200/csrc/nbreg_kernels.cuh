@@ -13,7 +13,9 @@
 // broadcast to both halves (SASS operand form `R.F32`), so a j value costs one register read and the
 // records need no duplication.  x = hi + lo with hi = fl32(x), lo = fl32(x - hi): positions carry 48
 // significant bits, so (hi_j - hi_i) + (lo_j - lo_i) is the FP64 difference rounded once to FP32 --
-// the pair arithmetic after that is plain FP32.
+// the pair arithmetic after that is plain FP32.  A warp whose i-particles sit
+// close together (relative to their neighbour radii) differences in its OWN frame instead: one add per
+// component (see force_kernel).  Small blocks read the FP64 state directly and predict in the kernel.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -78,6 +80,21 @@ __device__ __forceinline__ float rsqrt_sfu(float x) {   // one MUFU.RSQ, no deno
     return y;
 }
 
+// Debug builds (-DNBREG_TIMELINE): thread 0 of every CTA stamps %globaltimer at a few points.
+#ifdef NBREG_TIMELINE
+__device__ unsigned long long *g_timeline = nullptr;      // [CTA][8]
+__device__ __forceinline__ void tl_stamp(int cta, int q) {
+    if (threadIdx.x == 0 && g_timeline) {
+        unsigned long long t;
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+        g_timeline[(size_t)cta * 8 + q] = t;
+    }
+}
+#define TL_STAMP(cta, q) tl_stamp(cta, q)
+#else
+#define TL_STAMP(cta, q)
+#endif
+
 // ------------------------------------------------------------------ a1: re-layout
 // in: m[N], x0[N][3], v0[N][3], a0[N][3], j0[N][3], t0[N]  ->  soa[14][Ns] (component-major, streamed
 // by the predictor) and aos[N][16] (one 128 B line per body: m, x0, v0, a0, j0, t0, 2 pad -- gathered
@@ -95,6 +112,7 @@ __device__ __forceinline__ void store_body(int64_t j, int64_t Ns, double m, cons
         soa[(7 + c) * Ns + j] = a[c];
         soa[(10 + c) * Ns + j] = jk[c];
     }
+    if (!aos) return;       // the gather copy exists only once a NEXT-2 / NEXT-3 call has asked for it
     double2 *o = reinterpret_cast<double2 *>(aos + j * AOS_D);
     o[0] = make_double2(m, x[0]);     o[1] = make_double2(x[1], x[2]);
     o[2] = make_double2(v[0], v[1]);  o[3] = make_double2(v[2], a[0]);
@@ -134,6 +152,30 @@ __global__ void __launch_bounds__(256) update_j_kernel(int32_t n, int64_t Ns, co
         x[c] = x0[3 * q + c]; v[c] = v0[3 * q + c]; a[c] = a0[3 * q + c]; jk[c] = j0[3 * q + c];
     }
     store_body(idx[q], Ns, m[q], x, v, a, jk, t0[q], soa, aos);
+}
+
+// Padding bodies N .. Npad-1 of the FP64 state: massless ghosts far away (written once at nb_open; the
+// fused force kernel predicts whole tiles, the predictor writes the same ghost into the records).
+__global__ void __launch_bounds__(256) ghost_pad_kernel(int64_t N, int64_t Npad, int64_t Ns, double *__restrict__ soa) {
+    const int64_t j = N + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= Npad) return;
+#pragma unroll
+    for (int c = 0; c < 14; ++c) soa[c * Ns + j] = (c >= 1 && c <= 3) ? (double)GHOST_POS : 0.0;
+}
+
+// Build the gather copy from the SoA state (first NEXT-2 / NEXT-3 call on a context).
+__global__ void __launch_bounds__(256) soa_to_aos_kernel(int64_t N, int64_t Ns, const double *__restrict__ soa,
+                                                         double *__restrict__ aos) {
+    const int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= N) return;
+    double v[14];
+#pragma unroll
+    for (int c = 0; c < 14; ++c) v[c] = soa[c * Ns + j];
+    double2 *o = reinterpret_cast<double2 *>(aos + j * AOS_D);
+    o[0] = make_double2(v[0], v[1]);  o[1] = make_double2(v[2], v[3]);
+    o[2] = make_double2(v[4], v[5]);  o[3] = make_double2(v[6], v[7]);
+    o[4] = make_double2(v[8], v[9]);  o[5] = make_double2(v[10], v[11]);
+    o[6] = make_double2(v[12], v[13]); o[7] = make_double2(0.0, 0.0);
 }
 
 // ------------------------------------------------------------------ a2: predictor
@@ -245,14 +287,158 @@ __global__ void __launch_bounds__(256) predict_i_kernel(int32_t n_i, int32_t n_i
     irec[(size_t)C_M * n_i_pad + k] = __double2float_rn(m);
 }
 
+// ------------------------------------------------------------------ a3: spatial order of a large active block
+// The local frame of force_kernel needs the 64 i-particles of a warp to sit close together.  A block
+// arrives in the caller's order (NBODY6++GPU: the step-sorted list, P:89 -- not spatial), so for large
+// blocks the library sorts the SLOTS of the block along a Morton curve of the predicted positions:
+// bounding box (integer atomics on ordered keys: order-independent), 63-bit keys (21 bits per axis on
+// the box), ties broken by k, bitonic sort (no atomics: the permutation is a pure function of the
+// inputs, so results stay bitwise reproducible).  perm[slot] = k.
+__device__ __forceinline__ uint32_t ordered_u32(float x) {             // monotone map float -> uint32
+    const uint32_t b = __float_as_uint(x);
+    return (b >> 31) ? ~b : (b | 0x80000000u);
+}
+__device__ __forceinline__ float ordered_to_float(uint32_t k) {
+    return __uint_as_float((k >> 31) ? (k & 0x7fffffffu) : ~k);
+}
+__device__ __forceinline__ unsigned long long spread21(uint32_t v) {   // bit i -> bit 3 i
+    unsigned long long x = v & 0x1fffffu;
+    x = (x | x << 32) & 0x1f00000000ffffull;
+    x = (x | x << 16) & 0x1f0000ff0000ffull;
+    x = (x | x << 8) & 0x100f00f00f00f00full;
+    x = (x | x << 4) & 0x10c30c30c30c30c3ull;
+    x = (x | x << 2) & 0x1249249249249249ull;
+    return x;
+}
+__device__ __forceinline__ const float *irec_or_rec(const float *rec, const float *irec, const int32_t *idx_i, int k,
+                                                    int64_t n_i_pad, int64_t &cs) {
+    cs = irec ? n_i_pad : TJ;
+    return irec ? irec + k : rec_slot(rec, idx_i ? idx_i[k] : k);
+}
+
+// box[0..2] = min of ordered(x), box[3..5] = min of ~ordered(x) (i.e. the maximum), all initialised to ~0.
+__global__ void __launch_bounds__(256) block_bbox_kernel(int32_t n_i, int64_t n_i_pad, const int32_t *__restrict__ idx_i,
+                                                         const float *__restrict__ rec, const float *__restrict__ irec,
+                                                         uint32_t *__restrict__ box) {
+    uint32_t lo[3] = {~0u, ~0u, ~0u}, hi[3] = {~0u, ~0u, ~0u};
+    for (int k = blockIdx.x * blockDim.x + threadIdx.x; k < n_i; k += gridDim.x * blockDim.x) {
+        int64_t cs;
+        const float *r = irec_or_rec(rec, irec, idx_i, k, n_i_pad, cs);
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            const uint32_t o = ordered_u32(r[(C_XH + c) * cs]);
+            lo[c] = min(lo[c], o); hi[c] = min(hi[c], ~o);
+        }
+    }
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+#pragma unroll
+        for (int off = 16; off > 0; off >>= 1) {
+            lo[c] = min(lo[c], __shfl_xor_sync(0xffffffffu, lo[c], off));
+            hi[c] = min(hi[c], __shfl_xor_sync(0xffffffffu, hi[c], off));
+        }
+        if ((threadIdx.x & 31) == 0) { atomicMin(box + c, lo[c]); atomicMin(box + 3 + c, hi[c]); }
+    }
+}
+
+// keys[s], vals[s] for the n2 = 2^m >= n_i slots of the sort; slots >= n_i sort to the end.
+__global__ void __launch_bounds__(256) morton_key_kernel(int32_t n_i, int32_t n2, int64_t n_i_pad,
+                                                         const int32_t *__restrict__ idx_i, const float *__restrict__ rec,
+                                                         const float *__restrict__ irec, const uint32_t *__restrict__ box,
+                                                         unsigned long long *__restrict__ keys, int32_t *__restrict__ vals) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= n2) return;
+    if (k >= n_i) { keys[k] = ~0ull; vals[k] = 0x7fffffff; return; }
+    int64_t cs;
+    const float *r = irec_or_rec(rec, irec, idx_i, k, n_i_pad, cs);
+    unsigned long long key = 0;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const float mn = ordered_to_float(box[c]), mx = ordered_to_float(~box[3 + c]);
+        const float ext = mx - mn;
+        const float u = ext > 0.f ? (r[(C_XH + c) * cs] - mn) / ext : 0.f;             // in [0, 1]
+        const uint32_t q = min((uint32_t)(u * 2097152.0f), 2097151u);                   // 21 bits
+        key |= spread21(q) << (2 - c);
+    }
+    keys[k] = key;
+    vals[k] = k;
+}
+
+// Bitonic sort of (key, val) pairs, ascending by key then val.  SORT_CH pairs per CTA live in shared memory.
+constexpr int SORT_CH = 8192;
+constexpr int SORT_T = 1024;
+__device__ __forceinline__ bool pair_gt(unsigned long long ka, int32_t va, unsigned long long kb, int32_t vb) {
+    return ka > kb || (ka == kb && va > vb);
+}
+// MODE 0: full sort of each chunk (sizes 2 .. chunk).  MODE 1: the strides chunk/2 .. 1 of merge size `size`.
+template <int MODE>
+__global__ void __launch_bounds__(SORT_T) bitonic_chunk_kernel(int32_t n2, int32_t size, unsigned long long *__restrict__ keys,
+                                                              int32_t *__restrict__ vals) {
+    extern __shared__ unsigned long long sk[];                                  // [ch] keys, then [ch] vals
+    const int ch = min(n2, SORT_CH);
+    int32_t *sv = reinterpret_cast<int32_t *>(sk + ch);
+    const int base = blockIdx.x * ch;
+    for (int e = threadIdx.x; e < ch; e += SORT_T) { sk[e] = keys[base + e]; sv[e] = vals[base + e]; }
+    __syncthreads();
+    for (int sz = (MODE == 0 ? 2 : size); sz <= (MODE == 0 ? ch : size); sz <<= 1) {
+        for (int stride = min(sz >> 1, ch >> 1); stride > 0; stride >>= 1) {
+            for (int e = threadIdx.x; e < (ch >> 1); e += SORT_T) {
+                const int lo = 2 * e - (e & (stride - 1)), hi = lo + stride;
+                const bool up = ((base + lo) & sz) == 0;
+                const unsigned long long ka = sk[lo], kb = sk[hi];
+                const int32_t va = sv[lo], vb = sv[hi];
+                if (pair_gt(ka, va, kb, vb) == up) { sk[lo] = kb; sk[hi] = ka; sv[lo] = vb; sv[hi] = va; }
+            }
+            __syncthreads();
+        }
+    }
+    for (int e = threadIdx.x; e < ch; e += SORT_T) { keys[base + e] = sk[e]; vals[base + e] = sv[e]; }
+}
+// One compare-exchange step (merge size `size`, stride >= SORT_CH) in global memory.
+__global__ void __launch_bounds__(256) bitonic_global_kernel(int32_t n2, int32_t size, int32_t stride,
+                                                            unsigned long long *__restrict__ keys, int32_t *__restrict__ vals) {
+    const int e = blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= (n2 >> 1)) return;
+    const int lo = 2 * e - (e & (stride - 1)), hi = lo + stride;
+    const bool up = (lo & size) == 0;
+    const unsigned long long ka = keys[lo], kb = keys[hi];
+    const int32_t va = vals[lo], vb = vals[hi];
+    if (pair_gt(ka, va, kb, vb) == up) { keys[lo] = kb; keys[hi] = ka; vals[lo] = vb; vals[hi] = va; }
+}
+
 // ------------------------------------------------------------------ a3-a6: force kernel
+// Source of the j-data a CTA streams through its bulk-copy ring:
+//   SRC_REC    the predicted records nb_predict_all wrote (40 B/body, one 10 KB bulk copy per tile);
+//   SRC_STATE  the FP64 j-state itself (112 B/body, fourteen 2 KB bulk copies per tile): every warp
+//              PREDICTS the j's it is about to consume, with the predictor's own arithmetic -- the
+//              fused predict + force path of small blocks (one reader per j-tile; no predict launch
+//              and no 40 B/body round trip through HBM).
+enum { SRC_REC = 0, SRC_STATE = 1 };
+constexpr int STATE_D = 14;                                   // doubles per body of the FP64 state
+constexpr int STATE_TILE_DOUBLES = STATE_D * TJ;              // 28 KB per tile
+template <int SRC> struct SrcCfg;
+template <> struct SrcCfg<SRC_REC> {
+    static constexpr int NST = NSTAGE;                                         // stages in the ring
+    static constexpr uint32_t STAGE_BYTES = TILE_FLOATS * sizeof(float);       // 10 KB
+    static constexpr int SLICE_COMP = 3;                                       // x', y', z' per j of the warp's share
+};
+template <> struct SrcCfg<SRC_STATE> {
+    static constexpr int NST = 2;
+    static constexpr uint32_t STAGE_BYTES = STATE_TILE_DOUBLES * sizeof(double);   // 28 KB
+    static constexpr int SLICE_COMP = RECF;                                    // a whole record per j of the warp's share
+};
+
 struct ForceParams {
-    const float *rec;             // predicted records, [Npad / TJ][RECF][TJ]
+    const float *rec;             // SRC_REC: predicted records, [Npad / TJ][RECF][TJ]
+    const double *soa;            // SRC_STATE: FP64 state [14][Ns] (padding bodies are massless ghosts)
+    int64_t Ns;
+    double t;                     // SRC_STATE: time to predict to
     const int32_t *idx_i;         // [n_i], or NULL: the block is 0..n_i-1
     const double *h2_i;           // [n_i]
+    const int32_t *perm;          // NULL, or slot -> k of a block the library put in Morton order (lanes hold slots)
     int32_t n_i;
     int32_t n_i_pad;              // n_i rounded up to the CTA's i-block
-    const float *irec;            // NULL, or the active particles' own records [RECF][n_i_pad] (nb_step_host)
+    const float *irec;            // NULL, or the active particles' own records [RECF][n_i_pad] (nb_step_host, shards)
     int32_t tile0;                // first j-tile of this launch (0 unless the j-range arrives in chunks)
     int32_t ntiles;               // end of this launch's j-tile range (Npad / TJ for a whole pass)
     int32_t split0;               // first row of `partial` this launch writes
@@ -260,13 +446,16 @@ struct ForceParams {
                                   // the self test use global indices, idx_i is global when irec is given
     int32_t tiles_per_split;      // contiguous tiles per blockIdx.y
     int32_t cap;
+    float g2;                     // local-frame guard: a warp differences in its own frame iff every one of its
+                                  // i has |x_i - c|^2 <= g2 * h2_i (c = centre of the warp's bounding box); 0: never
     int32_t *cnt;                 // [>= n_i] neighbour counters, zero on entry (finalize re-zeroes)
     int32_t *nblist;              // caller's [n_i][cap], or NULL: neighbours are only counted
     double *partial;              // [S][7][n_i_pad]
+    unsigned int *stats;          // NULL, or {warps in the local frame, warps} (diagnostics; integer atomics)
 };
 
 // Two active particles (halves .x / .y) held in registers, NEGATED so that every difference is one
-// packed add:  d = j + (-i).
+// packed add:  d = j + (-i).  Local frame: nxh.. hold -(x_i - c) and the lo parts are unused.
 struct IPair {
     float2 nxh, nyh, nzh, nxl, nyl, nzl, nvx, nvy, nvz, h2;
 };
@@ -330,28 +519,144 @@ __device__ __forceinline__ void pair_terms(Acc7 &A, const IPair &I, float2 dx, f
     A.jz = pfma(mrinv3, pfma(alpha, dz, dvz), A.jz);
 }
 
+// Where a warp finds the components of its share of a tile (shared memory, floats).  Positions: px + c * SX
+// (LOCAL: x' = x_j - c of the warp; else the hi parts, with the lo parts at pl + c * SX); velocities
+// pv + c * SV; masses pm.
+struct JPtrs {
+    const float *px, *pl, *pv, *pm;
+};
+
+// All pairs of the warp's i-pair(s) with SUBN consecutive j of one tile.  LOCAL: positions are already
+// differenced against the warp's origin -- ONE packed add per component (27 packed FP32 instructions
+// per 2 i x 1 j); otherwise hi/lo differencing, three adds per component (33).
+template <bool LOCAL, bool JP, int SUBN, int SX, int SV>
+__device__ __forceinline__ void tile_pairs(Acc7 &A, const IPair &I, const JPtrs P, int32_t jbase,
+                                           const int32_t (&my_idx)[2], const int32_t (&my_k)[2],
+                                           const ForceParams &p) {
+    constexpr int NU = JP ? 2 : 4;           // packed iterations per group of four j
+#pragma unroll GROUP_UNROLL
+    for (int g = 0; g < SUBN; g += UNROLL_J) {
+        // warp-uniform addresses: LDS.128 broadcasts of one component of 4 consecutive j
+        float4 cx = *reinterpret_cast<const float4 *>(P.px + g);
+        float4 cy = *reinterpret_cast<const float4 *>(P.px + SX + g);
+        float4 cz = *reinterpret_cast<const float4 *>(P.px + 2 * SX + g);
+        float4 lx, ly, lz;
+        if constexpr (!LOCAL) {
+            lx = *reinterpret_cast<const float4 *>(P.pl + g);
+            ly = *reinterpret_cast<const float4 *>(P.pl + SX + g);
+            lz = *reinterpret_cast<const float4 *>(P.pl + 2 * SX + g);
+        }
+        const float4 cvx = *reinterpret_cast<const float4 *>(P.pv + g);
+        const float4 cvy = *reinterpret_cast<const float4 *>(P.pv + SV + g);
+        const float4 cvz = *reinterpret_cast<const float4 *>(P.pv + 2 * SV + g);
+        const float4 cm = *reinterpret_cast<const float4 *>(P.pm + g);
+        // phase 1: differences and r^2 of the group's 4 j against the i-pair
+        float2 dx[NU], dy[NU], dz[NU], r2[NU], rinv[NU];
+#pragma unroll
+        for (int u = 0; u < NU; ++u) {
+            if constexpr (LOCAL) {
+                dx[u] = padd(jop<JP>(cx, u), I.nxh);
+                dy[u] = padd(jop<JP>(cy, u), I.nyh);
+                dz[u] = padd(jop<JP>(cz, u), I.nzh);
+            } else {
+                dx[u] = padd(padd(jop<JP>(cx, u), I.nxh), padd(jop<JP>(lx, u), I.nxl));
+                dy[u] = padd(padd(jop<JP>(cy, u), I.nyh), padd(jop<JP>(ly, u), I.nyl));
+                dz[u] = padd(padd(jop<JP>(cz, u), I.nzh), padd(jop<JP>(lz, u), I.nzl));
+            }
+            r2[u] = pfma(dz[u], dz[u], pfma(dy[u], dy[u], pmul(dx[u], dx[u])));
+            rinv[u].x = rsqrt_sfu(r2[u].x);        // issued before the vote: SFU latency overlaps the test
+            rinv[u].y = rsqrt_sfu(r2[u].y);
+        }
+        // one test per i for the whole group (FMNMX3): a neighbour, or the self pair (r2 == 0)?
+        float mn0, mn1;
+        if constexpr (JP) {
+            mn0 = fminf(r2[0].x, r2[1].x);
+            mn1 = fminf(r2[0].y, r2[1].y);
+        } else {
+            mn0 = fminf(fminf(fminf(r2[0].x, r2[1].x), r2[2].x), r2[3].x);
+            mn1 = fminf(fminf(fminf(r2[0].y, r2[1].y), r2[2].y), r2[3].y);
+        }
+        const bool hit = (mn0 < I.h2.x) | (mn1 < I.h2.y);
+        if (!__any_sync(0xffffffffu, hit)) {    // ~95 % of groups at N_b ~ 150, N = 1M: nothing to mask
+#pragma unroll
+            for (int u = 0; u < NU; ++u)
+                pair_terms<false>(A, I, dx[u], dy[u], dz[u], r2[u], rinv[u], jop<JP>(cvx, u), jop<JP>(cvy, u),
+                                  jop<JP>(cvz, u), jop<JP>(cm, u));
+        } else {
+#pragma unroll
+            for (int u = 0; u < NU; ++u)
+                pair_terms<true>(A, I, dx[u], dy[u], dz[u], r2[u], rinv[u], jop<JP>(cvx, u), jop<JP>(cvy, u),
+                                 jop<JP>(cvz, u), jop<JP>(cm, u));
+            if (hit) {      // rare: lanes hold different i, each takes slots of its own rows
+#pragma unroll
+                for (int u = 0; u < NU; ++u) {
+                    // half .x / .y of iteration u: (i, j) = (my i 0, j u) / (my i 1, j u), or, j-packed,
+                    // (my i, j 2u) / (my i, j 2u + 1)
+                    const int32_t jg0 = jbase + g + (JP ? 2 * u : u), jg1 = JP ? jg0 + 1 : jg0;
+                    if (r2[u].x < I.h2.x && jg0 != my_idx[0]) append_one(my_k[0], jg0, p.cap, p.cnt, p.nblist);
+                    if (r2[u].y < I.h2.y && jg1 != my_idx[1]) append_one(my_k[1], jg1, p.cap, p.cnt, p.nblist);
+                }
+            }
+        }
+    }
+}
+
+// Shared-memory plan of one force-kernel CTA (host and device use the same numbers).
+template <int WI, int WJ, bool JP, int SRC>
+struct ForceSmem {
+    static constexpr int NW = WI * WJ, NT = 32 * NW, NH = JP ? 1 : 2, SUB = TJ / WJ;
+    static constexpr size_t RING = (size_t)SrcCfg<SRC>::NST * SrcCfg<SRC>::STAGE_BYTES;     // bulk-copy ring
+    static constexpr size_t SLICES = (size_t)NW * SrcCfg<SRC>::SLICE_COMP * SUB * sizeof(float);   // one per warp
+    static constexpr size_t ACC = (size_t)7 * NH * NT * sizeof(double);                     // FP64 running sums
+    static constexpr size_t BARS = (size_t)SrcCfg<SRC>::NST * (sizeof(uint64_t) + sizeof(int));
+    static constexpr size_t TOTAL = RING + SLICES + ACC + BARS + 64;
+    static_assert(WJ == 1 || (size_t)WJ * 7 * 32 * NH * WI * sizeof(double) <= RING + SLICES,
+                  "the WJ reduction reuses the ring and the slices");
+};
+
+// The Taylor predictor for one body of an FP64 state tile in shared memory ([14][TJ] doubles).
+__device__ __forceinline__ void predict_from_tile(const double *st, int b, double t, double (&xp)[3], double (&vp)[3],
+                                                  double &m) {
+    m = st[b];
+    const double dt = t - st[13 * TJ + b];
+    const double c2 = taylor_c2(dt), c3 = taylor_c3(dt);
+#pragma unroll
+    for (int c = 0; c < 3; ++c)
+        predict_component(st[(1 + c) * TJ + b], st[(4 + c) * TJ + b], st[(7 + c) * TJ + b], st[(10 + c) * TJ + b], dt,
+                          c2, c3, xp[c], vp[c]);
+}
+
 // Each thread owns one PAIR of i-particles; WI warps along i (64 i each), WJ warps along j (each
 // takes TJ/WJ j's of every tile).  CTA = 32*WI*WJ threads, i-block = 64*WI.
 // JP (blocks of <= 32 active particles, and the ragged tail of small blocks): each thread owns ONE
 // i-particle and the packed halves are two consecutive j; i-block = 32*WI.
-template <int WI, int WJ, int MINB, bool JP = false>
+//
+// Local frame.  Every warp takes the centre c of the bounding box of ITS i-particles as origin.  If all of
+// them satisfy |x_i - c|^2 <= g2 * h2_i the warp re-expresses its share of every j-tile in that frame
+// once per tile (x'_j = fl(fl(xh_j - c) + xl_j), into a warp-private slice of shared memory; from the FP64
+// state: x'_j = fl(x_j - c)) and the pair loop needs ONE add per component: 27 packed instructions per
+// (2 i x 1 j) instead of 33.  Error of the difference: <= 1.8e-7 |dx| + 2.4e-7 |x_i - c| (half of that from
+// the FP64 state), and regular pairs have |dx| >= h_i, so the guard bounds the relative error by
+// 1.8e-7 + 2.4e-7 sqrt(g2) -- inside the tolerance budget and translation invariant.
+// The i-particle is transformed with the same two operations, so its own record still sits at r = 0
+// exactly.  A warp that fails the guard (scattered block, h2 <= 0) keeps the hi/lo differencing.
+template <int WI, int WJ, int MINB, bool JP = false, int SRC = SRC_REC>
 __global__ void __launch_bounds__(32 * WI *WJ, MINB) force_kernel(const ForceParams p) {
-    constexpr int NW = WI * WJ;
-    constexpr int NH = JP ? 1 : 2;           // i-particles per thread
-    constexpr int NU = JP ? 2 : 4;           // packed iterations per group of four j
+    using SM = ForceSmem<WI, WJ, JP, SRC>;
+    using SC = SrcCfg<SRC>;
+    constexpr int NW = SM::NW, NT = SM::NT, NH = SM::NH, SUB = SM::SUB, NST = SC::NST;
     constexpr int IB = 32 * NH * WI;
-    constexpr int SUB = TJ / WJ;
-    constexpr uint32_t TILE_BYTES = TILE_FLOATS * sizeof(float);
+    constexpr int SLICE = SC::SLICE_COMP * SUB;
     static_assert(SUB % UNROLL_J == 0 && UNROLL_J == 4, "a group is one LDS.128 per component");
 
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    float *srec = reinterpret_cast<float *>(smem_raw);                         // [NSTAGE][RECF][TJ]
-    // FP64 running sums live in shared memory ([14][threads], touched once per flush): 28 registers
-    // per thread go to the pair arithmetic instead.
-    double *acc64 = reinterpret_cast<double *>(smem_raw + (size_t)NSTAGE * TILE_BYTES) + threadIdx.x;
-    constexpr int NT = 32 * WI * WJ;
-    uint64_t *full = reinterpret_cast<uint64_t *>(smem_raw + (size_t)NSTAGE * TILE_BYTES + (size_t)14 * NT * sizeof(double));
-    int *done = reinterpret_cast<int *>(full + NSTAGE);                        // warps finished with a stage
+    unsigned char *ring = smem_raw;                                            // [NST][STAGE_BYTES]
+    float *slice = reinterpret_cast<float *>(smem_raw + SM::RING) + (threadIdx.x >> 5) * SLICE;   // this warp's
+    // FP64 running sums live in shared memory ([7 NH][threads], touched once per flush): the registers
+    // go to the pair arithmetic instead.
+    double *acc64 = reinterpret_cast<double *>(smem_raw + SM::RING + SM::SLICES) + threadIdx.x;
+    uint64_t *full = reinterpret_cast<uint64_t *>(smem_raw + SM::RING + SM::SLICES + SM::ACC);
+    int *done = reinterpret_cast<int *>(full + NST);                           // warps finished with a stage
 
     const int tid = threadIdx.x;
     const int warp = tid >> 5, lane = tid & 31;
@@ -360,41 +665,11 @@ __global__ void __launch_bounds__(32 * WI *WJ, MINB) force_kernel(const ForcePar
     const int tile_begin = p.tile0 + blockIdx.y * p.tiles_per_split;
     const int tile_end = min(tile_begin + p.tiles_per_split, p.ntiles);
     const int ntile = max(tile_end - tile_begin, 0);
-
-    // ---- a3: gather the i-state (the i-particle IS predicted record idx_i[k]; reading R3)
-    IPair I;
-    int32_t my_idx[2], my_k[2];
-    {
-        float v[2][10];
-#pragma unroll
-        for (int h = 0; h < 2; ++h) {
-            const int k = blockIdx.x * IB + wi * (32 * NH) + (JP ? 0 : h * 32) + lane;   // JP: both halves = the same i
-            my_k[h] = k;
-            if (k < p.n_i) {
-                const int32_t idx = p.idx_i ? p.idx_i[k] : k;      // NULL = identity block (full-N pass)
-                const float *r = p.irec ? p.irec + k : rec_slot(p.rec, idx);
-                const int64_t cs = p.irec ? p.n_i_pad : TJ;        // component stride
-                my_idx[h] = idx;
-#pragma unroll
-                for (int c = 0; c < 9; ++c) v[h][c] = -r[c * cs];
-                v[h][9] = fmaxf(__double2float_rn(p.h2_i[k]), TINY_H2);
-            } else {    // padding lane: far from everything (also from the ghost j's), result discarded
-                my_idx[h] = -1;
-                v[h][0] = v[h][1] = v[h][2] = GHOST_POS;        // i.e. position -GHOST_POS
-                v[h][3] = v[h][4] = v[h][5] = v[h][6] = v[h][7] = v[h][8] = 0.f;
-                v[h][9] = TINY_H2;
-            }
-        }
-        I.nxh = make_float2(v[0][C_XH], v[1][C_XH]); I.nyh = make_float2(v[0][C_YH], v[1][C_YH]);
-        I.nzh = make_float2(v[0][C_ZH], v[1][C_ZH]); I.nxl = make_float2(v[0][C_XL], v[1][C_XL]);
-        I.nyl = make_float2(v[0][C_YL], v[1][C_YL]); I.nzl = make_float2(v[0][C_ZL], v[1][C_ZL]);
-        I.nvx = make_float2(v[0][C_VX], v[1][C_VX]); I.nvy = make_float2(v[0][C_VY], v[1][C_VY]);
-        I.nvz = make_float2(v[0][C_VZ], v[1][C_VZ]); I.h2 = make_float2(v[0][9], v[1][9]);
-    }
+    TL_STAMP(blockIdx.y * gridDim.x + blockIdx.x, 0);
 
     if (tid == 0) {
 #pragma unroll
-        for (int s = 0; s < NSTAGE; ++s) {
+        for (int s = 0; s < NST; ++s) {
             mbar_init(&full[s], 1);
             done[s] = 0;
         }
@@ -402,75 +677,261 @@ __global__ void __launch_bounds__(32 * WI *WJ, MINB) force_kernel(const ForcePar
     }
     __syncthreads();
 
-    auto issue = [&](int tile, int s) {     // one bulk copy per tile (10 KB), completion on full[s]
-        mbar_arrive_expect_tx(&full[s], TILE_BYTES);
-        bulk_g2s(srec + (size_t)s * TILE_FLOATS, p.rec + (size_t)tile * TILE_FLOATS, TILE_BYTES, &full[s]);
+    auto issue = [&](int tile, int s) {     // one tile into stage s, completion counted in bytes on full[s]
+        mbar_arrive_expect_tx(&full[s], SC::STAGE_BYTES);
+        if constexpr (SRC == SRC_REC) {
+            bulk_g2s(ring + (size_t)s * SC::STAGE_BYTES, p.rec + (size_t)tile * TILE_FLOATS, SC::STAGE_BYTES, &full[s]);
+        } else {
+            double *dst = reinterpret_cast<double *>(ring + (size_t)s * SC::STAGE_BYTES);
+#pragma unroll
+            for (int c = 0; c < STATE_D; ++c)      // row c of the state: 256 consecutive doubles
+                bulk_g2s(dst + c * TJ, p.soa + (size_t)c * p.Ns + (size_t)tile * TJ, TJ * sizeof(double), &full[s]);
+        }
     };
-    if (tid == 0) {
-        for (int s = 0; s < NSTAGE && s < ntile; ++s) issue(tile_begin + s, s);
+    if (tid == 0) {     // the first copies fly while the i-state is gathered
+        for (int s = 0; s < NST && s < ntile; ++s) issue(tile_begin + s, s);
     }
 
+    // ---- a3: gather the i-state (the i-particle IS predicted record idx_i[k]; reading R3), choose the frame
+    IPair I;
+    int32_t my_idx[2], my_k[2];
+    bool local;
+    float org[3];
+    {
+        float ph[2][3], pl[2][3], pv[2][3], ph2[2];
+        double pd[2][3];
+        bool valid[2];
 #pragma unroll
-    for (int c = 0; c < 14; ++c) acc64[c * NT] = 0.0;          // slot h * 7 + c of this thread
-
-    Acc7 A;                   // FP32 partial sums of at most TJ pair terms (WJ tile shares of SUB j each)
-    A.ax = A.ay = A.az = A.jx = A.jy = A.jz = A.ph = make_float2(0.f, 0.f);
-
-    for (int it = 0; it < ntile; ++it) {
-        const int s = it % NSTAGE;
-        mbar_wait(&full[s], (uint32_t)((it / NSTAGE) & 1));
-        const float *tsub = srec + (size_t)s * TILE_FLOATS + wj * SUB;      // &tile[0][wj * SUB]
-        const int32_t jbase = p.j_offset + (tile_begin + it) * TJ + wj * SUB;
-
-#pragma unroll GROUP_UNROLL
-        for (int g = 0; g < SUB; g += UNROLL_J) {
-            float4 c4[RECF];                                   // component rows of 4 consecutive j
+        for (int h = 0; h < NH; ++h) {
+            const int slot = blockIdx.x * IB + wi * (32 * NH) + h * 32 + lane;
+            valid[h] = slot < p.n_i;
+            const int k = (valid[h] && p.perm) ? p.perm[slot] : slot;      // caller's numbering: rows, counters, inputs
+            my_k[h] = k;
+            my_idx[h] = -1;
 #pragma unroll
-            for (int c = 0; c < RECF; ++c)                     // warp-uniform address: LDS.128 broadcast
-                c4[c] = *reinterpret_cast<const float4 *>(tsub + c * TJ + g);
-            // phase 1: FP64-equivalent differences and r^2 of the group's 4 j against the i-pair
-            float2 dx[NU], dy[NU], dz[NU], r2[NU], rinv[NU];
+            for (int c = 0; c < 3; ++c) { ph[h][c] = pl[h][c] = pv[h][c] = 0.f; pd[h][c] = 0.0; }
+            ph2[h] = TINY_H2;
+            // Only the warps with wj == 0 go to global memory: the other WJ - 1 warps of the CTA hold the
+            // same i and get the values through shared memory below (every CTA of the grid asks L2 for
+            // the same few lines at the same moment; eight times fewer requests shorten that queue).
+            if (valid[h] && (WJ == 1 || wj == 0)) {
+                const int32_t idx = p.idx_i ? p.idx_i[k] : k;      // NULL = identity block (full-N pass)
+                my_idx[h] = idx;
+                ph2[h] = fmaxf(__double2float_rn(p.h2_i[k]), TINY_H2);
+                if constexpr (SRC == SRC_STATE) {                  // the predictor's own arithmetic on body idx
+                    const double *s0 = p.soa + idx;
+                    const double dt = p.t - s0[(size_t)13 * p.Ns];
+                    const double c2 = taylor_c2(dt), c3 = taylor_c3(dt);
 #pragma unroll
-            for (int u = 0; u < NU; ++u) {
-                dx[u] = padd(padd(jop<JP>(c4[C_XH], u), I.nxh), padd(jop<JP>(c4[C_XL], u), I.nxl));
-                dy[u] = padd(padd(jop<JP>(c4[C_YH], u), I.nyh), padd(jop<JP>(c4[C_YL], u), I.nyl));
-                dz[u] = padd(padd(jop<JP>(c4[C_ZH], u), I.nzh), padd(jop<JP>(c4[C_ZL], u), I.nzl));
-                r2[u] = pfma(dz[u], dz[u], pfma(dy[u], dy[u], pmul(dx[u], dx[u])));
-                rinv[u].x = rsqrt_sfu(r2[u].x);        // issued before the vote: SFU latency overlaps the test
-                rinv[u].y = rsqrt_sfu(r2[u].y);
-            }
-            // one test per i for the whole group (FMNMX3): a neighbour, or the self pair (r2 == 0)?
-            float mn0, mn1;
-            if constexpr (JP) {
-                mn0 = fminf(r2[0].x, r2[1].x);
-                mn1 = fminf(r2[0].y, r2[1].y);
-            } else {
-                mn0 = fminf(fminf(fminf(r2[0].x, r2[1].x), r2[2].x), r2[3].x);
-                mn1 = fminf(fminf(fminf(r2[0].y, r2[1].y), r2[2].y), r2[3].y);
-            }
-            const bool hit = (mn0 < I.h2.x) | (mn1 < I.h2.y);
-            if (!__any_sync(0xffffffffu, hit)) {    // ~95 % of groups at N_b ~ 150, N = 1M: nothing to mask
+                    for (int c = 0; c < 3; ++c) {
+                        double xp, vp;
+                        predict_component(s0[(size_t)(1 + c) * p.Ns], s0[(size_t)(4 + c) * p.Ns],
+                                          s0[(size_t)(7 + c) * p.Ns], s0[(size_t)(10 + c) * p.Ns], dt, c2, c3, xp, vp);
+                        pd[h][c] = xp;
+                        ph[h][c] = __double2float_rn(xp);
+                        pl[h][c] = __double2float_rn(xp - (double)ph[h][c]);
+                        pv[h][c] = __double2float_rn(vp);
+                    }
+                } else {
+                    const float *r = p.irec ? p.irec + k : rec_slot(p.rec, idx);
+                    const int64_t cs = p.irec ? p.n_i_pad : TJ;    // component stride
 #pragma unroll
-                for (int u = 0; u < NU; ++u)
-                    pair_terms<false>(A, I, dx[u], dy[u], dz[u], r2[u], rinv[u], jop<JP>(c4[C_VX], u),
-                                      jop<JP>(c4[C_VY], u), jop<JP>(c4[C_VZ], u), jop<JP>(c4[C_M], u));
-            } else {
-#pragma unroll
-                for (int u = 0; u < NU; ++u)
-                    pair_terms<true>(A, I, dx[u], dy[u], dz[u], r2[u], rinv[u], jop<JP>(c4[C_VX], u),
-                                     jop<JP>(c4[C_VY], u), jop<JP>(c4[C_VZ], u), jop<JP>(c4[C_M], u));
-                if (hit) {      // rare: lanes hold different i, each takes slots of its own rows
-#pragma unroll
-                    for (int u = 0; u < NU; ++u) {
-                        // half .x / .y of iteration u: (i, j) = (my i 0, j u) / (my i 1, j u), or, j-packed,
-                        // (my i, j 2u) / (my i, j 2u + 1)
-                        const int32_t jg0 = jbase + g + (JP ? 2 * u : u), jg1 = JP ? jg0 + 1 : jg0;
-                        if (r2[u].x < I.h2.x && jg0 != my_idx[0]) append_one(my_k[0], jg0, p.cap, p.cnt, p.nblist);
-                        if (r2[u].y < I.h2.y && jg1 != my_idx[1]) append_one(my_k[1], jg1, p.cap, p.cnt, p.nblist);
+                    for (int c = 0; c < 3; ++c) {
+                        ph[h][c] = r[(C_XH + c) * cs];
+                        pl[h][c] = r[(C_XL + c) * cs];
+                        pv[h][c] = r[(C_VX + c) * cs];
                     }
                 }
             }
         }
+        if constexpr (WJ > 1) {
+            constexpr int NF = (SRC == SRC_STATE) ? 17 : 11;       // words per (i-warp, half, lane)
+            static_assert((size_t)WI * 2 * NF * 32 * sizeof(float) <= SM::ACC, "the exchange uses the (still unused) FP64 sums");
+            float *xch = reinterpret_cast<float *>(smem_raw + SM::RING + SM::SLICES) + (size_t)wi * 2 * NF * 32 + lane;
+#pragma unroll
+            for (int h = 0; h < NH; ++h) {
+                float *x = xch + h * NF * 32;
+                if (wj == 0) {
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) { x[c * 32] = ph[h][c]; x[(3 + c) * 32] = pl[h][c]; x[(6 + c) * 32] = pv[h][c]; }
+                    x[9 * 32] = ph2[h];
+                    x[10 * 32] = __int_as_float(my_idx[h]);
+                    if constexpr (SRC == SRC_STATE) {
+#pragma unroll
+                        for (int c = 0; c < 3; ++c) {
+                            x[(11 + 2 * c) * 32] = __int_as_float(__double2hiint(pd[h][c]));
+                            x[(12 + 2 * c) * 32] = __int_as_float(__double2loint(pd[h][c]));
+                        }
+                    }
+                }
+            }
+            __syncthreads();
+#pragma unroll
+            for (int h = 0; h < NH; ++h) {
+                const float *x = xch + h * NF * 32;
+                if (wj != 0) {
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) { ph[h][c] = x[c * 32]; pl[h][c] = x[(3 + c) * 32]; pv[h][c] = x[(6 + c) * 32]; }
+                    ph2[h] = x[9 * 32];
+                    my_idx[h] = __float_as_int(x[10 * 32]);
+                    if constexpr (SRC == SRC_STATE) {
+#pragma unroll
+                        for (int c = 0; c < 3; ++c)
+                            pd[h][c] = __hiloint2double(__float_as_int(x[(11 + 2 * c) * 32]), __float_as_int(x[(12 + 2 * c) * 32]));
+                    }
+                }
+            }
+            __syncthreads();                                       // the region becomes the FP64 sums below
+        }
+        if constexpr (JP) {       // both halves of the registers hold the same i
+            my_k[1] = my_k[0]; my_idx[1] = my_idx[0]; valid[1] = valid[0]; ph2[1] = ph2[0];
+#pragma unroll
+            for (int c = 0; c < 3; ++c) { ph[1][c] = ph[0][c]; pl[1][c] = pl[0][c]; pv[1][c] = pv[0][c]; pd[1][c] = pd[0][c]; }
+        }
+        // the warp's origin: centre of the bounding box of its valid i (an FP32 number; any value is correct)
+        float mn[3], mx[3];
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            mn[c] = 3.0e38f; mx[c] = -3.0e38f;
+#pragma unroll
+            for (int h = 0; h < 2; ++h)
+                if (valid[h]) { mn[c] = fminf(mn[c], ph[h][c]); mx[c] = fmaxf(mx[c], ph[h][c]); }
+#pragma unroll
+            for (int off = 16; off > 0; off >>= 1) {
+                mn[c] = fminf(mn[c], __shfl_xor_sync(0xffffffffu, mn[c], off));
+                mx[c] = fmaxf(mx[c], __shfl_xor_sync(0xffffffffu, mx[c], off));
+            }
+            org[c] = mn[c] <= mx[c] ? __fmul_rn(0.5f, __fadd_rn(mn[c], mx[c])) : 0.f;
+        }
+        float ip[2][3];
+        bool ok = true;
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            float d2 = 0.f;
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                // EXACTLY the operations the staging applies to a j: the particle's own record lands on itself
+                if constexpr (SRC == SRC_STATE) ip[h][c] = __double2float_rn(pd[h][c] - (double)org[c]);
+                else ip[h][c] = __fadd_rn(__fadd_rn(ph[h][c], -org[c]), pl[h][c]);
+                d2 = fmaf(ip[h][c], ip[h][c], d2);
+            }
+            ok = ok && (!valid[h] || d2 <= p.g2 * ph2[h]);
+        }
+        local = (p.g2 > 0.f) && __all_sync(0xffffffffu, ok);
+        if (p.stats && lane == 0) {
+            atomicAdd(p.stats + 1, 1u);
+            if (local) atomicAdd(p.stats, 1u);
+        }
+        float nx[2][3], nl[2][3];
+#pragma unroll
+        for (int h = 0; h < 2; ++h)
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                // padding lane: far from everything (also from the ghost j's), result discarded
+                nx[h][c] = !valid[h] ? GHOST_POS : local ? -ip[h][c] : -ph[h][c];
+                nl[h][c] = (!valid[h] || local) ? 0.f : -pl[h][c];
+            }
+        I.nxh = make_float2(nx[0][0], nx[1][0]); I.nyh = make_float2(nx[0][1], nx[1][1]);
+        I.nzh = make_float2(nx[0][2], nx[1][2]); I.nxl = make_float2(nl[0][0], nl[1][0]);
+        I.nyl = make_float2(nl[0][1], nl[1][1]); I.nzl = make_float2(nl[0][2], nl[1][2]);
+        I.nvx = make_float2(-pv[0][0], -pv[1][0]); I.nvy = make_float2(-pv[0][1], -pv[1][1]);
+        I.nvz = make_float2(-pv[0][2], -pv[1][2]); I.h2 = make_float2(ph2[0], ph2[1]);
+    }
+
+#pragma unroll
+    for (int c = 0; c < 7 * NH; ++c) acc64[c * NT] = 0.0;      // slot h * 7 + c of this thread
+
+    Acc7 A;                   // FP32 partial sums of at most TJ pair terms (WJ tile shares of SUB j each)
+    A.ax = A.ay = A.az = A.jx = A.jy = A.jz = A.ph = make_float2(0.f, 0.f);
+
+    // Stage hand-back without a CTA barrier: the LAST warp to finish with stage s refills it, so
+    // warps drift up to NST-1 tiles apart instead of meeting at a __syncthreads every tile.
+    auto release = [&](int it, int s) {
+        __syncwarp();
+        if (lane == 0) {
+            __threadfence_block();                       // my reads of stage s are done (release)
+            if (atomicAdd(&done[s], 1) == NW - 1) {
+                done[s] = 0;
+                __threadfence_block();
+                if (it + NST < ntile) {
+                    fence_proxy_async_smem();            // generic reads -> async-proxy overwrite
+                    issue(tile_begin + it + NST, s);
+                }
+            }
+        }
+    };
+
+    TL_STAMP(blockIdx.y * gridDim.x + blockIdx.x, 1);
+    for (int it = 0; it < ntile; ++it) {
+        const int s = it % NST;
+        mbar_wait(&full[s], (uint32_t)((it / NST) & 1));
+        if (it == 0) TL_STAMP(blockIdx.y * gridDim.x + blockIdx.x, 2);
+        const int32_t jbase = p.j_offset + (tile_begin + it) * TJ + wj * SUB;
+
+        if constexpr (SRC == SRC_STATE) {
+            // predict the j's this warp is about to consume into its slice; the stage is free right after
+            const double *st = reinterpret_cast<const double *>(ring + (size_t)s * SC::STAGE_BYTES);
+#pragma unroll
+            for (int q = lane; q < SUB; q += 32) {
+                double xp[3], vp[3], m;
+                predict_from_tile(st, wj * SUB + q, p.t, xp, vp, m);
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    if (local) {
+                        slice[c * SUB + q] = __double2float_rn(xp[c] - (double)org[c]);
+                        slice[(3 + c) * SUB + q] = __double2float_rn(vp[c]);
+                    } else {
+                        const float hi = __double2float_rn(xp[c]);
+                        slice[c * SUB + q] = hi;
+                        slice[(3 + c) * SUB + q] = __double2float_rn(xp[c] - (double)hi);
+                        slice[(6 + c) * SUB + q] = __double2float_rn(vp[c]);
+                    }
+                }
+                slice[(local ? 6 : 9) * SUB + q] = __double2float_rn(m);
+            }
+            release(it, s);                              // (starts with __syncwarp: the slice is complete)
+            if (local) {
+                const JPtrs P = {slice, nullptr, slice + 3 * SUB, slice + 6 * SUB};
+                tile_pairs<true, JP, SUB, SUB, SUB>(A, I, P, jbase, my_idx, my_k, p);
+            } else {
+                const JPtrs P = {slice, slice + 3 * SUB, slice + 6 * SUB, slice + 9 * SUB};
+                tile_pairs<false, JP, SUB, SUB, SUB>(A, I, P, jbase, my_idx, my_k, p);
+            }
+            __syncwarp();                                // every lane is out of the slice before it is rewritten
+        } else {
+            const float *tsub = reinterpret_cast<const float *>(ring + (size_t)s * SC::STAGE_BYTES) + wj * SUB;
+            if (local) {
+                // x'_j = fl(fl(xh_j - c) + xl_j) for the warp's share of the tile (the i got the same two operations)
+                if constexpr (SUB >= 128) {
+#pragma unroll
+                    for (int q = 4 * lane; q < SUB; q += 128)
+#pragma unroll
+                        for (int c = 0; c < 3; ++c) {
+                            const float4 hi = *reinterpret_cast<const float4 *>(tsub + (C_XH + c) * TJ + q);
+                            const float4 lo = *reinterpret_cast<const float4 *>(tsub + (C_XL + c) * TJ + q);
+                            const float2 no = make_float2(-org[c], -org[c]);
+                            const float2 a = padd(padd(make_float2(hi.x, hi.y), no), make_float2(lo.x, lo.y));
+                            const float2 b = padd(padd(make_float2(hi.z, hi.w), no), make_float2(lo.z, lo.w));
+                            *reinterpret_cast<float4 *>(slice + c * SUB + q) = make_float4(a.x, a.y, b.x, b.y);
+                        }
+                } else {
+#pragma unroll
+                    for (int q = lane; q < SUB; q += 32)
+#pragma unroll
+                        for (int c = 0; c < 3; ++c)
+                            slice[c * SUB + q] =
+                                __fadd_rn(__fadd_rn(tsub[(C_XH + c) * TJ + q], -org[c]), tsub[(C_XL + c) * TJ + q]);
+                }
+                __syncwarp();
+                const JPtrs P = {slice, nullptr, tsub + C_VX * TJ, tsub + C_M * TJ};
+                tile_pairs<true, JP, SUB, SUB, TJ>(A, I, P, jbase, my_idx, my_k, p);
+            } else {
+                const JPtrs P = {tsub, tsub + C_XL * TJ, tsub + C_VX * TJ, tsub + C_M * TJ};
+                tile_pairs<false, JP, SUB, TJ, TJ>(A, I, P, jbase, my_idx, my_k, p);
+            }
+            release(it, s);                              // (its __syncwarp also frees the slice)
+        }
+
         // flush: FP32 partial sums of <= WJ * SUB = TJ terms go into the FP64 running sums
         if ((it + 1) % WJ == 0 || it + 1 == ntile) {
             const float2 *Av = &A.ax;       // ax, ay, az, jx, jy, jz, ph
@@ -485,23 +946,9 @@ __global__ void __launch_bounds__(32 * WI *WJ, MINB) force_kernel(const ForcePar
             }
             A.ax = A.ay = A.az = A.jx = A.jy = A.jz = A.ph = make_float2(0.f, 0.f);
         }
-
-        // Stage hand-back without a CTA barrier: the LAST warp to finish with stage s refills it, so
-        // warps drift up to NSTAGE-1 tiles apart instead of meeting at a __syncthreads every tile.
-        __syncwarp();
-        if (lane == 0) {
-            __threadfence_block();                       // my reads of stage s are done (release)
-            if (atomicAdd(&done[s], 1) == NW - 1) {
-                done[s] = 0;
-                __threadfence_block();
-                if (it + NSTAGE < ntile) {
-                    fence_proxy_async_smem();            // generic reads -> async-proxy overwrite
-                    issue(tile_begin + it + NSTAGE, s);
-                }
-            }
-        }
     }
 
+    TL_STAMP(blockIdx.y * gridDim.x + blockIdx.x, 3);
     // ---- a6: fixed-order reduction over the WJ warps that shared these i, then one partial per split
     double out64[NH][7];
 #pragma unroll
@@ -509,8 +956,8 @@ __global__ void __launch_bounds__(32 * WI *WJ, MINB) force_kernel(const ForcePar
 #pragma unroll
         for (int c = 0; c < 7; ++c) out64[h][c] = acc64[(h * 7 + c) * NT];
     if constexpr (WJ > 1) {
-        double *red = reinterpret_cast<double *>(smem_raw);     // reuse the tile ring: [WJ][7][IB]
-        __syncthreads();                                         // every warp is out of the ring
+        double *red = reinterpret_cast<double *>(smem_raw);     // reuse the ring and the slices: [WJ][7][IB]
+        __syncthreads();                                         // every warp is out of both
 #pragma unroll
         for (int h = 0; h < NH; ++h) {
             const int il = wi * (32 * NH) + h * 32 + lane;
@@ -534,26 +981,29 @@ __global__ void __launch_bounds__(32 * WI *WJ, MINB) force_kernel(const ForcePar
     if (wj == 0) {
 #pragma unroll
         for (int h = 0; h < NH; ++h) {
-            const int k = my_k[h];    // k < n_i_pad always
+            const int slot = blockIdx.x * IB + wi * (32 * NH) + h * 32 + lane;    // slot < n_i_pad always
 #pragma unroll
             for (int c = 0; c < 7; ++c)
-                p.partial[((size_t)(p.split0 + blockIdx.y) * 7 + c) * p.n_i_pad + k] = out64[h][c];
+                p.partial[((size_t)(p.split0 + blockIdx.y) * 7 + c) * p.n_i_pad + slot] = out64[h][c];
         }
     }
+    TL_STAMP(blockIdx.y * gridDim.x + blockIdx.x, 4);
 }
 
 // ------------------------------------------------------------------ a6-a7: finalize
-// ONE launch, two roles, grid = (ceil(n_i / 32), 7 + ceil(32 / sortW)), CTA = 32 x W threads:
+// ONE launch, two roles, grid = (ceil(n_i / 32), 7 + 32), CTA = 32 x W threads:
 //   blockIdx.y <  7 : fixed-order sum of the S split partials of quantity q = blockIdx.y for 32
-//                     consecutive active particles -- lanes along i (coalesced 256 B rows), warps along
-//                     the splits with eight loads in flight each, then the W warps in order.
-//   blockIdx.y >= 7 : one warp per list row: nnb / overflow from the row counter (re-zeroed for the next
-//                     call) and a bitonic sort of the stored entries in shared memory (sortP ints per
-//                     warp, sortW <= W warps per CTA; sortP = 0: rows too long, left in append order).  Sorting makes the list
-//                     output deterministic and equal to the oracle's ascending rows.
+//                     consecutive SLOTS of the (possibly reordered) block -- lanes along i (coalesced
+//                     256 B rows), warps along the splits with eight loads in flight each, then the W
+//                     warps in order; slot s is active particle k = perm[s] (perm = NULL: k = s).
+//   blockIdx.y >= 7 : ONE list row per CTA (k = 32 blockIdx.x + blockIdx.y - 7): nnb / overflow from the
+//                     row counter (re-zeroed for the next call) and a bitonic sort of the stored entries
+//                     in shared memory by the whole CTA (sortP ints; sortP = 0: rows too long, left in
+//                     append order).  Sorting makes the list output deterministic and equal to the
+//                     oracle's ascending rows.
 template <int W>
 __global__ void __launch_bounds__(32 * W) finalize_kernel(int32_t n_i, int32_t n_i_pad, int32_t S, int32_t cap,
-                                                          int32_t sortP, int32_t sortW,
+                                                          int32_t sortP, const int32_t *__restrict__ perm,
                                                           const double *__restrict__ partial,
                                                           int32_t *__restrict__ cnt, double *__restrict__ acc,
                                                           double *__restrict__ jerk, double *__restrict__ pot,
@@ -561,14 +1011,17 @@ __global__ void __launch_bounds__(32 * W) finalize_kernel(int32_t n_i, int32_t n
                                                           int32_t *__restrict__ overflow) {
     extern __shared__ int32_t sbuf[];
     __shared__ double red[W][32];
+    __shared__ int32_t row_cnt;
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    TL_STAMP(4096 + blockIdx.y * gridDim.x + blockIdx.x, 0);
     // launched with programmatic stream serialization: the grid is resident before the force kernel
     // has drained; everything it reads is valid after this wait (a no-op in an ordinary launch)
     asm volatile("griddepcontrol.wait;" ::: "memory");
+    TL_STAMP(4096 + blockIdx.y * gridDim.x + blockIdx.x, 1);
     if (blockIdx.y < 7) {
         const int q = blockIdx.y;
-        const int k = blockIdx.x * 32 + lane;          // k < n_i_pad always (n_i_pad is a multiple of 32)
-        const double *src = partial + (size_t)q * n_i_pad + k;
+        const int slot = blockIdx.x * 32 + lane;       // slot < n_i_pad always (n_i_pad is a multiple of 32)
+        const double *src = partial + (size_t)q * n_i_pad + slot;
         const size_t stride = (size_t)7 * n_i_pad;
         double s = 0.0;
         for (int base = w; base < S; base += 8 * W) {
@@ -583,47 +1036,50 @@ __global__ void __launch_bounds__(32 * W) finalize_kernel(int32_t n_i, int32_t n
         }
         red[w][lane] = s;
         __syncthreads();
-        if (w == 0 && k < n_i) {
+        if (w == 0 && slot < n_i) {
             double t = red[0][lane];
 #pragma unroll
             for (int ww = 1; ww < W; ++ww) t += red[ww][lane];
+            const int k = perm ? perm[slot] : slot;
             if (q < 3) acc[3 * k + q] = t;
             else if (q < 6) jerk[3 * k + q - 3] = t;
             else pot[k] = -t;
         }
+        TL_STAMP(4096 + blockIdx.y * gridDim.x + blockIdx.x, 2);
         return;
     }
-    const int r = (blockIdx.y - 7) * sortW + w;                  // row of this 32-row chunk
-    const int k = blockIdx.x * 32 + r;
-    if (w >= sortW || r >= 32 || k >= n_i) return;
-    int c = 0;
-    if (lane == 0) {
-        c = cnt[k];
-        nnb[k] = c;
-        overflow[k] = c > cap ? 1 : 0;
+    const int k = blockIdx.x * 32 + (blockIdx.y - 7);
+    if (k >= n_i) return;
+    if (threadIdx.x == 0) {
+        const int32_t c0 = cnt[k];
+        nnb[k] = c0;
+        overflow[k] = c0 > cap ? 1 : 0;
         cnt[k] = 0;     // keep the counters zero between calls
+        row_cnt = c0;
     }
-    c = min(__shfl_sync(0xffffffffu, c, 0), cap);
+    __syncthreads();
+    const int c = min(row_cnt, cap);
     if (c < 2 || !nblist || sortP == 0) return;
     int Pk = 32;
     while (Pk < c) Pk <<= 1;                                     // this row's power of two (<= sortP)
-    int32_t *b = sbuf + (size_t)w * sortP;
     int32_t *row = nblist + (int64_t)k * cap;
-    for (int e = lane; e < Pk; e += 32) b[e] = e < c ? row[e] : 0x7fffffff;
-    __syncwarp();
+    const int T = 32 * W;
+    for (int e = threadIdx.x; e < Pk; e += T) sbuf[e] = e < c ? row[e] : 0x7fffffff;
+    __syncthreads();
     for (int size = 2; size <= Pk; size <<= 1) {
         for (int stride = size >> 1; stride > 0; stride >>= 1) {
-            for (int e = lane; e < (Pk >> 1); e += 32) {
+            for (int e = threadIdx.x; e < (Pk >> 1); e += T) {
                 const int lo = 2 * e - (e & (stride - 1));       // index with bit `stride` clear
                 const int hi = lo + stride;
                 const bool up = (lo & size) == 0;
-                const int32_t x = b[lo], y = b[hi];
-                if ((x > y) == up) { b[lo] = y; b[hi] = x; }
+                const int32_t x = sbuf[lo], y = sbuf[hi];
+                if ((x > y) == up) { sbuf[lo] = y; sbuf[hi] = x; }
             }
-            __syncwarp();
+            __syncthreads();
         }
     }
-    for (int e = lane; e < c; e += 32) row[e] = b[e];
+    for (int e = threadIdx.x; e < c; e += T) row[e] = sbuf[e];
+    TL_STAMP(4096 + blockIdx.y * gridDim.x + blockIdx.x, 3);
 }
 
 // ------------------------------------------------------------------ NEXT-2: neighbour (irregular) force
