@@ -26,7 +26,8 @@ most double, doubling only at commensurate times) hold along an integration; a P
 conserves energy.  ``aarseth_step``: for harmonic motion a(t) = A cos(wt) e the criterion is exactly
 sqrt(eta) / w at every phase and amplitude (closed form), plus two cases worked by hand with a2 handed
 in at the start of the step (so "a2 advanced by dt a3" is pinned); ``initial_step``: hand cases on and
-off a power of two and at the dt_max cap.  Thirteen single-term mutations of those two functions (no
+off a power of two and at the dt_max cap; the degenerate-criterion rule R32 (dt_req = 0 / NaN keeps
+the step, nothing falls below dt_max 2^-40) on hand cases.  Thirteen single-term mutations of those two functions (no
 sqrt, swapped or dropped products, wrong powers, a2 at the start, ceil for floor, ...) each fail a test.
 """
 from __future__ import annotations
@@ -84,26 +85,40 @@ def aarseth_step(a1, j1, a2_0, a3, dt, eta):
     return np.sqrt(eta * (na * n2 + nj * nj) / (nj * n3 + n2 * n2))
 
 
-def quantize_step(dt_req, dt_old, t1, dt_max):
+DT_MIN_LEVELS = 40      # reading R32: no step below dt_max * 2^-40
+
+
+def quantize_step(dt_req, dt_old, t1, dt_max, dt_min=None):
     """Block-step rule (steps are integer powers of 0.5).  Candidate = dt_old; it is doubled once
     if dt_req >= 2 dt_old, 2 dt_old <= dt_max and t1 is a multiple of 2 dt_old (so that t0 stays a
-    multiple of dt); otherwise it is halved while it exceeds dt_req."""
+    multiple of dt); otherwise it is halved while it exceeds dt_req.
+    Degenerate criterion (reading R32; the paper is silent): dt_req = 0 or NaN (a body with
+    a1 = j1 = 0, or every derivative zero) carries no information -- the step is KEPT; and no step is
+    halved below dt_min = dt_max 2^-40, so the block loop can never stall on a vanishing step."""
     dt_req = np.asarray(dt_req, dtype=np.float64)
     out = np.array(dt_old, dtype=np.float64, copy=True)
+    if dt_min is None:
+        dt_min = dt_max * 2.0 ** -DT_MIN_LEVELS
     for k in range(out.shape[0]):
         d = out[k]
+        if not dt_req[k] > 0.0:                 # 0 or NaN: keep the step
+            continue
         if dt_req[k] >= 2.0 * d and 2.0 * d <= dt_max and (t1 / (2.0 * d)) == np.floor(t1 / (2.0 * d)):
             d = 2.0 * d
         else:
-            while d > dt_req[k]:
+            while d > dt_req[k] and d > dt_min:
                 d *= 0.5
         out[k] = d
     return out
 
 
 def initial_step(a, j, eta_s, dt_max):
-    """Start-up step: the largest power of 0.5 not above min(eta_s |a| / |j|, dt_max)."""
-    req = np.minimum(eta_s * _norm(a) / _norm(j), dt_max)
+    """Start-up step: the largest power of 0.5 not above min(eta_s |a| / |j|, dt_max), and not below
+    dt_max 2^-40; |a| = |j| = 0 (no information: NaN) gives dt_max (reading R32)."""
+    with np.errstate(divide="ignore", invalid="ignore"):
+        req = eta_s * _norm(a) / _norm(j)
+    req = np.where(np.isnan(req), dt_max, req)
+    req = np.clip(req, dt_max * 2.0 ** -DT_MIN_LEVELS, dt_max)
     return 2.0 ** np.floor(np.log2(req))
 
 

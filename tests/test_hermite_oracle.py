@@ -207,3 +207,25 @@ def test_initial_step_hand_cases():
     assert H.initial_step(a[1:2], j[1:2], 0.02, 2.0**-6)[0] == 2.0**-6
     assert H.initial_step(a[2:3], j[2:3], 1.0, 1.0)[0] == 2.0**-2
     assert H.initial_step(a[3:], j[3:], 0.01, 1.0)[0] == 2.0**-3
+
+
+def test_degenerate_step_criterion_keeps_the_step_and_has_a_floor():
+    """DESIGN.md reading R32 (the paper is silent): dt_req = 0 or NaN keeps the step instead of
+    halving for ever; halving stops at dt_max 2^-40; start-up steps are clipped to [dt_max 2^-40, dt_max] and
+    |a| = |j| = 0 gives dt_max.  All by hand."""
+    q = H.quantize_step
+    d = 2.0**-6
+    assert q([0.0], [d], 4 * d, 1.0)[0] == d                       # no information: keep
+    assert q([np.nan], [d], 4 * d, 1.0)[0] == d
+    assert q([np.inf], [d], 4 * d, 1.0)[0] == 2 * d                # constant force: may grow as usual
+    assert q([1e-300], [d], 4 * d, 1.0)[0] == 2.0**-40             # floor = dt_max 2^-40
+    assert q([1e-300], [d], 4 * d, 2.0**-3)[0] == 2.0**-43
+    assert q([1e-300], [d], 4 * d, 1.0, dt_min=2.0**-10)[0] == 2.0**-10
+    # isolated body feeling nothing: a1 = j1 = 0 with non-zero old derivatives -> criterion 0 -> step kept
+    z = np.zeros((1, 3))
+    req = H.aarseth_step(z, z, np.array([[1.0, 0, 0]]), np.array([[0, 2.0, 0]]), np.array([d]), 0.02)
+    assert req[0] == 0.0 and q(req, [d], 4 * d, 1.0)[0] == d
+    one = np.array([[1.0, 0.0, 0.0]])
+    assert H.initial_step(z, one, 0.02, 0.125)[0] == 0.125 * 2.0**-40      # |a| = 0: the floor
+    assert H.initial_step(one, z, 0.02, 0.125)[0] == 0.125                 # |j| = 0: dt_max
+    assert H.initial_step(z, z, 0.02, 0.125)[0] == 0.125                   # nothing known: dt_max
