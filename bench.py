@@ -444,7 +444,39 @@ def run_b200(args):
         act = torch.empty(N, dtype=torch.int32, device=dev)
         ms_sel = timed(lambda: ctx.next_block(act))
         ms_cor = timed(lambda: ctx.correct(t_pred, idx, out["acc"], out["jerk"], 0.02, 2.0 ** -3))
+        # NEXT-3 as ONE call per block: 100 consecutive blocks from a mid-run state (t0 = last block time before
+        # 0.3 at each body's level); what a block costs outside its force kernel (selection + its host read-back,
+        # finalize, corrector, launches)
+        lev = np.asarray(cfg["levels"], dtype=np.float64)
+        dt_np = 2.0 ** -lev
+        bctx = nb.nb_open(N, 8, stream)
+        bstate = list(jstate)
+        bstate[5] = f64(np.floor(0.3 / dt_np) * dt_np)
+        bctx.set_j(*bstate)
+        bctx.set_steps(f64(dt_np))
+        for _ in range(5):
+            bctx.block_step(None, 0.02, 2.0 ** -6)
+        torch.cuda.synchronize()
+        bctx.tune("profile", 1)
+        nblk, sizes, fused_blk = 100, [], 0
+        tw0 = time.perf_counter()
+        for _ in range(nblk):
+            _, nn_b = bctx.block_step(None, 0.02, 2.0 ** -6)
+            sizes.append(nn_b); fused_blk += bctx.info("last_fused")
+        torch.cuda.synchronize()
+        wall_us = (time.perf_counter() - tw0) * 1e6
+        force_us = bctx.info("force_kernel_ns") * 1e-3
+        assert bctx.info("force_kernel_count") == nblk
+        bctx.tune("profile", 0)
+        bctx.close()
+        blockstep = {"blocks": nblk, "n_act_median": float(np.median(sizes)), "n_act_min": int(min(sizes)),
+                     "n_act_max": int(max(sizes)), "fused_blocks": int(fused_blk), "us_per_block": wall_us / nblk,
+                     "us_force_kernel_per_block": force_us / nblk,
+                     "us_per_block_outside_force_kernel": (wall_us - force_us) / nblk,
+                     "note": "wall clock over 100 back-to-back nb_block_step calls (h2 = NULL: total force); the force "
+                             "kernel's own time from CUDA events around each of its launches"}
         extras = {
+            "nb_block_step": blockstep,
             "nb_irregular": {"n_i": n_i, "neighbour_pairs": nn, "ms": ms_irr, "pairs_per_s": nn / (ms_irr * 1e-3),
                              "gather_GBps": nn * 128 / (ms_irr * 1e-3) / 1e9, "dtype": "f64"},
             "nb_update_j": {"n": n_i, "ms": ms_upd},

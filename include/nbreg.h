@@ -164,7 +164,8 @@ int nb_irregular(nb_ctx *ctx, double t, int32_t n_i, const int32_t *idx_i, const
 /* Block time steps dt[N] (each an integer power of 0.5 with t0[j] a multiple of dt[j]; unchecked).
  * Copied.  Requires nb_set_j. */
 int nb_set_steps(nb_ctx *ctx, const double *dt);
-/* Start-up steps from the stored a0, j0: dt_j = largest power of 0.5 <= min(eta_s |a0| / |j0|, dt_max). */
+/* Start-up steps from the stored a0, j0: dt_j = largest power of 0.5 <= min(eta_s |a0| / |j0|, dt_max),
+ * clipped below at dt_max 2^-40; |a0| = |j0| = 0 gives dt_max (reading R32). */
 int nb_init_steps(nb_ctx *ctx, double eta_s, double dt_max);
 
 /* Active selection for the next block ("active particles ... are integrated together"; P:89
@@ -182,11 +183,32 @@ int nb_next_block(nb_ctx *ctx, double *t_next, int32_t *n_act, int32_t *idx_act)
  *     v1 = v0 + a0 h + j0 h^2/2 + a2 h^3/6 + a3 h^4/24
  *     dt_req = sqrt( eta (|a1| |a2'| + |j1|^2) / (|j1| |a3| + |a2'|^2) ),  a2' = a2 + h a3
  *     new step: 2 dt if dt_req >= 2 dt, 2 dt <= dt_max and t is a multiple of 2 dt; else dt halved
- *     while it exceeds dt_req.
+ *     while it exceeds dt_req, but never below dt_max 2^-40; dt_req = 0 or NaN keeps the step (reading R32).
  * The stored state of these bodies becomes (x1, v1, a1, j1, t0 = t, new step); the predicted records
  * become stale (nb_regular needs a new nb_predict_all).  FP64.  idx unique, in range, unchecked. */
 int nb_correct(nb_ctx *ctx, double t, int32_t n, const int32_t *idx, const double *acc1,
                const double *jerk1, double eta, double dt_max);
+
+/* One whole block step in ONE call (SURVEY 8(f) NEXT-3 "device-side block loop"; P:47 block steps, P:89 the
+ * cost of selection against small deep blocks, P:45 corrector):
+ *     selection  t_next = min_j (t0_j + dt_j), active = {j : t0_j + dt_j = t_next} ascending (one cooperative
+ *                launch; its {t_next, n} is the only host read-back of the step: the launch plan needs n)
+ *  -> prediction to t_next + regular force of the active block (a2-a7; blocks of <= 128 particles predict
+ *                inside the force kernel)
+ *  -> if h2_all != NULL: the neighbour force on the lists just written, added in place
+ *  -> nb_correct for the block (corrector, Aarseth step, block rule; reading R31: one total force per body).
+ * h2_all: DEVICE [N] squared neighbour radii indexed by BODY, or NULL: no neighbours (the regular pass gives
+ * the total force, no lists are built).  If t_next > t_stop nothing is integrated: *n_act = 0, the state is
+ * untouched (use t_stop = the end of the run; DBL_MAX never stops).  HOST outputs *t_next, *n_act.  The block's
+ * results stay in library-owned DEVICE buffers until the next nb_block_step (nb_get_block copies them out).  The kernels
+ * after the selection are enqueued without a further synchronisation.  Requires nb_set_j and steps. */
+int nb_block_step(nb_ctx *ctx, const double *h2_all, double eta, double dt_max, double t_stop,
+                  double *t_next, int32_t *n_act);
+/* Copy the last block's results into the caller's DEVICE buffers (any may be NULL; n = the *n_act the step
+ * returned): idx_act[n], acc[n][3], jerk[n][3], pot[n] -- the TOTAL force handed to the corrector --, nnb[n],
+ * nblist[n][nb_cap] (NB_ESTATE if the step ran without h2_all), overflow[n].  Enqueued on the stream. */
+int nb_get_block(nb_ctx *ctx, int32_t *idx_act, double *acc, double *jerk, double *pot, int32_t *nnb,
+                 int32_t *nblist, int32_t *overflow);
 
 /* Inspection / checkpoint: the stored FP64 state in the caller's layout: m[N], x0[N][3], v0[N][3],
  * a0[N][3], j0[N][3], t0[N] and (optional, may be NULL) the steps dt[N]. */

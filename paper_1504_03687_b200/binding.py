@@ -60,6 +60,8 @@ def load_library(build: bool = True) -> ctypes.CDLL:
     lib.nb_next_block.argtypes = [_vp, ctypes.POINTER(dbl), ctypes.POINTER(i32), _vp]
     lib.nb_correct.argtypes = [_vp, dbl, i32, _vp, _vp, _vp, dbl, dbl]
     lib.nb_get_state.argtypes = [_vp] + [_vp] * 7
+    lib.nb_block_step.argtypes = [_vp, _vp, dbl, dbl, dbl, ctypes.POINTER(dbl), ctypes.POINTER(i32)]
+    lib.nb_get_block.argtypes = [_vp] + [_vp] * 7
     lib.nb_set_j_offset.argtypes = [_vp, i64]
     lib.nb_regular_shard.argtypes = [_vp, dbl, i32] + [_vp] * 9
     lib.nb_plan_regular.argtypes = [i64, i64, i32, i32] + [ctypes.POINTER(i32)] * 4
@@ -246,6 +248,31 @@ class NbContext:
         _check(self._lib.nb_correct(self._ctx, float(t), n, _dev_ptr(idx, torch.int32, n, "idx"),
                                     _dev_ptr(acc1, f8, 3 * n, "acc1"), _dev_ptr(jerk1, f8, 3 * n, "jerk1"),
                                     float(eta), float(dt_max)), "nb_correct", self._ctx)
+
+    def block_step(self, h2_all, eta: float, dt_max: float, t_stop: float = float("inf")):
+        """nb_block_step -> (t_next, n_act); h2_all: float64 CUDA tensor [N] indexed by body, or None."""
+        import torch
+        t, n = ctypes.c_double(), ctypes.c_int32()
+        h2 = _vp() if h2_all is None else _dev_ptr(h2_all, torch.float64, self.N, "h2_all")
+        t_stop = min(float(t_stop), 1.7976931348623157e308)
+        _check(self._lib.nb_block_step(self._ctx, h2, float(eta), float(dt_max), t_stop, ctypes.byref(t),
+                                       ctypes.byref(n)), "nb_block_step", self._ctx)
+        return t.value, n.value
+
+    def get_block(self, n: int, want_list: bool = False) -> dict:
+        """nb_get_block: the last block's results (n = the n_act block_step returned) as new CUDA tensors."""
+        import torch
+        f8, i4, dev = torch.float64, torch.int32, "cuda"
+        out = dict(idx_act=torch.empty(n, dtype=i4, device=dev), acc=torch.empty((n, 3), dtype=f8, device=dev),
+                   jerk=torch.empty((n, 3), dtype=f8, device=dev), pot=torch.empty(n, dtype=f8, device=dev),
+                   nnb=torch.empty(n, dtype=i4, device=dev), overflow=torch.empty(n, dtype=i4, device=dev))
+        if want_list:
+            out["nblist"] = torch.empty((n, self.cap), dtype=i4, device=dev)
+        if n:
+            ptr = lambda k: _vp(out[k].data_ptr()) if k in out else _vp()
+            _check(self._lib.nb_get_block(self._ctx, *(ptr(k) for k in ("idx_act", "acc", "jerk", "pot", "nnb", "nblist",
+                                                                          "overflow"))), "nb_get_block", self._ctx)
+        return out
 
     def get_state(self, with_steps: bool = True):
         import torch

@@ -78,6 +78,15 @@ struct nb_ctx {
     unsigned long long *sel_key = nullptr;          // min_j (t0 + dt) as an ordered integer key
     int32_t *sel_counts = nullptr;                  // [ceil(N / SEL_CHUNK)]
     double *sel_result = nullptr, *h_sel_result = nullptr;   // {t_next, n_active}: device / pinned host
+    // nb_block_step: one cooperative selection launch (two alternating minimum slots), the block's own buffers
+    unsigned long long *blk_key = nullptr;          // [2]
+    int blk_parity = 0, blk_grid = 0;
+    int32_t *blk_idx = nullptr;                     // [N] active indices of the last block
+    double *blk_out = nullptr;                      // acc[3n] jerk[3n] pot[n]
+    int32_t *blk_nnb = nullptr, *blk_ovf = nullptr, *blk_list = nullptr;
+    int64_t blk_n = 0, blk_list_n = 0, blk_last_n = 0;
+    bool blk_had_list = false;
+    int32_t h2_by_body = 0;                         // the h2 array of the launch in flight is indexed by body
     // planning / introspection
     Variant var[NVARIANT];                  // reading the predicted records
     Variant fvar[NVARIANT];                 // reading the FP64 state (entries FUSED_FIRST.. only)
@@ -237,7 +246,7 @@ int launch_force_range(nb_ctx *c, int vi, bool fused, int32_t n_i, const int32_t
     p.rec = c->rec;
     p.soa = c->soa; p.Ns = c->Ns; p.t = c->pred_t;
     p.g2 = (float)(c->local_g * c->local_g); p.stats = c->stats;
-    p.idx_i = idx_i; p.h2_i = h2_i; p.perm = perm;
+    p.idx_i = idx_i; p.h2_i = h2_i; p.perm = perm; p.h2_by_body = c->h2_by_body;
     p.n_i = n_i; p.n_i_pad = (int32_t)(n_ib * v.iblock);
     p.irec = irec;
     p.tile0 = (int32_t)tile0; p.ntiles = (int32_t)tile1; p.split0 = (int32_t)split0;
@@ -510,6 +519,8 @@ int nb_close(nb_ctx *c) {
     cudaStreamSynchronize(c->stream);
     cudaFree(c->soa); cudaFree(c->aos); cudaFree(c->rec); cudaFree(c->cnt); cudaFree(c->stats);
     cudaFree(c->sort_keys); cudaFree(c->sort_vals); cudaFree(c->sort_box);
+    cudaFree(c->blk_key); cudaFree(c->blk_idx); cudaFree(c->blk_out); cudaFree(c->blk_nnb); cudaFree(c->blk_ovf);
+    cudaFree(c->blk_list);
     cudaFree(c->partial); cudaFree(c->stage_j);
     cudaFree(c->st_idx); cudaFree(c->st_nnb); cudaFree(c->st_ovf); cudaFree(c->st_list);
     cudaFree(c->st_h2); cudaFree(c->st_out);
@@ -604,8 +615,8 @@ int nb_irregular(nb_ctx *c, double t, int32_t n_i, const int32_t *idx_i, const i
     if (!idx_i || !nnb || !nblist || !acc || !jerk) return NB_EINVAL;
     rc = ensure_aos(c);
     if (rc != NB_OK) return rc;
-    irregular_kernel<<<(unsigned)((n_i + 7) / 8), 256, 0, c->stream>>>(n_i, c->cap, t, idx_i, nnb, nblist, c->aos, acc,
-                                                                       jerk, pot);
+    irregular_kernel<false><<<(unsigned)((n_i + 7) / 8), 256, 0, c->stream>>>(n_i, c->cap, t, idx_i, nnb, nblist, c->aos,
+                                                                              acc, jerk, pot);
     NB_CUDA(c, cudaGetLastError());
     c->launches += 1;
     return NB_OK;
@@ -902,6 +913,109 @@ int nb_correct(nb_ctx *c, double t, int32_t n, const int32_t *idx, const double 
     NB_CUDA(c, cudaGetLastError());
     c->launches += 1;
     c->have_pred = false; c->pred_pending = false;
+    return NB_OK;
+}
+
+int nb_block_step(nb_ctx *c, const double *h2_all, double eta, double dt_max, double t_stop, double *t_next,
+                  int32_t *n_act) {
+    int rc = check_live(c);
+    if (rc != NB_OK) return rc;
+    if (!t_next || !n_act || !(eta > 0.0) || !(dt_max > 0.0)) return NB_EINVAL;
+    if (!c->have_j || !c->have_steps) return NB_ESTATE;
+    const int64_t N = c->N;
+    const int nchunk = (int)((N + SEL_CHUNK - 1) / SEL_CHUNK);
+    if (!c->blk_key) {
+        NB_CUDA(c, cudaMalloc(&c->blk_key, 2 * sizeof(unsigned long long)));
+        NB_CUDA(c, cudaMemsetAsync(c->blk_key, 0xff, 2 * sizeof(unsigned long long), c->stream));
+        NB_CUDA(c, cudaMalloc(&c->blk_idx, sizeof(int32_t) * N));
+        if (!c->sel_counts) NB_CUDA(c, cudaMalloc(&c->sel_counts, sizeof(int32_t) * nchunk));
+        if (!c->sel_result) NB_CUDA(c, cudaMalloc(&c->sel_result, sizeof(double) * 2));
+        if (!c->h_sel_result) NB_CUDA(c, cudaMallocHost(&c->h_sel_result, sizeof(double) * 2));
+        int per_sm = 0;
+        NB_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, select_block_kernel, 256, 0));
+        c->blk_grid = std::max(1, std::min(nchunk, per_sm * c->sm_count));
+    }
+    // ---- selection: ONE cooperative launch, then the only host read-back of the step (the grid sizes need n)
+    {
+        const double *t0 = c->soa + 13 * c->Ns;
+        const double *dtj = c->dtj;
+        unsigned long long *key = c->blk_key + c->blk_parity, *key_next = c->blk_key + (1 - c->blk_parity);
+        int64_t Nn = N;
+        void *args[] = {&Nn, &t0, &dtj, &key, &key_next, &c->sel_counts, &c->blk_idx, &c->sel_result};
+        NB_CUDA(c, cudaLaunchCooperativeKernel((const void *)select_block_kernel, dim3(c->blk_grid), dim3(256), args, 0,
+                                               c->stream));
+        c->blk_parity ^= 1;
+        c->launches += 1;
+        NB_CUDA(c, cudaMemcpyAsync(c->h_sel_result, c->sel_result, sizeof(double) * 2, cudaMemcpyDeviceToHost, c->stream));
+        NB_CUDA(c, cudaStreamSynchronize(c->stream));
+    }
+    const double t = c->h_sel_result[0];
+    const int32_t n = (int32_t)c->h_sel_result[1];
+    *t_next = t;
+    *n_act = 0;
+    c->blk_last_n = 0;
+    if (t > t_stop || n <= 0) return NB_OK;          // nothing is due before t_stop: the state is untouched
+    if (n > c->blk_n) {
+        cudaFree(c->blk_out); cudaFree(c->blk_nnb); cudaFree(c->blk_ovf);
+        c->blk_out = nullptr; c->blk_nnb = c->blk_ovf = nullptr; c->blk_n = 0;
+        const int64_t m = std::min<int64_t>(N, std::max<int64_t>(n, 1024) * 5 / 4);
+        NB_CUDA(c, cudaMalloc(&c->blk_out, sizeof(double) * 7 * m));
+        NB_CUDA(c, cudaMalloc(&c->blk_nnb, sizeof(int32_t) * m));
+        NB_CUDA(c, cudaMalloc(&c->blk_ovf, sizeof(int32_t) * m));
+        c->blk_n = m;
+    }
+    if (h2_all && (int64_t)n * c->cap > c->blk_list_n) {
+        cudaFree(c->blk_list); c->blk_list = nullptr; c->blk_list_n = 0;
+        const int64_t m = std::min<int64_t>(N, std::max<int64_t>(n, 1024) * 5 / 4) * c->cap;
+        NB_CUDA(c, cudaMalloc(&c->blk_list, sizeof(int32_t) * m));
+        c->blk_list_n = m;
+    }
+    double *acc = c->blk_out, *jerk = c->blk_out + 3 * (int64_t)n, *pot = c->blk_out + 6 * (int64_t)n;
+    // ---- a2-a7 for the block: prediction (inside the force kernel for small blocks) + regular force
+    c->have_pred = true; c->pred_pending = true; c->pred_t = t;
+    if (!c->fuse) {
+        rc = materialize_pred(c);
+        if (rc != NB_OK) return rc;
+    }
+    c->h2_by_body = 1;
+    rc = regular_device(c, n, c->blk_idx, h2_all, acc, jerk, pot, c->blk_nnb, h2_all ? c->blk_list : nullptr, c->blk_ovf);
+    c->h2_by_body = 0;
+    if (rc != NB_OK) return rc;
+    rc = ensure_aos(c);
+    if (rc != NB_OK) return rc;
+    if (h2_all) {       // the neighbour force on the lists just written, added in place (regular + irregular)
+        irregular_kernel<true><<<(unsigned)((n + 7) / 8), 256, 0, c->stream>>>(n, c->cap, t, c->blk_idx, c->blk_nnb,
+                                                                                c->blk_list, c->aos, acc, jerk, pot);
+        c->launches += 1;
+    }
+    correct_kernel<<<(unsigned)((n + 127) / 128), 128, 0, c->stream>>>(n, c->Ns, t, eta, dt_max, c->blk_idx, acc, jerk,
+                                                                       c->soa, c->aos, c->dtj);
+    NB_CUDA(c, cudaGetLastError());
+    c->launches += 1;
+    c->have_pred = false; c->pred_pending = false;
+    c->blk_last_n = n;
+    c->blk_had_list = h2_all != nullptr;
+    *n_act = n;
+    return NB_OK;
+}
+
+int nb_get_block(nb_ctx *c, int32_t *idx_act, double *acc, double *jerk, double *pot, int32_t *nnb, int32_t *nblist,
+                 int32_t *overflow) {
+    int rc = check_live(c);
+    if (rc != NB_OK) return rc;
+    const int64_t n = c->blk_last_n;
+    if (n == 0) return NB_OK;
+    const cudaMemcpyKind dd = cudaMemcpyDeviceToDevice;
+    if (idx_act) NB_CUDA(c, cudaMemcpyAsync(idx_act, c->blk_idx, sizeof(int32_t) * n, dd, c->stream));
+    if (acc) NB_CUDA(c, cudaMemcpyAsync(acc, c->blk_out, sizeof(double) * 3 * n, dd, c->stream));
+    if (jerk) NB_CUDA(c, cudaMemcpyAsync(jerk, c->blk_out + 3 * n, sizeof(double) * 3 * n, dd, c->stream));
+    if (pot) NB_CUDA(c, cudaMemcpyAsync(pot, c->blk_out + 6 * n, sizeof(double) * n, dd, c->stream));
+    if (nnb) NB_CUDA(c, cudaMemcpyAsync(nnb, c->blk_nnb, sizeof(int32_t) * n, dd, c->stream));
+    if (overflow) NB_CUDA(c, cudaMemcpyAsync(overflow, c->blk_ovf, sizeof(int32_t) * n, dd, c->stream));
+    if (nblist) {
+        if (!c->blk_had_list) return NB_ESTATE;       // the step ran without h2_all: no lists were built
+        NB_CUDA(c, cudaMemcpyAsync(nblist, c->blk_list, sizeof(int32_t) * n * c->cap, dd, c->stream));
+    }
     return NB_OK;
 }
 

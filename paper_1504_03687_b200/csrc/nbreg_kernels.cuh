@@ -17,6 +17,7 @@
 // close together (relative to their neighbour radii) differences in its OWN frame instead: one add per
 // component (see force_kernel).  Small blocks read the FP64 state directly and predict in the kernel.
 #pragma once
+#include <cooperative_groups.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -434,7 +435,8 @@ struct ForceParams {
     int64_t Ns;
     double t;                     // SRC_STATE: time to predict to
     const int32_t *idx_i;         // [n_i], or NULL: the block is 0..n_i-1
-    const double *h2_i;           // [n_i]
+    const double *h2_i;           // [n_i]; or [N] indexed by body when h2_by_body; or NULL: every h2 = 0
+    int32_t h2_by_body;
     const int32_t *perm;          // NULL, or slot -> k of a block the library put in Morton order (lanes hold slots)
     int32_t n_i;
     int32_t n_i_pad;              // n_i rounded up to the CTA's i-block
@@ -717,7 +719,8 @@ __global__ void __launch_bounds__(32 * WI *WJ, MINB) force_kernel(const ForcePar
             if (valid[h] && (WJ == 1 || wj == 0)) {
                 const int32_t idx = p.idx_i ? p.idx_i[k] : k;      // NULL = identity block (full-N pass)
                 my_idx[h] = idx;
-                ph2[h] = fmaxf(__double2float_rn(p.h2_i[k]), TINY_H2);
+                // h2_i NULL: no neighbours (total force); h2_by_body: the array is indexed by body, not by k
+                ph2[h] = p.h2_i ? fmaxf(__double2float_rn(p.h2_i[p.h2_by_body ? idx : k]), TINY_H2) : TINY_H2;
                 if constexpr (SRC == SRC_STATE) {                  // the predictor's own arithmetic on body idx
                     const double *s0 = p.soa + idx;
                     const double dt = p.t - s0[(size_t)13 * p.Ns];
@@ -1102,6 +1105,8 @@ __device__ __forceinline__ BodyD predict_body(const double *__restrict__ aos, in
     return b;
 }
 
+// ACCUM: add to acc / jerk / pot instead of overwriting them (nb_block_step: regular + irregular = total).
+template <bool ACCUM>
 __global__ void __launch_bounds__(256) irregular_kernel(int32_t n_i, int32_t cap, double t,
                                                         const int32_t *__restrict__ idx_i,
                                                         const int32_t *__restrict__ nnb,
@@ -1142,9 +1147,15 @@ __global__ void __launch_bounds__(256) irregular_kernel(int32_t n_i, int32_t cap
 #pragma unroll
         for (int q = 0; q < 7; ++q) s[q] += __shfl_xor_sync(0xffffffffu, s[q], off);
     if (lane == 0) {
-        acc[3 * k + 0] = s[0]; acc[3 * k + 1] = s[1]; acc[3 * k + 2] = s[2];
-        jerk[3 * k + 0] = s[3]; jerk[3 * k + 1] = s[4]; jerk[3 * k + 2] = s[5];
-        if (pot) pot[k] = s[6];
+        if (ACCUM) {
+#pragma unroll
+            for (int q = 0; q < 3; ++q) { acc[3 * k + q] += s[q]; jerk[3 * k + q] += s[3 + q]; }
+            if (pot) pot[k] += s[6];
+        } else {
+            acc[3 * k + 0] = s[0]; acc[3 * k + 1] = s[1]; acc[3 * k + 2] = s[2];
+            jerk[3 * k + 0] = s[3]; jerk[3 * k + 1] = s[4]; jerk[3 * k + 2] = s[5];
+            if (pot) pot[k] = s[6];
+        }
     }
 }
 
@@ -1241,6 +1252,102 @@ __global__ void __launch_bounds__(256) select_active_kernel(int64_t N, const dou
     }
 }
 
+// The same selection as ONE cooperative launch (nb_block_step): grid-stride over the 2048-body chunks,
+// grid.sync() between the three phases; `key` is this call's minimum slot (~0 on entry), `key_next` the
+// other slot, reset here for the next call.  result = {t_next, n_active}.
+__global__ void __launch_bounds__(256) select_block_kernel(int64_t N, const double *__restrict__ t0,
+                                                           const double *__restrict__ dtj, unsigned long long *key,
+                                                           unsigned long long *key_next, int32_t *__restrict__ counts,
+                                                           int32_t *__restrict__ idx_act, double *__restrict__ result) {
+    namespace cg = cooperative_groups;
+    cg::grid_group grid = cg::this_grid();
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const int nchunk = (int)((N + SEL_CHUNK - 1) / SEL_CHUNK);
+    __shared__ unsigned long long wbest[8];
+    __shared__ int32_t wsum[8];
+    __shared__ int32_t base_s;
+    // ---- phase 1: t_next = min_j (t0_j + dt_j)
+    unsigned long long best = ~0ull;
+    for (int b = blockIdx.x; b < nchunk; b += gridDim.x)
+        for (int s = 0; s < SEL_CHUNK; s += 256) {
+            const int64_t j = (int64_t)b * SEL_CHUNK + s + threadIdx.x;
+            if (j < N) best = min(best, ordered_key(t0[j] + dtj[j]));
+        }
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) best = min(best, __shfl_xor_sync(0xffffffffu, best, off));
+    if (lane == 0) wbest[w] = best;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int q = 1; q < 8; ++q) best = min(best, wbest[q]);
+        atomicMin(key, best);
+        if (blockIdx.x == 0) *key_next = ~0ull;
+    }
+    grid.sync();
+    const double tn = key_to_double(*key);
+    // ---- phase 2: active bodies per chunk
+    for (int b = blockIdx.x; b < nchunk; b += gridDim.x) {
+        int32_t cntc = 0;
+        for (int s = 0; s < SEL_CHUNK; s += 256) {
+            const int64_t j = (int64_t)b * SEL_CHUNK + s + threadIdx.x;
+            cntc += (j < N && (t0[j] + dtj[j] == tn)) ? 1 : 0;
+        }
+#pragma unroll
+        for (int off = 16; off > 0; off >>= 1) cntc += __shfl_xor_sync(0xffffffffu, cntc, off);
+        __syncthreads();
+        if (lane == 0) wsum[w] = cntc;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            int32_t tsum = 0;
+#pragma unroll
+            for (int q = 0; q < 8; ++q) tsum += wsum[q];
+            counts[b] = tsum;
+        }
+    }
+    grid.sync();
+    // ---- phase 3: ordered compaction (ascending indices)
+    for (int b = blockIdx.x; b < nchunk; b += gridDim.x) {
+        int32_t part = 0;
+        for (int q = threadIdx.x; q < b; q += 256) part += counts[q];
+#pragma unroll
+        for (int off = 16; off > 0; off >>= 1) part += __shfl_xor_sync(0xffffffffu, part, off);
+        __syncthreads();
+        if (lane == 0) wsum[w] = part;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            int32_t tsum = 0;
+#pragma unroll
+            for (int q = 0; q < 8; ++q) tsum += wsum[q];
+            base_s = tsum;
+        }
+        __syncthreads();
+        int32_t running = base_s;
+        for (int s = 0; s < SEL_CHUNK; s += 256) {
+            const int64_t j = (int64_t)b * SEL_CHUNK + s + threadIdx.x;
+            const bool act = j < N && (t0[j] + dtj[j] == tn);
+            const unsigned bal = __ballot_sync(0xffffffffu, act);
+            __syncthreads();
+            if (lane == 0) wsum[w] = __popc(bal);
+            __syncthreads();
+            int32_t before = 0, slab = 0;
+#pragma unroll
+            for (int q = 0; q < 8; ++q) {
+                const int32_t cq = wsum[q];
+                before += q < w ? cq : 0;
+                slab += cq;
+            }
+            if (act) idx_act[running + before + __popc(bal & ((1u << lane) - 1u))] = (int32_t)j;
+            running += slab;
+        }
+        if (b == nchunk - 1 && threadIdx.x == 0) {
+            result[0] = tn;
+            result[1] = (double)running;
+        }
+        __syncthreads();
+    }
+}
+
+constexpr double DT_MIN_FACTOR = 1.0 / 1099511627776.0;     // 2^-40: no step below dt_max 2^-40 (reading R32)
 // Largest power of two not above x (x > 0, normal): clear the mantissa.
 __device__ __forceinline__ double pow2_floor(double x) {
     return __longlong_as_double(__double_as_longlong(x) & 0x7ff0000000000000ll);
@@ -1255,7 +1362,9 @@ __global__ void __launch_bounds__(256) init_steps_kernel(int64_t N, int64_t Ns, 
     double a[3], jk[3];
 #pragma unroll
     for (int c = 0; c < 3; ++c) { a[c] = soa[(7 + c) * Ns + j]; jk[c] = soa[(10 + c) * Ns + j]; }
-    dtj[j] = pow2_floor(fmin(eta_s * norm3(a) / norm3(jk), dt_max));
+    double req = eta_s * norm3(a) / norm3(jk);
+    if (req != req) req = dt_max;                                   // |a| = |j| = 0: nothing known (reading R32)
+    dtj[j] = pow2_floor(fmin(fmax(req, dt_max * DT_MIN_FACTOR), dt_max));
 }
 
 // Fourth-order Hermite corrector + new block step for the n active bodies (Makino & Aarseth 1992):
@@ -1294,10 +1403,12 @@ __global__ void __launch_bounds__(128) correct_kernel(int32_t n, int64_t Ns, dou
     const double na = norm3(a1), nj = norm3(j1), n2 = norm3(a2e), n3 = norm3(a3);
     const double req = sqrt(eta * (na * n2 + nj * nj) / (nj * n3 + n2 * n2));
     double d = h;
-    const double d2 = 2.0 * d, ratio = t1 / d2;
-    if (req >= d2 && d2 <= dt_max && ratio == floor(ratio)) d = d2;
-    else
-        while (d > req) d *= 0.5;
+    if (req > 0.0) {        // req = 0 or NaN carries no information: the step is kept (reading R32)
+        const double d2 = 2.0 * d, ratio = t1 / d2, dmin = dt_max * DT_MIN_FACTOR;
+        if (req >= d2 && d2 <= dt_max && ratio == floor(ratio)) d = d2;
+        else
+            while (d > req && d > dmin) d *= 0.5;
+    }
     store_body(i, Ns, m, x1, v1, a1, j1, t1, soa, aos);
     dtj[i] = d;
 }

@@ -222,3 +222,157 @@ def test_ac_split_block_loop_at_65536_bodies_follows_the_oracle():
     print("AC-split loop: block sizes", sizes, "step decisions that differ", int(flips))
     assert flips <= 1e-3 * sum(sizes)      # FP32 pair terms move dt_req by ~1e-7: a flip needs dt_req that close to 2^-k
     ctx.close()
+
+
+# ----------------------------------------------------------------------------- nb_block_step (one call per block)
+
+def _oracle_block(st, m, eta, dt_max, h2_np=None, cap=None):
+    """One block step of the oracle on the state dict st (in place): selection, predictor, total force
+    (regular with h2 = 0, or regular + irregular on the oracle's own lists), corrector, new step."""
+    import oracle
+    t, act = H.next_block(st["t0"], st["dt"])
+    xp, vp = oracle.predict(st["x0"], st["v0"], st["a0"], st["j0"], st["t0"], t)
+    if h2_np is None:
+        r = oracle.regular(m, xp, vp, act, np.zeros(act.size), 8, want_list=False)
+        a1, j1, nnb = r["acc"], r["jerk"], None
+    else:
+        r = oracle.regular(m, xp, vp, act, h2_np[act], cap)
+        i = oracle.irregular(m, st["x0"], st["v0"], st["a0"], st["j0"], st["t0"], t, act, r["nnb"], r["nblist"], cap)
+        a1, j1, nnb = r["acc"] + i["acc"], r["jerk"] + i["jerk"], r["nnb"]
+    x1, v1, a2, a3 = H.correct(st["x0"][act], st["v0"][act], st["a0"][act], st["j0"][act], st["dt"][act], a1, j1)
+    new = H.quantize_step(H.aarseth_step(a1, j1, a2, a3, st["dt"][act], eta), st["dt"][act], t, dt_max)
+    st["x0"][act], st["v0"][act], st["a0"][act], st["j0"][act] = x1, v1, a1, j1
+    st["t0"][act], st["dt"][act] = t, new
+    return t, act, nnb
+
+
+def test_block_step_200_blocks_at_65536_in_lockstep_with_the_oracle():
+    """nb_block_step (selection -> fused prediction + regular force -> corrector, one call
+    and one host read-back per block) for 200 consecutive blocks of a 65536-body cluster with power-law block
+    occupancy (deep levels hold few bodies), against the oracle doing the same 200 blocks.  Active sets
+    must be identical block by block; a step decision may flip where dt_req sits within FP32 force rounding
+    of a power of two -- flips are counted and adopted so that the two runs stay comparable."""
+    import paper_1504_03687_b200 as nb
+    cfg = nbgen.make_config(3, N=65536)
+    N = cfg["N"]
+    dt = 2.0 ** -cfg["levels"].astype(np.float64)
+    st = dict(x0=cfg["x0"].copy(), v0=cfg["v0"].copy(), a0=cfg["a0"].copy(), j0=cfg["j0"].copy(),
+              t0=np.floor(0.3 / dt) * dt, dt=dt.copy())
+    m = cfg["m"]
+    eta, dt_max = 0.02, 2.0**-6
+    ctx = nb.nb_open(N, 8)
+    nb.nb_set_j(ctx, *(_dev(a) for a in (m, st["x0"], st["v0"], st["a0"], st["j0"], st["t0"])))
+    ctx.set_steps(_dev(st["dt"]))
+    sizes, flips, fused = [], 0, 0
+    for b in range(200):
+        t, n = ctx.block_step(None, eta, dt_max)
+        fused += ctx.info("last_fused")
+        t_ref, act, _ = _oracle_block(st, m, eta, dt_max)
+        blk = ctx.get_block(n)
+        assert t == t_ref and n == act.size, (b, t, t_ref, n, act.size)
+        assert np.array_equal(blk["idx_act"].cpu().numpy(), act), b
+        sizes.append(n)
+        # adopt flipped step decisions so the runs stay in lockstep.  (a2 ~ (a0 - a1) / dt^2 amplifies the FP32
+        # rounding of the force at tiny steps: dt_req moves by ~1e-3 relative, so a body whose dt_req sits that
+        # close to a power of two may decide differently)
+        g_dt = _state(ctx)["dt"]
+        diff = np.flatnonzero(g_dt != st["dt"])
+        assert np.isin(diff, act).all()
+        flips += diff.size
+        st["dt"][diff] = g_dt[diff]
+    got = _state(ctx)
+    print("block_step x200: sizes min/median/max", min(sizes), int(np.median(sizes)), max(sizes), "particle steps",
+          sum(sizes), "flips", flips, "fused blocks", fused)
+    assert min(sizes) < 128 and fused > 50                       # small deep blocks took the fused path
+    assert flips <= max(2, int(1e-3 * sum(sizes)))
+    assert np.array_equal(got["t0"], st["t0"])
+    # the corrector turns a force error da into dx ~ 0.35 da dt^2 and dv ~ 1.5 da dt per step; the FP32 pair
+    # arithmetic gives da <~ 1e-6 |a|, and the Kroupa cluster has bodies with |a| ~ 1e3 next to a heavy neighbour
+    # on steps up to 2^-8: dx <~ 5e-9, dv <~ 6e-6 in the worst case
+    ex, ev = np.abs(got["x0"] - st["x0"]).max(), np.abs(got["v0"] - st["v0"]).max()
+    print("block_step x200: max |dx|", ex, "max |dv|", ev, "max |a|", np.abs(st["a0"]).max())
+    assert ex < 5e-9 and ev < 6e-6
+    scale = np.linalg.norm(st["a0"], axis=1)
+    assert np.max(np.linalg.norm(got["a0"] - st["a0"], axis=1) / scale) <= 1e-5
+    ctx.close()
+
+
+def test_block_step_with_neighbour_radii_adds_the_irregular_force():
+    """nb_block_step with h2_all: regular force with lists + neighbour force on those lists, added in place
+    (P:49), then the corrector -- five blocks against the oracle's regular + irregular + corrector; the
+    block's own buffers (nb_get_block) carry the total force and the neighbour counts."""
+    import paper_1504_03687_b200 as nb
+    cfg = nbgen.make_config(2, N=20000, n_i=16)
+    N, cap = cfg["N"], cfg["cap"]
+    dt = 2.0 ** -cfg["levels"].astype(np.float64)
+    st = dict(x0=cfg["x0"].copy(), v0=cfg["v0"].copy(), a0=cfg["a0"].copy(), j0=cfg["j0"].copy(),
+              t0=np.floor(0.3 / dt) * dt, dt=dt.copy())
+    m = cfg["m"]
+    h2_np = np.minimum(cfg["h2_all"], 0.01)
+    eta, dt_max = 0.02, 2.0**-6
+    ctx = nb.nb_open(N, cap)
+    nb.nb_set_j(ctx, *(_dev(a) for a in (m, st["x0"], st["v0"], st["a0"], st["j0"], st["t0"])))
+    ctx.set_steps(_dev(st["dt"]))
+    h2_d = _dev(h2_np)
+    for b in range(5):
+        t, n = ctx.block_step(h2_d, eta, dt_max)
+        before = {k: st[k].copy() for k in ("a0", "j0")}
+        t_ref, act, nnb = _oracle_block(st, m, eta, dt_max, h2_np, cap)
+        blk = ctx.get_block(n, want_list=True)
+        assert t == t_ref and np.array_equal(blk["idx_act"].cpu().numpy(), act)
+        assert np.array_equal(blk["nnb"].cpu().numpy(), nnb) and nnb.max() <= cap and nnb.max() > 0
+        a1 = st["a0"][act]
+        assert np.abs(blk["acc"].cpu().numpy() - a1).max() <= 1e-5 * np.abs(a1).max()
+    got = _state(ctx)
+    assert np.array_equal(got["t0"], st["t0"])
+    assert np.abs(got["x0"] - st["x0"]).max() < 1e-11 and np.abs(got["v0"] - st["v0"]).max() < 1e-9
+    assert (got["dt"] != st["dt"]).sum() <= 2
+    ctx.close()
+
+
+def test_block_step_stops_at_t_stop_and_closed_loop_conserves_energy():
+    """The closed loop of test_block_loop_... driven by nb_block_step alone: N = 1024 Plummer sphere to
+    t = 1/8; t_stop leaves the state untouched once nothing is due; energy conserved; same particle steps
+    as the oracle integration."""
+    import paper_1504_03687_b200 as nb
+    N = 1024
+    cfg = nbgen.make_config(1, N=N)
+    m, x, v = cfg["m"], cfg["x0"], cfg["v0"]
+    eta, eta_s, dt_max, t_end = 0.01, 0.01, 2.0**-4, 0.125
+    ref = H.integrate(m, x, v, t_end, eta, eta_s, dt_max, _oracle_force)
+    ctx = nb.nb_open(N, 8)
+    kw = dict(dtype=torch.float64, device="cuda")
+    z3, z1 = torch.zeros((N, 3), **kw), torch.zeros(N, **kw)
+    all_idx = torch.arange(N, dtype=torch.int32, device="cuda")
+
+    def energy(t):
+        ctx.predict_all(t)
+        out = ctx.regular_alloc(all_idx, z1)
+        ctx.synchronize()
+        s_ = _state(ctx, with_steps=False)
+        return 0.5 * (s_["m"] * (s_["v0"] ** 2).sum(1)).sum() + 0.5 * (s_["m"] * out["pot"].cpu().numpy()).sum(), out
+
+    nb.nb_set_j(ctx, _dev(m), _dev(x), _dev(v), z3, z3, z1)
+    e0, out = energy(0.0)
+    nb.nb_set_j(ctx, _dev(m), _dev(x), _dev(v), out["acc"].clone(), out["jerk"].clone(), z1)
+    ctx.init_steps(eta_s, dt_max)
+    blocks = psteps = 0
+    while True:
+        t, n = ctx.block_step(None, eta, dt_max, t_stop=t_end)
+        if n == 0:
+            assert t > t_end
+            break
+        blocks += 1
+        psteps += n
+    s1 = _state(ctx)
+    t2, n2 = ctx.block_step(None, eta, dt_max, t_stop=t_end)            # again: still nothing due, state untouched
+    s2 = _state(ctx)
+    assert n2 == 0 and t2 == t and all(np.array_equal(s1[k], s2[k]) for k in s1)
+    assert np.all(s1["t0"] == t_end)
+    e1, _ = energy(t_end)
+    print("block_step loop: blocks", blocks, "particle steps", psteps, "oracle", ref["blocks"], ref["particle_steps"],
+          "dE/E", (e1 - e0) / e0)
+    assert abs((e1 - e0) / e0) < 5e-6
+    assert abs(psteps - ref["particle_steps"]) <= 0.01 * ref["particle_steps"]
+    assert np.abs(s1["x0"] - ref["x0"]).max() < 1e-5
+    ctx.close()
