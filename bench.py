@@ -45,6 +45,7 @@ def parse():
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--variant", type=int, default=-1, help="force a force-kernel variant (tuning experiments)")
     ap.add_argument("--no-sweep", action="store_true")
+    ap.add_argument("--no-extras", action="store_true", help="skip the NEXT-row timings (nb_block_step, nb_irregular, ...)")
     ap.add_argument("--all-configs", action="store_true",
                     help="also sweep BASELINE.json configs 3 (N=262144) and 5 (King core, overflowing rows); slower start-up")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -417,7 +418,7 @@ def run_b200(args):
 
     # ---- the steps either side of the path, timed alone; not part of `value`
     extras = None
-    if not args.no_sweep and world == 1:
+    if not args.no_extras and world == 1:
         def timed(fn, reps=5):
             best = 1e30
             for _ in range(reps):
@@ -458,23 +459,34 @@ def run_b200(args):
             bctx.block_step(None, 0.02, 2.0 ** -6)
         torch.cuda.synchronize()
         bctx.tune("profile", 1)
-        nblk, sizes, fused_blk = 100, [], 0
-        tw0 = time.perf_counter()
+        nblk, sizes, fused_blk, stamps, last_launch = 150, [], [], [time.perf_counter()], []
         for _ in range(nblk):
             _, nn_b = bctx.block_step(None, 0.02, 2.0 ** -6)
-            sizes.append(nn_b); fused_blk += bctx.info("last_fused")
+            stamps.append(time.perf_counter())
+            sizes.append(nn_b); fused_blk.append(bctx.info("last_fused"))
+            last_launch.append(bctx.info("force_kernel_count") - 1)   # a mis-speculated block launched a no-op first
         torch.cuda.synchronize()
-        wall_us = (time.perf_counter() - tw0) * 1e6
-        force_us = bctx.info("force_kernel_ns") * 1e-3
-        assert bctx.info("force_kernel_count") == nblk
+        assert last_launch[-1] < 256
+        force_us = np.array([bctx.info("force_kernel_ns_at", q) * 1e-3 for q in last_launch])
+        spec = {"hits": bctx.info("spec_hits"), "misses": bctx.info("spec_misses")}
         bctx.tune("profile", 0)
         bctx.close()
-        blockstep = {"blocks": nblk, "n_act_median": float(np.median(sizes)), "n_act_min": int(min(sizes)),
-                     "n_act_max": int(max(sizes)), "fused_blocks": int(fused_blk), "us_per_block": wall_us / nblk,
-                     "us_force_kernel_per_block": force_us / nblk,
-                     "us_per_block_outside_force_kernel": (wall_us - force_us) / nblk,
-                     "note": "wall clock over 100 back-to-back nb_block_step calls (h2 = NULL: total force); the force "
-                             "kernel's own time from CUDA events around each of its launches"}
+        # call k returns after ENQUEUEING block k; its kernels run while call k+1 waits for its selection:
+        # the interval between the returns of calls k and k+1 holds block k's force kernel
+        cycle_us = np.diff(np.array(stamps))[1:] * 1e6              # [k] = return(k+1) - return(k), k = 0 .. nblk-2
+        sizes_a, fused_a = np.array(sizes), np.array(fused_blk)
+        small = (sizes_a[:-1] <= 128) & (sizes_a[1:] <= 128)
+        outside = cycle_us - force_us[:-1]
+        blockstep = {"blocks": nblk, "n_act_median": float(np.median(sizes_a)), "n_act_min": int(sizes_a.min()),
+                     "n_act_max": int(sizes_a.max()), "fused_blocks": int(fused_a.sum()), "speculation": spec,
+                     "small_blocks_measured": int(small.sum()),
+                     "us_per_small_block": float(np.median(cycle_us[small])) if small.any() else None,
+                     "us_force_kernel_per_small_block": float(np.median(force_us[:-1][small])) if small.any() else None,
+                     "us_per_small_block_outside_force_kernel": float(np.median(outside[small])) if small.any() else None,
+                     "us_per_block_outside_force_kernel_all_median": float(np.median(outside)),
+                     "note": "150 back-to-back nb_block_step calls (h2 = NULL: total force) from a mid-run state; cycle = host "
+                             "wall clock between the returns of consecutive calls; force kernel = CUDA events around its "
+                             "launch; small = blocks of <= 128 active bodies (fused prediction)"}
         extras = {
             "nb_block_step": blockstep,
             "nb_irregular": {"n_i": n_i, "neighbour_pairs": nn, "ms": ms_irr, "pairs_per_s": nn / (ms_irr * 1e-3),

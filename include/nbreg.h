@@ -199,7 +199,8 @@ int nb_correct(nb_ctx *ctx, double t, int32_t n, const int32_t *idx, const doubl
  *  -> nb_correct for the block (corrector, Aarseth step, block rule; reading R31: one total force per body).
  * h2_all: DEVICE [N] squared neighbour radii indexed by BODY, or NULL: no neighbours (the regular pass gives
  * the total force, no lists are built).  If t_next > t_stop nothing is integrated: *n_act = 0, the state is
- * untouched (use t_stop = the end of the run; DBL_MAX never stops).  HOST outputs *t_next, *n_act.  The block's
+ * untouched (use t_stop = the end of the run; DBL_MAX never stops).  HOST outputs *t_next, *n_act.  Small
+ * blocks are enqueued speculatively (NB_TUNE_SPECULATE), so the GPU does not wait for the host.  The block's
  * results stay in library-owned DEVICE buffers until the next nb_block_step (nb_get_block copies them out).  The kernels
  * after the selection are enqueued without a further synchronisation.  Requires nb_set_j and steps. */
 int nb_block_step(nb_ctx *ctx, const double *h2_all, double eta, double dt_max, double t_stop,
@@ -260,7 +261,7 @@ enum {
                                         consumer writes the records first.  set 0: nb_predict_all launches
                                         the predictor at once and nb_regular always reads the records      */
     NB_TUNE_LOCAL_G_MILLI = 24,      /* set: 1000 G of the local-frame guard |x_i - c| <= G h_i under which a
-                                        warp differences positions in its own frame (default 4000; 0 = never:
+                                        warp differences positions in its own frame (default 8000; 0 = never:
                                         hi/lo differencing everywhere)                                      */
     NB_TUNE_STATS = 25,              /* set 1: count, from now on, the warps of the force kernel and those
                                         that took the local frame; set 0: off                               */
@@ -271,7 +272,15 @@ enum {
                                         order inside the library before the force kernel, so that the 64
                                         particles of a warp sit close together and take the local frame
                                         (default 4096; 0 = never).  Outputs keep the caller's order.        */
-    NB_INFO_LAST_REORDERED = 30      /* get: 1 if the last block was reordered                              */
+    NB_INFO_LAST_REORDERED = 30,     /* get: 1 if the last block was reordered                              */
+    NB_TUNE_SPECULATE = 31,          /* set 1 (default): nb_block_step enqueues the chain of a SMALL block (size class
+                                        of the previous one: 32 / 64 / 128) before the host has read {t_next, n}: the
+                                        kernels take both from device memory and do nothing if the block is larger,
+                                        in which case the ordinary launches follow.  set 0: always wait for n      */
+    NB_INFO_SPEC_HITS = 32,          /* get: blocks integrated by a speculative chain                               */
+    NB_INFO_SPEC_MISSES = 33,        /* get: speculative chains that turned out to be no-ops                        */
+    NB_INFO_FORCE_KERNEL_NS_AT = 1000 /* get, key = 1000 + q (q < 256): device time in ns of the q-th bracketed
+                                        force-kernel launch since NB_TUNE_PROFILE was set (synchronises)    */
 };
 int nb_get_info(nb_ctx *ctx, int32_t key, int64_t *value);
 int nb_set_tuning(nb_ctx *ctx, int32_t key, int64_t value);

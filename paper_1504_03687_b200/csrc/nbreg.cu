@@ -26,7 +26,7 @@ struct Variant {
 constexpr int NVARIANT = 5;
 constexpr int NAUTO = 5;        // variants the planner picks from; the rest only by NB_TUNE_FORCE_VARIANT
 constexpr int FUSED_FIRST = 2;  // variants 2..4 (128, 64, 32 i per CTA) also exist reading the FP64 state (fused predictor)
-constexpr double DEFAULT_LOCAL_G = 4.0;     // local-frame guard |x_i - c| <= G h_i
+constexpr double DEFAULT_LOCAL_G = 8.0;     // local-frame guard |x_i - c| <= G h_i
 
 }  // namespace
 
@@ -87,6 +87,12 @@ struct nb_ctx {
     int64_t blk_n = 0, blk_list_n = 0, blk_last_n = 0;
     bool blk_had_list = false;
     int32_t h2_by_body = 0;                         // the h2 array of the launch in flight is indexed by body
+    const double *spec_dev = nullptr;               // non-NULL while nb_block_step enqueues a SPECULATIVE chain: the
+    double spec_t_stop = 0.0;                       // kernels take {t, n} from this device address
+    cudaEvent_t ev_sel = nullptr;
+    int64_t blk_stride = 0;                         // acc / jerk / pot of the last block sit at 0, 3, 6 x this in blk_out
+    int64_t spec_hits = 0, spec_misses = 0, blk_prev_n = 0;
+    bool spec_enabled = true;                       // NB_TUNE_SPECULATE
     // planning / introspection
     Variant var[NVARIANT];                  // reading the predicted records
     Variant fvar[NVARIANT];                 // reading the FP64 state (entries FUSED_FIRST.. only)
@@ -136,7 +142,15 @@ void launch_force(const Variant &v, dim3 grid, cudaStream_t st, const ForceParam
 // variants <8,1>, <4,2>, <2,4>, <1,8> and the j-packed <1,8> (32 i per CTA).  The cost factors are
 // measured: time per padded i-slot at n_i = 8256 and 16500, N = 1M, relative to <8,1>.
 constexpr int VAR_IBLOCK[NVARIANT] = {512, 256, 128, 64, 32};
-constexpr double VAR_OVH[NVARIANT] = {0.5, 0.75, 1.5, 3.0, 3.0};
+// Planning model, fitted to launches of n_i = 4096 .. 16384 at N = 1M with 19 .. 148 splits (B200):
+//   time ~ (waves + TAIL) x (tiles per split + per-CTA overhead) + finalize cost per split
+// in units of one tile's compute of the variant.  A CTA's tile takes iblock x 256 pairs at half an SM's rate
+// (two CTAs share it: 3.6e9 pairs/s), its prologue + epilogue about 5 us, and the final reduction reads one
+// more partial row per split (~0.005 us each).  TAIL: the last wave drains with half-empty SMs.
+constexpr double PLAN_TAIL = 0.13, PLAN_CTA_US = 5.0, PLAN_FIN_US_PER_SPLIT = 0.005;
+constexpr double var_tile_us(int v) { return VAR_IBLOCK[v] * 256.0 / 3.6e9 * 1.0e6; }
+constexpr double VAR_OVH[NVARIANT] = {PLAN_CTA_US / var_tile_us(0), PLAN_CTA_US / var_tile_us(1), PLAN_CTA_US / var_tile_us(2),
+                                      PLAN_CTA_US / var_tile_us(3), PLAN_CTA_US / var_tile_us(4)};
 constexpr double VAR_COST[NVARIANT] = {1.0, 1.01, 1.025, 1.03, 1.11};
 
 // Pick the kernel variant: least padded work weighted by the variant's rate, ties to the larger i-block
@@ -158,7 +172,7 @@ int pick_variant(const nb_ctx *c, int32_t n_i) {
 // Pick the number of j-splits S: minimise waves x (tiles per split + per-CTA overhead); among plans
 // within 0.3 % take the smallest S (less scratch, shorter final reduction).
 int plan_split(const nb_ctx *c, const Variant &v, int64_t n_ib, int64_t ntiles);
-int plan_split_pure(int64_t conc, double ovh_tiles, int64_t n_ib, int64_t ntiles);
+int plan_split_pure(int64_t conc, double ovh_tiles, double tile_us, int64_t n_ib, int64_t ntiles);
 int plan_chunks_pure(int64_t ntiles, int64_t want, int64_t *ctile);
 
 int pick_split(nb_ctx *c, const Variant &v, int64_t n_ib, int64_t ntiles) {
@@ -173,24 +187,22 @@ int pick_split(nb_ctx *c, const Variant &v, int64_t n_ib, int64_t ntiles) {
 }
 
 int plan_split(const nb_ctx *c, const Variant &v, int64_t n_ib, int64_t ntiles) {
-    return plan_split_pure((int64_t)c->sm_count * v.ctas_per_sm, v.ovh_tiles, n_ib, ntiles);
+    return plan_split_pure((int64_t)c->sm_count * v.ctas_per_sm, v.ovh_tiles, v.iblock * 256.0 / 3.6e9 * 1.0e6, n_ib, ntiles);
 }
 
-int plan_split_pure(int64_t conc, double ovh_tiles, int64_t n_ib, int64_t ntiles) {
+int plan_split_pure(int64_t conc, double ovh_tiles, double tile_us, int64_t n_ib, int64_t ntiles) {
     const int64_t smax = std::min<int64_t>(ntiles, 8192);
+    auto cost = [&](int64_t S, int64_t &Seff) {
+        const int64_t tps = (ntiles + S - 1) / S;
+        Seff = (ntiles + tps - 1) / tps;                     // splits that actually get tiles
+        const int64_t waves = (n_ib * Seff + conc - 1) / conc;
+        return ((double)waves + PLAN_TAIL) * ((double)tps + ovh_tiles) + PLAN_FIN_US_PER_SPLIT * (double)Seff / tile_us;
+    };
     double best = 1e300;
-    for (int64_t S = 1; S <= smax; ++S) {
-        const int64_t tps = (ntiles + S - 1) / S;
-        const int64_t Seff = (ntiles + tps - 1) / tps;      // splits that actually get tiles
-        const int64_t waves = (n_ib * Seff + conc - 1) / conc;
-        best = std::min(best, (double)waves * ((double)tps + ovh_tiles));
-    }
-    for (int64_t S = 1; S <= smax; ++S) {
-        const int64_t tps = (ntiles + S - 1) / S;
-        const int64_t Seff = (ntiles + tps - 1) / tps;
-        const int64_t waves = (n_ib * Seff + conc - 1) / conc;
-        if ((double)waves * ((double)tps + ovh_tiles) <= best * 1.003) return (int)Seff;
-    }
+    int64_t Seff = 1;
+    for (int64_t S = 1; S <= smax; ++S) best = std::min(best, cost(S, Seff));
+    for (int64_t S = 1; S <= smax; ++S)
+        if (cost(S, Seff) <= best * 1.015) return (int)Seff;      // within the model's accuracy: fewer splits, less scratch
     return 1;
 }
 
@@ -246,6 +258,7 @@ int launch_force_range(nb_ctx *c, int vi, bool fused, int32_t n_i, const int32_t
     p.rec = c->rec;
     p.soa = c->soa; p.Ns = c->Ns; p.t = c->pred_t;
     p.g2 = (float)(c->local_g * c->local_g); p.stats = c->stats;
+    p.blk_dev = c->spec_dev; p.t_stop = c->spec_t_stop;
     p.idx_i = idx_i; p.h2_i = h2_i; p.perm = perm; p.h2_by_body = c->h2_by_body;
     p.n_i = n_i; p.n_i_pad = (int32_t)(n_ib * v.iblock);
     p.irec = irec;
@@ -324,13 +337,14 @@ int launch_finalize(nb_ctx *c, int32_t n_i, int64_t n_i_pad, int S, const int32_
     cfg.attrs = attr;
     cfg.numAttrs = 1;
     const int32_t n_i_pad32 = (int32_t)n_i_pad, S32 = S, cap32 = c->cap, sortP32 = sortP;
-    const double *partial = c->partial;
+    const double *partial = c->partial, *blk_dev = c->spec_dev;
+    const double t_stop = c->spec_t_stop;
     if (W == 4)
-        NB_CUDA(c, cudaLaunchKernelEx(&cfg, finalize_kernel<4>, n_i, n_i_pad32, S32, cap32, sortP32, perm, partial,
-                                      c->cnt, acc, jerk, pot, nnb, nblist, overflow));
+        NB_CUDA(c, cudaLaunchKernelEx(&cfg, finalize_kernel<4>, n_i, n_i_pad32, S32, cap32, sortP32, perm, blk_dev, t_stop,
+                                      partial, c->cnt, acc, jerk, pot, nnb, nblist, overflow));
     else
-        NB_CUDA(c, cudaLaunchKernelEx(&cfg, finalize_kernel<16>, n_i, n_i_pad32, S32, cap32, sortP32, perm, partial,
-                                      c->cnt, acc, jerk, pot, nnb, nblist, overflow));
+        NB_CUDA(c, cudaLaunchKernelEx(&cfg, finalize_kernel<16>, n_i, n_i_pad32, S32, cap32, sortP32, perm, blk_dev, t_stop,
+                                      partial, c->cnt, acc, jerk, pot, nnb, nblist, overflow));
     NB_CUDA(c, cudaGetLastError());
     c->launches += 1;
     c->last_S = S;
@@ -527,6 +541,7 @@ int nb_close(nb_ctx *c) {
     cudaFree(c->d_ist); cudaFree(c->irec); cudaFreeHost(c->h_ist);
     cudaFree(c->dtj); cudaFree(c->sel_key); cudaFree(c->sel_counts); cudaFree(c->sel_result);
     cudaFreeHost(c->h_sel_result);
+    if (c->ev_sel) cudaEventDestroy(c->ev_sel);
     if (c->ev_enter) cudaEventDestroy(c->ev_enter);
     if (c->ev_i) cudaEventDestroy(c->ev_i);
     for (int q = 0; q < nb_ctx::MAXCHUNK; ++q) {
@@ -615,8 +630,8 @@ int nb_irregular(nb_ctx *c, double t, int32_t n_i, const int32_t *idx_i, const i
     if (!idx_i || !nnb || !nblist || !acc || !jerk) return NB_EINVAL;
     rc = ensure_aos(c);
     if (rc != NB_OK) return rc;
-    irregular_kernel<false><<<(unsigned)((n_i + 7) / 8), 256, 0, c->stream>>>(n_i, c->cap, t, idx_i, nnb, nblist, c->aos,
-                                                                              acc, jerk, pot);
+    irregular_kernel<false><<<(unsigned)((n_i + 7) / 8), 256, 0, c->stream>>>(n_i, c->cap, t, nullptr, 0.0, idx_i, nnb,
+                                                                              nblist, c->aos, acc, jerk, pot);
     NB_CUDA(c, cudaGetLastError());
     c->launches += 1;
     return NB_OK;
@@ -908,8 +923,8 @@ int nb_correct(nb_ctx *c, double t, int32_t n, const int32_t *idx, const double 
     if (!idx || !acc1 || !jerk1) return NB_EINVAL;
     rc = ensure_aos(c);
     if (rc != NB_OK) return rc;
-    correct_kernel<<<(unsigned)((n + 127) / 128), 128, 0, c->stream>>>(n, c->Ns, t, eta, dt_max, idx, acc1, jerk1, c->soa,
-                                                                       c->aos, c->dtj);
+    correct_kernel<<<(unsigned)((n + 127) / 128), 128, 0, c->stream>>>(n, c->Ns, t, eta, dt_max, nullptr, 0.0, idx, acc1,
+                                                                       jerk1, c->soa, c->aos, c->dtj);
     NB_CUDA(c, cudaGetLastError());
     c->launches += 1;
     c->have_pred = false; c->pred_pending = false;
@@ -935,7 +950,34 @@ int nb_block_step(nb_ctx *c, const double *h2_all, double eta, double dt_max, do
         NB_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, select_block_kernel, 256, 0));
         c->blk_grid = std::max(1, std::min(nchunk, per_sm * c->sm_count));
     }
-    // ---- selection: ONE cooperative launch, then the only host read-back of the step (the grid sizes need n)
+    if (!c->ev_sel) NB_CUDA(c, cudaEventCreateWithFlags(&c->ev_sel, cudaEventDisableTiming));
+    // buffers for blocks of up to 1024 bodies exist before anything is enqueued (the speculative chain uses them)
+    auto ensure_block_buffers = [&](int64_t n, bool lists) -> int {
+        if (n > c->blk_n) {
+            NB_CUDA(c, cudaStreamSynchronize(c->stream));
+            cudaFree(c->blk_out); cudaFree(c->blk_nnb); cudaFree(c->blk_ovf);
+            c->blk_out = nullptr; c->blk_nnb = c->blk_ovf = nullptr; c->blk_n = 0;
+            const int64_t m = std::min<int64_t>(std::max<int64_t>(N, 1024), std::max<int64_t>(n, 1024) * 5 / 4);
+            NB_CUDA(c, cudaMalloc(&c->blk_out, sizeof(double) * 7 * m));
+            NB_CUDA(c, cudaMalloc(&c->blk_nnb, sizeof(int32_t) * m));
+            NB_CUDA(c, cudaMalloc(&c->blk_ovf, sizeof(int32_t) * m));
+            c->blk_n = m;
+        }
+        if (lists && n * c->cap > c->blk_list_n) {
+            NB_CUDA(c, cudaStreamSynchronize(c->stream));
+            cudaFree(c->blk_list); c->blk_list = nullptr; c->blk_list_n = 0;
+            const int64_t m = std::min<int64_t>(std::max<int64_t>(N, 1024), std::max<int64_t>(n, 1024) * 5 / 4) * c->cap;
+            NB_CUDA(c, cudaMalloc(&c->blk_list, sizeof(int32_t) * m));
+            c->blk_list_n = m;
+        }
+        return NB_OK;
+    };
+    rc = ensure_block_buffers(128, h2_all != nullptr);
+    if (rc != NB_OK) return rc;
+    rc = ensure_aos(c);
+    if (rc != NB_OK) return rc;
+    // ---- selection: ONE cooperative launch; its {t_next, n} goes to the host (the launch plan of a large
+    //      block needs n) and stays in device memory for the speculative chain below
     {
         const double *t0 = c->soa + 13 * c->Ns;
         const double *dtj = c->dtj;
@@ -947,52 +989,65 @@ int nb_block_step(nb_ctx *c, const double *h2_all, double eta, double dt_max, do
         c->blk_parity ^= 1;
         c->launches += 1;
         NB_CUDA(c, cudaMemcpyAsync(c->h_sel_result, c->sel_result, sizeof(double) * 2, cudaMemcpyDeviceToHost, c->stream));
-        NB_CUDA(c, cudaStreamSynchronize(c->stream));
+        NB_CUDA(c, cudaEventRecord(c->ev_sel, c->stream));
     }
+    // One block's chain a2-a7 + neighbour force + corrector.  spec_cap > 0: SPECULATIVE -- enqueued before the
+    // host knows the block: the kernels read {t, n} from device memory and do nothing unless n <= spec_cap and
+    // t <= t_stop, so the GPU goes from the selection straight into the force kernel while the host is still
+    // waiting for the read-back (deep blocks hold few particles -- the common case).
+    auto enqueue_chain = [&](int32_t n, double t, int32_t spec_cap) -> int {
+        const int64_t stride = spec_cap > 0 ? spec_cap : n;
+        double *acc = c->blk_out, *jerk = c->blk_out + 3 * stride, *pot = c->blk_out + 6 * stride;
+        c->spec_dev = spec_cap > 0 ? c->sel_result : nullptr;
+        c->spec_t_stop = t_stop;
+        c->have_pred = true; c->pred_pending = true; c->pred_t = t;
+        int rc2 = NB_OK;
+        if (!c->fuse) rc2 = materialize_pred(c);
+        c->h2_by_body = 1;
+        if (rc2 == NB_OK)
+            rc2 = regular_device(c, n, c->blk_idx, h2_all, acc, jerk, pot, c->blk_nnb, h2_all ? c->blk_list : nullptr, c->blk_ovf);
+        c->h2_by_body = 0;
+        if (rc2 == NB_OK && h2_all) {   // the neighbour force on the lists just written, added in place
+            irregular_kernel<true><<<(unsigned)((n + 7) / 8), 256, 0, c->stream>>>(n, c->cap, t, c->spec_dev, t_stop, c->blk_idx,
+                                                                                    c->blk_nnb, c->blk_list, c->aos, acc, jerk, pot);
+            c->launches += 1;
+        }
+        if (rc2 == NB_OK) {
+            correct_kernel<<<(unsigned)((n + 127) / 128), 128, 0, c->stream>>>(n, c->Ns, t, eta, dt_max, c->spec_dev, t_stop,
+                                                                               c->blk_idx, acc, jerk, c->soa, c->aos, c->dtj);
+            c->launches += 1;
+            if (cudaGetLastError() != cudaSuccess) rc2 = NB_ECUDA;
+        }
+        c->spec_dev = nullptr;
+        c->have_pred = false; c->pred_pending = false;
+        c->blk_stride = stride;
+        return rc2;
+    };
+    // speculate on the size class of the previous block (32 / 64 / 128: the variants with a fused predictor)
+    int32_t spec_cap = 0;
+    if (c->fuse && c->spec_enabled && c->blk_prev_n > 0 && c->blk_prev_n <= 128)
+        spec_cap = c->blk_prev_n <= 32 ? 32 : c->blk_prev_n <= 64 ? 64 : 128;
+    if (spec_cap > 0) {
+        rc = enqueue_chain(spec_cap, 0.0, spec_cap);
+        if (rc != NB_OK) return rc;
+    }
+    NB_CUDA(c, cudaEventSynchronize(c->ev_sel));
     const double t = c->h_sel_result[0];
     const int32_t n = (int32_t)c->h_sel_result[1];
     *t_next = t;
     *n_act = 0;
     c->blk_last_n = 0;
     if (t > t_stop || n <= 0) return NB_OK;          // nothing is due before t_stop: the state is untouched
-    if (n > c->blk_n) {
-        cudaFree(c->blk_out); cudaFree(c->blk_nnb); cudaFree(c->blk_ovf);
-        c->blk_out = nullptr; c->blk_nnb = c->blk_ovf = nullptr; c->blk_n = 0;
-        const int64_t m = std::min<int64_t>(N, std::max<int64_t>(n, 1024) * 5 / 4);
-        NB_CUDA(c, cudaMalloc(&c->blk_out, sizeof(double) * 7 * m));
-        NB_CUDA(c, cudaMalloc(&c->blk_nnb, sizeof(int32_t) * m));
-        NB_CUDA(c, cudaMalloc(&c->blk_ovf, sizeof(int32_t) * m));
-        c->blk_n = m;
-    }
-    if (h2_all && (int64_t)n * c->cap > c->blk_list_n) {
-        cudaFree(c->blk_list); c->blk_list = nullptr; c->blk_list_n = 0;
-        const int64_t m = std::min<int64_t>(N, std::max<int64_t>(n, 1024) * 5 / 4) * c->cap;
-        NB_CUDA(c, cudaMalloc(&c->blk_list, sizeof(int32_t) * m));
-        c->blk_list_n = m;
-    }
-    double *acc = c->blk_out, *jerk = c->blk_out + 3 * (int64_t)n, *pot = c->blk_out + 6 * (int64_t)n;
-    // ---- a2-a7 for the block: prediction (inside the force kernel for small blocks) + regular force
-    c->have_pred = true; c->pred_pending = true; c->pred_t = t;
-    if (!c->fuse) {
-        rc = materialize_pred(c);
+    c->blk_prev_n = n;
+    if (spec_cap > 0 && n <= spec_cap) {
+        c->spec_hits += 1;                           // the speculative chain is this block
+    } else {
+        if (spec_cap > 0) c->spec_misses += 1;       // those launches were no-ops
+        rc = ensure_block_buffers(n, h2_all != nullptr);
+        if (rc != NB_OK) return rc;
+        rc = enqueue_chain(n, t, 0);
         if (rc != NB_OK) return rc;
     }
-    c->h2_by_body = 1;
-    rc = regular_device(c, n, c->blk_idx, h2_all, acc, jerk, pot, c->blk_nnb, h2_all ? c->blk_list : nullptr, c->blk_ovf);
-    c->h2_by_body = 0;
-    if (rc != NB_OK) return rc;
-    rc = ensure_aos(c);
-    if (rc != NB_OK) return rc;
-    if (h2_all) {       // the neighbour force on the lists just written, added in place (regular + irregular)
-        irregular_kernel<true><<<(unsigned)((n + 7) / 8), 256, 0, c->stream>>>(n, c->cap, t, c->blk_idx, c->blk_nnb,
-                                                                                c->blk_list, c->aos, acc, jerk, pot);
-        c->launches += 1;
-    }
-    correct_kernel<<<(unsigned)((n + 127) / 128), 128, 0, c->stream>>>(n, c->Ns, t, eta, dt_max, c->blk_idx, acc, jerk,
-                                                                       c->soa, c->aos, c->dtj);
-    NB_CUDA(c, cudaGetLastError());
-    c->launches += 1;
-    c->have_pred = false; c->pred_pending = false;
     c->blk_last_n = n;
     c->blk_had_list = h2_all != nullptr;
     *n_act = n;
@@ -1008,8 +1063,8 @@ int nb_get_block(nb_ctx *c, int32_t *idx_act, double *acc, double *jerk, double 
     const cudaMemcpyKind dd = cudaMemcpyDeviceToDevice;
     if (idx_act) NB_CUDA(c, cudaMemcpyAsync(idx_act, c->blk_idx, sizeof(int32_t) * n, dd, c->stream));
     if (acc) NB_CUDA(c, cudaMemcpyAsync(acc, c->blk_out, sizeof(double) * 3 * n, dd, c->stream));
-    if (jerk) NB_CUDA(c, cudaMemcpyAsync(jerk, c->blk_out + 3 * n, sizeof(double) * 3 * n, dd, c->stream));
-    if (pot) NB_CUDA(c, cudaMemcpyAsync(pot, c->blk_out + 6 * n, sizeof(double) * n, dd, c->stream));
+    if (jerk) NB_CUDA(c, cudaMemcpyAsync(jerk, c->blk_out + 3 * c->blk_stride, sizeof(double) * 3 * n, dd, c->stream));
+    if (pot) NB_CUDA(c, cudaMemcpyAsync(pot, c->blk_out + 6 * c->blk_stride, sizeof(double) * n, dd, c->stream));
     if (nnb) NB_CUDA(c, cudaMemcpyAsync(nnb, c->blk_nnb, sizeof(int32_t) * n, dd, c->stream));
     if (overflow) NB_CUDA(c, cudaMemcpyAsync(overflow, c->blk_ovf, sizeof(int32_t) * n, dd, c->stream));
     if (nblist) {
@@ -1109,6 +1164,9 @@ int nb_get_info(nb_ctx *c, int32_t key, int64_t *value) {
         case NB_TUNE_STATS: *value = c->stats ? 1 : 0; break;
         case NB_INFO_LAST_FUSED: *value = c->last_fused; break;
         case NB_INFO_LAST_REORDERED: *value = c->last_reordered; break;
+        case NB_TUNE_SPECULATE: *value = c->spec_enabled ? 1 : 0; break;
+        case NB_INFO_SPEC_HITS: *value = c->spec_hits; break;
+        case NB_INFO_SPEC_MISSES: *value = c->spec_misses; break;
         case NB_TUNE_REORDER_MIN: *value = c->reorder_min; break;
         case NB_INFO_LOCAL_WARPS:
         case NB_INFO_TOTAL_WARPS: {
@@ -1134,7 +1192,18 @@ int nb_get_info(nb_ctx *c, int32_t key, int64_t *value) {
             *value = (int64_t)(ns + 0.5);
             break;
         }
-        default: return NB_EINVAL;
+        default:
+            if (key >= NB_INFO_FORCE_KERNEL_NS_AT && key < NB_INFO_FORCE_KERNEL_NS_AT + nb_ctx::PROF_RING) {
+                const int64_t q = key - NB_INFO_FORCE_KERNEL_NS_AT;       // the q-th bracketed launch
+                if (q >= c->prof_n) return NB_EINVAL;
+                if (c->cuda_err != cudaSuccess) return NB_ECUDA;
+                NB_CUDA(c, cudaStreamSynchronize(c->stream));
+                float ms = 0.f;
+                NB_CUDA(c, cudaEventElapsedTime(&ms, c->ev0[q], c->ev1[q]));
+                *value = (int64_t)((double)ms * 1.0e6 + 0.5);
+                break;
+            }
+            return NB_EINVAL;
     }
     return NB_OK;
 }
@@ -1159,6 +1228,9 @@ int nb_set_tuning(nb_ctx *c, int32_t key, int64_t value) {
         case NB_TUNE_LOCAL_G_MILLI:
             if (value < 0 || value > 1000000) return NB_EINVAL;
             c->local_g = (double)value / 1000.0; break;
+        case NB_TUNE_SPECULATE:
+            if (value != 0 && value != 1) return NB_EINVAL;
+            c->spec_enabled = value != 0; break;
         case NB_TUNE_REORDER_MIN:
             if (value < 0) return NB_EINVAL;
             c->reorder_min = value; break;
@@ -1194,7 +1266,7 @@ int nb_plan_regular(int64_t N, int64_t n_i, int32_t sm_count, int32_t ctas_per_s
     if (!variant || !iblock || !jsplit || !tiles_per_split) return NB_EINVAL;
     const int vi = pick_variant_pure(n_i);
     const int64_t ib = VAR_IBLOCK[vi], n_ib = (n_i + ib - 1) / ib, ntiles = (N + TJ - 1) / TJ;
-    const int S = plan_split_pure((int64_t)sm_count * ctas_per_sm, VAR_OVH[vi], n_ib, ntiles);
+    const int S = plan_split_pure((int64_t)sm_count * ctas_per_sm, VAR_OVH[vi], var_tile_us(vi), n_ib, ntiles);
     *variant = vi; *iblock = (int32_t)ib; *jsplit = S; *tiles_per_split = (int32_t)((ntiles + S - 1) / S);
     return NB_OK;
 }

@@ -454,7 +454,19 @@ struct ForceParams {
     int32_t *nblist;              // caller's [n_i][cap], or NULL: neighbours are only counted
     double *partial;              // [S][7][n_i_pad]
     unsigned int *stats;          // NULL, or {warps in the local frame, warps} (diagnostics; integer atomics)
+    const double *blk_dev;        // NULL, or {t_next, n_active} written by select_block_kernel: a SPECULATIVE launch of
+    double t_stop;                // nb_block_step -- the block's time and size come from device memory; the launch is
+                                  // a no-op if the block is larger than n_i (its capacity) or not due before t_stop
 };
+// The block a speculative launch works on: false = nothing to do.  n and t are overwritten from blk_dev.
+__device__ __forceinline__ bool spec_block(const double *blk_dev, double t_stop, int32_t &n, double &t) {
+    if (!blk_dev) return true;
+    const double tn = blk_dev[0];
+    const int32_t nd = (int32_t)blk_dev[1];
+    if (tn > t_stop || nd > n || nd <= 0) return false;
+    n = nd; t = tn;
+    return true;
+}
 
 // Two active particles (halves .x / .y) held in registers, NEGATED so that every difference is one
 // packed add:  d = j + (-i).  Local frame: nxh.. hold -(x_i - c) and the lo parts are unused.
@@ -663,6 +675,9 @@ __global__ void __launch_bounds__(32 * WI *WJ, MINB) force_kernel(const ForcePar
     const int tid = threadIdx.x;
     const int warp = tid >> 5, lane = tid & 31;
     const int wi = warp % WI, wj = warp / WI;
+    int32_t n_i = p.n_i;
+    double t_pred = p.t;
+    if (!spec_block(p.blk_dev, p.t_stop, n_i, t_pred)) return;    // (uniform over the grid, before any barrier)
 
     const int tile_begin = p.tile0 + blockIdx.y * p.tiles_per_split;
     const int tile_end = min(tile_begin + p.tiles_per_split, p.ntiles);
@@ -706,7 +721,7 @@ __global__ void __launch_bounds__(32 * WI *WJ, MINB) force_kernel(const ForcePar
 #pragma unroll
         for (int h = 0; h < NH; ++h) {
             const int slot = blockIdx.x * IB + wi * (32 * NH) + h * 32 + lane;
-            valid[h] = slot < p.n_i;
+            valid[h] = slot < n_i;
             const int k = (valid[h] && p.perm) ? p.perm[slot] : slot;      // caller's numbering: rows, counters, inputs
             my_k[h] = k;
             my_idx[h] = -1;
@@ -723,7 +738,7 @@ __global__ void __launch_bounds__(32 * WI *WJ, MINB) force_kernel(const ForcePar
                 ph2[h] = p.h2_i ? fmaxf(__double2float_rn(p.h2_i[p.h2_by_body ? idx : k]), TINY_H2) : TINY_H2;
                 if constexpr (SRC == SRC_STATE) {                  // the predictor's own arithmetic on body idx
                     const double *s0 = p.soa + idx;
-                    const double dt = p.t - s0[(size_t)13 * p.Ns];
+                    const double dt = t_pred - s0[(size_t)13 * p.Ns];
                     const double c2 = taylor_c2(dt), c3 = taylor_c3(dt);
 #pragma unroll
                     for (int c = 0; c < 3; ++c) {
@@ -877,7 +892,7 @@ __global__ void __launch_bounds__(32 * WI *WJ, MINB) force_kernel(const ForcePar
 #pragma unroll
             for (int q = lane; q < SUB; q += 32) {
                 double xp[3], vp[3], m;
-                predict_from_tile(st, wj * SUB + q, p.t, xp, vp, m);
+                predict_from_tile(st, wj * SUB + q, t_pred, xp, vp, m);
 #pragma unroll
                 for (int c = 0; c < 3; ++c) {
                     if (local) {
@@ -1007,6 +1022,7 @@ __global__ void __launch_bounds__(32 * WI *WJ, MINB) force_kernel(const ForcePar
 template <int W>
 __global__ void __launch_bounds__(32 * W) finalize_kernel(int32_t n_i, int32_t n_i_pad, int32_t S, int32_t cap,
                                                           int32_t sortP, const int32_t *__restrict__ perm,
+                                                          const double *__restrict__ blk_dev, double t_stop,
                                                           const double *__restrict__ partial,
                                                           int32_t *__restrict__ cnt, double *__restrict__ acc,
                                                           double *__restrict__ jerk, double *__restrict__ pot,
@@ -1021,6 +1037,10 @@ __global__ void __launch_bounds__(32 * W) finalize_kernel(int32_t n_i, int32_t n
     // has drained; everything it reads is valid after this wait (a no-op in an ordinary launch)
     asm volatile("griddepcontrol.wait;" ::: "memory");
     TL_STAMP(4096 + blockIdx.y * gridDim.x + blockIdx.x, 1);
+    {
+        double t_unused = 0.0;
+        if (!spec_block(blk_dev, t_stop, n_i, t_unused)) return;
+    }
     if (blockIdx.y < 7) {
         const int q = blockIdx.y;
         const int slot = blockIdx.x * 32 + lane;       // slot < n_i_pad always (n_i_pad is a multiple of 32)
@@ -1108,6 +1128,7 @@ __device__ __forceinline__ BodyD predict_body(const double *__restrict__ aos, in
 // ACCUM: add to acc / jerk / pot instead of overwriting them (nb_block_step: regular + irregular = total).
 template <bool ACCUM>
 __global__ void __launch_bounds__(256) irregular_kernel(int32_t n_i, int32_t cap, double t,
+                                                        const double *__restrict__ blk_dev, double t_stop,
                                                         const int32_t *__restrict__ idx_i,
                                                         const int32_t *__restrict__ nnb,
                                                         const int32_t *__restrict__ nblist,
@@ -1115,6 +1136,7 @@ __global__ void __launch_bounds__(256) irregular_kernel(int32_t n_i, int32_t cap
                                                         double *__restrict__ jerk, double *__restrict__ pot) {
     const int lane = threadIdx.x & 31;
     const int k = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    if (!spec_block(blk_dev, t_stop, n_i, t)) return;
     if (k >= n_i) return;
     const int32_t i = idx_i[k];
     const BodyD I = predict_body(aos, i, t);
@@ -1374,11 +1396,13 @@ __global__ void __launch_bounds__(256) init_steps_kernel(int64_t N, int64_t Ns, 
 // then the block rule (double once if allowed and t1 is commensurate, else halve while too long).
 // One thread per active body; reads its 128 B line of the gather copy, writes both copies.  FP64.
 __global__ void __launch_bounds__(128) correct_kernel(int32_t n, int64_t Ns, double t1, double eta, double dt_max,
+                                                      const double *__restrict__ blk_dev, double t_stop,
                                                       const int32_t *__restrict__ idx,
                                                       const double *__restrict__ acc1,
                                                       const double *__restrict__ jerk1, double *__restrict__ soa,
                                                       double *__restrict__ aos, double *__restrict__ dtj) {
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (!spec_block(blk_dev, t_stop, n, t1)) return;
     if (k >= n) return;
     const int64_t i = idx[k];
     const double2 *p = reinterpret_cast<const double2 *>(aos + i * AOS_D);

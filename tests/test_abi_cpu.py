@@ -65,12 +65,13 @@ def test_i_sharding_covers_block_exactly_once():
 
 def test_plan_regular_fills_the_chip_and_covers_the_j_range():
     """nb_plan_regular (pure host function of the library): the split covers every j-tile, pads the
-    block as little as any variant can, and its modelled cost (waves x tiles per split) is within
-    1 % of the best over all splits."""
+    block as little as any variant can, and its modelled cost -- (waves + 0.13) x (tiles per split + per-CTA
+    overhead) + finalize cost per split, DESIGN.md section 7 -- is within 1.5 % of the best over all splits,
+    with no smaller split count inside that window."""
     import paper_1504_03687_b200 as nb
     sm, per_sm = 148, 2
     conc = sm * per_sm
-    ovh = {512: 0.5, 256: 0.75, 128: 1.5, 64: 3.0, 32: 3.0}
+    tile_us = lambda ib: ib * 256 / 3.6e9 * 1e6
     rate = {512: 1.0, 256: 1.01, 128: 1.025, 64: 1.03, 32: 1.11}     # cost per padded i-slot (DESIGN.md section 7)
     for N in (1024, 65536, 262144, 1048576, 1000003):
         ntiles = -(-N // 256)
@@ -84,9 +85,17 @@ def test_plan_regular_fills_the_chip_and_covers_the_j_range():
             assert abs(pad * rate[ib] - min(-(-n_i // b) * b * rate[b] for b in rate)) < 1e-9 * pad   # least rate-weighted padded work
             assert 1 <= S <= ntiles and tps == -(-ntiles // S) and (S - 1) * tps < ntiles <= S * tps
             n_ib = pad // ib
-            cost = lambda s: -(-(n_ib * -(-ntiles // -(-ntiles // s))) // conc) * (-(-ntiles // s) + ovh[ib])
-            best = min(cost(s) for s in range(1, min(ntiles, 8192) + 1))
-            assert cost(S) <= 1.01 * best
+
+            def cost(s):
+                t = -(-ntiles // s)
+                seff = -(-ntiles // t)
+                waves = -(-(n_ib * seff) // conc)
+                return (waves + 0.13) * (t + 5.0 / tile_us(ib)) + 0.005 * seff / tile_us(ib)
+
+            costs = {s: cost(s) for s in range(1, min(ntiles, 8192) + 1)}
+            best = min(costs.values())
+            assert costs[S] <= 1.0151 * best
+            assert all(costs[s] > 1.0149 * best for s in range(1, S) if -(-ntiles // -(-ntiles // s)) != S)
     p = nb.nb_plan_regular(1048576, 8192, sm, per_sm)
     assert p["iblock"] == 512 and p["jsplit"] * (8192 // p["iblock"]) % conc == 0   # the headline block: whole waves
     assert nb.nb_plan_regular(1048576, 32)["iblock"] == 32 and nb.nb_plan_regular(1048576, 64)["iblock"] == 64

