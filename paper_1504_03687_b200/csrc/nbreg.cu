@@ -46,8 +46,7 @@ struct nb_ctx {
     unsigned int *stats = nullptr;          // {warps in the local frame, warps} since NB_TUNE_STATS was set
     // Morton reordering of large blocks (reorder_block): sort scratch, bounding box
     int64_t reorder_min = 4096;             // NB_TUNE_REORDER_MIN: blocks of at least this many particles; 0 = never
-    unsigned long long *sort_keys = nullptr;
-    int32_t *sort_vals = nullptr;           // after the sort: perm[slot] = k
+    unsigned long long *sort_keys = nullptr;   // after the sort: slot -> k = key & PERM_MASK
     uint32_t *sort_box = nullptr;
     int64_t sort_n = 0;
     int64_t last_reordered = 0;
@@ -250,7 +249,7 @@ int ensure_partial(nb_ctx *c, size_t bytes) {
 // One force-kernel launch over the j-tiles [tile0, tile1) split S ways, writing partial rows
 // [split0, split0 + S).
 int launch_force_range(nb_ctx *c, int vi, bool fused, int32_t n_i, const int32_t *idx_i, const double *h2_i,
-                       const float *irec, const int32_t *perm, int64_t j_offset, int32_t *nblist, int64_t tile0,
+                       const float *irec, const unsigned long long *perm, int64_t j_offset, int32_t *nblist, int64_t tile0,
                        int64_t tile1, int S, int64_t split0) {
     const Variant &v = fused ? c->fvar[vi] : c->var[vi];
     const int64_t n_ib = (n_i + v.iblock - 1) / v.iblock;
@@ -316,9 +315,11 @@ int ensure_aos(nb_ctx *c) {
 
 // a6-a7: fixed-order sum of the S partial rows, counters, sorted list rows.  perm (or NULL): slot -> k of
 // a block the library reordered (Morton order, reorder_block).
-int launch_finalize(nb_ctx *c, int32_t n_i, int64_t n_i_pad, int S, const int32_t *perm, double *acc, double *jerk,
+int launch_finalize(nb_ctx *c, int32_t n_i, int64_t n_i_pad, int S, const unsigned long long *perm, double *acc, double *jerk,
                     double *pot, int32_t *nnb, int32_t *nblist, int32_t *overflow) {
-    const int W = S <= 8 ? 4 : 16;
+    // small blocks: 16 warps share the S partial rows (latency); large blocks have CTAs enough: 4 warps, and a
+    // row's sort gets a 128-thread CTA
+    const int W = (S > 8 && n_i <= 512) ? 16 : 4;
     const size_t row_bytes = (size_t)c->sort_P * sizeof(int32_t);
     const int sortP = (nblist && row_bytes <= c->sort_smem_max) ? c->sort_P : 0;   // 0: rows stay in append order
     const dim3 fgrid((unsigned)((n_i + 31) / 32), (unsigned)(7 + 32));
@@ -351,17 +352,16 @@ int launch_finalize(nb_ctx *c, int32_t n_i, int64_t n_i_pad, int S, const int32_
     return NB_OK;
 }
 
-// Morton order of a large block (a3): c->sort_vals[slot] = k afterwards.  Reads the predicted records of
-// the active particles (irec if given, else rec[idx_i[k]]); everything on the context's stream.
+// Morton order of a large block (a3): c->sort_keys[slot] & PERM_MASK = k afterwards.  Reads the predicted
+// records of the active particles (irec if given, else rec[idx_i[k]]); everything on the context's stream.
 int reorder_block(nb_ctx *c, int32_t n_i, const int32_t *idx_i, const float *irec, int64_t n_i_pad) {
     int64_t n2 = 2;
     while (n2 < n_i) n2 <<= 1;
     if (n2 > c->sort_n) {
         NB_CUDA(c, cudaStreamSynchronize(c->stream));
-        cudaFree(c->sort_keys); cudaFree(c->sort_vals);
-        c->sort_keys = nullptr; c->sort_vals = nullptr; c->sort_n = 0;
+        cudaFree(c->sort_keys);
+        c->sort_keys = nullptr; c->sort_n = 0;
         NB_CUDA(c, cudaMalloc(&c->sort_keys, sizeof(unsigned long long) * n2));
-        NB_CUDA(c, cudaMalloc(&c->sort_vals, sizeof(int32_t) * n2));
         c->sort_n = n2;
     }
     if (!c->sort_box) NB_CUDA(c, cudaMalloc(&c->sort_box, 6 * sizeof(uint32_t)));
@@ -369,27 +369,25 @@ int reorder_block(nb_ctx *c, int32_t n_i, const int32_t *idx_i, const float *ire
     const unsigned gb = (unsigned)std::min<int64_t>((n_i + 255) / 256, (int64_t)c->sm_count * 4);
     block_bbox_kernel<<<gb, 256, 0, c->stream>>>(n_i, n_i_pad, idx_i, c->rec, irec, c->sort_box);
     morton_key_kernel<<<(unsigned)((n2 + 255) / 256), 256, 0, c->stream>>>(n_i, (int32_t)n2, n_i_pad, idx_i, c->rec, irec,
-                                                                          c->sort_box, c->sort_keys, c->sort_vals);
+                                                                          c->sort_box, c->sort_keys);
     const int64_t ch = std::min<int64_t>(n2, SORT_CH);
     const unsigned chunks = (unsigned)(n2 / ch);
-    const size_t smem = (size_t)ch * (sizeof(unsigned long long) + sizeof(int32_t));
-    bitonic_chunk_kernel<0><<<chunks, SORT_T, smem, c->stream>>>((int32_t)n2, 0, c->sort_keys, c->sort_vals);
+    bitonic_chunk_kernel<0><<<chunks, SORT_T, 0, c->stream>>>((int32_t)n2, 0, c->sort_keys);
     c->launches += 3;
     for (int64_t size = 2 * ch; size <= n2; size <<= 1) {
         for (int64_t stride = size / 2; stride >= ch; stride >>= 1) {
             bitonic_global_kernel<<<(unsigned)((n2 / 2 + 255) / 256), 256, 0, c->stream>>>((int32_t)n2, (int32_t)size,
-                                                                                          (int32_t)stride, c->sort_keys,
-                                                                                          c->sort_vals);
+                                                                                          (int32_t)stride, c->sort_keys);
             c->launches += 1;
         }
-        bitonic_chunk_kernel<1><<<chunks, SORT_T, smem, c->stream>>>((int32_t)n2, (int32_t)size, c->sort_keys, c->sort_vals);
+        bitonic_chunk_kernel<1><<<chunks, SORT_T, 0, c->stream>>>((int32_t)n2, (int32_t)size, c->sort_keys);
         c->launches += 1;
     }
     NB_CUDA(c, cudaGetLastError());
     return NB_OK;
 }
 bool want_reorder(const nb_ctx *c, int32_t n_i) {
-    return c->local_g > 0.0 && c->reorder_min > 0 && n_i >= c->reorder_min;
+    return c->local_g > 0.0 && c->reorder_min > 0 && n_i >= c->reorder_min && (int64_t)n_i <= (int64_t)PERM_MASK;
 }
 
 int regular_device(nb_ctx *c, int32_t n_i, const int32_t *idx_i, const double *h2_i, double *acc, double *jerk,
@@ -407,12 +405,12 @@ int regular_device(nb_ctx *c, int32_t n_i, const int32_t *idx_i, const double *h
     const int64_t n_i_pad = n_ib * v.iblock;
     rc = ensure_partial(c, (size_t)S * 7 * n_i_pad * sizeof(double));
     if (rc != NB_OK) return rc;
-    const int32_t *perm = nullptr;
+    const unsigned long long *perm = nullptr;
     c->last_reordered = 0;
     if (!fused && want_reorder(c, n_i)) {
         rc = reorder_block(c, n_i, idx_i, nullptr, n_i_pad);
         if (rc != NB_OK) return rc;
-        perm = c->sort_vals; c->last_reordered = 1;
+        perm = c->sort_keys; c->last_reordered = 1;
     }
     rc = launch_force_range(c, vi, fused, n_i, idx_i, h2_i, nullptr, perm, 0, nblist, 0, ntiles, S, 0);
     if (rc != NB_OK) return rc;
@@ -519,11 +517,6 @@ int nb_open(int64_t N, int32_t nb_cap, nb_ctx **out) {
     NB_CUDA(c, (setup_variant<2, 4, 2, false, SRC_STATE>(c->fvar[2], VAR_OVH[2])));
     NB_CUDA(c, (setup_variant<1, 8, 2, false, SRC_STATE>(c->fvar[3], VAR_OVH[3])));
     NB_CUDA(c, (setup_variant<1, 8, 2, true, SRC_STATE>(c->fvar[4], VAR_OVH[4])));
-    {
-        const int sort_smem = SORT_CH * (int)(sizeof(unsigned long long) + sizeof(int32_t));
-        NB_CUDA(c, cudaFuncSetAttribute(bitonic_chunk_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, sort_smem));
-        NB_CUDA(c, cudaFuncSetAttribute(bitonic_chunk_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, sort_smem));
-    }
     NB_CUDA(c, cudaStreamSynchronize(nullptr));     // the ghost padding is in place before any stream uses the state
     return NB_OK;
 }
@@ -532,7 +525,7 @@ int nb_close(nb_ctx *c) {
     if (!c) return NB_EINVAL;
     cudaStreamSynchronize(c->stream);
     cudaFree(c->soa); cudaFree(c->aos); cudaFree(c->rec); cudaFree(c->cnt); cudaFree(c->stats);
-    cudaFree(c->sort_keys); cudaFree(c->sort_vals); cudaFree(c->sort_box);
+    cudaFree(c->sort_keys); cudaFree(c->sort_box);
     cudaFree(c->blk_key); cudaFree(c->blk_idx); cudaFree(c->blk_out); cudaFree(c->blk_nnb); cudaFree(c->blk_ovf);
     cudaFree(c->blk_list);
     cudaFree(c->partial); cudaFree(c->stage_j);
@@ -839,12 +832,12 @@ int nb_step_host(nb_ctx *c, const double *m, const double *x0, const double *v0,
         predict_i_kernel<false><<<(unsigned)((n_i + 255) / 256), 256, 0, c->stream>>>(n_i, (int32_t)n_i_pad, t, isrc, c->irec);
     NB_CUDA(c, cudaGetLastError());
     c->launches += 1;
-    const int32_t *perm = nullptr;
+    const unsigned long long *perm = nullptr;
     c->last_reordered = 0;
     if (want_reorder(c, n_i)) {        // from the active particles' own records: no chunk of the j-state is needed
         rc = reorder_block(c, n_i, c->st_idx, c->irec, n_i_pad);
         if (rc != NB_OK) return rc;
-        perm = c->sort_vals; c->last_reordered = 1;
+        perm = c->sort_keys; c->last_reordered = 1;
     }
     int64_t split0 = 0;
     for (int q = 0; q < nchunk; ++q) {
@@ -1133,12 +1126,12 @@ int nb_regular_shard(nb_ctx *c, double t, int32_t n_i, const int32_t *idx_i, con
     predict_i_kernel<false><<<(unsigned)((n_i + 255) / 256), 256, 0, c->stream>>>(n_i, (int32_t)n_i_pad, t, isrc, c->irec);
     NB_CUDA(c, cudaGetLastError());
     c->launches += 1;
-    const int32_t *perm = nullptr;
+    const unsigned long long *perm = nullptr;
     c->last_reordered = 0;
     if (want_reorder(c, n_i)) {
         rc = reorder_block(c, n_i, idx_i, c->irec, n_i_pad);
         if (rc != NB_OK) return rc;
-        perm = c->sort_vals; c->last_reordered = 1;
+        perm = c->sort_keys; c->last_reordered = 1;
     }
     rc = launch_force_range(c, vi, false, n_i, idx_i, h2_i, c->irec, perm, c->j_offset, nblist, 0, ntiles, S, 0);
     if (rc != NB_OK) return rc;

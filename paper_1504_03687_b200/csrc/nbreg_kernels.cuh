@@ -292,9 +292,9 @@ __global__ void __launch_bounds__(256) predict_i_kernel(int32_t n_i, int32_t n_i
 // The local frame of force_kernel needs the 64 i-particles of a warp to sit close together.  A block
 // arrives in the caller's order (NBODY6++GPU: the step-sorted list, P:89 -- not spatial), so for large
 // blocks the library sorts the SLOTS of the block along a Morton curve of the predicted positions:
-// bounding box (integer atomics on ordered keys: order-independent), 63-bit keys (21 bits per axis on
+// bounding box (integer atomics on ordered keys: order-independent), 42-bit keys (14 bits per axis on
 // the box), ties broken by k, bitonic sort (no atomics: the permutation is a pure function of the
-// inputs, so results stay bitwise reproducible).  perm[slot] = k.
+// inputs, so results stay bitwise reproducible).
 __device__ __forceinline__ uint32_t ordered_u32(float x) {             // monotone map float -> uint32
     const uint32_t b = __float_as_uint(x);
     return (b >> 31) ? ~b : (b | 0x80000000u);
@@ -342,14 +342,22 @@ __global__ void __launch_bounds__(256) block_bbox_kernel(int32_t n_i, int64_t n_
     }
 }
 
-// keys[s], vals[s] for the n2 = 2^m >= n_i slots of the sort; slots >= n_i sort to the end.
+// keys[s] for the n2 = 2^m >= n_i slots of the sort: (42-bit Morton code of the position on the block's
+// bounding box, 14 bits per axis) << 22 | k -- ONE 64-bit compare orders by cell and breaks ties by k, and
+// after the sort perm[slot] = key & PERM_MASK.  Slots >= n_i sort to the end.  (k < 2^22: blocks of up to
+// 4M particles; larger blocks are not reordered.)
+constexpr int PERM_BITS = 22;
+constexpr unsigned long long PERM_MASK = (1ull << PERM_BITS) - 1;
+__device__ __forceinline__ int32_t perm_slot(const unsigned long long *perm, int slot) {
+    return (int32_t)(perm[slot] & PERM_MASK);
+}
 __global__ void __launch_bounds__(256) morton_key_kernel(int32_t n_i, int32_t n2, int64_t n_i_pad,
                                                          const int32_t *__restrict__ idx_i, const float *__restrict__ rec,
                                                          const float *__restrict__ irec, const uint32_t *__restrict__ box,
-                                                         unsigned long long *__restrict__ keys, int32_t *__restrict__ vals) {
+                                                         unsigned long long *__restrict__ keys) {
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= n2) return;
-    if (k >= n_i) { keys[k] = ~0ull; vals[k] = 0x7fffffff; return; }
+    if (k >= n_i) { keys[k] = ~0ull; return; }
     int64_t cs;
     const float *r = irec_or_rec(rec, irec, idx_i, k, n_i_pad, cs);
     unsigned long long key = 0;
@@ -358,28 +366,23 @@ __global__ void __launch_bounds__(256) morton_key_kernel(int32_t n_i, int32_t n2
         const float mn = ordered_to_float(box[c]), mx = ordered_to_float(~box[3 + c]);
         const float ext = mx - mn;
         const float u = ext > 0.f ? (r[(C_XH + c) * cs] - mn) / ext : 0.f;             // in [0, 1]
-        const uint32_t q = min((uint32_t)(u * 2097152.0f), 2097151u);                   // 21 bits
+        const uint32_t q = min((uint32_t)(u * 16384.0f), 16383u);                       // 14 bits
         key |= spread21(q) << (2 - c);
     }
-    keys[k] = key;
-    vals[k] = k;
+    keys[k] = (key << PERM_BITS) | (unsigned long long)k;
 }
 
-// Bitonic sort of (key, val) pairs, ascending by key then val.  SORT_CH pairs per CTA live in shared memory.
-constexpr int SORT_CH = 8192;
+// Bitonic sort of the 64-bit keys, ascending.  SORT_CH keys per CTA live in shared memory (one
+// compare-exchange per thread and step); merges across chunks go through global memory.
+constexpr int SORT_CH = 2048;
 constexpr int SORT_T = 1024;
-__device__ __forceinline__ bool pair_gt(unsigned long long ka, int32_t va, unsigned long long kb, int32_t vb) {
-    return ka > kb || (ka == kb && va > vb);
-}
 // MODE 0: full sort of each chunk (sizes 2 .. chunk).  MODE 1: the strides chunk/2 .. 1 of merge size `size`.
 template <int MODE>
-__global__ void __launch_bounds__(SORT_T) bitonic_chunk_kernel(int32_t n2, int32_t size, unsigned long long *__restrict__ keys,
-                                                              int32_t *__restrict__ vals) {
-    extern __shared__ unsigned long long sk[];                                  // [ch] keys, then [ch] vals
+__global__ void __launch_bounds__(SORT_T) bitonic_chunk_kernel(int32_t n2, int32_t size, unsigned long long *__restrict__ keys) {
+    __shared__ unsigned long long sk[SORT_CH];
     const int ch = min(n2, SORT_CH);
-    int32_t *sv = reinterpret_cast<int32_t *>(sk + ch);
     const int base = blockIdx.x * ch;
-    for (int e = threadIdx.x; e < ch; e += SORT_T) { sk[e] = keys[base + e]; sv[e] = vals[base + e]; }
+    for (int e = threadIdx.x; e < ch; e += SORT_T) sk[e] = keys[base + e];
     __syncthreads();
     for (int sz = (MODE == 0 ? 2 : size); sz <= (MODE == 0 ? ch : size); sz <<= 1) {
         for (int stride = min(sz >> 1, ch >> 1); stride > 0; stride >>= 1) {
@@ -387,24 +390,22 @@ __global__ void __launch_bounds__(SORT_T) bitonic_chunk_kernel(int32_t n2, int32
                 const int lo = 2 * e - (e & (stride - 1)), hi = lo + stride;
                 const bool up = ((base + lo) & sz) == 0;
                 const unsigned long long ka = sk[lo], kb = sk[hi];
-                const int32_t va = sv[lo], vb = sv[hi];
-                if (pair_gt(ka, va, kb, vb) == up) { sk[lo] = kb; sk[hi] = ka; sv[lo] = vb; sv[hi] = va; }
+                if ((ka > kb) == up) { sk[lo] = kb; sk[hi] = ka; }
             }
             __syncthreads();
         }
     }
-    for (int e = threadIdx.x; e < ch; e += SORT_T) { keys[base + e] = sk[e]; vals[base + e] = sv[e]; }
+    for (int e = threadIdx.x; e < ch; e += SORT_T) keys[base + e] = sk[e];
 }
 // One compare-exchange step (merge size `size`, stride >= SORT_CH) in global memory.
 __global__ void __launch_bounds__(256) bitonic_global_kernel(int32_t n2, int32_t size, int32_t stride,
-                                                            unsigned long long *__restrict__ keys, int32_t *__restrict__ vals) {
+                                                            unsigned long long *__restrict__ keys) {
     const int e = blockIdx.x * blockDim.x + threadIdx.x;
     if (e >= (n2 >> 1)) return;
     const int lo = 2 * e - (e & (stride - 1)), hi = lo + stride;
     const bool up = (lo & size) == 0;
     const unsigned long long ka = keys[lo], kb = keys[hi];
-    const int32_t va = vals[lo], vb = vals[hi];
-    if (pair_gt(ka, va, kb, vb) == up) { keys[lo] = kb; keys[hi] = ka; vals[lo] = vb; vals[hi] = va; }
+    if ((ka > kb) == up) { keys[lo] = kb; keys[hi] = ka; }
 }
 
 // ------------------------------------------------------------------ a3-a6: force kernel
@@ -437,7 +438,7 @@ struct ForceParams {
     const int32_t *idx_i;         // [n_i], or NULL: the block is 0..n_i-1
     const double *h2_i;           // [n_i]; or [N] indexed by body when h2_by_body; or NULL: every h2 = 0
     int32_t h2_by_body;
-    const int32_t *perm;          // NULL, or slot -> k of a block the library put in Morton order (lanes hold slots)
+    const unsigned long long *perm;   // NULL, or sorted keys of a block the library put in Morton order: slot -> k = key & PERM_MASK
     int32_t n_i;
     int32_t n_i_pad;              // n_i rounded up to the CTA's i-block
     const float *irec;            // NULL, or the active particles' own records [RECF][n_i_pad] (nb_step_host, shards)
@@ -722,7 +723,7 @@ __global__ void __launch_bounds__(32 * WI *WJ, MINB) force_kernel(const ForcePar
         for (int h = 0; h < NH; ++h) {
             const int slot = blockIdx.x * IB + wi * (32 * NH) + h * 32 + lane;
             valid[h] = slot < n_i;
-            const int k = (valid[h] && p.perm) ? p.perm[slot] : slot;      // caller's numbering: rows, counters, inputs
+            const int k = (valid[h] && p.perm) ? perm_slot(p.perm, slot) : slot;   // caller's numbering: rows, counters, inputs
             my_k[h] = k;
             my_idx[h] = -1;
 #pragma unroll
@@ -1021,7 +1022,7 @@ __global__ void __launch_bounds__(32 * WI *WJ, MINB) force_kernel(const ForcePar
 //                     oracle's ascending rows.
 template <int W>
 __global__ void __launch_bounds__(32 * W) finalize_kernel(int32_t n_i, int32_t n_i_pad, int32_t S, int32_t cap,
-                                                          int32_t sortP, const int32_t *__restrict__ perm,
+                                                          int32_t sortP, const unsigned long long *__restrict__ perm,
                                                           const double *__restrict__ blk_dev, double t_stop,
                                                           const double *__restrict__ partial,
                                                           int32_t *__restrict__ cnt, double *__restrict__ acc,
@@ -1063,7 +1064,7 @@ __global__ void __launch_bounds__(32 * W) finalize_kernel(int32_t n_i, int32_t n
             double t = red[0][lane];
 #pragma unroll
             for (int ww = 1; ww < W; ++ww) t += red[ww][lane];
-            const int k = perm ? perm[slot] : slot;
+            const int k = perm ? perm_slot(perm, slot) : slot;
             if (q < 3) acc[3 * k + q] = t;
             else if (q < 6) jerk[3 * k + q - 3] = t;
             else pot[k] = -t;
@@ -1288,9 +1289,18 @@ __global__ void __launch_bounds__(256) select_block_kernel(int64_t N, const doub
     __shared__ unsigned long long wbest[8];
     __shared__ int32_t wsum[8];
     __shared__ int32_t base_s;
-    // ---- phase 1: t_next = min_j (t0_j + dt_j)
+    // ---- phase 1: t_next = min_j (t0_j + dt_j).  The CTA's FIRST chunk stays in registers for the other two
+    //      phases (at N <= grid x 2048 that is everything: one pass over memory instead of three).
+    constexpr int PER = SEL_CHUNK / 256;
+    double first[PER];
     unsigned long long best = ~0ull;
-    for (int b = blockIdx.x; b < nchunk; b += gridDim.x)
+#pragma unroll
+    for (int u = 0; u < PER; ++u) {
+        const int64_t j = (int64_t)blockIdx.x * SEL_CHUNK + u * 256 + threadIdx.x;
+        first[u] = (blockIdx.x < nchunk && j < N) ? t0[j] + dtj[j] : __longlong_as_double(0x7ff8000000000000ll);   // NaN: never due
+        if (first[u] == first[u]) best = min(best, ordered_key(first[u]));
+    }
+    for (int b = blockIdx.x + gridDim.x; b < nchunk; b += gridDim.x)
         for (int s = 0; s < SEL_CHUNK; s += 256) {
             const int64_t j = (int64_t)b * SEL_CHUNK + s + threadIdx.x;
             if (j < N) best = min(best, ordered_key(t0[j] + dtj[j]));
@@ -1310,9 +1320,14 @@ __global__ void __launch_bounds__(256) select_block_kernel(int64_t N, const doub
     // ---- phase 2: active bodies per chunk
     for (int b = blockIdx.x; b < nchunk; b += gridDim.x) {
         int32_t cntc = 0;
-        for (int s = 0; s < SEL_CHUNK; s += 256) {
-            const int64_t j = (int64_t)b * SEL_CHUNK + s + threadIdx.x;
-            cntc += (j < N && (t0[j] + dtj[j] == tn)) ? 1 : 0;
+        if (b == (int)blockIdx.x) {
+#pragma unroll
+            for (int u = 0; u < PER; ++u) cntc += first[u] == tn ? 1 : 0;
+        } else {
+            for (int s = 0; s < SEL_CHUNK; s += 256) {
+                const int64_t j = (int64_t)b * SEL_CHUNK + s + threadIdx.x;
+                cntc += (j < N && (t0[j] + dtj[j] == tn)) ? 1 : 0;
+            }
         }
 #pragma unroll
         for (int off = 16; off > 0; off >>= 1) cntc += __shfl_xor_sync(0xffffffffu, cntc, off);
@@ -1344,9 +1359,11 @@ __global__ void __launch_bounds__(256) select_block_kernel(int64_t N, const doub
         }
         __syncthreads();
         int32_t running = base_s;
-        for (int s = 0; s < SEL_CHUNK; s += 256) {
+#pragma unroll
+        for (int u = 0; u < PER; ++u) {
+            const int s = u * 256;
             const int64_t j = (int64_t)b * SEL_CHUNK + s + threadIdx.x;
-            const bool act = j < N && (t0[j] + dtj[j] == tn);
+            const bool act = b == (int)blockIdx.x ? first[u] == tn : (j < N && (t0[j] + dtj[j] == tn));
             const unsigned bal = __ballot_sync(0xffffffffu, act);
             __syncthreads();
             if (lane == 0) wsum[w] = __popc(bal);
