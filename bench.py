@@ -44,6 +44,10 @@ def parse():
     ap.add_argument("--N", type=int, default=1048576, help="override N (debug only; the metric is N=1M)")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--variant", type=int, default=-1, help="force a force-kernel variant (tuning experiments)")
+    ap.add_argument("--shard", default="i", choices=["i", "j"],
+                    help="N > 1 ranks: i = every rank holds all N bodies and takes its share of a world x n_i block (no "
+                         "collective, weak scaling; default); j = every rank holds N / world bodies and all ranks evaluate "
+                         "the SAME n_i block (SURVEY 8(f) NEXT-4: state all-reduce, sums / lists all-gather; strong scaling)")
     ap.add_argument("--no-sweep", action="store_true")
     ap.add_argument("--no-extras", action="store_true", help="skip the NEXT-row timings (nb_block_step, nb_irregular, ...)")
     ap.add_argument("--all-configs", action="store_true",
@@ -209,6 +213,8 @@ def run_b200(args):
 
     import nbgen
     N = args.N
+    if args.shard == "j":
+        return run_b200_jsharded(args, world, rank, local)
     cfg, idx_all, h2_all = build_workload(N, args.n_i * world)
     idx_np, h2_np = nbgen.shard_active_block(idx_all, h2_all, rank, world)   # i-sharding, no collective
     n_i = int(idx_np.shape[0])
@@ -521,6 +527,85 @@ def run_b200(args):
         "cpu_baseline": cpu, "sweep": sweep, "other_configs": other, "extras": extras, "peaks_source": pk_src,
     }
     print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def run_b200_jsharded(args, world, rank, local):
+    """--shard j: each rank owns a contiguous N / world slice of the bodies in its own context; every step all
+    ranks evaluate the same active block with nb_regular_shard and exchange the partial results
+    (paper_1504_03687_b200.parallel: Table 2).  Total work is fixed: strong scaling."""
+    import torch
+    import torch.distributed as dist
+    import nbgen
+    import paper_1504_03687_b200 as nb
+    from paper_1504_03687_b200 import parallel as par
+    N = args.N
+    cfg, idx_np, h2_np = build_workload(N, args.n_i)
+    n_i, cap, t_pred = int(idx_np.shape[0]), cfg["cap"], float(cfg["t"])
+    dev = torch.device("cuda", local)
+    stream = torch.cuda.current_stream()
+    b = par.shard_bounds(N, world)
+    lo, hi = b[rank], b[rank + 1]
+    f64 = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float64)).to(dev)
+    state = {k: f64(cfg[k][lo:hi]) for k in par.STATE_KEYS}
+    ctx = nb.nb_open(hi - lo, cap, stream)
+    ctx.set_j_offset(lo)
+    idx, h2 = torch.from_numpy(np.ascontiguousarray(idx_np)).to(dev), f64(h2_np)
+
+    def step():
+        ctx.set_j(*(state[k] for k in par.STATE_KEYS))
+        ctx.predict_all(t_pred)
+        return par.regular_jsharded(ctx, state, lo, t_pred, idx, h2)
+
+    for _ in range(max(args.warmup, 3)):
+        res = step()
+    torch.cuda.synchronize()
+    launches0 = ctx.info("kernel_launches")
+    sampler = ClockSampler(local) if rank == 0 else None
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    w0 = time.time()
+    e0.record(stream)
+    for _ in range(args.steps):
+        res = step()
+    e1.record(stream)
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    w1 = time.time()
+    ms = e0.elapsed_time(e1)
+    launches = ctx.info("kernel_launches") - launches0
+    if world > 1:
+        tt = torch.tensor([ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        ms = float(tt.item())
+        tl = torch.tensor([launches], dtype=torch.int64, device=dev)
+        dist.all_reduce(tl, op=dist.ReduceOp.SUM)
+        launches = int(tl.item())
+    clocks = sampler.stop(w0, w1) if sampler else None
+    if rank == 0:
+        pk, pk_src = peaks()
+        sm_max_mhz = float((clocks or {}).get("sm_max_mhz") or pk.get("sm_max_mhz", 1965.0))
+        peak_tflops = ctx.info("sm_count") * 128 * 2 * sm_max_mhz * 1e6 / 1e12
+        value = float(n_i) * N * args.steps / (ms * 1e-3)
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "strong",
+            "vs_baseline": None, "dtype": "f32 pair math (x differenced in warp-local f32 frames or as hi/lo f32 pairs, f64 sums)",
+            "data": "synthetic",
+            "config": {"workload": WORKLOAD, "N": N, "n_i": n_i, "nb_cap": cap, "parallelism": f"j-shard x{world}",
+                       "step": "per rank: nb_set_j(shard) + nb_predict_all + nb_regular_shard; state all-reduce, "
+                               "sums + list rows all-gather (paper_1504_03687_b200.parallel)",
+                       "l2": "each step streams the shard's state through set_j + predict before the force kernel"},
+            "frac_fp32_peak": value / world * FLOP_PER_INTERACTION / 1e12 / peak_tflops, "clocks": clocks, "e2e": None,
+            "gpu_launches": int(launches), "roofline": None, "cpu_baseline": None,
+            "checksum_pot": float(res["pot"].sum()), "peaks_source": pk_src,
+        }
+        print(json.dumps(line), flush=True)
+    ctx.close()
     if world > 1:
         dist.destroy_process_group()
 

@@ -4,8 +4,9 @@ P:127: "each GPU has a similar particle dataset size ... all GPUs in the same no
 complete particle dataset"; Table 2: calculation O(N_i N) against communication O(N_i).  Every
 rank owns a contiguous shard of the bodies in its own `NbContext` (nb_open(N_shard), nb_set_j,
 nb_set_j_offset) and evaluates its shard's contribution to the active block with nb_regular_shard;
-what crosses the wire per active particle is its 14-double state (in), 7 doubles + 1 count (sums,
-all-reduce) and its list row (all-gather).  The collectives are plain `torch.distributed` calls
+what crosses the wire per active particle is its 14-double state (in, one all-reduce with a single non-zero
+contributor per column: exact), 7 doubles + 1 count per shard (all-gather, summed in rank order: deterministic)
+and its list row (all-gather).  The collectives are plain `torch.distributed` calls
 (NCCL over NVLink on GPUs, gloo in the CPU tests): a few hundred KB against milliseconds of pair
 arithmetic -- there is no compute step to fuse them into.
 
@@ -17,6 +18,38 @@ import torch
 import torch.distributed as dist
 
 STATE_KEYS = ("m", "x0", "v0", "a0", "j0", "t0")       # order of nb_set_j and of the istate rows
+
+
+def _world(group=None) -> int:
+    return dist.get_world_size(group) if dist.is_initialized() else 1
+
+
+def _via_host(t: torch.Tensor, group=None) -> bool:
+    """gloo has no CUDA all_gather: with that backend (two ranks sharing one GPU in the tests) the few hundred
+    KB of a block go through host memory; NCCL takes the device tensors as they are."""
+    return t.is_cuda and dist.get_backend(group) == "gloo"
+
+
+def _all_reduce_sum(t: torch.Tensor, group=None) -> torch.Tensor:
+    if _world(group) == 1:
+        return t
+    if _via_host(t, group):
+        h = t.cpu()
+        dist.all_reduce(h, op=dist.ReduceOp.SUM, group=group)
+        return h.to(t.device)
+    dist.all_reduce(t, op=dist.ReduceOp.SUM, group=group)
+    return t
+
+
+def _all_gather(t: torch.Tensor, group=None) -> torch.Tensor:
+    """[world, *t.shape], rank order."""
+    world = _world(group)
+    if world == 1:
+        return t[None]
+    src = t.cpu().contiguous() if _via_host(t, group) else t.contiguous()
+    parts = [torch.empty_like(src) for _ in range(world)]
+    dist.all_gather(parts, src, group=group)
+    return torch.stack(parts).to(t.device)
 
 
 def shard_bounds(N: int, world: int, tile: int = 256) -> list[int]:
@@ -41,9 +74,7 @@ def gather_istate(state: dict, offset: int, idx_global: torch.Tensor, group=None
     ist[13, mine] = state["t0"][sel]
     for r0, key in ((1, "x0"), (4, "v0"), (7, "a0"), (10, "j0")):
         ist[r0:r0 + 3, mine] = state[key][sel].T
-    if dist.is_initialized() and dist.get_world_size(group) > 1:
-        dist.all_reduce(ist, op=dist.ReduceOp.SUM, group=group)
-    return ist
+    return _all_reduce_sum(ist, group)
 
 
 def merge_list_rows(rows: torch.Tensor, counts: torch.Tensor, cap: int):
@@ -63,22 +94,19 @@ def merge_list_rows(rows: torch.Tensor, counts: torch.Tensor, cap: int):
 
 
 def combine(part: dict, cap: int, group=None) -> dict:
-    """Per-shard partial outputs of nb_regular_shard -> the block's results on every rank."""
-    n = part["pot"].shape[0]
-    world = dist.get_world_size(group) if dist.is_initialized() else 1
+    """Per-shard partial outputs of nb_regular_shard -> the block's results on every rank.  The seven sums
+    per active particle are all-gathered and added IN RANK ORDER on every rank (not all-reduced: the order of
+    an all-reduce is the collective library's choice), so the FP64 result is bitwise the same on every rank
+    and from run to run (reading R19; copies must not diverge)."""
     sums = torch.cat([part["acc"], part["jerk"], part["pot"][:, None]], dim=1).contiguous()    # [n][7]
-    counts = part["nnb"].to(torch.int64)
-    if world > 1:
-        dist.all_reduce(sums, op=dist.ReduceOp.SUM, group=group)
-        rows_all = [torch.empty_like(part["nblist"]) for _ in range(world)]
-        cnt_all = [torch.empty_like(counts) for _ in range(world)]
-        dist.all_gather(rows_all, part["nblist"].contiguous(), group=group)
-        dist.all_gather(cnt_all, counts, group=group)
-        rows, cnts = torch.stack(rows_all), torch.stack(cnt_all)
-    else:
-        rows, cnts = part["nblist"][None], counts[None]
+    all_sums = _all_gather(sums, group)                                                         # [G][n][7]
+    total = all_sums[0].clone()
+    for g in range(1, all_sums.shape[0]):
+        total += all_sums[g]
+    rows = _all_gather(part["nblist"], group)
+    cnts = _all_gather(part["nnb"].to(torch.int64), group)
     nblist, nnb, overflow = merge_list_rows(rows, cnts, cap)
-    return dict(acc=sums[:, 0:3].contiguous(), jerk=sums[:, 3:6].contiguous(), pot=sums[:, 6].contiguous(),
+    return dict(acc=total[:, 0:3].contiguous(), jerk=total[:, 3:6].contiguous(), pot=total[:, 6].contiguous(),
                 nnb=nnb, nblist=nblist, overflow=overflow)
 
 
