@@ -493,7 +493,20 @@ def run_b200(args):
                      "note": "150 back-to-back nb_block_step calls (h2 = NULL: total force) from a mid-run state; cycle = host "
                              "wall clock between the returns of consecutive calls; force kernel = CUDA events around its "
                              "launch; small = blocks of <= 128 active bodies (fused prediction)"}
+        # NEXT-1: the full-N pass: every body active, counts only (no 2 GiB list), h2 = the block radii
+        h2_full = f64(cfg["h2_all"])
+        fo = dict(acc=torch.empty((N, 3), dtype=torch.float64, device=dev), jerk=torch.empty((N, 3), dtype=torch.float64, device=dev),
+                  pot=torch.empty(N, dtype=torch.float64, device=dev), nnb=torch.empty(N, dtype=torch.int32, device=dev),
+                  overflow=torch.empty(N, dtype=torch.int32, device=dev))
+        ctx.predict_all(t_pred)
+        ms_full = timed(lambda: ctx.regular_all(h2_full, fo["acc"], fo["jerk"], fo["pot"], fo["nnb"], None, fo["overflow"]), reps=2)
+        fullpass = {"N": N, "ms": ms_full, "pairs_per_s": float(N) * N / (ms_full * 1e-3),
+                    "frac_fp32_peak": float(N) * N * FLOP_PER_INTERACTION / (ms_full * 1e-3) / 1e12 / peak_tflops,
+                    "jsplit": ctx.info("last_jsplit"), "reordered": ctx.info("last_reordered"),
+                    "note": "nb_regular_all, nblist = NULL (neighbours counted), includes the Morton sort of the block and finalize"}
+        del fo, h2_full
         extras = {
+            "nb_regular_all": fullpass,
             "nb_block_step": blockstep,
             "nb_irregular": {"n_i": n_i, "neighbour_pairs": nn, "ms": ms_irr, "pairs_per_s": nn / (ms_irr * 1e-3),
                              "gather_GBps": nn * 128 / (ms_irr * 1e-3) / 1e9, "dtype": "f64"},

@@ -884,3 +884,54 @@ def test_morton_reordered_block_equals_callers_order(oracle, k, N, n_i):
     for key, tol in (("acc", 3e-6), ("jerk", 3e-5), ("pot", 3e-7)):       # rows with the same classification of every pair
         a = got[key].reshape(n_i, -1)[same]; b = plain[key].reshape(n_i, -1)[same]
         assert np.max(np.linalg.norm(a - b, axis=1) / np.linalg.norm(b, axis=1)) < tol, key
+
+
+def test_regular_all_at_the_papers_size(oracle):
+    """SURVEY 8(f) NEXT-1 at the size the paper runs it (initialisation of forces and neighbour lists
+    and the O(N^2) potential energy of a million-body run): nb_regular_all at N = 1,048,576 (config 4) with
+    lists on a 2 GiB buffer, 1024 seeded rows against the oracle; then counts only (nblist = NULL) with
+    h2 = 0: W = 1/2 sum m phi against the Plummer closed form -3 pi / 32 G M^2 / a = -0.3843 (config 4's a)."""
+    cfg, ctx, (xp, vp) = _config4(oracle)
+    N, cap = cfg["N"], cfg["cap"]
+    mk = lambda *s, dt=torch.float64: torch.empty(*s, dtype=dt, device="cuda")
+    out = dict(acc=mk(N, 3), jerk=mk(N, 3), pot=mk(N), nnb=mk(N, dt=torch.int32),
+               nblist=torch.empty((N, cap), dtype=torch.int32, device="cuda"), overflow=mk(N, dt=torch.int32))
+    h2_all = _dev(cfg["h2_all"])
+    ctx.regular_all(h2_all, **out)
+    ctx.synchronize()
+    assert ctx.info("last_reordered") == 1
+    sel = np.sort(np.random.default_rng(11).choice(N, 1024, replace=False)).astype(np.int32)
+    sel_d = _dev(sel).long()
+    got = {k: v[sel_d].cpu().numpy() for k, v in out.items()}
+    ref = parity.oracle_reference(oracle, cfg["m"], xp, vp, sel, cfg["h2_all"][sel], cap)
+    rep = parity.compare(got, ref, cap)
+    print("regular_all N=1M sample", rep, "S", ctx.info("last_jsplit"))
+    nnb_all = out["nnb"].cpu().numpy()
+    assert 100 < np.median(nnb_all) < 220          # (halo bodies get radii that hold far more: the median is the target)
+    del out["nblist"]
+    torch.cuda.empty_cache()
+    # potential energy: h2 = 0, counts only
+    ctx.regular_all(_dev(np.zeros(N)), out["acc"], out["jerk"], out["pot"], out["nnb"], None, out["overflow"])
+    ctx.synchronize()
+    assert int(out["nnb"].abs().sum()) == 0
+    m_d = _dev(cfg["m"])
+    W = 0.5 * float((m_d * out["pot"]).sum())
+    f = (m_d[:, None] * out["acc"]).sum(0).cpu().numpy()                       # momentum conservation of the whole pass
+    ftot = float((m_d[:, None] * out["acc"]).abs().sum())
+    tot = oracle.regular(cfg["m"], xp, vp, sel, np.zeros(1024), cap, want_list=False)
+    pg = out["pot"][sel_d].cpu().numpy()
+    assert np.max(np.abs(pg - tot["pot"]) / np.abs(tot["pot"])) < 1e-6
+    a_pl = cfg["a_plummer"]
+    W_plummer = -3.0 * np.pi / 32.0 / a_pl
+    # the generator rejects r > 25 a (SURVEY 8(d) recipe), i.e. samples the model truncated there and renormalised
+    # to M = 1: W_trunc = -(1 / f^2) int_0^25a G M(r) dM(r) / r, f = M(25 a) -- 0.48 % more bound than the infinite sphere
+    r = np.linspace(0.0, 25.0 * a_pl, 2000001)[1:]
+    Mr = r**3 / (r * r + a_pl * a_pl) ** 1.5
+    rho = 3.0 / (4.0 * np.pi * a_pl**3) * (1.0 + r * r / a_pl**2) ** -2.5
+    W_trunc = -np.trapezoid(Mr * rho * 4.0 * np.pi * r, r) / Mr[-1] ** 2
+    print("W", W, "Plummer", W_plummer, "truncated at 25a", W_trunc, "ratio", W / W_trunc,
+          "|sum m a| / sum |m a|", np.abs(f).max() / ftot)
+    assert abs(W_trunc / W_plummer - 1.0048) < 3e-4
+    # finite-N scatter with the Kroupa IMF (a few 100-Msun stars carry ~1e-4 of the mass each): ~0.3 % (1 sigma)
+    assert abs(W / W_trunc - 1.0) < 0.008
+    assert np.abs(f).max() < 1e-6 * ftot
