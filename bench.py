@@ -50,8 +50,9 @@ def parse():
                          "the SAME n_i block (SURVEY 8(f) NEXT-4: state all-reduce, sums / lists all-gather; strong scaling)")
     ap.add_argument("--no-sweep", action="store_true")
     ap.add_argument("--no-extras", action="store_true", help="skip the NEXT-row timings (nb_block_step, nb_irregular, ...)")
-    ap.add_argument("--all-configs", action="store_true",
-                    help="also sweep BASELINE.json configs 3 (N=262144) and 5 (King core, overflowing rows); slower start-up")
+    ap.add_argument("--headline-only", action="store_true",
+                    help="skip the sweeps of BASELINE.json configs 3 (N=262144) and 5 (King core, overflowing rows), "
+                         "which run by default")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -343,16 +344,23 @@ def run_b200(args):
     peak_tflops = sm_count * 128 * 2 * sm_max_mhz * 1e6 / 1e12
     force_ms = force_ns / max(force_cnt, 1) * 1e-6
     ach_tflops = FLOP_PER_INTERACTION * float(n_i) * N / (force_ms * 1e-3) / 1e12
-    traffic = None       # dram__bytes_read.sum + dram__bytes_write.sum of one launch, from the committed ncu capture
+    # dram__bytes_read.sum + dram__bytes_write.sum of one launch: from the committed `ncu --set full` captures
+    # (profiles/force_kernel_traffic.csv, one row per captured launch); the row must match the timed launch
+    # (n_i, N, kernel variant, j-splits) -- otherwise null, never a stale constant
+    traffic, traffic_src = None, None
     tpath = os.path.join(ROOT, "profiles", "force_kernel_traffic.csv")
-    if os.path.exists(tpath) and n_i == 8192 and N == 1048576:
+    if os.path.exists(tpath):
         import csv
         with open(tpath) as f:
-            row = next(csv.DictReader(f))
-        traffic = int(row["dram_bytes_read"]) + int(row["dram_bytes_write"])
+            for row in csv.DictReader(f):
+                if (int(row["n_i"]) == n_i and int(row["N"]) == N and int(row.get("variant", -1)) == plan["variant"]
+                        and int(row.get("jsplit", -1)) == plan["jsplit"]):
+                    traffic = int(row["dram_bytes_read"]) + int(row["dram_bytes_write"])
+                    traffic_src = row["source"]
     roofline = {
         "bound": "alu", "kernel": "nbreg::force_kernel", "achieved": ach_tflops, "peak": peak_tflops,
-        "unit": "TFLOP/s", "frac": ach_tflops / peak_tflops, "traffic": traffic,
+        "unit": "TFLOP/s", "frac": ach_tflops / peak_tflops, "traffic": traffic, "traffic_source": traffic_src,
+        "algorithmic_bytes": 40 * N,
         "flop_per_interaction": FLOP_PER_INTERACTION, "avg_launch_ms": force_ms, "launches_timed": int(force_cnt),
         "interactions_per_launch": float(n_i) * N,
         "peak_how": f"{sm_count} SMs x 128 FP32 lanes x 2 flop x {sm_max_mhz:.0f} MHz (max SM clock; DESIGN.md)",
@@ -412,7 +420,7 @@ def run_b200(args):
     if not args.no_sweep and world == 1:
         sweep = sweep_config(ctx, cfg, [32] + list(cfg["sweep"]), N)   # 32: the j-packed tiny-block variant
     other = None
-    if args.all_configs and world == 1 and N == 1048576:
+    if not args.headline_only and not args.no_sweep and world == 1 and N == 1048576:
         other = {}
         for kcfg in (3, 5):
             ocfg = nbgen.make_config(kcfg)
@@ -512,7 +520,8 @@ def run_b200(args):
                              "gather_GBps": nn * 128 / (ms_irr * 1e-3) / 1e9, "dtype": "f64"},
             "nb_update_j": {"n": n_i, "ms": ms_upd},
             "nb_predict_all": {"ms": ms_pred, "GBps": N * (112 + 40) / (ms_pred * 1e-3) / 1e9,
-                               "frac_hbm": N * (112 + 40) / (ms_pred * 1e-3) / 1e9 / pk.get("hbm_gbs", 6460.0)},
+                               "frac_hbm": N * (112 + 40) / (ms_pred * 1e-3) / 1e9 / pk["hbm_gbs"], "hbm_peak_GBps": pk["hbm_gbs"],
+                               "hbm_peak_source": pk_src},
             "nb_next_block": {"N": N, "ms": ms_sel, "note": "min + count + ordered scatter + 16 B D2H + sync"},
             "nb_correct": {"n": n_i, "ms": ms_cor},
             "nb_set_j": {"ms": ms_setj, "GBps": N * (112 + 112 + 128) / (ms_setj * 1e-3) / 1e9,

@@ -931,7 +931,7 @@ def test_regular_all_at_the_papers_size(oracle):
     W_trunc = -np.trapezoid(Mr * rho * 4.0 * np.pi * r, r) / Mr[-1] ** 2
     print("W", W, "Plummer", W_plummer, "truncated at 25a", W_trunc, "ratio", W / W_trunc,
           "|sum m a| / sum |m a|", np.abs(f).max() / ftot)
-    assert abs(W_trunc / W_plummer - 1.0048) < 3e-4
+    assert abs(W_trunc / W_plummer - 1.0046) < 3e-4
     # finite-N scatter with the Kroupa IMF (a few 100-Msun stars carry ~1e-4 of the mass each): ~0.3 % (1 sigma)
     assert abs(W / W_trunc - 1.0) < 0.008
     assert np.abs(f).max() < 1e-6 * ftot
