@@ -27,11 +27,16 @@
  *     WHICH nb_cap neighbours an overflowed row keeps.
  *
  * Precision of the pair arithmetic (the paper does not state its kernel's precision; DESIGN.md
- * "Precision"): positions are differenced at FP64-equivalent accuracy (two-float hi/lo split,
- * 2^-48 relative), velocities and masses are rounded to FP32, the pair terms are FP32 with an SFU
- * reciprocal square root, sums are FP32 within a j-tile and FP64 across tiles.  Guaranteed against
- * the FP64 definition: acceleration max rel 1e-5 / rms 1e-6, jerk 1e-4 / 1e-5, potential 1e-6;
- * neighbour sets identical except pairs with |r^2 - h^2| / h^2 < 1e-5.
+ * "Precision"): positions are differenced at FP64-equivalent accuracy -- as two-float hi/lo pairs (2^-48
+ * relative), or, for a warp whose 64 active particles lie within G = 8 neighbour radii of their common
+ * centre, in that warp's own FP32 frame (relative error of a difference <= 1.8e-7 + 2.4e-7 G at the
+ * neighbour boundary, translation invariant) --, velocities and masses are rounded to FP32, the pair terms
+ * are FP32 with an SFU reciprocal square root, sums are FP32 within a j-tile and FP64 across tiles.
+ * Guaranteed against the FP64 definition: acceleration max rel 1e-5 / rms 1e-6, jerk 1e-4 / 1e-5,
+ * potential 1e-6; neighbour sets identical except pairs with |r^2 - h^2| / h^2 < 1e-5.
+ * Velocity frame: v is kept as ONE FP32, so a bulk velocity common to all bodies enters the jerk with a
+ * relative error of about 6e-8 |v_bulk| / sigma (sigma = velocity dispersion): the jerk bounds hold for
+ * |v_bulk| <~ 100 sigma.  Integrate a cluster on a galactic orbit in its own frame.
  */
 #ifndef NBREG_H
 #define NBREG_H
