@@ -401,6 +401,15 @@ def run_b200(args):
                 torch.cuda.synchronize()
                 if rep_ >= 3:
                     t_blk.append(a.elapsed_time(b))
+            # the same block cost back to back in the stream (what a block loop sees: no idle-to-launch latency)
+            a, b = (torch.cuda.Event(enable_timing=True) for _ in range(2))
+            n_stream = 20 if n <= 4096 else 4
+            a.record(stream)
+            for _ in range(n_stream):
+                sctx.predict_all(st_pred); sctx.regular(si_d, sh_d, **so)
+            b.record(stream)
+            torch.cuda.synchronize()
+            t_stream = a.elapsed_time(b) / n_stream
             sctx.tune("stats", 1)                         # how many warps differenced in their local frame
             sctx.regular(si_d, sh_d, **so)
             lw, tw = sctx.info("local_warps"), sctx.info("total_warps")
@@ -408,6 +417,7 @@ def run_b200(args):
             best, med = min(t_reg), float(np.median(t_reg))
             rate = float(n) * sN / (best * 1e-3)
             rows.append({"n_i": n, "ms": best, "ms_median": med, "ms_predict_plus_regular": float(np.median(t_blk)),
+                         "ms_predict_plus_regular_in_stream": t_stream,
                          "pairs_per_s": rate, "frac_fp32_peak": rate * FLOP_PER_INTERACTION / 1e12 / peak_tflops,
                          "variant": sctx.info("last_variant"), "jsplit": sctx.info("last_jsplit"),
                          "fused_predict": sctx.info("last_fused"), "reordered": sctx.info("last_reordered"),

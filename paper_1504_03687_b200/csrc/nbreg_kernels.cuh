@@ -418,14 +418,17 @@ __global__ void __launch_bounds__(256) bitonic_global_kernel(int32_t n2, int32_t
 enum { SRC_REC = 0, SRC_STATE = 1 };
 constexpr int STATE_D = 14;                                   // doubles per body of the FP64 state
 constexpr int STATE_TILE_DOUBLES = STATE_D * TJ;              // 28 KB per tile
-template <int SRC> struct SrcCfg;
-template <> struct SrcCfg<SRC_REC> {
+#ifndef NBREG_STATE_NST_JP
+#define NBREG_STATE_NST_JP 3
+#endif
+template <int SRC, bool JP = false> struct SrcCfg;
+template <bool JP> struct SrcCfg<SRC_REC, JP> {
     static constexpr int NST = NSTAGE;                                         // stages in the ring
     static constexpr uint32_t STAGE_BYTES = TILE_FLOATS * sizeof(float);       // 10 KB
     static constexpr int SLICE_COMP = 3;                                       // x', y', z' per j of the warp's share
 };
-template <> struct SrcCfg<SRC_STATE> {
-    static constexpr int NST = 2;
+template <bool JP> struct SrcCfg<SRC_STATE, JP> {
+    static constexpr int NST = JP ? NBREG_STATE_NST_JP : 2;    // 28 KB stages: what two CTAs per SM leave room for
     static constexpr uint32_t STAGE_BYTES = STATE_TILE_DOUBLES * sizeof(double);   // 28 KB
     static constexpr int SLICE_COMP = RECF;                                    // a whole record per j of the warp's share
 };
@@ -620,10 +623,10 @@ __device__ __forceinline__ void tile_pairs(Acc7 &A, const IPair &I, const JPtrs 
 template <int WI, int WJ, bool JP, int SRC>
 struct ForceSmem {
     static constexpr int NW = WI * WJ, NT = 32 * NW, NH = JP ? 1 : 2, SUB = TJ / WJ;
-    static constexpr size_t RING = (size_t)SrcCfg<SRC>::NST * SrcCfg<SRC>::STAGE_BYTES;     // bulk-copy ring
-    static constexpr size_t SLICES = (size_t)NW * SrcCfg<SRC>::SLICE_COMP * SUB * sizeof(float);   // one per warp
+    static constexpr size_t RING = (size_t)SrcCfg<SRC, JP>::NST * SrcCfg<SRC, JP>::STAGE_BYTES;     // bulk-copy ring
+    static constexpr size_t SLICES = (size_t)NW * SrcCfg<SRC, JP>::SLICE_COMP * SUB * sizeof(float);   // one per warp
     static constexpr size_t ACC = (size_t)7 * NH * NT * sizeof(double);                     // FP64 running sums
-    static constexpr size_t BARS = (size_t)SrcCfg<SRC>::NST * (sizeof(uint64_t) + sizeof(int));
+    static constexpr size_t BARS = (size_t)SrcCfg<SRC, JP>::NST * (sizeof(uint64_t) + sizeof(int));
     static constexpr size_t TOTAL = RING + SLICES + ACC + BARS + 64;
     static_assert(WJ == 1 || (size_t)WJ * 7 * 32 * NH * WI * sizeof(double) <= RING + SLICES,
                   "the WJ reduction reuses the ring and the slices");
@@ -658,7 +661,7 @@ __device__ __forceinline__ void predict_from_tile(const double *st, int b, doubl
 template <int WI, int WJ, int MINB, bool JP = false, int SRC = SRC_REC>
 __global__ void __launch_bounds__(32 * WI *WJ, MINB) force_kernel(const ForceParams p) {
     using SM = ForceSmem<WI, WJ, JP, SRC>;
-    using SC = SrcCfg<SRC>;
+    using SC = SrcCfg<SRC, JP>;
     constexpr int NW = SM::NW, NT = SM::NT, NH = SM::NH, SUB = SM::SUB, NST = SC::NST;
     constexpr int IB = 32 * NH * WI;
     constexpr int SLICE = SC::SLICE_COMP * SUB;
@@ -706,7 +709,7 @@ __global__ void __launch_bounds__(32 * WI *WJ, MINB) force_kernel(const ForcePar
                 bulk_g2s(dst + c * TJ, p.soa + (size_t)c * p.Ns + (size_t)tile * TJ, TJ * sizeof(double), &full[s]);
         }
     };
-    if (tid == 0) {     // the first copies fly while the i-state is gathered
+    if (tid == NT - 32) {     // the first copies fly while the i-state is gathered (issued by the last warp: warp 0 gathers)
         for (int s = 0; s < NST && s < ntile; ++s) issue(tile_begin + s, s);
     }
 
