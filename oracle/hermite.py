@@ -82,7 +82,8 @@ def aarseth_step(a1, j1, a2_0, a3, dt, eta):
     dt_req = sqrt( eta (|a||a2| + |j|^2) / (|j||a3| + |a2|^2) )."""
     a2 = a2_0 + np.asarray(dt)[:, None] * a3
     na, nj, n2, n3 = _norm(a1), _norm(j1), _norm(a2), _norm(a3)
-    return np.sqrt(eta * (na * n2 + nj * nj) / (nj * n3 + n2 * n2))
+    with np.errstate(divide="ignore", invalid="ignore"):        # 0/0 (no force at all) -> NaN: handled by quantize_step (R32)
+        return np.sqrt(eta * (na * n2 + nj * nj) / (nj * n3 + n2 * n2))
 
 
 DT_MIN_LEVELS = 40      # reading R32: no step below dt_max * 2^-40
