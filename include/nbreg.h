@@ -55,7 +55,8 @@ enum {
     NB_ESTATE = 2, /* nb_predict_all before nb_set_j, nb_regular before nb_predict_all; also: the
                       current CUDA device is not the one the context was opened on                 */
     NB_ENOMEM = 3, /* device (or staging) allocation failed                                        */
-    NB_ECUDA = 4   /* CUDA error (sticky); nb_last_cuda_error() returns the cudaError_t            */
+    NB_ECUDA = 4,  /* CUDA error (sticky); nb_last_cuda_error() returns the cudaError_t            */
+    NB_EOVERFLOW = 5 /* two-level AC stepping only: a neighbour list overflowed nb_cap (not sticky)  */
 };
 
 /* Create a context for N j-particles and a neighbour-list capacity of nb_cap entries per active
@@ -215,6 +216,41 @@ int nb_block_step(nb_ctx *ctx, const double *h2_all, double eta, double dt_max, 
  * nblist[n][nb_cap] (NB_ESTATE if the step ran without h2_all), overflow[n].  Enqueued on the stream. */
 int nb_get_block(nb_ctx *ctx, int32_t *idx_act, double *acc, double *jerk, double *pot, int32_t *nnb,
                  int32_t *nblist, int32_t *overflow);
+
+/* ---- Two-level Ahmad-Cohen stepping ("the full force of one particle is separated
+ * into two parts: regular and irregular forces ... there are regular (large) time steps and irregular (small)
+ * time steps ... During the irregular step, the regular force and its first order derivative calculated at the
+ * last regular step are used for the particle position and velocity prediction"; P:215 and Table A1: eta_I,
+ * eta_R).  The paper prints no formulas: DESIGN.md readings R33-R38 (the Hermite AC scheme of Makino & Aarseth
+ * 1992).  The library keeps per body the irregular force aI, jI (at its last irregular time, over its list), the
+ * regular force aR, jR (at its last regular time tR), the steps dtI <= dtR and its neighbour list; the j-state
+ * read by the predictor holds the TOTAL a0 = aI + aR + jR (t0 - tR), j0 = jI + jR.
+ *
+ * nb_ac_init: after nb_set_j with every t0[j] = t_start (a0, j0 are ignored and overwritten): full regular pass
+ * with the radii h2_all[N] (DEVICE, copied; squared, indexed by body) -> aR, jR and every list; neighbour force
+ * over the lists -> aI, jI; start-up steps dtR = initial step of the regular force, dtI = min(initial step of the
+ * irregular force, dtR), dtI = dtR for a body without neighbours.  *n_overflow (HOST, may be NULL) = number of
+ * lists longer than nb_cap; if any, returns NB_EOVERFLOW and AC stepping stays unavailable (shrink the radii:
+ * radius control is the caller's, reading R38).  Allocates 6 N vectors + N x nb_cap list entries. */
+int nb_ac_init(nb_ctx *ctx, double t_start, const double *h2_all, double eta_s, double dt_max,
+               int32_t *n_overflow);
+/* One block of the two-level scheme: t_next = min_j (t0_j + dtI_j); the bodies due then take an IRREGULAR step
+ * (neighbour force over their lists at the predicted state, regular force extrapolated linearly, Hermite corrector
+ * over dtI, new dtI with eta_I, never above dtR); those whose regular step is due as well (tR + dtR = t_next)
+ * take a REGULAR step too: regular force with new lists (nb_regular of that sub-block, prediction fused for small
+ * ones), neighbour force over the new lists, regular force w.r.t. the old list = total - irregular(old), the regular
+ * correction a2R dtR^4/24 + a3R dtR^5/120 (v: dtR^3/6, dtR^4/24) added to the corrected state, both polynomials
+ * restarted from the new list, new dtR with eta_R.  HOST outputs *t_next, *n_irr (all active bodies), *n_reg.
+ * If t_next > t_stop nothing happens (*n_irr = 0).  If a new list overflows, NB_EOVERFLOW is returned BEFORE
+ * anything is corrected (*n_reg = number of overflowed rows; the state is untouched).  Blocks without a regular
+ * step cost O(n_irr x neighbours), not O(N).  One host read-back per block (two when regular steps are due). */
+int nb_ac_step(nb_ctx *ctx, double eta_I, double eta_R, double dt_max, double t_stop, double *t_next,
+               int32_t *n_irr, int32_t *n_reg);
+/* Inspection: copies of the AC state into the caller's DEVICE buffers (any may be NULL): the last block's
+ * idx_act[N] / idx_reg[N] (first n_irr / n_reg entries valid), aI, jI, aR, jR [N][3], tR, dtR [N], nnb[N],
+ * nblist[N][nb_cap].  (x0, v0, total a0 / j0, t0 and dtI come from nb_get_state.) */
+int nb_ac_get(nb_ctx *ctx, int32_t *idx_act, int32_t *idx_reg, double *aI, double *jI, double *aR, double *jR,
+              double *tR, double *dtR, int32_t *nnb, int32_t *nblist);
 
 /* Inspection / checkpoint: the stored FP64 state in the caller's layout: m[N], x0[N][3], v0[N][3],
  * a0[N][3], j0[N][3], t0[N] and (optional, may be NULL) the steps dt[N]. */

@@ -7,7 +7,7 @@ from pathlib import Path
 
 from .build import LIB, build_lib
 
-NB_OK, NB_EINVAL, NB_ESTATE, NB_ENOMEM, NB_ECUDA = 0, 1, 2, 3, 4
+NB_OK, NB_EINVAL, NB_ESTATE, NB_ENOMEM, NB_ECUDA, NB_EOVERFLOW = 0, 1, 2, 3, 4, 5
 INFO = dict(kernel_launches=0, last_jsplit=1, last_iblock=2, last_grid=3, sm_count=4, n_padded=5,
             force_jsplit=16, force_variant=17, last_variant=18, profile=19, force_kernel_ns=20,
             force_kernel_count=21, step_chunks=22, fuse_predict=23, local_g_milli=24, stats=25,
@@ -63,6 +63,9 @@ def load_library(build: bool = True) -> ctypes.CDLL:
     lib.nb_get_state.argtypes = [_vp] + [_vp] * 7
     lib.nb_block_step.argtypes = [_vp, _vp, dbl, dbl, dbl, ctypes.POINTER(dbl), ctypes.POINTER(i32)]
     lib.nb_get_block.argtypes = [_vp] + [_vp] * 7
+    lib.nb_ac_init.argtypes = [_vp, dbl, _vp, dbl, dbl, ctypes.POINTER(i32)]
+    lib.nb_ac_step.argtypes = [_vp, dbl, dbl, dbl, dbl, ctypes.POINTER(dbl), ctypes.POINTER(i32), ctypes.POINTER(i32)]
+    lib.nb_ac_get.argtypes = [_vp] + [_vp] * 10
     lib.nb_set_j_offset.argtypes = [_vp, i64]
     lib.nb_regular_shard.argtypes = [_vp, dbl, i32] + [_vp] * 9
     lib.nb_plan_regular.argtypes = [i64, i64, i32, i32] + [ctypes.POINTER(i32)] * 4
@@ -273,6 +276,39 @@ class NbContext:
             ptr = lambda k: _vp(out[k].data_ptr()) if k in out else _vp()
             _check(self._lib.nb_get_block(self._ctx, *(ptr(k) for k in ("idx_act", "acc", "jerk", "pot", "nnb", "nblist",
                                                                           "overflow"))), "nb_get_block", self._ctx)
+        return out
+
+    # -- two-level Ahmad-Cohen stepping
+    def ac_init(self, t_start: float, h2_all, eta_s: float, dt_max: float) -> int:
+        """nb_ac_init -> number of overflowed lists (raises NbregError(NB_EOVERFLOW) if any)."""
+        import torch
+        n = ctypes.c_int32()
+        rc = self._lib.nb_ac_init(self._ctx, float(t_start), _dev_ptr(h2_all, torch.float64, self.N, "h2_all"),
+                                  float(eta_s), float(dt_max), ctypes.byref(n))
+        _check(rc, "nb_ac_init", self._ctx)
+        return n.value
+
+    def ac_step(self, eta_I: float, eta_R: float, dt_max: float, t_stop: float = float("inf")):
+        """nb_ac_step -> (t_next, n_irr, n_reg)."""
+        t, ni, nr = ctypes.c_double(), ctypes.c_int32(), ctypes.c_int32()
+        t_stop = min(float(t_stop), 1.7976931348623157e308)
+        _check(self._lib.nb_ac_step(self._ctx, float(eta_I), float(eta_R), float(dt_max), t_stop, ctypes.byref(t),
+                                    ctypes.byref(ni), ctypes.byref(nr)), "nb_ac_step", self._ctx)
+        return t.value, ni.value, nr.value
+
+    def ac_get(self, with_lists: bool = False) -> dict:
+        import torch
+        N, f8, i4, dev = self.N, torch.float64, torch.int32, "cuda"
+        out = dict(idx_act=torch.empty(N, dtype=i4, device=dev), idx_reg=torch.empty(N, dtype=i4, device=dev),
+                   aI=torch.empty((N, 3), dtype=f8, device=dev), jI=torch.empty((N, 3), dtype=f8, device=dev),
+                   aR=torch.empty((N, 3), dtype=f8, device=dev), jR=torch.empty((N, 3), dtype=f8, device=dev),
+                   tR=torch.empty(N, dtype=f8, device=dev), dtR=torch.empty(N, dtype=f8, device=dev),
+                   nnb=torch.empty(N, dtype=i4, device=dev))
+        if with_lists:
+            out["nblist"] = torch.empty((N, self.cap), dtype=i4, device=dev)
+        ptr = lambda k: _vp(out[k].data_ptr()) if k in out else _vp()
+        _check(self._lib.nb_ac_get(self._ctx, *(ptr(k) for k in ("idx_act", "idx_reg", "aI", "jI", "aR", "jR", "tR", "dtR",
+                                                                  "nnb", "nblist"))), "nb_ac_get", self._ctx)
         return out
 
     def get_state(self, with_steps: bool = True):

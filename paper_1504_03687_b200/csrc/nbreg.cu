@@ -90,6 +90,14 @@ struct nb_ctx {
     double spec_t_stop = 0.0;                       // kernels take {t, n} from this device address
     cudaEvent_t ev_sel = nullptr;
     int64_t blk_stride = 0;                         // acc / jerk / pot of the last block sit at 0, 3, 6 x this in blk_out
+    // two-level AC stepping (nb_ac_init / nb_ac_step): per-body force polynomials, persistent lists, scratch
+    AcState ac = {};
+    double *ac_h2 = nullptr, *ac_aIo = nullptr, *ac_jIo = nullptr;     // radii; irregular force over the old list (by body)
+    int32_t *ac_reg_idx = nullptr, *ac_counts2 = nullptr, *ac_novf = nullptr, *h_ac_novf = nullptr;
+    double *ac_in = nullptr;                                           // new-list irregular force of a block: acc[3n] jerk[3n]
+    int64_t ac_in_n = 0;
+    bool have_ac = false;
+    int ac_grid = 0;
     int64_t spec_hits = 0, spec_misses = 0, blk_prev_n = 0;
     bool spec_enabled = true;                       // NB_TUNE_SPECULATE
     // planning / introspection
@@ -528,6 +536,9 @@ int nb_close(nb_ctx *c) {
     cudaFree(c->sort_keys); cudaFree(c->sort_box);
     cudaFree(c->blk_key); cudaFree(c->blk_idx); cudaFree(c->blk_out); cudaFree(c->blk_nnb); cudaFree(c->blk_ovf);
     cudaFree(c->blk_list);
+    cudaFree(c->ac.aI); cudaFree(c->ac.jI); cudaFree(c->ac.aR); cudaFree(c->ac.jR); cudaFree(c->ac.tR); cudaFree(c->ac.dtR);
+    cudaFree(c->ac.nnb); cudaFree(c->ac.list); cudaFree(c->ac_h2); cudaFree(c->ac_aIo); cudaFree(c->ac_jIo);
+    cudaFree(c->ac_reg_idx); cudaFree(c->ac_counts2); cudaFree(c->ac_novf); cudaFree(c->ac_in); cudaFreeHost(c->h_ac_novf);
     cudaFree(c->partial); cudaFree(c->stage_j);
     cudaFree(c->st_idx); cudaFree(c->st_nnb); cudaFree(c->st_ovf); cudaFree(c->st_list);
     cudaFree(c->st_h2); cudaFree(c->st_out);
@@ -623,7 +634,7 @@ int nb_irregular(nb_ctx *c, double t, int32_t n_i, const int32_t *idx_i, const i
     if (!idx_i || !nnb || !nblist || !acc || !jerk) return NB_EINVAL;
     rc = ensure_aos(c);
     if (rc != NB_OK) return rc;
-    irregular_kernel<false><<<(unsigned)((n_i + 7) / 8), 256, 0, c->stream>>>(n_i, c->cap, t, nullptr, 0.0, idx_i, nnb,
+    irregular_kernel<false><<<(unsigned)((n_i + 7) / 8), 256, 0, c->stream>>>(n_i, c->cap, t, nullptr, 0.0, 0, 0, idx_i, nnb,
                                                                               nblist, c->aos, acc, jerk, pot);
     NB_CUDA(c, cudaGetLastError());
     c->launches += 1;
@@ -888,8 +899,8 @@ int nb_next_block(nb_ctx *c, double *t_next, int32_t *n_act, int32_t *idx_act) {
     if (!c->sel_key) {
         NB_CUDA(c, cudaMalloc(&c->sel_key, sizeof(unsigned long long)));
         NB_CUDA(c, cudaMalloc(&c->sel_counts, sizeof(int32_t) * nchunk));
-        NB_CUDA(c, cudaMalloc(&c->sel_result, sizeof(double) * 2));
-        NB_CUDA(c, cudaMallocHost(&c->h_sel_result, sizeof(double) * 2));
+        NB_CUDA(c, cudaMalloc(&c->sel_result, sizeof(double) * 4));
+        NB_CUDA(c, cudaMallocHost(&c->h_sel_result, sizeof(double) * 4));
     }
     const double *t0 = c->soa + 13 * c->Ns;
     NB_CUDA(c, cudaMemsetAsync(c->sel_key, 0xff, sizeof(unsigned long long), c->stream));
@@ -937,10 +948,10 @@ int nb_block_step(nb_ctx *c, const double *h2_all, double eta, double dt_max, do
         NB_CUDA(c, cudaMemsetAsync(c->blk_key, 0xff, 2 * sizeof(unsigned long long), c->stream));
         NB_CUDA(c, cudaMalloc(&c->blk_idx, sizeof(int32_t) * N));
         if (!c->sel_counts) NB_CUDA(c, cudaMalloc(&c->sel_counts, sizeof(int32_t) * nchunk));
-        if (!c->sel_result) NB_CUDA(c, cudaMalloc(&c->sel_result, sizeof(double) * 2));
-        if (!c->h_sel_result) NB_CUDA(c, cudaMallocHost(&c->h_sel_result, sizeof(double) * 2));
+        if (!c->sel_result) NB_CUDA(c, cudaMalloc(&c->sel_result, sizeof(double) * 4));
+        if (!c->h_sel_result) NB_CUDA(c, cudaMallocHost(&c->h_sel_result, sizeof(double) * 4));
         int per_sm = 0;
-        NB_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, select_block_kernel, 256, 0));
+        NB_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, select_block_kernel<false>, 256, 0));
         c->blk_grid = std::max(1, std::min(nchunk, per_sm * c->sm_count));
     }
     if (!c->ev_sel) NB_CUDA(c, cudaEventCreateWithFlags(&c->ev_sel, cudaEventDisableTiming));
@@ -976,8 +987,10 @@ int nb_block_step(nb_ctx *c, const double *h2_all, double eta, double dt_max, do
         const double *dtj = c->dtj;
         unsigned long long *key = c->blk_key + c->blk_parity, *key_next = c->blk_key + (1 - c->blk_parity);
         int64_t Nn = N;
-        void *args[] = {&Nn, &t0, &dtj, &key, &key_next, &c->sel_counts, &c->blk_idx, &c->sel_result};
-        NB_CUDA(c, cudaLaunchCooperativeKernel((const void *)select_block_kernel, dim3(c->blk_grid), dim3(256), args, 0,
+        const double *nul_d = nullptr;
+        int32_t *nul_i = nullptr;
+        void *args[] = {&Nn, &t0, &dtj, &key, &key_next, &c->sel_counts, &c->blk_idx, &c->sel_result, &nul_d, &nul_d, &nul_i, &nul_i};
+        NB_CUDA(c, cudaLaunchCooperativeKernel((const void *)select_block_kernel<false>, dim3(c->blk_grid), dim3(256), args, 0,
                                                c->stream));
         c->blk_parity ^= 1;
         c->launches += 1;
@@ -1001,7 +1014,7 @@ int nb_block_step(nb_ctx *c, const double *h2_all, double eta, double dt_max, do
             rc2 = regular_device(c, n, c->blk_idx, h2_all, acc, jerk, pot, c->blk_nnb, h2_all ? c->blk_list : nullptr, c->blk_ovf);
         c->h2_by_body = 0;
         if (rc2 == NB_OK && h2_all) {   // the neighbour force on the lists just written, added in place
-            irregular_kernel<true><<<(unsigned)((n + 7) / 8), 256, 0, c->stream>>>(n, c->cap, t, c->spec_dev, t_stop, c->blk_idx,
+            irregular_kernel<true><<<(unsigned)((n + 7) / 8), 256, 0, c->stream>>>(n, c->cap, t, c->spec_dev, t_stop, 0, 0, c->blk_idx,
                                                                                     c->blk_nnb, c->blk_list, c->aos, acc, jerk, pot);
             c->launches += 1;
         }
@@ -1044,6 +1057,179 @@ int nb_block_step(nb_ctx *c, const double *h2_all, double eta, double dt_max, do
     c->blk_last_n = n;
     c->blk_had_list = h2_all != nullptr;
     *n_act = n;
+    return NB_OK;
+}
+
+int nb_ac_init(nb_ctx *c, double t_start, const double *h2_all, double eta_s, double dt_max, int32_t *n_overflow) {
+    int rc = check_live(c);
+    if (rc != NB_OK) return rc;
+    if (!h2_all || !(eta_s > 0.0) || !(dt_max > 0.0)) return NB_EINVAL;
+    if (!c->have_j) return NB_ESTATE;
+    if (c->j_offset != 0) return NB_ESTATE;
+    const int64_t N = c->N;
+    const int nchunk = (int)((N + SEL_CHUNK - 1) / SEL_CHUNK);
+    if (!c->ac.aI) {
+        const size_t v3 = sizeof(double) * 3 * N;
+        NB_CUDA(c, cudaMalloc(&c->ac.aI, v3)); NB_CUDA(c, cudaMalloc(&c->ac.jI, v3));
+        NB_CUDA(c, cudaMalloc(&c->ac.aR, v3)); NB_CUDA(c, cudaMalloc(&c->ac.jR, v3));
+        NB_CUDA(c, cudaMalloc(&c->ac_aIo, v3)); NB_CUDA(c, cudaMalloc(&c->ac_jIo, v3));
+        NB_CUDA(c, cudaMalloc(&c->ac.tR, sizeof(double) * N)); NB_CUDA(c, cudaMalloc(&c->ac.dtR, sizeof(double) * N));
+        NB_CUDA(c, cudaMalloc(&c->ac_h2, sizeof(double) * N));
+        NB_CUDA(c, cudaMalloc(&c->ac.nnb, sizeof(int32_t) * N));
+        NB_CUDA(c, cudaMalloc(&c->ac.list, sizeof(int32_t) * N * c->cap));
+        NB_CUDA(c, cudaMalloc(&c->ac_reg_idx, sizeof(int32_t) * N));
+        NB_CUDA(c, cudaMalloc(&c->ac_counts2, sizeof(int32_t) * nchunk));
+        NB_CUDA(c, cudaMalloc(&c->ac_novf, sizeof(int32_t)));
+        NB_CUDA(c, cudaMallocHost(&c->h_ac_novf, sizeof(int32_t)));
+        if (!c->dtj) NB_CUDA(c, cudaMalloc(&c->dtj, sizeof(double) * N));
+        if (!c->blk_key) {
+            NB_CUDA(c, cudaMalloc(&c->blk_key, 2 * sizeof(unsigned long long)));
+            NB_CUDA(c, cudaMemsetAsync(c->blk_key, 0xff, 2 * sizeof(unsigned long long), c->stream));
+            NB_CUDA(c, cudaMalloc(&c->blk_idx, sizeof(int32_t) * N));
+        }
+        if (!c->sel_counts) NB_CUDA(c, cudaMalloc(&c->sel_counts, sizeof(int32_t) * nchunk));
+        if (!c->sel_result) NB_CUDA(c, cudaMalloc(&c->sel_result, sizeof(double) * 4));
+        if (!c->h_sel_result) NB_CUDA(c, cudaMallocHost(&c->h_sel_result, sizeof(double) * 4));
+        int per_sm = 0;
+        NB_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, select_block_kernel<true>, 256, 0));
+        c->ac_grid = std::max(1, std::min(nchunk, per_sm * c->sm_count));
+        if (!c->ev_sel) NB_CUDA(c, cudaEventCreateWithFlags(&c->ev_sel, cudaEventDisableTiming));
+    }
+    NB_CUDA(c, cudaMemcpyAsync(c->ac_h2, h2_all, sizeof(double) * N, cudaMemcpyDeviceToDevice, c->stream));
+    // forces at t_start: every t0[j] must equal t_start, so the prediction is the state itself
+    c->have_pred = true; c->pred_pending = true; c->pred_t = t_start;
+    rc = ensure_aos(c);
+    if (rc != NB_OK) return rc;
+    int32_t *ovf_all = c->ac_reg_idx;               // scratch: free until the first step
+    rc = regular_device(c, (int32_t)N, nullptr, c->ac_h2, c->ac.aR, c->ac.jR, c->ac_aIo /* pot: scratch */, c->ac.nnb,
+                        c->ac.list, ovf_all);
+    if (rc != NB_OK) return rc;
+    irregular_kernel<false><<<(unsigned)((N + 7) / 8), 256, 0, c->stream>>>((int32_t)N, c->cap, t_start, nullptr, 0.0, 0, 0, nullptr,
+                                                                            c->ac.nnb, c->ac.list, c->aos, c->ac.aI, c->ac.jI, nullptr);
+    NB_CUDA(c, cudaMemsetAsync(c->ac_novf, 0, sizeof(int32_t), c->stream));
+    ac_start_kernel<<<(unsigned)((N + 127) / 128), 128, 0, c->stream>>>(N, c->Ns, c->cap, t_start, eta_s, dt_max, c->ac, c->soa,
+                                                                        c->aos, c->dtj, c->ac_novf);
+    NB_CUDA(c, cudaGetLastError());
+    c->launches += 2;
+    NB_CUDA(c, cudaMemcpyAsync(c->h_ac_novf, c->ac_novf, sizeof(int32_t), cudaMemcpyDeviceToHost, c->stream));
+    NB_CUDA(c, cudaStreamSynchronize(c->stream));
+    c->have_pred = false; c->pred_pending = false;
+    c->have_steps = true;
+    if (n_overflow) *n_overflow = *c->h_ac_novf;
+    c->have_ac = *c->h_ac_novf == 0;
+    return c->have_ac ? NB_OK : NB_EOVERFLOW;
+}
+
+int nb_ac_step(nb_ctx *c, double eta_I, double eta_R, double dt_max, double t_stop, double *t_next, int32_t *n_irr,
+               int32_t *n_reg) {
+    int rc = check_live(c);
+    if (rc != NB_OK) return rc;
+    if (!t_next || !n_irr || !n_reg || !(eta_I > 0.0) || !(eta_R > 0.0) || !(dt_max > 0.0)) return NB_EINVAL;
+    if (!c->have_ac) return NB_ESTATE;
+    const int64_t N = c->N;
+    {   // selection: active = irregular step due; among them the bodies whose regular step is due too
+        const double *t0 = c->soa + 13 * c->Ns;
+        const double *dtj = c->dtj, *tR = c->ac.tR, *dtR = c->ac.dtR;
+        unsigned long long *key = c->blk_key + c->blk_parity, *key_next = c->blk_key + (1 - c->blk_parity);
+        int64_t Nn = N;
+        void *args[] = {&Nn, &t0, &dtj, &key, &key_next, &c->sel_counts, &c->blk_idx, &c->sel_result, &tR, &dtR,
+                        &c->ac_counts2, &c->ac_reg_idx};
+        NB_CUDA(c, cudaLaunchCooperativeKernel((const void *)select_block_kernel<true>, dim3(c->ac_grid), dim3(256), args, 0,
+                                               c->stream));
+        c->blk_parity ^= 1;
+        c->launches += 1;
+        NB_CUDA(c, cudaMemcpyAsync(c->h_sel_result, c->sel_result, sizeof(double) * 3, cudaMemcpyDeviceToHost, c->stream));
+        NB_CUDA(c, cudaStreamSynchronize(c->stream));
+    }
+    const double t = c->h_sel_result[0];
+    const int32_t n = (int32_t)c->h_sel_result[1], nr = (int32_t)c->h_sel_result[2];
+    *t_next = t; *n_irr = 0; *n_reg = 0;
+    c->blk_last_n = 0;
+    if (t > t_stop || n <= 0) return NB_OK;
+    // irregular force over the OLD lists of every active body (rows and outputs by body)
+    irregular_kernel<false><<<(unsigned)((n + 7) / 8), 256, 0, c->stream>>>(n, c->cap, t, nullptr, 0.0, 1, 1, c->blk_idx, c->ac.nnb,
+                                                                            c->ac.list, c->aos, c->ac_aIo, c->ac_jIo, nullptr);
+    c->launches += 1;
+    double *rg_acc = nullptr, *rg_jerk = nullptr, *in_acc = nullptr, *in_jerk = nullptr;
+    if (nr > 0) {
+        // block buffers for the regular-active bodies: regular force / lists (new), irregular force over the new lists
+        if (nr > c->blk_n) {
+            cudaFree(c->blk_out); cudaFree(c->blk_nnb); cudaFree(c->blk_ovf);
+            c->blk_out = nullptr; c->blk_nnb = c->blk_ovf = nullptr; c->blk_n = 0;
+            const int64_t m = std::min<int64_t>(std::max<int64_t>(N, 1024), std::max<int64_t>(nr, 1024) * 5 / 4);
+            NB_CUDA(c, cudaMalloc(&c->blk_out, sizeof(double) * 7 * m));
+            NB_CUDA(c, cudaMalloc(&c->blk_nnb, sizeof(int32_t) * m));
+            NB_CUDA(c, cudaMalloc(&c->blk_ovf, sizeof(int32_t) * m));
+            c->blk_n = m;
+        }
+        if ((int64_t)nr * c->cap > c->blk_list_n) {
+            cudaFree(c->blk_list); c->blk_list = nullptr; c->blk_list_n = 0;
+            const int64_t m = std::min<int64_t>(std::max<int64_t>(N, 1024), std::max<int64_t>(nr, 1024) * 5 / 4) * c->cap;
+            NB_CUDA(c, cudaMalloc(&c->blk_list, sizeof(int32_t) * m));
+            c->blk_list_n = m;
+        }
+        if (nr > c->ac_in_n) {
+            cudaFree(c->ac_in); c->ac_in = nullptr; c->ac_in_n = 0;
+            const int64_t m = std::min<int64_t>(std::max<int64_t>(N, 1024), std::max<int64_t>(nr, 1024) * 5 / 4);
+            NB_CUDA(c, cudaMalloc(&c->ac_in, sizeof(double) * 6 * m));
+            c->ac_in_n = m;
+        }
+        rg_acc = c->blk_out; rg_jerk = c->blk_out + 3 * (int64_t)nr;
+        double *rg_pot = c->blk_out + 6 * (int64_t)nr;
+        in_acc = c->ac_in; in_jerk = c->ac_in + 3 * (int64_t)nr;
+        c->have_pred = true; c->pred_pending = true; c->pred_t = t;
+        if (!c->fuse) {
+            rc = materialize_pred(c);
+            if (rc != NB_OK) return rc;
+        }
+        c->h2_by_body = 1;
+        rc = regular_device(c, nr, c->ac_reg_idx, c->ac_h2, rg_acc, rg_jerk, rg_pot, c->blk_nnb, c->blk_list, c->blk_ovf);
+        c->h2_by_body = 0;
+        if (rc != NB_OK) return rc;
+        irregular_kernel<false><<<(unsigned)((nr + 7) / 8), 256, 0, c->stream>>>(nr, c->cap, t, nullptr, 0.0, 0, 0, c->ac_reg_idx,
+                                                                                 c->blk_nnb, c->blk_list, c->aos, in_acc, in_jerk, nullptr);
+        // a list that overflowed would break regular + irregular = total (R38): checked BEFORE anything is corrected
+        NB_CUDA(c, cudaMemsetAsync(c->ac_novf, 0, sizeof(int32_t), c->stream));
+        count_overflow_kernel<<<(unsigned)std::min<int64_t>((nr + 255) / 256, 1024), 256, 0, c->stream>>>(nr, c->blk_ovf, c->ac_novf);
+        NB_CUDA(c, cudaMemcpyAsync(c->h_ac_novf, c->ac_novf, sizeof(int32_t), cudaMemcpyDeviceToHost, c->stream));
+        NB_CUDA(c, cudaStreamSynchronize(c->stream));
+        c->launches += 2;
+        c->have_pred = false; c->pred_pending = false;
+        if (*c->h_ac_novf > 0) {
+            *n_reg = *c->h_ac_novf;                 // the number of overflowed rows; the state is untouched
+            return NB_EOVERFLOW;
+        }
+    }
+    ac_correct_kernel<<<(unsigned)((n + 127) / 128), 128, 0, c->stream>>>(n, c->Ns, t, eta_I, eta_R, dt_max, c->blk_idx, c->ac_aIo,
+                                                                          c->ac_jIo, nr, c->ac_reg_idx, rg_acc, rg_jerk, in_acc,
+                                                                          in_jerk, c->blk_nnb, c->ac, c->soa, c->aos, c->dtj);
+    if (nr > 0)
+        ac_store_rows_kernel<<<(unsigned)((nr + 7) / 8), 256, 0, c->stream>>>(nr, c->cap, c->ac_reg_idx, c->blk_nnb, c->blk_list,
+                                                                              c->ac.list);
+    NB_CUDA(c, cudaGetLastError());
+    c->launches += nr > 0 ? 2 : 1;
+    c->have_pred = false; c->pred_pending = false;
+    *n_irr = n; *n_reg = nr;
+    return NB_OK;
+}
+
+int nb_ac_get(nb_ctx *c, int32_t *idx_act, int32_t *idx_reg, double *aI, double *jI, double *aR, double *jR, double *tR,
+              double *dtR, int32_t *nnb, int32_t *nblist) {
+    int rc = check_live(c);
+    if (rc != NB_OK) return rc;
+    if (!c->ac.aI) return NB_ESTATE;
+    const int64_t N = c->N;
+    const cudaMemcpyKind dd = cudaMemcpyDeviceToDevice;
+    if (idx_act) NB_CUDA(c, cudaMemcpyAsync(idx_act, c->blk_idx, sizeof(int32_t) * N, dd, c->stream));
+    if (idx_reg) NB_CUDA(c, cudaMemcpyAsync(idx_reg, c->ac_reg_idx, sizeof(int32_t) * N, dd, c->stream));
+    if (aI) NB_CUDA(c, cudaMemcpyAsync(aI, c->ac.aI, sizeof(double) * 3 * N, dd, c->stream));
+    if (jI) NB_CUDA(c, cudaMemcpyAsync(jI, c->ac.jI, sizeof(double) * 3 * N, dd, c->stream));
+    if (aR) NB_CUDA(c, cudaMemcpyAsync(aR, c->ac.aR, sizeof(double) * 3 * N, dd, c->stream));
+    if (jR) NB_CUDA(c, cudaMemcpyAsync(jR, c->ac.jR, sizeof(double) * 3 * N, dd, c->stream));
+    if (tR) NB_CUDA(c, cudaMemcpyAsync(tR, c->ac.tR, sizeof(double) * N, dd, c->stream));
+    if (dtR) NB_CUDA(c, cudaMemcpyAsync(dtR, c->ac.dtR, sizeof(double) * N, dd, c->stream));
+    if (nnb) NB_CUDA(c, cudaMemcpyAsync(nnb, c->ac.nnb, sizeof(int32_t) * N, dd, c->stream));
+    if (nblist) NB_CUDA(c, cudaMemcpyAsync(nblist, c->ac.list, sizeof(int32_t) * N * c->cap, dd, c->stream));
     return NB_OK;
 }
 
@@ -1289,6 +1475,7 @@ const char *nb_strerror(int code) {
         case NB_ESTATE: return "call out of order (set_j -> predict_all -> regular)";
         case NB_ENOMEM: return "out of device memory";
         case NB_ECUDA: return "CUDA error or no sm_100 device (see nb_last_cuda_error)";
+        case NB_EOVERFLOW: return "neighbour list overflow during two-level AC stepping (shrink the radii)";
         default: return "unknown nbreg status";
     }
 }

@@ -1130,9 +1130,12 @@ __device__ __forceinline__ BodyD predict_body(const double *__restrict__ aos, in
 }
 
 // ACCUM: add to acc / jerk / pot instead of overwriting them (nb_block_step: regular + irregular = total).
+// idx_i = NULL: the identity block.  rows_by_body / out_by_body: the list rows (and nnb) / the outputs are
+// indexed by BODY (the persistent lists and scratch of the two-level AC stepping) instead of by k.
 template <bool ACCUM>
 __global__ void __launch_bounds__(256) irregular_kernel(int32_t n_i, int32_t cap, double t,
                                                         const double *__restrict__ blk_dev, double t_stop,
+                                                        int32_t rows_by_body, int32_t out_by_body,
                                                         const int32_t *__restrict__ idx_i,
                                                         const int32_t *__restrict__ nnb,
                                                         const int32_t *__restrict__ nblist,
@@ -1142,10 +1145,11 @@ __global__ void __launch_bounds__(256) irregular_kernel(int32_t n_i, int32_t cap
     const int k = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     if (!spec_block(blk_dev, t_stop, n_i, t)) return;
     if (k >= n_i) return;
-    const int32_t i = idx_i[k];
+    const int32_t i = idx_i ? idx_i[k] : k;
     const BodyD I = predict_body(aos, i, t);
-    const int cnt = min(nnb[k], cap);
-    const int32_t *row = nblist + (int64_t)k * cap;
+    const int64_t kr = rows_by_body ? i : k, ko = out_by_body ? i : k;
+    const int cnt = min(nnb[kr], cap);
+    const int32_t *row = nblist + kr * cap;
     double s[7];
 #pragma unroll
     for (int q = 0; q < 7; ++q) s[q] = 0.0;
@@ -1175,12 +1179,12 @@ __global__ void __launch_bounds__(256) irregular_kernel(int32_t n_i, int32_t cap
     if (lane == 0) {
         if (ACCUM) {
 #pragma unroll
-            for (int q = 0; q < 3; ++q) { acc[3 * k + q] += s[q]; jerk[3 * k + q] += s[3 + q]; }
-            if (pot) pot[k] += s[6];
+            for (int q = 0; q < 3; ++q) { acc[3 * ko + q] += s[q]; jerk[3 * ko + q] += s[3 + q]; }
+            if (pot) pot[ko] += s[6];
         } else {
-            acc[3 * k + 0] = s[0]; acc[3 * k + 1] = s[1]; acc[3 * k + 2] = s[2];
-            jerk[3 * k + 0] = s[3]; jerk[3 * k + 1] = s[4]; jerk[3 * k + 2] = s[5];
-            if (pot) pot[k] = s[6];
+            acc[3 * ko + 0] = s[0]; acc[3 * ko + 1] = s[1]; acc[3 * ko + 2] = s[2];
+            jerk[3 * ko + 0] = s[3]; jerk[3 * ko + 1] = s[4]; jerk[3 * ko + 2] = s[5];
+            if (pot) pot[ko] = s[6];
         }
     }
 }
@@ -1281,17 +1285,22 @@ __global__ void __launch_bounds__(256) select_active_kernel(int64_t N, const dou
 // The same selection as ONE cooperative launch (nb_block_step): grid-stride over the 2048-body chunks,
 // grid.sync() between the three phases; `key` is this call's minimum slot (~0 on entry), `key_next` the
 // other slot, reset here for the next call.  result = {t_next, n_active}.
+// TWO (two-level AC stepping): among the active bodies those whose REGULAR step is due as well
+// (tR_j + dtR_j == t_next) are also listed, ascending, in idx_reg; result[2] = their number.
+template <bool TWO>
 __global__ void __launch_bounds__(256) select_block_kernel(int64_t N, const double *__restrict__ t0,
                                                            const double *__restrict__ dtj, unsigned long long *key,
                                                            unsigned long long *key_next, int32_t *__restrict__ counts,
-                                                           int32_t *__restrict__ idx_act, double *__restrict__ result) {
+                                                           int32_t *__restrict__ idx_act, double *__restrict__ result,
+                                                           const double *__restrict__ tR, const double *__restrict__ dtR,
+                                                           int32_t *__restrict__ counts2, int32_t *__restrict__ idx_reg) {
     namespace cg = cooperative_groups;
     cg::grid_group grid = cg::this_grid();
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     const int nchunk = (int)((N + SEL_CHUNK - 1) / SEL_CHUNK);
     __shared__ unsigned long long wbest[8];
-    __shared__ int32_t wsum[8];
-    __shared__ int32_t base_s;
+    __shared__ int32_t wsum[8], wsum2[8];
+    __shared__ int32_t base_s, base2_s;
     // ---- phase 1: t_next = min_j (t0_j + dt_j).  The CTA's FIRST chunk stays in registers for the other two
     //      phases (at N <= grid x 2048 that is everything: one pass over memory instead of three).
     constexpr int PER = SEL_CHUNK / 256;
@@ -1322,68 +1331,80 @@ __global__ void __launch_bounds__(256) select_block_kernel(int64_t N, const doub
     const double tn = key_to_double(*key);
     // ---- phase 2: active bodies per chunk
     for (int b = blockIdx.x; b < nchunk; b += gridDim.x) {
-        int32_t cntc = 0;
-        if (b == (int)blockIdx.x) {
+        int32_t cntc = 0, cnt2 = 0;
 #pragma unroll
-            for (int u = 0; u < PER; ++u) cntc += first[u] == tn ? 1 : 0;
-        } else {
-            for (int s = 0; s < SEL_CHUNK; s += 256) {
-                const int64_t j = (int64_t)b * SEL_CHUNK + s + threadIdx.x;
-                cntc += (j < N && (t0[j] + dtj[j] == tn)) ? 1 : 0;
-            }
+        for (int u = 0; u < PER; ++u) {
+            const int64_t j = (int64_t)b * SEL_CHUNK + u * 256 + threadIdx.x;
+            const bool act = b == (int)blockIdx.x ? first[u] == tn : (j < N && (t0[j] + dtj[j] == tn));
+            cntc += act ? 1 : 0;
+            if (TWO) cnt2 += (act && tR[j] + dtR[j] == tn) ? 1 : 0;
         }
 #pragma unroll
-        for (int off = 16; off > 0; off >>= 1) cntc += __shfl_xor_sync(0xffffffffu, cntc, off);
+        for (int off = 16; off > 0; off >>= 1) {
+            cntc += __shfl_xor_sync(0xffffffffu, cntc, off);
+            if (TWO) cnt2 += __shfl_xor_sync(0xffffffffu, cnt2, off);
+        }
         __syncthreads();
-        if (lane == 0) wsum[w] = cntc;
+        if (lane == 0) { wsum[w] = cntc; wsum2[w] = cnt2; }
         __syncthreads();
         if (threadIdx.x == 0) {
-            int32_t tsum = 0;
+            int32_t tsum = 0, tsum2 = 0;
 #pragma unroll
-            for (int q = 0; q < 8; ++q) tsum += wsum[q];
+            for (int q = 0; q < 8; ++q) { tsum += wsum[q]; tsum2 += wsum2[q]; }
             counts[b] = tsum;
+            if (TWO) counts2[b] = tsum2;
         }
     }
     grid.sync();
     // ---- phase 3: ordered compaction (ascending indices)
     for (int b = blockIdx.x; b < nchunk; b += gridDim.x) {
-        int32_t part = 0;
-        for (int q = threadIdx.x; q < b; q += 256) part += counts[q];
+        int32_t part = 0, part2 = 0;
+        for (int q = threadIdx.x; q < b; q += 256) { part += counts[q]; if (TWO) part2 += counts2[q]; }
 #pragma unroll
-        for (int off = 16; off > 0; off >>= 1) part += __shfl_xor_sync(0xffffffffu, part, off);
-        __syncthreads();
-        if (lane == 0) wsum[w] = part;
-        __syncthreads();
-        if (threadIdx.x == 0) {
-            int32_t tsum = 0;
-#pragma unroll
-            for (int q = 0; q < 8; ++q) tsum += wsum[q];
-            base_s = tsum;
+        for (int off = 16; off > 0; off >>= 1) {
+            part += __shfl_xor_sync(0xffffffffu, part, off);
+            if (TWO) part2 += __shfl_xor_sync(0xffffffffu, part2, off);
         }
         __syncthreads();
-        int32_t running = base_s;
+        if (lane == 0) { wsum[w] = part; wsum2[w] = part2; }
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            int32_t tsum = 0, tsum2 = 0;
+#pragma unroll
+            for (int q = 0; q < 8; ++q) { tsum += wsum[q]; tsum2 += wsum2[q]; }
+            base_s = tsum; base2_s = tsum2;
+        }
+        __syncthreads();
+        int32_t running = base_s, running2 = base2_s;
 #pragma unroll
         for (int u = 0; u < PER; ++u) {
             const int s = u * 256;
             const int64_t j = (int64_t)b * SEL_CHUNK + s + threadIdx.x;
             const bool act = b == (int)blockIdx.x ? first[u] == tn : (j < N && (t0[j] + dtj[j] == tn));
+            const bool due = TWO && act && (tR[j] + dtR[j] == tn);
             const unsigned bal = __ballot_sync(0xffffffffu, act);
+            const unsigned bal2 = __ballot_sync(0xffffffffu, due);
             __syncthreads();
-            if (lane == 0) wsum[w] = __popc(bal);
+            if (lane == 0) { wsum[w] = __popc(bal); wsum2[w] = __popc(bal2); }
             __syncthreads();
-            int32_t before = 0, slab = 0;
+            int32_t before = 0, slab = 0, before2 = 0, slab2 = 0;
 #pragma unroll
             for (int q = 0; q < 8; ++q) {
-                const int32_t cq = wsum[q];
+                const int32_t cq = wsum[q], cq2 = wsum2[q];
                 before += q < w ? cq : 0;
                 slab += cq;
+                before2 += q < w ? cq2 : 0;
+                slab2 += cq2;
             }
             if (act) idx_act[running + before + __popc(bal & ((1u << lane) - 1u))] = (int32_t)j;
+            if (due) idx_reg[running2 + before2 + __popc(bal2 & ((1u << lane) - 1u))] = (int32_t)j;
             running += slab;
+            running2 += slab2;
         }
         if (b == nchunk - 1 && threadIdx.x == 0) {
             result[0] = tn;
             result[1] = (double)running;
+            if (TWO) result[2] = (double)running2;
         }
         __syncthreads();
     }
@@ -1455,6 +1476,164 @@ __global__ void __launch_bounds__(128) correct_kernel(int32_t n, int64_t Ns, dou
     }
     store_body(i, Ns, m, x1, v1, a1, j1, t1, soa, aos);
     dtj[i] = d;
+}
+
+// ------------------------------------------------------------------ NEXT-3: two-level Ahmad-Cohen stepping
+// (regular force from outside the neighbour radius on large steps, irregular force from the neighbours on
+// small steps, the regular force and its first derivative extrapolated in between; readings R33-R38.)
+struct AcState {
+    double *aI, *jI, *aR, *jR;        // [N][3] irregular force at t0 over the body's list; regular force at tR
+    double *tR, *dtR;                 // [N] last regular time, regular step (the irregular step is dtj)
+    int32_t *nnb, *list;              // [N], [N][cap] the body's neighbour list (from its last regular step)
+};
+__device__ __forceinline__ double aarseth_req(const double *a, const double *j, const double *a2e, const double *a3,
+                                              double eta) {
+    const double na = norm3(a), nj = norm3(j), n2 = norm3(a2e), n3 = norm3(a3);
+    return sqrt(eta * (na * n2 + nj * nj) / (nj * n3 + n2 * n2));
+}
+// Block rule (readings R29, R32): candidate d; doubled once if allowed, else halved while above req.
+__device__ __forceinline__ double block_rule(double req, double d, double t1, double dt_max) {
+    if (req > 0.0) {
+        const double d2 = 2.0 * d, ratio = t1 / d2, dmin = dt_max * DT_MIN_FACTOR;
+        if (req >= d2 && d2 <= dt_max && ratio == floor(ratio)) d = d2;
+        else
+            while (d > req && d > dmin) d *= 0.5;
+    }
+    return d;
+}
+
+// Start-up (R37): forces are in place (aR, jR, lists from the full regular pass; aI, jI over those lists);
+// writes the total a0, j0 into the stored state and the two steps; counts overflowed lists (R38).
+__global__ void __launch_bounds__(128) ac_start_kernel(int64_t N, int64_t Ns, int32_t cap, double t_start, double eta_s,
+                                                       double dt_max, const AcState A, double *__restrict__ soa,
+                                                       double *__restrict__ aos, double *__restrict__ dtj,
+                                                       int32_t *__restrict__ n_overflow) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const double2 *p = reinterpret_cast<const double2 *>(aos + i * AOS_D);
+    const double2 q0 = p[0], q1 = p[1], q2 = p[2], q3 = p[3];
+    const double x0[3] = {q0.y, q1.x, q1.y}, v0[3] = {q2.x, q2.y, q3.x};
+    double aI[3], jI[3], aR[3], jR[3], a0[3], j0[3];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        aI[c] = A.aI[3 * i + c]; jI[c] = A.jI[3 * i + c]; aR[c] = A.aR[3 * i + c]; jR[c] = A.jR[3 * i + c];
+        a0[c] = aI[c] + aR[c]; j0[c] = jI[c] + jR[c];
+    }
+    auto init_step = [&](const double *a, const double *j) {
+        double req = eta_s * norm3(a) / norm3(j);
+        if (req != req) req = dt_max;
+        return pow2_floor(fmin(fmax(req, dt_max * DT_MIN_FACTOR), dt_max));
+    };
+    const double dR = init_step(aR, jR);
+    const int32_t nn = A.nnb[i];
+    const double dI = nn == 0 ? dR : fmin(init_step(aI, jI), dR);
+    if (nn > cap) atomicAdd(n_overflow, 1);
+    store_body(i, Ns, q0.x, x0, v0, a0, j0, t_start, soa, aos);
+    A.tR[i] = t_start; A.dtR[i] = dR; dtj[i] = dI;
+}
+
+// Both correctors for the n irregular-active bodies idx[0..n) at time t (R34, R35).  aIo / jIo: irregular
+// force over the OLD list, indexed by body.  A body whose regular step is due as well (tR + dtR == t) finds
+// its slot r in the ascending idx_reg[0..n_reg) and there the new-list forces: regular rg_acc/rg_jerk[r],
+// irregular in_acc/in_jerk[r], new count rg_nnb[r] (rows are copied by ac_store_rows_kernel afterwards).
+__global__ void __launch_bounds__(128) ac_correct_kernel(int32_t n, int64_t Ns, double t, double eta_I, double eta_R,
+                                                         double dt_max, const int32_t *__restrict__ idx,
+                                                         const double *__restrict__ aIo, const double *__restrict__ jIo,
+                                                         int32_t n_reg, const int32_t *__restrict__ idx_reg,
+                                                         const double *__restrict__ rg_acc, const double *__restrict__ rg_jerk,
+                                                         const double *__restrict__ in_acc, const double *__restrict__ in_jerk,
+                                                         const int32_t *__restrict__ rg_nnb, const AcState A,
+                                                         double *__restrict__ soa, double *__restrict__ aos,
+                                                         double *__restrict__ dtj) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= n) return;
+    const int64_t i = idx[k];
+    const double2 *p = reinterpret_cast<const double2 *>(aos + i * AOS_D);
+    const double2 q0 = p[0], q1 = p[1], q2 = p[2], q3 = p[3], q4 = p[4], q5 = p[5], q6 = p[6];
+    const double m = q0.x;
+    const double x0[3] = {q0.y, q1.x, q1.y}, v0[3] = {q2.x, q2.y, q3.x}, a0[3] = {q3.y, q4.x, q4.y};
+    const double j0[3] = {q5.x, q5.y, q6.x};
+    const double h = dtj[i];                                   // = t - t0: the irregular step
+    const double tR = A.tR[i], hR = A.dtR[i];
+    const bool due = tR + hR == t;
+    const double h2 = h * h, h3 = h2 * h, h4 = h2 * h2, h5 = h4 * h;
+    double x1[3], v1[3], a1[3], j1[3], a2e[3], a3[3], aI1[3], jI1[3], aR0[3], jR0[3];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        aI1[c] = aIo[3 * i + c]; jI1[c] = jIo[3 * i + c];
+        aR0[c] = A.aR[3 * i + c]; jR0[c] = A.jR[3 * i + c];
+        a1[c] = aI1[c] + (aR0[c] + jR0[c] * (t - tR));         // regular force extrapolated
+        j1[c] = jI1[c] + jR0[c];
+        const double da = a0[c] - a1[c];
+        const double a2 = (-6.0 * da - h * (4.0 * j0[c] + 2.0 * j1[c])) / h2;
+        a3[c] = (12.0 * da + 6.0 * h * (j0[c] + j1[c])) / h3;
+        x1[c] = x0[c] + v0[c] * h + a0[c] * h2 / 2.0 + j0[c] * h3 / 6.0 + a2 * h4 / 24.0 + a3[c] * h5 / 120.0;
+        v1[c] = v0[c] + a0[c] * h + j0[c] * h2 / 2.0 + a2 * h3 / 6.0 + a3[c] * h4 / 24.0;
+        a2e[c] = a2 + h * a3[c];
+    }
+    double dI, dR = hR;
+    int32_t nn = A.nnb[i];
+    if (!due) {
+        dI = block_rule(aarseth_req(aI1, jI1, a2e, a3, eta_I), h, t, dt_max);
+    } else {
+        int lo = 0, hi = n_reg - 1;                             // slot of body i in the ascending regular list
+        while (lo < hi) {
+            const int mid = (lo + hi) >> 1;
+            if (idx_reg[mid] < (int32_t)i) lo = mid + 1; else hi = mid;
+        }
+        const int r = lo;
+        const double g2 = hR * hR, g3 = g2 * hR, g4 = g2 * g2, g5 = g4 * hR;
+        double aRn[3], jRn[3], aIn[3], jIn[3], a2Re[3], a3R[3];
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            aRn[c] = rg_acc[3 * r + c]; jRn[c] = rg_jerk[3 * r + c];
+            aIn[c] = in_acc[3 * r + c]; jIn[c] = in_jerk[3 * r + c];
+            const double atot = aRn[c] + aIn[c], jtot = jRn[c] + jIn[c];
+            const double aR1 = atot - aI1[c], jR1 = jtot - jI1[c];          // regular force w.r.t. the OLD list
+            const double da = aR0[c] - aR1;
+            const double a2R = (-6.0 * da - hR * (4.0 * jR0[c] + 2.0 * jR1)) / g2;
+            a3R[c] = (12.0 * da + 6.0 * hR * (jR0[c] + jR1)) / g3;
+            x1[c] = x1[c] + (a2R * g4 / 24.0 + a3R[c] * g5 / 120.0);       // the regular correction (R35)
+            v1[c] = v1[c] + (a2R * g3 / 6.0 + a3R[c] * g4 / 24.0);
+            a2Re[c] = a2R + hR * a3R[c];
+            a1[c] = atot; j1[c] = jtot;
+        }
+        dR = block_rule(aarseth_req(aRn, jRn, a2Re, a3R, eta_R), hR, t, dt_max);
+        dI = block_rule(aarseth_req(aIn, jIn, a2e, a3, eta_I), h, t, dt_max);
+        nn = rg_nnb[r];
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            aI1[c] = aIn[c]; jI1[c] = jIn[c];
+            A.aR[3 * i + c] = aRn[c]; A.jR[3 * i + c] = jRn[c];
+        }
+        A.tR[i] = t; A.dtR[i] = dR; A.nnb[i] = nn;
+    }
+    dI = nn == 0 ? dR : fmin(dI, dR);                          // R36; never above the regular step
+#pragma unroll
+    for (int c = 0; c < 3; ++c) { A.aI[3 * i + c] = aI1[c]; A.jI[3 * i + c] = jI1[c]; }
+    store_body(i, Ns, m, x1, v1, a1, j1, t, soa, aos);
+    dtj[i] = dI;
+}
+
+// New list rows of the regular-active bodies into the persistent by-body lists: one warp per row.
+__global__ void __launch_bounds__(256) ac_store_rows_kernel(int32_t n_reg, int32_t cap, const int32_t *__restrict__ idx_reg,
+                                                            const int32_t *__restrict__ rg_nnb,
+                                                            const int32_t *__restrict__ rg_list, int32_t *__restrict__ list) {
+    const int lane = threadIdx.x & 31;
+    const int r = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    if (r >= n_reg) return;
+    const int64_t i = idx_reg[r];
+    const int c = min(rg_nnb[r], cap);
+    for (int e = lane; e < c; e += 32) list[i * cap + e] = rg_list[(int64_t)r * cap + e];
+}
+
+// block-level overflow count of the regular pass (R38)
+__global__ void __launch_bounds__(256) count_overflow_kernel(int32_t n, const int32_t *__restrict__ ovf, int32_t *__restrict__ out) {
+    int32_t c = 0;
+    for (int k = blockIdx.x * blockDim.x + threadIdx.x; k < n; k += gridDim.x * blockDim.x) c += ovf[k] ? 1 : 0;
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) c += __shfl_xor_sync(0xffffffffu, c, off);
+    if ((threadIdx.x & 31) == 0 && c) atomicAdd(out, c);
 }
 
 // Inspection: the FP64 state back in the caller's layout (tests, energy checks, checkpoints).

@@ -1,0 +1,161 @@
+"""Two-level Ahmad-Cohen stepping on the GPU (nb_ac_init / nb_ac_step, readings R33-R38) against
+oracle/hermite_ac.py on the same seeded inputs.  Needs a B200."""
+import numpy as np
+import pytest
+
+import nbgen
+from oracle import hermite_ac as AC
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+def _dev(a, dtype=None):
+    t = torch.from_numpy(np.ascontiguousarray(a))
+    if dtype is not None:
+        t = t.to(dtype)
+    return t.cuda()
+
+
+def _radii(x, k):
+    d2 = ((x[:, None, :] - x[None, :, :]) ** 2).sum(-1)
+    return np.sort(d2, axis=1)[:, k] * 1.002
+
+
+def _open(m, x, v, cap):
+    import paper_1504_03687_b200 as nb
+    N = m.shape[0]
+    ctx = nb.nb_open(N, cap)
+    z3, z1 = np.zeros((N, 3)), np.zeros(N)
+    nb.nb_set_j(ctx, _dev(m), _dev(x), _dev(v), _dev(z3), _dev(z3), _dev(z1))
+    return ctx
+
+
+def _gpu_state(ctx, lists=False):
+    st = {k: v.cpu().numpy() for k, v in ctx.get_state(True).items()}
+    st.update({k: v.cpu().numpy() for k, v in ctx.ac_get(lists).items()})
+    return st
+
+
+def _rel(a, b):
+    s = np.linalg.norm(b, axis=1)
+    return np.max(np.linalg.norm(a - b, axis=1) / np.where(s > 0, s, 1.0))
+
+
+def test_ac_start_and_blocks_in_lockstep_with_the_oracle(oracle):
+    N, cap = 1024, 128
+    cfg = nbgen.make_config(1, N=N)
+    m, x, v = cfg["m"], cfg["x0"], cfg["v0"]
+    h2 = _radii(x, 16)
+    eta_I, eta_R, eta_s, dt_max = 0.01, 0.02, 0.01, 2.0**-4
+    st = AC.start(oracle, m, x, v, h2, cap, eta_s, dt_max)
+    ctx = _open(m, x, v, cap)
+    assert ctx.ac_init(0.0, _dev(h2), eta_s, dt_max) == 0
+    g = _gpu_state(ctx, lists=True)
+    assert np.array_equal(g["nnb"], st["nnb"])
+    for i in range(N):
+        assert np.array_equal(g["nblist"][i, :g["nnb"][i]], st["list"][i, :st["nnb"][i]])
+    assert _rel(g["aI"], st["aI"]) < 1e-12 and _rel(g["jI"], st["jI"]) < 1e-11       # FP64 neighbour force
+    assert _rel(g["aR"], st["aR"]) < 1e-5 and _rel(g["jR"], st["jR"]) < 1e-4         # FP32 pair arithmetic
+    assert _rel(g["a0"], st["a0"]) < 1e-5
+    flips = int((g["dt"] != st["dtI"]).sum() + (g["dtR"] != st["dtR"]).sum())
+    st["dtI"], st["dtR"] = g["dt"].copy(), g["dtR"].copy()                            # adopt flipped decisions
+    nblocks, isteps, rsteps, pure_irr = 300, 0, 0, 0
+    for b in range(nblocks):
+        t, n, nr = ctx.ac_step(eta_I, eta_R, dt_max)
+        t_ref, act, reg = AC.block_step(oracle, m, st, h2, cap, eta_I, eta_R, dt_max)
+        g = _gpu_state(ctx)
+        assert t == t_ref and n == act.size and nr == reg.size, (b, t, t_ref, n, act.size, nr, reg.size)
+        assert np.array_equal(g["idx_act"][:n], act) and np.array_equal(g["idx_reg"][:nr], reg)
+        isteps += n; rsteps += nr; pure_irr += int(nr == 0)
+        dI, dR = np.flatnonzero(g["dt"] != st["dtI"]), np.flatnonzero(g["dtR"] != st["dtR"])
+        assert np.isin(dI, act).all() and np.isin(dR, reg).all()
+        flips += dI.size + dR.size
+        st["dtI"][dI] = g["dt"][dI]; st["dtR"][dR] = g["dtR"][dR]
+        assert np.all(g["dt"] <= g["dtR"])
+    g = _gpu_state(ctx, lists=True)
+    print("AC lockstep: blocks", nblocks, "irregular steps", isteps, "regular steps", rsteps, "blocks without a regular step",
+          pure_irr, "flips", flips, "max |dx|", np.abs(g["x0"] - st["x0"]).max())
+    assert pure_irr > nblocks // 3 and rsteps > 0
+    assert flips <= max(3, int(2e-3 * (isteps + rsteps)))
+    assert np.array_equal(g["t0"], st["t0"]) and np.array_equal(g["tR"], st["tR"])
+    assert np.abs(g["x0"] - st["x0"]).max() < 1e-9 and np.abs(g["v0"] - st["v0"]).max() < 1e-7
+    assert _rel(g["aI"], st["aI"]) < 1e-7 and _rel(g["aR"], st["aR"]) < 1e-5
+    same_lists = sum(np.array_equal(g["nblist"][i, :g["nnb"][i]], st["list"][i, :st["nnb"][i]]) for i in range(N))
+    assert same_lists >= N - 2                                   # (a band pair may be classified differently)
+    ctx.close()
+
+
+def test_ac_without_neighbours_is_the_single_level_block_step_on_the_gpu():
+    """Every h2 = 0: no lists, dtI = dtR, and nb_ac_step must reproduce nb_block_step (same force kernel, the
+    corrector written as irregular corrector + regular correction): same blocks, same steps, states to rounding."""
+    import paper_1504_03687_b200 as nb
+    N = 2048
+    cfg = nbgen.make_config(2, N=N, n_i=16)
+    m, x, v = cfg["m"], cfg["x0"], cfg["v0"]
+    eta, eta_s, dt_max = 0.02, 0.02, 2.0**-5
+    a = _open(m, x, v, 8)
+    assert a.ac_init(0.0, _dev(np.zeros(N)), eta_s, dt_max) == 0
+    ga = _gpu_state(a)
+    b = nb.nb_open(N, 8)
+    z1 = np.zeros(N)
+    nb.nb_set_j(b, _dev(m), _dev(x), _dev(v), _dev(ga["a0"]), _dev(ga["j0"]), _dev(z1))
+    b.init_steps(eta_s, dt_max)
+    for blk in range(60):
+        ta, na, nra = a.ac_step(0.005, eta, dt_max)
+        tb, nb_ = b.block_step(None, eta, dt_max)
+        assert ta == tb and na == nb_ == nra, (blk, ta, tb, na, nb_, nra)
+    ga = _gpu_state(a)
+    gb = {k: v.cpu().numpy() for k, v in b.get_state(True).items()}
+    assert np.array_equal(ga["dt"], gb["dt"]) and np.array_equal(ga["dtR"], gb["dt"]) and np.array_equal(ga["t0"], gb["t0"])
+    # the two correctors group the same terms differently (x' + (A + B) against ((x' + A) + B)): a 1e-16 difference
+    # in x now and then flips an FP32 rounding inside the next force sum (1e-7 of a pair term), so the two runs agree
+    # to the noise of the FP32 force, ~1e-7 |a| dt^2, not to FP64 rounding; a missing correction term would be ~1e-5
+    assert np.abs(ga["x0"] - gb["x0"]).max() < 1e-10 and np.abs(ga["v0"] - gb["v0"]).max() < 1e-8
+    assert not ga["aI"].any() and ga["nnb"].sum() == 0
+    a.close(); b.close()
+
+
+def test_ac_run_conserves_energy_and_overflow_is_reported(oracle):
+    import paper_1504_03687_b200 as nb
+    N, cap = 1024, 128
+    cfg = nbgen.make_config(1, N=N)
+    m, x, v = cfg["m"], cfg["x0"], cfg["v0"]
+    h2 = _radii(x, 16)
+    eta_I, eta_R, eta_s, dt_max, t_end = 0.01, 0.02, 0.01, 2.0**-4, 0.125
+
+    def energy(xx, vv):
+        pot = oracle.regular(m, xx, vv, np.arange(N, dtype=np.int32), np.zeros(N), 8, want_list=False)["pot"]
+        return 0.5 * (m * (vv * vv).sum(1)).sum() + 0.5 * (m * pot).sum()
+
+    e0 = energy(x, v)
+    ctx = _open(m, x, v, cap)
+    ctx.ac_init(0.0, _dev(h2), eta_s, dt_max)
+    blocks = isteps = rsteps = 0
+    while True:
+        t, n, nr = ctx.ac_step(eta_I, eta_R, dt_max, t_stop=t_end)
+        if n == 0:
+            assert t > t_end
+            break
+        blocks += 1; isteps += n; rsteps += nr
+    g = _gpu_state(ctx)
+    assert np.all(g["t0"] == t_end) and np.all(g["tR"] == t_end)
+    e1 = energy(g["x0"], g["v0"])
+    ref = AC.integrate(oracle, m, x, v, h2, cap, t_end, eta_I, eta_R, eta_s, dt_max)
+    print("AC run on the GPU: blocks", blocks, "irregular steps", isteps, "regular steps", rsteps, "dE/E", (e1 - e0) / e0,
+          "oracle", ref["blocks"], ref["irregular_steps"], ref["regular_steps"], "max |dx| vs oracle", np.abs(g["x0"] - ref["x0"]).max())
+    assert abs((e1 - e0) / e0) < 5e-6
+    assert isteps > 2 * rsteps > 0
+    assert abs(isteps - ref["irregular_steps"]) <= 0.01 * ref["irregular_steps"]
+    assert np.abs(g["x0"] - ref["x0"]).max() < 1e-5
+    ctx.close()
+    # radii that hold more bodies than the lists can: an error of the start-up, nothing is integrated
+    ctx = _open(m, x, v, 8)
+    with pytest.raises(nb.NbregError) as e:
+        ctx.ac_init(0.0, _dev(h2), eta_s, dt_max)
+    assert e.value.code == nb.NB_EOVERFLOW
+    with pytest.raises(nb.NbregError) as e:
+        ctx.ac_step(eta_I, eta_R, dt_max)
+    assert e.value.code == nb.NB_ESTATE
+    ctx.close()
