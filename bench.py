@@ -523,7 +523,39 @@ def run_b200(args):
                     "jsplit": ctx.info("last_jsplit"), "reordered": ctx.info("last_reordered"),
                     "note": "nb_regular_all, nblist = NULL (neighbours counted), includes the Morton sort of the block and finalize"}
         del fo, h2_full
+        # NEXT-3, two-level Ahmad-Cohen stepping: start-up (full regular pass with lists + neighbour force) and
+        # 120 blocks; a block without a regular step never touches all N bodies' forces
+        actx = nb.nb_open(N, cap, stream)
+        astate = list(jstate)
+        astate[5] = torch.zeros(N, dtype=torch.float64, device=dev)
+        actx.set_j(*astate)
+        a0_, a1_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a0_.record(stream)
+        actx.ac_init(0.0, f64(cfg["h2_all"]), 0.02, 2.0 ** -6)
+        a1_.record(stream); torch.cuda.synchronize()
+        ms_acinit = a0_.elapsed_time(a1_)
+        for _ in range(5):
+            actx.ac_step(0.02, 0.03, 2.0 ** -6)
+        torch.cuda.synchronize()
+        stamps_a, kinds = [time.perf_counter()], []
+        for _ in range(120):
+            _, ni_a, nr_a = actx.ac_step(0.02, 0.03, 2.0 ** -6)
+            stamps_a.append(time.perf_counter()); kinds.append((ni_a, nr_a))
+        torch.cuda.synchronize()
+        actx.close()
+        cyc = np.diff(np.array(stamps_a))[1:] * 1e6
+        kinds_a = np.array(kinds)
+        irr_only = (kinds_a[:-1, 1] == 0) & (kinds_a[1:, 1] == 0)
+        with_reg = kinds_a[:-1, 1] > 0
+        acstep = {"nb_ac_init_ms": ms_acinit, "blocks": 120, "n_irr_median": float(np.median(kinds_a[:, 0])),
+                  "blocks_without_regular_step": int((kinds_a[:, 1] == 0).sum()),
+                  "us_per_block_without_regular_step": float(np.median(cyc[irr_only])) if irr_only.any() else None,
+                  "us_per_block_with_regular_step": float(np.median(cyc[with_reg])) if with_reg.any() else None,
+                  "n_reg_median_when_due": float(np.median(kinds_a[kinds_a[:, 1] > 0, 1])) if (kinds_a[:, 1] > 0).any() else None,
+                  "note": "config 4 at t = 0 with the block radii (150 neighbours, cap 512); host wall clock between the returns "
+                          "of consecutive nb_ac_step calls"}
         extras = {
+            "nb_ac_step": acstep,
             "nb_regular_all": fullpass,
             "nb_block_step": blockstep,
             "nb_irregular": {"n_i": n_i, "neighbour_pairs": nn, "ms": ms_irr, "pairs_per_s": nn / (ms_irr * 1e-3),
