@@ -246,6 +246,16 @@ int nb_ac_init(nb_ctx *ctx, double t_start, const double *h2_all, double eta_s, 
  * step cost O(n_irr x neighbours), not O(N).  One host read-back per block (two when regular steps are due). */
 int nb_ac_step(nb_ctx *ctx, double eta_I, double eta_R, double dt_max, double t_stop, double *t_next,
                int32_t *n_irr, int32_t *n_reg);
+/* The block loop itself (SURVEY 8(f) NEXT-3 "device-side block loop"): nb_ac_step / nb_block_step repeated inside
+ * the library until nothing is due before t_stop or max_blocks blocks are done -- no per-block call overhead on
+ * the caller's side.  HOST outputs: *t_next (time of the next block that was NOT integrated, or of the last one
+ * tried), the number of blocks and of particle steps taken.  An error of a step (e.g. NB_EOVERFLOW) ends the
+ * loop and is returned; the counters tell how far it got. */
+int nb_ac_run(nb_ctx *ctx, double eta_I, double eta_R, double dt_max, double t_stop, int64_t max_blocks,
+              double *t_next, int64_t *blocks, int64_t *irregular_steps, int64_t *regular_steps);
+int nb_run_blocks(nb_ctx *ctx, const double *h2_all, double eta, double dt_max, double t_stop,
+                  int64_t max_blocks, double *t_next, int64_t *blocks, int64_t *particle_steps);
+
 /* Inspection: copies of the AC state into the caller's DEVICE buffers (any may be NULL): the last block's
  * idx_act[N] / idx_reg[N] (first n_irr / n_reg entries valid), aI, jI, aR, jR [N][3], tR, dtR [N], nnb[N],
  * nblist[N][nb_cap].  (x0, v0, total a0 / j0, t0 and dtI come from nb_get_state.) */

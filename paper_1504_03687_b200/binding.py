@@ -66,6 +66,8 @@ def load_library(build: bool = True) -> ctypes.CDLL:
     lib.nb_ac_init.argtypes = [_vp, dbl, _vp, dbl, dbl, ctypes.POINTER(i32)]
     lib.nb_ac_step.argtypes = [_vp, dbl, dbl, dbl, dbl, ctypes.POINTER(dbl), ctypes.POINTER(i32), ctypes.POINTER(i32)]
     lib.nb_ac_get.argtypes = [_vp] + [_vp] * 10
+    lib.nb_ac_run.argtypes = [_vp, dbl, dbl, dbl, dbl, i64, ctypes.POINTER(dbl)] + [ctypes.POINTER(i64)] * 3
+    lib.nb_run_blocks.argtypes = [_vp, _vp, dbl, dbl, dbl, i64, ctypes.POINTER(dbl)] + [ctypes.POINTER(i64)] * 2
     lib.nb_set_j_offset.argtypes = [_vp, i64]
     lib.nb_regular_shard.argtypes = [_vp, dbl, i32] + [_vp] * 9
     lib.nb_plan_regular.argtypes = [i64, i64, i32, i32] + [ctypes.POINTER(i32)] * 4
@@ -295,6 +297,26 @@ class NbContext:
         _check(self._lib.nb_ac_step(self._ctx, float(eta_I), float(eta_R), float(dt_max), t_stop, ctypes.byref(t),
                                     ctypes.byref(ni), ctypes.byref(nr)), "nb_ac_step", self._ctx)
         return t.value, ni.value, nr.value
+
+    def ac_run(self, eta_I: float, eta_R: float, dt_max: float, t_stop: float = float("inf"), max_blocks: int = 1 << 62):
+        """nb_ac_run -> (t_next, blocks, irregular_steps, regular_steps)."""
+        t = ctypes.c_double()
+        nb_, ni, nr = ctypes.c_int64(), ctypes.c_int64(), ctypes.c_int64()
+        t_stop = min(float(t_stop), 1.7976931348623157e308)
+        _check(self._lib.nb_ac_run(self._ctx, float(eta_I), float(eta_R), float(dt_max), t_stop, int(max_blocks),
+                                   ctypes.byref(t), ctypes.byref(nb_), ctypes.byref(ni), ctypes.byref(nr)), "nb_ac_run", self._ctx)
+        return t.value, nb_.value, ni.value, nr.value
+
+    def run_blocks(self, h2_all, eta: float, dt_max: float, t_stop: float = float("inf"), max_blocks: int = 1 << 62):
+        """nb_run_blocks -> (t_next, blocks, particle_steps)."""
+        import torch
+        t = ctypes.c_double()
+        nb_, ns = ctypes.c_int64(), ctypes.c_int64()
+        h2 = _vp() if h2_all is None else _dev_ptr(h2_all, torch.float64, self.N, "h2_all")
+        t_stop = min(float(t_stop), 1.7976931348623157e308)
+        _check(self._lib.nb_run_blocks(self._ctx, h2, float(eta), float(dt_max), t_stop, int(max_blocks), ctypes.byref(t),
+                                       ctypes.byref(nb_), ctypes.byref(ns)), "nb_run_blocks", self._ctx)
+        return t.value, nb_.value, ns.value
 
     def ac_get(self, with_lists: bool = False) -> dict:
         import torch

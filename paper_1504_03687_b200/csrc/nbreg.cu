@@ -1031,7 +1031,7 @@ int nb_block_step(nb_ctx *c, const double *h2_all, double eta, double dt_max, do
     };
     // speculate on the size class of the previous block (32 / 64 / 128: the variants with a fused predictor)
     int32_t spec_cap = 0;
-    if (c->fuse && c->spec_enabled && c->blk_prev_n > 0 && c->blk_prev_n <= 128)
+    if (c->fuse && c->spec_enabled && t_stop >= 0.0 && c->blk_prev_n > 0 && c->blk_prev_n <= 128)
         spec_cap = c->blk_prev_n <= 32 ? 32 : c->blk_prev_n <= 64 ? 64 : 128;
     if (spec_cap > 0) {
         rc = enqueue_chain(spec_cap, 0.0, spec_cap);
@@ -1139,13 +1139,39 @@ int nb_ac_step(nb_ctx *c, double eta_I, double eta_R, double dt_max, double t_st
         c->blk_parity ^= 1;
         c->launches += 1;
         NB_CUDA(c, cudaMemcpyAsync(c->h_sel_result, c->sel_result, sizeof(double) * 3, cudaMemcpyDeviceToHost, c->stream));
-        NB_CUDA(c, cudaStreamSynchronize(c->stream));
+        NB_CUDA(c, cudaEventRecord(c->ev_sel, c->stream));
     }
+    // Most blocks of the two-level scheme hold a few bodies and NO regular step (irregular steps are the
+    // small ones).  Their chain -- neighbour force over the lists, corrector -- is enqueued before the host knows
+    // the block: the kernels take {t, n, n_reg} from device memory and do nothing unless n <= AC_SPEC_CAP,
+    // n_reg = 0 and t <= t_stop, so the GPU does not idle while the host waits for the read-back.
+    constexpr int32_t AC_SPEC_CAP = 1024;
+    const bool spec = c->spec_enabled && t_stop >= 0.0;
+    if (spec) {
+        const double ts_enc = -std::max(t_stop, 4.9406564584124654e-324);     // negative: "and no regular step due"
+        irregular_kernel<false><<<(AC_SPEC_CAP + 7) / 8, 256, 0, c->stream>>>(AC_SPEC_CAP, c->cap, 0.0, c->sel_result, ts_enc, 1, 1,
+                                                                              c->blk_idx, c->ac.nnb, c->ac.list, c->aos, c->ac_aIo,
+                                                                              c->ac_jIo, nullptr);
+        ac_correct_kernel<<<(AC_SPEC_CAP + 127) / 128, 128, 0, c->stream>>>(AC_SPEC_CAP, c->Ns, 0.0, eta_I, eta_R, dt_max, c->sel_result,
+                                                                            ts_enc, c->blk_idx, c->ac_aIo, c->ac_jIo, 0, c->ac_reg_idx,
+                                                                            nullptr, nullptr, nullptr, nullptr, c->blk_nnb, c->ac, c->soa,
+                                                                            c->aos, c->dtj);
+        NB_CUDA(c, cudaGetLastError());
+        c->launches += 2;
+    }
+    NB_CUDA(c, cudaEventSynchronize(c->ev_sel));
     const double t = c->h_sel_result[0];
     const int32_t n = (int32_t)c->h_sel_result[1], nr = (int32_t)c->h_sel_result[2];
     *t_next = t; *n_irr = 0; *n_reg = 0;
     c->blk_last_n = 0;
     if (t > t_stop || n <= 0) return NB_OK;
+    if (spec && nr == 0 && n <= AC_SPEC_CAP) {      // the speculative chain was this block
+        c->spec_hits += 1;
+        c->have_pred = false; c->pred_pending = false;
+        *n_irr = n;
+        return NB_OK;
+    }
+    if (spec) c->spec_misses += 1;
     // irregular force over the OLD lists of every active body (rows and outputs by body)
     irregular_kernel<false><<<(unsigned)((n + 7) / 8), 256, 0, c->stream>>>(n, c->cap, t, nullptr, 0.0, 1, 1, c->blk_idx, c->ac.nnb,
                                                                             c->ac.list, c->aos, c->ac_aIo, c->ac_jIo, nullptr);
@@ -1200,7 +1226,7 @@ int nb_ac_step(nb_ctx *c, double eta_I, double eta_R, double dt_max, double t_st
             return NB_EOVERFLOW;
         }
     }
-    ac_correct_kernel<<<(unsigned)((n + 127) / 128), 128, 0, c->stream>>>(n, c->Ns, t, eta_I, eta_R, dt_max, c->blk_idx, c->ac_aIo,
+    ac_correct_kernel<<<(unsigned)((n + 127) / 128), 128, 0, c->stream>>>(n, c->Ns, t, eta_I, eta_R, dt_max, nullptr, 0.0, c->blk_idx, c->ac_aIo,
                                                                           c->ac_jIo, nr, c->ac_reg_idx, rg_acc, rg_jerk, in_acc,
                                                                           in_jerk, c->blk_nnb, c->ac, c->soa, c->aos, c->dtj);
     if (nr > 0)
@@ -1211,6 +1237,34 @@ int nb_ac_step(nb_ctx *c, double eta_I, double eta_R, double dt_max, double t_st
     c->have_pred = false; c->pred_pending = false;
     *n_irr = n; *n_reg = nr;
     return NB_OK;
+}
+
+int nb_ac_run(nb_ctx *c, double eta_I, double eta_R, double dt_max, double t_stop, int64_t max_blocks, double *t_next,
+              int64_t *blocks, int64_t *irregular_steps, int64_t *regular_steps) {
+    if (!t_next || !blocks || !irregular_steps || !regular_steps || max_blocks < 0) return NB_EINVAL;
+    *blocks = *irregular_steps = *regular_steps = 0;
+    int rc = NB_OK;
+    while (*blocks < max_blocks) {
+        int32_t ni = 0, nr = 0;
+        rc = nb_ac_step(c, eta_I, eta_R, dt_max, t_stop, t_next, &ni, &nr);
+        if (rc != NB_OK || ni == 0) break;          // error, or nothing due before t_stop
+        *blocks += 1; *irregular_steps += ni; *regular_steps += nr;
+    }
+    return rc;
+}
+
+int nb_run_blocks(nb_ctx *c, const double *h2_all, double eta, double dt_max, double t_stop, int64_t max_blocks,
+                  double *t_next, int64_t *blocks, int64_t *particle_steps) {
+    if (!t_next || !blocks || !particle_steps || max_blocks < 0) return NB_EINVAL;
+    *blocks = *particle_steps = 0;
+    int rc = NB_OK;
+    while (*blocks < max_blocks) {
+        int32_t n = 0;
+        rc = nb_block_step(c, h2_all, eta, dt_max, t_stop, t_next, &n);
+        if (rc != NB_OK || n == 0) break;
+        *blocks += 1; *particle_steps += n;
+    }
+    return rc;
 }
 
 int nb_ac_get(nb_ctx *c, int32_t *idx_act, int32_t *idx_reg, double *aI, double *jI, double *aR, double *jR, double *tR,

@@ -463,10 +463,16 @@ struct ForceParams {
                                   // a no-op if the block is larger than n_i (its capacity) or not due before t_stop
 };
 // The block a speculative launch works on: false = nothing to do.  n and t are overwritten from blk_dev.
+// t_stop < 0 encodes "and only if NO regular step is due in this block" (two-level AC stepping: blk_dev[2] = 0)
+// with the real bound -t_stop (block times are >= 0).
 __device__ __forceinline__ bool spec_block(const double *blk_dev, double t_stop, int32_t &n, double &t) {
     if (!blk_dev) return true;
     const double tn = blk_dev[0];
     const int32_t nd = (int32_t)blk_dev[1];
+    if (t_stop < 0.0) {
+        if (blk_dev[2] != 0.0) return false;
+        t_stop = -t_stop;
+    }
     if (tn > t_stop || nd > n || nd <= 0) return false;
     n = nd; t = tn;
     return true;
@@ -1537,7 +1543,8 @@ __global__ void __launch_bounds__(128) ac_start_kernel(int64_t N, int64_t Ns, in
 // its slot r in the ascending idx_reg[0..n_reg) and there the new-list forces: regular rg_acc/rg_jerk[r],
 // irregular in_acc/in_jerk[r], new count rg_nnb[r] (rows are copied by ac_store_rows_kernel afterwards).
 __global__ void __launch_bounds__(128) ac_correct_kernel(int32_t n, int64_t Ns, double t, double eta_I, double eta_R,
-                                                         double dt_max, const int32_t *__restrict__ idx,
+                                                         double dt_max, const double *__restrict__ blk_dev, double t_stop,
+                                                         const int32_t *__restrict__ idx,
                                                          const double *__restrict__ aIo, const double *__restrict__ jIo,
                                                          int32_t n_reg, const int32_t *__restrict__ idx_reg,
                                                          const double *__restrict__ rg_acc, const double *__restrict__ rg_jerk,
@@ -1546,6 +1553,7 @@ __global__ void __launch_bounds__(128) ac_correct_kernel(int32_t n, int64_t Ns, 
                                                          double *__restrict__ soa, double *__restrict__ aos,
                                                          double *__restrict__ dtj) {
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (!spec_block(blk_dev, t_stop, n, t)) return;
     if (k >= n) return;
     const int64_t i = idx[k];
     const double2 *p = reinterpret_cast<const double2 *>(aos + i * AOS_D);

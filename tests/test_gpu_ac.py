@@ -132,13 +132,12 @@ def test_ac_run_conserves_energy_and_overflow_is_reported(oracle):
     e0 = energy(x, v)
     ctx = _open(m, x, v, cap)
     ctx.ac_init(0.0, _dev(h2), eta_s, dt_max)
-    blocks = isteps = rsteps = 0
-    while True:
-        t, n, nr = ctx.ac_step(eta_I, eta_R, dt_max, t_stop=t_end)
-        if n == 0:
-            assert t > t_end
-            break
-        blocks += 1; isteps += n; rsteps += nr
+    t, blocks, isteps, rsteps = ctx.ac_run(eta_I, eta_R, dt_max, t_stop=t_end, max_blocks=100)      # the loop inside the library
+    assert blocks == 100 and t < t_end
+    t, b2, i2, r2 = ctx.ac_run(eta_I, eta_R, dt_max, t_stop=t_end)
+    assert t > t_end and b2 > 0
+    blocks += b2; isteps += i2; rsteps += r2
+    assert ctx.ac_run(eta_I, eta_R, dt_max, t_stop=t_end)[1:] == (0, 0, 0)                        # nothing left before t_end
     g = _gpu_state(ctx)
     assert np.all(g["t0"] == t_end) and np.all(g["tR"] == t_end)
     e1 = energy(g["x0"], g["v0"])

@@ -357,13 +357,14 @@ def test_block_step_stops_at_t_stop_and_closed_loop_conserves_energy():
     nb.nb_set_j(ctx, _dev(m), _dev(x), _dev(v), out["acc"].clone(), out["jerk"].clone(), z1)
     ctx.init_steps(eta_s, dt_max)
     blocks = psteps = 0
-    while True:
+    for _ in range(40):                                                   # one call per block ...
         t, n = ctx.block_step(None, eta, dt_max, t_stop=t_end)
-        if n == 0:
-            assert t > t_end
-            break
+        assert n > 0
         blocks += 1
         psteps += n
+    t, b2, p2 = ctx.run_blocks(None, eta, dt_max, t_stop=t_end)           # ... and the loop inside the library
+    assert t > t_end and b2 > 0
+    blocks += b2; psteps += p2
     s1 = _state(ctx)
     t2, n2 = ctx.block_step(None, eta, dt_max, t_stop=t_end)            # again: still nothing due, state untouched
     s2 = _state(ctx)
