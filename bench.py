@@ -542,10 +542,14 @@ def run_b200(args):
             _, ni_a, nr_a = actx.ac_step(0.02, 0.03, 2.0 ** -6)
             stamps_a.append(time.perf_counter()); kinds.append((ni_a, nr_a))
         torch.cuda.synchronize()
-        tw = time.perf_counter()
-        _, nb_run, ni_run, nr_run = actx.ac_run(0.02, 0.03, 2.0 ** -6, max_blocks=400)      # the loop inside the library
-        torch.cuda.synchronize()
-        us_run = (time.perf_counter() - tw) * 1e6 / max(nb_run, 1)
+        segs = []                                         # the loop inside the library, in segments of 100 blocks
+        for _ in range(6):
+            tw = time.perf_counter()
+            _, nb_run, ni_run, nr_run = actx.ac_run(0.02, 0.03, 2.0 ** -6, max_blocks=100)
+            torch.cuda.synchronize()
+            segs.append({"blocks": int(nb_run), "irregular_steps": int(ni_run), "regular_steps": int(nr_run),
+                         "us_per_block_mean": (time.perf_counter() - tw) * 1e6 / max(nb_run, 1)})
+        spec_ac = {"hits": actx.info("spec_hits"), "misses": actx.info("spec_misses")}
         actx.close()
         cyc = np.diff(np.array(stamps_a))[1:] * 1e6
         kinds_a = np.array(kinds)
@@ -555,8 +559,7 @@ def run_b200(args):
                   "blocks_without_regular_step": int((kinds_a[:, 1] == 0).sum()),
                   "us_per_block_without_regular_step": float(np.median(cyc[irr_only])) if irr_only.any() else None,
                   "us_per_block_with_regular_step": float(np.median(cyc[with_reg])) if with_reg.any() else None,
-                  "nb_ac_run": {"blocks": int(nb_run), "irregular_steps": int(ni_run), "regular_steps": int(nr_run),
-                                "us_per_block_mean": us_run},
+                  "nb_ac_run_segments_of_100_blocks": segs, "speculation": spec_ac,
                   "n_reg_median_when_due": float(np.median(kinds_a[kinds_a[:, 1] > 0, 1])) if (kinds_a[:, 1] > 0).any() else None,
                   "note": "config 4 at t = 0 with the block radii (150 neighbours, cap 512); host wall clock between the returns "
                           "of consecutive nb_ac_step calls"}

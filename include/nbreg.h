@@ -197,8 +197,9 @@ int nb_correct(nb_ctx *ctx, double t, int32_t n, const int32_t *idx, const doubl
 
 /* One whole block step in ONE call (SURVEY 8(f) NEXT-3 "device-side block loop"; P:47 block steps, P:89 the
  * cost of selection against small deep blocks, P:45 corrector):
- *     selection  t_next = min_j (t0_j + dt_j), active = {j : t0_j + dt_j = t_next} ascending (one cooperative
- *                launch; its {t_next, n} is the only host read-back of the step: the launch plan needs n)
+ *     selection  t_next = min_j (t0_j + dt_j), active = {j : t0_j + dt_j = t_next} ascending (two launches: a
+ *                minimum pass and a count / look-back prefix / ordered scatter pass; the block descriptor
+ *                {t_next, n, status} is stored straight into mapped host memory -- the only host read of the step)
  *  -> prediction to t_next + regular force of the active block (a2-a7; blocks of <= 128 particles predict
  *                inside the force kernel)
  *  -> if h2_all != NULL: the neighbour force on the lists just written, added in place

@@ -5,6 +5,7 @@
 #include "nbreg_kernels.cuh"
 
 #include <algorithm>
+#include <atomic>
 #include <cmath>
 #include <cstdlib>
 #include <cstring>
@@ -79,25 +80,30 @@ struct nb_ctx {
     double *sel_result = nullptr, *h_sel_result = nullptr;   // {t_next, n_active}: device / pinned host
     // nb_block_step: one cooperative selection launch (two alternating minimum slots), the block's own buffers
     unsigned long long *blk_key = nullptr;          // [2]
-    int blk_parity = 0, blk_grid = 0;
+    int blk_parity = 0;
     int32_t *blk_idx = nullptr;                     // [N] active indices of the last block
     double *blk_out = nullptr;                      // acc[3n] jerk[3n] pot[n]
     int32_t *blk_nnb = nullptr, *blk_ovf = nullptr, *blk_list = nullptr;
     int64_t blk_n = 0, blk_list_n = 0, blk_last_n = 0;
     bool blk_had_list = false;
     int32_t h2_by_body = 0;                         // the h2 array of the launch in flight is indexed by body
-    const double *spec_dev = nullptr;               // non-NULL while nb_block_step enqueues a SPECULATIVE chain: the
-    double spec_t_stop = 0.0;                       // kernels take {t, n} from this device address
+    const double *spec_dev = nullptr;               // non-NULL while a SPECULATIVE chain is enqueued: the kernels take the
+                                                    // block's {t, n, status} from this device address
     cudaEvent_t ev_sel = nullptr;
     int64_t blk_stride = 0;                         // acc / jerk / pot of the last block sit at 0, 3, 6 x this in blk_out
     // two-level AC stepping (nb_ac_init / nb_ac_step): per-body force polynomials, persistent lists, scratch
     AcState ac = {};
     double *ac_h2 = nullptr, *ac_aIo = nullptr, *ac_jIo = nullptr;     // radii; irregular force over the old list (by body)
-    int32_t *ac_reg_idx = nullptr, *ac_counts2 = nullptr, *ac_novf = nullptr, *h_ac_novf = nullptr;
+    int32_t *ac_reg_idx = nullptr, *ac_novf = nullptr, *h_ac_novf = nullptr;
     double *ac_in = nullptr;                                           // new-list irregular force of a block: acc[3n] jerk[3n]
     int64_t ac_in_n = 0;
     bool have_ac = false;
-    int ac_grid = 0;
+    double *blk_ring = nullptr, *h_blk_ring = nullptr;                 // descriptors of a batch of blocks: {t, n, n_reg, status}
+    unsigned long long *blk_pub = nullptr;                             // per-chunk counts of the selection, epoch-tagged
+    uint32_t blk_epoch = 0;
+    int32_t *blk_stall = nullptr;                                      // set by the first block of a batch that needs the host
+    bool blk_stall_dirty = true;                                       // the flag must be cleared before the next batch
+    int blk_batch = 1;                                                 // blocks enqueued per host round trip (adaptive)
     int64_t spec_hits = 0, spec_misses = 0, blk_prev_n = 0;
     bool spec_enabled = true;                       // NB_TUNE_SPECULATE
     // planning / introspection
@@ -265,7 +271,7 @@ int launch_force_range(nb_ctx *c, int vi, bool fused, int32_t n_i, const int32_t
     p.rec = c->rec;
     p.soa = c->soa; p.Ns = c->Ns; p.t = c->pred_t;
     p.g2 = (float)(c->local_g * c->local_g); p.stats = c->stats;
-    p.blk_dev = c->spec_dev; p.t_stop = c->spec_t_stop;
+    p.blk_dev = c->spec_dev;
     p.idx_i = idx_i; p.h2_i = h2_i; p.perm = perm; p.h2_by_body = c->h2_by_body;
     p.n_i = n_i; p.n_i_pad = (int32_t)(n_ib * v.iblock);
     p.irec = irec;
@@ -347,12 +353,11 @@ int launch_finalize(nb_ctx *c, int32_t n_i, int64_t n_i_pad, int S, const unsign
     cfg.numAttrs = 1;
     const int32_t n_i_pad32 = (int32_t)n_i_pad, S32 = S, cap32 = c->cap, sortP32 = sortP;
     const double *partial = c->partial, *blk_dev = c->spec_dev;
-    const double t_stop = c->spec_t_stop;
     if (W == 4)
-        NB_CUDA(c, cudaLaunchKernelEx(&cfg, finalize_kernel<4>, n_i, n_i_pad32, S32, cap32, sortP32, perm, blk_dev, t_stop,
+        NB_CUDA(c, cudaLaunchKernelEx(&cfg, finalize_kernel<4>, n_i, n_i_pad32, S32, cap32, sortP32, perm, blk_dev,
                                       partial, c->cnt, acc, jerk, pot, nnb, nblist, overflow));
     else
-        NB_CUDA(c, cudaLaunchKernelEx(&cfg, finalize_kernel<16>, n_i, n_i_pad32, S32, cap32, sortP32, perm, blk_dev, t_stop,
+        NB_CUDA(c, cudaLaunchKernelEx(&cfg, finalize_kernel<16>, n_i, n_i_pad32, S32, cap32, sortP32, perm, blk_dev,
                                       partial, c->cnt, acc, jerk, pot, nnb, nblist, overflow));
     NB_CUDA(c, cudaGetLastError());
     c->launches += 1;
@@ -538,7 +543,8 @@ int nb_close(nb_ctx *c) {
     cudaFree(c->blk_list);
     cudaFree(c->ac.aI); cudaFree(c->ac.jI); cudaFree(c->ac.aR); cudaFree(c->ac.jR); cudaFree(c->ac.tR); cudaFree(c->ac.dtR);
     cudaFree(c->ac.nnb); cudaFree(c->ac.list); cudaFree(c->ac_h2); cudaFree(c->ac_aIo); cudaFree(c->ac_jIo);
-    cudaFree(c->ac_reg_idx); cudaFree(c->ac_counts2); cudaFree(c->ac_novf); cudaFree(c->ac_in); cudaFreeHost(c->h_ac_novf);
+    cudaFree(c->ac_reg_idx); cudaFree(c->ac_novf); cudaFree(c->ac_in); cudaFreeHost(c->h_ac_novf);
+    cudaFree(c->blk_stall); cudaFree(c->blk_pub); cudaFreeHost(c->h_blk_ring);
     cudaFree(c->partial); cudaFree(c->stage_j);
     cudaFree(c->st_idx); cudaFree(c->st_nnb); cudaFree(c->st_ovf); cudaFree(c->st_list);
     cudaFree(c->st_h2); cudaFree(c->st_out);
@@ -634,7 +640,7 @@ int nb_irregular(nb_ctx *c, double t, int32_t n_i, const int32_t *idx_i, const i
     if (!idx_i || !nnb || !nblist || !acc || !jerk) return NB_EINVAL;
     rc = ensure_aos(c);
     if (rc != NB_OK) return rc;
-    irregular_kernel<false><<<(unsigned)((n_i + 7) / 8), 256, 0, c->stream>>>(n_i, c->cap, t, nullptr, 0.0, 0, 0, idx_i, nnb,
+    irregular_kernel<false><<<(unsigned)((n_i + 7) / 8), 256, 0, c->stream>>>(n_i, c->cap, t, nullptr, 0, 0, idx_i, nnb,
                                                                               nblist, c->aos, acc, jerk, pot);
     NB_CUDA(c, cudaGetLastError());
     c->launches += 1;
@@ -927,7 +933,7 @@ int nb_correct(nb_ctx *c, double t, int32_t n, const int32_t *idx, const double 
     if (!idx || !acc1 || !jerk1) return NB_EINVAL;
     rc = ensure_aos(c);
     if (rc != NB_OK) return rc;
-    correct_kernel<<<(unsigned)((n + 127) / 128), 128, 0, c->stream>>>(n, c->Ns, t, eta, dt_max, nullptr, 0.0, idx, acc1,
+    correct_kernel<<<(unsigned)((n + 127) / 128), 128, 0, c->stream>>>(n, c->Ns, t, eta, dt_max, nullptr, idx, acc1,
                                                                        jerk1, c->soa, c->aos, c->dtj);
     NB_CUDA(c, cudaGetLastError());
     c->launches += 1;
@@ -935,129 +941,300 @@ int nb_correct(nb_ctx *c, double t, int32_t n, const int32_t *idx, const double 
     return NB_OK;
 }
 
+}  // extern "C"
+
+namespace {
+
+// ---------------------------------------------------------------------------------------------------------
+// The block loop (nb_block_step / nb_run_blocks, nb_ac_step / nb_ac_run): ONE engine.  A BATCH of blocks is
+// enqueued without the host in between: per block the cooperative selection kernel, then the chain that can
+// integrate a small block with {t, n} taken from device memory (speculative: a no-op unless the selection
+// marked the block BLK_SPECULATIVE).  The first block of a batch that needs the host (too large, a regular
+// step due, past t_stop) sets the device stall flag; the rest of the batch does nothing and that block's lists
+// stay in place.  The host reads the batch's descriptors once, finishes the stalled block by the ordinary
+// launches, and enqueues the next batch.
+constexpr int BLK_BATCH_MAX = 16;
+constexpr int32_t AC_SPEC_CAP = 1024;
+
+int blk_setup(nb_ctx *c) {
+    if (c->blk_key) return NB_OK;
+    const int64_t N = c->N;
+    const int nchunk = (int)((N + SEL_CHUNK - 1) / SEL_CHUNK);
+    NB_CUDA(c, cudaMalloc(&c->blk_key, 2 * sizeof(unsigned long long)));
+    NB_CUDA(c, cudaMemsetAsync(c->blk_key, 0xff, 2 * sizeof(unsigned long long), c->stream));
+    NB_CUDA(c, cudaMalloc(&c->blk_idx, sizeof(int32_t) * N));
+    NB_CUDA(c, cudaMalloc(&c->ac_reg_idx, sizeof(int32_t) * N));
+    NB_CUDA(c, cudaMalloc(&c->blk_pub, sizeof(unsigned long long) * nchunk));
+    NB_CUDA(c, cudaMemsetAsync(c->blk_pub, 0, sizeof(unsigned long long) * nchunk, c->stream));
+    if (!c->sel_result) NB_CUDA(c, cudaMalloc(&c->sel_result, sizeof(double) * 4));
+    if (!c->h_sel_result) NB_CUDA(c, cudaMallocHost(&c->h_sel_result, sizeof(double) * 4));
+    // the descriptors of a batch live in MAPPED pinned host memory: the selection kernel stores them there itself
+    // (status word last, after a system-wide fence), the host polls -- no copy operation or event in the stream
+    NB_CUDA(c, cudaHostAlloc(&c->h_blk_ring, sizeof(double) * 4 * BLK_BATCH_MAX, cudaHostAllocMapped));
+    NB_CUDA(c, cudaHostGetDevicePointer(reinterpret_cast<void **>(&c->blk_ring), c->h_blk_ring, 0));
+    NB_CUDA(c, cudaMalloc(&c->blk_stall, sizeof(int32_t)));
+    if (!c->ev_sel) NB_CUDA(c, cudaEventCreateWithFlags(&c->ev_sel, cudaEventDisableTiming));
+    return NB_OK;
+}
+
+// buffers of a block of n bodies (the speculative chains use them: they exist before anything is enqueued)
+int blk_buffers(nb_ctx *c, int64_t n, bool lists, bool ac) {
+    const int64_t N = c->N;
+    const int64_t m = std::min<int64_t>(std::max<int64_t>(N, 1024), std::max<int64_t>(n, 1024) * 5 / 4);
+    if (n > c->blk_n) {
+        NB_CUDA(c, cudaStreamSynchronize(c->stream));
+        cudaFree(c->blk_out); cudaFree(c->blk_nnb); cudaFree(c->blk_ovf);
+        c->blk_out = nullptr; c->blk_nnb = c->blk_ovf = nullptr; c->blk_n = 0;
+        NB_CUDA(c, cudaMalloc(&c->blk_out, sizeof(double) * 7 * m));
+        NB_CUDA(c, cudaMalloc(&c->blk_nnb, sizeof(int32_t) * m));
+        NB_CUDA(c, cudaMalloc(&c->blk_ovf, sizeof(int32_t) * m));
+        c->blk_n = m;
+    }
+    if (lists && n * c->cap > c->blk_list_n) {
+        NB_CUDA(c, cudaStreamSynchronize(c->stream));
+        cudaFree(c->blk_list); c->blk_list = nullptr; c->blk_list_n = 0;
+        NB_CUDA(c, cudaMalloc(&c->blk_list, sizeof(int32_t) * m * c->cap));
+        c->blk_list_n = m * c->cap;
+    }
+    if (ac && n > c->ac_in_n) {
+        NB_CUDA(c, cudaStreamSynchronize(c->stream));
+        cudaFree(c->ac_in); c->ac_in = nullptr; c->ac_in_n = 0;
+        NB_CUDA(c, cudaMalloc(&c->ac_in, sizeof(double) * 6 * m));
+        c->ac_in_n = m;
+    }
+    return NB_OK;
+}
+
+// selection of the next block into blk_idx (and ac_reg_idx), descriptor into sel_result and ring slot `slot`
+int blk_enqueue_select(nb_ctx *c, bool two, double t_stop, int32_t spec_cap, int slot) {
+    const int64_t N = c->N;
+    const double *t0 = c->soa + 13 * c->Ns;
+    unsigned long long *key = c->blk_key + c->blk_parity, *key_next = c->blk_key + (1 - c->blk_parity);
+    double *ring = c->blk_ring + 4 * slot;
+    const unsigned nchunk = (unsigned)((N + SEL_CHUNK - 1) / SEL_CHUNK);
+    const unsigned gmin = (unsigned)std::min<int64_t>((N + 255) / 256, (int64_t)c->sm_count * 8);
+    c->blk_epoch += 1;
+    select_min_kernel<<<gmin, 256, 0, c->stream>>>(N, t0, c->dtj, key, key_next, c->blk_stall, ring);
+    if (two)
+        select_scatter_kernel<true><<<nchunk, 256, 0, c->stream>>>(N, t0, c->dtj, key, c->blk_pub, c->blk_epoch, c->blk_idx,
+                                                                   c->sel_result, c->ac.tR, c->ac.dtR, c->ac_reg_idx, t_stop,
+                                                                   spec_cap, c->blk_stall, ring);
+    else
+        select_scatter_kernel<false><<<nchunk, 256, 0, c->stream>>>(N, t0, c->dtj, key, c->blk_pub, c->blk_epoch, c->blk_idx,
+                                                                    c->sel_result, nullptr, nullptr, c->ac_reg_idx, t_stop,
+                                                                    spec_cap, c->blk_stall, ring);
+    NB_CUDA(c, cudaGetLastError());
+    c->blk_parity ^= 1;
+    c->launches += 2;
+    return NB_OK;
+}
+
+// Single-level chain of one block: a2-a7 [+ neighbour force added in place, P:49] + corrector.  spec_cap > 0:
+// speculative (n, t from the device descriptor; buffers laid out for spec_cap bodies).
+int sl_enqueue_chain(nb_ctx *c, const double *h2_all, double eta, double dt_max, int32_t n, double t, int32_t spec_cap) {
+    const int64_t stride = spec_cap > 0 ? spec_cap : n;
+    double *acc = c->blk_out, *jerk = c->blk_out + 3 * stride, *pot = c->blk_out + 6 * stride;
+    c->spec_dev = spec_cap > 0 ? c->sel_result : nullptr;
+    c->have_pred = true; c->pred_pending = true; c->pred_t = t;
+    int rc = NB_OK;
+    if (!c->fuse) rc = materialize_pred(c);
+    c->h2_by_body = 1;
+    if (rc == NB_OK)
+        rc = regular_device(c, n, c->blk_idx, h2_all, acc, jerk, pot, c->blk_nnb, h2_all ? c->blk_list : nullptr, c->blk_ovf);
+    c->h2_by_body = 0;
+    if (rc == NB_OK && h2_all) {
+        irregular_kernel<true><<<(unsigned)((n + 7) / 8), 256, 0, c->stream>>>(n, c->cap, t, c->spec_dev, 0, 0, c->blk_idx, c->blk_nnb,
+                                                                                c->blk_list, c->aos, acc, jerk, pot);
+        c->launches += 1;
+    }
+    if (rc == NB_OK) {
+        correct_kernel<<<(unsigned)((n + 127) / 128), 128, 0, c->stream>>>(n, c->Ns, t, eta, dt_max, c->spec_dev, c->blk_idx, acc,
+                                                                           jerk, c->soa, c->aos, c->dtj);
+        c->launches += 1;
+        if (cudaGetLastError() != cudaSuccess) { c->cuda_err = cudaErrorUnknown; rc = NB_ECUDA; }
+    }
+    c->spec_dev = nullptr;
+    c->have_pred = false; c->pred_pending = false;
+    c->blk_stride = stride;
+    return rc;
+}
+
+// Two-level chain of a block WITHOUT a regular step (speculative or not): neighbour force over the lists, corrector.
+int ac_enqueue_irregular_chain(nb_ctx *c, double eta_I, double eta_R, double dt_max, int32_t n, double t, bool spec) {
+    const double *dev = spec ? c->sel_result : nullptr;
+    irregular_kernel<false><<<(unsigned)((n + 7) / 8), 256, 0, c->stream>>>(n, c->cap, t, dev, 1, 1, c->blk_idx, c->ac.nnb, c->ac.list,
+                                                                            c->aos, c->ac_aIo, c->ac_jIo, nullptr);
+    ac_correct_kernel<<<(unsigned)((n + 127) / 128), 128, 0, c->stream>>>(n, c->Ns, t, eta_I, eta_R, dt_max, dev, c->blk_idx, c->ac_aIo,
+                                                                          c->ac_jIo, 0, c->ac_reg_idx, nullptr, nullptr, nullptr, nullptr,
+                                                                          c->blk_nnb, c->ac, c->soa, c->aos, c->dtj);
+    NB_CUDA(c, cudaGetLastError());
+    c->launches += 2;
+    return NB_OK;
+}
+
+// Two-level block with nr > 0 regular steps, by the ordinary launches (the lists are in blk_idx / ac_reg_idx).
+// *n_overflow > 0 and NB_EOVERFLOW: a new list overflowed; nothing was corrected (reading R38).
+int ac_finish_block(nb_ctx *c, double eta_I, double eta_R, double dt_max, double t, int32_t n, int32_t nr, int32_t *n_overflow) {
+    *n_overflow = 0;
+    int rc = blk_buffers(c, nr, true, true);
+    if (rc != NB_OK) return rc;
+    irregular_kernel<false><<<(unsigned)((n + 7) / 8), 256, 0, c->stream>>>(n, c->cap, t, nullptr, 1, 1, c->blk_idx, c->ac.nnb,
+                                                                            c->ac.list, c->aos, c->ac_aIo, c->ac_jIo, nullptr);
+    c->launches += 1;
+    double *rg_acc = c->blk_out, *rg_jerk = c->blk_out + 3 * (int64_t)nr, *rg_pot = c->blk_out + 6 * (int64_t)nr;
+    double *in_acc = c->ac_in, *in_jerk = c->ac_in + 3 * (int64_t)nr;
+    c->have_pred = true; c->pred_pending = true; c->pred_t = t;
+    if (!c->fuse) {
+        rc = materialize_pred(c);
+        if (rc != NB_OK) return rc;
+    }
+    c->h2_by_body = 1;
+    rc = regular_device(c, nr, c->ac_reg_idx, c->ac_h2, rg_acc, rg_jerk, rg_pot, c->blk_nnb, c->blk_list, c->blk_ovf);
+    c->h2_by_body = 0;
+    c->have_pred = false; c->pred_pending = false;
+    if (rc != NB_OK) return rc;
+    irregular_kernel<false><<<(unsigned)((nr + 7) / 8), 256, 0, c->stream>>>(nr, c->cap, t, nullptr, 0, 0, c->ac_reg_idx, c->blk_nnb,
+                                                                             c->blk_list, c->aos, in_acc, in_jerk, nullptr);
+    // a list that overflowed would break regular + irregular = total (R38): checked BEFORE anything is corrected
+    NB_CUDA(c, cudaMemsetAsync(c->ac_novf, 0, sizeof(int32_t), c->stream));
+    count_overflow_kernel<<<(unsigned)std::min<int64_t>((nr + 255) / 256, 1024), 256, 0, c->stream>>>(nr, c->blk_ovf, c->ac_novf);
+    NB_CUDA(c, cudaMemcpyAsync(c->h_ac_novf, c->ac_novf, sizeof(int32_t), cudaMemcpyDeviceToHost, c->stream));
+    NB_CUDA(c, cudaStreamSynchronize(c->stream));
+    c->launches += 2;
+    if (*c->h_ac_novf > 0) {
+        *n_overflow = *c->h_ac_novf;
+        return NB_EOVERFLOW;
+    }
+    ac_correct_kernel<<<(unsigned)((n + 127) / 128), 128, 0, c->stream>>>(n, c->Ns, t, eta_I, eta_R, dt_max, nullptr, c->blk_idx, c->ac_aIo,
+                                                                          c->ac_jIo, nr, c->ac_reg_idx, rg_acc, rg_jerk, in_acc, in_jerk,
+                                                                          c->blk_nnb, c->ac, c->soa, c->aos, c->dtj);
+    ac_store_rows_kernel<<<(unsigned)((nr + 7) / 8), 256, 0, c->stream>>>(nr, c->cap, c->ac_reg_idx, c->blk_nnb, c->blk_list, c->ac.list);
+    NB_CUDA(c, cudaGetLastError());
+    c->launches += 2;
+    return NB_OK;
+}
+
+struct BlockRun {
+    bool two;                         // two-level AC stepping
+    const double *h2_all;             // single level: radii by body or NULL
+    double eta, eta_R, dt_max, t_stop;
+    int64_t max_blocks;
+    // results
+    double t_next = 0.0;
+    int64_t blocks = 0, steps = 0, reg_steps = 0;
+    int32_t last_n = 0, last_nr = 0, n_overflow = 0;
+};
+
+int run_blocks(nb_ctx *c, BlockRun &R) {
+    int rc = blk_setup(c);
+    if (rc != NB_OK) return rc;
+    rc = blk_buffers(c, R.two ? 1 : 128, R.h2_all != nullptr, R.two);
+    if (rc != NB_OK) return rc;
+    rc = ensure_aos(c);
+    if (rc != NB_OK) return rc;
+    c->blk_last_n = 0;
+    while (R.blocks < R.max_blocks) {
+        // speculative capacity of this batch: two-level: any block without a regular step up to AC_SPEC_CAP bodies;
+        // single level: the size class of the last block (32 / 64 / 128: the variants with a fused predictor)
+        int32_t spec_cap = 0;
+        if (c->spec_enabled) {
+            if (R.two) spec_cap = AC_SPEC_CAP;
+            else if (c->fuse && c->blk_prev_n > 0 && c->blk_prev_n <= 128)
+                spec_cap = c->blk_prev_n <= 32 ? 32 : c->blk_prev_n <= 64 ? 64 : 128;
+        }
+        // batch size: 1 after a stall, doubled after every batch that ran without the host (a stalled batch wastes the
+        // launches behind the stall)
+        const int batch = (int)std::min<int64_t>(spec_cap > 0 ? c->blk_batch : 1, R.max_blocks - R.blocks);
+        if (c->blk_stall_dirty) {
+            NB_CUDA(c, cudaMemsetAsync(c->blk_stall, 0, sizeof(int32_t), c->stream));
+            c->blk_stall_dirty = false;
+        }
+        volatile double *hring = c->h_blk_ring;
+        for (int k = 0; k < batch; ++k) hring[4 * k + 3] = -1.0;          // "not written yet"
+        for (int k = 0; k < batch; ++k) {
+            rc = blk_enqueue_select(c, R.two, R.t_stop, spec_cap, k);
+            if (rc != NB_OK) return rc;
+            if (spec_cap > 0) {
+                rc = R.two ? ac_enqueue_irregular_chain(c, R.eta, R.eta_R, R.dt_max, spec_cap, 0.0, true)
+                           : sl_enqueue_chain(c, R.h2_all, R.eta, R.dt_max, spec_cap, 0.0, spec_cap);
+                if (rc != NB_OK) return rc;
+            }
+        }
+        // wait for the LAST selection's descriptor (not for the chain behind it); the stream is queried now and then
+        // so that a failed launch cannot leave the host spinning
+        for (uint64_t spin = 0; hring[4 * (batch - 1) + 3] < 0.0; ++spin) {
+            if ((spin & 0xfff) == 0xfff) {
+                const cudaError_t q = cudaStreamQuery(c->stream);
+                if (q != cudaSuccess && q != cudaErrorNotReady) { c->cuda_err = q; return NB_ECUDA; }
+                if (q == cudaSuccess && hring[4 * (batch - 1) + 3] < 0.0) { c->cuda_err = cudaErrorUnknown; return NB_ECUDA; }
+            }
+        }
+        std::atomic_thread_fence(std::memory_order_acquire);
+        bool stop = false;
+        for (int k = 0; k < batch && !stop; ++k) {
+            const double *d = c->h_blk_ring + 4 * k;
+            const double t = d[0];
+            const int32_t n = (int32_t)d[1], nr = (int32_t)d[2];
+            const int status = (int)d[3];
+            if (status == BLK_SKIPPED) break;                    // (cannot precede the block that stalled the batch)
+            R.t_next = t;
+            if (status == BLK_PAST_T_STOP || n <= 0) {                       // nothing is due before t_stop
+                c->blk_stall_dirty = true; c->blk_batch = 1;
+                return NB_OK;
+            }
+            if (status == BLK_SPECULATIVE) {
+                c->spec_hits += 1;
+            } else {                                             // BLK_NEEDS_HOST: the lists are in place, finish it here
+                if (spec_cap > 0) c->spec_misses += 1;
+                if (R.two) {
+                    if (nr == 0) rc = ac_enqueue_irregular_chain(c, R.eta, R.eta_R, R.dt_max, n, t, false);
+                    else rc = ac_finish_block(c, R.eta, R.eta_R, R.dt_max, t, n, nr, &R.n_overflow);
+                } else {
+                    rc = blk_buffers(c, n, R.h2_all != nullptr, false);
+                    if (rc == NB_OK) rc = sl_enqueue_chain(c, R.h2_all, R.eta, R.dt_max, n, t, 0);
+                }
+                if (rc != NB_OK) { c->blk_stall_dirty = true; c->blk_batch = 1; return rc; }
+                stop = true;                                     // the rest of the batch did nothing
+            }
+            R.blocks += 1; R.steps += n; R.reg_steps += nr;
+            R.last_n = n; R.last_nr = nr;
+            c->blk_prev_n = n;
+            c->blk_last_n = n;
+            c->blk_had_list = !R.two && R.h2_all != nullptr;
+        }
+        if (stop) { c->blk_stall_dirty = true; c->blk_batch = 1; }
+        else if (spec_cap > 0) c->blk_batch = std::min(2 * c->blk_batch, BLK_BATCH_MAX);
+    }
+    return NB_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
 int nb_block_step(nb_ctx *c, const double *h2_all, double eta, double dt_max, double t_stop, double *t_next,
                   int32_t *n_act) {
     int rc = check_live(c);
     if (rc != NB_OK) return rc;
     if (!t_next || !n_act || !(eta > 0.0) || !(dt_max > 0.0)) return NB_EINVAL;
     if (!c->have_j || !c->have_steps) return NB_ESTATE;
-    const int64_t N = c->N;
-    const int nchunk = (int)((N + SEL_CHUNK - 1) / SEL_CHUNK);
-    if (!c->blk_key) {
-        NB_CUDA(c, cudaMalloc(&c->blk_key, 2 * sizeof(unsigned long long)));
-        NB_CUDA(c, cudaMemsetAsync(c->blk_key, 0xff, 2 * sizeof(unsigned long long), c->stream));
-        NB_CUDA(c, cudaMalloc(&c->blk_idx, sizeof(int32_t) * N));
-        if (!c->sel_counts) NB_CUDA(c, cudaMalloc(&c->sel_counts, sizeof(int32_t) * nchunk));
-        if (!c->sel_result) NB_CUDA(c, cudaMalloc(&c->sel_result, sizeof(double) * 4));
-        if (!c->h_sel_result) NB_CUDA(c, cudaMallocHost(&c->h_sel_result, sizeof(double) * 4));
-        int per_sm = 0;
-        NB_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, select_block_kernel<false>, 256, 0));
-        c->blk_grid = std::max(1, std::min(nchunk, per_sm * c->sm_count));
-    }
-    if (!c->ev_sel) NB_CUDA(c, cudaEventCreateWithFlags(&c->ev_sel, cudaEventDisableTiming));
-    // buffers for blocks of up to 1024 bodies exist before anything is enqueued (the speculative chain uses them)
-    auto ensure_block_buffers = [&](int64_t n, bool lists) -> int {
-        if (n > c->blk_n) {
-            NB_CUDA(c, cudaStreamSynchronize(c->stream));
-            cudaFree(c->blk_out); cudaFree(c->blk_nnb); cudaFree(c->blk_ovf);
-            c->blk_out = nullptr; c->blk_nnb = c->blk_ovf = nullptr; c->blk_n = 0;
-            const int64_t m = std::min<int64_t>(std::max<int64_t>(N, 1024), std::max<int64_t>(n, 1024) * 5 / 4);
-            NB_CUDA(c, cudaMalloc(&c->blk_out, sizeof(double) * 7 * m));
-            NB_CUDA(c, cudaMalloc(&c->blk_nnb, sizeof(int32_t) * m));
-            NB_CUDA(c, cudaMalloc(&c->blk_ovf, sizeof(int32_t) * m));
-            c->blk_n = m;
-        }
-        if (lists && n * c->cap > c->blk_list_n) {
-            NB_CUDA(c, cudaStreamSynchronize(c->stream));
-            cudaFree(c->blk_list); c->blk_list = nullptr; c->blk_list_n = 0;
-            const int64_t m = std::min<int64_t>(std::max<int64_t>(N, 1024), std::max<int64_t>(n, 1024) * 5 / 4) * c->cap;
-            NB_CUDA(c, cudaMalloc(&c->blk_list, sizeof(int32_t) * m));
-            c->blk_list_n = m;
-        }
-        return NB_OK;
-    };
-    rc = ensure_block_buffers(128, h2_all != nullptr);
+    BlockRun R = {false, h2_all, eta, 0.0, dt_max, t_stop, 1};
+    rc = run_blocks(c, R);
+    *t_next = R.t_next;
+    *n_act = R.blocks ? R.last_n : 0;
+    return rc;
+}
+
+int nb_run_blocks(nb_ctx *c, const double *h2_all, double eta, double dt_max, double t_stop, int64_t max_blocks,
+                  double *t_next, int64_t *blocks, int64_t *particle_steps) {
+    int rc = check_live(c);
     if (rc != NB_OK) return rc;
-    rc = ensure_aos(c);
-    if (rc != NB_OK) return rc;
-    // ---- selection: ONE cooperative launch; its {t_next, n} goes to the host (the launch plan of a large
-    //      block needs n) and stays in device memory for the speculative chain below
-    {
-        const double *t0 = c->soa + 13 * c->Ns;
-        const double *dtj = c->dtj;
-        unsigned long long *key = c->blk_key + c->blk_parity, *key_next = c->blk_key + (1 - c->blk_parity);
-        int64_t Nn = N;
-        const double *nul_d = nullptr;
-        int32_t *nul_i = nullptr;
-        void *args[] = {&Nn, &t0, &dtj, &key, &key_next, &c->sel_counts, &c->blk_idx, &c->sel_result, &nul_d, &nul_d, &nul_i, &nul_i};
-        NB_CUDA(c, cudaLaunchCooperativeKernel((const void *)select_block_kernel<false>, dim3(c->blk_grid), dim3(256), args, 0,
-                                               c->stream));
-        c->blk_parity ^= 1;
-        c->launches += 1;
-        NB_CUDA(c, cudaMemcpyAsync(c->h_sel_result, c->sel_result, sizeof(double) * 2, cudaMemcpyDeviceToHost, c->stream));
-        NB_CUDA(c, cudaEventRecord(c->ev_sel, c->stream));
-    }
-    // One block's chain a2-a7 + neighbour force + corrector.  spec_cap > 0: SPECULATIVE -- enqueued before the
-    // host knows the block: the kernels read {t, n} from device memory and do nothing unless n <= spec_cap and
-    // t <= t_stop, so the GPU goes from the selection straight into the force kernel while the host is still
-    // waiting for the read-back (deep blocks hold few particles -- the common case).
-    auto enqueue_chain = [&](int32_t n, double t, int32_t spec_cap) -> int {
-        const int64_t stride = spec_cap > 0 ? spec_cap : n;
-        double *acc = c->blk_out, *jerk = c->blk_out + 3 * stride, *pot = c->blk_out + 6 * stride;
-        c->spec_dev = spec_cap > 0 ? c->sel_result : nullptr;
-        c->spec_t_stop = t_stop;
-        c->have_pred = true; c->pred_pending = true; c->pred_t = t;
-        int rc2 = NB_OK;
-        if (!c->fuse) rc2 = materialize_pred(c);
-        c->h2_by_body = 1;
-        if (rc2 == NB_OK)
-            rc2 = regular_device(c, n, c->blk_idx, h2_all, acc, jerk, pot, c->blk_nnb, h2_all ? c->blk_list : nullptr, c->blk_ovf);
-        c->h2_by_body = 0;
-        if (rc2 == NB_OK && h2_all) {   // the neighbour force on the lists just written, added in place
-            irregular_kernel<true><<<(unsigned)((n + 7) / 8), 256, 0, c->stream>>>(n, c->cap, t, c->spec_dev, t_stop, 0, 0, c->blk_idx,
-                                                                                    c->blk_nnb, c->blk_list, c->aos, acc, jerk, pot);
-            c->launches += 1;
-        }
-        if (rc2 == NB_OK) {
-            correct_kernel<<<(unsigned)((n + 127) / 128), 128, 0, c->stream>>>(n, c->Ns, t, eta, dt_max, c->spec_dev, t_stop,
-                                                                               c->blk_idx, acc, jerk, c->soa, c->aos, c->dtj);
-            c->launches += 1;
-            if (cudaGetLastError() != cudaSuccess) rc2 = NB_ECUDA;
-        }
-        c->spec_dev = nullptr;
-        c->have_pred = false; c->pred_pending = false;
-        c->blk_stride = stride;
-        return rc2;
-    };
-    // speculate on the size class of the previous block (32 / 64 / 128: the variants with a fused predictor)
-    int32_t spec_cap = 0;
-    if (c->fuse && c->spec_enabled && t_stop >= 0.0 && c->blk_prev_n > 0 && c->blk_prev_n <= 128)
-        spec_cap = c->blk_prev_n <= 32 ? 32 : c->blk_prev_n <= 64 ? 64 : 128;
-    if (spec_cap > 0) {
-        rc = enqueue_chain(spec_cap, 0.0, spec_cap);
-        if (rc != NB_OK) return rc;
-    }
-    NB_CUDA(c, cudaEventSynchronize(c->ev_sel));
-    const double t = c->h_sel_result[0];
-    const int32_t n = (int32_t)c->h_sel_result[1];
-    *t_next = t;
-    *n_act = 0;
-    c->blk_last_n = 0;
-    if (t > t_stop || n <= 0) return NB_OK;          // nothing is due before t_stop: the state is untouched
-    c->blk_prev_n = n;
-    if (spec_cap > 0 && n <= spec_cap) {
-        c->spec_hits += 1;                           // the speculative chain is this block
-    } else {
-        if (spec_cap > 0) c->spec_misses += 1;       // those launches were no-ops
-        rc = ensure_block_buffers(n, h2_all != nullptr);
-        if (rc != NB_OK) return rc;
-        rc = enqueue_chain(n, t, 0);
-        if (rc != NB_OK) return rc;
-    }
-    c->blk_last_n = n;
-    c->blk_had_list = h2_all != nullptr;
-    *n_act = n;
-    return NB_OK;
+    if (!t_next || !blocks || !particle_steps || max_blocks < 0 || !(eta > 0.0) || !(dt_max > 0.0)) return NB_EINVAL;
+    if (!c->have_j || !c->have_steps) return NB_ESTATE;
+    BlockRun R = {false, h2_all, eta, 0.0, dt_max, t_stop, max_blocks};
+    rc = run_blocks(c, R);
+    *t_next = R.t_next; *blocks = R.blocks; *particle_steps = R.steps;
+    return rc;
 }
 
 int nb_ac_init(nb_ctx *c, double t_start, const double *h2_all, double eta_s, double dt_max, int32_t *n_overflow) {
@@ -1067,7 +1244,6 @@ int nb_ac_init(nb_ctx *c, double t_start, const double *h2_all, double eta_s, do
     if (!c->have_j) return NB_ESTATE;
     if (c->j_offset != 0) return NB_ESTATE;
     const int64_t N = c->N;
-    const int nchunk = (int)((N + SEL_CHUNK - 1) / SEL_CHUNK);
     if (!c->ac.aI) {
         const size_t v3 = sizeof(double) * 3 * N;
         NB_CUDA(c, cudaMalloc(&c->ac.aI, v3)); NB_CUDA(c, cudaMalloc(&c->ac.jI, v3));
@@ -1077,24 +1253,12 @@ int nb_ac_init(nb_ctx *c, double t_start, const double *h2_all, double eta_s, do
         NB_CUDA(c, cudaMalloc(&c->ac_h2, sizeof(double) * N));
         NB_CUDA(c, cudaMalloc(&c->ac.nnb, sizeof(int32_t) * N));
         NB_CUDA(c, cudaMalloc(&c->ac.list, sizeof(int32_t) * N * c->cap));
-        NB_CUDA(c, cudaMalloc(&c->ac_reg_idx, sizeof(int32_t) * N));
-        NB_CUDA(c, cudaMalloc(&c->ac_counts2, sizeof(int32_t) * nchunk));
         NB_CUDA(c, cudaMalloc(&c->ac_novf, sizeof(int32_t)));
         NB_CUDA(c, cudaMallocHost(&c->h_ac_novf, sizeof(int32_t)));
         if (!c->dtj) NB_CUDA(c, cudaMalloc(&c->dtj, sizeof(double) * N));
-        if (!c->blk_key) {
-            NB_CUDA(c, cudaMalloc(&c->blk_key, 2 * sizeof(unsigned long long)));
-            NB_CUDA(c, cudaMemsetAsync(c->blk_key, 0xff, 2 * sizeof(unsigned long long), c->stream));
-            NB_CUDA(c, cudaMalloc(&c->blk_idx, sizeof(int32_t) * N));
-        }
-        if (!c->sel_counts) NB_CUDA(c, cudaMalloc(&c->sel_counts, sizeof(int32_t) * nchunk));
-        if (!c->sel_result) NB_CUDA(c, cudaMalloc(&c->sel_result, sizeof(double) * 4));
-        if (!c->h_sel_result) NB_CUDA(c, cudaMallocHost(&c->h_sel_result, sizeof(double) * 4));
-        int per_sm = 0;
-        NB_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, select_block_kernel<true>, 256, 0));
-        c->ac_grid = std::max(1, std::min(nchunk, per_sm * c->sm_count));
-        if (!c->ev_sel) NB_CUDA(c, cudaEventCreateWithFlags(&c->ev_sel, cudaEventDisableTiming));
     }
+    rc = blk_setup(c);
+    if (rc != NB_OK) return rc;
     NB_CUDA(c, cudaMemcpyAsync(c->ac_h2, h2_all, sizeof(double) * N, cudaMemcpyDeviceToDevice, c->stream));
     // forces at t_start: every t0[j] must equal t_start, so the prediction is the state itself
     c->have_pred = true; c->pred_pending = true; c->pred_t = t_start;
@@ -1104,7 +1268,7 @@ int nb_ac_init(nb_ctx *c, double t_start, const double *h2_all, double eta_s, do
     rc = regular_device(c, (int32_t)N, nullptr, c->ac_h2, c->ac.aR, c->ac.jR, c->ac_aIo /* pot: scratch */, c->ac.nnb,
                         c->ac.list, ovf_all);
     if (rc != NB_OK) return rc;
-    irregular_kernel<false><<<(unsigned)((N + 7) / 8), 256, 0, c->stream>>>((int32_t)N, c->cap, t_start, nullptr, 0.0, 0, 0, nullptr,
+    irregular_kernel<false><<<(unsigned)((N + 7) / 8), 256, 0, c->stream>>>((int32_t)N, c->cap, t_start, nullptr, 0, 0, nullptr,
                                                                             c->ac.nnb, c->ac.list, c->aos, c->ac.aI, c->ac.jI, nullptr);
     NB_CUDA(c, cudaMemsetAsync(c->ac_novf, 0, sizeof(int32_t), c->stream));
     ac_start_kernel<<<(unsigned)((N + 127) / 128), 128, 0, c->stream>>>(N, c->Ns, c->cap, t_start, eta_s, dt_max, c->ac, c->soa,
@@ -1126,144 +1290,24 @@ int nb_ac_step(nb_ctx *c, double eta_I, double eta_R, double dt_max, double t_st
     if (rc != NB_OK) return rc;
     if (!t_next || !n_irr || !n_reg || !(eta_I > 0.0) || !(eta_R > 0.0) || !(dt_max > 0.0)) return NB_EINVAL;
     if (!c->have_ac) return NB_ESTATE;
-    const int64_t N = c->N;
-    {   // selection: active = irregular step due; among them the bodies whose regular step is due too
-        const double *t0 = c->soa + 13 * c->Ns;
-        const double *dtj = c->dtj, *tR = c->ac.tR, *dtR = c->ac.dtR;
-        unsigned long long *key = c->blk_key + c->blk_parity, *key_next = c->blk_key + (1 - c->blk_parity);
-        int64_t Nn = N;
-        void *args[] = {&Nn, &t0, &dtj, &key, &key_next, &c->sel_counts, &c->blk_idx, &c->sel_result, &tR, &dtR,
-                        &c->ac_counts2, &c->ac_reg_idx};
-        NB_CUDA(c, cudaLaunchCooperativeKernel((const void *)select_block_kernel<true>, dim3(c->ac_grid), dim3(256), args, 0,
-                                               c->stream));
-        c->blk_parity ^= 1;
-        c->launches += 1;
-        NB_CUDA(c, cudaMemcpyAsync(c->h_sel_result, c->sel_result, sizeof(double) * 3, cudaMemcpyDeviceToHost, c->stream));
-        NB_CUDA(c, cudaEventRecord(c->ev_sel, c->stream));
-    }
-    // Most blocks of the two-level scheme hold a few bodies and NO regular step (irregular steps are the
-    // small ones).  Their chain -- neighbour force over the lists, corrector -- is enqueued before the host knows
-    // the block: the kernels take {t, n, n_reg} from device memory and do nothing unless n <= AC_SPEC_CAP,
-    // n_reg = 0 and t <= t_stop, so the GPU does not idle while the host waits for the read-back.
-    constexpr int32_t AC_SPEC_CAP = 1024;
-    const bool spec = c->spec_enabled && t_stop >= 0.0;
-    if (spec) {
-        const double ts_enc = -std::max(t_stop, 4.9406564584124654e-324);     // negative: "and no regular step due"
-        irregular_kernel<false><<<(AC_SPEC_CAP + 7) / 8, 256, 0, c->stream>>>(AC_SPEC_CAP, c->cap, 0.0, c->sel_result, ts_enc, 1, 1,
-                                                                              c->blk_idx, c->ac.nnb, c->ac.list, c->aos, c->ac_aIo,
-                                                                              c->ac_jIo, nullptr);
-        ac_correct_kernel<<<(AC_SPEC_CAP + 127) / 128, 128, 0, c->stream>>>(AC_SPEC_CAP, c->Ns, 0.0, eta_I, eta_R, dt_max, c->sel_result,
-                                                                            ts_enc, c->blk_idx, c->ac_aIo, c->ac_jIo, 0, c->ac_reg_idx,
-                                                                            nullptr, nullptr, nullptr, nullptr, c->blk_nnb, c->ac, c->soa,
-                                                                            c->aos, c->dtj);
-        NB_CUDA(c, cudaGetLastError());
-        c->launches += 2;
-    }
-    NB_CUDA(c, cudaEventSynchronize(c->ev_sel));
-    const double t = c->h_sel_result[0];
-    const int32_t n = (int32_t)c->h_sel_result[1], nr = (int32_t)c->h_sel_result[2];
-    *t_next = t; *n_irr = 0; *n_reg = 0;
-    c->blk_last_n = 0;
-    if (t > t_stop || n <= 0) return NB_OK;
-    if (spec && nr == 0 && n <= AC_SPEC_CAP) {      // the speculative chain was this block
-        c->spec_hits += 1;
-        c->have_pred = false; c->pred_pending = false;
-        *n_irr = n;
-        return NB_OK;
-    }
-    if (spec) c->spec_misses += 1;
-    // irregular force over the OLD lists of every active body (rows and outputs by body)
-    irregular_kernel<false><<<(unsigned)((n + 7) / 8), 256, 0, c->stream>>>(n, c->cap, t, nullptr, 0.0, 1, 1, c->blk_idx, c->ac.nnb,
-                                                                            c->ac.list, c->aos, c->ac_aIo, c->ac_jIo, nullptr);
-    c->launches += 1;
-    double *rg_acc = nullptr, *rg_jerk = nullptr, *in_acc = nullptr, *in_jerk = nullptr;
-    if (nr > 0) {
-        // block buffers for the regular-active bodies: regular force / lists (new), irregular force over the new lists
-        if (nr > c->blk_n) {
-            cudaFree(c->blk_out); cudaFree(c->blk_nnb); cudaFree(c->blk_ovf);
-            c->blk_out = nullptr; c->blk_nnb = c->blk_ovf = nullptr; c->blk_n = 0;
-            const int64_t m = std::min<int64_t>(std::max<int64_t>(N, 1024), std::max<int64_t>(nr, 1024) * 5 / 4);
-            NB_CUDA(c, cudaMalloc(&c->blk_out, sizeof(double) * 7 * m));
-            NB_CUDA(c, cudaMalloc(&c->blk_nnb, sizeof(int32_t) * m));
-            NB_CUDA(c, cudaMalloc(&c->blk_ovf, sizeof(int32_t) * m));
-            c->blk_n = m;
-        }
-        if ((int64_t)nr * c->cap > c->blk_list_n) {
-            cudaFree(c->blk_list); c->blk_list = nullptr; c->blk_list_n = 0;
-            const int64_t m = std::min<int64_t>(std::max<int64_t>(N, 1024), std::max<int64_t>(nr, 1024) * 5 / 4) * c->cap;
-            NB_CUDA(c, cudaMalloc(&c->blk_list, sizeof(int32_t) * m));
-            c->blk_list_n = m;
-        }
-        if (nr > c->ac_in_n) {
-            cudaFree(c->ac_in); c->ac_in = nullptr; c->ac_in_n = 0;
-            const int64_t m = std::min<int64_t>(std::max<int64_t>(N, 1024), std::max<int64_t>(nr, 1024) * 5 / 4);
-            NB_CUDA(c, cudaMalloc(&c->ac_in, sizeof(double) * 6 * m));
-            c->ac_in_n = m;
-        }
-        rg_acc = c->blk_out; rg_jerk = c->blk_out + 3 * (int64_t)nr;
-        double *rg_pot = c->blk_out + 6 * (int64_t)nr;
-        in_acc = c->ac_in; in_jerk = c->ac_in + 3 * (int64_t)nr;
-        c->have_pred = true; c->pred_pending = true; c->pred_t = t;
-        if (!c->fuse) {
-            rc = materialize_pred(c);
-            if (rc != NB_OK) return rc;
-        }
-        c->h2_by_body = 1;
-        rc = regular_device(c, nr, c->ac_reg_idx, c->ac_h2, rg_acc, rg_jerk, rg_pot, c->blk_nnb, c->blk_list, c->blk_ovf);
-        c->h2_by_body = 0;
-        if (rc != NB_OK) return rc;
-        irregular_kernel<false><<<(unsigned)((nr + 7) / 8), 256, 0, c->stream>>>(nr, c->cap, t, nullptr, 0.0, 0, 0, c->ac_reg_idx,
-                                                                                 c->blk_nnb, c->blk_list, c->aos, in_acc, in_jerk, nullptr);
-        // a list that overflowed would break regular + irregular = total (R38): checked BEFORE anything is corrected
-        NB_CUDA(c, cudaMemsetAsync(c->ac_novf, 0, sizeof(int32_t), c->stream));
-        count_overflow_kernel<<<(unsigned)std::min<int64_t>((nr + 255) / 256, 1024), 256, 0, c->stream>>>(nr, c->blk_ovf, c->ac_novf);
-        NB_CUDA(c, cudaMemcpyAsync(c->h_ac_novf, c->ac_novf, sizeof(int32_t), cudaMemcpyDeviceToHost, c->stream));
-        NB_CUDA(c, cudaStreamSynchronize(c->stream));
-        c->launches += 2;
-        c->have_pred = false; c->pred_pending = false;
-        if (*c->h_ac_novf > 0) {
-            *n_reg = *c->h_ac_novf;                 // the number of overflowed rows; the state is untouched
-            return NB_EOVERFLOW;
-        }
-    }
-    ac_correct_kernel<<<(unsigned)((n + 127) / 128), 128, 0, c->stream>>>(n, c->Ns, t, eta_I, eta_R, dt_max, nullptr, 0.0, c->blk_idx, c->ac_aIo,
-                                                                          c->ac_jIo, nr, c->ac_reg_idx, rg_acc, rg_jerk, in_acc,
-                                                                          in_jerk, c->blk_nnb, c->ac, c->soa, c->aos, c->dtj);
-    if (nr > 0)
-        ac_store_rows_kernel<<<(unsigned)((nr + 7) / 8), 256, 0, c->stream>>>(nr, c->cap, c->ac_reg_idx, c->blk_nnb, c->blk_list,
-                                                                              c->ac.list);
-    NB_CUDA(c, cudaGetLastError());
-    c->launches += nr > 0 ? 2 : 1;
-    c->have_pred = false; c->pred_pending = false;
-    *n_irr = n; *n_reg = nr;
-    return NB_OK;
+    BlockRun R = {true, nullptr, eta_I, eta_R, dt_max, t_stop, 1};
+    rc = run_blocks(c, R);
+    *t_next = R.t_next;
+    *n_irr = R.blocks ? R.last_n : 0;
+    *n_reg = rc == NB_EOVERFLOW ? R.n_overflow : (R.blocks ? R.last_nr : 0);
+    return rc;
 }
 
 int nb_ac_run(nb_ctx *c, double eta_I, double eta_R, double dt_max, double t_stop, int64_t max_blocks, double *t_next,
               int64_t *blocks, int64_t *irregular_steps, int64_t *regular_steps) {
+    int rc = check_live(c);
+    if (rc != NB_OK) return rc;
     if (!t_next || !blocks || !irregular_steps || !regular_steps || max_blocks < 0) return NB_EINVAL;
-    *blocks = *irregular_steps = *regular_steps = 0;
-    int rc = NB_OK;
-    while (*blocks < max_blocks) {
-        int32_t ni = 0, nr = 0;
-        rc = nb_ac_step(c, eta_I, eta_R, dt_max, t_stop, t_next, &ni, &nr);
-        if (rc != NB_OK || ni == 0) break;          // error, or nothing due before t_stop
-        *blocks += 1; *irregular_steps += ni; *regular_steps += nr;
-    }
-    return rc;
-}
-
-int nb_run_blocks(nb_ctx *c, const double *h2_all, double eta, double dt_max, double t_stop, int64_t max_blocks,
-                  double *t_next, int64_t *blocks, int64_t *particle_steps) {
-    if (!t_next || !blocks || !particle_steps || max_blocks < 0) return NB_EINVAL;
-    *blocks = *particle_steps = 0;
-    int rc = NB_OK;
-    while (*blocks < max_blocks) {
-        int32_t n = 0;
-        rc = nb_block_step(c, h2_all, eta, dt_max, t_stop, t_next, &n);
-        if (rc != NB_OK || n == 0) break;
-        *blocks += 1; *particle_steps += n;
-    }
+    if (!(eta_I > 0.0) || !(eta_R > 0.0) || !(dt_max > 0.0)) return NB_EINVAL;
+    if (!c->have_ac) return NB_ESTATE;
+    BlockRun R = {true, nullptr, eta_I, eta_R, dt_max, t_stop, max_blocks};
+    rc = run_blocks(c, R);
+    *t_next = R.t_next; *blocks = R.blocks; *irregular_steps = R.steps; *regular_steps = R.reg_steps;
     return rc;
 }
 

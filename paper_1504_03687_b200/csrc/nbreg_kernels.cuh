@@ -17,7 +17,6 @@
 // close together (relative to their neighbour radii) differences in its OWN frame instead: one add per
 // component (see force_kernel).  Small blocks read the FP64 state directly and predict in the kernel.
 #pragma once
-#include <cooperative_groups.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -458,23 +457,18 @@ struct ForceParams {
     int32_t *nblist;              // caller's [n_i][cap], or NULL: neighbours are only counted
     double *partial;              // [S][7][n_i_pad]
     unsigned int *stats;          // NULL, or {warps in the local frame, warps} (diagnostics; integer atomics)
-    const double *blk_dev;        // NULL, or {t_next, n_active} written by select_block_kernel: a SPECULATIVE launch of
-    double t_stop;                // nb_block_step -- the block's time and size come from device memory; the launch is
-                                  // a no-op if the block is larger than n_i (its capacity) or not due before t_stop
+    const double *blk_dev;        // NULL, or the block descriptor {t_next, n_active, n_regular, status} written by
+                                  // select_block_kernel: a SPECULATIVE launch of nb_block_step / nb_ac_step -- the block's
+                                  // time and size come from device memory and the launch is a no-op unless status = 1
 };
+// Status of a selected block: may the speculative chain enqueued behind the selection integrate it?
+enum { BLK_SKIPPED = 0, BLK_SPECULATIVE = 1, BLK_NEEDS_HOST = 2, BLK_PAST_T_STOP = 3 };
 // The block a speculative launch works on: false = nothing to do.  n and t are overwritten from blk_dev.
-// t_stop < 0 encodes "and only if NO regular step is due in this block" (two-level AC stepping: blk_dev[2] = 0)
-// with the real bound -t_stop (block times are >= 0).
-__device__ __forceinline__ bool spec_block(const double *blk_dev, double t_stop, int32_t &n, double &t) {
+__device__ __forceinline__ bool spec_block(const double *blk_dev, int32_t &n, double &t) {
     if (!blk_dev) return true;
-    const double tn = blk_dev[0];
-    const int32_t nd = (int32_t)blk_dev[1];
-    if (t_stop < 0.0) {
-        if (blk_dev[2] != 0.0) return false;
-        t_stop = -t_stop;
-    }
-    if (tn > t_stop || nd > n || nd <= 0) return false;
-    n = nd; t = tn;
+    if (blk_dev[3] != (double)BLK_SPECULATIVE) return false;
+    t = blk_dev[0];
+    n = (int32_t)blk_dev[1];
     return true;
 }
 
@@ -687,7 +681,7 @@ __global__ void __launch_bounds__(32 * WI *WJ, MINB) force_kernel(const ForcePar
     const int wi = warp % WI, wj = warp / WI;
     int32_t n_i = p.n_i;
     double t_pred = p.t;
-    if (!spec_block(p.blk_dev, p.t_stop, n_i, t_pred)) return;    // (uniform over the grid, before any barrier)
+    if (!spec_block(p.blk_dev, n_i, t_pred)) return;    // (uniform over the grid, before any barrier)
 
     const int tile_begin = p.tile0 + blockIdx.y * p.tiles_per_split;
     const int tile_end = min(tile_begin + p.tiles_per_split, p.ntiles);
@@ -1032,7 +1026,7 @@ __global__ void __launch_bounds__(32 * WI *WJ, MINB) force_kernel(const ForcePar
 template <int W>
 __global__ void __launch_bounds__(32 * W) finalize_kernel(int32_t n_i, int32_t n_i_pad, int32_t S, int32_t cap,
                                                           int32_t sortP, const unsigned long long *__restrict__ perm,
-                                                          const double *__restrict__ blk_dev, double t_stop,
+                                                          const double *__restrict__ blk_dev,
                                                           const double *__restrict__ partial,
                                                           int32_t *__restrict__ cnt, double *__restrict__ acc,
                                                           double *__restrict__ jerk, double *__restrict__ pot,
@@ -1049,7 +1043,7 @@ __global__ void __launch_bounds__(32 * W) finalize_kernel(int32_t n_i, int32_t n
     TL_STAMP(4096 + blockIdx.y * gridDim.x + blockIdx.x, 1);
     {
         double t_unused = 0.0;
-        if (!spec_block(blk_dev, t_stop, n_i, t_unused)) return;
+        if (!spec_block(blk_dev, n_i, t_unused)) return;
     }
     if (blockIdx.y < 7) {
         const int q = blockIdx.y;
@@ -1140,7 +1134,7 @@ __device__ __forceinline__ BodyD predict_body(const double *__restrict__ aos, in
 // indexed by BODY (the persistent lists and scratch of the two-level AC stepping) instead of by k.
 template <bool ACCUM>
 __global__ void __launch_bounds__(256) irregular_kernel(int32_t n_i, int32_t cap, double t,
-                                                        const double *__restrict__ blk_dev, double t_stop,
+                                                        const double *__restrict__ blk_dev,
                                                         int32_t rows_by_body, int32_t out_by_body,
                                                         const int32_t *__restrict__ idx_i,
                                                         const int32_t *__restrict__ nnb,
@@ -1149,7 +1143,7 @@ __global__ void __launch_bounds__(256) irregular_kernel(int32_t n_i, int32_t cap
                                                         double *__restrict__ jerk, double *__restrict__ pot) {
     const int lane = threadIdx.x & 31;
     const int k = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-    if (!spec_block(blk_dev, t_stop, n_i, t)) return;
+    if (!spec_block(blk_dev, n_i, t)) return;
     if (k >= n_i) return;
     const int32_t i = idx_i ? idx_i[k] : k;
     const BodyD I = predict_body(aos, i, t);
@@ -1288,108 +1282,113 @@ __global__ void __launch_bounds__(256) select_active_kernel(int64_t N, const dou
     }
 }
 
-// The same selection as ONE cooperative launch (nb_block_step): grid-stride over the 2048-body chunks,
-// grid.sync() between the three phases; `key` is this call's minimum slot (~0 on entry), `key_next` the
-// other slot, reset here for the next call.  result = {t_next, n_active}.
-// TWO (two-level AC stepping): among the active bodies those whose REGULAR step is due as well
-// (tR_j + dtR_j == t_next) are also listed, ascending, in idx_reg; result[2] = their number.
-template <bool TWO>
-__global__ void __launch_bounds__(256) select_block_kernel(int64_t N, const double *__restrict__ t0,
-                                                           const double *__restrict__ dtj, unsigned long long *key,
-                                                           unsigned long long *key_next, int32_t *__restrict__ counts,
-                                                           int32_t *__restrict__ idx_act, double *__restrict__ result,
-                                                           const double *__restrict__ tR, const double *__restrict__ dtR,
-                                                           int32_t *__restrict__ counts2, int32_t *__restrict__ idx_reg) {
-    namespace cg = cooperative_groups;
-    cg::grid_group grid = cg::this_grid();
-    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    const int nchunk = (int)((N + SEL_CHUNK - 1) / SEL_CHUNK);
-    __shared__ unsigned long long wbest[8];
-    __shared__ int32_t wsum[8], wsum2[8];
-    __shared__ int32_t base_s, base2_s;
-    // ---- phase 1: t_next = min_j (t0_j + dt_j).  The CTA's FIRST chunk stays in registers for the other two
-    //      phases (at N <= grid x 2048 that is everything: one pass over memory instead of three).
-    constexpr int PER = SEL_CHUNK / 256;
-    double first[PER];
-    unsigned long long best = ~0ull;
-#pragma unroll
-    for (int u = 0; u < PER; ++u) {
-        const int64_t j = (int64_t)blockIdx.x * SEL_CHUNK + u * 256 + threadIdx.x;
-        first[u] = (blockIdx.x < nchunk && j < N) ? t0[j] + dtj[j] : __longlong_as_double(0x7ff8000000000000ll);   // NaN: never due
-        if (first[u] == first[u]) best = min(best, ordered_key(first[u]));
-    }
-    for (int b = blockIdx.x + gridDim.x; b < nchunk; b += gridDim.x)
-        for (int s = 0; s < SEL_CHUNK; s += 256) {
-            const int64_t j = (int64_t)b * SEL_CHUNK + s + threadIdx.x;
-            if (j < N) best = min(best, ordered_key(t0[j] + dtj[j]));
+// The selection of the block loop (nb_block_step / nb_ac_step and their loops): TWO ordinary launches, no grid-wide
+// synchronisation.  (1) select_min_kernel: t_next = min_j (t0_j + dt_j) into `key` (~0 on entry; the other slot is
+// reset for the next call).  (2) select_scatter_kernel: one CTA per 2048-body chunk counts its active bodies,
+// publishes the count tagged with this call's epoch, sums the counts of the chunks before it as they appear
+// (decoupled look-back: lower chunks are scheduled first and never wait for higher ones) and writes its bodies
+// in ascending order; the last chunk writes the block descriptor {t_next, n, n_regular, status} to device memory
+// and to the host's ring.  TWO (two-level AC stepping): the active bodies whose REGULAR step is due as well
+// (tR_j + dtR_j == t_next) are also listed, ascending, in idx_reg.
+// A BATCH of blocks is enqueued without the host in between: once a block needs the host (too large for the
+// speculative chain, a regular step due, past t_stop) `*stall` is set and every later selection of the batch does
+// nothing, so that block's lists stay in place.  (The flag is written by an EARLIER kernel only.)
+__global__ void __launch_bounds__(256) select_min_kernel(int64_t N, const double *__restrict__ t0,
+                                                         const double *__restrict__ dtj, unsigned long long *key,
+                                                         unsigned long long *key_next, const int32_t *stall,
+                                                         double *__restrict__ ring) {
+    if (*stall) {
+        if (blockIdx.x == 0 && threadIdx.x == 0) {
+            *key_next = ~0ull;
+            *reinterpret_cast<volatile double *>(ring + 3) = (double)BLK_SKIPPED;
         }
+        return;
+    }
+    unsigned long long best = ~0ull;
+    for (int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; j < N; j += (int64_t)gridDim.x * blockDim.x)
+        best = min(best, ordered_key(t0[j] + dtj[j]));
 #pragma unroll
     for (int off = 16; off > 0; off >>= 1) best = min(best, __shfl_xor_sync(0xffffffffu, best, off));
-    if (lane == 0) wbest[w] = best;
+    __shared__ unsigned long long wbest[8];
+    if ((threadIdx.x & 31) == 0) wbest[threadIdx.x >> 5] = best;
     __syncthreads();
     if (threadIdx.x == 0) {
 #pragma unroll
-        for (int q = 1; q < 8; ++q) best = min(best, wbest[q]);
+        for (int w = 1; w < 8; ++w) best = min(best, wbest[w]);
         atomicMin(key, best);
         if (blockIdx.x == 0) *key_next = ~0ull;
     }
-    grid.sync();
+}
+
+template <bool TWO>
+__global__ void __launch_bounds__(256) select_scatter_kernel(int64_t N, const double *__restrict__ t0,
+                                                             const double *__restrict__ dtj, const unsigned long long *key,
+                                                             unsigned long long *pub, uint32_t epoch,
+                                                             int32_t *__restrict__ idx_act, double *__restrict__ result,
+                                                             const double *__restrict__ tR, const double *__restrict__ dtR,
+                                                             int32_t *__restrict__ idx_reg, double t_stop, int32_t spec_cap,
+                                                             int32_t *stall, double *__restrict__ ring) {
+    if (*stall) return;
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const int b = blockIdx.x, nchunk = gridDim.x;
+    constexpr int PER = SEL_CHUNK / 256;
+    __shared__ int32_t wsum[8], wsum2[8];
+    __shared__ int32_t base_s, base2_s;
     const double tn = key_to_double(*key);
-    // ---- phase 2: active bodies per chunk
-    for (int b = blockIdx.x; b < nchunk; b += gridDim.x) {
-        int32_t cntc = 0, cnt2 = 0;
+    // ---- this chunk's active bodies (kept as flags) and their number
+    bool act[PER], due[PER];
+    int32_t cntc = 0, cnt2 = 0;
+#pragma unroll
+    for (int u = 0; u < PER; ++u) {
+        const int64_t j = (int64_t)b * SEL_CHUNK + u * 256 + threadIdx.x;
+        act[u] = j < N && (t0[j] + dtj[j] == tn);
+        due[u] = TWO && act[u] && (tR[j] + dtR[j] == tn);
+        cntc += act[u] ? 1 : 0;
+        cnt2 += due[u] ? 1 : 0;
+    }
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) {
+        cntc += __shfl_xor_sync(0xffffffffu, cntc, off);
+        cnt2 += __shfl_xor_sync(0xffffffffu, cnt2, off);
+    }
+    if (lane == 0) { wsum[w] = cntc; wsum2[w] = cnt2; }
+    __syncthreads();
+    int32_t mine = 0, mine2 = 0;
+#pragma unroll
+    for (int q = 0; q < 8; ++q) { mine += wsum[q]; mine2 += wsum2[q]; }
+    if (threadIdx.x == 0)       // publish: epoch (32 bits) | regular count (16 bits) | count (16 bits); a chunk holds <= 2048
+        atomicExch(pub + b, ((unsigned long long)epoch << 32) | ((unsigned long long)mine2 << 16) | (unsigned long long)mine);
+    // ---- look-back: the counts of all chunks before this one, as they appear
+    int32_t part = 0, part2 = 0;
+    for (int q = threadIdx.x; q < b; q += 256) {
+        unsigned long long v;
+        do { v = *reinterpret_cast<volatile unsigned long long *>(pub + q); } while ((uint32_t)(v >> 32) != epoch);
+        part += (int32_t)(v & 0xffffu);
+        part2 += (int32_t)((v >> 16) & 0xffffu);
+    }
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) {
+        part += __shfl_xor_sync(0xffffffffu, part, off);
+        part2 += __shfl_xor_sync(0xffffffffu, part2, off);
+    }
+    __syncthreads();
+    if (lane == 0) { wsum[w] = part; wsum2[w] = part2; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int32_t tsum = 0, tsum2 = 0;
+#pragma unroll
+        for (int q = 0; q < 8; ++q) { tsum += wsum[q]; tsum2 += wsum2[q]; }
+        base_s = tsum; base2_s = tsum2;
+    }
+    __syncthreads();
+    int32_t running = base_s, running2 = base2_s;
+    // ---- ordered compaction (ascending indices)
+    if (mine > 0) {
 #pragma unroll
         for (int u = 0; u < PER; ++u) {
             const int64_t j = (int64_t)b * SEL_CHUNK + u * 256 + threadIdx.x;
-            const bool act = b == (int)blockIdx.x ? first[u] == tn : (j < N && (t0[j] + dtj[j] == tn));
-            cntc += act ? 1 : 0;
-            if (TWO) cnt2 += (act && tR[j] + dtR[j] == tn) ? 1 : 0;
-        }
-#pragma unroll
-        for (int off = 16; off > 0; off >>= 1) {
-            cntc += __shfl_xor_sync(0xffffffffu, cntc, off);
-            if (TWO) cnt2 += __shfl_xor_sync(0xffffffffu, cnt2, off);
-        }
-        __syncthreads();
-        if (lane == 0) { wsum[w] = cntc; wsum2[w] = cnt2; }
-        __syncthreads();
-        if (threadIdx.x == 0) {
-            int32_t tsum = 0, tsum2 = 0;
-#pragma unroll
-            for (int q = 0; q < 8; ++q) { tsum += wsum[q]; tsum2 += wsum2[q]; }
-            counts[b] = tsum;
-            if (TWO) counts2[b] = tsum2;
-        }
-    }
-    grid.sync();
-    // ---- phase 3: ordered compaction (ascending indices)
-    for (int b = blockIdx.x; b < nchunk; b += gridDim.x) {
-        int32_t part = 0, part2 = 0;
-        for (int q = threadIdx.x; q < b; q += 256) { part += counts[q]; if (TWO) part2 += counts2[q]; }
-#pragma unroll
-        for (int off = 16; off > 0; off >>= 1) {
-            part += __shfl_xor_sync(0xffffffffu, part, off);
-            if (TWO) part2 += __shfl_xor_sync(0xffffffffu, part2, off);
-        }
-        __syncthreads();
-        if (lane == 0) { wsum[w] = part; wsum2[w] = part2; }
-        __syncthreads();
-        if (threadIdx.x == 0) {
-            int32_t tsum = 0, tsum2 = 0;
-#pragma unroll
-            for (int q = 0; q < 8; ++q) { tsum += wsum[q]; tsum2 += wsum2[q]; }
-            base_s = tsum; base2_s = tsum2;
-        }
-        __syncthreads();
-        int32_t running = base_s, running2 = base2_s;
-#pragma unroll
-        for (int u = 0; u < PER; ++u) {
-            const int s = u * 256;
-            const int64_t j = (int64_t)b * SEL_CHUNK + s + threadIdx.x;
-            const bool act = b == (int)blockIdx.x ? first[u] == tn : (j < N && (t0[j] + dtj[j] == tn));
-            const bool due = TWO && act && (tR[j] + dtR[j] == tn);
-            const unsigned bal = __ballot_sync(0xffffffffu, act);
-            const unsigned bal2 = __ballot_sync(0xffffffffu, due);
+            const unsigned bal = __ballot_sync(0xffffffffu, act[u]);
+            const unsigned bal2 = __ballot_sync(0xffffffffu, due[u]);
             __syncthreads();
             if (lane == 0) { wsum[w] = __popc(bal); wsum2[w] = __popc(bal2); }
             __syncthreads();
@@ -1402,17 +1401,23 @@ __global__ void __launch_bounds__(256) select_block_kernel(int64_t N, const doub
                 before2 += q < w ? cq2 : 0;
                 slab2 += cq2;
             }
-            if (act) idx_act[running + before + __popc(bal & ((1u << lane) - 1u))] = (int32_t)j;
-            if (due) idx_reg[running2 + before2 + __popc(bal2 & ((1u << lane) - 1u))] = (int32_t)j;
+            if (act[u]) idx_act[running + before + __popc(bal & ((1u << lane) - 1u))] = (int32_t)j;
+            if (due[u]) idx_reg[running2 + before2 + __popc(bal2 & ((1u << lane) - 1u))] = (int32_t)j;
             running += slab;
             running2 += slab2;
         }
-        if (b == nchunk - 1 && threadIdx.x == 0) {
-            result[0] = tn;
-            result[1] = (double)running;
-            if (TWO) result[2] = (double)running2;
-        }
-        __syncthreads();
+    }
+    if (b == nchunk - 1 && threadIdx.x == 0) {
+        const int32_t n1 = base_s + mine, n2 = base2_s + mine2;
+        // spec_cap = 0: no speculative chain follows.  TWO: that chain cannot take a regular step.
+        const int status = tn > t_stop ? BLK_PAST_T_STOP
+                           : (n1 > 0 && n1 <= spec_cap && n2 == 0) ? BLK_SPECULATIVE : BLK_NEEDS_HOST;
+        result[0] = tn; result[1] = (double)n1; result[2] = (double)n2; result[3] = (double)status;
+        if (status != BLK_SPECULATIVE) *stall = 1;
+        volatile double *rv = ring;      // mapped host memory: the status word last, after the rest is visible system-wide
+        rv[0] = tn; rv[1] = (double)n1; rv[2] = (double)n2;
+        __threadfence_system();
+        rv[3] = (double)status;
     }
 }
 
@@ -1443,13 +1448,13 @@ __global__ void __launch_bounds__(256) init_steps_kernel(int64_t N, int64_t Ns, 
 // then the block rule (double once if allowed and t1 is commensurate, else halve while too long).
 // One thread per active body; reads its 128 B line of the gather copy, writes both copies.  FP64.
 __global__ void __launch_bounds__(128) correct_kernel(int32_t n, int64_t Ns, double t1, double eta, double dt_max,
-                                                      const double *__restrict__ blk_dev, double t_stop,
+                                                      const double *__restrict__ blk_dev,
                                                       const int32_t *__restrict__ idx,
                                                       const double *__restrict__ acc1,
                                                       const double *__restrict__ jerk1, double *__restrict__ soa,
                                                       double *__restrict__ aos, double *__restrict__ dtj) {
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
-    if (!spec_block(blk_dev, t_stop, n, t1)) return;
+    if (!spec_block(blk_dev, n, t1)) return;
     if (k >= n) return;
     const int64_t i = idx[k];
     const double2 *p = reinterpret_cast<const double2 *>(aos + i * AOS_D);
@@ -1543,7 +1548,7 @@ __global__ void __launch_bounds__(128) ac_start_kernel(int64_t N, int64_t Ns, in
 // its slot r in the ascending idx_reg[0..n_reg) and there the new-list forces: regular rg_acc/rg_jerk[r],
 // irregular in_acc/in_jerk[r], new count rg_nnb[r] (rows are copied by ac_store_rows_kernel afterwards).
 __global__ void __launch_bounds__(128) ac_correct_kernel(int32_t n, int64_t Ns, double t, double eta_I, double eta_R,
-                                                         double dt_max, const double *__restrict__ blk_dev, double t_stop,
+                                                         double dt_max, const double *__restrict__ blk_dev,
                                                          const int32_t *__restrict__ idx,
                                                          const double *__restrict__ aIo, const double *__restrict__ jIo,
                                                          int32_t n_reg, const int32_t *__restrict__ idx_reg,
@@ -1553,7 +1558,7 @@ __global__ void __launch_bounds__(128) ac_correct_kernel(int32_t n, int64_t Ns, 
                                                          double *__restrict__ soa, double *__restrict__ aos,
                                                          double *__restrict__ dtj) {
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
-    if (!spec_block(blk_dev, t_stop, n, t)) return;
+    if (!spec_block(blk_dev, n, t)) return;
     if (k >= n) return;
     const int64_t i = idx[k];
     const double2 *p = reinterpret_cast<const double2 *>(aos + i * AOS_D);
