@@ -68,6 +68,8 @@ struct nb_ctx {
     // pipelined HOST step (nb_step_host): copy stream, per-chunk events, the active particles' own state
     static constexpr int MAXCHUNK = 8;
     cudaStream_t copy_stream = nullptr, prep_stream = nullptr;   // H2D copies / re-layout + predictor of landed chunks
+    cudaStream_t force_stream[MAXCHUNK] = {};                    // one per chunk: the per-chunk force launches overlap
+    cudaEvent_t ev_force[MAXCHUNK] = {}, ev_iready = nullptr;
     cudaEvent_t ev_enter = nullptr, ev_i = nullptr, ev_copied[MAXCHUNK] = {}, ev_chunk[MAXCHUNK] = {};
     double *h_ist = nullptr, *d_ist = nullptr;      // [14][n_i] gathered FP64 state (pinned host / device)
     float *irec = nullptr;                          // [RECF][n_i_pad] their predicted records
@@ -89,7 +91,6 @@ struct nb_ctx {
     int32_t h2_by_body = 0;                         // the h2 array of the launch in flight is indexed by body
     const double *spec_dev = nullptr;               // non-NULL while a SPECULATIVE chain is enqueued: the kernels take the
                                                     // block's {t, n, status} from this device address
-    cudaEvent_t ev_sel = nullptr;
     int64_t blk_stride = 0;                         // acc / jerk / pot of the last block sit at 0, 3, 6 x this in blk_out
     // two-level AC stepping (nb_ac_init / nb_ac_step): per-body force polynomials, persistent lists, scratch
     AcState ac = {};
@@ -264,7 +265,8 @@ int ensure_partial(nb_ctx *c, size_t bytes) {
 // [split0, split0 + S).
 int launch_force_range(nb_ctx *c, int vi, bool fused, int32_t n_i, const int32_t *idx_i, const double *h2_i,
                        const float *irec, const unsigned long long *perm, int64_t j_offset, int32_t *nblist, int64_t tile0,
-                       int64_t tile1, int S, int64_t split0) {
+                       int64_t tile1, int S, int64_t split0, cudaStream_t st = nullptr, bool own_stream = true) {
+    if (own_stream) st = c->stream;
     const Variant &v = fused ? c->fvar[vi] : c->var[vi];
     const int64_t n_ib = (n_i + v.iblock - 1) / v.iblock;
     ForceParams p;
@@ -281,25 +283,25 @@ int launch_force_range(nb_ctx *c, int vi, bool fused, int32_t n_i, const int32_t
     p.cap = c->cap; p.cnt = c->cnt; p.nblist = nblist; p.partial = c->partial;
     const dim3 grid((unsigned)n_ib, (unsigned)S);
     const int slot = (int)(c->prof_n % nb_ctx::PROF_RING);
-    if (c->profile) NB_CUDA(c, cudaEventRecord(c->ev0[slot], c->stream));
+    if (c->profile) NB_CUDA(c, cudaEventRecord(c->ev0[slot], st));
     if (fused) {
         switch (vi) {
-            case 2: launch_force<2, 4, 2, false, SRC_STATE>(v, grid, c->stream, p); break;
-            case 3: launch_force<1, 8, 2, false, SRC_STATE>(v, grid, c->stream, p); break;
-            default: launch_force<1, 8, 2, true, SRC_STATE>(v, grid, c->stream, p); break;
+            case 2: launch_force<2, 4, 2, false, SRC_STATE>(v, grid, st, p); break;
+            case 3: launch_force<1, 8, 2, false, SRC_STATE>(v, grid, st, p); break;
+            default: launch_force<1, 8, 2, true, SRC_STATE>(v, grid, st, p); break;
         }
     } else {
         switch (vi) {
-            case 0: launch_force<8, 1, 2>(v, grid, c->stream, p); break;
-            case 1: launch_force<4, 2, 2>(v, grid, c->stream, p); break;
-            case 2: launch_force<2, 4, 2>(v, grid, c->stream, p); break;
-            case 3: launch_force<1, 8, 2>(v, grid, c->stream, p); break;
-            default: launch_force<1, 8, 2, true>(v, grid, c->stream, p); break;
+            case 0: launch_force<8, 1, 2>(v, grid, st, p); break;
+            case 1: launch_force<4, 2, 2>(v, grid, st, p); break;
+            case 2: launch_force<2, 4, 2>(v, grid, st, p); break;
+            case 3: launch_force<1, 8, 2>(v, grid, st, p); break;
+            default: launch_force<1, 8, 2, true>(v, grid, st, p); break;
         }
     }
     NB_CUDA(c, cudaGetLastError());
     if (c->profile) {
-        NB_CUDA(c, cudaEventRecord(c->ev1[slot], c->stream));
+        NB_CUDA(c, cudaEventRecord(c->ev1[slot], st));
         c->prof_n += 1;
     }
     c->launches += 1;
@@ -551,13 +553,17 @@ int nb_close(nb_ctx *c) {
     cudaFree(c->d_ist); cudaFree(c->irec); cudaFreeHost(c->h_ist);
     cudaFree(c->dtj); cudaFree(c->sel_key); cudaFree(c->sel_counts); cudaFree(c->sel_result);
     cudaFreeHost(c->h_sel_result);
-    if (c->ev_sel) cudaEventDestroy(c->ev_sel);
     if (c->ev_enter) cudaEventDestroy(c->ev_enter);
     if (c->ev_i) cudaEventDestroy(c->ev_i);
     for (int q = 0; q < nb_ctx::MAXCHUNK; ++q) {
         if (c->ev_chunk[q]) cudaEventDestroy(c->ev_chunk[q]);
         if (c->ev_copied[q]) cudaEventDestroy(c->ev_copied[q]);
     }
+    for (int q = 0; q < nb_ctx::MAXCHUNK; ++q) {
+        if (c->force_stream[q]) cudaStreamDestroy(c->force_stream[q]);
+        if (c->ev_force[q]) cudaEventDestroy(c->ev_force[q]);
+    }
+    if (c->ev_iready) cudaEventDestroy(c->ev_iready);
     if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
     if (c->prep_stream) cudaStreamDestroy(c->prep_stream);
     for (int q = 0; q < nb_ctx::PROF_RING; ++q) {
@@ -856,12 +862,27 @@ int nb_step_host(nb_ctx *c, const double *m, const double *x0, const double *v0,
         if (rc != NB_OK) return rc;
         perm = c->sort_keys; c->last_reordered = 1;
     }
+    // The per-chunk force launches are independent (own partial rows; the row counters are integer atomics): each
+    // goes to its own stream behind its chunk's predictor, so that the CTAs of a chunk fill the drain of the one
+    // before it instead of queueing behind its last CTA.
+    if (!c->force_stream[0]) {
+        for (int q = 0; q < nb_ctx::MAXCHUNK; ++q) {
+            NB_CUDA(c, cudaStreamCreateWithFlags(&c->force_stream[q], cudaStreamNonBlocking));
+            NB_CUDA(c, cudaEventCreateWithFlags(&c->ev_force[q], cudaEventDisableTiming));
+        }
+        NB_CUDA(c, cudaEventCreateWithFlags(&c->ev_iready, cudaEventDisableTiming));
+    }
+    NB_CUDA(c, cudaEventRecord(c->ev_iready, c->stream));       // i-records, Morton order, scratch: ready
     int64_t split0 = 0;
     for (int q = 0; q < nchunk; ++q) {
-        NB_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_chunk[q], 0));
+        cudaStream_t fs = c->force_stream[q];
+        NB_CUDA(c, cudaStreamWaitEvent(fs, c->ev_iready, 0));
+        NB_CUDA(c, cudaStreamWaitEvent(fs, c->ev_chunk[q], 0));
         rc = launch_force_range(c, vi, false, n_i, c->st_idx, c->st_h2, c->irec, perm, 0, c->st_list, ctile[q], ctile[q + 1], S_c[q],
-                                split0);
+                                split0, fs, false);
         if (rc != NB_OK) return rc;
+        NB_CUDA(c, cudaEventRecord(c->ev_force[q], fs));
+        NB_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_force[q], 0));
         split0 += S_c[q];
     }
     double *d_acc = c->st_out, *d_jerk = c->st_out + 3 * (int64_t)n_i, *d_pot = c->st_out + 6 * (int64_t)n_i;
@@ -973,7 +994,6 @@ int blk_setup(nb_ctx *c) {
     NB_CUDA(c, cudaHostAlloc(&c->h_blk_ring, sizeof(double) * 4 * BLK_BATCH_MAX, cudaHostAllocMapped));
     NB_CUDA(c, cudaHostGetDevicePointer(reinterpret_cast<void **>(&c->blk_ring), c->h_blk_ring, 0));
     NB_CUDA(c, cudaMalloc(&c->blk_stall, sizeof(int32_t)));
-    if (!c->ev_sel) NB_CUDA(c, cudaEventCreateWithFlags(&c->ev_sel, cudaEventDisableTiming));
     return NB_OK;
 }
 
