@@ -232,7 +232,10 @@ int nb_get_block(nb_ctx *ctx, int32_t *idx_act, double *acc, double *jerk, doubl
  * over the lists -> aI, jI; start-up steps dtR = initial step of the regular force, dtI = min(initial step of the
  * irregular force, dtR), dtI = dtR for a body without neighbours.  *n_overflow (HOST, may be NULL) = number of
  * lists longer than nb_cap; if any, returns NB_EOVERFLOW and AC stepping stays unavailable (shrink the radii:
- * radius control is the caller's, reading R38).  Allocates 6 N vectors + N x nb_cap list entries. */
+ * radius control is the caller's, reading R38).  Allocates 6 N vectors + N x nb_cap list entries.
+ * Any call that replaces or advances the state outside the two-level scheme (nb_set_j, nb_set_j_host,
+ * nb_step_host, nb_update_j, nb_set_steps, nb_init_steps, nb_correct, nb_block_step, nb_run_blocks) ends it:
+ * nb_ac_step then returns NB_ESTATE until the next nb_ac_init. */
 int nb_ac_init(nb_ctx *ctx, double t_start, const double *h2_all, double eta_s, double dt_max,
                int32_t *n_overflow);
 /* One block of the two-level scheme: t_next = min_j (t0_j + dtI_j); the bodies due then take an IRREGULAR step

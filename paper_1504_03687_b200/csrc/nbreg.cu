@@ -599,6 +599,7 @@ int nb_set_j(nb_ctx *c, const double *m, const double *x0, const double *v0, con
     c->launches += 1;
     c->have_j = true;
     c->have_pred = false; c->pred_pending = false;
+    c->have_ac = false;         // the AC force polynomials belong to the state that was just replaced
     return NB_OK;
 }
 
@@ -633,6 +634,7 @@ int nb_update_j(nb_ctx *c, int32_t n, const int32_t *idx, const double *m, const
     NB_CUDA(c, cudaGetLastError());
     c->launches += 1;
     c->have_pred = false; c->pred_pending = false;   // the predicted records are stale until the next nb_predict_all
+    c->have_ac = false;
     return NB_OK;
 }
 
@@ -900,6 +902,7 @@ int nb_set_steps(nb_ctx *c, const double *dt) {
     if (!c->dtj) NB_CUDA(c, cudaMalloc(&c->dtj, sizeof(double) * c->N));
     NB_CUDA(c, cudaMemcpyAsync(c->dtj, dt, sizeof(double) * c->N, cudaMemcpyDeviceToDevice, c->stream));
     c->have_steps = true;
+    c->have_ac = false;         // dtj is the irregular step of the two-level scheme: replaced here
     return NB_OK;
 }
 
@@ -913,6 +916,7 @@ int nb_init_steps(nb_ctx *c, double eta_s, double dt_max) {
     NB_CUDA(c, cudaGetLastError());
     c->launches += 1;
     c->have_steps = true;
+    c->have_ac = false;
     return NB_OK;
 }
 
@@ -959,6 +963,7 @@ int nb_correct(nb_ctx *c, double t, int32_t n, const int32_t *idx, const double 
     NB_CUDA(c, cudaGetLastError());
     c->launches += 1;
     c->have_pred = false; c->pred_pending = false;
+    c->have_ac = false;         // the single-level corrector knows nothing of the AC force polynomials
     return NB_OK;
 }
 
@@ -1239,6 +1244,7 @@ int nb_block_step(nb_ctx *c, const double *h2_all, double eta, double dt_max, do
     if (!t_next || !n_act || !(eta > 0.0) || !(dt_max > 0.0)) return NB_EINVAL;
     if (!c->have_j || !c->have_steps) return NB_ESTATE;
     BlockRun R = {false, h2_all, eta, 0.0, dt_max, t_stop, 1};
+    c->have_ac = false;         // single-level steps leave the AC force polynomials behind
     rc = run_blocks(c, R);
     *t_next = R.t_next;
     *n_act = R.blocks ? R.last_n : 0;
@@ -1252,6 +1258,7 @@ int nb_run_blocks(nb_ctx *c, const double *h2_all, double eta, double dt_max, do
     if (!t_next || !blocks || !particle_steps || max_blocks < 0 || !(eta > 0.0) || !(dt_max > 0.0)) return NB_EINVAL;
     if (!c->have_j || !c->have_steps) return NB_ESTATE;
     BlockRun R = {false, h2_all, eta, 0.0, dt_max, t_stop, max_blocks};
+    c->have_ac = false;
     rc = run_blocks(c, R);
     *t_next = R.t_next; *blocks = R.blocks; *particle_steps = R.steps;
     return rc;

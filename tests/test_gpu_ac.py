@@ -158,3 +158,122 @@ def test_ac_run_conserves_energy_and_overflow_is_reported(oracle):
         ctx.ac_step(eta_I, eta_R, dt_max)
     assert e.value.code == nb.NB_ESTATE
     ctx.close()
+    # a call that advances the state outside the two-level scheme ends it until the next nb_ac_init
+    ctx = _open(m, x, v, cap)
+    ctx.ac_init(0.0, _dev(h2), eta_s, dt_max)
+    ctx.ac_step(eta_I, eta_R, dt_max)
+    ctx.block_step(None, eta_R, dt_max)
+    with pytest.raises(nb.NbregError) as e:
+        ctx.ac_step(eta_I, eta_R, dt_max)
+    assert e.value.code == nb.NB_ESTATE
+    ctx.close()
+
+
+def test_batched_loops_equal_block_by_block_stepping():
+    """nb_ac_run / nb_run_blocks enqueue batches of blocks without the host in between (speculative chains, device
+    stall flag, adaptive batch size).  Whatever the batching, the kernels and their order are the same: the state
+    after K blocks must be BIT-identical to K single calls, with and without speculation."""
+    import paper_1504_03687_b200 as nb
+    N, cap = 3000, 96
+    cfg = nbgen.make_config(1, N=N)
+    m, x, v = cfg["m"], cfg["x0"], cfg["v0"]
+    h2 = _radii(x, 12)
+    eta_I, eta_R, eta_s, dt_max = 0.01, 0.02, 0.01, 2.0**-4
+    runs = {}
+    for mode in ("steps", "run", "run_nospec"):
+        ctx = _open(m, x, v, cap)
+        if mode == "run_nospec":
+            ctx.tune("speculate", 0)
+        ctx.ac_init(0.0, _dev(h2), eta_s, dt_max)
+        K, ni, nr = 260, 0, 0
+        if mode == "steps":
+            for _ in range(K):
+                t, a, b = ctx.ac_step(eta_I, eta_R, dt_max)
+                ni += a; nr += b
+        else:
+            t, blocks, ni, nr = ctx.ac_run(eta_I, eta_R, dt_max, max_blocks=100)
+            t, b2, i2, r2 = ctx.ac_run(eta_I, eta_R, dt_max, max_blocks=K - 100)
+            assert blocks == 100 and b2 == K - 100
+            ni += i2; nr += r2
+        runs[mode] = (_gpu_state(ctx, lists=True), t, ni, nr, ctx.info("spec_hits"), ctx.info("spec_misses"))
+        ctx.close()
+    ref, t, ni, nr, hits, misses = runs["steps"]
+    assert hits > 100 and nr > 0
+    print("batched loops: irregular steps", ni, "regular steps", nr, "speculation hits / misses: steps", (hits, misses),
+          "run", runs["run"][4:], "run without speculation", runs["run_nospec"][4:])
+    assert runs["run_nospec"][4] == 0
+    for mode in ("run", "run_nospec"):
+        g, t2, ni2, nr2 = runs[mode][:4]
+        assert (t2, ni2, nr2) == (t, ni, nr)
+        for key in ("x0", "v0", "a0", "j0", "t0", "dt", "aI", "jI", "aR", "jR", "tR", "dtR", "nnb"):
+            assert np.array_equal(g[key], ref[key]), (mode, key)
+        for i in range(N):
+            assert np.array_equal(g["nblist"][i, :g["nnb"][i]], ref["nblist"][i, :ref["nnb"][i]])
+    # the single-level loop likewise
+    states = []
+    for mode in ("steps", "run"):
+        ctx = nb.nb_open(N, 8)
+        nb.nb_set_j(ctx, _dev(m), _dev(x), _dev(v), _dev(ref["a0"] * 0 + runs["steps"][0]["a0"]), _dev(runs["steps"][0]["j0"]),
+                    _dev(np.zeros(N)))
+        ctx.init_steps(eta_s, dt_max)
+        if mode == "steps":
+            tot = 0
+            for _ in range(150):
+                tt, n = ctx.block_step(None, 0.02, dt_max)
+                tot += n
+        else:
+            tt, blocks, tot = ctx.run_blocks(None, 0.02, dt_max, max_blocks=150)
+            assert blocks == 150
+        states.append(({k: v_.cpu().numpy() for k, v_ in ctx.get_state(True).items()}, tt, tot))
+        ctx.close()
+    assert states[0][1:] == states[1][1:]
+    for key in states[0][0]:
+        assert np.array_equal(states[0][0][key], states[1][0][key]), key
+
+
+def test_ac_overflow_in_mid_run_is_reported_at_the_same_block_as_the_oracle(oracle):
+    """Lists sized exactly for the start-up state: as the cluster moves some body collects one neighbour too many at
+    a regular step.  The library must return NB_EOVERFLOW for the very block at which the oracle raises, BEFORE
+    correcting anything (the state is untouched and the same call fails again), reading R38."""
+    import paper_1504_03687_b200 as nb
+    N = 512
+    cfg = nbgen.make_config(1, N=N)
+    m, x, v = cfg["m"], cfg["x0"], cfg["v0"]
+    h2 = _radii(x, 10)
+    eta_I, eta_R, eta_s, dt_max = 0.01, 0.02, 0.01, 2.0**-4
+    probe = AC.start(oracle, m, x, v, h2, N, eta_s, dt_max)
+    cap = int(probe["nnb"].max())                      # no slack at all
+    st = AC.start(oracle, m, x, v, h2, cap, eta_s, dt_max)
+    ctx = _open(m, x, v, cap)
+    assert ctx.ac_init(0.0, _dev(h2), eta_s, dt_max) == 0
+    g = _gpu_state(ctx)
+    st["dtI"], st["dtR"] = g["dt"].copy(), g["dtR"].copy()
+    for b in range(4000):
+        before = _gpu_state(ctx)
+        try:
+            t_ref, act, reg = AC.block_step(oracle, m, st, h2, cap, eta_I, eta_R, dt_max)
+            orc_raised = False
+        except OverflowError:
+            orc_raised = True
+        try:
+            t, n, nr = ctx.ac_step(eta_I, eta_R, dt_max)
+            gpu_raised = False
+        except nb.NbregError as e:
+            assert e.code == nb.NB_EOVERFLOW
+            gpu_raised = True
+        assert orc_raised == gpu_raised, (b, orc_raised, gpu_raised)
+        if gpu_raised:
+            after = _gpu_state(ctx)
+            for key in ("x0", "v0", "a0", "j0", "t0", "dt", "aI", "aR", "tR", "dtR", "nnb"):
+                assert np.array_equal(before[key], after[key]), key            # nothing was corrected
+            with pytest.raises(nb.NbregError) as e2:
+                ctx.ac_step(eta_I, eta_R, dt_max)                               # the same block, the same error
+            assert e2.value.code == nb.NB_EOVERFLOW
+            print("overflow reported at block", b, "cap", cap)
+            break
+        g = _gpu_state(ctx)
+        dI, dR = np.flatnonzero(g["dt"] != st["dtI"]), np.flatnonzero(g["dtR"] != st["dtR"])
+        st["dtI"][dI] = g["dt"][dI]; st["dtR"][dR] = g["dtR"][dR]
+    else:
+        pytest.fail("no overflow within 4000 blocks: the test set-up does not exercise the error path")
+    ctx.close()
