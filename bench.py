@@ -428,7 +428,7 @@ def run_b200(args):
 
     sweep = None
     if not args.no_sweep and world == 1:
-        sweep = sweep_config(ctx, cfg, [32] + list(cfg["sweep"]), N)   # 32: the j-packed tiny-block variant
+        sweep = sweep_config(ctx, cfg, [8, 16, 32] + list(cfg["sweep"]), N)   # 8, 16, 32: the j-packed tiny-block variants
     other = None
     if not args.headline_only and not args.no_sweep and world == 1 and N == 1048576:
         other = {}

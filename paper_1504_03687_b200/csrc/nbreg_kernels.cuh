@@ -547,13 +547,26 @@ struct JPtrs {
 // All pairs of the warp's i-pair(s) with SUBN consecutive j of one tile.  LOCAL: positions are already
 // differenced against the warp's origin -- ONE packed add per component (27 packed FP32 instructions
 // per 2 i x 1 j); otherwise hi/lo differencing, three adds per component (33).
-template <bool LOCAL, bool JP, int SUBN, int SX, int SV>
-__device__ __forceinline__ void tile_pairs(Acc7 &A, const IPair &I, const JPtrs P, int32_t jbase,
+// j-packed variants, tiny blocks (js = 2, 4: a CTA with at most 16 / 8 active particles): the lanes of the warp
+// are js groups of 32 / js; group q holds the same 32 / js i-particles and takes the q-th part of the SUBN
+// j's, so the addresses are uniform per group (one LDS.128 wavefront: the groups read different 16 B pieces
+// of the same rows) and the padded pair work shrinks from 32 to 16 / 8 i-slots.
+template <bool LOCAL, bool JP, int SUBN, int SX, int SV, bool GROUPED = false>
+__device__ __forceinline__ void tile_pairs(Acc7 &A, const IPair &I, JPtrs P, int32_t jbase,
                                            const int32_t (&my_idx)[2], const int32_t (&my_k)[2],
-                                           const ForceParams &p) {
+                                           const ForceParams &p, int js = 1, int q = 0) {
     constexpr int NU = JP ? 2 : 4;           // packed iterations per group of four j
+    static_assert(!GROUPED || (JP && SUBN % (4 * UNROLL_J) == 0), "lane groups along j: j-packed, up to four per warp");
+    int span = SUBN;                         // j's of this lane (a compile-time constant unless GROUPED)
+    if constexpr (GROUPED) {
+        span = SUBN / js;
+        const int off = q * span;
+        P.px += off; P.pv += off; P.pm += off;
+        if constexpr (!LOCAL) P.pl += off;
+        jbase += off;
+    }
 #pragma unroll GROUP_UNROLL
-    for (int g = 0; g < SUBN; g += UNROLL_J) {
+    for (int g = 0; g < span; g += UNROLL_J) {
         // warp-uniform addresses: LDS.128 broadcasts of one component of 4 consecutive j
         float4 cx = *reinterpret_cast<const float4 *>(P.px + g);
         float4 cy = *reinterpret_cast<const float4 *>(P.px + SX + g);
@@ -682,6 +695,15 @@ __global__ void __launch_bounds__(32 * WI *WJ, MINB) force_kernel(const ForcePar
     int32_t n_i = p.n_i;
     double t_pred = p.t;
     if (!spec_block(p.blk_dev, n_i, t_pred)) return;    // (uniform over the grid, before any barrier)
+    // j-packed variants: a CTA with <= 16 / 8 active particles (the tiny blocks of the deep levels; the tail
+    // of a small block) groups its lanes 2 / 4 ways along j -- decided here, from the block size, so that a
+    // speculative launch (n_i from device memory) takes the right mapping too
+    int js = 1;
+    if constexpr (JP) {
+        const int nv = n_i - (int)blockIdx.x * IB;
+        js = nv <= 8 ? 4 : nv <= 16 ? 2 : 1;
+    }
+    const int il = 32 / js, li = lane & (il - 1), lq = lane / il;      // i-slot of the lane, its group along j
 
     const int tile_begin = p.tile0 + blockIdx.y * p.tiles_per_split;
     const int tile_end = min(tile_begin + p.tiles_per_split, p.ntiles);
@@ -724,7 +746,7 @@ __global__ void __launch_bounds__(32 * WI *WJ, MINB) force_kernel(const ForcePar
         bool valid[2];
 #pragma unroll
         for (int h = 0; h < NH; ++h) {
-            const int slot = blockIdx.x * IB + wi * (32 * NH) + h * 32 + lane;
+            const int slot = blockIdx.x * IB + wi * (32 * NH) + h * 32 + li;
             valid[h] = slot < n_i;
             const int k = (valid[h] && p.perm) ? perm_slot(p.perm, slot) : slot;   // caller's numbering: rows, counters, inputs
             my_k[h] = k;
@@ -914,10 +936,12 @@ __global__ void __launch_bounds__(32 * WI *WJ, MINB) force_kernel(const ForcePar
             release(it, s);                              // (starts with __syncwarp: the slice is complete)
             if (local) {
                 const JPtrs P = {slice, nullptr, slice + 3 * SUB, slice + 6 * SUB};
-                tile_pairs<true, JP, SUB, SUB, SUB>(A, I, P, jbase, my_idx, my_k, p);
+                if (JP && js > 1) tile_pairs<true, JP, SUB, SUB, SUB, JP>(A, I, P, jbase, my_idx, my_k, p, js, lq);
+                else tile_pairs<true, JP, SUB, SUB, SUB>(A, I, P, jbase, my_idx, my_k, p);
             } else {
                 const JPtrs P = {slice, slice + 3 * SUB, slice + 6 * SUB, slice + 9 * SUB};
-                tile_pairs<false, JP, SUB, SUB, SUB>(A, I, P, jbase, my_idx, my_k, p);
+                if (JP && js > 1) tile_pairs<false, JP, SUB, SUB, SUB, JP>(A, I, P, jbase, my_idx, my_k, p, js, lq);
+                else tile_pairs<false, JP, SUB, SUB, SUB>(A, I, P, jbase, my_idx, my_k, p);
             }
             __syncwarp();                                // every lane is out of the slice before it is rewritten
         } else {
@@ -946,10 +970,12 @@ __global__ void __launch_bounds__(32 * WI *WJ, MINB) force_kernel(const ForcePar
                 }
                 __syncwarp();
                 const JPtrs P = {slice, nullptr, tsub + C_VX * TJ, tsub + C_M * TJ};
-                tile_pairs<true, JP, SUB, SUB, TJ>(A, I, P, jbase, my_idx, my_k, p);
+                if (JP && js > 1) tile_pairs<true, JP, SUB, SUB, TJ, JP>(A, I, P, jbase, my_idx, my_k, p, js, lq);
+                else tile_pairs<true, JP, SUB, SUB, TJ>(A, I, P, jbase, my_idx, my_k, p);
             } else {
                 const JPtrs P = {tsub, tsub + C_XL * TJ, tsub + C_VX * TJ, tsub + C_M * TJ};
-                tile_pairs<false, JP, SUB, TJ, TJ>(A, I, P, jbase, my_idx, my_k, p);
+                if (JP && js > 1) tile_pairs<false, JP, SUB, TJ, TJ, JP>(A, I, P, jbase, my_idx, my_k, p, js, lq);
+                else tile_pairs<false, JP, SUB, TJ, TJ>(A, I, P, jbase, my_idx, my_k, p);
             }
             release(it, s);                              // (its __syncwarp also frees the slice)
         }
@@ -977,33 +1003,40 @@ __global__ void __launch_bounds__(32 * WI *WJ, MINB) force_kernel(const ForcePar
     for (int h = 0; h < NH; ++h)
 #pragma unroll
         for (int c = 0; c < 7; ++c) out64[h][c] = acc64[(h * 7 + c) * NT];
+    if constexpr (JP) {         // the js lane groups hold shares of the same i: fixed xor tree, every lane gets the sum
+        for (int off = il; off < 32; off <<= 1)
+#pragma unroll
+            for (int c = 0; c < 7; ++c) out64[0][c] += __shfl_xor_sync(0xffffffffu, out64[0][c], off);
+    }
     if constexpr (WJ > 1) {
         double *red = reinterpret_cast<double *>(smem_raw);     // reuse the ring and the slices: [WJ][7][IB]
         __syncthreads();                                         // every warp is out of both
-#pragma unroll
-        for (int h = 0; h < NH; ++h) {
-            const int il = wi * (32 * NH) + h * 32 + lane;
-#pragma unroll
-            for (int c = 0; c < 7; ++c) red[((size_t)wj * 7 + c) * IB + il] = out64[h][c];
-        }
-        __syncthreads();
-        if (wj == 0) {
+        if (lq == 0) {
 #pragma unroll
             for (int h = 0; h < NH; ++h) {
-                const int il = wi * (32 * NH) + h * 32 + lane;
+                const int irow = wi * (32 * NH) + h * 32 + li;
+#pragma unroll
+                for (int c = 0; c < 7; ++c) red[((size_t)wj * 7 + c) * IB + irow] = out64[h][c];
+            }
+        }
+        __syncthreads();
+        if (wj == 0 && lq == 0) {
+#pragma unroll
+            for (int h = 0; h < NH; ++h) {
+                const int irow = wi * (32 * NH) + h * 32 + li;
 #pragma unroll
                 for (int c = 0; c < 7; ++c) {
                     double ssum = out64[h][c];
-                    for (int w = 1; w < WJ; ++w) ssum += red[((size_t)w * 7 + c) * IB + il];
+                    for (int w = 1; w < WJ; ++w) ssum += red[((size_t)w * 7 + c) * IB + irow];
                     out64[h][c] = ssum;
                 }
             }
         }
     }
-    if (wj == 0) {
+    if (wj == 0 && lq == 0) {
 #pragma unroll
         for (int h = 0; h < NH; ++h) {
-            const int slot = blockIdx.x * IB + wi * (32 * NH) + h * 32 + lane;    // slot < n_i_pad always
+            const int slot = blockIdx.x * IB + wi * (32 * NH) + h * 32 + li;    // slot < n_i_pad always
 #pragma unroll
             for (int c = 0; c < 7; ++c)
                 p.partial[((size_t)(p.split0 + blockIdx.y) * 7 + c) * p.n_i_pad + slot] = out64[h][c];

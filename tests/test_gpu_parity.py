@@ -117,7 +117,7 @@ def test_config2(oracle):
 
 # ----------------------------------------------------------------------------- every variant, ragged sizes
 
-@pytest.mark.parametrize("n_i", [1, 7, 31, 32, 33, 64, 100, 128, 257, 512, 1000, 3000])
+@pytest.mark.parametrize("n_i", [1, 2, 7, 8, 9, 16, 17, 31, 32, 33, 64, 100, 128, 257, 512, 1000, 3000])
 def test_block_sizes_ragged_N(oracle, n_i):
     cfg = nbgen.make_config(3, N=9001, n_i=n_i)        # 9001 = 35 tiles + a tail of 41
     ctx = open_ctx(cfg)
@@ -496,6 +496,37 @@ def test_config5_full_size_king_core(oracle):
     assert 0 < over < 512                                       # mixes overflowing and fitting rows
 
 
+@pytest.mark.parametrize("k,n_i", [(4, 3), (4, 8), (4, 16), (5, 8), (5, 16)])
+def test_tiny_blocks_full_size(oracle, k, n_i):
+    """The deep block levels hold a handful of particles: blocks of <= 16 take the j-packed
+    variant with its lanes grouped along j (8 or 16 i-slots per warp instead of 32 padded ones).  N = 1,048,576,
+    every active particle against the oracle, by both routes (FP64 state in with the predictor fused, and the
+    predicted records); config 5's core rows overflow the 512 cap."""
+    import paper_1504_03687_b200 as nb
+    if k == 4:
+        cfg, ctx, (xp, vp) = _config4(oracle)
+    else:
+        cfg = nbgen.make_config(5)
+        ctx = open_ctx(cfg)
+        xp, vp = oracle.predict(cfg["x0"], cfg["v0"], cfg["a0"], cfg["j0"], cfg["t0"], cfg["t"])
+    idx, h2 = nbgen.active_block(cfg, n_i)
+    ref = parity.oracle_reference(oracle, cfg["m"], xp, vp, idx, h2, cfg["cap"])
+    out = {}
+    for fused in (1, 0):
+        nb.nb_predict_all(ctx, cfg["t"])                     # pending prediction: a small block fuses it
+        ctx.tune("fuse_predict", fused)
+        got = gpu_regular(ctx, idx, h2)
+        assert ctx.info("last_fused") == fused and ctx.info("last_variant") == 4
+        rep = parity.compare(got, ref, cfg["cap"])
+        print("tiny block config", k, n_i, "fused" if fused else "records", rep, "S", ctx.info("last_jsplit"))
+        out[fused] = got
+    ctx.tune("fuse_predict", 1)
+    assert np.array_equal(out[0]["nnb"], out[1]["nnb"]) and np.array_equal(out[0]["overflow"], out[1]["overflow"])
+    if k == 5:
+        assert out[1]["overflow"].sum() > 0
+        ctx.close()
+
+
 def test_config3_block_sweep_sampled(oracle):
     """BASELINE.json configs[2] at its full size (N = 262,144, 5 % binaries): the five block sizes of
     the sweep; the oracle checks every i up to n_i = 1024 and a seeded sample of 256 above."""
@@ -770,7 +801,7 @@ def _warp_stats(ctx, fn):
     return out, loc, tot
 
 
-@pytest.mark.parametrize("n_i", [32, 64, 128, 300, 2000])
+@pytest.mark.parametrize("n_i", [5, 8, 16, 32, 64, 128, 300, 2000])
 def test_local_frame_and_hilo_agree_and_match_the_oracle(oracle, n_i):
     """A compact block (config 3: the n_i deepest-level = innermost bodies) takes the warp-local frame (one
     add per component); with the guard switched off (G = 0) the same call differences hi/lo pairs.  Both
@@ -815,7 +846,7 @@ def test_scattered_and_two_subcluster_blocks_fall_back_to_hilo(oracle):
     print("fallbacks", rep, rep2, rep3)
 
 
-@pytest.mark.parametrize("n_i", [1, 31, 32, 64, 100, 128])
+@pytest.mark.parametrize("n_i", [1, 5, 8, 13, 16, 31, 32, 64, 100, 128])
 def test_fused_predictor_equals_the_two_kernel_route(oracle, n_i):
     """nb_predict_all + nb_regular on a small block predicts inside the force kernel (FP64 state in, no
     records written).  With hi/lo differencing on both routes (G = 0) the records are bit for bit the
