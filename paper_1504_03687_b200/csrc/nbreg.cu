@@ -147,9 +147,23 @@ cudaError_t setup_variant(Variant &v, double ovh) {
     return e;
 }
 
+// Launch with programmatic stream serialization: the grid is placed while its predecessor in the stream drains, so
+// the launch latency is not on the path of a chain of short kernels (block loop; nb_regular of a small block).  Every
+// kernel launched this way starts with pdl_wait() (griddepcontrol.wait) before it reads anything.
+template <typename... KArgs, typename... Args>
+cudaError_t launch_chain(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args &&...args) {
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kernel, KArgs(std::forward<Args>(args))...);
+}
+
 template <int WI, int WJ, int MINB, bool JP = false, int SRC = SRC_REC>
 void launch_force(const Variant &v, dim3 grid, cudaStream_t st, const ForceParams &p) {
-    force_kernel<WI, WJ, MINB, JP, SRC><<<grid, v.threads, v.smem, st>>>(p);
+    launch_chain(force_kernel<WI, WJ, MINB, JP, SRC>, grid, dim3(v.threads), v.smem, st, p);
 }
 
 // i-particles per CTA, planning overhead (in tile units) and relative cost per padded i-slot of the
@@ -1039,15 +1053,15 @@ int blk_enqueue_select(nb_ctx *c, bool two, double t_stop, int32_t spec_cap, int
     const unsigned nchunk = (unsigned)((N + SEL_CHUNK - 1) / SEL_CHUNK);
     const unsigned gmin = (unsigned)std::min<int64_t>((N + 255) / 256, (int64_t)c->sm_count * 8);
     c->blk_epoch += 1;
-    select_min_kernel<<<gmin, 256, 0, c->stream>>>(N, t0, c->dtj, key, key_next, c->blk_stall, ring);
+    NB_CUDA(c, launch_chain(select_min_kernel, dim3(gmin), dim3(256), 0, c->stream, N, t0, c->dtj, key, key_next, c->blk_stall, ring));
     if (two)
-        select_scatter_kernel<true><<<nchunk, 256, 0, c->stream>>>(N, t0, c->dtj, key, c->blk_pub, c->blk_epoch, c->blk_idx,
-                                                                   c->sel_result, c->ac.tR, c->ac.dtR, c->ac_reg_idx, t_stop,
-                                                                   spec_cap, c->blk_stall, ring);
+        NB_CUDA(c, launch_chain(select_scatter_kernel<true>, dim3(nchunk), dim3(256), 0, c->stream, N, t0, c->dtj, key, c->blk_pub,
+                                c->blk_epoch, c->blk_idx, c->sel_result, c->ac.tR, c->ac.dtR, c->ac_reg_idx, t_stop, spec_cap,
+                                c->blk_stall, ring));
     else
-        select_scatter_kernel<false><<<nchunk, 256, 0, c->stream>>>(N, t0, c->dtj, key, c->blk_pub, c->blk_epoch, c->blk_idx,
-                                                                    c->sel_result, nullptr, nullptr, c->ac_reg_idx, t_stop,
-                                                                    spec_cap, c->blk_stall, ring);
+        NB_CUDA(c, launch_chain(select_scatter_kernel<false>, dim3(nchunk), dim3(256), 0, c->stream, N, t0, c->dtj, key, c->blk_pub,
+                                c->blk_epoch, c->blk_idx, c->sel_result, nullptr, nullptr, c->ac_reg_idx, t_stop, spec_cap,
+                                c->blk_stall, ring));
     NB_CUDA(c, cudaGetLastError());
     c->blk_parity ^= 1;
     c->launches += 2;
@@ -1068,13 +1082,13 @@ int sl_enqueue_chain(nb_ctx *c, const double *h2_all, double eta, double dt_max,
         rc = regular_device(c, n, c->blk_idx, h2_all, acc, jerk, pot, c->blk_nnb, h2_all ? c->blk_list : nullptr, c->blk_ovf);
     c->h2_by_body = 0;
     if (rc == NB_OK && h2_all) {
-        irregular_kernel<true><<<(unsigned)((n + 7) / 8), 256, 0, c->stream>>>(n, c->cap, t, c->spec_dev, 0, 0, c->blk_idx, c->blk_nnb,
-                                                                                c->blk_list, c->aos, acc, jerk, pot);
+        launch_chain(irregular_kernel<true>, dim3((unsigned)((n + 7) / 8)), dim3(256), 0, c->stream, n, c->cap, t, c->spec_dev, 0, 0,
+                     c->blk_idx, c->blk_nnb, c->blk_list, c->aos, acc, jerk, pot);
         c->launches += 1;
     }
     if (rc == NB_OK) {
-        correct_kernel<<<(unsigned)((n + 127) / 128), 128, 0, c->stream>>>(n, c->Ns, t, eta, dt_max, c->spec_dev, c->blk_idx, acc,
-                                                                           jerk, c->soa, c->aos, c->dtj);
+        launch_chain(correct_kernel, dim3((unsigned)((n + 127) / 128)), dim3(128), 0, c->stream, n, c->Ns, t, eta, dt_max, c->spec_dev,
+                     c->blk_idx, acc, jerk, c->soa, c->aos, c->dtj);
         c->launches += 1;
         if (cudaGetLastError() != cudaSuccess) { c->cuda_err = cudaErrorUnknown; rc = NB_ECUDA; }
     }
@@ -1087,11 +1101,11 @@ int sl_enqueue_chain(nb_ctx *c, const double *h2_all, double eta, double dt_max,
 // Two-level chain of a block WITHOUT a regular step (speculative or not): neighbour force over the lists, corrector.
 int ac_enqueue_irregular_chain(nb_ctx *c, double eta_I, double eta_R, double dt_max, int32_t n, double t, bool spec) {
     const double *dev = spec ? c->sel_result : nullptr;
-    irregular_kernel<false><<<(unsigned)((n + 7) / 8), 256, 0, c->stream>>>(n, c->cap, t, dev, 1, 1, c->blk_idx, c->ac.nnb, c->ac.list,
-                                                                            c->aos, c->ac_aIo, c->ac_jIo, nullptr);
-    ac_correct_kernel<<<(unsigned)((n + 127) / 128), 128, 0, c->stream>>>(n, c->Ns, t, eta_I, eta_R, dt_max, dev, c->blk_idx, c->ac_aIo,
-                                                                          c->ac_jIo, 0, c->ac_reg_idx, nullptr, nullptr, nullptr, nullptr,
-                                                                          c->blk_nnb, c->ac, c->soa, c->aos, c->dtj);
+    NB_CUDA(c, launch_chain(irregular_kernel<false>, dim3((unsigned)((n + 7) / 8)), dim3(256), 0, c->stream, n, c->cap, t, dev, 1, 1,
+                            c->blk_idx, c->ac.nnb, c->ac.list, c->aos, c->ac_aIo, c->ac_jIo, nullptr));
+    NB_CUDA(c, launch_chain(ac_correct_kernel, dim3((unsigned)((n + 127) / 128)), dim3(128), 0, c->stream, n, c->Ns, t, eta_I, eta_R,
+                            dt_max, dev, c->blk_idx, c->ac_aIo, c->ac_jIo, 0, c->ac_reg_idx, nullptr, nullptr, nullptr, nullptr,
+                            c->blk_nnb, c->ac, c->soa, c->aos, c->dtj));
     NB_CUDA(c, cudaGetLastError());
     c->launches += 2;
     return NB_OK;

@@ -74,6 +74,10 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
 __device__ __forceinline__ void fence_proxy_async_smem() {   // generic-proxy accesses before, async-proxy (TMA) after
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
 }
+// Kernels of the block chains are launched with programmatic stream serialization (launch_chain in nbreg.cu): the
+// grid is placed while its predecessor in the stream drains; nothing the predecessors wrote may be read before
+// this wait.  A no-op in an ordinary launch.
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 __device__ __forceinline__ float rsqrt_sfu(float x) {   // one MUFU.RSQ, no denormal fix-up code
     float y;
     asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
@@ -694,6 +698,7 @@ __global__ void __launch_bounds__(32 * WI *WJ, MINB) force_kernel(const ForcePar
     const int wi = warp % WI, wj = warp / WI;
     int32_t n_i = p.n_i;
     double t_pred = p.t;
+    pdl_wait();
     if (!spec_block(p.blk_dev, n_i, t_pred)) return;    // (uniform over the grid, before any barrier)
     // j-packed variants: a CTA with <= 16 / 8 active particles (the tiny blocks of the deep levels; the tail
     // of a small block) groups its lanes 2 / 4 ways along j -- decided here, from the block size, so that a
@@ -1072,7 +1077,7 @@ __global__ void __launch_bounds__(32 * W) finalize_kernel(int32_t n_i, int32_t n
     TL_STAMP(4096 + blockIdx.y * gridDim.x + blockIdx.x, 0);
     // launched with programmatic stream serialization: the grid is resident before the force kernel
     // has drained; everything it reads is valid after this wait (a no-op in an ordinary launch)
-    asm volatile("griddepcontrol.wait;" ::: "memory");
+    pdl_wait();
     TL_STAMP(4096 + blockIdx.y * gridDim.x + blockIdx.x, 1);
     {
         double t_unused = 0.0;
@@ -1176,6 +1181,7 @@ __global__ void __launch_bounds__(256) irregular_kernel(int32_t n_i, int32_t cap
                                                         double *__restrict__ jerk, double *__restrict__ pot) {
     const int lane = threadIdx.x & 31;
     const int k = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    pdl_wait();
     if (!spec_block(blk_dev, n_i, t)) return;
     if (k >= n_i) return;
     const int32_t i = idx_i ? idx_i[k] : k;
@@ -1330,6 +1336,7 @@ __global__ void __launch_bounds__(256) select_min_kernel(int64_t N, const double
                                                          const double *__restrict__ dtj, unsigned long long *key,
                                                          unsigned long long *key_next, const int32_t *stall,
                                                          double *__restrict__ ring) {
+    pdl_wait();
     if (*stall) {
         if (blockIdx.x == 0 && threadIdx.x == 0) {
             *key_next = ~0ull;
@@ -1361,6 +1368,7 @@ __global__ void __launch_bounds__(256) select_scatter_kernel(int64_t N, const do
                                                              const double *__restrict__ tR, const double *__restrict__ dtR,
                                                              int32_t *__restrict__ idx_reg, double t_stop, int32_t spec_cap,
                                                              int32_t *stall, double *__restrict__ ring) {
+    pdl_wait();
     if (*stall) return;
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     const int b = blockIdx.x, nchunk = gridDim.x;
@@ -1487,6 +1495,7 @@ __global__ void __launch_bounds__(128) correct_kernel(int32_t n, int64_t Ns, dou
                                                       const double *__restrict__ jerk1, double *__restrict__ soa,
                                                       double *__restrict__ aos, double *__restrict__ dtj) {
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    pdl_wait();
     if (!spec_block(blk_dev, n, t1)) return;
     if (k >= n) return;
     const int64_t i = idx[k];
@@ -1591,6 +1600,7 @@ __global__ void __launch_bounds__(128) ac_correct_kernel(int32_t n, int64_t Ns, 
                                                          double *__restrict__ soa, double *__restrict__ aos,
                                                          double *__restrict__ dtj) {
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    pdl_wait();
     if (!spec_block(blk_dev, n, t)) return;
     if (k >= n) return;
     const int64_t i = idx[k];
