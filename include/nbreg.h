@@ -334,6 +334,10 @@ enum {
                                         in which case the ordinary launches follow.  set 0: always wait for n      */
     NB_INFO_SPEC_HITS = 32,          /* get: blocks integrated by a speculative chain                               */
     NB_INFO_SPEC_MISSES = 33,        /* get: speculative chains that turned out to be no-ops                        */
+    NB_TUNE_SELECT_CHUNKS = 34,      /* set 1 (default): the block loops keep min (t0 + dt) per chunk of 2048 bodies between
+                                        blocks and rescan only the chunks the last corrector touched (the search for
+                                        the due particles must not cost O(N) per block); 0 = scan all N every block.  The
+                                        selected blocks do not depend on it                                            */
     NB_INFO_FORCE_KERNEL_NS_AT = 1000 /* get, key = 1000 + q (q < 256): device time in ns of the q-th bracketed
                                         force-kernel launch since NB_TUNE_PROFILE was set (synchronises)    */
 };

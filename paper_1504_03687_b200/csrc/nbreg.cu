@@ -102,6 +102,10 @@ struct nb_ctx {
     double *blk_ring = nullptr, *h_blk_ring = nullptr;                 // descriptors of a batch of blocks: {t, n, n_reg, status}
     unsigned long long *blk_pub = nullptr;                             // per-chunk counts of the selection, epoch-tagged
     uint32_t blk_epoch = 0;
+    unsigned long long *sel_cmin = nullptr;                            // [chunks of SEL_CHUNK bodies] min of t0 + dt, kept between blocks
+    int32_t *sel_dirty = nullptr;                                      // [chunks] set by the correctors: rescan this chunk
+    bool sel_all_dirty = true;                                         // the state or the steps were replaced: rescan everything
+    bool sel_chunks = true;                                            // NB_TUNE_SELECT_CHUNKS
     int32_t *blk_stall = nullptr;                                      // set by the first block of a batch that needs the host
     bool blk_stall_dirty = true;                                       // the flag must be cleared before the next batch
     int blk_batch = 1;                                                 // blocks enqueued per host round trip (adaptive)
@@ -560,7 +564,7 @@ int nb_close(nb_ctx *c) {
     cudaFree(c->ac.aI); cudaFree(c->ac.jI); cudaFree(c->ac.aR); cudaFree(c->ac.jR); cudaFree(c->ac.tR); cudaFree(c->ac.dtR);
     cudaFree(c->ac.nnb); cudaFree(c->ac.list); cudaFree(c->ac_h2); cudaFree(c->ac_aIo); cudaFree(c->ac_jIo);
     cudaFree(c->ac_reg_idx); cudaFree(c->ac_novf); cudaFree(c->ac_in); cudaFreeHost(c->h_ac_novf);
-    cudaFree(c->blk_stall); cudaFree(c->blk_pub); cudaFreeHost(c->h_blk_ring);
+    cudaFree(c->blk_stall); cudaFree(c->blk_pub); cudaFree(c->sel_cmin); cudaFree(c->sel_dirty); cudaFreeHost(c->h_blk_ring);
     cudaFree(c->partial); cudaFree(c->stage_j);
     cudaFree(c->st_idx); cudaFree(c->st_nnb); cudaFree(c->st_ovf); cudaFree(c->st_list);
     cudaFree(c->st_h2); cudaFree(c->st_out);
@@ -612,6 +616,7 @@ int nb_set_j(nb_ctx *c, const double *m, const double *x0, const double *v0, con
     NB_CUDA(c, cudaGetLastError());
     c->launches += 1;
     c->have_j = true;
+    c->sel_all_dirty = true;    // t0 changed: the per-chunk minima of t0 + dt are stale
     c->have_pred = false; c->pred_pending = false;
     c->have_ac = false;         // the AC force polynomials belong to the state that was just replaced
     return NB_OK;
@@ -648,6 +653,7 @@ int nb_update_j(nb_ctx *c, int32_t n, const int32_t *idx, const double *m, const
     NB_CUDA(c, cudaGetLastError());
     c->launches += 1;
     c->have_pred = false; c->pred_pending = false;   // the predicted records are stale until the next nb_predict_all
+    c->sel_all_dirty = true;
     c->have_ac = false;
     return NB_OK;
 }
@@ -861,6 +867,7 @@ int nb_step_host(nb_ctx *c, const double *m, const double *x0, const double *v0,
         c->launches += 2;
     }
     c->have_j = true;
+    c->sel_all_dirty = true;
     c->have_pred = true; c->pred_pending = false;     // every chunk is predicted as it lands
     c->pred_t = t;
 
@@ -916,6 +923,7 @@ int nb_set_steps(nb_ctx *c, const double *dt) {
     if (!c->dtj) NB_CUDA(c, cudaMalloc(&c->dtj, sizeof(double) * c->N));
     NB_CUDA(c, cudaMemcpyAsync(c->dtj, dt, sizeof(double) * c->N, cudaMemcpyDeviceToDevice, c->stream));
     c->have_steps = true;
+    c->sel_all_dirty = true;
     c->have_ac = false;         // dtj is the irregular step of the two-level scheme: replaced here
     return NB_OK;
 }
@@ -930,6 +938,7 @@ int nb_init_steps(nb_ctx *c, double eta_s, double dt_max) {
     NB_CUDA(c, cudaGetLastError());
     c->launches += 1;
     c->have_steps = true;
+    c->sel_all_dirty = true;
     c->have_ac = false;
     return NB_OK;
 }
@@ -973,7 +982,7 @@ int nb_correct(nb_ctx *c, double t, int32_t n, const int32_t *idx, const double 
     rc = ensure_aos(c);
     if (rc != NB_OK) return rc;
     correct_kernel<<<(unsigned)((n + 127) / 128), 128, 0, c->stream>>>(n, c->Ns, t, eta, dt_max, nullptr, idx, acc1,
-                                                                       jerk1, c->soa, c->aos, c->dtj);
+                                                                       jerk1, c->soa, c->aos, c->dtj, c->sel_dirty);
     NB_CUDA(c, cudaGetLastError());
     c->launches += 1;
     c->have_pred = false; c->pred_pending = false;
@@ -1013,6 +1022,9 @@ int blk_setup(nb_ctx *c) {
     NB_CUDA(c, cudaHostAlloc(&c->h_blk_ring, sizeof(double) * 4 * BLK_BATCH_MAX, cudaHostAllocMapped));
     NB_CUDA(c, cudaHostGetDevicePointer(reinterpret_cast<void **>(&c->blk_ring), c->h_blk_ring, 0));
     NB_CUDA(c, cudaMalloc(&c->blk_stall, sizeof(int32_t)));
+    NB_CUDA(c, cudaMalloc(&c->sel_cmin, sizeof(unsigned long long) * nchunk));
+    NB_CUDA(c, cudaMalloc(&c->sel_dirty, sizeof(int32_t) * nchunk));
+    c->sel_all_dirty = true;
     return NB_OK;
 }
 
@@ -1053,15 +1065,26 @@ int blk_enqueue_select(nb_ctx *c, bool two, double t_stop, int32_t spec_cap, int
     const unsigned nchunk = (unsigned)((N + SEL_CHUNK - 1) / SEL_CHUNK);
     const unsigned gmin = (unsigned)std::min<int64_t>((N + 255) / 256, (int64_t)c->sm_count * 8);
     c->blk_epoch += 1;
-    NB_CUDA(c, launch_chain(select_min_kernel, dim3(gmin), dim3(256), 0, c->stream, N, t0, c->dtj, key, key_next, c->blk_stall, ring));
+    const unsigned long long *cmin = c->sel_chunks ? c->sel_cmin : nullptr;
+    if (c->sel_chunks) {
+        if (c->sel_all_dirty) {       // any non-zero word means "rescan"
+            NB_CUDA(c, cudaMemsetAsync(c->sel_dirty, 1, sizeof(int32_t) * nchunk, c->stream));
+            c->sel_all_dirty = false;
+        }
+        NB_CUDA(c, launch_chain(select_min_chunks_kernel, dim3(nchunk), dim3(256), 0, c->stream, N, t0, c->dtj, c->sel_cmin,
+                                c->sel_dirty, key, key_next, c->blk_stall, ring));
+    } else {
+        c->sel_all_dirty = true;      // the per-chunk minima are not maintained on this route
+        NB_CUDA(c, launch_chain(select_min_kernel, dim3(gmin), dim3(256), 0, c->stream, N, t0, c->dtj, key, key_next, c->blk_stall, ring));
+    }
     if (two)
         NB_CUDA(c, launch_chain(select_scatter_kernel<true>, dim3(nchunk), dim3(256), 0, c->stream, N, t0, c->dtj, key, c->blk_pub,
                                 c->blk_epoch, c->blk_idx, c->sel_result, c->ac.tR, c->ac.dtR, c->ac_reg_idx, t_stop, spec_cap,
-                                c->blk_stall, ring));
+                                c->blk_stall, ring, cmin));
     else
         NB_CUDA(c, launch_chain(select_scatter_kernel<false>, dim3(nchunk), dim3(256), 0, c->stream, N, t0, c->dtj, key, c->blk_pub,
                                 c->blk_epoch, c->blk_idx, c->sel_result, nullptr, nullptr, c->ac_reg_idx, t_stop, spec_cap,
-                                c->blk_stall, ring));
+                                c->blk_stall, ring, cmin));
     NB_CUDA(c, cudaGetLastError());
     c->blk_parity ^= 1;
     c->launches += 2;
@@ -1088,7 +1111,7 @@ int sl_enqueue_chain(nb_ctx *c, const double *h2_all, double eta, double dt_max,
     }
     if (rc == NB_OK) {
         launch_chain(correct_kernel, dim3((unsigned)((n + 127) / 128)), dim3(128), 0, c->stream, n, c->Ns, t, eta, dt_max, c->spec_dev,
-                     c->blk_idx, acc, jerk, c->soa, c->aos, c->dtj);
+                     c->blk_idx, acc, jerk, c->soa, c->aos, c->dtj, c->sel_dirty);
         c->launches += 1;
         if (cudaGetLastError() != cudaSuccess) { c->cuda_err = cudaErrorUnknown; rc = NB_ECUDA; }
     }
@@ -1105,7 +1128,7 @@ int ac_enqueue_irregular_chain(nb_ctx *c, double eta_I, double eta_R, double dt_
                             c->blk_idx, c->ac.nnb, c->ac.list, c->aos, c->ac_aIo, c->ac_jIo, nullptr));
     NB_CUDA(c, launch_chain(ac_correct_kernel, dim3((unsigned)((n + 127) / 128)), dim3(128), 0, c->stream, n, c->Ns, t, eta_I, eta_R,
                             dt_max, dev, c->blk_idx, c->ac_aIo, c->ac_jIo, 0, c->ac_reg_idx, nullptr, nullptr, nullptr, nullptr,
-                            c->blk_nnb, c->ac, c->soa, c->aos, c->dtj));
+                            c->blk_nnb, c->ac, c->soa, c->aos, c->dtj, c->sel_dirty));
     NB_CUDA(c, cudaGetLastError());
     c->launches += 2;
     return NB_OK;
@@ -1146,7 +1169,7 @@ int ac_finish_block(nb_ctx *c, double eta_I, double eta_R, double dt_max, double
     }
     ac_correct_kernel<<<(unsigned)((n + 127) / 128), 128, 0, c->stream>>>(n, c->Ns, t, eta_I, eta_R, dt_max, nullptr, c->blk_idx, c->ac_aIo,
                                                                           c->ac_jIo, nr, c->ac_reg_idx, rg_acc, rg_jerk, in_acc, in_jerk,
-                                                                          c->blk_nnb, c->ac, c->soa, c->aos, c->dtj);
+                                                                          c->blk_nnb, c->ac, c->soa, c->aos, c->dtj, c->sel_dirty);
     ac_store_rows_kernel<<<(unsigned)((nr + 7) / 8), 256, 0, c->stream>>>(nr, c->cap, c->ac_reg_idx, c->blk_nnb, c->blk_list, c->ac.list);
     NB_CUDA(c, cudaGetLastError());
     c->launches += 2;
@@ -1320,6 +1343,7 @@ int nb_ac_init(nb_ctx *c, double t_start, const double *h2_all, double eta_s, do
     NB_CUDA(c, cudaStreamSynchronize(c->stream));
     c->have_pred = false; c->pred_pending = false;
     c->have_steps = true;
+    c->sel_all_dirty = true;
     if (n_overflow) *n_overflow = *c->h_ac_novf;
     c->have_ac = *c->h_ac_novf == 0;
     return c->have_ac ? NB_OK : NB_EOVERFLOW;
@@ -1486,6 +1510,7 @@ int nb_get_info(nb_ctx *c, int32_t key, int64_t *value) {
         case NB_INFO_SPEC_HITS: *value = c->spec_hits; break;
         case NB_INFO_SPEC_MISSES: *value = c->spec_misses; break;
         case NB_TUNE_REORDER_MIN: *value = c->reorder_min; break;
+        case NB_TUNE_SELECT_CHUNKS: *value = c->sel_chunks ? 1 : 0; break;
         case NB_INFO_LOCAL_WARPS:
         case NB_INFO_TOTAL_WARPS: {
             if (!c->stats) return NB_ESTATE;
@@ -1552,6 +1577,9 @@ int nb_set_tuning(nb_ctx *c, int32_t key, int64_t value) {
         case NB_TUNE_REORDER_MIN:
             if (value < 0) return NB_EINVAL;
             c->reorder_min = value; break;
+        case NB_TUNE_SELECT_CHUNKS:
+            if (value != 0 && value != 1) return NB_EINVAL;
+            c->sel_chunks = value != 0; break;
         case NB_TUNE_STATS:
             if (value != 0 && value != 1) return NB_EINVAL;
             if (value) {

@@ -1360,6 +1360,54 @@ __global__ void __launch_bounds__(256) select_min_kernel(int64_t N, const double
     }
 }
 
+// The same minimum from per-chunk minima (section 3.3.1: the search for the due particles must not cost O(N)
+// per block when the deep blocks hold a handful of particles).  cmin[b] = min over chunk b of t0 + dt, kept
+// between blocks; the correctors flag the chunks of the bodies they integrate (dirty[b] = 1) and only those
+// chunks are scanned again here.  One CTA per chunk; everything else reads one word.  The library flags every
+// chunk when the state or the steps are replaced from outside the chain.
+__global__ void __launch_bounds__(256) select_min_chunks_kernel(int64_t N, const double *__restrict__ t0,
+                                                                const double *__restrict__ dtj,
+                                                                unsigned long long *__restrict__ cmin,
+                                                                int32_t *__restrict__ dirty, unsigned long long *key,
+                                                                unsigned long long *key_next, const int32_t *stall,
+                                                                double *__restrict__ ring) {
+    pdl_wait();
+    if (*stall) {
+        if (blockIdx.x == 0 && threadIdx.x == 0) {
+            *key_next = ~0ull;
+            *reinterpret_cast<volatile double *>(ring + 3) = (double)BLK_SKIPPED;
+        }
+        return;
+    }
+    const int b = blockIdx.x;
+    if (!dirty[b]) {                                  // (uniform over the CTA)
+        if (threadIdx.x == 0) {
+            atomicMin(key, cmin[b]);
+            if (b == 0) *key_next = ~0ull;
+        }
+        return;
+    }
+    unsigned long long best = ~0ull;
+#pragma unroll
+    for (int u = 0; u < SEL_CHUNK / 256; ++u) {
+        const int64_t j = (int64_t)b * SEL_CHUNK + u * 256 + threadIdx.x;
+        if (j < N) best = min(best, ordered_key(t0[j] + dtj[j]));
+    }
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) best = min(best, __shfl_xor_sync(0xffffffffu, best, off));
+    __shared__ unsigned long long wbest[8];
+    if ((threadIdx.x & 31) == 0) wbest[threadIdx.x >> 5] = best;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int w = 1; w < 8; ++w) best = min(best, wbest[w]);
+        cmin[b] = best;
+        dirty[b] = 0;
+        atomicMin(key, best);
+        if (b == 0) *key_next = ~0ull;
+    }
+}
+
 template <bool TWO>
 __global__ void __launch_bounds__(256) select_scatter_kernel(int64_t N, const double *__restrict__ t0,
                                                              const double *__restrict__ dtj, const unsigned long long *key,
@@ -1367,7 +1415,8 @@ __global__ void __launch_bounds__(256) select_scatter_kernel(int64_t N, const do
                                                              int32_t *__restrict__ idx_act, double *__restrict__ result,
                                                              const double *__restrict__ tR, const double *__restrict__ dtR,
                                                              int32_t *__restrict__ idx_reg, double t_stop, int32_t spec_cap,
-                                                             int32_t *stall, double *__restrict__ ring) {
+                                                             int32_t *stall, double *__restrict__ ring,
+                                                             const unsigned long long *__restrict__ cmin) {
     pdl_wait();
     if (*stall) return;
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
@@ -1375,14 +1424,16 @@ __global__ void __launch_bounds__(256) select_scatter_kernel(int64_t N, const do
     constexpr int PER = SEL_CHUNK / 256;
     __shared__ int32_t wsum[8], wsum2[8];
     __shared__ int32_t base_s, base2_s;
-    const double tn = key_to_double(*key);
+    const unsigned long long kmin = *key;
+    const double tn = key_to_double(kmin);
+    const bool here = !cmin || cmin[b] == kmin;     // only a chunk whose own minimum is t_next holds due bodies
     // ---- this chunk's active bodies (kept as flags) and their number
     bool act[PER], due[PER];
     int32_t cntc = 0, cnt2 = 0;
 #pragma unroll
     for (int u = 0; u < PER; ++u) {
         const int64_t j = (int64_t)b * SEL_CHUNK + u * 256 + threadIdx.x;
-        act[u] = j < N && (t0[j] + dtj[j] == tn);
+        act[u] = here && j < N && (t0[j] + dtj[j] == tn);
         due[u] = TWO && act[u] && (tR[j] + dtR[j] == tn);
         cntc += act[u] ? 1 : 0;
         cnt2 += due[u] ? 1 : 0;
@@ -1493,7 +1544,8 @@ __global__ void __launch_bounds__(128) correct_kernel(int32_t n, int64_t Ns, dou
                                                       const int32_t *__restrict__ idx,
                                                       const double *__restrict__ acc1,
                                                       const double *__restrict__ jerk1, double *__restrict__ soa,
-                                                      double *__restrict__ aos, double *__restrict__ dtj) {
+                                                      double *__restrict__ aos, double *__restrict__ dtj,
+                                                      int32_t *__restrict__ sel_dirty) {
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
     pdl_wait();
     if (!spec_block(blk_dev, n, t1)) return;
@@ -1529,6 +1581,7 @@ __global__ void __launch_bounds__(128) correct_kernel(int32_t n, int64_t Ns, dou
     }
     store_body(i, Ns, m, x1, v1, a1, j1, t1, soa, aos);
     dtj[i] = d;
+    if (sel_dirty) sel_dirty[i / SEL_CHUNK] = 1;      // this chunk's minimum of t0 + dt is out of date (select_min_chunks_kernel)
 }
 
 // ------------------------------------------------------------------ NEXT-3: two-level Ahmad-Cohen stepping
@@ -1598,7 +1651,7 @@ __global__ void __launch_bounds__(128) ac_correct_kernel(int32_t n, int64_t Ns, 
                                                          const double *__restrict__ in_acc, const double *__restrict__ in_jerk,
                                                          const int32_t *__restrict__ rg_nnb, const AcState A,
                                                          double *__restrict__ soa, double *__restrict__ aos,
-                                                         double *__restrict__ dtj) {
+                                                         double *__restrict__ dtj, int32_t *__restrict__ sel_dirty) {
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
     pdl_wait();
     if (!spec_block(blk_dev, n, t)) return;
@@ -1669,6 +1722,7 @@ __global__ void __launch_bounds__(128) ac_correct_kernel(int32_t n, int64_t Ns, 
     for (int c = 0; c < 3; ++c) { A.aI[3 * i + c] = aI1[c]; A.jI[3 * i + c] = jI1[c]; }
     store_body(i, Ns, m, x1, v1, a1, j1, t, soa, aos);
     dtj[i] = dI;
+    if (sel_dirty) sel_dirty[i / SEL_CHUNK] = 1;
 }
 
 // New list rows of the regular-active bodies into the persistent by-body lists: one warp per row.

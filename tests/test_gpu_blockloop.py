@@ -377,3 +377,49 @@ def test_block_step_stops_at_t_stop_and_closed_loop_conserves_energy():
     assert abs(psteps - ref["particle_steps"]) <= 0.01 * ref["particle_steps"]
     assert np.abs(s1["x0"] - ref["x0"]).max() < 1e-5
     ctx.close()
+
+
+def test_selection_from_chunk_minima_equals_the_full_scan():
+    """The block loops keep min (t0 + dt) per 2048-body chunk and rescan only the chunks the last corrector
+    touched (section 3.3.1: the search for the due particles must not cost O(N) per block).  Same blocks,
+    bit-identical state as with the full scan (NB_TUNE_SELECT_CHUNKS = 0) -- over single calls and batched
+    loops, and after the state and the steps were replaced from outside the chain (nb_update_j with new t0,
+    nb_set_steps), which must invalidate every stored minimum.  N spans several chunks and a ragged one."""
+    import paper_1504_03687_b200 as nb
+    cfg = nbgen.make_config(3, N=20000, n_i=16)
+    N = cfg["N"]
+    dt = 2.0 ** -cfg["levels"].astype(np.float64)
+    t0 = np.floor(0.3 / dt) * dt
+    eta, dt_max = 0.02, 2.0**-6
+    rng = np.random.default_rng(5)
+    upd = np.sort(rng.choice(N, 37, replace=False)).astype(np.int32)
+
+    def run(chunks):
+        ctx = nb.nb_open(N, 8)
+        ctx.tune("select_chunks", chunks)
+        nb.nb_set_j(ctx, *(_dev(a) for a in (cfg["m"], cfg["x0"], cfg["v0"], cfg["a0"], cfg["j0"], t0)))
+        ctx.set_steps(_dev(dt))
+        log = []
+        for _ in range(25):
+            log.append(ctx.block_step(None, eta, dt_max))
+        log.append(ctx.run_blocks(None, eta, dt_max, t_stop=1.0e9, max_blocks=40))
+        # replace 37 bodies (earlier t0: they become the next block) and then every step
+        s = _state(ctx)
+        t_now = log[-1][0]
+        ctx.update_j(_dev(upd), *(_dev(a) for a in (cfg["m"][upd], s["x0"][upd], s["v0"][upd], s["a0"][upd], s["j0"][upd],
+                                                    np.full(upd.size, t_now - 2.0**-9))))
+        log.append(ctx.block_step(None, eta, dt_max))
+        log.append(ctx.run_blocks(None, eta, dt_max, t_stop=1.0e9, max_blocks=10))
+        ctx.set_steps(_dev(np.minimum(_state(ctx)["dt"], 2.0**-12)))
+        for _ in range(6):
+            log.append(ctx.block_step(None, eta, dt_max))
+        log.append(ctx.run_blocks(None, eta, dt_max, t_stop=1.0e9, max_blocks=30))
+        out = _state(ctx)
+        ctx.close()
+        return log, out
+
+    log1, s1 = run(1)
+    log0, s0 = run(0)
+    assert log1 == log0
+    assert 0 < log1[26][1] <= upd.size and log1[26][0] < log1[25][0]   # the replaced bodies (earlier t0) were found
+    assert all(np.array_equal(s1[k], s0[k]) for k in s1)
