@@ -17,6 +17,19 @@ def test_library_builds_and_exports_every_declared_symbol():
     assert lib.nb_strerror(0) == b"ok" and b"invalid" in lib.nb_strerror(1)
 
 
+def test_binding_keys_match_the_header_enum():
+    """nb_get_info / nb_set_tuning keys: the binding's table carries the numbers include/nbreg.h defines."""
+    import re
+    from pathlib import Path
+    from paper_1504_03687_b200.binding import INFO
+    text = (Path(__file__).resolve().parent.parent / "include" / "nbreg.h").read_text()
+    enum = {m.group(2).lower(): int(m.group(3)) for m in re.finditer(r"\b(NB_INFO|NB_TUNE)_([A-Z_]+)\s*=\s*(\d+)", text)}
+    assert len(enum) >= 20
+    for key, val in INFO.items():
+        assert enum.get(key) == val, key
+    assert set(enum) == set(INFO)
+
+
 def test_argument_validation_without_compute():
     import paper_1504_03687_b200 as nb
     lib = nb.load_library()
