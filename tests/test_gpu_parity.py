@@ -231,6 +231,37 @@ def test_everyone_is_a_neighbour(oracle):
     assert np.all(got["nnb"] == 1999) and not got["acc"].any() and not got["pot"].any()
 
 
+@pytest.mark.parametrize("N", [1, 2, 3, 37, 255, 256, 257, 513])
+def test_degenerate_sizes_everybody_active(oracle, N):
+    """The smallest problems: N = 1 (no pair at all: exact zeros), 2, 3, one ragged tile, exactly one tile, one
+    tile + 1, two tiles + 1 -- everybody active, seeded uniform cube with random masses / velocities / steps, a
+    radius that gives a few neighbours, cap 4 (some rows overflow).  By both routes (records; FP64 state with the
+    predictor fused where the block is small enough) and with h2 = 0 (momentum: sum m a = 0)."""
+    rng = np.random.default_rng(1000 + N)
+    x0 = rng.uniform(-1, 1, (N, 3)); v0 = rng.normal(0, 0.3, (N, 3))
+    a0 = rng.normal(0, 0.5, (N, 3)); j0 = rng.normal(0, 0.5, (N, 3))
+    t0 = 1.0 - 2.0 ** -rng.integers(3, 9, N).astype(np.float64)
+    m = rng.uniform(0.5, 1.5, N) / N
+    cfg = dict(N=N, cap=4, m=m, x0=x0, v0=v0, a0=a0, j0=j0, t0=t0, t=1.0)
+    idx = np.arange(N, dtype=np.int32)
+    h2 = np.full(N, (0.9 * (8.0 / max(N, 2)) ** (1.0 / 3.0)) ** 2)        # ~3 neighbours each
+    for fuse in (1, 0):
+        ctx = open_ctx(cfg)
+        ctx.tune("fuse_predict", fuse)
+        rep, got, ref = check(oracle, ctx, cfg, idx_i=idx, h2_i=h2, cap=4)
+        assert ctx.info("last_fused") == (1 if fuse and N <= 128 else 0)
+        if N == 1:
+            assert not got["acc"].any() and not got["jerk"].any() and got["pot"][0] == 0 and got["nnb"][0] == 0
+        if N >= 37:
+            assert got["nnb"].max() > 0
+        rep0, got0, _ = check(oracle, ctx, cfg, idx_i=idx, h2_i=np.zeros(N), cap=4)
+        assert got0["nnb"].sum() == 0
+        if N > 1:
+            f = (m[:, None] * got0["acc"]).sum(0)
+            assert np.abs(f).max() < 2e-6 * np.abs(m[:, None] * got0["acc"]).sum()
+        ctx.close()
+
+
 def test_two_body_closed_form():
     import paper_1504_03687_b200 as nb
     cfg = dict(N=2, cap=4, m=np.array([1.0, 1.0]), x0=np.array([[0, 0, 0], [3.0, 4.0, 0]]),
