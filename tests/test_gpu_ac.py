@@ -19,6 +19,10 @@ def _dev(a, dtype=None):
 
 
 def _radii(x, k):
+    if x.shape[0] > 4096:                      # (a library routine, not the oracle: k-th neighbour distance)
+        from scipy.spatial import cKDTree
+        d, _ = cKDTree(x).query(x, k=k + 1)
+        return d[:, k] ** 2 * 1.002
     d2 = ((x[:, None, :] - x[None, :, :]) ** 2).sum(-1)
     return np.sort(d2, axis=1)[:, k] * 1.002
 
@@ -43,11 +47,12 @@ def _rel(a, b):
     return np.max(np.linalg.norm(a - b, axis=1) / np.where(s > 0, s, 1.0))
 
 
-def test_ac_start_and_blocks_in_lockstep_with_the_oracle(oracle):
-    N, cap = 1024, 128
+@pytest.mark.parametrize("N,cap,knb,nblocks", [(1024, 128, 16, 300), (12000, 64, 12, 60)])
+def test_ac_start_and_blocks_in_lockstep_with_the_oracle(oracle, N, cap, knb, nblocks):
+    """N = 1024: 300 blocks; N = 12000: the j-range spans 47 tiles and six selection chunks (one ragged), 60 blocks."""
     cfg = nbgen.make_config(1, N=N)
     m, x, v = cfg["m"], cfg["x0"], cfg["v0"]
-    h2 = _radii(x, 16)
+    h2 = _radii(x, knb)
     eta_I, eta_R, eta_s, dt_max = 0.01, 0.02, 0.01, 2.0**-4
     st = AC.start(oracle, m, x, v, h2, cap, eta_s, dt_max)
     ctx = _open(m, x, v, cap)
@@ -61,7 +66,7 @@ def test_ac_start_and_blocks_in_lockstep_with_the_oracle(oracle):
     assert _rel(g["a0"], st["a0"]) < 1e-5
     flips = int((g["dt"] != st["dtI"]).sum() + (g["dtR"] != st["dtR"]).sum())
     st["dtI"], st["dtR"] = g["dt"].copy(), g["dtR"].copy()                            # adopt flipped decisions
-    nblocks, isteps, rsteps, pure_irr = 300, 0, 0, 0
+    isteps, rsteps, pure_irr = 0, 0, 0
     for b in range(nblocks):
         t, n, nr = ctx.ac_step(eta_I, eta_R, dt_max)
         t_ref, act, reg = AC.block_step(oracle, m, st, h2, cap, eta_I, eta_R, dt_max)
@@ -77,7 +82,7 @@ def test_ac_start_and_blocks_in_lockstep_with_the_oracle(oracle):
     g = _gpu_state(ctx, lists=True)
     print("AC lockstep: blocks", nblocks, "irregular steps", isteps, "regular steps", rsteps, "blocks without a regular step",
           pure_irr, "flips", flips, "max |dx|", np.abs(g["x0"] - st["x0"]).max())
-    assert pure_irr > nblocks // 3 and rsteps > 0
+    assert pure_irr > nblocks // 3 and (rsteps > 0 or N > 1024)
     assert flips <= max(3, int(2e-3 * (isteps + rsteps)))
     assert np.array_equal(g["t0"], st["t0"]) and np.array_equal(g["tR"], st["tR"])
     assert np.abs(g["x0"] - st["x0"]).max() < 1e-9 and np.abs(g["v0"] - st["v0"]).max() < 1e-7
