@@ -549,6 +549,11 @@ def run_b200(args):
             torch.cuda.synchronize()
             segs.append({"blocks": int(nb_run), "irregular_steps": int(ni_run), "regular_steps": int(nr_run),
                          "us_per_block_mean": (time.perf_counter() - tw) * 1e6 / max(nb_run, 1)})
+        tw = time.perf_counter()                          # and a long stretch: 2000 blocks in one call
+        _, nb_long, ni_long, nr_long = actx.ac_run(0.02, 0.03, 2.0 ** -6, max_blocks=2000)
+        torch.cuda.synchronize()
+        ac_long = {"blocks": int(nb_long), "irregular_steps": int(ni_long), "regular_steps": int(nr_long),
+                   "ms": (time.perf_counter() - tw) * 1e3, "us_per_block_mean": (time.perf_counter() - tw) * 1e6 / max(nb_long, 1)}
         spec_ac = {"hits": actx.info("spec_hits"), "misses": actx.info("spec_misses")}
         actx.close()
         cyc = np.diff(np.array(stamps_a))[1:] * 1e6
@@ -559,7 +564,7 @@ def run_b200(args):
                   "blocks_without_regular_step": int((kinds_a[:, 1] == 0).sum()),
                   "us_per_block_without_regular_step": float(np.median(cyc[irr_only])) if irr_only.any() else None,
                   "us_per_block_with_regular_step": float(np.median(cyc[with_reg])) if with_reg.any() else None,
-                  "nb_ac_run_segments_of_100_blocks": segs, "speculation": spec_ac,
+                  "nb_ac_run_segments_of_100_blocks": segs, "nb_ac_run_2000_blocks": ac_long, "speculation": spec_ac,
                   "n_reg_median_when_due": float(np.median(kinds_a[kinds_a[:, 1] > 0, 1])) if (kinds_a[:, 1] > 0).any() else None,
                   "note": "config 4 at t = 0 with the block radii (150 neighbours, cap 512); host wall clock between the returns "
                           "of consecutive nb_ac_step calls"}

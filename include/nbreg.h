@@ -158,7 +158,9 @@ int nb_step_host(nb_ctx *ctx, const double *m, const double *x0, const double *v
  *     pot[k] = - sum_j m_j / r           (pot may be NULL)
  * in FP64 throughout (max rel. error vs the FP64 definition ~1e-13).  nnb / nblist have the layout
  * nb_regular writes ([n_i], [n_i][nb_cap]) and may be its outputs unchanged; a row that overflowed
- * contributes its nb_cap stored entries.  DEVICE pointers.  Requires nb_set_j. */
+ * contributes its nb_cap stored entries.  A large block (NB_TUNE_IRR_PRED_MIN bodies or more) predicts all N bodies
+ * once into library-owned 64 B records and gathers those; the results are the same bits.  DEVICE pointers.
+ * Requires nb_set_j. */
 int nb_irregular(nb_ctx *ctx, double t, int32_t n_i, const int32_t *idx_i, const int32_t *nnb,
                  const int32_t *nblist, double *acc, double *jerk, double *pot);
 
@@ -338,6 +340,9 @@ enum {
                                         blocks and rescan only the chunks the last corrector touched (the search for
                                         the due particles must not cost O(N) per block); 0 = scan all N every block.  The
                                         selected blocks do not depend on it                                            */
+    NB_TUNE_IRR_PRED_MIN = 35,       /* set: the neighbour force of a block of at least this many bodies (default 24576; 0 =
+                                        never) predicts every body once into 64 B records and gathers those instead of
+                                        predicting each listed neighbour from its 128 B state line.  Same bits either way   */
     NB_INFO_FORCE_KERNEL_NS_AT = 1000 /* get, key = 1000 + q (q < 256): device time in ns of the q-th bracketed
                                         force-kernel launch since NB_TUNE_PROFILE was set (synchronises)    */
 };

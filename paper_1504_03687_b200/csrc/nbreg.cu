@@ -106,6 +106,8 @@ struct nb_ctx {
     int32_t *sel_dirty = nullptr;                                      // [chunks] set by the correctors: rescan this chunk
     bool sel_all_dirty = true;                                         // the state or the steps were replaced: rescan everything
     bool sel_chunks = true;                                            // NB_TUNE_SELECT_CHUNKS
+    double *p64 = nullptr;                                             // [N][8] FP64 predicted records of a large block's neighbour force
+    int64_t irr_pred_min = 24576;                                      // NB_TUNE_IRR_PRED_MIN: blocks of at least this many bodies use them
     int32_t *blk_stall = nullptr;                                      // set by the first block of a batch that needs the host
     bool blk_stall_dirty = true;                                       // the flag must be cleared before the next batch
     int blk_batch = 1;                                                 // blocks enqueued per host round trip (adaptive)
@@ -347,6 +349,38 @@ int ensure_aos(nb_ctx *c) {
     return NB_OK;
 }
 
+// NEXT-2 launch: the neighbour force of n bodies at time t.  A large block (not a speculative launch, whose size
+// the host does not know) predicts every body once into 64 B records and gathers those (irregular_kernel<., true>);
+// p64_ready: the records of this t are in place already (second pass of the same block).
+template <bool ACCUM>
+int launch_irregular(nb_ctx *c, bool chain, int32_t n, double t, const double *dev, int32_t rows_by_body, int32_t out_by_body,
+                     const int32_t *idx, const int32_t *nnb, const int32_t *list, double *acc, double *jerk, double *pot,
+                     bool p64_ready = false) {
+    const bool pred = dev == nullptr && c->irr_pred_min > 0 && n >= c->irr_pred_min;
+    if (pred && !p64_ready) {
+        if (!c->p64) NB_CUDA(c, cudaMalloc(&c->p64, sizeof(double) * P64_D * c->N));
+        predict64_kernel<<<(unsigned)((c->N + 255) / 256), 256, 0, c->stream>>>(c->N, t, c->aos, c->p64);
+        NB_CUDA(c, cudaGetLastError());
+        c->launches += 1;
+    }
+    const dim3 grid((unsigned)((n + 7) / 8)), block(256);
+    const double *src = pred ? c->p64 : c->aos;
+    if (chain) {
+        if (pred) NB_CUDA(c, launch_chain(irregular_kernel<ACCUM, true>, grid, block, 0, c->stream, n, c->cap, t, dev, rows_by_body,
+                                          out_by_body, idx, nnb, list, src, acc, jerk, pot));
+        else NB_CUDA(c, launch_chain(irregular_kernel<ACCUM, false>, grid, block, 0, c->stream, n, c->cap, t, dev, rows_by_body,
+                                     out_by_body, idx, nnb, list, src, acc, jerk, pot));
+    } else {
+        if (pred) irregular_kernel<ACCUM, true><<<grid, block, 0, c->stream>>>(n, c->cap, t, dev, rows_by_body, out_by_body, idx, nnb,
+                                                                              list, src, acc, jerk, pot);
+        else irregular_kernel<ACCUM, false><<<grid, block, 0, c->stream>>>(n, c->cap, t, dev, rows_by_body, out_by_body, idx, nnb,
+                                                                          list, src, acc, jerk, pot);
+        NB_CUDA(c, cudaGetLastError());
+    }
+    c->launches += 1;
+    return NB_OK;
+}
+
 // a6-a7: fixed-order sum of the S partial rows, counters, sorted list rows.  perm (or NULL): slot -> k of
 // a block the library reordered (Morton order, reorder_block).
 int launch_finalize(nb_ctx *c, int32_t n_i, int64_t n_i_pad, int S, const unsigned long long *perm, double *acc, double *jerk,
@@ -564,7 +598,7 @@ int nb_close(nb_ctx *c) {
     cudaFree(c->ac.aI); cudaFree(c->ac.jI); cudaFree(c->ac.aR); cudaFree(c->ac.jR); cudaFree(c->ac.tR); cudaFree(c->ac.dtR);
     cudaFree(c->ac.nnb); cudaFree(c->ac.list); cudaFree(c->ac_h2); cudaFree(c->ac_aIo); cudaFree(c->ac_jIo);
     cudaFree(c->ac_reg_idx); cudaFree(c->ac_novf); cudaFree(c->ac_in); cudaFreeHost(c->h_ac_novf);
-    cudaFree(c->blk_stall); cudaFree(c->blk_pub); cudaFree(c->sel_cmin); cudaFree(c->sel_dirty); cudaFreeHost(c->h_blk_ring);
+    cudaFree(c->blk_stall); cudaFree(c->blk_pub); cudaFree(c->sel_cmin); cudaFree(c->sel_dirty); cudaFree(c->p64); cudaFreeHost(c->h_blk_ring);
     cudaFree(c->partial); cudaFree(c->stage_j);
     cudaFree(c->st_idx); cudaFree(c->st_nnb); cudaFree(c->st_ovf); cudaFree(c->st_list);
     cudaFree(c->st_h2); cudaFree(c->st_out);
@@ -668,11 +702,7 @@ int nb_irregular(nb_ctx *c, double t, int32_t n_i, const int32_t *idx_i, const i
     if (!idx_i || !nnb || !nblist || !acc || !jerk) return NB_EINVAL;
     rc = ensure_aos(c);
     if (rc != NB_OK) return rc;
-    irregular_kernel<false><<<(unsigned)((n_i + 7) / 8), 256, 0, c->stream>>>(n_i, c->cap, t, nullptr, 0, 0, idx_i, nnb,
-                                                                              nblist, c->aos, acc, jerk, pot);
-    NB_CUDA(c, cudaGetLastError());
-    c->launches += 1;
-    return NB_OK;
+    return launch_irregular<false>(c, false, n_i, t, nullptr, 0, 0, idx_i, nnb, nblist, acc, jerk, pot);
 }
 
 int nb_predict_all(nb_ctx *c, double t) {
@@ -1105,9 +1135,7 @@ int sl_enqueue_chain(nb_ctx *c, const double *h2_all, double eta, double dt_max,
         rc = regular_device(c, n, c->blk_idx, h2_all, acc, jerk, pot, c->blk_nnb, h2_all ? c->blk_list : nullptr, c->blk_ovf);
     c->h2_by_body = 0;
     if (rc == NB_OK && h2_all) {
-        launch_chain(irregular_kernel<true>, dim3((unsigned)((n + 7) / 8)), dim3(256), 0, c->stream, n, c->cap, t, c->spec_dev, 0, 0,
-                     c->blk_idx, c->blk_nnb, c->blk_list, c->aos, acc, jerk, pot);
-        c->launches += 1;
+        rc = launch_irregular<true>(c, true, n, t, c->spec_dev, 0, 0, c->blk_idx, c->blk_nnb, c->blk_list, acc, jerk, pot);
     }
     if (rc == NB_OK) {
         launch_chain(correct_kernel, dim3((unsigned)((n + 127) / 128)), dim3(128), 0, c->stream, n, c->Ns, t, eta, dt_max, c->spec_dev,
@@ -1124,13 +1152,13 @@ int sl_enqueue_chain(nb_ctx *c, const double *h2_all, double eta, double dt_max,
 // Two-level chain of a block WITHOUT a regular step (speculative or not): neighbour force over the lists, corrector.
 int ac_enqueue_irregular_chain(nb_ctx *c, double eta_I, double eta_R, double dt_max, int32_t n, double t, bool spec) {
     const double *dev = spec ? c->sel_result : nullptr;
-    NB_CUDA(c, launch_chain(irregular_kernel<false>, dim3((unsigned)((n + 7) / 8)), dim3(256), 0, c->stream, n, c->cap, t, dev, 1, 1,
-                            c->blk_idx, c->ac.nnb, c->ac.list, c->aos, c->ac_aIo, c->ac_jIo, nullptr));
+    int rc = launch_irregular<false>(c, true, n, t, dev, 1, 1, c->blk_idx, c->ac.nnb, c->ac.list, c->ac_aIo, c->ac_jIo, nullptr);
+    if (rc != NB_OK) return rc;
     NB_CUDA(c, launch_chain(ac_correct_kernel, dim3((unsigned)((n + 127) / 128)), dim3(128), 0, c->stream, n, c->Ns, t, eta_I, eta_R,
                             dt_max, dev, c->blk_idx, c->ac_aIo, c->ac_jIo, 0, c->ac_reg_idx, nullptr, nullptr, nullptr, nullptr,
                             c->blk_nnb, c->ac, c->soa, c->aos, c->dtj, c->sel_dirty));
     NB_CUDA(c, cudaGetLastError());
-    c->launches += 2;
+    c->launches += 1;
     return NB_OK;
 }
 
@@ -1140,9 +1168,9 @@ int ac_finish_block(nb_ctx *c, double eta_I, double eta_R, double dt_max, double
     *n_overflow = 0;
     int rc = blk_buffers(c, nr, true, true);
     if (rc != NB_OK) return rc;
-    irregular_kernel<false><<<(unsigned)((n + 7) / 8), 256, 0, c->stream>>>(n, c->cap, t, nullptr, 1, 1, c->blk_idx, c->ac.nnb,
-                                                                            c->ac.list, c->aos, c->ac_aIo, c->ac_jIo, nullptr);
-    c->launches += 1;
+    rc = launch_irregular<false>(c, false, n, t, nullptr, 1, 1, c->blk_idx, c->ac.nnb, c->ac.list, c->ac_aIo, c->ac_jIo, nullptr);
+    if (rc != NB_OK) return rc;
+    const bool p64_ready = c->irr_pred_min > 0 && n >= c->irr_pred_min;      // the block's records are in place (nr <= n)
     double *rg_acc = c->blk_out, *rg_jerk = c->blk_out + 3 * (int64_t)nr, *rg_pot = c->blk_out + 6 * (int64_t)nr;
     double *in_acc = c->ac_in, *in_jerk = c->ac_in + 3 * (int64_t)nr;
     c->have_pred = true; c->pred_pending = true; c->pred_t = t;
@@ -1155,8 +1183,9 @@ int ac_finish_block(nb_ctx *c, double eta_I, double eta_R, double dt_max, double
     c->h2_by_body = 0;
     c->have_pred = false; c->pred_pending = false;
     if (rc != NB_OK) return rc;
-    irregular_kernel<false><<<(unsigned)((nr + 7) / 8), 256, 0, c->stream>>>(nr, c->cap, t, nullptr, 0, 0, c->ac_reg_idx, c->blk_nnb,
-                                                                             c->blk_list, c->aos, in_acc, in_jerk, nullptr);
+    rc = launch_irregular<false>(c, false, nr, t, nullptr, 0, 0, c->ac_reg_idx, c->blk_nnb, c->blk_list, in_acc, in_jerk, nullptr,
+                                 p64_ready);
+    if (rc != NB_OK) return rc;
     // a list that overflowed would break regular + irregular = total (R38): checked BEFORE anything is corrected
     NB_CUDA(c, cudaMemsetAsync(c->ac_novf, 0, sizeof(int32_t), c->stream));
     count_overflow_kernel<<<(unsigned)std::min<int64_t>((nr + 255) / 256, 1024), 256, 0, c->stream>>>(nr, c->blk_ovf, c->ac_novf);
@@ -1332,8 +1361,9 @@ int nb_ac_init(nb_ctx *c, double t_start, const double *h2_all, double eta_s, do
     rc = regular_device(c, (int32_t)N, nullptr, c->ac_h2, c->ac.aR, c->ac.jR, c->ac_aIo /* pot: scratch */, c->ac.nnb,
                         c->ac.list, ovf_all);
     if (rc != NB_OK) return rc;
-    irregular_kernel<false><<<(unsigned)((N + 7) / 8), 256, 0, c->stream>>>((int32_t)N, c->cap, t_start, nullptr, 0, 0, nullptr,
-                                                                            c->ac.nnb, c->ac.list, c->aos, c->ac.aI, c->ac.jI, nullptr);
+    rc = launch_irregular<false>(c, false, (int32_t)N, t_start, nullptr, 0, 0, nullptr, c->ac.nnb, c->ac.list, c->ac.aI, c->ac.jI,
+                                 nullptr);
+    if (rc != NB_OK) return rc;
     NB_CUDA(c, cudaMemsetAsync(c->ac_novf, 0, sizeof(int32_t), c->stream));
     ac_start_kernel<<<(unsigned)((N + 127) / 128), 128, 0, c->stream>>>(N, c->Ns, c->cap, t_start, eta_s, dt_max, c->ac, c->soa,
                                                                         c->aos, c->dtj, c->ac_novf);
@@ -1511,6 +1541,7 @@ int nb_get_info(nb_ctx *c, int32_t key, int64_t *value) {
         case NB_INFO_SPEC_MISSES: *value = c->spec_misses; break;
         case NB_TUNE_REORDER_MIN: *value = c->reorder_min; break;
         case NB_TUNE_SELECT_CHUNKS: *value = c->sel_chunks ? 1 : 0; break;
+        case NB_TUNE_IRR_PRED_MIN: *value = c->irr_pred_min; break;
         case NB_INFO_LOCAL_WARPS:
         case NB_INFO_TOTAL_WARPS: {
             if (!c->stats) return NB_ESTATE;
@@ -1580,6 +1611,9 @@ int nb_set_tuning(nb_ctx *c, int32_t key, int64_t value) {
         case NB_TUNE_SELECT_CHUNKS:
             if (value != 0 && value != 1) return NB_EINVAL;
             c->sel_chunks = value != 0; break;
+        case NB_TUNE_IRR_PRED_MIN:
+            if (value < 0) return NB_EINVAL;
+            c->irr_pred_min = value; break;
         case NB_TUNE_STATS:
             if (value != 0 && value != 1) return NB_EINVAL;
             if (value) {

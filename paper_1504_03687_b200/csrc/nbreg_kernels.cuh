@@ -1167,10 +1167,40 @@ __device__ __forceinline__ BodyD predict_body(const double *__restrict__ aos, in
     return b;
 }
 
+// Large blocks (NB_TUNE_IRR_PRED_MIN): every body is predicted ONCE to the block time into a 64 B record
+// {m, x[3], v[3], pad} -- the values predict_body returns, bit for bit -- and the neighbour loop gathers those
+// records instead of predicting each listed neighbour again from its 128 B state line: half the gathered bytes
+// and no Taylor polynomial per pair.  Pays once the block's lists hold more lines than the one pass over all N
+// moves (~10^4 bodies at 150 neighbours).
+constexpr int P64_D = 8;
+__global__ void __launch_bounds__(256) predict64_kernel(int64_t N, double t, const double *__restrict__ aos,
+                                                        double *__restrict__ p64) {
+    const int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= N) return;
+    const BodyD b = predict_body(aos, (int32_t)j, t);
+    double2 *o = reinterpret_cast<double2 *>(p64 + j * P64_D);
+    o[0] = make_double2(b.m, b.x[0]); o[1] = make_double2(b.x[1], b.x[2]);
+    o[2] = make_double2(b.v[0], b.v[1]); o[3] = make_double2(b.v[2], 0.0);
+}
+// The predicted body j at time t: from its record (PRED) or from its state line.
+template <bool PRED>
+__device__ __forceinline__ BodyD body_at(const double *__restrict__ src, int32_t j, double t) {
+    if constexpr (PRED) {
+        const double2 *p = reinterpret_cast<const double2 *>(src + (int64_t)j * P64_D);
+        const double2 q0 = p[0], q1 = p[1], q2 = p[2], q3 = p[3];
+        BodyD b;
+        b.m = q0.x; b.x[0] = q0.y; b.x[1] = q1.x; b.x[2] = q1.y; b.v[0] = q2.x; b.v[1] = q2.y; b.v[2] = q3.x;
+        return b;
+    } else {
+        return predict_body(src, j, t);
+    }
+}
+
 // ACCUM: add to acc / jerk / pot instead of overwriting them (nb_block_step: regular + irregular = total).
+// PRED: `aos` is the array of predicted records (predict64_kernel) instead of the state lines.
 // idx_i = NULL: the identity block.  rows_by_body / out_by_body: the list rows (and nnb) / the outputs are
 // indexed by BODY (the persistent lists and scratch of the two-level AC stepping) instead of by k.
-template <bool ACCUM>
+template <bool ACCUM, bool PRED = false>
 __global__ void __launch_bounds__(256) irregular_kernel(int32_t n_i, int32_t cap, double t,
                                                         const double *__restrict__ blk_dev,
                                                         int32_t rows_by_body, int32_t out_by_body,
@@ -1185,7 +1215,7 @@ __global__ void __launch_bounds__(256) irregular_kernel(int32_t n_i, int32_t cap
     if (!spec_block(blk_dev, n_i, t)) return;
     if (k >= n_i) return;
     const int32_t i = idx_i ? idx_i[k] : k;
-    const BodyD I = predict_body(aos, i, t);
+    const BodyD I = body_at<PRED>(aos, i, t);
     const int64_t kr = rows_by_body ? i : k, ko = out_by_body ? i : k;
     const int cnt = min(nnb[kr], cap);
     const int32_t *row = nblist + kr * cap;
@@ -1195,7 +1225,7 @@ __global__ void __launch_bounds__(256) irregular_kernel(int32_t n_i, int32_t cap
     for (int e = lane; e < cnt; e += 32) {
         const int32_t j = row[e];
         if (j == i) continue;                                    // a list never holds its owner; be safe
-        const BodyD J = predict_body(aos, j, t);
+        const BodyD J = body_at<PRED>(aos, j, t);
         const double dx = J.x[0] - I.x[0], dy = J.x[1] - I.x[1], dz = J.x[2] - I.x[2];
         const double dvx = J.v[0] - I.v[0], dvy = J.v[1] - I.v[1], dvz = J.v[2] - I.v[2];
         const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));

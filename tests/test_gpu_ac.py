@@ -177,7 +177,9 @@ def test_ac_run_conserves_energy_and_overflow_is_reported(oracle):
 def test_batched_loops_equal_block_by_block_stepping():
     """nb_ac_run / nb_run_blocks enqueue batches of blocks without the host in between (speculative chains, device
     stall flag, adaptive batch size).  Whatever the batching, the kernels and their order are the same: the state
-    after K blocks must be BIT-identical to K single calls, with and without speculation."""
+    after K blocks must be BIT-identical to K single calls, with and without speculation, and with the neighbour
+    force of the host-driven blocks (start-up, regular steps, large blocks) gathering predicted 64 B records
+    (NB_TUNE_IRR_PRED_MIN = 1) instead of predicting every listed neighbour from its state line."""
     import paper_1504_03687_b200 as nb
     N, cap = 3000, 96
     cfg = nbgen.make_config(1, N=N)
@@ -185,10 +187,12 @@ def test_batched_loops_equal_block_by_block_stepping():
     h2 = _radii(x, 12)
     eta_I, eta_R, eta_s, dt_max = 0.01, 0.02, 0.01, 2.0**-4
     runs = {}
-    for mode in ("steps", "run", "run_nospec"):
+    for mode in ("steps", "run", "run_nospec", "run_pred"):
         ctx = _open(m, x, v, cap)
         if mode == "run_nospec":
             ctx.tune("speculate", 0)
+        if mode == "run_pred":               # every host-driven neighbour-force launch gathers predicted records
+            ctx.tune("irr_pred_min", 1)
         ctx.ac_init(0.0, _dev(h2), eta_s, dt_max)
         K, ni, nr = 260, 0, 0
         if mode == "steps":
@@ -207,7 +211,7 @@ def test_batched_loops_equal_block_by_block_stepping():
     print("batched loops: irregular steps", ni, "regular steps", nr, "speculation hits / misses: steps", (hits, misses),
           "run", runs["run"][4:], "run without speculation", runs["run_nospec"][4:])
     assert runs["run_nospec"][4] == 0
-    for mode in ("run", "run_nospec"):
+    for mode in ("run", "run_nospec", "run_pred"):
         g, t2, ni2, nr2 = runs[mode][:4]
         assert (t2, ni2, nr2) == (t, ni, nr)
         for key in ("x0", "v0", "a0", "j0", "t0", "dt", "aI", "jI", "aR", "jR", "tR", "dtR", "nnb"):

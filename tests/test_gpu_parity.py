@@ -696,6 +696,15 @@ def test_irregular_force_matches_oracle_and_completes_the_total(oracle):
     for key, tol in (("acc", 1e-5), ("jerk", 1e-4), ("pot", 1e-6)):
         g = (reg[key] + out[key]).cpu().numpy().reshape(n, -1); r = tot[key].reshape(n, -1)
         assert np.max(np.linalg.norm(g - r, axis=1) / np.linalg.norm(r, axis=1)) < tol, key
+    # large blocks predict every body once into 64 B records and gather those (NB_TUNE_IRR_PRED_MIN): the same bits
+    base = {k: v.clone() for k, v in out.items()}
+    ctx.tune("irr_pred_min", 1)
+    for v in out.values():
+        v.zero_()
+    ctx.irregular(cfg["t"], _dev(idx, torch.int32), reg["nnb"], reg["nblist"], **out)
+    ctx.synchronize()
+    assert all(torch.equal(out[k], base[k]) for k in out)
+    ctx.tune("irr_pred_min", 24576)
     # pot = NULL is allowed; an empty list gives exact zeros
     z = torch.zeros(n, dtype=torch.int32, device="cuda")
     ctx.irregular(cfg["t"], _dev(idx, torch.int32), z, reg["nblist"], out["acc"], out["jerk"], None)
