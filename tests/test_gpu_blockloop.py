@@ -423,3 +423,46 @@ def test_selection_from_chunk_minima_equals_the_full_scan():
     assert log1 == log0
     assert 0 < log1[26][1] <= upd.size and log1[26][0] < log1[25][0]   # the replaced bodies (earlier t0) were found
     assert all(np.array_equal(s1[k], s0[k]) for k in s1)
+
+
+def test_hot_path_calls_between_blocks_do_not_disturb_the_loop(oracle):
+    """The block loop and the hot path share a context (predicted records, the deferred predictor, selection minima,
+    speculative descriptors).  nb_predict_all + nb_regular on arbitrary blocks -- small (fused predictor), large
+    (records, Morton reordering) -- and nb_get_predicted between block steps must leave the integration untouched:
+    the state after the mixed sequence equals the state after the block steps alone, bit for bit, and the
+    interleaved nb_regular results still match the oracle at the time they were asked for."""
+    import paper_1504_03687_b200 as nb
+    from tests import parity
+    cfg = nbgen.make_config(3, N=20000, n_i=16)
+    N, cap = cfg["N"], cfg["cap"]
+    dt = 2.0 ** -cfg["levels"].astype(np.float64)
+    t0 = np.floor(0.3 / dt) * dt
+    eta, dt_max = 0.02, 2.0**-6
+
+    def run(mixed):
+        ctx = nb.nb_open(N, cap)
+        nb.nb_set_j(ctx, *(_dev(a) for a in (cfg["m"], cfg["x0"], cfg["v0"], cfg["a0"], cfg["j0"], t0)))
+        ctx.set_steps(_dev(dt))
+        log = []
+        for b in range(30):
+            log.append(ctx.block_step(None, eta, dt_max))
+            if mixed and b % 3 == 1:
+                n_i = (7, 100, 5000)[(b // 3) % 3]
+                idx, h2 = nbgen.active_block(cfg, n_i)
+                t_q = log[-1][0] + 2.0**-20
+                ctx.predict_all(t_q)
+                got = parity.to_numpy(ctx.regular_alloc(_dev(idx, torch.int32), _dev(h2)))
+                ctx.synchronize()
+                s = _state(ctx, with_steps=False)
+                xp, vp = oracle.predict(s["x0"], s["v0"], s["a0"], s["j0"], s["t0"], t_q)
+                ref = parity.oracle_reference(oracle, s["m"], xp, vp, idx, h2, cap)
+                parity.compare(got, ref, cap)
+        log.append(ctx.run_blocks(None, eta, dt_max, t_stop=1.0e9, max_blocks=20))
+        out = _state(ctx)
+        ctx.close()
+        return log, out
+
+    log0, s0 = run(False)
+    log1, s1 = run(True)
+    assert log0 == log1
+    assert all(np.array_equal(s0[k], s1[k]) for k in s0)
