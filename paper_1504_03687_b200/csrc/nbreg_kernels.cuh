@@ -1154,9 +1154,9 @@ __global__ void __launch_bounds__(32 * W) finalize_kernel(int32_t n_i, int32_t n
 // lanes stride over the list row (one 128 B line of the AoS copy per neighbour: gather-bound); the
 // seven sums are reduced with a fixed xor-shuffle tree.
 struct BodyD { double m, x[3], v[3]; };
-__device__ __forceinline__ BodyD predict_body(const double *__restrict__ aos, int32_t j, double t) {
-    const double2 *p = reinterpret_cast<const double2 *>(aos + (int64_t)j * AOS_D);
-    const double2 q0 = p[0], q1 = p[1], q2 = p[2], q3 = p[3], q4 = p[4], q5 = p[5], q6 = p[6];
+// The body of a 128 B state line (seven 16 B pieces q0..q6) predicted to time t.
+__device__ __forceinline__ BodyD predict_line(double2 q0, double2 q1, double2 q2, double2 q3, double2 q4, double2 q5, double2 q6,
+                                              double t) {
     const double x[3] = {q0.y, q1.x, q1.y}, v[3] = {q2.x, q2.y, q3.x}, a[3] = {q3.y, q4.x, q4.y};
     const double jk[3] = {q5.x, q5.y, q6.x};
     const double dt = t - q6.y, c2 = taylor_c2(dt), c3 = taylor_c3(dt);
@@ -1165,6 +1165,10 @@ __device__ __forceinline__ BodyD predict_body(const double *__restrict__ aos, in
 #pragma unroll
     for (int c = 0; c < 3; ++c) predict_component(x[c], v[c], a[c], jk[c], dt, c2, c3, b.x[c], b.v[c]);
     return b;
+}
+__device__ __forceinline__ BodyD predict_body(const double *__restrict__ aos, int32_t j, double t) {
+    const double2 *p = reinterpret_cast<const double2 *>(aos + (int64_t)j * AOS_D);
+    return predict_line(p[0], p[1], p[2], p[3], p[4], p[5], p[6], t);
 }
 
 // Large blocks (NB_TUNE_IRR_PRED_MIN): every body is predicted ONCE to the block time into a 64 B record
@@ -1222,10 +1226,36 @@ __global__ void __launch_bounds__(256) irregular_kernel(int32_t n_i, int32_t cap
     double s[7];
 #pragma unroll
     for (int q = 0; q < 7; ++q) s[q] = 0.0;
-    for (int e = lane; e < cnt; e += 32) {
-        const int32_t j = row[e];
-        if (j == i) continue;                                    // a list never holds its owner; be safe
-        const BodyD J = body_at<PRED>(aos, j, t);
+    // State lines: the 32 neighbours of a batch are fetched COOPERATIVELY -- eight lanes read the 16 B pieces of one
+    // 128 B line (one tag look-up in L1 per neighbour instead of seven: the scattered 16 B loads of a lane-per-line
+    // gather kept the L1 tag stage 94 % busy), the lines go through a warp-private slice of shared memory, and every
+    // lane then takes ITS neighbour (entry e0 + lane, as a lane-strided loop would: same terms, same order of the
+    // sums).  Predicted records (64 B, four pieces) gain nothing from it (measured) and keep the direct gather.
+    constexpr int PIECES = 8, STRIDE = PIECES + 1;               // (stride 144 B: the LDS.128 of a quarter-warp hit distinct banks)
+    __shared__ double2 sbuf[PRED ? 1 : 8][PRED ? 1 : 32 * STRIDE];
+    double2 *wb = sbuf[PRED ? 0 : threadIdx.x >> 5];
+    const double2 *src2 = reinterpret_cast<const double2 *>(aos);
+    for (int e0 = 0; e0 < cnt; e0 += 32) {
+        const int32_t j = e0 + lane < cnt ? row[e0 + lane] : -1;
+        BodyD J;
+        if constexpr (PRED) {
+            if (j < 0 || j == i) continue;                       // (past the end; a list never holds its owner: be safe)
+            J = body_at<true>(aos, j, t);
+        } else {
+#pragma unroll
+            for (int r = 0; r < PIECES; ++r) {
+                const int slot = r * (32 / PIECES) + lane / PIECES, piece = lane % PIECES;
+                const int32_t js = __shfl_sync(0xffffffffu, j, slot);
+                if (js >= 0 && piece < 7) wb[slot * STRIDE + piece] = src2[(int64_t)js * (AOS_D / 2) + piece];
+            }
+            __syncwarp();
+            if (j >= 0 && j != i) {
+                const double2 *q = wb + lane * STRIDE;
+                J = predict_line(q[0], q[1], q[2], q[3], q[4], q[5], q[6], t);
+            }
+            __syncwarp();
+            if (j < 0 || j == i) continue;
+        }
         const double dx = J.x[0] - I.x[0], dy = J.x[1] - I.x[1], dz = J.x[2] - I.x[2];
         const double dvx = J.v[0] - I.v[0], dvy = J.v[1] - I.v[1], dvz = J.v[2] - I.v[2];
         const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
