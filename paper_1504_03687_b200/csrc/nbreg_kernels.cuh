@@ -1230,24 +1230,28 @@ __global__ void __launch_bounds__(256) irregular_kernel(int32_t n_i, int32_t cap
     // 128 B line (one tag look-up in L1 per neighbour instead of seven: the scattered 16 B loads of a lane-per-line
     // gather kept the L1 tag stage 94 % busy), the lines go through a warp-private slice of shared memory, and every
     // lane then takes ITS neighbour (entry e0 + lane, as a lane-strided loop would: same terms, same order of the
-    // sums).  Predicted records (64 B, four pieces) gain nothing from it (measured) and keep the direct gather.
+    // sums).  Predicted records (64 B, four pieces) gain nothing from it (measured) and keep the direct gather; so do
+    // tiny blocks (<= COOP_MIN bodies: latency matters there, not throughput, and the direct gather is a shorter chain).
     constexpr int PIECES = 8, STRIDE = PIECES + 1;               // (stride 144 B: the LDS.128 of a quarter-warp hit distinct banks)
+    constexpr int COOP_MIN = 64;
     __shared__ double2 sbuf[PRED ? 1 : 8][PRED ? 1 : 32 * STRIDE];
     double2 *wb = sbuf[PRED ? 0 : threadIdx.x >> 5];
     const double2 *src2 = reinterpret_cast<const double2 *>(aos);
     for (int e0 = 0; e0 < cnt; e0 += 32) {
         const int32_t j = e0 + lane < cnt ? row[e0 + lane] : -1;
         BodyD J;
-        if constexpr (PRED) {
+        if (PRED || n_i <= COOP_MIN) {                           // (uniform over the grid)
             if (j < 0 || j == i) continue;                       // (past the end; a list never holds its owner: be safe)
-            J = body_at<true>(aos, j, t);
+            J = body_at<PRED>(aos, j, t);
         } else {
+            double2 pc[PIECES];
 #pragma unroll
-            for (int r = 0; r < PIECES; ++r) {
-                const int slot = r * (32 / PIECES) + lane / PIECES, piece = lane % PIECES;
-                const int32_t js = __shfl_sync(0xffffffffu, j, slot);
-                if (js >= 0 && piece < 7) wb[slot * STRIDE + piece] = src2[(int64_t)js * (AOS_D / 2) + piece];
+            for (int r = 0; r < PIECES; ++r) {                   // straight-line: the eight loads are in flight together
+                const int32_t js = __shfl_sync(0xffffffffu, j, r * (32 / PIECES) + lane / PIECES);
+                pc[r] = src2[(int64_t)(js >= 0 ? js : i) * (AOS_D / 2) + (lane % PIECES)];     // (past the end: any valid line)
             }
+#pragma unroll
+            for (int r = 0; r < PIECES; ++r) wb[(r * (32 / PIECES) + lane / PIECES) * STRIDE + lane % PIECES] = pc[r];
             __syncwarp();
             if (j >= 0 && j != i) {
                 const double2 *q = wb + lane * STRIDE;
