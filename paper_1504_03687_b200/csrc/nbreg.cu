@@ -1229,7 +1229,7 @@ int run_blocks(nb_ctx *c, BlockRun &R) {
         // single level: the size class of the last block (32 / 64 / 128: the variants with a fused predictor)
         int32_t spec_cap = 0;
         if (c->spec_enabled) {
-            if (R.two) spec_cap = AC_SPEC_CAP;
+            if (R.two) spec_cap = (int32_t)std::min<int64_t>(AC_SPEC_CAP, c->N);
             else if (c->fuse && c->blk_prev_n > 0 && c->blk_prev_n <= 128)
                 spec_cap = c->blk_prev_n <= 32 ? 32 : c->blk_prev_n <= 64 ? 64 : 128;
         }

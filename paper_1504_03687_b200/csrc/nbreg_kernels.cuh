@@ -1216,9 +1216,12 @@ __global__ void __launch_bounds__(256) irregular_kernel(int32_t n_i, int32_t cap
     const int lane = threadIdx.x & 31;
     const int k = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     pdl_wait();
+    // (a speculative launch: the index is requested together with the descriptor; n_i is still the launch's capacity
+    // here, which the host keeps <= N, the size of the list buffer)
+    const int32_t i_spec = (blk_dev && idx_i && k < n_i) ? idx_i[k] : 0;
     if (!spec_block(blk_dev, n_i, t)) return;
     if (k >= n_i) return;
-    const int32_t i = idx_i ? idx_i[k] : k;
+    const int32_t i = blk_dev && idx_i ? i_spec : idx_i ? idx_i[k] : k;
     const BodyD I = body_at<PRED>(aos, i, t);
     const int64_t kr = rows_by_body ? i : k, ko = out_by_body ? i : k;
     const int cnt = min(nnb[kr], cap);
@@ -1436,17 +1439,20 @@ __global__ void __launch_bounds__(256) select_min_chunks_kernel(int64_t N, const
                                                                 unsigned long long *key_next, const int32_t *stall,
                                                                 double *__restrict__ ring) {
     pdl_wait();
-    if (*stall) {
+    const int b = blockIdx.x;
+    // (the three words the decision rests on are requested together: one trip to L2, not three in a row)
+    const int32_t stalled = *stall, is_dirty = dirty[b];
+    const unsigned long long old_min = cmin[b];
+    if (stalled) {
         if (blockIdx.x == 0 && threadIdx.x == 0) {
             *key_next = ~0ull;
             *reinterpret_cast<volatile double *>(ring + 3) = (double)BLK_SKIPPED;
         }
         return;
     }
-    const int b = blockIdx.x;
-    if (!dirty[b]) {                                  // (uniform over the CTA)
+    if (!is_dirty) {                                  // (uniform over the CTA)
         if (threadIdx.x == 0) {
-            atomicMin(key, cmin[b]);
+            atomicMin(key, old_min);
             if (b == 0) *key_next = ~0ull;
         }
         return;
@@ -1482,15 +1488,17 @@ __global__ void __launch_bounds__(256) select_scatter_kernel(int64_t N, const do
                                                              int32_t *stall, double *__restrict__ ring,
                                                              const unsigned long long *__restrict__ cmin) {
     pdl_wait();
-    if (*stall) return;
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     const int b = blockIdx.x, nchunk = gridDim.x;
+    // (requested together: one trip to L2)
+    const int32_t stalled = *stall;
+    const unsigned long long kmin = *key, my_min = cmin ? cmin[b] : 0ull;
+    if (stalled) return;
     constexpr int PER = SEL_CHUNK / 256;
     __shared__ int32_t wsum[8], wsum2[8];
     __shared__ int32_t base_s, base2_s;
-    const unsigned long long kmin = *key;
     const double tn = key_to_double(kmin);
-    const bool here = !cmin || cmin[b] == kmin;     // only a chunk whose own minimum is t_next holds due bodies
+    const bool here = !cmin || my_min == kmin;      // only a chunk whose own minimum is t_next holds due bodies
     // ---- this chunk's active bodies (kept as flags) and their number
     bool act[PER], due[PER];
     int32_t cntc = 0, cnt2 = 0;
@@ -1718,9 +1726,10 @@ __global__ void __launch_bounds__(128) ac_correct_kernel(int32_t n, int64_t Ns, 
                                                          double *__restrict__ dtj, int32_t *__restrict__ sel_dirty) {
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
     pdl_wait();
+    const int32_t i_spec = (blk_dev && k < n) ? idx[k] : 0;    // (requested together with the descriptor; n: the launch's capacity <= N)
     if (!spec_block(blk_dev, n, t)) return;
     if (k >= n) return;
-    const int64_t i = idx[k];
+    const int64_t i = blk_dev ? i_spec : idx[k];
     const double2 *p = reinterpret_cast<const double2 *>(aos + i * AOS_D);
     const double2 q0 = p[0], q1 = p[1], q2 = p[2], q3 = p[3], q4 = p[4], q5 = p[5], q6 = p[6];
     const double m = q0.x;
