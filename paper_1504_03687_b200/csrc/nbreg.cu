@@ -1041,7 +1041,7 @@ int blk_setup(nb_ctx *c) {
     const int nchunk = (int)((N + SEL_CHUNK - 1) / SEL_CHUNK);
     NB_CUDA(c, cudaMalloc(&c->blk_key, 2 * sizeof(unsigned long long)));
     NB_CUDA(c, cudaMemsetAsync(c->blk_key, 0xff, 2 * sizeof(unsigned long long), c->stream));
-    NB_CUDA(c, cudaMalloc(&c->blk_idx, sizeof(int32_t) * N));
+    NB_CUDA(c, cudaMalloc(&c->blk_idx, sizeof(int32_t) * std::max<int64_t>(N, 1024)));   // (speculative launches read up to their capacity)
     NB_CUDA(c, cudaMalloc(&c->ac_reg_idx, sizeof(int32_t) * N));
     NB_CUDA(c, cudaMalloc(&c->blk_pub, sizeof(unsigned long long) * nchunk));
     NB_CUDA(c, cudaMemsetAsync(c->blk_pub, 0, sizeof(unsigned long long) * nchunk, c->stream));

@@ -1620,9 +1620,10 @@ __global__ void __launch_bounds__(128) correct_kernel(int32_t n, int64_t Ns, dou
                                                       int32_t *__restrict__ sel_dirty) {
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
     pdl_wait();
+    const int32_t i_spec = (blk_dev && k < n) ? idx[k] : 0;    // (requested together with the descriptor; n: the launch's capacity)
     if (!spec_block(blk_dev, n, t1)) return;
     if (k >= n) return;
-    const int64_t i = idx[k];
+    const int64_t i = blk_dev ? i_spec : idx[k];
     const double2 *p = reinterpret_cast<const double2 *>(aos + i * AOS_D);
     const double2 q0 = p[0], q1 = p[1], q2 = p[2], q3 = p[3], q4 = p[4], q5 = p[5], q6 = p[6];
     const double m = q0.x;
