@@ -340,7 +340,7 @@ enum {
                                         blocks and rescan only the chunks the last corrector touched (the search for
                                         the due particles must not cost O(N) per block); 0 = scan all N every block.  The
                                         selected blocks do not depend on it                                            */
-    NB_TUNE_IRR_PRED_MIN = 35,       /* set: the neighbour force of a block of at least this many bodies (default 65536; 0 =
+    NB_TUNE_IRR_PRED_MIN = 35,       /* set: the neighbour force of a block of at least this many bodies (default 49152; 0 =
                                         never) predicts every body once into 64 B records and gathers those instead of
                                         predicting each listed neighbour from its 128 B state line.  Same bits either way   */
     NB_INFO_FORCE_KERNEL_NS_AT = 1000 /* get, key = 1000 + q (q < 256): device time in ns of the q-th bracketed

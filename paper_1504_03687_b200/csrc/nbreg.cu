@@ -107,7 +107,7 @@ struct nb_ctx {
     bool sel_all_dirty = true;                                         // the state or the steps were replaced: rescan everything
     bool sel_chunks = true;                                            // NB_TUNE_SELECT_CHUNKS
     double *p64 = nullptr;                                             // [N][8] FP64 predicted records of a large block's neighbour force
-    int64_t irr_pred_min = 65536;                                      // NB_TUNE_IRR_PRED_MIN: blocks of at least this many bodies use them
+    int64_t irr_pred_min = 49152;                                      // NB_TUNE_IRR_PRED_MIN: blocks of at least this many bodies use them
     int32_t *blk_stall = nullptr;                                      // set by the first block of a batch that needs the host
     bool blk_stall_dirty = true;                                       // the flag must be cleared before the next batch
     int blk_batch = 1;                                                 // blocks enqueued per host round trip (adaptive)

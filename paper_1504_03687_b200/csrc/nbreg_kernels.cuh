@@ -1186,14 +1186,20 @@ __global__ void __launch_bounds__(256) predict64_kernel(int64_t N, double t, con
     o[0] = make_double2(b.m, b.x[0]); o[1] = make_double2(b.x[1], b.x[2]);
     o[2] = make_double2(b.v[0], b.v[1]); o[3] = make_double2(b.v[2], 0.0);
 }
+// One 256-bit load (sm_100: LDG.E.256): 32 B-aligned, read-only data.  A scattered gather is bound by the tag look-ups
+// of L1, one per lane and instruction: half as many instructions per record, half as many look-ups.
+__device__ __forceinline__ void ld256(const double *p, double &a, double &b, double &c, double &d) {
+    asm volatile("ld.global.nc.v4.f64 {%0, %1, %2, %3}, [%4];" : "=d"(a), "=d"(b), "=d"(c), "=d"(d) : "l"(p));
+}
 // The predicted body j at time t: from its record (PRED) or from its state line.
 template <bool PRED>
 __device__ __forceinline__ BodyD body_at(const double *__restrict__ src, int32_t j, double t) {
     if constexpr (PRED) {
-        const double2 *p = reinterpret_cast<const double2 *>(src + (int64_t)j * P64_D);
-        const double2 q0 = p[0], q1 = p[1], q2 = p[2], q3 = p[3];
+        const double *p = src + (int64_t)j * P64_D;
         BodyD b;
-        b.m = q0.x; b.x[0] = q0.y; b.x[1] = q1.x; b.x[2] = q1.y; b.v[0] = q2.x; b.v[1] = q2.y; b.v[2] = q3.x;
+        double pad;
+        ld256(p, b.m, b.x[0], b.x[1], b.x[2]);
+        ld256(p + 4, b.v[0], b.v[1], b.v[2], pad);
         return b;
     } else {
         return predict_body(src, j, t);
@@ -1233,7 +1239,8 @@ __global__ void __launch_bounds__(256) irregular_kernel(int32_t n_i, int32_t cap
     // 128 B line (one tag look-up in L1 per neighbour instead of seven: the scattered 16 B loads of a lane-per-line
     // gather kept the L1 tag stage 94 % busy), the lines go through a warp-private slice of shared memory, and every
     // lane then takes ITS neighbour (entry e0 + lane, as a lane-strided loop would: same terms, same order of the
-    // sums).  Predicted records (64 B, four pieces) gain nothing from it (measured) and keep the direct gather; so do
+    // sums).  Predicted records (64 B: two 256-bit loads per lane) gain nothing from it (measured; nor do 256-bit loads
+    // help the cooperative fetch) and keep the direct gather; so do
     // tiny blocks (<= COOP_MIN bodies: latency matters there, not throughput, and the direct gather is a shorter chain).
     constexpr int PIECES = 8, STRIDE = PIECES + 1;               // (stride 144 B: the LDS.128 of a quarter-warp hit distinct banks)
     constexpr int COOP_MIN = 64;

@@ -704,7 +704,7 @@ def test_irregular_force_matches_oracle_and_completes_the_total(oracle):
     ctx.irregular(cfg["t"], _dev(idx, torch.int32), reg["nnb"], reg["nblist"], **out)
     ctx.synchronize()
     assert all(torch.equal(out[k], base[k]) for k in out)
-    ctx.tune("irr_pred_min", 65536)
+    ctx.tune("irr_pred_min", 49152)
     # pot = NULL is allowed; an empty list gives exact zeros
     z = torch.zeros(n, dtype=torch.int32, device="cuda")
     ctx.irregular(cfg["t"], _dev(idx, torch.int32), z, reg["nblist"], out["acc"], out["jerk"], None)
