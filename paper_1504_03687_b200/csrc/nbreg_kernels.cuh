@@ -1166,9 +1166,17 @@ __device__ __forceinline__ BodyD predict_line(double2 q0, double2 q1, double2 q2
     for (int c = 0; c < 3; ++c) predict_component(x[c], v[c], a[c], jk[c], dt, c2, c3, b.x[c], b.v[c]);
     return b;
 }
+// One 256-bit load (sm_100: LDG.E.256): 32 B-aligned, read-only data.  A scattered gather is bound by the tag look-ups
+// of L1, one per lane and instruction: half as many instructions per record, half as many look-ups.
+__device__ __forceinline__ void ld256(const double *p, double &a, double &b, double &c, double &d) {
+    asm volatile("ld.global.nc.v4.f64 {%0, %1, %2, %3}, [%4];" : "=d"(a), "=d"(b), "=d"(c), "=d"(d) : "l"(p));
+}
 __device__ __forceinline__ BodyD predict_body(const double *__restrict__ aos, int32_t j, double t) {
-    const double2 *p = reinterpret_cast<const double2 *>(aos + (int64_t)j * AOS_D);
-    return predict_line(p[0], p[1], p[2], p[3], p[4], p[5], p[6], t);
+    const double *p = aos + (int64_t)j * AOS_D;
+    double2 q0, q1, q2, q3, q4, q5, q6, q7;
+    ld256(p, q0.x, q0.y, q1.x, q1.y); ld256(p + 4, q2.x, q2.y, q3.x, q3.y);
+    ld256(p + 8, q4.x, q4.y, q5.x, q5.y); ld256(p + 12, q6.x, q6.y, q7.x, q7.y);
+    return predict_line(q0, q1, q2, q3, q4, q5, q6, t);
 }
 
 // Large blocks (NB_TUNE_IRR_PRED_MIN): every body is predicted ONCE to the block time into a 64 B record
@@ -1185,11 +1193,6 @@ __global__ void __launch_bounds__(256) predict64_kernel(int64_t N, double t, con
     double2 *o = reinterpret_cast<double2 *>(p64 + j * P64_D);
     o[0] = make_double2(b.m, b.x[0]); o[1] = make_double2(b.x[1], b.x[2]);
     o[2] = make_double2(b.v[0], b.v[1]); o[3] = make_double2(b.v[2], 0.0);
-}
-// One 256-bit load (sm_100: LDG.E.256): 32 B-aligned, read-only data.  A scattered gather is bound by the tag look-ups
-// of L1, one per lane and instruction: half as many instructions per record, half as many look-ups.
-__device__ __forceinline__ void ld256(const double *p, double &a, double &b, double &c, double &d) {
-    asm volatile("ld.global.nc.v4.f64 {%0, %1, %2, %3}, [%4];" : "=d"(a), "=d"(b), "=d"(c), "=d"(d) : "l"(p));
 }
 // The predicted body j at time t: from its record (PRED) or from its state line.
 template <bool PRED>
