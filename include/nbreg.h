@@ -56,7 +56,8 @@ enum {
                       current CUDA device is not the one the context was opened on                 */
     NB_ENOMEM = 3, /* device (or staging) allocation failed                                        */
     NB_ECUDA = 4,  /* CUDA error (sticky); nb_last_cuda_error() returns the cudaError_t            */
-    NB_EOVERFLOW = 5 /* two-level AC stepping only: a neighbour list overflowed nb_cap (not sticky)  */
+    NB_EOVERFLOW = 5, /* two-level AC stepping only: a neighbour list overflowed nb_cap (not sticky) */
+    NB_ELIMIT = 6  /* nb_next_block_static only: N is larger than NB_STATIC_MAX_N                    */
 };
 
 /* Create a context for N j-particles and a neighbour-list capacity of nb_cap entries per active
@@ -292,6 +293,37 @@ int nb_set_j_offset(nb_ctx *ctx, int64_t j_offset);
 int nb_regular_shard(nb_ctx *ctx, double t, int32_t n_i, const int32_t *idx_i, const double *istate,
                      const double *h2_i, double *acc, double *jerk, double *pot, int32_t *nnb,
                      int32_t *nblist, int32_t *overflow);
+
+/* ---- Block selection for callers that must not allocate (P:47 block time steps; section 3.3.1: the search
+ * for the particles due next).  Same result as nb_set_steps + nb_next_block, without a context.
+ *
+ * Use it where a cudaMalloc is not an option: inside an application whose own memory pool has already claimed the
+ * device (a stray allocation fails or eats into its budget), inside a hook that runs beside other streams and must
+ * not trigger the device-wide synchronisation that cudaMalloc / cudaFree imply, or after an out-of-memory condition.
+ * nb_open allocates the j-state, so none of the context calls qualify; this one makes no allocation of its own, host or
+ * device: it calls neither cudaMalloc / cudaFree nor any routine that allocates.
+ *
+ * Inputs, DEVICE: t0[N], dt[N] (time of the last step and current step of every body).  Outputs, DEVICE, caller-owned:
+ * idx_act with room for N int32 -- the bodies with t0 + dt == min_j (t0_j + dt_j), ascending, in its first n entries,
+ * the rest untouched --, block[2] = {t_next, (double) n}.  Enqueued on cuda_stream (NULL = the legacy default stream)
+ * on the CURRENT device; returns without synchronising, outputs valid once that stream has been synchronised.
+ * Three kernels and one 8-byte memset.
+ *
+ * Working memory: a fixed 33,024-byte array inside the library image (the running minimum and one count per 2048
+ * bodies).  Every GPU that loads libnbreg holds it from load until the process exits.  Hence the LIMIT:
+ * N <= NB_STATIC_MAX_N = 16,777,216; a larger N returns NB_ELIMIT before anything is launched or written.
+ * The array is shared by all calls of the process on that device and keeps the last call's contents; the call resets
+ * the part that must start clean (the minimum) on the stream, in order, before its kernels.  Two calls whose GPU
+ * work can OVERLAP -- different streams without an event between them, or two host threads on different streams --
+ * race on it and return garbage; calls on one stream, or ordered by events, are safe.
+ * The FIRST call on each device looks up the array's device address (and the SM count) and keeps it; that look-up may
+ * initialise the device's CUDA context and load the library's kernels, so make one call per device during start-up,
+ * before any stream capture begins.  Later calls only enqueue.
+ * Errors: NB_EINVAL (NULL pointer, N <= 0), NB_ELIMIT, NB_ECUDA (the look-up or a launch failed -- e.g. the current
+ * device is not sm_100; not sticky, there is no context to stick to). */
+#define NB_STATIC_MAX_N 16777216
+int nb_next_block_static(int64_t N, const double *t0, const double *dt, int32_t *idx_act, double *block,
+                         void *cuda_stream);
 
 /* Tuning / introspection.  Keys: */
 enum {

@@ -21,6 +21,8 @@ from .binding import (  # noqa: F401
     nb_plan_chunks,
     nb_update_j,
     nb_irregular,
+    nb_next_block_static,
+    NB_ELIMIT, NB_STATIC_MAX_N,
     NB_OK, NB_EINVAL, NB_ESTATE, NB_ENOMEM, NB_ECUDA, NB_EOVERFLOW,
 )
 from .build import build_lib  # noqa: F401

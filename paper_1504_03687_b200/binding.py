@@ -7,7 +7,8 @@ from pathlib import Path
 
 from .build import LIB, build_lib
 
-NB_OK, NB_EINVAL, NB_ESTATE, NB_ENOMEM, NB_ECUDA, NB_EOVERFLOW = 0, 1, 2, 3, 4, 5
+NB_OK, NB_EINVAL, NB_ESTATE, NB_ENOMEM, NB_ECUDA, NB_EOVERFLOW, NB_ELIMIT = 0, 1, 2, 3, 4, 5, 6
+NB_STATIC_MAX_N = 16777216      # include/nbreg.h
 INFO = dict(kernel_launches=0, last_jsplit=1, last_iblock=2, last_grid=3, sm_count=4, n_padded=5,
             force_jsplit=16, force_variant=17, last_variant=18, profile=19, force_kernel_ns=20,
             force_kernel_count=21, step_chunks=22, fuse_predict=23, local_g_milli=24, stats=25,
@@ -59,6 +60,7 @@ def load_library(build: bool = True) -> ctypes.CDLL:
     lib.nb_set_steps.argtypes = [_vp, _vp]
     lib.nb_init_steps.argtypes = [_vp, dbl, dbl]
     lib.nb_next_block.argtypes = [_vp, ctypes.POINTER(dbl), ctypes.POINTER(i32), _vp]
+    lib.nb_next_block_static.argtypes = [i64, _vp, _vp, _vp, _vp, _vp]
     lib.nb_correct.argtypes = [_vp, dbl, i32, _vp, _vp, _vp, dbl, dbl]
     lib.nb_get_state.argtypes = [_vp] + [_vp] * 7
     lib.nb_block_step.argtypes = [_vp, _vp, dbl, dbl, dbl, ctypes.POINTER(dbl), ctypes.POINTER(i32)]
@@ -427,6 +429,23 @@ def nb_plan_chunks(N: int, chunks: int = 0) -> list[int]:
     n = ctypes.c_int32()
     _check(lib.nb_plan_chunks(N, chunks, fb, ctypes.byref(n)), "nb_plan_chunks")
     return [fb[q] for q in range(n.value + 1)]
+
+
+def nb_next_block_static(t0, dt, idx_act, block, stream=None):
+    """nb_next_block_static: the next block's time and members from t0 and dt alone, for callers that cannot
+    allocate GPU memory where they run (a plug-in under an application whose pool owns the device, a hook that must
+    not stall other streams with cudaMalloc's device-wide synchronisation).  No context: t0, dt (float64 CUDA
+    tensors [N]), idx_act (int32 CUDA tensor [N]) and block (float64 CUDA tensor [2] <- {t_next, n}) are the
+    caller's; the working memory is a fixed array inside the library, so N <= NB_STATIC_MAX_N (NbregError with
+    NB_ELIMIT beyond).  Enqueues on `stream` (a torch stream; None = the legacy default stream) and returns without
+    synchronising.  Calls whose GPU work overlaps share that array and race: keep them on one stream."""
+    import torch
+    N = int(t0.numel())
+    handle = _vp() if stream is None else _vp(stream.cuda_stream)
+    rc = load_library().nb_next_block_static(N, _dev_ptr(t0, torch.float64, N, "t0"), _dev_ptr(dt, torch.float64, N, "dt"),
+                                             _dev_ptr(idx_act, torch.int32, N, "idx_act"),
+                                             _dev_ptr(block, torch.float64, 2, "block"), handle)
+    _check(rc, "nb_next_block_static")
 
 
 # Function-style aliases with the C names (north_star: nb_open / nb_set_j / nb_predict_all / nb_regular)

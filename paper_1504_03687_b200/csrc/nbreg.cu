@@ -9,6 +9,7 @@
 #include <cmath>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <unordered_map>
 
@@ -1677,8 +1678,84 @@ const char *nb_strerror(int code) {
         case NB_ENOMEM: return "out of device memory";
         case NB_ECUDA: return "CUDA error or no sm_100 device (see nb_last_cuda_error)";
         case NB_EOVERFLOW: return "neighbour list overflow during two-level AC stepping (shrink the radii)";
+        case NB_ELIMIT: return "N exceeds NB_STATIC_MAX_N, the fixed capacity of nb_next_block_static's built-in scratch";
         default: return "unknown nbreg status";
     }
 }
 
 }  // extern "C"
+
+// ------------------------------------------------------------------ nb_next_block_static: block selection without a context
+// Who this is for: code that must pick the next block of due particles but is not allowed to allocate GPU memory at
+// the point where it runs -- a plug-in living inside a host application whose memory pool already owns the whole
+// device (the application hands out buffers, and a stray cudaMalloc either fails or steals from its budget), a
+// real-time / in-situ analysis hook where the implicit device synchronisation of cudaMalloc and cudaFree would stall
+// the simulation's other streams, or a caller running after an out-of-memory condition that still wants to know
+// which bodies are due.  Such a caller cannot use nb_open (which allocates the j-state) and so cannot reach
+// nb_next_block.  Here the caller brings t0, dt and the output buffers; the only working memory -- the running
+// minimum and one count per 2048-body chunk -- sits in the fixed array below, which is part of the library image:
+// every device that loads libnbreg reserves these 33 KB from load to exit, whether or not this call is ever made.
+namespace {
+
+constexpr int64_t SEL_STATIC_CHUNKS = NB_STATIC_MAX_N / SEL_CHUNK;                 // 8192 counts
+constexpr size_t SEL_STATIC_COUNTS_OFF = 256;                                      // [0, 8): the minimum's key
+constexpr size_t SEL_STATIC_BYTES = SEL_STATIC_COUNTS_OFF + sizeof(int32_t) * SEL_STATIC_CHUNKS;
+static_assert(NB_STATIC_MAX_N % SEL_CHUNK == 0, "the limit is a whole number of selection chunks");
+
+// In HOST code this name is only the host-side shadow of the symbol: it is never passed to a kernel or to
+// cudaMemsetAsync.  static_scratch() asks the runtime for the array's address on the current device.
+static __device__ __align__(256) unsigned char g_sel_static[SEL_STATIC_BYTES];
+
+struct StaticScratch {
+    unsigned char *base = nullptr;      // device address of g_sel_static on this device
+    int sm_count = 0;
+};
+constexpr int STATIC_MAX_DEVICES = 64;
+StaticScratch g_static_dev[STATIC_MAX_DEVICES];        // filled once per device, under g_static_mu
+std::mutex g_static_mu;
+
+// Set-up, once per device, with that device current (it is: the caller's pointers live on it).  Neither call
+// allocates; cudaGetSymbolAddress may initialise the device's context and load the module if nothing of the library
+// ran on it yet -- which is why the first call on a device belongs before any stream capture.
+cudaError_t static_scratch(StaticScratch *out) {
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    const bool cached = dev >= 0 && dev < STATIC_MAX_DEVICES;
+    std::lock_guard<std::mutex> hold(g_static_mu);
+    StaticScratch s = cached ? g_static_dev[dev] : StaticScratch{};
+    if (!s.base) {
+        void *p = nullptr;
+        e = cudaGetSymbolAddress(&p, g_sel_static);
+        if (e == cudaSuccess) e = cudaDeviceGetAttribute(&s.sm_count, cudaDevAttrMultiProcessorCount, dev);
+        if (e == cudaSuccess && (!p || s.sm_count <= 0)) e = cudaErrorInvalidSymbol;
+        if (e == cudaSuccess) {
+            s.base = static_cast<unsigned char *>(p);
+            if (cached) g_static_dev[dev] = s;
+        }
+    }
+    if (e == cudaSuccess) *out = s;
+    return e;
+}
+
+}  // namespace
+
+extern "C" int nb_next_block_static(int64_t N, const double *t0, const double *dt, int32_t *idx_act,
+                                    double *block, void *cuda_stream) {
+    if (!t0 || !dt || !idx_act || !block || N <= 0) return NB_EINVAL;
+    if (N > NB_STATIC_MAX_N) return NB_ELIMIT;           // before any CUDA call: nothing was touched
+    StaticScratch s;
+    if (static_scratch(&s) != cudaSuccess) return NB_ECUDA;
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    unsigned long long *key = reinterpret_cast<unsigned long long *>(s.base);
+    int32_t *counts = reinterpret_cast<int32_t *>(s.base + SEL_STATIC_COUNTS_OFF);
+    // The array keeps what the previous call left: the key must start at "no time yet" (all ones) or the minimum
+    // of an earlier call would win.  The counts need no clearing -- pass 0 writes every chunk pass 1 reads.
+    if (cudaMemsetAsync(key, 0xff, sizeof(unsigned long long), stream) != cudaSuccess) return NB_ECUDA;
+    const unsigned nchunk = (unsigned)((N + SEL_CHUNK - 1) / SEL_CHUNK);
+    const unsigned g = (unsigned)std::min<int64_t>((N + 255) / 256, (int64_t)s.sm_count * 8);
+    next_time_kernel<<<g, 256, 0, stream>>>(N, t0, dt, key);
+    select_active_kernel<0><<<nchunk, 256, 0, stream>>>(N, t0, dt, key, counts, idx_act, block);
+    select_active_kernel<1><<<nchunk, 256, 0, stream>>>(N, t0, dt, key, counts, idx_act, block);
+    return cudaGetLastError() == cudaSuccess ? NB_OK : NB_ECUDA;
+}
