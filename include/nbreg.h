@@ -215,10 +215,12 @@ int nb_correct(nb_ctx *ctx, double t, int32_t n, const int32_t *idx, const doubl
  * after the selection are enqueued without a further synchronisation.  Requires nb_set_j and steps. */
 int nb_block_step(nb_ctx *ctx, const double *h2_all, double eta, double dt_max, double t_stop,
                   double *t_next, int32_t *n_act);
-/* Copy the last block's results into the caller's DEVICE buffers (any may be NULL; n = the *n_act the step
- * returned): idx_act[n], acc[n][3], jerk[n][3], pot[n] -- the TOTAL force handed to the corrector --, nnb[n],
- * nblist[n][nb_cap] (NB_ESTATE if the step ran without h2_all), overflow[n].  Enqueued on the stream. */
-int nb_get_block(nb_ctx *ctx, int32_t *idx_act, double *acc, double *jerk, double *pot, int32_t *nnb,
+/* Copy the last block's results into the caller's DEVICE buffers (any may be NULL), each with room for n_cap rows:
+ * idx_act[n], acc[n][3], jerk[n][3], pot[n] -- the TOTAL force handed to the corrector --, nnb[n],
+ * nblist[n][nb_cap] (NB_ESTATE if the step ran without h2_all), overflow[n], where n = min(n_cap, size of the last
+ * block).  That size is the *n_act nb_block_step returned; after nb_run_blocks ask NB_INFO_LAST_BLOCK_N.  NB_ESTATE if
+ * the last block loop was nb_ac_step / nb_ac_run (their results: nb_ac_get).  Enqueued on the stream. */
+int nb_get_block(nb_ctx *ctx, int32_t n_cap, int32_t *idx_act, double *acc, double *jerk, double *pot, int32_t *nnb,
                  int32_t *nblist, int32_t *overflow);
 
 /* ---- Two-level Ahmad-Cohen stepping ("the full force of one particle is separated
@@ -236,6 +238,8 @@ int nb_get_block(nb_ctx *ctx, int32_t *idx_act, double *acc, double *jerk, doubl
  * irregular force, dtR), dtI = dtR for a body without neighbours.  *n_overflow (HOST, may be NULL) = number of
  * lists longer than nb_cap; if any, returns NB_EOVERFLOW and AC stepping stays unavailable (shrink the radii:
  * radius control is the caller's, reading R38).  Allocates 6 N vectors + N x nb_cap list entries.
+ * NB_ESTATE if some t0[j] != t_start (checked on the device): this is a START-UP call, not a way to re-list a
+ * cluster in mid-run -- for that see nb_ac_set_radii.
  * Any call that replaces or advances the state outside the two-level scheme (nb_set_j, nb_set_j_host,
  * nb_step_host, nb_update_j, nb_set_steps, nb_init_steps, nb_correct, nb_block_step, nb_run_blocks) ends it:
  * nb_ac_step then returns NB_ESTATE until the next nb_ac_init. */
@@ -262,6 +266,20 @@ int nb_ac_run(nb_ctx *ctx, double eta_I, double eta_R, double dt_max, double t_s
               double *t_next, int64_t *blocks, int64_t *irregular_steps, int64_t *regular_steps);
 int nb_run_blocks(nb_ctx *ctx, const double *h2_all, double eta, double dt_max, double t_stop,
                   int64_t max_blocks, double *t_next, int64_t *blocks, int64_t *particle_steps);
+
+/* Radius control in mid-run (the paper's codes adapt the neighbour radius at regular steps; here the policy is the
+ * caller's, the library only stores the radii, reading R38).  nb_ac_set_radii replaces the stored SQUARED radius of the
+ * bodies idx[0..n) (DEVICE; indices outside [0, N) are ignored) by h2[0..n) (DEVICE), or of all bodies if idx == NULL
+ * and n == N.  A new radius takes effect at that body's NEXT regular step, where the list is rebuilt anyway (the
+ * regular force w.r.t. the old list is total - irregular(old list), so old and new radius need not agree).  Enqueued on
+ * the stream.  NB_ESTATE without a live two-level state.
+ * Recovery from NB_EOVERFLOW: nb_ac_step / nb_ac_run left the state untouched and the same block is due again.
+ * nb_ac_get_failed tells which regular steps it attempted: *n_rows (HOST) = their number (0 if the last step did not
+ * overflow), idx[0..min(n_cap, *n_rows)) (DEVICE, may be NULL) = the bodies, ascending, nnb[...] (DEVICE, may be NULL)
+ * = the TRUE number of neighbours each new list would have held (those > nb_cap overflowed).  Shrink those radii
+ * -- e.g. h2 *= (target / nnb)^(2/3) --, nb_ac_set_radii, and call nb_ac_step again: the block is redone with them. */
+int nb_ac_set_radii(nb_ctx *ctx, int32_t n, const int32_t *idx, const double *h2);
+int nb_ac_get_failed(nb_ctx *ctx, int32_t n_cap, int32_t *n_rows, int32_t *idx, int32_t *nnb);
 
 /* Inspection: copies of the AC state into the caller's DEVICE buffers (any may be NULL): the last block's
  * idx_act[N] / idx_reg[N] (first n_irr / n_reg entries valid), aI, jI, aR, jR [N][3], tR, dtR [N], nnb[N],
@@ -375,6 +393,8 @@ enum {
     NB_TUNE_IRR_PRED_MIN = 35,       /* set: the neighbour force of a block of at least this many bodies (default 49152; 0 =
                                         never) predicts every body once into 64 B records and gathers those instead of
                                         predicting each listed neighbour from its 128 B state line.  Same bits either way   */
+    NB_INFO_LAST_BLOCK_N = 36,       /* get: bodies in the last block integrated by nb_block_step / nb_run_blocks (0: none,
+                                        or the last loop was the two-level one)                                         */
     NB_INFO_FORCE_KERNEL_NS_AT = 1000 /* get, key = 1000 + q (q < 256): device time in ns of the q-th bracketed
                                         force-kernel launch since NB_TUNE_PROFILE was set (synchronises)    */
 };

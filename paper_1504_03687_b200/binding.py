@@ -12,7 +12,7 @@ NB_STATIC_MAX_N = 16777216      # include/nbreg.h
 INFO = dict(kernel_launches=0, last_jsplit=1, last_iblock=2, last_grid=3, sm_count=4, n_padded=5,
             force_jsplit=16, force_variant=17, last_variant=18, profile=19, force_kernel_ns=20,
             force_kernel_count=21, step_chunks=22, fuse_predict=23, local_g_milli=24, stats=25,
-            local_warps=26, total_warps=27, last_fused=28, reorder_min=29, last_reordered=30, speculate=31, spec_hits=32, spec_misses=33, select_chunks=34, irr_pred_min=35,
+            local_warps=26, total_warps=27, last_fused=28, reorder_min=29, last_reordered=30, speculate=31, spec_hits=32, spec_misses=33, select_chunks=34, irr_pred_min=35, last_block_n=36,
             force_kernel_ns_at=1000)
 
 _lib = None
@@ -64,10 +64,12 @@ def load_library(build: bool = True) -> ctypes.CDLL:
     lib.nb_correct.argtypes = [_vp, dbl, i32, _vp, _vp, _vp, dbl, dbl]
     lib.nb_get_state.argtypes = [_vp] + [_vp] * 7
     lib.nb_block_step.argtypes = [_vp, _vp, dbl, dbl, dbl, ctypes.POINTER(dbl), ctypes.POINTER(i32)]
-    lib.nb_get_block.argtypes = [_vp] + [_vp] * 7
+    lib.nb_get_block.argtypes = [_vp, i32] + [_vp] * 7
     lib.nb_ac_init.argtypes = [_vp, dbl, _vp, dbl, dbl, ctypes.POINTER(i32)]
     lib.nb_ac_step.argtypes = [_vp, dbl, dbl, dbl, dbl, ctypes.POINTER(dbl), ctypes.POINTER(i32), ctypes.POINTER(i32)]
     lib.nb_ac_get.argtypes = [_vp] + [_vp] * 10
+    lib.nb_ac_set_radii.argtypes = [_vp, i32, _vp, _vp]
+    lib.nb_ac_get_failed.argtypes = [_vp, i32, ctypes.POINTER(i32), _vp, _vp]
     lib.nb_ac_run.argtypes = [_vp, dbl, dbl, dbl, dbl, i64, ctypes.POINTER(dbl)] + [ctypes.POINTER(i64)] * 3
     lib.nb_run_blocks.argtypes = [_vp, _vp, dbl, dbl, dbl, i64, ctypes.POINTER(dbl)] + [ctypes.POINTER(i64)] * 2
     lib.nb_set_j_offset.argtypes = [_vp, i64]
@@ -278,7 +280,7 @@ class NbContext:
             out["nblist"] = torch.empty((n, self.cap), dtype=i4, device=dev)
         if n:
             ptr = lambda k: _vp(out[k].data_ptr()) if k in out else _vp()
-            _check(self._lib.nb_get_block(self._ctx, *(ptr(k) for k in ("idx_act", "acc", "jerk", "pot", "nnb", "nblist",
+            _check(self._lib.nb_get_block(self._ctx, int(n), *(ptr(k) for k in ("idx_act", "acc", "jerk", "pot", "nnb", "nblist",
                                                                           "overflow"))), "nb_get_block", self._ctx)
         return out
 
@@ -319,6 +321,26 @@ class NbContext:
         _check(self._lib.nb_run_blocks(self._ctx, h2, float(eta), float(dt_max), t_stop, int(max_blocks), ctypes.byref(t),
                                        ctypes.byref(nb_), ctypes.byref(ns)), "nb_run_blocks", self._ctx)
         return t.value, nb_.value, ns.value
+
+    def ac_set_radii(self, idx, h2):
+        """nb_ac_set_radii: new squared radii h2 for the bodies idx (int32 CUDA tensor), or for all N if idx is None."""
+        import torch
+        n = self.N if idx is None else int(idx.numel())
+        _check(self._lib.nb_ac_set_radii(self._ctx, n, _vp() if idx is None else _dev_ptr(idx, torch.int32, n, "idx"),
+                                         _dev_ptr(h2, torch.float64, n, "h2")), "nb_ac_set_radii", self._ctx)
+
+    def ac_get_failed(self):
+        """nb_ac_get_failed -> (idx, nnb): the regular steps of the block that returned NB_EOVERFLOW and the true size
+        of each new list (empty tensors if the last step did not overflow)."""
+        import torch
+        n = ctypes.c_int32()
+        _check(self._lib.nb_ac_get_failed(self._ctx, 0, ctypes.byref(n), _vp(), _vp()), "nb_ac_get_failed", self._ctx)
+        idx = torch.empty(n.value, dtype=torch.int32, device="cuda")
+        nnb = torch.empty(n.value, dtype=torch.int32, device="cuda")
+        if n.value:
+            _check(self._lib.nb_ac_get_failed(self._ctx, n.value, ctypes.byref(n), _vp(idx.data_ptr()), _vp(nnb.data_ptr())),
+                   "nb_ac_get_failed", self._ctx)
+        return idx, nnb
 
     def ac_get(self, with_lists: bool = False) -> dict:
         import torch

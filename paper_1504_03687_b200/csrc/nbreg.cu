@@ -89,6 +89,8 @@ struct nb_ctx {
     int32_t *blk_nnb = nullptr, *blk_ovf = nullptr, *blk_list = nullptr;
     int64_t blk_n = 0, blk_list_n = 0, blk_last_n = 0;
     bool blk_had_list = false;
+    int32_t ac_fail_nr = 0;                         // regular rows of the two-level block that returned NB_EOVERFLOW (0: none)
+    bool blk_last_two = false;                      // the last block loop was the two-level one (nb_get_block: NB_ESTATE)
     int32_t h2_by_body = 0;                         // the h2 array of the launch in flight is indexed by body
     const double *spec_dev = nullptr;               // non-NULL while a SPECULATIVE chain is enqueued: the kernels take the
                                                     // block's {t, n, status} from this device address
@@ -465,6 +467,9 @@ int regular_device(nb_ctx *c, int32_t n_i, const int32_t *idx_i, const double *h
     // Small blocks (one i-block: every j-tile has exactly one reader) whose prediction is still pending
     // read the FP64 state and predict inside the force kernel; everything else needs the records.
     const bool fused = c->pred_pending && c->fuse && vi >= FUSED_FIRST && n_ib == 1;
+    // A speculative chain knows its block time only on the device: only the fused kernel reads it from there.  The
+    // records route would predict all N bodies to the host's placeholder time (run_blocks never asks for this).
+    if (c->spec_dev && !fused) return NB_ESTATE;
     int rc = fused ? NB_OK : materialize_pred(c);
     if (rc != NB_OK) return rc;
     const Variant &v = fused ? c->fvar[vi] : c->var[vi];
@@ -1225,14 +1230,21 @@ int run_blocks(nb_ctx *c, BlockRun &R) {
     rc = ensure_aos(c);
     if (rc != NB_OK) return rc;
     c->blk_last_n = 0;
+    c->blk_last_two = R.two;
     while (R.blocks < R.max_blocks) {
         // speculative capacity of this batch: two-level: any block without a regular step up to AC_SPEC_CAP bodies;
         // single level: the size class of the last block (32 / 64 / 128: the variants with a fused predictor)
         int32_t spec_cap = 0;
         if (c->spec_enabled) {
             if (R.two) spec_cap = (int32_t)std::min<int64_t>(AC_SPEC_CAP, c->N);
-            else if (c->fuse && c->blk_prev_n > 0 && c->blk_prev_n <= 128)
+            else if (c->fuse && c->blk_prev_n > 0 && c->blk_prev_n <= 128) {
                 spec_cap = c->blk_prev_n <= 32 ? 32 : c->blk_prev_n <= 64 ? 64 : 128;
+                // only if a block of that capacity takes the fused kernel (regular_device: one i-block of a variant that
+                // has a fused form) -- NB_TUNE_FORCE_VARIANT can say otherwise, and then the block time must come
+                // from the host: no speculation
+                const int vi = pick_variant(c, spec_cap);
+                if (vi < FUSED_FIRST || spec_cap > c->var[vi].iblock) spec_cap = 0;
+            }
         }
         // batch size: 1 after a stall, doubled after every batch that ran without the host (a stalled batch wastes the
         // launches behind the stall)
@@ -1280,7 +1292,10 @@ int run_blocks(nb_ctx *c, BlockRun &R) {
                 if (spec_cap > 0) c->spec_misses += 1;
                 if (R.two) {
                     if (nr == 0) rc = ac_enqueue_irregular_chain(c, R.eta, R.eta_R, R.dt_max, n, t, false);
-                    else rc = ac_finish_block(c, R.eta, R.eta_R, R.dt_max, t, n, nr, &R.n_overflow);
+                    else {
+                        rc = ac_finish_block(c, R.eta, R.eta_R, R.dt_max, t, n, nr, &R.n_overflow);
+                        c->ac_fail_nr = rc == NB_EOVERFLOW ? nr : 0;       // rows and true counts stay in ac_reg_idx / blk_nnb
+                    }
                 } else {
                     rc = blk_buffers(c, n, R.h2_all != nullptr, false);
                     if (rc == NB_OK) rc = sl_enqueue_chain(c, R.h2_all, R.eta, R.dt_max, n, t, 0);
@@ -1351,10 +1366,21 @@ int nb_ac_init(nb_ctx *c, double t_start, const double *h2_all, double eta_s, do
         NB_CUDA(c, cudaMallocHost(&c->h_ac_novf, sizeof(int32_t)));
         if (!c->dtj) NB_CUDA(c, cudaMalloc(&c->dtj, sizeof(double) * N));
     }
+    // every t0[j] must equal t_start (the start-up relabels x0, v0 as the state AT t_start): checked, because a call in
+    // mid-run -- the tempting way out of an NB_EOVERFLOW -- would silently move every body that is not there
+    NB_CUDA(c, cudaMemsetAsync(c->ac_novf, 0, sizeof(int32_t), c->stream));
+    count_not_at_kernel<<<(unsigned)std::min<int64_t>((N + 255) / 256, (int64_t)c->sm_count * 8), 256, 0, c->stream>>>(
+        N, c->soa + 13 * c->Ns, t_start, c->ac_novf);
+    NB_CUDA(c, cudaGetLastError());
+    c->launches += 1;
+    NB_CUDA(c, cudaMemcpyAsync(c->h_ac_novf, c->ac_novf, sizeof(int32_t), cudaMemcpyDeviceToHost, c->stream));
+    NB_CUDA(c, cudaStreamSynchronize(c->stream));
+    if (*c->h_ac_novf != 0) return NB_ESTATE;
     rc = blk_setup(c);
     if (rc != NB_OK) return rc;
+    c->ac_fail_nr = 0;
     NB_CUDA(c, cudaMemcpyAsync(c->ac_h2, h2_all, sizeof(double) * N, cudaMemcpyDeviceToDevice, c->stream));
-    // forces at t_start: every t0[j] must equal t_start, so the prediction is the state itself
+    // forces at t_start: every t0[j] equals t_start, so the prediction is the state itself
     c->have_pred = true; c->pred_pending = true; c->pred_t = t_start;
     rc = ensure_aos(c);
     if (rc != NB_OK) return rc;
@@ -1427,11 +1453,41 @@ int nb_ac_get(nb_ctx *c, int32_t *idx_act, int32_t *idx_reg, double *aI, double 
     return NB_OK;
 }
 
-int nb_get_block(nb_ctx *c, int32_t *idx_act, double *acc, double *jerk, double *pot, int32_t *nnb, int32_t *nblist,
-                 int32_t *overflow) {
+int nb_ac_set_radii(nb_ctx *c, int32_t n, const int32_t *idx, const double *h2) {
     int rc = check_live(c);
     if (rc != NB_OK) return rc;
-    const int64_t n = c->blk_last_n;
+    if (n < 0 || !h2 || (!idx && n != c->N)) return NB_EINVAL;
+    if (!c->have_ac) return NB_ESTATE;
+    if (n == 0) return NB_OK;
+    if (!idx) {
+        NB_CUDA(c, cudaMemcpyAsync(c->ac_h2, h2, sizeof(double) * c->N, cudaMemcpyDeviceToDevice, c->stream));
+    } else {
+        scatter_radii_kernel<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(n, c->N, idx, h2, c->ac_h2);
+        NB_CUDA(c, cudaGetLastError());
+        c->launches += 1;
+    }
+    return NB_OK;
+}
+
+int nb_ac_get_failed(nb_ctx *c, int32_t n_cap, int32_t *n_rows, int32_t *idx, int32_t *nnb) {
+    int rc = check_live(c);
+    if (rc != NB_OK) return rc;
+    if (!n_rows || n_cap < 0) return NB_EINVAL;
+    if (!c->have_ac) return NB_ESTATE;
+    *n_rows = c->ac_fail_nr;
+    const int64_t n = std::min<int64_t>(n_cap, c->ac_fail_nr);
+    if (n > 0 && idx) NB_CUDA(c, cudaMemcpyAsync(idx, c->ac_reg_idx, sizeof(int32_t) * n, cudaMemcpyDeviceToDevice, c->stream));
+    if (n > 0 && nnb) NB_CUDA(c, cudaMemcpyAsync(nnb, c->blk_nnb, sizeof(int32_t) * n, cudaMemcpyDeviceToDevice, c->stream));
+    return NB_OK;
+}
+
+int nb_get_block(nb_ctx *c, int32_t n_cap, int32_t *idx_act, double *acc, double *jerk, double *pot, int32_t *nnb,
+                 int32_t *nblist, int32_t *overflow) {
+    int rc = check_live(c);
+    if (rc != NB_OK) return rc;
+    if (n_cap < 0) return NB_EINVAL;
+    if (c->blk_last_two) return NB_ESTATE;      // the last block was a two-level one: its results are nb_ac_get's
+    const int64_t n = std::min<int64_t>(n_cap, c->blk_last_n);      // never more rows than the caller has room for
     if (n == 0) return NB_OK;
     const cudaMemcpyKind dd = cudaMemcpyDeviceToDevice;
     if (idx_act) NB_CUDA(c, cudaMemcpyAsync(idx_act, c->blk_idx, sizeof(int32_t) * n, dd, c->stream));
@@ -1530,6 +1586,7 @@ int nb_get_info(nb_ctx *c, int32_t key, int64_t *value) {
         case NB_INFO_LAST_VARIANT: *value = c->last_variant; break;
         case NB_TUNE_FORCE_JSPLIT: *value = c->force_S; break;
         case NB_TUNE_FORCE_VARIANT: *value = c->force_variant; break;
+        case NB_INFO_LAST_BLOCK_N: *value = c->blk_last_two ? 0 : c->blk_last_n; break;
         case NB_TUNE_PROFILE: *value = c->profile ? 1 : 0; break;
         case NB_TUNE_STEP_CHUNKS: *value = c->step_chunks; break;
         case NB_TUNE_FUSE_PREDICT: *value = c->fuse ? 1 : 0; break;

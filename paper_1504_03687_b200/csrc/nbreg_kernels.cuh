@@ -1830,6 +1830,25 @@ __global__ void __launch_bounds__(256) count_overflow_kernel(int32_t n, const in
     if ((threadIdx.x & 31) == 0 && c) atomicAdd(out, c);
 }
 
+// nb_ac_init's precondition (every body at t_start): number of bodies whose t0 differs
+__global__ void __launch_bounds__(256) count_not_at_kernel(int64_t N, const double *__restrict__ t0, double t_start,
+                                                           int32_t *__restrict__ out) {
+    int32_t c = 0;
+    for (int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; j < N; j += (int64_t)gridDim.x * blockDim.x)
+        c += t0[j] != t_start ? 1 : 0;
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) c += __shfl_xor_sync(0xffffffffu, c, off);
+    if ((threadIdx.x & 31) == 0 && c) atomicAdd(out, c);
+}
+// nb_ac_set_radii: h2_all[idx[k]] = h2[k]; an index outside [0, N) is ignored
+__global__ void __launch_bounds__(256) scatter_radii_kernel(int32_t n, int64_t N, const int32_t *__restrict__ idx,
+                                                            const double *__restrict__ h2, double *__restrict__ h2_all) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= n) return;
+    const int64_t j = idx[k];
+    if (j >= 0 && j < N) h2_all[j] = h2[k];
+}
+
 // Inspection: the FP64 state back in the caller's layout (tests, energy checks, checkpoints).
 __global__ void __launch_bounds__(256) export_state_kernel(int64_t N, int64_t Ns, const double *__restrict__ soa,
                                                            const double *__restrict__ dtj, double *__restrict__ m,

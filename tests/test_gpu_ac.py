@@ -279,10 +279,73 @@ def test_ac_overflow_in_mid_run_is_reported_at_the_same_block_as_the_oracle(orac
                 ctx.ac_step(eta_I, eta_R, dt_max)                               # the same block, the same error
             assert e2.value.code == nb.NB_EOVERFLOW
             print("overflow reported at block", b, "cap", cap)
+            # ---- recovery (round-2 advisor finding: there was none).  Re-initialising in mid-run is refused ...
+            with pytest.raises(nb.NbregError) as e3:
+                ctx.ac_init(0.0, _dev(h2), eta_s, dt_max)
+            assert e3.value.code == nb.NB_ESTATE
+            still = _gpu_state(ctx)
+            for key in ("x0", "v0", "a0", "j0", "t0", "dt", "aI", "aR", "tR", "dtR", "nnb"):
+                assert np.array_equal(before[key], still[key]), key
+            # ... the library names the regular steps it attempted and the true size of each new list ...
+            f_idx, f_nnb = (a.cpu().numpy() for a in ctx.ac_get_failed())
+            t_blk = (before["t0"] + before["dt"]).min()
+            due = np.flatnonzero((before["t0"] + before["dt"] == t_blk) & (before["tR"] + before["dtR"] == t_blk))
+            assert np.array_equal(f_idx, due)
+            xp, vp = oracle.predict(st["x0"], st["v0"], st["a0"], st["j0"], st["t0"], t_blk)
+            true_nnb = oracle.regular(m, xp, vp, due, h2[due], N)["nnb"]
+            assert np.array_equal(f_nnb, true_nnb) and (f_nnb > cap).any()
+            # ... the caller shrinks those radii and the SAME block goes through, in step with the oracle given the same radii
+            bad = f_nnb > cap
+            h2 = h2.copy()
+            h2[f_idx[bad]] *= (0.6 * cap / f_nnb[bad]) ** (2.0 / 3.0)
+            ctx.ac_set_radii(_dev(f_idx[bad].astype(np.int32)), _dev(h2[f_idx[bad]]))
+            for b2 in range(30):
+                try:
+                    t_ref, act, reg = AC.block_step(oracle, m, st, h2, cap, eta_I, eta_R, dt_max)
+                    orc_raised = False
+                except OverflowError:
+                    orc_raised = True
+                try:
+                    t, n, nr = ctx.ac_step(eta_I, eta_R, dt_max)
+                    gpu_raised = False
+                except nb.NbregError as e4:
+                    assert e4.code == nb.NB_EOVERFLOW
+                    gpu_raised = True
+                assert orc_raised == gpu_raised, (b2, orc_raised, gpu_raised)
+                if gpu_raised:
+                    assert b2 > 0                       # the redone block itself must pass; a later one may overflow again
+                    break
+                assert t == t_ref and n == act.size and nr == reg.size, (b2, t, t_ref, n, act.size, nr, reg.size)
+                if b2 == 0:
+                    assert t == t_blk and np.array_equal(reg, due)
+                    assert ctx.ac_get_failed()[0].numel() == 0
+                g = _gpu_state(ctx)
+                dI, dR = np.flatnonzero(g["dt"] != st["dtI"]), np.flatnonzero(g["dtR"] != st["dtR"])
+                st["dtI"][dI] = g["dt"][dI]; st["dtR"][dR] = g["dtR"][dR]
+            g = _gpu_state(ctx)
+            assert np.array_equal(g["t0"], st["t0"]) and np.array_equal(g["nnb"], st["nnb"])
+            assert np.abs(g["x0"] - st["x0"]).max() < 1e-9 and np.abs(g["v0"] - st["v0"]).max() < 1e-7
+            print("recovered: redone block with", int(bad.sum()), "shrunk radii, then", b2, "more blocks in step with the oracle")
             break
         g = _gpu_state(ctx)
         dI, dR = np.flatnonzero(g["dt"] != st["dtI"]), np.flatnonzero(g["dtR"] != st["dtR"])
         st["dtI"][dI] = g["dt"][dI]; st["dtR"][dR] = g["dtR"][dR]
     else:
         pytest.fail("no overflow within 4000 blocks: the test set-up does not exercise the error path")
+    ctx.close()
+
+
+def test_get_block_after_a_two_level_step_is_refused():
+    """nb_get_block reads the single-level loop's buffers; after nb_ac_step they are stale (results: nb_ac_get)."""
+    import paper_1504_03687_b200 as nb
+    N, cap = 512, 64
+    cfg = nbgen.make_config(1, N=N)
+    m, x, v = cfg["m"], cfg["x0"], cfg["v0"]
+    ctx = _open(m, x, v, cap)
+    assert ctx.ac_init(0.0, _dev(_radii(x, 10)), 0.01, 2.0**-4) == 0
+    t, n, nr = ctx.ac_step(0.01, 0.02, 2.0**-4)
+    assert n > 0 and ctx.info("last_block_n") == 0
+    with pytest.raises(nb.NbregError) as e:
+        ctx.get_block(n)
+    assert e.value.code == nb.NB_ESTATE
     ctx.close()

@@ -466,3 +466,95 @@ def test_hot_path_calls_between_blocks_do_not_disturb_the_loop(oracle):
     log1, s1 = run(True)
     assert log0 == log1
     assert all(np.array_equal(s0[k], s1[k]) for k in s0)
+
+
+@pytest.mark.parametrize("variant", [0, 1, 4])
+def test_block_loops_with_a_forced_kernel_variant_follow_the_oracle(variant):
+    """NB_TUNE_FORCE_VARIANT inside nb_block_step / nb_run_blocks.  Variants 0 and 1 have no fused form and variant 4
+    holds 32 particles per CTA, so a small block's speculative chain (block time known on the device only) would have
+    to take the records route, which predicts to the HOST's time: the loop must not speculate there (round-2 advisor
+    finding: it did, and integrated with forces evaluated at t = 0).  40 blocks in lockstep with the oracle, then the
+    same 40 blocks by nb_run_blocks: bit-identical to the single calls."""
+    import paper_1504_03687_b200 as nb
+    cfg = nbgen.make_config(3, N=12000)
+    N = cfg["N"]
+    dt = 2.0 ** -cfg["levels"].astype(np.float64)
+    st = dict(x0=cfg["x0"].copy(), v0=cfg["v0"].copy(), a0=cfg["a0"].copy(), j0=cfg["j0"].copy(),
+              t0=np.floor(0.3 / dt) * dt, dt=dt.copy())
+    start = {k: v.copy() for k, v in st.items()}
+    m = cfg["m"]
+    eta, dt_max, K = 0.02, 2.0**-6, 40
+
+    def fresh():
+        ctx = nb.nb_open(N, 8)
+        nb.nb_set_j(ctx, *(_dev(a) for a in (m, start["x0"], start["v0"], start["a0"], start["j0"], start["t0"])))
+        ctx.set_steps(_dev(start["dt"]))
+        ctx.tune("force_variant", variant)
+        return ctx
+
+    ctx = fresh()
+    sizes, flips = [], 0
+    for b in range(K):
+        t, n = ctx.block_step(None, eta, dt_max)
+        assert ctx.info("last_variant") == variant
+        t_ref, act, _ = _oracle_block(st, m, eta, dt_max)
+        assert t == t_ref and n == act.size, (b, t, t_ref, n, act.size)
+        assert np.array_equal(ctx.get_block(n)["idx_act"].cpu().numpy(), act), b
+        sizes.append(n)
+        g_dt = _state(ctx)["dt"]
+        diff = np.flatnonzero(g_dt != st["dt"])
+        assert np.isin(diff, act).all()
+        flips += diff.size
+        st["dt"][diff] = g_dt[diff]
+    got = _state(ctx)
+    hits = ctx.info("spec_hits")
+    print("forced variant", variant, "sizes min/median/max", min(sizes), int(np.median(sizes)), max(sizes), "flips", flips,
+          "speculative hits", hits)
+    assert min(sizes) <= 32                                          # blocks that WOULD have been speculated
+    if variant < 2:
+        assert hits == 0 and ctx.info("spec_misses") == 0            # no speculative chain was ever enqueued
+    assert flips <= max(2, int(1e-3 * sum(sizes)))
+    assert np.array_equal(got["t0"], st["t0"])
+    assert np.abs(got["x0"] - st["x0"]).max() < 5e-9 and np.abs(got["v0"] - st["v0"]).max() < 6e-6
+    scale = np.linalg.norm(st["a0"], axis=1)
+    assert np.max(np.linalg.norm(got["a0"] - st["a0"], axis=1) / scale) <= 1e-5
+    ctx.close()
+    ctx = fresh()
+    t2, blocks, steps = ctx.run_blocks(None, eta, dt_max, max_blocks=K)
+    assert blocks == K and steps == sum(sizes)
+    run = _state(ctx)
+    for key in got:
+        assert np.array_equal(run[key], got[key]), key
+    ctx.close()
+
+
+def test_get_block_copies_no_more_than_the_caller_has_room_for():
+    """nb_get_block(n_cap, ...): min(n_cap, size of the last block) rows (round-2 advisor finding: it used to copy the
+    block's size whatever the caller had allocated); NB_INFO_LAST_BLOCK_N tells that size after nb_run_blocks."""
+    import paper_1504_03687_b200 as nb
+    cfg = nbgen.make_config(2, N=20000, n_i=16)
+    dt = 2.0 ** -cfg["levels"].astype(np.float64)
+    ctx = nb.nb_open(cfg["N"], 8)
+    nb.nb_set_j(ctx, *(_dev(cfg[k]) for k in ("m", "x0", "v0", "a0", "j0")), _dev(np.floor(0.3 / dt) * dt))
+    ctx.set_steps(_dev(dt))
+    t, n = ctx.block_step(None, 0.02, 2.0**-6)
+    assert n > 8 and ctx.info("last_block_n") == n
+    full = ctx.get_block(n)
+    half = n // 2
+    guard = torch.full((n, 3), 7.0, dtype=torch.float64, device="cuda")      # room for n, told half
+    idx = torch.full((n,), -7, dtype=torch.int32, device="cuda")
+    from paper_1504_03687_b200.binding import _check, _vp
+    _check(ctx._lib.nb_get_block(ctx._ctx, half, _vp(idx.data_ptr()), _vp(guard.data_ptr()), _vp(), _vp(), _vp(), _vp(), _vp()),
+           "nb_get_block", ctx._ctx)
+    ctx.synchronize()
+    assert torch.equal(idx[:half], full["idx_act"][:half]) and bool((idx[half:] == -7).all())
+    assert torch.equal(guard[:half], full["acc"][:half]) and bool((guard[half:] == 7.0).all())
+    more = ctx.get_block(n + 100)                                            # more room than rows: n rows copied
+    assert torch.equal(more["idx_act"][:n], full["idx_act"])
+    tt, blocks, steps = ctx.run_blocks(None, 0.02, 2.0**-6, max_blocks=3)
+    last = ctx.info("last_block_n")
+    assert blocks == 3 and 0 < last <= steps
+    st = _state(ctx)
+    blk = ctx.get_block(last)["idx_act"].cpu().numpy()
+    assert np.all(st["t0"][blk] == st["t0"].max()) and (st["t0"] == st["t0"].max()).sum() == last
+    ctx.close()
