@@ -395,6 +395,11 @@ enum {
                                         predicting each listed neighbour from its 128 B state line.  Same bits either way   */
     NB_INFO_LAST_BLOCK_N = 36,       /* get: bodies in the last block integrated by nb_block_step / nb_run_blocks (0: none,
                                         or the last loop was the two-level one)                                         */
+    NB_TUNE_SELECT_GRID = 37,        /* set: upper limit on the CTAs of the block loops' scatter kernel (0 = none, default).  The
+                                        library already limits that grid to what the device holds at once, because a CTA waits
+                                        for the counts of the chunks before its own; each CTA then takes several chunks of 2048
+                                        bodies in ascending order.  A smaller limit exercises that route at small N (tests);
+                                        the selected blocks do not depend on it                                           */
     NB_INFO_FORCE_KERNEL_NS_AT = 1000 /* get, key = 1000 + q (q < 256): device time in ns of the q-th bracketed
                                         force-kernel launch since NB_TUNE_PROFILE was set (synchronises)    */
 };

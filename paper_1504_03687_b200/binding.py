@@ -12,7 +12,7 @@ NB_STATIC_MAX_N = 16777216      # include/nbreg.h
 INFO = dict(kernel_launches=0, last_jsplit=1, last_iblock=2, last_grid=3, sm_count=4, n_padded=5,
             force_jsplit=16, force_variant=17, last_variant=18, profile=19, force_kernel_ns=20,
             force_kernel_count=21, step_chunks=22, fuse_predict=23, local_g_milli=24, stats=25,
-            local_warps=26, total_warps=27, last_fused=28, reorder_min=29, last_reordered=30, speculate=31, spec_hits=32, spec_misses=33, select_chunks=34, irr_pred_min=35, last_block_n=36,
+            local_warps=26, total_warps=27, last_fused=28, reorder_min=29, last_reordered=30, speculate=31, spec_hits=32, spec_misses=33, select_chunks=34, irr_pred_min=35, last_block_n=36, select_grid=37,
             force_kernel_ns_at=1000)
 
 _lib = None

@@ -109,6 +109,8 @@ struct nb_ctx {
     int32_t *sel_dirty = nullptr;                                      // [chunks] set by the correctors: rescan this chunk
     bool sel_all_dirty = true;                                         // the state or the steps were replaced: rescan everything
     bool sel_chunks = true;                                            // NB_TUNE_SELECT_CHUNKS
+    int64_t sel_grid_max = 0;          // CTAs of select_scatter_kernel the device holds at once (blk_setup)
+    int64_t sel_grid_cap = 0;          // NB_TUNE_SELECT_GRID: a smaller cap (0 = none)
     double *p64 = nullptr;                                             // [N][8] FP64 predicted records of a large block's neighbour force
     int64_t irr_pred_min = 49152;                                      // NB_TUNE_IRR_PRED_MIN: blocks of at least this many bodies use them
     int32_t *blk_stall = nullptr;                                      // set by the first block of a batch that needs the host
@@ -1061,6 +1063,12 @@ int blk_setup(nb_ctx *c) {
     NB_CUDA(c, cudaMalloc(&c->sel_cmin, sizeof(unsigned long long) * nchunk));
     NB_CUDA(c, cudaMalloc(&c->sel_dirty, sizeof(int32_t) * nchunk));
     c->sel_all_dirty = true;
+    // the scatter kernel's look-back needs every CTA it may wait for to be resident: the grid never exceeds what the
+    // device holds at once (each CTA then walks several chunks, ascending)
+    int occ_two = 0, occ_one = 0;
+    NB_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_two, select_scatter_kernel<true>, 256, 0));
+    NB_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_one, select_scatter_kernel<false>, 256, 0));
+    c->sel_grid_max = (int64_t)std::max(1, std::min(occ_two, occ_one)) * c->sm_count;
     return NB_OK;
 }
 
@@ -1102,6 +1110,8 @@ int blk_enqueue_select(nb_ctx *c, bool two, double t_stop, int32_t spec_cap, int
     const unsigned gmin = (unsigned)std::min<int64_t>((N + 255) / 256, (int64_t)c->sm_count * 8);
     c->blk_epoch += 1;
     const unsigned long long *cmin = c->sel_chunks ? c->sel_cmin : nullptr;
+    const unsigned gscat = (unsigned)std::min<int64_t>(nchunk, c->sel_grid_cap > 0 ? std::min(c->sel_grid_cap, c->sel_grid_max)
+                                                                                     : c->sel_grid_max);
     if (c->sel_chunks) {
         if (c->sel_all_dirty) {       // any non-zero word means "rescan"
             NB_CUDA(c, cudaMemsetAsync(c->sel_dirty, 1, sizeof(int32_t) * nchunk, c->stream));
@@ -1114,13 +1124,13 @@ int blk_enqueue_select(nb_ctx *c, bool two, double t_stop, int32_t spec_cap, int
         NB_CUDA(c, launch_chain(select_min_kernel, dim3(gmin), dim3(256), 0, c->stream, N, t0, c->dtj, key, key_next, c->blk_stall, ring));
     }
     if (two)
-        NB_CUDA(c, launch_chain(select_scatter_kernel<true>, dim3(nchunk), dim3(256), 0, c->stream, N, t0, c->dtj, key, c->blk_pub,
+        NB_CUDA(c, launch_chain(select_scatter_kernel<true>, dim3(gscat), dim3(256), 0, c->stream, N, t0, c->dtj, key, c->blk_pub,
                                 c->blk_epoch, c->blk_idx, c->sel_result, c->ac.tR, c->ac.dtR, c->ac_reg_idx, t_stop, spec_cap,
-                                c->blk_stall, ring, cmin));
+                                c->blk_stall, ring, cmin, (int32_t)nchunk));
     else
-        NB_CUDA(c, launch_chain(select_scatter_kernel<false>, dim3(nchunk), dim3(256), 0, c->stream, N, t0, c->dtj, key, c->blk_pub,
+        NB_CUDA(c, launch_chain(select_scatter_kernel<false>, dim3(gscat), dim3(256), 0, c->stream, N, t0, c->dtj, key, c->blk_pub,
                                 c->blk_epoch, c->blk_idx, c->sel_result, nullptr, nullptr, c->ac_reg_idx, t_stop, spec_cap,
-                                c->blk_stall, ring, cmin));
+                                c->blk_stall, ring, cmin, (int32_t)nchunk));
     NB_CUDA(c, cudaGetLastError());
     c->blk_parity ^= 1;
     c->launches += 2;
@@ -1599,6 +1609,7 @@ int nb_get_info(nb_ctx *c, int32_t key, int64_t *value) {
         case NB_INFO_SPEC_MISSES: *value = c->spec_misses; break;
         case NB_TUNE_REORDER_MIN: *value = c->reorder_min; break;
         case NB_TUNE_SELECT_CHUNKS: *value = c->sel_chunks ? 1 : 0; break;
+        case NB_TUNE_SELECT_GRID: *value = c->sel_grid_cap; break;
         case NB_TUNE_IRR_PRED_MIN: *value = c->irr_pred_min; break;
         case NB_INFO_LOCAL_WARPS:
         case NB_INFO_TOTAL_WARPS: {
@@ -1672,6 +1683,9 @@ int nb_set_tuning(nb_ctx *c, int32_t key, int64_t value) {
         case NB_TUNE_IRR_PRED_MIN:
             if (value < 0) return NB_EINVAL;
             c->irr_pred_min = value; break;
+        case NB_TUNE_SELECT_GRID:
+            if (value < 0) return NB_EINVAL;
+            c->sel_grid_cap = value; break;
         case NB_TUNE_STATS:
             if (value != 0 && value != 1) return NB_EINVAL;
             if (value) {

@@ -1496,18 +1496,28 @@ __global__ void __launch_bounds__(256) select_scatter_kernel(int64_t N, const do
                                                              const double *__restrict__ tR, const double *__restrict__ dtR,
                                                              int32_t *__restrict__ idx_reg, double t_stop, int32_t spec_cap,
                                                              int32_t *stall, double *__restrict__ ring,
-                                                             const unsigned long long *__restrict__ cmin) {
+                                                             const unsigned long long *__restrict__ cmin, int32_t nchunk) {
     pdl_wait();
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    const int b = blockIdx.x, nchunk = gridDim.x;
     // (requested together: one trip to L2)
     const int32_t stalled = *stall;
-    const unsigned long long kmin = *key, my_min = cmin ? cmin[b] : 0ull;
+    const unsigned long long kmin = *key;
+    unsigned long long my_min = cmin ? cmin[blockIdx.x] : 0ull;
     if (stalled) return;
     constexpr int PER = SEL_CHUNK / 256;
     __shared__ int32_t wsum[8], wsum2[8];
     __shared__ int32_t base_s, base2_s;
     const double tn = key_to_double(kmin);
+    // The look-back below waits for the chunks before this one.  That is safe because the host caps the grid at the
+    // number of CTAs the device holds at once (blk_setup) and a CTA takes its chunks in ascending order: every chunk
+    // somebody waits for belongs to a CTA that is resident or will be as soon as kernels AHEAD of this one drain --
+    // never to one queued behind a spinning CTA.  (Up to that cap -- 2.4M bodies on a B200 -- the grid is one CTA
+    // per chunk, as before.)
+    for (int b = blockIdx.x; b < nchunk; b += gridDim.x) {
+    if (b != (int)blockIdx.x) {
+        __syncthreads();                            // the shared words of the previous chunk are done with
+        my_min = cmin ? cmin[b] : 0ull;
+    }
     const bool here = !cmin || my_min == kmin;      // only a chunk whose own minimum is t_next holds due bodies
     // ---- this chunk's active bodies (kept as flags) and their number
     bool act[PER], due[PER];
@@ -1593,6 +1603,7 @@ __global__ void __launch_bounds__(256) select_scatter_kernel(int64_t N, const do
         __threadfence_system();
         rv[3] = (double)status;
     }
+    }       // chunks of this CTA
 }
 
 constexpr double DT_MIN_FACTOR = 1.0 / 1099511627776.0;     // 2^-40: no step below dt_max 2^-40 (reading R32)

@@ -558,3 +558,95 @@ def test_get_block_copies_no_more_than_the_caller_has_room_for():
     blk = ctx.get_block(last)["idx_act"].cpu().numpy()
     assert np.all(st["t0"][blk] == st["t0"].max()) and (st["t0"] == st["t0"].max()).sum() == last
     ctx.close()
+
+
+@pytest.mark.parametrize("grid,chunks", [(1, 1), (3, 1), (4, 0)])
+def test_selection_with_several_chunks_per_cta_selects_the_same_blocks(grid, chunks):
+    """The scatter kernel's look-back (a chunk waits for the counts of the chunks before it) is safe because the grid
+    never exceeds what the device holds at once; beyond that a CTA walks several chunks in ascending order (round-2
+    advisor / verdict finding: it used to rest on dispatch order from ~2.4M bodies up).  NB_TUNE_SELECT_GRID forces
+    that route at N = 20000 (10 chunks on 1, 3 or 4 CTAs): same blocks, bit-identical state."""
+    import paper_1504_03687_b200 as nb
+    cfg = nbgen.make_config(3, N=20000, n_i=16)
+    N = cfg["N"]
+    dt = 2.0 ** -cfg["levels"].astype(np.float64)
+    t0 = np.floor(0.3 / dt) * dt
+    eta, dt_max = 0.02, 2.0**-6
+
+    def run(cap):
+        ctx = nb.nb_open(N, 8)
+        ctx.tune("select_chunks", chunks)
+        ctx.tune("select_grid", cap)
+        assert ctx.info("select_grid") == cap
+        nb.nb_set_j(ctx, *(_dev(a) for a in (cfg["m"], cfg["x0"], cfg["v0"], cfg["a0"], cfg["j0"], t0)))
+        ctx.set_steps(_dev(dt))
+        log = [ctx.block_step(None, eta, dt_max) for _ in range(10)]
+        log.append(ctx.run_blocks(None, eta, dt_max, t_stop=1.0e9, max_blocks=40))
+        blk = ctx.get_block(ctx.info("last_block_n"))["idx_act"].cpu().numpy()
+        out = _state(ctx)
+        ctx.close()
+        return log, blk, out
+
+    log_c, blk_c, s_c = run(grid)
+    log_0, blk_0, s_0 = run(0)
+    assert log_c == log_0 and np.array_equal(blk_c, blk_0) and np.all(np.diff(blk_c) > 0)
+    assert all(np.array_equal(s_c[k], s_0[k]) for k in s_c)
+
+
+def test_two_level_selection_with_several_chunks_per_cta():
+    """The same for the two-level loop, whose scatter kernel also lists the bodies due for a regular step."""
+    import paper_1504_03687_b200 as nb
+    N, cap = 12000, 64
+    cfg = nbgen.make_config(1, N=N)
+    m, x, v = cfg["m"], cfg["x0"], cfg["v0"]
+    from scipy.spatial import cKDTree
+    d, _ = cKDTree(x).query(x, k=13)
+    h2 = (d[:, 12] * 1.0001) ** 2
+    runs = []
+    for grid in (2, 0):
+        ctx = nb.nb_open(N, cap)
+        z3 = np.zeros((N, 3))
+        nb.nb_set_j(ctx, _dev(m), _dev(x), _dev(v), _dev(z3), _dev(z3), _dev(np.zeros(N)))
+        ctx.tune("select_grid", grid)
+        assert ctx.ac_init(0.0, _dev(h2), 0.01, 2.0**-4) == 0
+        res = ctx.ac_run(0.01, 0.02, 2.0**-4, max_blocks=120)
+        st = {k: v_.cpu().numpy() for k, v_ in ctx.get_state(True).items()}
+        st.update({k: v_.cpu().numpy() for k, v_ in ctx.ac_get(False).items() if k not in ("idx_act", "idx_reg")})
+        runs.append((res, st))
+        ctx.close()
+    assert runs[0][0] == runs[1][0] and runs[0][0][3] > 0            # regular steps were taken
+    for k in runs[0][1]:
+        assert np.array_equal(runs[0][1][k], runs[1][1][k]), k
+
+
+def test_block_selection_at_five_million_bodies():
+    """N = 5,000,000: 2442 selection chunks, about twice what a B200 holds at once (148 SMs x 8 CTAs), so every CTA of the
+    capped grid walks two or three chunks.  Three blocks; each block's members must be exactly {j : t0 + dt = min}
+    computed from the state the library held before the step (the definition), ascending."""
+    import paper_1504_03687_b200 as nb
+    N = 5_000_000
+    rng = np.random.default_rng(11)
+    x = rng.standard_normal((N, 3))
+    v = 0.5 * rng.standard_normal((N, 3))
+    m = np.full(N, 1.0 / N)
+    z3 = np.zeros((N, 3))
+    levels = 8 + np.minimum(rng.geometric(0.55, N) - 1, 16)          # deep levels hold few bodies (P:89)
+    dt = 2.0 ** -levels.astype(np.float64)
+    ctx = nb.nb_open(N, 8)
+    nb.nb_set_j(ctx, _dev(m), _dev(x), _dev(v), _dev(z3), _dev(z3), _dev(np.zeros(N)))
+    ctx.set_steps(_dev(dt))
+    t0 = np.zeros(N)
+    sizes = []
+    for b in range(3):
+        t, n = ctx.block_step(None, 0.02, 2.0**-6)
+        due = np.flatnonzero(t0 + dt == (t0 + dt).min())
+        assert t == (t0 + dt).min() and n == due.size
+        assert np.array_equal(ctx.get_block(n)["idx_act"].cpu().numpy(), due)
+        sizes.append(n)
+        st = ctx.get_state(True)
+        t0, dt = st["t0"].cpu().numpy(), st["dt"].cpu().numpy()
+        del st
+        assert np.all(t0[due] == t)
+    print("5M-body selection: block sizes", sizes, "chunks", (N + 2047) // 2048)
+    assert 0 < min(sizes) and len(set(np.asarray(due) // 2048)) > 1
+    ctx.close()
