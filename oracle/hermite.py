@@ -27,8 +27,9 @@ conserves energy.  ``aarseth_step``: for harmonic motion a(t) = A cos(wt) e the 
 sqrt(eta) / w at every phase and amplitude (closed form), plus two cases worked by hand with a2 handed
 in at the start of the step (so "a2 advanced by dt a3" is pinned); ``initial_step``: hand cases on and
 off a power of two and at the dt_max cap; the degenerate-criterion rule R32 (dt_req = 0 / NaN keeps
-the step, nothing falls below dt_max 2^-40) on hand cases.  Thirteen single-term mutations of those two functions (no
-sqrt, swapped or dropped products, wrong powers, a2 at the start, ceil for floor, ...) each fail a test.
+the step, nothing falls below dt_max 2^-40) on hand cases.  tests/test_oracle_mutations.py applies 22 single-term
+mutations to correct / aarseth_step / quantize_step / initial_step (no sqrt, swapped or dropped products, wrong powers,
+a2 at the start, ceil for floor, ...) and checks that each makes a pin fail.
 """
 from __future__ import annotations
 

@@ -111,19 +111,16 @@ def combine(part: dict, cap: int, group=None) -> dict:
 
 
 def regular_jsharded(ctx, state: dict, offset: int, t: float, idx_global: torch.Tensor, h2_i: torch.Tensor,
-                     group=None, compute_shard=None) -> dict:
+                     group=None) -> dict:
     """One regular-force block over a j-sharded system.  `ctx` holds this rank's shard (already
     nb_set_j / nb_set_j_offset / nb_predict_all(t)); `state` is the shard's FP64 state (tensors keyed by
     STATE_KEYS) used to publish the active particles' own state.  Returns the full outputs on every
-    rank.  `compute_shard(t, idx, istate, h2) -> partial dict` replaces the library call in CPU tests."""
-    n, cap = idx_global.numel(), ctx.cap if ctx is not None else None
+    rank.  The shard's partial sums come from ctx.regular_shard (the library) and from nowhere else."""
+    n, cap = idx_global.numel(), ctx.cap
     ist = gather_istate(state, offset, idx_global, group)
-    if compute_shard is not None:
-        part, cap = compute_shard(t, idx_global, ist, h2_i)
-    else:
-        dev, f8, i4 = idx_global.device, torch.float64, torch.int32
-        part = dict(acc=torch.empty((n, 3), dtype=f8, device=dev), jerk=torch.empty((n, 3), dtype=f8, device=dev),
-                    pot=torch.empty(n, dtype=f8, device=dev), nnb=torch.empty(n, dtype=i4, device=dev),
-                    nblist=torch.full((n, cap), -1, dtype=i4, device=dev), overflow=torch.empty(n, dtype=i4, device=dev))
-        ctx.regular_shard(t, idx_global, ist.contiguous(), h2_i, **part)
+    dev, f8, i4 = idx_global.device, torch.float64, torch.int32
+    part = dict(acc=torch.empty((n, 3), dtype=f8, device=dev), jerk=torch.empty((n, 3), dtype=f8, device=dev),
+                pot=torch.empty(n, dtype=f8, device=dev), nnb=torch.empty(n, dtype=i4, device=dev),
+                nblist=torch.full((n, cap), -1, dtype=i4, device=dev), overflow=torch.empty(n, dtype=i4, device=dev))
+    ctx.regular_shard(t, idx_global, ist.contiguous(), h2_i, **part)
     return combine(part, cap, group)

@@ -76,7 +76,7 @@ def _jshard_worker(rank, world, port, q):
     state = {k: torch.from_numpy(np.ascontiguousarray(cfg[k][lo:hi])) for k in par.STATE_KEYS}
 
     def compute_shard(t_, idx_global, ist, h2):
-        """The shard's partial result with the CPU oracle standing in for nb_regular_shard: local bodies
+        """The shard's partial result with the CPU oracle standing in for the library call: local bodies
         plus massless copies of the active bodies other shards own (so that they can be i-particles)."""
         idx = idx_global.numpy().astype(np.int64)
         ist = ist.numpy()
@@ -102,8 +102,19 @@ def _jshard_worker(rank, world, port, q):
                     nnb=torch.from_numpy(nnb), nblist=torch.from_numpy(rows), overflow=torch.from_numpy((nnb > cap).astype(np.int32)))
         return part, cap
 
-    res = par.regular_jsharded(None, state, lo, t, torch.from_numpy(cfg["idx_i"].copy()), torch.from_numpy(cfg["h2_i"].copy()),
-                               compute_shard=compute_shard)
+    class StubContext:
+        """What parallel.py needs of a context, without a GPU: .cap and regular_shard filling the caller's tensors.
+        (The product has no hook for this: the test hands in an object with the context's interface.)"""
+        def __init__(self):
+            self.cap = cap
+
+        def regular_shard(self, t_, idx_global, ist, h2, **out):
+            part, _ = compute_shard(t_, idx_global, ist, h2)
+            for key, dst in out.items():
+                dst.copy_(part[key])
+
+    res = par.regular_jsharded(StubContext(), state, lo, t, torch.from_numpy(cfg["idx_i"].copy()),
+                               torch.from_numpy(cfg["h2_i"].copy()))
     q.put((rank, {k: v.numpy() for k, v in res.items()}))
     dist.barrier()
     dist.destroy_process_group()
