@@ -1166,10 +1166,13 @@ __device__ __forceinline__ BodyD predict_line(double2 q0, double2 q1, double2 q2
     for (int c = 0; c < 3; ++c) predict_component(x[c], v[c], a[c], jk[c], dt, c2, c3, b.x[c], b.v[c]);
     return b;
 }
-// One 256-bit load (sm_100: LDG.E.256): 32 B-aligned, read-only data.  A scattered gather is bound by the tag look-ups
-// of L1, one per lane and instruction: half as many instructions per record, half as many look-ups.
+// One 256-bit load (sm_100: LDG.E.256), 32 B-aligned.  A scattered gather is bound by the tag look-ups of L1, one per
+// lane and instruction: half as many instructions per record, half as many look-ups.  An ORDINARY global load, not
+// the read-only (.nc) path: the state lines and predicted records it fetches are rewritten by the kernels ahead in
+// the same programmatic chain (correctors, predict64_kernel), and only ordinary loads are ordered after
+// griddepcontrol.wait by construction rather than by where they happen to stand in the source.
 __device__ __forceinline__ void ld256(const double *p, double &a, double &b, double &c, double &d) {
-    asm volatile("ld.global.nc.v4.f64 {%0, %1, %2, %3}, [%4];" : "=d"(a), "=d"(b), "=d"(c), "=d"(d) : "l"(p));
+    asm volatile("ld.global.v4.f64 {%0, %1, %2, %3}, [%4];" : "=d"(a), "=d"(b), "=d"(c), "=d"(d) : "l"(p));
 }
 __device__ __forceinline__ BodyD predict_body(const double *__restrict__ aos, int32_t j, double t) {
     const double *p = aos + (int64_t)j * AOS_D;
