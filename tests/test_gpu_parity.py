@@ -594,8 +594,9 @@ def test_config4_largest_block_sampled_and_block_independent(oracle):
         if small["nnb"][k] <= cfg["cap"]:
             assert set(small["nblist"][k, :c].tolist()) == set(big["nblist"][k, :c].tolist())
     # the two calls put a particle into different warps, i.e. different local origins: each evaluation carries a
-    # position-difference error <= 1.8e-7 + 2.4e-7 G = 1.1e-6 at the default guard G = 4,
-    # so two evaluations agree to ~2e-6 in the worst case -- an order of magnitude inside the 1e-5 / 1e-4 budget
+    # position-difference error <= 1.8e-7 + 2.4e-7 G = 2.1e-6 at the default guard G = 8 for a
+    # particle AT the guard; the bulk sits far inside it (measured max 8.6e-7), so two evaluations agree to a few 1e-6
+    # at worst -- inside the 1e-5 / 1e-4 budget
     for key, tol in (("acc", 3e-6), ("jerk", 3e-5), ("pot", 3e-7)):
         a = small[key].reshape(8192, -1); b = big[key][:8192].reshape(8192, -1)
         assert np.max(np.linalg.norm(a - b, axis=1) / np.linalg.norm(b, axis=1)) < tol
